@@ -1,0 +1,263 @@
+/*
+ * lpf_oracle.c -- plain CPU oracle for the lineal path function L2 of a periodic
+ * two-phase pixel image (Havelka, Kucerova, Sykora, arXiv 1601.04359).
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, load or call it.
+ * It shares no code with the CUDA library under paper_1601_04359_b200/csrc and must
+ * never be imported from there.
+ *
+ * What it computes is the plain definition, shaped like the paper's Alg. 1
+ * ("for seg / for transl / for pix ... if A[...] != phase break"):
+ *
+ *   count_phi(v) = #{ (x,y) in [0,W)x[0,H) :
+ *                     I[(y+b) mod H][(x+a) mod W] == phi  for all (a,b) in P_v }
+ *
+ * with  L2_phi(v) = count_phi(v) / (W*H)   (Eq. 6's 1/(WH) normalisation, PAPER.md:99;
+ * Eq. 10 L2(0) = phi).  No bit packing, no trie, no SIMD, no symmetry
+ * shortcut unless the caller asks for the mirrored half (Eq. 12).
+ *
+ * Readings of the paper taken here (all listed in DESIGN.md "Readings"):
+ *   D1  |P_v| = max(|dx|,|dy|) + 1, both end pixels included (Eq. 15's max(i,j)).
+ *   D2  v in the canonical half D (Eq. 13: dy>0, or dy==0 and dx>=0):
+ *       Bresenham [20] from (0,0) to v in the incremental-error form below; ties go to
+ *       the larger |minor| coordinate; signs applied after.  The paper is silent on ties.
+ *   D3  v not in D:  P_v = reverse(P_{-v}) + v, the same pixel set as the canonical
+ *       segment ("the line segment x1x2 is identical to x2x1").
+ *   S2  x <-> column <-> W,  y <-> row <-> H  (Eq. 6: x%W, y%H).
+ *   S3  Alg. 1 loops pix = 0..D[seg]-1 and counts a hit iff no break.
+ *   S8  a pixel is "in phase phi" iff its byte equals phi (Alg. 1 line 4).
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): Eq. 15-17 and |D| closed forms, the worked
+ * paths/image in tests/golden/, stripes and run-length closed forms, scipy erosion,
+ * numpy FFT autocorrelation for |P_v| = 2 (Eq. 6/7), brute force by whole-array
+ * roll-and-AND on tiny images, Eq. 10/12 invariants, Bernoulli statistics.
+ * Parity with the AUTHORS' numbers is unpinned: the paper prints no L2 value.
+ *
+ * Build:  gcc -O2 -fopenmp -shared -fPIC -o liblpf_oracle.so lpf_oracle.c
+ */
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+static int iabs_(int v) { return v < 0 ? -v : v; }
+static int imax_(int a, int b) { return a > b ? a : b; }
+static int sgn_(int v) { return (v > 0) - (v < 0); }
+static int pmod_(int a, int n) { int r = a % n; return r < 0 ? r + n : r; }
+
+/* Is v in the canonical half-plane D of Eq. 13? */
+int lpf_oracle_in_half(int dx, int dy) { return dy > 0 || (dy == 0 && dx >= 0); }
+
+/* D2: Bresenham, incremental error form, for v in D.  xy = [len][2] (x then y). */
+static int canonical_path_(int dx, int dy, int16_t *xy)
+{
+    int ax = iabs_(dx), ay = iabs_(dy), sx = sgn_(dx), sy = sgn_(dy);
+    int x = 0, y = 0, n = 0;
+    xy[0] = 0; xy[1] = 0; n = 1;
+    if (ax >= ay) {                       /* x-major: one pixel per x step */
+        int e = ax;
+        for (int k = 0; k < ax; ++k) {
+            x += sx;
+            e += 2 * ay;
+            if (e >= 2 * ax) { y += sy; e -= 2 * ax; }
+            xy[2 * n] = (int16_t)x; xy[2 * n + 1] = (int16_t)y; ++n;
+        }
+    } else {                              /* y-major: one pixel per y step */
+        int e = ay;
+        for (int k = 0; k < ay; ++k) {
+            y += sy;
+            e += 2 * ax;
+            if (e >= 2 * ay) { x += sx; e -= 2 * ay; }
+            xy[2 * n] = (int16_t)x; xy[2 * n + 1] = (int16_t)y; ++n;
+        }
+    }
+    return n;
+}
+
+/* P_v for ANY v (D2 for v in D, D3 otherwise).  xy must hold max(|dx|,|dy|)+1 pairs.
+ * Returns |P_v|. */
+int lpf_oracle_path(int dx, int dy, int16_t *xy)
+{
+    if (lpf_oracle_in_half(dx, dy)) return canonical_path_(dx, dy, xy);
+    int n = canonical_path_(-dx, -dy, xy);            /* P_{-v} */
+    for (int i = 0, j = n - 1; i < j; ++i, --j) {      /* reverse the order */
+        int16_t tx = xy[2 * i], ty = xy[2 * i + 1];
+        xy[2 * i] = xy[2 * j]; xy[2 * i + 1] = xy[2 * j + 1];
+        xy[2 * j] = tx; xy[2 * j + 1] = ty;
+    }
+    for (int i = 0; i < n; ++i) {                      /* translate by v */
+        xy[2 * i] = (int16_t)(xy[2 * i] + dx);
+        xy[2 * i + 1] = (int16_t)(xy[2 * i + 1] + dy);
+    }
+    return n;
+}
+
+/* Alg. 1 lines 2-10 for ONE segment: translate over every start pixel, compare, count. */
+static int64_t count_one_(const uint8_t *img, int H, int W, int phase,
+                          const int16_t *xy, int n)
+{
+    int64_t hits = 0;
+    for (int y = 0; y < H; ++y) {                       /* "transl" */
+        for (int x = 0; x < W; ++x) {
+            int pix;
+            for (pix = 0; pix < n; ++pix) {             /* "pix" */
+                int xx = pmod_(x + xy[2 * pix], W);
+                int yy = pmod_(y + xy[2 * pix + 1], H);
+                if (img[(size_t)yy * W + xx] != phase) break;
+            }
+            if (pix == n) ++hits;                       /* Alg. 1 lines 8-9 */
+        }
+    }
+    return hits;
+}
+
+/* Counts for a caller-given list of vectors vecs = [n][2] (dx,dy); out[n].
+ * threads <= 0 means "all the OpenMP runtime gives". Returns the threads used. */
+int lpf_oracle_counts_list(const uint8_t *img, int H, int W, int phase,
+                           const int32_t *vecs, int64_t n, int64_t *out, int threads)
+{
+    int used = 1;
+#ifdef _OPENMP
+    if (threads <= 0) threads = omp_get_max_threads();
+    used = threads;
+#else
+    (void)threads;
+#endif
+#pragma omp parallel num_threads(used)
+    {
+        int16_t *xy = NULL; int cap = 0;
+#pragma omp for schedule(dynamic, 4)
+        for (int64_t i = 0; i < n; ++i) {
+            int dx = vecs[2 * i], dy = vecs[2 * i + 1];
+            int need = imax_(iabs_(dx), iabs_(dy)) + 1;
+            if (need > cap) { free(xy); cap = need; xy = (int16_t *)malloc(sizeof(int16_t) * 2 * (size_t)cap); }
+            int len = lpf_oracle_path(dx, dy, xy);
+            out[i] = count_one_(img, H, W, phase, xy, len);
+        }
+        free(xy);
+    }
+    return used;
+}
+
+/* The whole template |dx|,|dy| <= m: counts[(dy+m)*(2m+1) + (dx+m)].
+ *   full_template = 1: every one of the (2m+1)^2 vectors is evaluated on its own path
+ *                      (nothing mirrored) -- used to SHOW Eq. 12 rather than assume it;
+ *   full_template = 0: only v in D is evaluated, counts[-v] = counts[v].
+ * Returns the threads used. */
+int lpf_oracle_counts(const uint8_t *img, int H, int W, int phase, int m,
+                      int64_t *counts, int full_template, int threads)
+{
+    int S = 2 * m + 1;
+    int64_t nvec = 0;
+    int32_t *vecs = (int32_t *)malloc(sizeof(int32_t) * 2 * (size_t)S * S);
+    int64_t *tmp = (int64_t *)malloc(sizeof(int64_t) * (size_t)S * S);
+    for (int dy = -m; dy <= m; ++dy)
+        for (int dx = -m; dx <= m; ++dx)
+            if (full_template || lpf_oracle_in_half(dx, dy)) {
+                vecs[2 * nvec] = dx; vecs[2 * nvec + 1] = dy; ++nvec;
+            }
+    int used = lpf_oracle_counts_list(img, H, W, phase, vecs, nvec, tmp, threads);
+    for (int64_t i = 0; i < nvec; ++i) {
+        int dx = vecs[2 * i], dy = vecs[2 * i + 1];
+        counts[(size_t)(dy + m) * S + (dx + m)] = tmp[i];
+        if (!full_template)
+            counts[(size_t)(-dy + m) * S + (-dx + m)] = tmp[i];
+    }
+    free(vecs); free(tmp);
+    return used;
+}
+
+/* Eq. 14 / Eq. 19 on integer counts: sum_k (c_k - t_k)^2, exact.
+ * (e = sse / (W*H)^2 is one IEEE division done by the caller.) */
+uint64_t lpf_oracle_sse(const int64_t *counts, const int64_t *target, int64_t K)
+{
+    uint64_t s = 0;
+    for (int64_t k = 0; k < K; ++k) {
+        int64_t d = counts[k] - target[k];
+        s += (uint64_t)(d * d);
+    }
+    return s;
+}
+
+/* Two-pixel swap ("interchanging two randomly chosen pixels from different
+ * phases"), BY DEFINITION: delta(v) = count(I', v) - count(I, v) with I' = I after the two
+ * pixels (xp,yp) and (xq,yq) exchange their bytes.  Full re-evaluation, twice. */
+int lpf_oracle_swap_delta_full(const uint8_t *img, int H, int W, int phase, int m,
+                               int xp, int yp, int xq, int yq, int32_t *delta, int threads)
+{
+    int S = 2 * m + 1;
+    size_t K = (size_t)S * S;
+    uint8_t *img2 = (uint8_t *)malloc((size_t)H * W);
+    int64_t *c0 = (int64_t *)malloc(sizeof(int64_t) * K);
+    int64_t *c1 = (int64_t *)malloc(sizeof(int64_t) * K);
+    memcpy(img2, img, (size_t)H * W);
+    uint8_t t = img2[(size_t)yp * W + xp];
+    img2[(size_t)yp * W + xp] = img2[(size_t)yq * W + xq];
+    img2[(size_t)yq * W + xq] = t;
+    int used = lpf_oracle_counts(img, H, W, phase, m, c0, 0, threads);
+    lpf_oracle_counts(img2, H, W, phase, m, c1, 0, threads);
+    for (size_t k = 0; k < K; ++k) delta[k] = (int32_t)(c1[k] - c0[k]);
+    free(img2); free(c0); free(c1);
+    return used;
+}
+
+/* Same delta, restricted to the start pixels whose segment can change: a segment (s,v)
+ * differs between I and I' only if it contains p or q, i.e. s = p - P_v[k] or q - P_v[k].
+ * Still the definition (each candidate start is tested on I and on I' pixel by pixel);
+ * pinned to lpf_oracle_swap_delta_full in tests/test_oracle_swap.py. */
+static int seg_in_phase_(const uint8_t *img, int H, int W, int phase,
+                         const int16_t *xy, int n, int sx, int sy)
+{
+    for (int pix = 0; pix < n; ++pix) {
+        int xx = pmod_(sx + xy[2 * pix], W);
+        int yy = pmod_(sy + xy[2 * pix + 1], H);
+        if (img[(size_t)yy * W + xx] != phase) return 0;
+    }
+    return 1;
+}
+
+void lpf_oracle_swap_delta_local(const uint8_t *img, int H, int W, int phase, int m,
+                                 int xp, int yp, int xq, int yq, int32_t *delta)
+{
+    int S = 2 * m + 1;
+    uint8_t *img2 = (uint8_t *)malloc((size_t)H * W);
+    int16_t *xy = (int16_t *)malloc(sizeof(int16_t) * 2 * (size_t)(m + 1));
+    int *sxs = (int *)malloc(sizeof(int) * 2 * (size_t)(m + 1));
+    int *sys = (int *)malloc(sizeof(int) * 2 * (size_t)(m + 1));
+    memcpy(img2, img, (size_t)H * W);
+    uint8_t t = img2[(size_t)yp * W + xp];
+    img2[(size_t)yp * W + xp] = img2[(size_t)yq * W + xq];
+    img2[(size_t)yq * W + xq] = t;
+    for (int dy = -m; dy <= m; ++dy)
+        for (int dx = -m; dx <= m; ++dx) {
+            int n = lpf_oracle_path(dx, dy, xy);
+            int ns = 0;
+            /* candidate starts, de-duplicated (p - P_v[k] may equal q - P_v[j]) */
+            for (int side = 0; side < 2; ++side)
+                for (int k = 0; k < n; ++k) {
+                    int sx = pmod_((side ? xq : xp) - xy[2 * k], W);
+                    int sy = pmod_((side ? yq : yp) - xy[2 * k + 1], H);
+                    int dup = 0;
+                    for (int j = 0; j < ns; ++j) if (sxs[j] == sx && sys[j] == sy) { dup = 1; break; }
+                    if (!dup) { sxs[ns] = sx; sys[ns] = sy; ++ns; }
+                }
+            int32_t d = 0;
+            for (int j = 0; j < ns; ++j)
+                d += seg_in_phase_(img2, H, W, phase, xy, n, sxs[j], sys[j])
+                   - seg_in_phase_(img,  H, W, phase, xy, n, sxs[j], sys[j]);
+            delta[(size_t)(dy + m) * S + (dx + m)] = d;
+        }
+    free(img2); free(xy); free(sxs); free(sys);
+}
+
+int lpf_oracle_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
