@@ -1,0 +1,131 @@
+/*
+ * lpf.h -- C ABI of the B200-native lineal path function library (liblpf.so).
+ *
+ * What the library computes (Havelka, Kucerova, Sykora, arXiv 1601.04359; citations are
+ * PAPER.md lines): for a periodic two-phase pixel image I[y][x] (0<=x<W columns, 0<=y<H
+ * rows), a phase phi and every vector v = (dx,dy) of the square template |dx|,|dy| <= m,
+ *
+ *     count_phi(v) = #{ (x,y) : I[(y+b) mod H][(x+a) mod W] == phi  for all (a,b) in P_v }
+ *
+ * i.e. the un-normalised lineal path function L2_phi(v) = count_phi(v) / (W*H)
+ * (Eq. 8-9; Alg. 1 "for seg / for transl / for pix").
+ * P_v is the Bresenham pixel path from (0,0) to v, |P_v| = max(|dx|,|dy|)+1,
+ * computed for the canonical half D = {dy>0} u {dy==0, dx>=0} (Eq. 13) with
+ * ties rounded up in |minor|, and P_v := reverse(P_{-v}) + v outside D (point symmetry,
+ * PAPER.md:140-148).  DESIGN.md "Readings" lists every reading of the paper taken here.
+ *
+ * Conventions
+ *   - Every function returns int: LPF_OK (0) or a negative LPF_E_* code.  Nothing throws,
+ *     nothing prints.  lpf_strerror() gives a static string.
+ *   - "dev" pointers are CUDA device pointers on the device given to lpf_build_paths;
+ *     "host" pointers are ordinary host memory.  All buffers are CALLER-OWNED; the library
+ *     owns only what lives inside lpf_paths (the path/trie tables and a packed-image
+ *     workspace that grows on demand).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
+ *     entry points are asynchronous on that stream and do not synchronise the host, except
+ *     that the first call for a new (B,H,W) shape may cudaMalloc workspace.
+ *   - One lpf_paths object must not be used from two streams/threads at the same time (the
+ *     workspace is shared).
+ *   - There is no CPU fallback: a device entry point called on a table built with
+ *     device < 0 returns LPF_E_INVAL.
+ */
+#ifndef LPF_H_
+#define LPF_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LPF_OK             0
+#define LPF_E_INVAL       -1   /* null pointer, B<1, phase not in {0,1}, m<0, m > min(H,W)-1, pair out of range */
+#define LPF_E_NOMEM       -2   /* host or device allocation failed */
+#define LPF_E_CUDA        -3   /* a CUDA runtime call failed (see lpf_last_cuda_error) */
+#define LPF_E_UNSUPPORTED -4   /* shape outside what the kernels take (m > 511, image+halo > shared memory) */
+
+/* flags of lpf_eval / lpf_eval_both */
+#define LPF_PRUNE    1u   /* paper's "enhanced" variant: skip a sub-trie whose running
+                             mask is all-zero for the whole block.  Exact: never changes a count. */
+#define LPF_NO_TRIE  2u   /* one chain per path P_v (no prefix sharing): the "one-path-per-warp" design
+                             variant, kept for the measurement in DESIGN.md. Same counts. */
+
+typedef struct lpf_paths lpf_paths;   /* opaque: path table + prefix trie + device programs for one m */
+
+const char* lpf_strerror(int code);
+/* Last CUDA error code (cudaError_t as int) recorded by a call that returned LPF_E_CUDA. */
+int lpf_last_cuda_error(void);
+
+/* Paper "step 1": rasterise P_v for every v in D with |dx|,|dy| <= m,
+ * build the prefix trie over the ordered pixel lists, and keep it (host) for program
+ * generation.  device >= 0: also binds the object to that CUDA device; device < 0: host-only
+ * table (lpf_paths_info / lpf_paths_get / lpf_paths_program work; device entry points refuse).
+ * Errors: m < 0 -> INVAL; m > 511 -> UNSUPPORTED; NOMEM; CUDA. Synchronous. */
+int  lpf_build_paths(int m, int device, lpf_paths** out);
+void lpf_free_paths(lpf_paths* p);
+
+/* Sizes of the table: |D| = 2m^2+2m+1, sum_v |P_v| (= Eq. 17 with W = m+1,
+ * PAPER.md:186-196), number of trie nodes (distinct path prefixes, root included), and the
+ * deepest node (= m). Any out pointer may be NULL. */
+int  lpf_paths_info(const lpf_paths* p, int64_t* n_half_vectors, int64_t* sum_path_len,
+                    int64_t* n_trie_nodes, int* max_depth);
+
+/* Host: P_v for ANY v of the template (|dx|,|dy| <= m).  xy = host [cap][2] int16 (x then y),
+ * *len = |P_v|; INVAL if v is outside the template or cap < |P_v|. */
+int  lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, int cap, int* len);
+
+/* Host, for tests and tools: the linearised walk program the eval kernel interprets
+ * (DESIGN.md "Node program").  The trie is cut into connected pieces of about `piece_nodes`
+ * nodes (<= 0: one piece); each piece is one work item = the chain from the root to the piece
+ * root followed by the piece in depth-first order.  flags: 0 or LPF_NO_TRIE.
+ *   entries  host [cap_entries] uint64 (may be NULL to query sizes)
+ *   items    host [cap_items][2] int64 = (first entry, number of entries) (may be NULL)
+ * *n_entries / *n_items / *n_slots (mask-stack slots the program needs) are always written. */
+int  lpf_paths_program(lpf_paths* p, int piece_nodes, unsigned flags,
+                       uint64_t* entries, int64_t cap_entries, int64_t* n_entries,
+                       int64_t* items, int64_t cap_items, int64_t* n_items, int* n_slots);
+
+/* Paper "steps 2-3" (Alg. 1 / Alg. 2) for a batch of B independent images
+ * of one size: translate every segment over every start pixel, compare, count.
+ *   images  dev uint8 [B][H][W]; a pixel is in phase phi iff its byte == phi
+ *   counts  dev int64 [B][2m+1][2m+1], index [b][dy+m][dx+m]; fully overwritten
+ *           (the half outside D is the mirror counts[-v] = counts[v])
+ * Errors: INVAL (see above; m > min(H,W)-1 is rejected because a path would wrap onto itself,
+ * and D stops at W-1,H-1: PAPER.md:154), UNSUPPORTED, NOMEM, CUDA. */
+int  lpf_eval(lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase,
+              int64_t* counts, unsigned flags, void* stream);
+
+/* Both phases in one call: counts dev int64 [B][2][2m+1][2m+1], index [b][phase][dy+m][dx+m]. */
+int  lpf_eval_both(lpf_paths* p, const uint8_t* images, int B, int H, int W,
+                   int64_t* counts, unsigned flags, void* stream);
+
+/* Least-square objective, Eq. 14 / Eq. 19 on integer counts:
+ *   sse[b] = sum_k (counts[b][k] - target[k])^2, exact in uint64 (wraps mod 2^64 if it overflows;
+ *   it cannot for counts <= 2^26 and K <= 2^12 ... see DESIGN.md).  e = sse / (W*H)^2 is the caller's.
+ *   counts dev int64 [B][K], target dev int64 [K], sse dev uint64 [B]. */
+int  lpf_objective(const int64_t* counts, const int64_t* target, int B, int64_t K,
+                   uint64_t* sse, void* stream);
+
+/* Two-pixel swap: for each of n INDEPENDENT proposals against one base
+ * image, delta[i][dy+m][dx+m] = count_phase(I_i', v) - count_phase(I, v), where I_i' is I with
+ * the bytes of pixels p_i and q_i exchanged.  Only segments through p or q are re-tested.
+ *   image dev uint8 [H][W]; pairs dev int32 [n][4] = x_p, y_p, x_q, y_q; delta dev int32 [n][2m+1][2m+1].
+ * Pairs are range-checked on the device; an out-of-range pair yields an all-zero delta and the
+ * call still returns LPF_OK (no host sync) -- validate on the host if needed. */
+int  lpf_swap_delta(lpf_paths* p, const uint8_t* image, int H, int W, int phase,
+                    const int32_t* pairs, int64_t n, int32_t* delta, void* stream);
+
+/* HOST-buffer convenience used by the end-to-end measurement: copies `images` (host, pinned or
+ * not) to the device, runs lpf_eval(_both if phase < 0), copies counts back, synchronises. */
+int  lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, int H, int W, int phase,
+                   int64_t* counts_host, unsigned flags);
+
+/* Counters of the most recent lpf_eval / lpf_eval_both on this object (host values known at
+ * launch time): kernels launched, work items, program entries walked per image-phase, grid,
+ * block, dynamic shared memory bytes, words per thread. out = host int64[8]. */
+int  lpf_last_launch_info(const lpf_paths* p, int64_t* out8);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LPF_H_ */

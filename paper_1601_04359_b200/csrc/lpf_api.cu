@@ -1,0 +1,365 @@
+// lpf_api.cu -- C ABI entry points of liblpf.so that touch the device (include/lpf.h).
+// Host logic only: argument checks, geometry, workspace, program upload, launches.  Every step
+// of the hot path runs in the kernels of lpf_kernels.cu.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstring>
+#include <new>
+
+#include "lpf_internal.h"
+#include "lpf_kernels.cuh"
+
+namespace lpf {
+
+int build_host_table(lpf_paths* p);   // lpf_paths.cpp
+
+static thread_local int g_last_cuda = 0;
+
+static int cuda_fail(cudaError_t e) {
+  g_last_cuda = (int)e;
+  (void)cudaGetLastError();
+  return e == cudaErrorMemoryAllocation ? LPF_E_NOMEM : LPF_E_CUDA;
+}
+#define LPF_CUDA(call)                                  \
+  do {                                                  \
+    cudaError_t e__ = (call);                           \
+    if (e__ != cudaSuccess) return lpf::cuda_fail(e__); \
+  } while (0)
+
+struct DeviceGuard {   // binds the calling thread to the table's device for the call, then restores
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+  }
+  ~DeviceGuard() {
+    int cur = -1;
+    if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+  }
+};
+
+static void free_program(Program& pr) {
+  if (pr.d_entries) cudaFree(pr.d_entries);
+  if (pr.d_skip) cudaFree(pr.d_skip);
+  if (pr.d_items) cudaFree(pr.d_items);
+  pr.d_entries = nullptr; pr.d_skip = nullptr; pr.d_items = nullptr;
+}
+
+static int upload_program(Program& pr) {
+  if (pr.d_entries) return LPF_OK;
+  LPF_CUDA(cudaMalloc(&pr.d_entries, sizeof(uint64_t) * std::max<size_t>(pr.entries.size(), 1)));
+  LPF_CUDA(cudaMalloc(&pr.d_skip, sizeof(uint32_t) * std::max<size_t>(pr.skip.size(), 1)));
+  LPF_CUDA(cudaMalloc(&pr.d_items, sizeof(int64_t) * std::max<size_t>(pr.items.size(), 2)));
+  LPF_CUDA(cudaMemcpy(pr.d_entries, pr.entries.data(), sizeof(uint64_t) * pr.entries.size(), cudaMemcpyHostToDevice));
+  LPF_CUDA(cudaMemcpy(pr.d_skip, pr.skip.data(), sizeof(uint32_t) * pr.skip.size(), cudaMemcpyHostToDevice));
+  LPF_CUDA(cudaMemcpy(pr.d_items, pr.items.data(), sizeof(int64_t) * pr.items.size(), cudaMemcpyHostToDevice));
+  return LPF_OK;
+}
+
+}  // namespace lpf
+
+using namespace lpf;
+
+extern "C" int lpf_last_cuda_error(void) { return lpf::g_last_cuda; }
+
+extern "C" int lpf_build_paths(int m, int device, lpf_paths** out) {
+  if (!out) return LPF_E_INVAL;
+  *out = nullptr;
+  if (m < 0) return LPF_E_INVAL;
+  if (m > MAX_M) return LPF_E_UNSUPPORTED;
+  lpf_paths* p = new (std::nothrow) lpf_paths();
+  if (!p) return LPF_E_NOMEM;
+  p->m = m;
+  p->device = device;
+  int rc = build_host_table(p);
+  if (rc != LPF_OK) { delete p; return rc; }
+  if (device >= 0) {
+    DeviceGuard g(device);
+    cudaDeviceProp prop;
+    cudaError_t e = g.ok ? cudaGetDeviceProperties(&prop, device) : cudaErrorInvalidDevice;
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_counter, sizeof(unsigned int) * 4);
+    if (e != cudaSuccess) { rc = cuda_fail(e); delete p; return rc; }
+    p->n_sm = prop.multiProcessorCount;
+    p->max_smem = (int)prop.sharedMemPerBlockOptin;
+  }
+  *out = p;
+  return LPF_OK;
+}
+
+extern "C" void lpf_free_paths(lpf_paths* p) {
+  if (!p) return;
+  if (p->device >= 0) {
+    DeviceGuard g(p->device);
+    for (auto& kv : p->programs) free_program(kv.second);
+    if (p->d_packed) cudaFree(p->d_packed);
+    if (p->d_counter) cudaFree(p->d_counter);
+    if (p->d_path_xy) cudaFree(p->d_path_xy);
+    if (p->d_path_off) cudaFree(p->d_path_off);
+    if (p->d_vecs) cudaFree(p->d_vecs);
+    if (p->d_io_in) cudaFree(p->d_io_in);
+    if (p->d_io_out) cudaFree(p->d_io_out);
+    if (p->io_stream) cudaStreamDestroy((cudaStream_t)p->io_stream);
+  }
+  delete p;
+}
+
+// ---- geometry ------------------------------------------------------------------------------------
+
+namespace lpf {
+
+cudaError_t launch_pack(const uint8_t* images, uint32_t* packed, const Geom& g, int B, int Bpad, int n_phase,
+                        int phase0, unsigned int* counter, int n_sm, cudaStream_t st);
+cudaError_t eval_occupancy(int T, int threads, size_t smem, int* blocks_per_sm);
+cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st);
+cudaError_t launch_mirror(unsigned long long* counts, int S, long long n_arrays, int n_sm, cudaStream_t st);
+cudaError_t launch_objective(const long long* counts, const long long* target, int B, long long K,
+                             unsigned long long* sse, int n_sm, cudaStream_t st);
+cudaError_t launch_swap_delta(const uint8_t* image, int H, int W, int m, int phase, const int* pairs, long long n,
+                              const int16_t* path_xy, const int* path_off, const int16_t* vecs, int n_half,
+                              int* delta, cudaStream_t st);
+
+// Packed-image geometry and CTA shape for (B, H, W, m).  Returns false if one image does not fit.
+static bool choose_geom(const lpf_paths* p, int B, int H, int W, Geom* out) {
+  Geom g;
+  g.H = H; g.W = W; g.m = p->m;
+  g.Wc = (W + 31) / 32;
+  g.CL = (p->m + 31) / 32;
+  const int CR = p->m / 32 + 1;
+  g.T = 4;
+  for (int T : {16, 8}) {
+    if ((long long)g.Wc * ((H + T - 1) / T) >= 32) { g.T = T; break; }
+  }
+  const int Hpad = (H + g.T - 1) / g.T * g.T;
+  g.rows = Hpad + p->m;
+  g.stride = g.Wc + g.CL + CR;
+  g.tpi = g.Wc * (Hpad / g.T);
+  g.wpi = (g.tpi + 31) / 32;
+  if (g.wpi * 32 > 1024) return false;
+  // pad the row stride so that the 32 lanes of a warp (consecutive word columns, then the next
+  // block of T rows) fall into distinct banks where possible
+  int best_pad = 0, best_conf = 1 << 30;
+  for (int pad = 0; pad < 16; ++pad) {
+    int bank[32] = {0}, conf = 0;
+    for (int l = 0; l < 32; ++l) {
+      const int j = l % g.Wc, rb = l / g.Wc;
+      conf = std::max(conf, ++bank[(rb * g.T * (g.stride + pad) + j) & 31]);
+    }
+    if (conf < best_conf) { best_conf = conf; best_pad = pad; }
+  }
+  g.stride += best_pad;
+  g.img_words = (g.rows * g.stride + 3) / 4 * 4;
+  const size_t img_bytes = (size_t)g.img_words * 4;
+  const size_t smem_cap = (size_t)p->max_smem - 1024;
+  if (img_bytes > smem_cap) return false;
+  int G = std::max(1, 512 / (g.wpi * 32));
+  G = std::min(G, B);
+  G = (int)std::min<size_t>((size_t)G, smem_cap / img_bytes);
+  g.G = std::max(G, 1);
+  *out = g;
+  return true;
+}
+
+static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, int n_phase, int phase0,
+                     int64_t* counts, unsigned flags, void* stream) {
+  if (!p || !images || !counts) return LPF_E_INVAL;
+  if (p->device < 0) return LPF_E_INVAL;
+  if (B < 1 || H < 1 || W < 1) return LPF_E_INVAL;
+  if (n_phase == 1 && phase0 != 0 && phase0 != 1) return LPF_E_INVAL;
+  if (p->m > std::min(H, W) - 1) return LPF_E_INVAL;
+  if (flags & ~(LPF_PRUNE | LPF_NO_TRIE)) return LPF_E_INVAL;
+  DeviceGuard dg(p->device);
+  if (!dg.ok) return LPF_E_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  Geom g;
+  if (!choose_geom(p, B, H, W, &g)) return LPF_E_UNSUPPORTED;
+
+  const int threads = g.G * g.wpi * 32;
+  const size_t smem = (size_t)g.G * g.img_words * 4;
+  int occ = 0;
+  LPF_CUDA(eval_occupancy(g.T, threads, smem, &occ));
+  if (occ < 1) return LPF_E_UNSUPPORTED;
+  const int Bpad = (B + g.G - 1) / g.G * g.G;
+  const int n_groups = (Bpad / g.G) * n_phase;
+  const int resident = p->n_sm * occ;
+
+  // work items: about 12 per resident CTA, pieces of 256 .. 16384 trie nodes
+  const long long n_nodes = (long long)p->nodes.size();
+  long long want_items = std::max<long long>(1, (12ll * resident + n_groups - 1) / n_groups);
+  long long piece = n_nodes / want_items;
+  piece = std::max<long long>(256, std::min<long long>(piece, 16384));
+  // quantise so that nearby shapes share one cached program
+  int q = 256;
+  while (q * 2 <= piece) q *= 2;
+  Program* pr;
+  try {
+    pr = &get_program(p, q, flags);
+  } catch (const std::bad_alloc&) {
+    return LPF_E_NOMEM;
+  }
+  if (pr->n_slots > MAX_SLOTS) return LPF_E_UNSUPPORTED;
+  int rc = upload_program(*pr);
+  if (rc != LPF_OK) return rc;
+
+  const size_t need = (size_t)n_phase * Bpad * g.img_words * 4;
+  if (need > p->packed_bytes) {
+    if (p->d_packed) { LPF_CUDA(cudaStreamSynchronize(st)); cudaFree(p->d_packed); p->d_packed = nullptr; p->packed_bytes = 0; }
+    LPF_CUDA(cudaMalloc(&p->d_packed, need));
+    p->packed_bytes = need;
+  }
+
+  const int S = 2 * p->m + 1;
+  LPF_CUDA(cudaMemsetAsync(counts, 0, sizeof(int64_t) * (size_t)B * n_phase * S * S, st));
+  LPF_CUDA(launch_pack(images, p->d_packed, g, B, Bpad, n_phase, phase0, p->d_counter, p->n_sm, st));
+
+  EvalParams ep;
+  ep.g = g;
+  ep.entries = pr->d_entries;
+  ep.skip = pr->d_skip;
+  ep.items = pr->d_items;
+  ep.n_items = (int)(pr->items.size() / 2);
+  ep.n_groups = n_groups;
+  ep.B = B;
+  ep.n_phase = n_phase;
+  ep.packed = p->d_packed;
+  ep.Bpad = Bpad;
+  ep.counts = (unsigned long long*)counts;
+  ep.S = S;
+  ep.counter = p->d_counter;
+  ep.prune = (flags & LPF_PRUNE) ? 1 : 0;
+  const long long total_work = (long long)ep.n_items * n_groups;
+  const int grid = (int)std::min<long long>(total_work, resident);
+  LPF_CUDA(launch_eval(ep, grid, threads, smem, st));
+  LPF_CUDA(launch_mirror((unsigned long long*)counts, S, (long long)B * n_phase, p->n_sm, st));
+
+  p->last_info[0] = 3;                                   // kernels launched (pack, eval, mirror)
+  p->last_info[1] = total_work;
+  p->last_info[2] = (int64_t)pr->entries.size();         // program entries walked per image-phase
+  p->last_info[3] = grid;
+  p->last_info[4] = threads;
+  p->last_info[5] = (int64_t)smem;
+  p->last_info[6] = g.T;
+  p->last_info[7] = g.G;
+  return LPF_OK;
+}
+
+}  // namespace lpf
+
+extern "C" int lpf_eval(lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase, int64_t* counts,
+                        unsigned flags, void* stream) {
+  return lpf::eval_impl(p, images, B, H, W, 1, phase, counts, flags, stream);
+}
+
+extern "C" int lpf_eval_both(lpf_paths* p, const uint8_t* images, int B, int H, int W, int64_t* counts,
+                             unsigned flags, void* stream) {
+  return lpf::eval_impl(p, images, B, H, W, 2, 0, counts, flags, stream);
+}
+
+extern "C" int lpf_last_launch_info(const lpf_paths* p, int64_t* out8) {
+  if (!p || !out8) return LPF_E_INVAL;
+  std::memcpy(out8, p->last_info, sizeof(p->last_info));
+  return LPF_OK;
+}
+
+extern "C" int lpf_objective(const int64_t* counts, const int64_t* target, int B, int64_t K, uint64_t* sse,
+                             void* stream) {
+  if (!counts || !target || !sse || B < 1 || K < 1) return LPF_E_INVAL;
+  int dev = 0, n_sm = 0;
+  LPF_CUDA(cudaGetDevice(&dev));
+  LPF_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  LPF_CUDA(lpf::launch_objective((const long long*)counts, (const long long*)target, B, (long long)K,
+                                 (unsigned long long*)sse, n_sm, (cudaStream_t)stream));
+  return LPF_OK;
+}
+
+// ---- swap delta ----------------------------------------------------------------------------------
+
+namespace lpf {
+
+// flattened canonical paths for the swap-delta kernel, built on first use
+static int ensure_path_table(lpf_paths* p) {
+  if (p->d_path_xy) return LPF_OK;
+  const int m = p->m;
+  try {
+    std::vector<int16_t> xy((size_t)p->sum_len * 2), vecs((size_t)p->n_half * 2), tmp(2 * (size_t)(m + 1));
+    std::vector<int32_t> off((size_t)p->n_half + 1);
+    size_t at = 0, v = 0;
+    for (int dy = 0; dy <= m; ++dy)
+      for (int dx = -m; dx <= m; ++dx) {
+        if (!in_half(dx, dy)) continue;
+        const int len = canonical_path(dx, dy, tmp.data());
+        off[v] = (int32_t)at;
+        vecs[2 * v] = (int16_t)dx;
+        vecs[2 * v + 1] = (int16_t)dy;
+        std::memcpy(&xy[2 * at], tmp.data(), sizeof(int16_t) * 2 * (size_t)len);
+        at += (size_t)len;
+        ++v;
+      }
+    off[v] = (int32_t)at;
+    LPF_CUDA(cudaMalloc(&p->d_path_xy, sizeof(int16_t) * xy.size()));
+    LPF_CUDA(cudaMalloc(&p->d_path_off, sizeof(int32_t) * off.size()));
+    LPF_CUDA(cudaMalloc(&p->d_vecs, sizeof(int16_t) * vecs.size()));
+    LPF_CUDA(cudaMemcpy(p->d_path_xy, xy.data(), sizeof(int16_t) * xy.size(), cudaMemcpyHostToDevice));
+    LPF_CUDA(cudaMemcpy(p->d_path_off, off.data(), sizeof(int32_t) * off.size(), cudaMemcpyHostToDevice));
+    LPF_CUDA(cudaMemcpy(p->d_vecs, vecs.data(), sizeof(int16_t) * vecs.size(), cudaMemcpyHostToDevice));
+  } catch (const std::bad_alloc&) {
+    return LPF_E_NOMEM;
+  }
+  return LPF_OK;
+}
+
+}  // namespace lpf
+
+extern "C" int lpf_swap_delta(lpf_paths* p, const uint8_t* image, int H, int W, int phase, const int32_t* pairs,
+                              int64_t n, int32_t* delta, void* stream) {
+  if (!p || !image || !pairs || !delta) return LPF_E_INVAL;
+  if (p->device < 0 || H < 1 || W < 1 || n < 0) return LPF_E_INVAL;
+  if (phase != 0 && phase != 1) return LPF_E_INVAL;
+  if (p->m > std::min(H, W) - 1) return LPF_E_INVAL;
+  if (n == 0) return LPF_OK;
+  DeviceGuard dg(p->device);
+  if (!dg.ok) return LPF_E_CUDA;
+  const size_t smem = (size_t)2 * H * ((W + 31) / 32) * 4;
+  if (smem > (size_t)p->max_smem) return LPF_E_UNSUPPORTED;
+  int rc = ensure_path_table(p);
+  if (rc != LPF_OK) return rc;
+  LPF_CUDA(launch_swap_delta(image, H, W, p->m, phase, pairs, (long long)n, p->d_path_xy, p->d_path_off, p->d_vecs,
+                             (int)p->n_half, delta, (cudaStream_t)stream));
+  return LPF_OK;
+}
+
+// ---- host-buffer convenience (end-to-end measurement) ---------------------------------------------
+
+extern "C" int lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, int H, int W, int phase,
+                             int64_t* counts_host, unsigned flags) {
+  if (!p || !images_host || !counts_host) return LPF_E_INVAL;
+  if (p->device < 0 || B < 1 || H < 1 || W < 1) return LPF_E_INVAL;
+  DeviceGuard dg(p->device);
+  if (!dg.ok) return LPF_E_CUDA;
+  const int n_phase = phase < 0 ? 2 : 1;
+  const int S = 2 * p->m + 1;
+  const size_t in_bytes = (size_t)B * H * W;
+  const size_t out_bytes = sizeof(int64_t) * (size_t)B * n_phase * S * S;
+  if (in_bytes > p->io_in_bytes) {
+    if (p->d_io_in) cudaFree(p->d_io_in);
+    p->d_io_in = nullptr; p->io_in_bytes = 0;
+    LPF_CUDA(cudaMalloc(&p->d_io_in, in_bytes));
+    p->io_in_bytes = in_bytes;
+  }
+  if (out_bytes > p->io_out_bytes) {
+    if (p->d_io_out) cudaFree(p->d_io_out);
+    p->d_io_out = nullptr; p->io_out_bytes = 0;
+    LPF_CUDA(cudaMalloc(&p->d_io_out, out_bytes));
+    p->io_out_bytes = out_bytes;
+  }
+  if (!p->io_stream) LPF_CUDA(cudaStreamCreateWithFlags((cudaStream_t*)&p->io_stream, cudaStreamNonBlocking));
+  cudaStream_t st = (cudaStream_t)p->io_stream;
+  LPF_CUDA(cudaMemcpyAsync(p->d_io_in, images_host, in_bytes, cudaMemcpyHostToDevice, st));
+  int rc = n_phase == 2 ? lpf_eval_both(p, (const uint8_t*)p->d_io_in, B, H, W, (int64_t*)p->d_io_out, flags, st)
+                        : lpf_eval(p, (const uint8_t*)p->d_io_in, B, H, W, phase, (int64_t*)p->d_io_out, flags, st);
+  if (rc != LPF_OK) return rc;
+  LPF_CUDA(cudaMemcpyAsync(counts_host, p->d_io_out, out_bytes, cudaMemcpyDeviceToHost, st));
+  LPF_CUDA(cudaStreamSynchronize(st));
+  return LPF_OK;
+}

@@ -1,0 +1,384 @@
+// lpf_kernels.cu -- CUDA kernels of liblpf.so (sm_100a).
+//   pack_kernel       uint8 image -> bit planes, 32 px / word, with the periodic halo laid out
+//                     exactly as the eval kernel wants it in shared memory
+//   eval_kernel<T>    the hot loop: walk the node program with a running AND mask (a3), POPC +
+//                     warp reduce at terminals (a4), optional zero-mask pruning (a5)
+//   mirror_kernel     counts[-v] = counts[v] (a6)
+//   objective_kernel  sum (c - t)^2 per image (a8, Eq. 14/19)
+#include <cuda_runtime.h>
+
+#include "lpf_internal.h"
+#include "lpf_kernels.cuh"
+
+namespace lpf {
+
+// ---------------------------------------------------------------------------------------------
+// bit-pack + halo.  One warp per output word: lane k tests one pixel, __ballot_sync packs.
+// Also zeroes the work-item counter for the eval kernel that follows on the same stream.
+// ---------------------------------------------------------------------------------------------
+__global__ void pack_kernel(const uint8_t* __restrict__ images, uint32_t* __restrict__ packed, Geom g, int B,
+                            int Bpad, int n_phase, int phase0, unsigned int* counter) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) *counter = 0u;
+  const int lane = threadIdx.x & 31;
+  const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+  const long long total = (long long)n_phase * Bpad * g.img_words;
+  for (long long w = warp; w < total; w += nwarps) {
+    const int word = (int)(w % g.img_words);
+    const long long ib = w / g.img_words;
+    const int b = (int)(ib % Bpad);
+    const int plane = (int)(ib / Bpad);
+    const int r = word / g.stride, i = word - r * g.stride;
+    bool bit = false;
+    if (b < B && r < g.rows) {
+      const int y = r % g.H;
+      int x = (32 * (i - g.CL) + lane) % g.W;
+      if (x < 0) x += g.W;
+      const int phase = (n_phase == 2) ? plane : phase0;
+      bit = images[((size_t)b * g.H + y) * g.W + x] == (uint8_t)phase;
+    }
+    const unsigned v = __ballot_sync(0xffffffffu, bit);
+    if (lane == 0) packed[w] = v;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// mbarrier / TMA bulk-copy helpers (cp.async.bulk -> SASS UBLKCP)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, unsigned parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+  while (!mbar_try_wait(bar, parity)) {
+  }
+}
+__device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------
+// eval kernel, version 1 (reference walker: no register caching of rows)
+//   CTA = G images x wpi warps.  Thread tau of an image owns start word column j = tau % Wc and
+//   the T start rows y0 .. y0+T-1, y0 = (tau / Wc) * T.  All warps of a CTA walk the same item.
+// ---------------------------------------------------------------------------------------------
+template <int T>
+__global__ void __launch_bounds__(1024) eval_kernel_v1(const EvalParams p) {
+  extern __shared__ __align__(128) uint32_t smem[];
+  __shared__ __align__(8) uint64_t bar;
+  __shared__ unsigned int s_work;
+
+  const Geom& g = p.g;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int img_local = warp / g.wpi;
+  const int tau = (warp % g.wpi) * 32 + lane;
+  const bool active = tau < g.tpi;
+  const int tau_c = active ? tau : 0;
+  const int j = tau_c % g.Wc;
+  const int y0 = (tau_c / g.Wc) * T;
+  const uint32_t* base = smem + (size_t)img_local * g.img_words + y0 * g.stride + j + g.CL;
+
+  uint32_t colmask = 0xffffffffu;                     // start pixels x = 32 j + k < W
+  if (32 * j + 32 > g.W) colmask = (g.W - 32 * j >= 32) ? 0xffffffffu : ((1u << (g.W - 32 * j)) - 1u);
+  if (!active) colmask = 0u;
+
+  uint32_t stack[MAX_SLOTS][T];
+  uint32_t M[T];
+
+  if (tid == 0) {
+    mbar_init(&bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  unsigned parity = 0;
+  const unsigned total_work = (unsigned)p.n_items * (unsigned)p.n_groups;
+  const int groups_per_plane = p.Bpad / g.G;
+  const unsigned img_bytes = (unsigned)g.img_words * 4u * (unsigned)g.G;
+
+  for (;;) {
+    if (tid == 0) s_work = atomicAdd(p.counter, 1u);
+    __syncthreads();                 // everybody is also done reading the previous image
+    const unsigned work = s_work;
+    if (work >= total_work) break;
+    const int item = (int)(work / (unsigned)p.n_groups);    // big items first, over all groups
+    const int gp = (int)(work % (unsigned)p.n_groups);
+    const int plane = gp / groups_per_plane;
+    const int b0 = (gp % groups_per_plane) * g.G;
+    if (tid == 0) {
+      mbar_expect_tx(&bar, img_bytes);
+      tma_bulk_g2s(smem, p.packed + ((size_t)plane * p.Bpad + b0) * g.img_words, img_bytes, &bar);
+    }
+    mbar_wait(&bar, parity);
+    parity ^= 1u;
+    __syncthreads();                 // s_work may be rewritten only after everyone has read it
+
+    const int b_img = b0 + img_local;
+    unsigned long long* cnt = p.counts + ((size_t)b_img * p.n_phase + plane) * (size_t)p.S * p.S;
+    const long long e0 = p.items[2 * item], e1 = e0 + p.items[2 * item + 1];
+    for (long long e = e0; e < e1; ++e) {
+      const uint64_t ent = __ldg(p.entries + e);
+      const uint32_t x = (uint32_t)ent, yw = (uint32_t)(ent >> 32);
+      const int sh = x & E_SH_MASK;
+      const int col = (int)((x >> E_COL_SHIFT) & E_COL_MASK) - E_COL_BIAS;
+      const int b = (x >> E_B_SHIFT) & E_B_MASK;
+      if (x & E_INIT) {
+#pragma unroll
+        for (int t = 0; t < T; ++t) M[t] = (y0 + t < g.H) ? colmask : 0u;
+      } else if (x & E_RESTORE) {
+        const int rs = (yw >> E_RSLOT_SHIFT) & E_SLOT_MASK;
+#pragma unroll
+        for (int t = 0; t < T; ++t) M[t] = stack[rs][t];
+      }
+      const uint32_t* rp = base + b * g.stride + col;
+#pragma unroll
+      for (int t = 0; t < T; ++t) {
+        const uint32_t lo = rp[t * g.stride], hi = rp[t * g.stride + 1];
+        M[t] &= __funnelshift_r(lo, hi, sh);
+      }
+      if (x & E_TERMINAL) {
+        int c = 0;
+#pragma unroll
+        for (int t = 0; t < T; ++t) c += __popc(M[t]);
+        c = __reduce_add_sync(0xffffffffu, c);
+        if (c != 0) {
+          if (lane == 0 && b_img < p.B) atomicAdd(cnt + (yw & E_CIDX_MASK), (unsigned long long)c);
+        } else if (p.prune) {
+          e += p.skip[e];            // paper's "enhanced" rule: nothing below can count
+          continue;
+        }
+      }
+      if (x & E_SAVE) {
+        const int ss = (yw >> E_SSLOT_SHIFT) & E_SLOT_MASK;
+#pragma unroll
+        for (int t = 0; t < T; ++t) stack[ss][t] = M[t];
+      }
+    }
+  }
+}
+
+template __global__ void eval_kernel_v1<4>(const EvalParams);
+template __global__ void eval_kernel_v1<8>(const EvalParams);
+template __global__ void eval_kernel_v1<16>(const EvalParams);
+
+// ---------------------------------------------------------------------------------------------
+// mirror: counts[-v] = counts[v] for v in D.  n_arrays = B * n_phase arrays of S*S.
+// ---------------------------------------------------------------------------------------------
+__global__ void mirror_kernel(unsigned long long* counts, int S, long long n_arrays) {
+  const int m = S / 2;
+  const long long K = (long long)S * S;
+  const long long total = n_arrays * K;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total;
+       i += (long long)gridDim.x * blockDim.x) {
+    const long long arr = i / K;
+    const int k = (int)(i - arr * K);
+    const int dy = k / S - m, dx = k % S - m;
+    if (!(dy > 0 || (dy == 0 && dx >= 0))) counts[i] = counts[arr * K + (K - 1 - k)];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// objective: sse[b] = sum_k (c[b][k] - t[k])^2, exact in uint64 (Eq. 14 / Eq. 19).
+// grid = (chunks, B); partial sums are combined with one 64-bit atomic per block.
+// ---------------------------------------------------------------------------------------------
+__global__ void objective_kernel(const long long* __restrict__ counts, const long long* __restrict__ target,
+                                 long long K, unsigned long long* sse) {
+  const int b = blockIdx.y;
+  const long long* c = counts + (size_t)b * K;
+  unsigned long long s = 0;
+  for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < K; k += (long long)gridDim.x * blockDim.x) {
+    const long long d = c[k] - target[k];
+    s += (unsigned long long)(d * d);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+  __shared__ unsigned long long ws[32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) ws[warp] = s;
+  __syncthreads();
+  if (warp == 0) {
+    s = (lane < (int)(blockDim.x >> 5)) ? ws[lane] : 0ull;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if (lane == 0) atomicAdd(sse + b, s);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// swap delta, version 1.  One CTA per proposal.
+//   Bit plane Bp of the base image in shared memory (no halo, modular addressing), and a second
+//   copy Bq with the two bits exchanged.  If the two bits are equal nothing changes.  Otherwise let
+//   u be the pixel whose bit becomes 1 and w the one whose bit becomes 0:
+//     delta(v) = #{k : segment started at u - P_v[k] lies in phase in I'}   (it contains u)
+//              - #{k : segment started at w - P_v[k] lies in phase in I }   (it contains w)
+//   Warp per vector of D, lane per candidate k; the other half is the mirror delta(-v) = delta(v).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool seg_in_phase(const uint32_t* plane, int Wc, int H, int W, const short2* path,
+                                             int len, int sx, int sy) {
+  for (int jx = 0; jx < len; ++jx) {
+    const short2 o = path[jx];
+    int x = sx + o.x, y = sy + o.y;
+    x += (x < 0) ? W : 0;
+    x -= (x >= W) ? W : 0;
+    y += (y < 0) ? H : 0;
+    y -= (y >= H) ? H : 0;
+    if (!((plane[y * Wc + (x >> 5)] >> (x & 31)) & 1u)) return false;
+  }
+  return true;
+}
+
+__global__ void __launch_bounds__(256) swap_delta_kernel_v1(const uint8_t* __restrict__ image, int H, int W, int m,
+                                                             int phase, const int* __restrict__ pairs,
+                                                             const short2* __restrict__ path_xy,
+                                                             const int* __restrict__ path_off,
+                                                             const short2* __restrict__ vecs, int n_half,
+                                                             int* __restrict__ delta) {
+  extern __shared__ __align__(16) uint32_t sm[];
+  const int Wc = (W + 31) >> 5;
+  uint32_t* P0 = sm;                  // base image plane
+  uint32_t* P1 = sm + H * Wc;         // plane after the swap
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
+  const long long sw = blockIdx.x;
+  const int S = 2 * m + 1;
+  int* out = delta + sw * (long long)S * S;
+  const int xp = pairs[4 * sw], yp = pairs[4 * sw + 1], xq = pairs[4 * sw + 2], yq = pairs[4 * sw + 3];
+  const bool ok = xp >= 0 && xp < W && xq >= 0 && xq < W && yp >= 0 && yp < H && yq >= 0 && yq < H;
+  for (int w = warp; w < H * Wc; w += nw) {
+    const int y = w / Wc, x = (w - y * Wc) * 32 + lane;
+    const bool bit = (x < W) && image[(size_t)y * W + x] == (uint8_t)phase;
+    const unsigned v = __ballot_sync(0xffffffffu, bit);
+    if (lane == 0) { P0[w] = v; P1[w] = v; }
+  }
+  __syncthreads();
+  int bp = 0, bq = 0;
+  if (ok) {
+    bp = (P0[yp * Wc + (xp >> 5)] >> (xp & 31)) & 1;
+    bq = (P0[yq * Wc + (xq >> 5)] >> (xq & 31)) & 1;
+  }
+  if (!ok || bp == bq) {              // nothing changes for this phase
+    for (int k = tid; k < S * S; k += blockDim.x) out[k] = 0;
+    return;
+  }
+  __syncthreads();
+  if (tid == 0) {                     // exchange the two bits in P1
+    P1[yp * Wc + (xp >> 5)] ^= 1u << (xp & 31);
+    P1[yq * Wc + (xq >> 5)] ^= 1u << (xq & 31);
+  }
+  __syncthreads();
+  const int ux = bp ? xq : xp, uy = bp ? yq : yp;   // bit 0 -> 1
+  const int wx = bp ? xp : xq, wy = bp ? yp : yq;   // bit 1 -> 0
+  for (int v = warp; v < n_half; v += nw) {
+    const int off = path_off[v], len = path_off[v + 1] - off;
+    const short2* path = path_xy + off;
+    int d = 0;
+    for (int c = lane; c < 2 * len; c += 32) {
+      const int k = (c < len) ? c : c - len;
+      const short2 o = path[k];
+      if (c < len) d += seg_in_phase(P1, Wc, H, W, path, len, ux - o.x, uy - o.y) ? 1 : 0;
+      else d -= seg_in_phase(P0, Wc, H, W, path, len, wx - o.x, wy - o.y) ? 1 : 0;
+    }
+    d = __reduce_add_sync(0xffffffffu, d);
+    if (lane == 0) {
+      const short2 vv = vecs[v];
+      out[(vv.y + m) * S + (vv.x + m)] = d;
+      out[(-vv.y + m) * S + (-vv.x + m)] = d;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host launch wrappers (called from lpf_api.cu)
+// ---------------------------------------------------------------------------------------------
+cudaError_t launch_pack(const uint8_t* images, uint32_t* packed, const Geom& g, int B, int Bpad, int n_phase,
+                        int phase0, unsigned int* counter, int n_sm, cudaStream_t st) {
+  const long long total = (long long)n_phase * Bpad * g.img_words;
+  long long blocks = (total + 7) / 8;
+  if (blocks > (long long)n_sm * 16) blocks = (long long)n_sm * 16;
+  if (blocks < 1) blocks = 1;
+  pack_kernel<<<(unsigned)blocks, 256, 0, st>>>(images, packed, g, B, Bpad, n_phase, phase0, counter);
+  return cudaGetLastError();
+}
+
+typedef void (*eval_fn)(const EvalParams);
+static eval_fn eval_fn_for(int T) {
+  switch (T) {
+    case 4: return eval_kernel_v1<4>;
+    case 8: return eval_kernel_v1<8>;
+    default: return eval_kernel_v1<16>;
+  }
+}
+
+cudaError_t eval_occupancy(int T, int threads, size_t smem, int* blocks_per_sm) {
+  eval_fn f = eval_fn_for(T);
+  cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, f, threads, smem);
+}
+
+cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st) {
+  eval_fn f = eval_fn_for(p.g.T);
+  f<<<grid, threads, smem, st>>>(p);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_mirror(unsigned long long* counts, int S, long long n_arrays, int n_sm, cudaStream_t st) {
+  const long long total = n_arrays * S * S;
+  long long blocks = (total + 255) / 256;
+  if (blocks > (long long)n_sm * 8) blocks = (long long)n_sm * 8;
+  mirror_kernel<<<(unsigned)blocks, 256, 0, st>>>(counts, S, n_arrays);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_objective(const long long* counts, const long long* target, int B, long long K,
+                             unsigned long long* sse, int n_sm, cudaStream_t st) {
+  cudaError_t e = cudaMemsetAsync(sse, 0, sizeof(unsigned long long) * (size_t)B, st);
+  if (e != cudaSuccess) return e;
+  long long chunks = (K + 256 * 8 - 1) / (256 * 8);
+  const long long want = ((long long)n_sm * 8 + B - 1) / B;     // enough blocks to fill the chip
+  if (chunks > want) chunks = want;
+  if (chunks < 1) chunks = 1;
+  // gridDim.y <= 65535: fold larger batches
+  for (int b0 = 0; b0 < B; b0 += 65535) {
+    const int nb = (B - b0 < 65535) ? (B - b0) : 65535;
+    objective_kernel<<<dim3((unsigned)chunks, (unsigned)nb), 256, 0, st>>>(counts + (size_t)b0 * K, target, K,
+                                                                             sse + b0);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t launch_swap_delta(const uint8_t* image, int H, int W, int m, int phase, const int* pairs, long long n,
+                              const int16_t* path_xy, const int* path_off, const int16_t* vecs, int n_half,
+                              int* delta, cudaStream_t st) {
+  const size_t smem = (size_t)2 * H * ((W + 31) / 32) * 4;
+  cudaError_t e = cudaFuncSetAttribute(swap_delta_kernel_v1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  const long long S2 = (long long)(2 * m + 1) * (2 * m + 1);
+  for (long long s0 = 0; s0 < n; s0 += (1ll << 30)) {
+    const long long cnt = (n - s0 < (1ll << 30)) ? (n - s0) : (1ll << 30);
+    swap_delta_kernel_v1<<<(unsigned)cnt, 256, smem, st>>>(image, H, W, m, phase, pairs + 4 * s0,
+                                                          (const short2*)path_xy, path_off, (const short2*)vecs,
+                                                          n_half, delta + s0 * S2);
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace lpf

@@ -1,0 +1,278 @@
+"""Thin ctypes binding over liblpf.so (C ABI: include/lpf.h).  Same names as the C entry points.
+
+Argument marshalling only: every step of the path (bit-pack, trie walk, count, mirror,
+objective, swap delta) runs in the CUDA kernels behind the C ABI.  torch is used for device
+memory and streams.  There is no CPU fallback: if liblpf.so is missing, loading raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "liblpf.so")
+
+LPF_OK, LPF_E_INVAL, LPF_E_NOMEM, LPF_E_CUDA, LPF_E_UNSUPPORTED = 0, -1, -2, -3, -4
+LPF_PRUNE, LPF_NO_TRIE = 1, 2
+
+EXPORTS = (
+    "lpf_strerror", "lpf_last_cuda_error", "lpf_build_paths", "lpf_free_paths", "lpf_paths_info",
+    "lpf_paths_get", "lpf_paths_program", "lpf_eval", "lpf_eval_both", "lpf_objective",
+    "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info",
+)
+
+_lib = None
+
+
+class LpfError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        self.code = code
+        msg = _lib.lpf_strerror(code).decode() if _lib is not None else str(code)
+        if code == LPF_E_CUDA and _lib is not None:
+            msg += " (cudaError %d)" % _lib.lpf_last_cuda_error()
+        super().__init__("%s: %s" % (what, msg))
+
+
+def load() -> ctypes.CDLL:
+    """dlopen liblpf.so.  Raises if it has not been built (python -m paper_1601_04359_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("liblpf.so is not built (%s): run `python -m paper_1601_04359_b200.build`; "
+                           "there is no CPU fallback" % LIB_PATH)
+    lib = ctypes.CDLL(LIB_PATH)
+    I, I64, U, VP = ctypes.c_int, ctypes.c_int64, ctypes.c_uint, ctypes.c_void_p
+    PI64, PI = ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int)
+    lib.lpf_strerror.argtypes = [I]
+    lib.lpf_strerror.restype = ctypes.c_char_p
+    lib.lpf_last_cuda_error.argtypes = []
+    lib.lpf_last_cuda_error.restype = I
+    lib.lpf_build_paths.argtypes = [I, I, ctypes.POINTER(VP)]
+    lib.lpf_build_paths.restype = I
+    lib.lpf_free_paths.argtypes = [VP]
+    lib.lpf_free_paths.restype = None
+    lib.lpf_paths_info.argtypes = [VP, PI64, PI64, PI64, PI]
+    lib.lpf_paths_info.restype = I
+    lib.lpf_paths_get.argtypes = [VP, I, I, VP, I, PI]
+    lib.lpf_paths_get.restype = I
+    lib.lpf_paths_program.argtypes = [VP, I, U, VP, I64, PI64, VP, I64, PI64, PI]
+    lib.lpf_paths_program.restype = I
+    lib.lpf_eval.argtypes = [VP, VP, I, I, I, I, VP, U, VP]
+    lib.lpf_eval.restype = I
+    lib.lpf_eval_both.argtypes = [VP, VP, I, I, I, VP, U, VP]
+    lib.lpf_eval_both.restype = I
+    lib.lpf_objective.argtypes = [VP, VP, I, I64, VP, VP]
+    lib.lpf_objective.restype = I
+    lib.lpf_swap_delta.argtypes = [VP, VP, I, I, I, VP, I64, VP, VP]
+    lib.lpf_swap_delta.restype = I
+    lib.lpf_eval_host.argtypes = [VP, VP, I, I, I, I, VP, U]
+    lib.lpf_eval_host.restype = I
+    lib.lpf_last_launch_info.argtypes = [VP, PI64]
+    lib.lpf_last_launch_info.restype = I
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != LPF_OK:
+        raise LpfError(rc, what)
+
+
+class Paths:
+    """Owner of one `lpf_paths*` (path table + prefix trie + device programs for one m)."""
+
+    def __init__(self, handle: int, m: int, device: int):
+        self._h = ctypes.c_void_p(handle)
+        self.m = m
+        self.device = device
+
+    @property
+    def handle(self) -> ctypes.c_void_p:
+        if not self._h:
+            raise RuntimeError("lpf_paths already freed")
+        return self._h
+
+    def close(self) -> None:
+        if self._h and _lib is not None:
+            _lib.lpf_free_paths(self._h)
+        self._h = ctypes.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def lpf_build_paths(m: int, device: int = 0) -> Paths:
+    """Paper step 1.  device < 0 builds a host-only table (no CUDA call is made)."""
+    lib = load()
+    h = ctypes.c_void_p(None)
+    _check(lib.lpf_build_paths(int(m), int(device), ctypes.byref(h)), "lpf_build_paths")
+    return Paths(h.value, int(m), int(device))
+
+
+def lpf_free_paths(p: Paths) -> None:
+    p.close()
+
+
+def lpf_paths_info(p: Paths) -> dict:
+    lib = load()
+    a, b, c, d = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int()
+    _check(lib.lpf_paths_info(p.handle, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c), ctypes.byref(d)),
+           "lpf_paths_info")
+    return dict(n_half_vectors=a.value, sum_path_len=b.value, n_trie_nodes=c.value, max_depth=d.value)
+
+
+def lpf_paths_get(p: Paths, dx: int, dy: int) -> np.ndarray:
+    """P_v as int16 [len, 2] (x, y), any v of the template."""
+    lib = load()
+    cap = max(abs(int(dx)), abs(int(dy))) + 1
+    xy = np.zeros((cap, 2), dtype=np.int16)
+    n = ctypes.c_int()
+    _check(lib.lpf_paths_get(p.handle, int(dx), int(dy), xy.ctypes.data, cap, ctypes.byref(n)), "lpf_paths_get")
+    return xy[: n.value]
+
+
+def lpf_paths_program(p: Paths, piece_nodes: int = 0, flags: int = 0):
+    """(entries uint64 [n], items int64 [k, 2], n_slots) of the linearised walk program."""
+    lib = load()
+    ne, ni, ns = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int()
+    _check(lib.lpf_paths_program(p.handle, int(piece_nodes), int(flags), None, 0, ctypes.byref(ne), None, 0,
+                                 ctypes.byref(ni), ctypes.byref(ns)), "lpf_paths_program")
+    entries = np.zeros(ne.value, dtype=np.uint64)
+    items = np.zeros((ni.value, 2), dtype=np.int64)
+    _check(lib.lpf_paths_program(p.handle, int(piece_nodes), int(flags), entries.ctypes.data, ne.value,
+                                 ctypes.byref(ne), items.ctypes.data, ni.value, ctypes.byref(ni),
+                                 ctypes.byref(ns)), "lpf_paths_program")
+    return entries, items, ns.value
+
+
+# ---- device entry points (torch tensors in, torch tensors out) -------------------------------
+
+def _torch():
+    import torch
+    return torch
+
+
+def _stream_ptr(stream) -> int:
+    torch = _torch()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def _dev_images(images, ndim: int):
+    torch = _torch()
+    if not (isinstance(images, torch.Tensor) and images.is_cuda and images.dtype == torch.uint8):
+        raise TypeError("images must be a CUDA uint8 tensor")
+    if images.dim() == ndim - 1:
+        images = images.unsqueeze(0)
+    if images.dim() != ndim:
+        raise ValueError("images must be [B, H, W] (or [H, W])")
+    return images.contiguous()
+
+
+def lpf_eval(p: Paths, images, phase: int, flags: int = 0, out=None, stream=None):
+    """counts int64 [B, 2m+1, 2m+1] on the device; index [b, dy+m, dx+m]."""
+    torch = _torch()
+    lib = load()
+    images = _dev_images(images, 3)
+    B, H, W = images.shape
+    S = 2 * p.m + 1
+    if out is None:
+        out = torch.empty((B, S, S), dtype=torch.int64, device=images.device)
+    assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() == B * S * S
+    _check(lib.lpf_eval(p.handle, images.data_ptr(), B, H, W, int(phase), out.data_ptr(), int(flags),
+                        _stream_ptr(stream)), "lpf_eval")
+    return out
+
+
+def lpf_eval_both(p: Paths, images, flags: int = 0, out=None, stream=None):
+    """counts int64 [B, 2, 2m+1, 2m+1]; index [b, phase, dy+m, dx+m]."""
+    torch = _torch()
+    lib = load()
+    images = _dev_images(images, 3)
+    B, H, W = images.shape
+    S = 2 * p.m + 1
+    if out is None:
+        out = torch.empty((B, 2, S, S), dtype=torch.int64, device=images.device)
+    assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() == B * 2 * S * S
+    _check(lib.lpf_eval_both(p.handle, images.data_ptr(), B, H, W, out.data_ptr(), int(flags),
+                             _stream_ptr(stream)), "lpf_eval_both")
+    return out
+
+
+def lpf_objective(counts, target, out=None, stream=None):
+    """sse[b] = sum_k (counts[b, k] - target[k])^2, exact; returned as an int64 tensor holding the
+    uint64 bit pattern (values < 2^63 read directly)."""
+    torch = _torch()
+    lib = load()
+    assert counts.is_cuda and counts.dtype == torch.int64 and target.is_cuda and target.dtype == torch.int64
+    counts = counts.contiguous()
+    target = target.contiguous()
+    K = target.numel()
+    assert K > 0 and counts.numel() % K == 0
+    B = counts.numel() // K
+    if out is None:
+        out = torch.empty((B,), dtype=torch.int64, device=counts.device)
+    with torch.cuda.device(counts.device):
+        _check(lib.lpf_objective(counts.data_ptr(), target.data_ptr(), B, K, out.data_ptr(), _stream_ptr(stream)),
+               "lpf_objective")
+    return out
+
+
+def lpf_swap_delta(p: Paths, image, phase: int, pairs, out=None, stream=None):
+    """delta int32 [n, 2m+1, 2m+1] for n independent two-pixel swaps (pairs int32 [n, 4])."""
+    torch = _torch()
+    lib = load()
+    image = _dev_images(image, 3)
+    if image.shape[0] != 1:
+        raise ValueError("lpf_swap_delta takes one base image")
+    _, H, W = image.shape
+    assert pairs.is_cuda and pairs.dtype == torch.int32 and pairs.dim() == 2 and pairs.shape[1] == 4
+    pairs = pairs.contiguous()
+    n = pairs.shape[0]
+    S = 2 * p.m + 1
+    if out is None:
+        out = torch.empty((n, S, S), dtype=torch.int32, device=image.device)
+    assert out.is_cuda and out.dtype == torch.int32 and out.is_contiguous() and out.numel() == n * S * S
+    _check(lib.lpf_swap_delta(p.handle, image.data_ptr(), H, W, int(phase), pairs.data_ptr(), n, out.data_ptr(),
+                              _stream_ptr(stream)), "lpf_swap_delta")
+    return out
+
+
+def lpf_eval_host(p: Paths, images_host, phase: int, counts_host=None, flags: int = 0):
+    """End-to-end call with HOST buffers (numpy arrays or CPU tensors, ideally pinned): H2D copy,
+    lpf_eval (phase 0/1) or lpf_eval_both (phase < 0), D2H copy, synchronise."""
+    lib = load()
+    a = images_host.numpy() if hasattr(images_host, "numpy") else np.asarray(images_host)
+    if a.dtype != np.uint8 or not a.flags.c_contiguous:
+        raise TypeError("images_host must be C-contiguous uint8")
+    if a.ndim == 2:
+        a = a[None]
+    B, H, W = a.shape
+    S = 2 * p.m + 1
+    shape = (B, 2, S, S) if phase < 0 else (B, S, S)
+    if counts_host is None:
+        counts_host = np.empty(shape, dtype=np.int64)
+    c = counts_host.numpy() if hasattr(counts_host, "numpy") else counts_host
+    assert c.dtype == np.int64 and c.flags.c_contiguous and c.size == int(np.prod(shape))
+    _check(lib.lpf_eval_host(p.handle, a.ctypes.data, B, H, W, int(phase), c.ctypes.data, int(flags)),
+           "lpf_eval_host")
+    return counts_host
+
+
+def lpf_last_launch_info(p: Paths) -> dict:
+    lib = load()
+    out = (ctypes.c_int64 * 8)()
+    _check(lib.lpf_last_launch_info(p.handle, out), "lpf_last_launch_info")
+    keys = ("kernels", "work_items", "program_entries", "grid", "block", "smem_bytes", "T", "G")
+    return dict(zip(keys, [int(v) for v in out]))
+
+
+def normalise(counts, H: int, W: int):
+    """L2 = count / (W*H): one IEEE double division of exact integers (reading S5)."""
+    return np.asarray(counts, dtype=np.float64) / float(int(W) * int(H))
