@@ -125,6 +125,13 @@ int  lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, int H, int W
  * block, dynamic shared memory bytes, words per thread. out = host int64[8]. */
 int  lpf_last_launch_info(const lpf_paths* p, int64_t* out8);
 
+/* Measurement hook: with enable != 0 every lpf_eval / lpf_eval_both on this object
+ * records one CUDA event before and one after the eval kernel (the dominant kernel) on the caller's
+ * stream; lpf_last_eval_kernel_ms waits for the second event and returns the elapsed device time of
+ * the most recent eval kernel in milliseconds.  INVAL if no timed eval has been issued. */
+int  lpf_set_timing(lpf_paths* p, int enable);
+int  lpf_last_eval_kernel_ms(lpf_paths* p, float* ms);
+
 #ifdef __cplusplus
 }
 #endif

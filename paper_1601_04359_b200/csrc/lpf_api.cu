@@ -101,6 +101,8 @@ extern "C" void lpf_free_paths(lpf_paths* p) {
     if (p->d_io_in) cudaFree(p->d_io_in);
     if (p->d_io_out) cudaFree(p->d_io_out);
     if (p->io_stream) cudaStreamDestroy((cudaStream_t)p->io_stream);
+    if (p->ev_start) cudaEventDestroy((cudaEvent_t)p->ev_start);
+    if (p->ev_stop) cudaEventDestroy((cudaEvent_t)p->ev_stop);
   }
   delete p;
 }
@@ -230,7 +232,15 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   ep.prune = (flags & LPF_PRUNE) ? 1 : 0;
   const long long total_work = (long long)ep.n_items * n_groups;
   const int grid = (int)std::min<long long>(total_work, resident);
+  if (p->timing) {
+    if (!p->ev_start) {
+      LPF_CUDA(cudaEventCreate((cudaEvent_t*)&p->ev_start));
+      LPF_CUDA(cudaEventCreate((cudaEvent_t*)&p->ev_stop));
+    }
+    LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_start, st));
+  }
   LPF_CUDA(launch_eval(ep, grid, threads, smem, st));
+  if (p->timing) LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_stop, st));
   LPF_CUDA(launch_mirror((unsigned long long*)counts, S, (long long)B * n_phase, p->n_sm, st));
 
   p->last_info[0] = 3;                                   // kernels launched (pack, eval, mirror)
@@ -254,6 +264,21 @@ extern "C" int lpf_eval(lpf_paths* p, const uint8_t* images, int B, int H, int W
 extern "C" int lpf_eval_both(lpf_paths* p, const uint8_t* images, int B, int H, int W, int64_t* counts,
                              unsigned flags, void* stream) {
   return lpf::eval_impl(p, images, B, H, W, 2, 0, counts, flags, stream);
+}
+
+extern "C" int lpf_set_timing(lpf_paths* p, int enable) {
+  if (!p || p->device < 0) return LPF_E_INVAL;
+  p->timing = enable ? 1 : 0;
+  return LPF_OK;
+}
+
+extern "C" int lpf_last_eval_kernel_ms(lpf_paths* p, float* ms) {
+  if (!p || !ms || p->device < 0 || !p->ev_start) return LPF_E_INVAL;
+  DeviceGuard dg(p->device);
+  if (!dg.ok) return LPF_E_CUDA;
+  LPF_CUDA(cudaEventSynchronize((cudaEvent_t)p->ev_stop));
+  LPF_CUDA(cudaEventElapsedTime(ms, (cudaEvent_t)p->ev_start, (cudaEvent_t)p->ev_stop));
+  return LPF_OK;
 }
 
 extern "C" int lpf_last_launch_info(const lpf_paths* p, int64_t* out8) {

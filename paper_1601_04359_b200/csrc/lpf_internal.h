@@ -91,6 +91,10 @@ struct lpf_paths {
   void* d_io_out = nullptr;
   size_t io_out_bytes = 0;
   void* io_stream = nullptr;
+  // lpf_set_timing: CUDA events recorded around the eval kernel alone
+  int timing = 0;
+  void* ev_start = nullptr;
+  void* ev_stop = nullptr;
   int64_t last_info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 };
 

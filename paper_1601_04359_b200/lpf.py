@@ -20,7 +20,7 @@ LPF_PRUNE, LPF_NO_TRIE = 1, 2
 EXPORTS = (
     "lpf_strerror", "lpf_last_cuda_error", "lpf_build_paths", "lpf_free_paths", "lpf_paths_info",
     "lpf_paths_get", "lpf_paths_program", "lpf_eval", "lpf_eval_both", "lpf_objective",
-    "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info",
+    "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
 )
 
 _lib = None
@@ -72,6 +72,10 @@ def load() -> ctypes.CDLL:
     lib.lpf_eval_host.restype = I
     lib.lpf_last_launch_info.argtypes = [VP, PI64]
     lib.lpf_last_launch_info.restype = I
+    lib.lpf_set_timing.argtypes = [VP, I]
+    lib.lpf_set_timing.restype = I
+    lib.lpf_last_eval_kernel_ms.argtypes = [VP, ctypes.POINTER(ctypes.c_float)]
+    lib.lpf_last_eval_kernel_ms.restype = I
     _lib = lib
     return lib
 
@@ -271,6 +275,16 @@ def lpf_last_launch_info(p: Paths) -> dict:
     _check(lib.lpf_last_launch_info(p.handle, out), "lpf_last_launch_info")
     keys = ("kernels", "work_items", "program_entries", "grid", "block", "smem_bytes", "T", "G")
     return dict(zip(keys, [int(v) for v in out]))
+
+
+def lpf_set_timing(p: Paths, enable: bool) -> None:
+    _check(load().lpf_set_timing(p.handle, int(bool(enable))), "lpf_set_timing")
+
+
+def lpf_last_eval_kernel_ms(p: Paths) -> float:
+    ms = ctypes.c_float()
+    _check(load().lpf_last_eval_kernel_ms(p.handle, ctypes.byref(ms)), "lpf_last_eval_kernel_ms")
+    return float(ms.value)
 
 
 def normalise(counts, H: int, W: int):

@@ -1,0 +1,245 @@
+"""GPU parity: the CUDA path behind the C ABI (liblpf.so) against the CPU oracle, bit-exact
+(integer counts: SURVEY.md 8(c) S14), on the same seeded inputs (paper_1601_04359_b200.inputs).
+
+Small/medium cases compare element by element; the full-size configs 3 and 4 compare sampled
+vectors / images that the oracle can compute one by one, plus properties that hold at any size
+(Eq. 10 and Eq. 12 of the paper; prefix monotonicity)."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import lpf_oracle as orc
+from paper_1601_04359_b200 import inputs, lpf
+
+pytestmark = pytest.mark.gpu
+
+_PATHS = {}
+
+
+def paths(m):
+    if m not in _PATHS:
+        _PATHS[m] = lpf.lpf_build_paths(m, 0)
+    return _PATHS[m]
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_counts(img, phase, m, flags=0):
+    a = img if img.ndim == 3 else img[None]
+    out = lpf.lpf_eval(paths(m), dev(a), phase, flags)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def test_extension_is_loaded_and_device_is_b200_class():
+    lib = lpf.load()
+    assert lib is not None and torch.cuda.is_available()
+    assert torch.cuda.get_device_capability(0)[0] >= 10
+
+
+def test_worked_image_golden_on_gpu():
+    rows = ["110111", "111101", "011111", "111011"]      # tests/golden/worked_image.txt
+    img = np.array([[int(c) for c in r] for r in rows], dtype=np.uint8)
+    c1 = gpu_counts(img, 1, 2)[0]
+    c0 = gpu_counts(img, 0, 2)[0]
+    assert np.array_equal(c1, orc.counts(img, 1, 2, full_template=True))
+    assert np.array_equal(c0, orc.counts(img, 0, 2, full_template=True))
+    assert c1[2, 2] == 20 and c1[2, 3] == 16 and c1[3, 2] == 16 and c0[1, 3] == 1
+
+
+@pytest.mark.parametrize("flags", [0, lpf.LPF_PRUNE, lpf.LPF_NO_TRIE, lpf.LPF_PRUNE | lpf.LPF_NO_TRIE])
+def test_config1_full_template_bit_exact(flags):
+    img = inputs.config_image(1)
+    want = orc.counts(img, 1, 16, full_template=True)      # every vector on its own path, no mirroring
+    got = gpu_counts(img, 1, 16, flags)[0]
+    assert got.dtype == np.int64 and np.array_equal(got, want)
+
+
+SHAPES = [(1, 1, 0), (1, 7, 0), (2, 2, 1), (3, 5, 2), (8, 8, 7), (12, 9, 8), (33, 31, 30), (31, 33, 12),
+          (40, 70, 39), (64, 96, 20), (100, 100, 50), (65, 129, 64), (50, 200, 17), (200, 50, 49)]
+
+
+@pytest.mark.parametrize("H,W,m", SHAPES)
+def test_ragged_shapes_both_phases_all_flags(H, W, m):
+    rng = np.random.default_rng(H * 1000 + W)
+    img = (rng.random((H, W)) < 0.8).astype(np.uint8)
+    img[rng.random((H, W)) < 0.02] = 7                     # bytes other than 0/1 belong to neither phase
+    for phase in (0, 1):
+        want = orc.counts(img, phase, m, full_template=(H * W <= 4096))
+        for flags in (0, lpf.LPF_PRUNE, lpf.LPF_NO_TRIE):
+            got = gpu_counts(img, phase, m, flags)[0]
+            assert np.array_equal(got, want), (phase, flags)
+
+
+def test_degenerate_images():
+    H, W, m = 48, 80, 20
+    S = 2 * m + 1
+    full = np.ones((H, W), dtype=np.uint8)
+    assert np.array_equal(gpu_counts(full, 1, m)[0], np.full((S, S), H * W))
+    assert np.array_equal(gpu_counts(full, 0, m)[0], np.zeros((S, S)))
+    assert np.array_equal(gpu_counts(1 - full, 1, m, lpf.LPF_PRUNE)[0], np.zeros((S, S)))
+    stripes = inputs.stripes(H, W, 8, 3, horizontal=True)
+    got = gpu_counts(stripes, 1, m)[0]
+    dy = np.abs(np.arange(-m, m + 1))[:, None]
+    want = np.broadcast_to(W * (H // 8) * np.maximum(0, 3 - dy), (S, S))
+    assert np.array_equal(got, want)
+
+
+def test_eval_both_and_batch_match_single_calls():
+    rng = np.random.default_rng(5)
+    imgs = (rng.random((5, 40, 64)) < 0.7).astype(np.uint8)
+    m = 24
+    both = lpf.lpf_eval_both(paths(m), dev(imgs)).cpu().numpy()
+    for b in range(5):
+        for phase in (0, 1):
+            assert np.array_equal(both[b, phase], orc.counts(imgs[b], phase, m))
+    one = gpu_counts(imgs, 1, m)
+    assert np.array_equal(one, both[:, 1])
+
+
+def test_error_codes_on_device():
+    p = paths(16)
+    img = dev(np.zeros((1, 16, 64), dtype=np.uint8))
+    with pytest.raises(lpf.LpfError) as e:
+        lpf.lpf_eval(p, img, 1)                            # m > min(H, W) - 1
+    assert e.value.code == lpf.LPF_E_INVAL
+    with pytest.raises(lpf.LpfError) as e:
+        lpf.lpf_eval(p, dev(np.zeros((1, 64, 64), dtype=np.uint8)), 2)
+    assert e.value.code == lpf.LPF_E_INVAL
+
+
+def test_config2_both_phases_bit_exact():
+    img = inputs.config_image(2)
+    got = lpf.lpf_eval_both(paths(128), dev(img[None])).cpu().numpy()[0]
+    for phase in (0, 1):
+        assert np.array_equal(got[phase], orc.counts(img, phase, 128)), phase
+
+
+def _properties(counts, img, phase, m):
+    S = 2 * m + 1
+    assert counts[m, m] == int((img == phase).sum())                 # Eq. 10
+    assert np.array_equal(counts, counts[::-1, ::-1])                 # Eq. 12
+    assert counts.max() == counts[m, m] and counts.min() >= 0
+    ax = counts[m, m:]
+    assert np.all(ax[1:] <= ax[:-1])                                  # axis-aligned: non-increasing
+    ay = counts[m:, m]
+    assert np.all(ay[1:] <= ay[:-1])
+    assert counts.shape == (S, S)
+
+
+def test_config3_sampled_vectors_and_properties():
+    img = inputs.config_image(3)
+    m = 256
+    got = lpf.lpf_eval_both(paths(m), dev(img[None])).cpu().numpy()[0]
+    rng = np.random.default_rng(3)
+    vecs = np.concatenate([rng.integers(-m, m + 1, size=(1500, 2)),
+                           np.array([[0, 0], [m, m], [-m, m], [m, 0], [0, m], [m, -m], [-m, -m], [1, 0], [255, 256],
+                                     [256, 255], [-256, 1], [31, 1], [32, 1], [33, 1], [-31, 2], [-32, 2], [-33, 2]])])
+    for phase in (0, 1):
+        want, _ = orc.counts_list(img, phase, vecs)
+        assert np.array_equal(got[phase][vecs[:, 1] + m, vecs[:, 0] + m], want), phase
+        _properties(got[phase], img, phase, m)
+    pruned = lpf.lpf_eval_both(paths(m), dev(img[None]), lpf.LPF_PRUNE).cpu().numpy()[0]
+    assert np.array_equal(pruned, got)
+
+
+def test_config4_sampled_images_properties_and_objective():
+    B = 1024
+    imgs, target_img = inputs.config4_batch(B)
+    m = 64
+    p = paths(m)
+    d_counts = lpf.lpf_eval(p, dev(imgs), 1)
+    d_target = lpf.lpf_eval(p, dev(target_img[None]), 1)
+    sse = lpf.lpf_objective(d_counts, d_target[0]).cpu().numpy()
+    counts = d_counts.cpu().numpy()
+    target = d_target.cpu().numpy()[0]
+    assert np.array_equal(target, orc.counts(target_img, 1, m))
+    for b in (0, 1, 511, 777, 1023):
+        want = orc.counts(imgs[b], 1, m)
+        assert np.array_equal(counts[b], want), b
+        assert int(sse[b]) == orc.sse(want, target)
+    # every image: Eq. 10, Eq. 12, and the objective recomputed from the GPU counts by the oracle's sse
+    assert np.array_equal(counts[:, m, m], imgs.reshape(B, -1).sum(axis=1))
+    assert np.array_equal(counts, counts[:, ::-1, ::-1])
+    for b in range(0, B, 37):
+        assert int(sse[b]) == orc.sse(counts[b], target)
+    # the same image twice gives sse 0
+    assert int(lpf.lpf_objective(d_target, d_target[0]).cpu().numpy()[0]) == 0
+
+
+def test_objective_exact_large_values():
+    rng = np.random.default_rng(11)
+    c = rng.integers(0, 2 ** 26, size=(7, 4099), dtype=np.int64)
+    t = rng.integers(0, 2 ** 26, size=(4099,), dtype=np.int64)
+    got = lpf.lpf_objective(dev(c), dev(t)).cpu().numpy()
+    for b in range(7):
+        assert int(got[b]) == orc.sse(c[b], t)
+
+
+def test_config5_swap_delta():
+    img = inputs.config_image(5)
+    m = 64
+    p = paths(m)
+    n = 100000
+    pairs = inputs.config5_pairs(img, n)
+    d_img = dev(img[None])
+    d_pairs = dev(pairs)
+    base = lpf.lpf_eval(p, d_img, 1)[0]
+    S = 2 * m + 1
+    # a chunk of the 100000 proposals at a time (6.66 GB of int32 in total)
+    chunk = 10000
+    checked = 0
+    sums = []
+    for s0 in range(0, n, chunk):
+        d = lpf.lpf_swap_delta(p, d_img, 1, d_pairs[s0:s0 + chunk])
+        assert d.shape == (chunk, S, S)
+        assert bool((d[:, m, m] == 0).all())                          # volume fraction preserved
+        assert bool((d == d.flip(1, 2)).all())                        # delta(v) = delta(-v)
+        sums.append(d.sum(dim=(1, 2)).cpu().numpy())
+        if s0 == 0:
+            dn = d[:64].cpu().numpy()
+            # oracle, local form, 24 proposals; full re-evaluation (the definition), 3 proposals
+            for i in range(24):
+                assert np.array_equal(dn[i], orc.swap_delta_local(img, 1, m, pairs[i])), i
+            for i in range(3):
+                assert np.array_equal(dn[i], orc.swap_delta_full(img, 1, m, pairs[i])), i
+            # GPU full re-evaluation of I' for 64 proposals
+            mod = np.repeat(img[None], 64, axis=0)
+            for i in range(64):
+                xp, yp, xq, yq = pairs[i]
+                mod[i, yp, xp], mod[i, yq, xq] = img[yq, xq], img[yp, xp]
+            re = lpf.lpf_eval(p, dev(mod), 1) - base[None]
+            assert np.array_equal(re.cpu().numpy(), dn.astype(np.int64))
+            checked += 64
+    assert checked == 64 and len(sums) == n // chunk
+    # phase 0 deltas of the same proposals
+    d0 = lpf.lpf_swap_delta(p, d_img, 0, d_pairs[:8]).cpu().numpy()
+    for i in range(4):
+        assert np.array_equal(d0[i], orc.swap_delta_local(img, 0, m, pairs[i]))
+
+
+def test_swap_delta_small_and_degenerate_pairs():
+    rng = np.random.default_rng(9)
+    H, W, m = 20, 45, 11
+    img = (rng.random((H, W)) < 0.6).astype(np.uint8)
+    p = paths(m)
+    pairs = inputs.swap_pairs(img, 40, 123)
+    pairs[0] = (3, 4, 3, 4)                                            # same pixel: nothing changes
+    zy, zx = np.nonzero(img == 0)
+    pairs[1] = (zx[0], zy[0], zx[1], zy[1])                            # same phase: nothing changes
+    pairs[2] = (-1, 0, 5, 5)                                           # out of range: all-zero delta
+    got = lpf.lpf_swap_delta(p, dev(img[None]), 1, dev(pairs)).cpu().numpy()
+    assert not got[0].any() and not got[1].any() and not got[2].any()
+    for i in range(3, 40):
+        assert np.array_equal(got[i], orc.swap_delta_full(img, 1, m, pairs[i])), i
+
+
+def test_eval_host_end_to_end_entry():
+    img = inputs.config_image(1)
+    got = lpf.lpf_eval_host(paths(16), img, 1)
+    assert np.array_equal(got[0], orc.counts(img, 1, 16))
+    both = lpf.lpf_eval_host(paths(16), img, -1)
+    assert np.array_equal(both[0, 0], orc.counts(img, 0, 16))

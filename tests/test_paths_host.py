@@ -1,0 +1,139 @@
+"""Host side of liblpf.so (no GPU): C-ABI exports, lpf_build_paths table vs the paper's closed
+forms (Eq. 13, 15-17), vs the worked paths in tests/golden/, and vs the
+oracle's independently written rasteriser; structure of the linearised node program."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import lpf_oracle as orc
+from paper_1601_04359_b200 import build as lpf_build
+from paper_1601_04359_b200 import lpf
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    lpf_build.build()
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "lpf.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(lpf_[a-z_0-9]+)\s*\(", hdr))
+    assert declared == set(lpf.EXPORTS)
+    lib = ctypes.CDLL(lpf.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_error_codes_on_host():
+    lib = lpf.load()
+    h = ctypes.c_void_p()
+    assert lib.lpf_build_paths(-1, -1, ctypes.byref(h)) == lpf.LPF_E_INVAL
+    assert lib.lpf_build_paths(512, -1, ctypes.byref(h)) == lpf.LPF_E_UNSUPPORTED
+    assert lib.lpf_build_paths(3, -1, None) == lpf.LPF_E_INVAL
+    p = lpf.lpf_build_paths(3, -1)
+    with pytest.raises(lpf.LpfError):
+        lpf.lpf_paths_get(p, 4, 0)
+    # a host-only table refuses the device entry points (no CPU fallback)
+    buf = (ctypes.c_uint8 * 64)()
+    out = (ctypes.c_int64 * 49)()
+    assert lib.lpf_eval(p.handle, buf, 1, 8, 8, 1, out, 0, None) == lpf.LPF_E_INVAL
+    assert lib.lpf_swap_delta(p.handle, buf, 8, 8, 1, buf, 1, out, None) == lpf.LPF_E_INVAL
+    assert lib.lpf_strerror(lpf.LPF_E_UNSUPPORTED) == b"unsupported shape"
+    lpf.lpf_free_paths(p)
+
+
+@pytest.mark.parametrize("m", [0, 1, 2, 5, 16, 64])
+def test_table_sizes_closed_forms(m):
+    p = lpf.lpf_build_paths(m, -1)
+    info = lpf.lpf_paths_info(p)
+    # |D| = 2HW - H - W + 1 at H = W = m + 1
+    assert info["n_half_vectors"] == 2 * (m + 1) ** 2 - 2 * (m + 1) + 1
+    # Eq. 17 with W = m + 1: (4 W^3 - 4 W + 3) / 3
+    Wd = m + 1
+    assert info["sum_path_len"] * 3 == 4 * Wd ** 3 - 4 * Wd + 3
+    assert info["max_depth"] == m
+    assert info["n_trie_nodes"] <= info["sum_path_len"]
+
+
+def test_trie_node_counts_of_the_five_configs():
+    # distinct prefixes for m = 16 / 64 / 128
+    for m, n in ((16, 1552), (64, 82072), (128, 635544)):
+        p = lpf.lpf_build_paths(m, -1)
+        assert lpf.lpf_paths_info(p)["n_trie_nodes"] == n
+
+
+def test_worked_paths_golden():
+    p = lpf.lpf_build_paths(8, -1)
+    for line in open(os.path.join(ROOT, "tests", "golden", "worked_paths.txt")):
+        line = line.split("#")[0].strip()
+        if not line:
+            continue
+        head, tail = line.split(":")
+        dx, dy = (int(t) for t in head.split())
+        want = [tuple(int(t) for t in pt.split(",")) for pt in tail.split()]
+        got = [tuple(int(t) for t in r) for r in lpf.lpf_paths_get(p, dx, dy)]
+        assert got == want, (dx, dy)
+
+
+@pytest.mark.parametrize("m", [1, 4, 13, 40])
+def test_closed_form_rasteriser_equals_oracle_incremental_form(m):
+    # two formulations, no shared code: library closed form vs oracle error accumulation
+    p = lpf.lpf_build_paths(m, -1)
+    for dy in range(-m, m + 1):
+        for dx in range(-m, m + 1):
+            assert np.array_equal(lpf.lpf_paths_get(p, dx, dy), orc.path(dx, dy)), (dx, dy)
+
+
+def _decode(entries):
+    x = (entries & np.uint64(0xffffffff)).astype(np.int64)
+    y = (entries >> np.uint64(32)).astype(np.int64)
+    sh = x & 31
+    col = ((x >> 5) & 63) - 16
+    a = col * 32 + sh
+    b = (x >> 11) & 1023
+    return dict(a=a, b=b, terminal=(x >> 21) & 1, save=(x >> 22) & 1, restore=(x >> 23) & 1,
+                init=(x >> 24) & 1, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 63, sslot=(y >> 26) & 63)
+
+
+@pytest.mark.parametrize("m,piece,flags", [(5, 0, 0), (12, 16, 0), (33, 256, 0), (12, 0, lpf.LPF_NO_TRIE),
+                                           (12, 64, lpf.LPF_NO_TRIE)])
+def test_program_walk_reproduces_every_canonical_path_once(m, piece, flags):
+    """Interpret the node program on the host with a stack of pixel lists instead of masks:
+    every terminal must be reached exactly once with exactly the pixel list P_v."""
+    p = lpf.lpf_build_paths(m, -1)
+    entries, items, n_slots = lpf.lpf_paths_program(p, piece, flags)
+    d = _decode(entries)
+    S = 2 * m + 1
+    seen = {}
+    covered = np.zeros(len(entries), dtype=bool)
+    for first, cnt in items:
+        cur, stack = None, {}
+        for e in range(first, first + cnt):
+            assert not covered[e]
+            covered[e] = True
+            if d["init"][e]:
+                cur = []
+            elif d["restore"][e]:
+                cur = list(stack[int(d["rslot"][e])])
+            assert cur is not None
+            cur = cur + [(int(d["a"][e]), int(d["b"][e]))]
+            if d["terminal"][e]:
+                cidx = int(d["cidx"][e])
+                dy, dx = cidx // S - m, cidx % S - m
+                assert (dx, dy) == cur[-1]
+                assert (dx, dy) not in seen
+                seen[(dx, dy)] = cur
+            if d["save"][e]:
+                assert int(d["sslot"][e]) < n_slots
+                stack[int(d["sslot"][e])] = list(cur)
+    assert covered.all()
+    assert len(seen) == 2 * m * m + 2 * m + 1
+    for (dx, dy), pix in seen.items():
+        assert orc.in_half(dx, dy)
+        assert pix == [tuple(int(t) for t in r) for r in orc.path(dx, dy)], (dx, dy)
