@@ -1,0 +1,325 @@
+"""bench.py -- lineal path function throughput on B200 (segment tests/s) and ALU roofline fraction.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg4|cfg2] [--flags prune,notrie]
+    python bench.py --impl reference ...      # the CPU oracle as it stands, bounded sample per step
+
+A step is one pass of the whole hot path (bit-pack + stage, trie walk, count, mirror,
+and for cfg4 the objective) over one batch of synthetic images already resident in HBM.  Nominal
+segment tests of a step = B * n_phases * H * W * (2m+1)^2.  The L2 is flushed
+(256 MiB memset) between timed steps, outside the per-step CUDA-event pairs; the reported time is
+the sum of the K per-step device times, max over ranks.  N > 1: one process per GPU, each rank
+evaluates its own independent images (weak scaling, no data-path collective)."""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1601_04359_b200 import inputs  # noqa: E402  (seeded generators only; no method arithmetic)
+
+METRIC = "segment tests/sec (start-pixel x vector)"
+UNIT = "segment tests/s"
+SM_COUNT = 148
+ALU_LANES_PER_CLK_PER_SM = 64     # 4 sub-partitions x 16 lanes: alu pipe issues one warp instruction per 2 clk
+                                  # per sub-partition (B300_MICROARCH.md "Pipe rates": rt_SMSP = 2)
+
+WORKLOADS = {
+    # name: (config number, H, W, m, phases, images per rank)
+    "cfg2": dict(cfg=2, H=256, W=256, m=128, n_phase=2, B=1),
+    "cfg3": dict(cfg=3, H=512, W=512, m=256, n_phase=2, B=1),
+    "cfg4": dict(cfg=4, H=128, W=128, m=64, n_phase=1, B=1024),
+}
+
+
+def make_images(w, rank):
+    """Synthetic images of the workload for this rank (rank r offsets the seed by 100000 r)."""
+    c = w["cfg"]
+    off = 100000 * rank
+    if c == 2:
+        return inputs.disks(256, 256, 8.0, 0.30, inputs.seed_for(2) + off)[None], None
+    if c == 3:
+        return inputs.gaussian_field(512, 512, 12.0, 0.40, inputs.seed_for(3) + off)[None], None
+    B = w["B"]
+    imgs = np.stack([inputs.disks(128, 128, 6.0, 0.35, inputs.seed_for(4, i) + off) for i in range(B)])
+    target = inputs.disks(128, 128, 6.0, 0.35, inputs.seed_for(4, B) + off)
+    return imgs, target
+
+
+def nominal_tests(w):
+    S = 2 * w["m"] + 1
+    return w["B"] * w["n_phase"] * w["H"] * w["W"] * S * S
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks/throttle reasons sampled during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([t.strip() for t in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+        self.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(w, imgs, seconds_hint, rng_seed=0, n_vec=None):
+    """The oracle as it stands on a bounded sample of the workload: a random subset of template vectors
+    (all start pixels, all phases of the workload) on the first image. Returns (tests, seconds, cores, what)."""
+    from oracle import lpf_oracle as orc
+    m = w["m"]
+    rng = np.random.default_rng(rng_seed)
+    if n_vec is None:
+        n_vec = {2: 6000, 3: 1500, 4: 20000}[w["cfg"]]
+    vecs = rng.integers(-m, m + 1, size=(n_vec, 2))
+    img = imgs[0]
+    t0 = time.perf_counter()
+    cores = 1
+    for phase in ((0, 1) if w["n_phase"] == 2 else (1,)):
+        _, cores = orc.counts_list(img, phase, vecs)
+    dt = time.perf_counter() - t0
+    tests = n_vec * w["H"] * w["W"] * w["n_phase"]
+    what = "%d random template vectors x all %dx%d start pixels x %d phase(s) of image 0" % (
+        n_vec, w["H"], w["W"], w["n_phase"])
+    return tests, dt, cores, what
+
+
+def run_reference(args, w, rank, world):
+    """--impl reference: the CPU oracle (oracle/), unmodified, on the host cores; rank 0 only."""
+    if rank != 0:
+        return
+    imgs, _ = make_images(w, 0)
+    total_tests, total_s, cores, what = 0, 0.0, 1, ""
+    for i in range(args.warmup + args.steps):
+        tests, dt, cores, what = oracle_sample(w, imgs, 0, rng_seed=i, n_vec={2: 2000, 3: 400, 4: 6000}[w["cfg"]])
+        if i >= args.warmup:
+            total_tests += tests
+            total_s += dt
+    value = total_tests / total_s
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_s / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+            "config": {"workload": args.workload_desc, "sample_per_step": what},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--flags", default="")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the secondary workloads in the same JSON line")
+    args = ap.parse_args()
+    w = WORKLOADS[args.workload]
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    S = 2 * w["m"] + 1
+    args.workload_desc = "config %d: %d x %dx%d periodic image(s), %d phase(s), template |dx|,|dy|<=%d (%d vectors)" % (
+        w["cfg"], w["B"], w["H"], w["W"], w["n_phase"], w["m"], S * S)
+    if args.impl == "reference":
+        run_reference(args, w, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1601_04359_b200 import build as lpf_build
+    from paper_1601_04359_b200 import lpf
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    lpf_build.build()
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    flags = 0
+    for f in [t for t in args.flags.split(",") if t]:
+        flags |= {"prune": lpf.LPF_PRUNE, "notrie": lpf.LPF_NO_TRIE}[f]
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def measure(wl, steps, warmup, with_e2e):
+        """Times `steps` steps of workload wl. Returns dict of results for this rank (max over ranks applied)."""
+        imgs, target_img = make_images(wl, rank)
+        p = lpf.lpf_build_paths(wl["m"], local_rank)      # paper step 1: untimed
+        info = lpf.lpf_paths_info(p)
+        d_imgs = torch.from_numpy(imgs).cuda()
+        Sw = 2 * wl["m"] + 1
+        shape = (wl["B"], 2, Sw, Sw) if wl["n_phase"] == 2 else (wl["B"], Sw, Sw)
+        d_counts = torch.empty(shape, dtype=torch.int64, device="cuda")
+        d_target = d_sse = None
+        if target_img is not None:
+            d_target = lpf.lpf_eval(p, torch.from_numpy(target_img[None]).cuda(), 1)[0].clone()
+            d_sse = torch.empty((wl["B"],), dtype=torch.int64, device="cuda")
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        stream = torch.cuda.current_stream()
+        lpf.lpf_set_timing(p, True)
+
+        def step():
+            if wl["n_phase"] == 2:
+                lpf.lpf_eval_both(p, d_imgs, flags, out=d_counts, stream=stream)
+            else:
+                lpf.lpf_eval(p, d_imgs, 1, flags, out=d_counts, stream=stream)
+            if d_target is not None:
+                lpf.lpf_objective(d_counts, d_target, out=d_sse, stream=stream)
+
+        for _ in range(warmup):
+            flush.zero_()
+            step()
+        barrier()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        kernel_ms = []
+        sampler = ClockSampler(local_rank) if (rank == 0 and with_e2e) else None
+        if sampler:
+            sampler.start()
+            time.sleep(0.3)
+        wall0 = time.perf_counter()
+        for i in range(steps):
+            flush.zero_()                         # L2 flush between timed iterations, outside the event pair
+            ev[i][0].record(stream)
+            step()
+            ev[i][1].record(stream)
+            kernel_ms.append(None)
+            ev[i][1].synchronize()
+            kernel_ms[i] = lpf.lpf_last_eval_kernel_ms(p)
+        barrier()
+        wall = time.perf_counter() - wall0
+        clocks = sampler.stop() if sampler else None
+        step_ms = [a.elapsed_time(b) for a, b in ev]
+        total_ms = float(sum(step_ms))
+        launch = lpf.lpf_last_launch_info(p)
+        launches_per_step = launch["kernels"] + (1 if d_target is not None else 0)
+
+        # end to end through the C ABI with HOST buffers: pinned input -> H2D -> hot path -> D2H of the counts
+        e2e = None
+        if with_e2e:
+            h_in = torch.from_numpy(imgs).pin_memory()
+            h_out = torch.empty(shape, dtype=torch.int64).pin_memory()
+            phase_arg = -1 if wl["n_phase"] == 2 else 1
+            k = max(3, min(steps, 5))
+            lpf.lpf_eval_host(p, h_in, phase_arg, h_out, flags)
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(k):
+                lpf.lpf_eval_host(p, h_in, phase_arg, h_out, flags)
+            torch.cuda.synchronize()
+            e2e_s = (time.perf_counter() - t0) / k
+            e2e = {"seconds_per_step": e2e_s, "h2d": int(h_in.numel()), "d2h": int(h_out.numel() * 8)}
+        t = torch.tensor([total_ms, float(np.mean(kernel_ms)), e2e["seconds_per_step"] if e2e else 0.0],
+                         dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, kern_ms, e2e_s = (float(v) for v in t.cpu())
+        lpf.lpf_free_paths(p)
+        return dict(total_ms=total_ms, kernel_ms=kern_ms, e2e_s=e2e_s, e2e=e2e, info=info, launch=launch,
+                    launches_per_step=launches_per_step, clocks=clocks, imgs=imgs, wall=wall)
+
+    r = measure(w, args.steps, args.warmup, True)
+    tests_per_step = nominal_tests(w) * world
+    value = tests_per_step * args.steps / (r["total_ms"] * 1e-3)
+    # roofline of the dominant kernel (eval): algorithmic INT ops per launch:
+    #   per image-phase Nw * (2 * trie nodes + 2 * half vectors): (SHF + LOP3) per word-node, (POPC + IADD) per word-terminal
+    Nw = w["H"] * w["W"] // 32
+    alg_ops = w["B"] * w["n_phase"] * Nw * (2 * r["info"]["n_trie_nodes"] + 2 * r["info"]["n_half_vectors"])
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    peak_ops = SM_COUNT * ALU_LANES_PER_CLK_PER_SM * sm_max_mhz * 1e6
+    achieved = alg_ops / (r["kernel_ms"] * 1e-3)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": r["total_ms"] / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32 bit-planes (u8 pixels in, int64 counts out)", "data": "synthetic",
+        "config": {"workload": args.workload_desc, "images_per_gpu": w["B"], "flags": args.flags or "none",
+                   "l2": "flushed with a 256 MiB memset between timed steps",
+                   "timing": "sum of per-step CUDA-event times on the launch stream, max over ranks",
+                   "launch": r["launch"]},
+        "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_ops / 1e12, "unit": "T int-op/s",
+                     "frac": achieved / peak_ops, "traffic": None,
+                     "kernel": "eval_kernel", "kernel_ms": r["kernel_ms"], "algorithmic_ops_per_launch": alg_ops,
+                     "peak_source": "derived: 148 SM x 64 alu lanes/clk x %.0f MHz (sm_max_mhz of MEASURED_PEAKS.json)"
+                                    % sm_max_mhz,
+                     "kernel_share_of_step": r["kernel_ms"] * args.steps / r["total_ms"]},
+        "e2e": {"value": tests_per_step / r["e2e_s"], "unit": UNIT, "h2d_bytes_per_step": r["e2e"]["h2d"],
+                "d2h_bytes_per_step": r["e2e"]["d2h"]},
+        "gpu_launches": r["launches_per_step"] * args.steps,
+        "clocks": r["clocks"],
+    }
+    if not args.no_extra and world == 1:
+        extra = {}
+        for name in sorted(WORKLOADS):
+            if name == args.workload:
+                continue
+            wl = WORKLOADS[name]
+            rr = measure(wl, max(3, args.steps // 2), 3, False)
+            nw = wl["H"] * wl["W"] // 32
+            ops = wl["B"] * wl["n_phase"] * nw * (2 * rr["info"]["n_trie_nodes"] + 2 * rr["info"]["n_half_vectors"])
+            k = max(3, args.steps // 2)
+            extra[name] = {"value": nominal_tests(wl) * k / (rr["total_ms"] * 1e-3), "unit": UNIT,
+                           "ms_per_step": rr["total_ms"] / k, "kernel_ms": rr["kernel_ms"],
+                           "roofline_frac": ops / (rr["kernel_ms"] * 1e-3) / peak_ops}
+        line["other_workloads"] = extra
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        tests, dt, cores, what = oracle_sample(w, r["imgs"], 20)
+        line["cpu_baseline"] = {"value": tests / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what,
+                                "seconds": dt}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
