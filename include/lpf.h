@@ -42,7 +42,7 @@ extern "C" {
 #define LPF_E_INVAL       -1   /* null pointer, B<1, phase not in {0,1}, m<0, m > min(H,W)-1, pair out of range */
 #define LPF_E_NOMEM       -2   /* host or device allocation failed */
 #define LPF_E_CUDA        -3   /* a CUDA runtime call failed (see lpf_last_cuda_error) */
-#define LPF_E_UNSUPPORTED -4   /* shape outside what the kernels take (m > 511, image+halo > shared memory) */
+#define LPF_E_UNSUPPORTED -4   /* shape outside what the kernels take (m > 511, one row band + halo > shared memory) */
 
 /* flags of lpf_eval / lpf_eval_both */
 #define LPF_PRUNE    1u   /* paper's "enhanced" variant: skip a sub-trie whose running
@@ -74,16 +74,22 @@ int  lpf_paths_info(const lpf_paths* p, int64_t* n_half_vectors, int64_t* sum_pa
  * *len = |P_v|; INVAL if v is outside the template or cap < |P_v|. */
 int  lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, int cap, int* len);
 
-/* Host, for tests and tools: the linearised walk program the eval kernel interprets
- * (DESIGN.md "Node program").  The trie is cut into connected pieces of about `piece_nodes`
- * nodes (<= 0: one piece); each piece is one work item = the chain from the root to the piece
- * root followed by the piece in depth-first order.  flags: 0 or LPF_NO_TRIE.
- *   entries  host [cap_entries] uint64 (may be NULL to query sizes)
- *   items    host [cap_items][2] int64 = (first entry, number of entries) (may be NULL)
- * *n_entries / *n_items / *n_slots (mask-stack slots the program needs) are always written. */
-int  lpf_paths_program(lpf_paths* p, int piece_nodes, unsigned flags,
+/* Host, for tests and tools: the linearised walk program the eval kernel interprets for H x W images
+ * (DESIGN.md "Node program").  Every v in D is walked in one of four octant VIEWS of the image (transposed /
+ * flipped so that the path is x-major with a' >= 0, 0 <= b' <= a'); each octant has its own prefix trie, cut
+ * into connected pieces of about `piece_nodes` nodes (<= 0: one piece per octant); each piece is one item =
+ * the chain from the root to the piece root followed by the piece in depth-first order.  flags: 0 or LPF_NO_TRIE.
+ *   entries  host [cap_entries] uint64 (may be NULL to query sizes); low word: bits 0-4 a' & 31, bit 5 reload,
+ *            6 terminal, 7 save, 8 restore, 9 init, bits 12-31 b' * stride + (a' >> 5); high word: bits 0-19
+ *            (dy+m)*(2m+1) + (dx+m) in IMAGE coordinates, 20-23 restore slot, 24-27 save slot
+ *   items    host [cap_items][4] int64 = (first entry, number of entries, octant, 0) (may be NULL)
+ *   strides  host int[4]: words per packed row of each octant view (decodes b', a' >> 5)
+ * *n_entries / *n_items / *n_slots (mask-stack slots the program needs) are always written.
+ * Octants (view coordinates a', b' from image coordinates a, b): 0: dx>=0, dy<=dx (a,b); 1: dx>=0, dy>dx (b,a);
+ * 2: dx<0, dy>-dx (b,-a); 3: dx<0, dy<=-dx (-a,b). */
+int  lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, unsigned flags,
                        uint64_t* entries, int64_t cap_entries, int64_t* n_entries,
-                       int64_t* items, int64_t cap_items, int64_t* n_items, int* n_slots);
+                       int64_t* items, int64_t cap_items, int64_t* n_items, int* n_slots, int* strides);
 
 /* Paper "steps 2-3" (Alg. 1 / Alg. 2) for a batch of B independent images
  * of one size: translate every segment over every start pixel, compare, count.
@@ -122,7 +128,8 @@ int  lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, int H, int W
 
 /* Counters of the most recent lpf_eval / lpf_eval_both on this object (host values known at
  * launch time): kernels launched, work items, program entries walked per image-phase, grid,
- * block, dynamic shared memory bytes, words per thread. out = host int64[8]. */
+ * block, dynamic shared memory bytes, thread tile code (100 TX + 10 TY + slots % 10), images per CTA.
+ * out = host int64[8]. */
 int  lpf_last_launch_info(const lpf_paths* p, int64_t* out8);
 
 /* Measurement hook: with enable != 0 every lpf_eval / lpf_eval_both on this object

@@ -43,18 +43,45 @@ struct DeviceGuard {   // binds the calling thread to the table's device for the
 static void free_program(Program& pr) {
   if (pr.d_entries) cudaFree(pr.d_entries);
   if (pr.d_skip) cudaFree(pr.d_skip);
-  if (pr.d_items) cudaFree(pr.d_items);
-  pr.d_entries = nullptr; pr.d_skip = nullptr; pr.d_items = nullptr;
+  if (pr.d_work) cudaFree(pr.d_work);
+  pr.d_entries = nullptr; pr.d_skip = nullptr; pr.d_work = nullptr;
 }
 
-static int upload_program(Program& pr) {
-  if (pr.d_entries) return LPF_OK;
-  LPF_CUDA(cudaMalloc(&pr.d_entries, sizeof(uint64_t) * std::max<size_t>(pr.entries.size(), 1)));
-  LPF_CUDA(cudaMalloc(&pr.d_skip, sizeof(uint32_t) * std::max<size_t>(pr.skip.size(), 1)));
-  LPF_CUDA(cudaMalloc(&pr.d_items, sizeof(int64_t) * std::max<size_t>(pr.items.size(), 2)));
-  LPF_CUDA(cudaMemcpy(pr.d_entries, pr.entries.data(), sizeof(uint64_t) * pr.entries.size(), cudaMemcpyHostToDevice));
-  LPF_CUDA(cudaMemcpy(pr.d_skip, pr.skip.data(), sizeof(uint32_t) * pr.skip.size(), cudaMemcpyHostToDevice));
-  LPF_CUDA(cudaMemcpy(pr.d_items, pr.items.data(), sizeof(int64_t) * pr.items.size(), cudaMemcpyHostToDevice));
+// uploads the program (once) and the work list expanded over (row band, strip band) of each octant
+static int upload_program(Program& pr, const Geom& g) {
+  if (!pr.d_entries) {
+    LPF_CUDA(cudaMalloc(&pr.d_entries, sizeof(uint64_t) * (pr.entries.size() + 1)));   // +1: the walker prefetches
+    LPF_CUDA(cudaMalloc(&pr.d_skip, sizeof(uint32_t) * std::max<size_t>(pr.skip.size(), 1)));
+    LPF_CUDA(cudaMemset(pr.d_entries, 0, sizeof(uint64_t) * (pr.entries.size() + 1)));
+    LPF_CUDA(cudaMemcpy(pr.d_entries, pr.entries.data(), sizeof(uint64_t) * pr.entries.size(), cudaMemcpyHostToDevice));
+    LPF_CUDA(cudaMemcpy(pr.d_skip, pr.skip.data(), sizeof(uint32_t) * pr.skip.size(), cudaMemcpyHostToDevice));
+  }
+  int bands[4];
+  bool same = pr.d_work != nullptr;
+  for (int o = 0; o < 4; ++o) {
+    const int sb = (g.v[o].n_strips + g.SB - 1) / g.SB;
+    bands[o] = g.v[o].n_bands * 65536 + sb;
+    same = same && bands[o] == pr.work_bands[o];
+  }
+  if (same) return LPF_OK;
+  if (pr.d_work) { cudaFree(pr.d_work); pr.d_work = nullptr; }
+  std::vector<int32_t> work;
+  const size_t n_items = pr.items.size() / 4;
+  for (size_t i = 0; i < n_items; ++i) {           // items are sorted big first; keep that order
+    const int o = (int)pr.items[4 * i + 2];
+    const int sb = (g.v[o].n_strips + g.SB - 1) / g.SB;
+    for (int band = 0; band < g.v[o].n_bands; ++band)
+      for (int s = 0; s < sb; ++s) {
+        work.push_back((int32_t)pr.items[4 * i]);
+        work.push_back((int32_t)pr.items[4 * i + 1]);
+        work.push_back(o | (s << 4));
+        work.push_back(band);
+      }
+  }
+  pr.n_work = (int64_t)work.size() / 4;
+  LPF_CUDA(cudaMalloc(&pr.d_work, sizeof(int32_t) * std::max<size_t>(work.size(), 4)));
+  LPF_CUDA(cudaMemcpy(pr.d_work, work.data(), sizeof(int32_t) * work.size(), cudaMemcpyHostToDevice));
+  for (int o = 0; o < 4; ++o) pr.work_bands[o] = bands[o];
   return LPF_OK;
 }
 
@@ -113,55 +140,14 @@ namespace lpf {
 
 cudaError_t launch_pack(const uint8_t* images, uint32_t* packed, const Geom& g, int B, int Bpad, int n_phase,
                         int phase0, unsigned int* counter, int n_sm, cudaStream_t st);
-cudaError_t eval_occupancy(int T, int threads, size_t smem, int* blocks_per_sm);
-cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st);
+cudaError_t eval_occupancy(int TX, int NS, int threads, size_t smem, int* blocks_per_sm);
+cudaError_t launch_eval(const EvalParams& p, int NS, int grid, int threads, size_t smem, cudaStream_t st);
 cudaError_t launch_mirror(unsigned long long* counts, int S, long long n_arrays, int n_sm, cudaStream_t st);
 cudaError_t launch_objective(const long long* counts, const long long* target, int B, long long K,
                              unsigned long long* sse, int n_sm, cudaStream_t st);
 cudaError_t launch_swap_delta(const uint8_t* image, int H, int W, int m, int phase, const int* pairs, long long n,
                               const int16_t* path_xy, const int* path_off, const int16_t* vecs, int n_half,
                               int* delta, cudaStream_t st);
-
-// Packed-image geometry and CTA shape for (B, H, W, m).  Returns false if one image does not fit.
-static bool choose_geom(const lpf_paths* p, int B, int H, int W, Geom* out) {
-  Geom g;
-  g.H = H; g.W = W; g.m = p->m;
-  g.Wc = (W + 31) / 32;
-  g.CL = (p->m + 31) / 32;
-  const int CR = p->m / 32 + 1;
-  g.T = 4;
-  for (int T : {16, 8}) {
-    if ((long long)g.Wc * ((H + T - 1) / T) >= 32) { g.T = T; break; }
-  }
-  const int Hpad = (H + g.T - 1) / g.T * g.T;
-  g.rows = Hpad + p->m;
-  g.stride = g.Wc + g.CL + CR;
-  g.tpi = g.Wc * (Hpad / g.T);
-  g.wpi = (g.tpi + 31) / 32;
-  if (g.wpi * 32 > 1024) return false;
-  // pad the row stride so that the 32 lanes of a warp (consecutive word columns, then the next
-  // block of T rows) fall into distinct banks where possible
-  int best_pad = 0, best_conf = 1 << 30;
-  for (int pad = 0; pad < 16; ++pad) {
-    int bank[32] = {0}, conf = 0;
-    for (int l = 0; l < 32; ++l) {
-      const int j = l % g.Wc, rb = l / g.Wc;
-      conf = std::max(conf, ++bank[(rb * g.T * (g.stride + pad) + j) & 31]);
-    }
-    if (conf < best_conf) { best_conf = conf; best_pad = pad; }
-  }
-  g.stride += best_pad;
-  g.img_words = (g.rows * g.stride + 3) / 4 * 4;
-  const size_t img_bytes = (size_t)g.img_words * 4;
-  const size_t smem_cap = (size_t)p->max_smem - 1024;
-  if (img_bytes > smem_cap) return false;
-  int G = std::max(1, 512 / (g.wpi * 32));
-  G = std::min(G, B);
-  G = (int)std::min<size_t>((size_t)G, smem_cap / img_bytes);
-  g.G = std::max(G, 1);
-  *out = g;
-  return true;
-}
 
 static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, int n_phase, int phase0,
                      int64_t* counts, unsigned flags, void* stream) {
@@ -175,36 +161,49 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   if (!dg.ok) return LPF_E_CUDA;
   cudaStream_t st = (cudaStream_t)stream;
   Geom g;
-  if (!choose_geom(p, B, H, W, &g)) return LPF_E_UNSUPPORTED;
-
-  const int threads = g.G * g.wpi * 32;
-  const size_t smem = (size_t)g.G * g.img_words * 4;
-  int occ = 0;
-  LPF_CUDA(eval_occupancy(g.T, threads, smem, &occ));
-  if (occ < 1) return LPF_E_UNSUPPORTED;
+  if (!choose_geom(p->m, H, W, B, p->max_smem, &g)) return LPF_E_UNSUPPORTED;
   const int Bpad = (B + g.G - 1) / g.G * g.G;
-  const int n_groups = (Bpad / g.G) * n_phase;
-  const int resident = p->n_sm * occ;
-
-  // work items: about 12 per resident CTA, pieces of 256 .. 16384 trie nodes
-  const long long n_nodes = (long long)p->nodes.size();
-  long long want_items = std::max<long long>(1, (12ll * resident + n_groups - 1) / n_groups);
-  long long piece = n_nodes / want_items;
-  piece = std::max<long long>(256, std::min<long long>(piece, 16384));
-  // quantise so that nearby shapes share one cached program
-  int q = 256;
-  while (q * 2 <= piece) q *= 2;
-  Program* pr;
-  try {
-    pr = &get_program(p, q, flags);
-  } catch (const std::bad_alloc&) {
-    return LPF_E_NOMEM;
+  long long off = 0;
+  int work_per_item = 0;                           // (row band x strip band) pairs summed over the octants / 4
+  for (int o = 0; o < 4; ++o) {
+    g.v[o].packed_off = off;
+    off += (long long)Bpad * g.v[o].view_words;
+    work_per_item += g.v[o].n_bands * ((g.v[o].n_strips + g.SB - 1) / g.SB);
   }
-  if (pr->n_slots > MAX_SLOTS) return LPF_E_UNSUPPORTED;
-  int rc = upload_program(*pr);
+  g.plane_words = off;
+  work_per_item = std::max(1, work_per_item / 4);
+  const int n_gp = (Bpad / g.G) * n_phase;
+
+  // work items: about 16 per resident CTA, pieces of 512 .. 16384 trie nodes; fewer mask slots than the
+  // kernel provides (a smaller piece needs fewer)
+  const int resident_guess = p->n_sm * 2;
+  long long n_nodes = 0;
+  for (int o = 0; o < 4; ++o) n_nodes += (long long)p->oct[o].size();
+  const long long want_items = std::max<long long>(1, 16ll * resident_guess / ((long long)n_gp * work_per_item));
+  long long piece = n_nodes / want_items;
+  piece = std::max<long long>(512, std::min<long long>(piece, 16384));
+  int q = 512;
+  while (q * 2 <= piece) q *= 2;                   // quantised so that nearby shapes share one cached program
+  Program* pr = nullptr;
+  for (;; q /= 2) {
+    try {
+      pr = &get_program(p, q, flags, g.v[0].stride, g.v[1].stride);
+    } catch (const std::bad_alloc&) {
+      return LPF_E_NOMEM;
+    }
+    if (pr->n_slots <= 10) break;
+    if (q <= 64) return LPF_E_UNSUPPORTED;
+  }
+  const int NS = pr->n_slots <= 6 ? 6 : 10;
+  int rc = upload_program(*pr, g);
   if (rc != LPF_OK) return rc;
 
-  const size_t need = (size_t)n_phase * Bpad * g.img_words * 4;
+  int occ = 0;
+  LPF_CUDA(eval_occupancy(g.TX, NS, g.threads, (size_t)g.smem_bytes, &occ));
+  if (occ < 1) return LPF_E_UNSUPPORTED;
+  const int resident = p->n_sm * occ;
+
+  const size_t need = (size_t)n_phase * (size_t)g.plane_words * 4;
   if (need > p->packed_bytes) {
     if (p->d_packed) { LPF_CUDA(cudaStreamSynchronize(st)); cudaFree(p->d_packed); p->d_packed = nullptr; p->packed_bytes = 0; }
     LPF_CUDA(cudaMalloc(&p->d_packed, need));
@@ -217,11 +216,11 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
 
   EvalParams ep;
   ep.g = g;
-  ep.entries = pr->d_entries;
+  ep.entries = (const uint2*)pr->d_entries;
   ep.skip = pr->d_skip;
-  ep.items = pr->d_items;
-  ep.n_items = (int)(pr->items.size() / 2);
-  ep.n_groups = n_groups;
+  ep.work = (const int4*)pr->d_work;
+  ep.n_work = (int)pr->n_work;
+  ep.n_gp = n_gp;
   ep.B = B;
   ep.n_phase = n_phase;
   ep.packed = p->d_packed;
@@ -230,7 +229,8 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   ep.S = S;
   ep.counter = p->d_counter;
   ep.prune = (flags & LPF_PRUNE) ? 1 : 0;
-  const long long total_work = (long long)ep.n_items * n_groups;
+  const long long total_work = (long long)ep.n_work * n_gp;
+  if (total_work >= (1ll << 32)) return LPF_E_UNSUPPORTED;
   const int grid = (int)std::min<long long>(total_work, resident);
   if (p->timing) {
     if (!p->ev_start) {
@@ -239,17 +239,17 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
     }
     LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_start, st));
   }
-  LPF_CUDA(launch_eval(ep, grid, threads, smem, st));
+  LPF_CUDA(launch_eval(ep, NS, grid, g.threads, (size_t)g.smem_bytes, st));
   if (p->timing) LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_stop, st));
   LPF_CUDA(launch_mirror((unsigned long long*)counts, S, (long long)B * n_phase, p->n_sm, st));
 
   p->last_info[0] = 3;                                   // kernels launched (pack, eval, mirror)
   p->last_info[1] = total_work;
-  p->last_info[2] = (int64_t)pr->entries.size();         // program entries walked per image-phase
+  p->last_info[2] = (int64_t)pr->entries.size();         // program entries (all four octants)
   p->last_info[3] = grid;
-  p->last_info[4] = threads;
-  p->last_info[5] = (int64_t)smem;
-  p->last_info[6] = g.T;
+  p->last_info[4] = g.threads;
+  p->last_info[5] = (int64_t)g.smem_bytes;
+  p->last_info[6] = g.TX * 100 + g.TY * 10 + NS % 10;    // thread tile TX, TY and mask slots (6 or 10 -> 0)
   p->last_info[7] = g.G;
   return LPF_OK;
 }

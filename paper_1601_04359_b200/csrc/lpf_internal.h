@@ -4,6 +4,7 @@
 #pragma once
 #include <cstdint>
 #include <map>
+#include <tuple>
 #include <utility>
 #include <vector>
 
@@ -11,59 +12,86 @@
 
 namespace lpf {
 
+// ---- octant views ----------------------------------------------
+// Every canonical vector v = (dx,dy) in D belongs to one octant; its path is walked on a
+// transposed / flipped VIEW of the image in which it is an x-major first-octant path
+// (a' >= 0, 0 <= b' <= a'), so that the walker only ever moves right along a row or steps down.
+//   o = 0: dx >= 0, dy <= dx      view (x',y') = I[y'][x']        (a',b') = ( a,  b)
+//   o = 1: dx >= 0, dy >  dx      view (x',y') = I[x'][y']        (a',b') = ( b,  a)
+//   o = 2: dx <  0, dy > -dx      view (x',y') = I[x'][-y' mod W] (a',b') = ( b, -a)
+//   o = 3: dx <  0, dy <= -dx     view (x',y') = I[y'][-x' mod W] (a',b') = (-a,  b)
+// The start pixels of a view are a bijection of the start pixels of the image, so the count of
+// a path is the same in its view.
+inline int octant_of(int dx, int dy) {
+  if (dx >= 0) return dy <= dx ? 0 : 1;
+  return dy > -dx ? 2 : 3;
+}
+inline void to_view(int o, int a, int b, int* av, int* bv) {
+  switch (o) {
+    case 0: *av = a; *bv = b; break;
+    case 1: *av = b; *bv = a; break;
+    case 2: *av = b; *bv = -a; break;
+    default: *av = -a; *bv = b; break;
+  }
+}
+inline void from_view(int o, int av, int bv, int* a, int* b) {
+  switch (o) {
+    case 0: *a = av; *b = bv; break;
+    case 1: *a = bv; *b = av; break;
+    case 2: *a = -bv; *b = av; break;
+    default: *a = -av; *b = bv; break;
+  }
+}
+
 // ---- node program entry (uint64), DESIGN.md "Node program" -------------------------------
 // low word x:
-//   [ 0.. 4] sh    = a & 31          bit offset of the window inside its word
-//   [ 5..10] col   = (a >> 5) + 16   word-column offset of the window, arithmetic shift
-//   [11..20] b                        row offset (0..m; canonical half has b >= 0)
-//   [21] TERMINAL  this prefix is a whole path P_v: count it
-//   [22] SAVE      copy the running mask to stack slot sslot (node has >= 2 children in its piece)
-//   [23] RESTORE   parent mask comes from stack slot rslot (not from the previous entry)
-//   [24] INIT      parent mask is "every valid start pixel" (first entry of a work item / chain)
-//   [25] ADV       (direct descents only) b == previous b + 1
-//   [26] RELOAD    (direct descents only) col differs from the previous entry's col
+//   [ 0.. 4] sh      = a' & 31        bit offset of the window inside its word
+//   [ 5] RELOAD      row or word column differs from the previous entry: reload the row strip
+//   [ 6] TERMINAL    this prefix is a whole path P_v: count it
+//   [ 7] SAVE        copy the running mask to stack slot sslot (node has >= 2 children in its piece)
+//   [ 8] RESTORE     parent mask comes from stack slot rslot (not from the previous entry)
+//   [ 9] INIT        parent mask is "every valid start pixel" (first entry of a work item / chain)
+//   [12..31] off     = b' * stride + (a' >> 5), word offset of the window in the packed view
 // high word y:
-//   [ 0..19] cidx  = (b + m) * (2m + 1) + (a + m), index into counts[2m+1][2m+1]
-//   [20..25] rslot
-//   [26..31] sslot
+//   [ 0..19] cidx    = (dy + m) * (2m + 1) + (dx + m), index into counts[2m+1][2m+1] (image coordinates)
+//   [20..23] rslot
+//   [24..27] sslot
 constexpr uint32_t E_SH_MASK = 31u;
-constexpr int E_COL_SHIFT = 5;
-constexpr uint32_t E_COL_MASK = 63u;
-constexpr int E_COL_BIAS = 16;
-constexpr int E_B_SHIFT = 11;
-constexpr uint32_t E_B_MASK = 1023u;
-constexpr uint32_t E_TERMINAL = 1u << 21;
-constexpr uint32_t E_SAVE = 1u << 22;
-constexpr uint32_t E_RESTORE = 1u << 23;
-constexpr uint32_t E_INIT = 1u << 24;
-constexpr uint32_t E_ADV = 1u << 25;
-constexpr uint32_t E_RELOAD = 1u << 26;
+constexpr uint32_t E_RELOAD = 1u << 5;
+constexpr uint32_t E_TERMINAL = 1u << 6;
+constexpr uint32_t E_SAVE = 1u << 7;
+constexpr uint32_t E_RESTORE = 1u << 8;
+constexpr uint32_t E_INIT = 1u << 9;
+constexpr int E_OFF_SHIFT = 12;
 constexpr uint32_t E_CIDX_MASK = (1u << 20) - 1u;
 constexpr int E_RSLOT_SHIFT = 20;
-constexpr int E_SSLOT_SHIFT = 26;
-constexpr uint32_t E_SLOT_MASK = 63u;
+constexpr int E_SSLOT_SHIFT = 24;
+constexpr uint32_t E_SLOT_MASK = 15u;
 
 constexpr int MAX_M = 511;
-constexpr int MAX_SLOTS = 28;   // mask-stack slots the kernels reserve per thread
+constexpr int MAX_SLOTS = 12;   // mask-stack slots the kernels provide per thread
 
 struct Node {
-  int16_t a, b;          // pixel offset of this node (last pixel of the prefix)
+  int16_t a, b;          // pixel offset of this node (last pixel of the prefix), view coordinates
   int32_t parent;
   int32_t first_child;
   int32_t next_sibling;
   int32_t size;          // nodes in the subtree (self included)
   int32_t depth;         // root = 0
-  uint8_t terminal;      // this prefix equals P_(a,b)
+  uint8_t terminal;      // this prefix is a whole path
 };
 
-struct Program {         // one linearisation of the trie (host copy + optional device copy)
+struct Program {         // one linearisation of the four octant tries for one set of view strides
   std::vector<uint64_t> entries;
   std::vector<uint32_t> skip;          // entries in the subtree below each entry (LPF_PRUNE jump)
-  std::vector<int64_t> items;          // [n_items][2] = first entry, count; sorted by count, descending
+  std::vector<int64_t> items;          // [n_items][4] = first entry, count, octant, 0; sorted by count, descending
   int n_slots = 0;
+  int stride[4] = {0, 0, 0, 0};
   uint64_t* d_entries = nullptr;
   uint32_t* d_skip = nullptr;
-  int64_t* d_items = nullptr;
+  int32_t* d_work = nullptr;           // expanded (item x band) list, see lpf_api.cu
+  int64_t n_work = 0;
+  int work_bands[4] = {0, 0, 0, 0};    // bands per octant the work list was expanded for
 };
 
 }  // namespace lpf
@@ -75,8 +103,10 @@ struct lpf_paths {
   int max_smem = 0;                  // opt-in dynamic shared memory per block, bytes
   int64_t n_half = 0;
   int64_t sum_len = 0;
-  std::vector<lpf::Node> nodes;                          // nodes[0] = root (0,0)
-  std::map<std::pair<int, unsigned>, lpf::Program> programs;   // key: (piece_nodes, flags & LPF_NO_TRIE)
+  int64_t n_trie_nodes = 0;          // distinct prefixes of all P_v, v in D (one trie, image coordinates)
+  std::vector<lpf::Node> oct[4];     // per-octant prefix tries in view coordinates; [0] = root (0,0)
+  // key: (piece_nodes, flags & LPF_NO_TRIE, stride0, stride1)   (stride2 = stride1, stride3 = stride0)
+  std::map<std::tuple<int, unsigned, int, int>, lpf::Program> programs;
   // device workspace (grown on demand)
   uint32_t* d_packed = nullptr;
   size_t packed_bytes = 0;
@@ -104,7 +134,7 @@ namespace lpf {
 int canonical_path(int dx, int dy, int16_t* xy);
 inline bool in_half(int dx, int dy) { return dy > 0 || (dy == 0 && dx >= 0); }
 
-// builds (or returns the cached) program for (piece_nodes, flags); host side only
-Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags);
+// builds (or returns the cached) program for (piece_nodes, flags, view strides); host side only
+Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride01, int stride12);
 
 }  // namespace lpf

@@ -1,10 +1,11 @@
 // lpf_kernels.cu -- CUDA kernels of liblpf.so (sm_100a).
-//   pack_kernel       uint8 image -> bit planes, 32 px / word, with the periodic halo laid out
-//                     exactly as the eval kernel wants it in shared memory
-//   eval_kernel<T>    the hot loop: walk the node program with a running AND mask (a3), POPC +
+//   pack_kernel       uint8 image -> bit planes, 32 px / word, four octant views per image, each with
+//                     its periodic halo laid out exactly as the eval kernel wants it in shared memory (a2)
+//   eval_kernel<..>   the hot loop: walk the node program with a running AND mask (a3), POPC +
 //                     warp reduce at terminals (a4), optional zero-mask pruning (a5)
 //   mirror_kernel     counts[-v] = counts[v] (a6)
 //   objective_kernel  sum (c - t)^2 per image (a8, Eq. 14/19)
+//   swap_delta_kernel per-proposal count deltas (a9)
 #include <cuda_runtime.h>
 
 #include "lpf_internal.h"
@@ -13,8 +14,9 @@
 namespace lpf {
 
 // ---------------------------------------------------------------------------------------------
-// bit-pack + halo.  One warp per output word: lane k tests one pixel, __ballot_sync packs.
-// Also zeroes the work-item counter for the eval kernel that follows on the same stream.
+// bit-pack + halo + octant views.  One warp per output word: lane k tests one pixel, __ballot_sync
+// packs.  Also zeroes the work counter for the eval kernel that follows on the same stream.
+//   view o of image I (lpf_internal.h): 0: I[y'][x']  1: I[x'][y']  2: I[x'][-y' mod W]  3: I[y'][-x' mod W]
 // ---------------------------------------------------------------------------------------------
 __global__ void pack_kernel(const uint8_t* __restrict__ images, uint32_t* __restrict__ packed, Geom g, int B,
                             int Bpad, int n_phase, int phase0, unsigned int* counter) {
@@ -22,23 +24,36 @@ __global__ void pack_kernel(const uint8_t* __restrict__ images, uint32_t* __rest
   const int lane = threadIdx.x & 31;
   const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
-  const long long total = (long long)n_phase * Bpad * g.img_words;
+  const long long total = (long long)n_phase * g.plane_words;
   for (long long w = warp; w < total; w += nwarps) {
-    const int word = (int)(w % g.img_words);
-    const long long ib = w / g.img_words;
-    const int b = (int)(ib % Bpad);
-    const int plane = (int)(ib / Bpad);
-    const int r = word / g.stride, i = word - r * g.stride;
+    const int plane = (int)(w / g.plane_words);
+    const long long wp = w - (long long)plane * g.plane_words;
+    int o = 0;
+#pragma unroll
+    for (int k = 1; k < 4; ++k)
+      if (wp >= g.v[k].packed_off) o = k;
+    const ViewGeom& v = g.v[o];
+    const long long rem = wp - v.packed_off;
+    const int b = (int)(rem / v.view_words);
+    const int idx = (int)(rem - (long long)b * v.view_words);
+    const int r = idx / v.stride, i = idx - r * v.stride;
+    const int rows = v.n_bands * g.band_rows + g.m;
     bool bit = false;
-    if (b < B && r < g.rows) {
-      const int y = r % g.H;
-      int x = (32 * (i - g.CL) + lane) % g.W;
-      if (x < 0) x += g.W;
+    if (b < B && r < rows) {
+      const int yv = r % v.Hv;
+      const int xv = (32 * i + lane) % v.Wv;
+      int x, y;
+      switch (o) {
+        case 0: x = xv; y = yv; break;
+        case 1: x = yv; y = xv; break;
+        case 2: x = yv ? g.W - yv : 0; y = xv; break;
+        default: x = xv ? g.W - xv : 0; y = yv; break;
+      }
       const int phase = (n_phase == 2) ? plane : phase0;
       bit = images[((size_t)b * g.H + y) * g.W + x] == (uint8_t)phase;
     }
-    const unsigned v = __ballot_sync(0xffffffffu, bit);
-    if (lane == 0) packed[w] = v;
+    const unsigned word = __ballot_sync(0xffffffffu, bit);
+    if (lane == 0) packed[w] = word;
   }
 }
 
@@ -78,12 +93,20 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, unsigne
 }
 
 // ---------------------------------------------------------------------------------------------
-// eval kernel, version 1 (reference walker: no register caching of rows)
-//   CTA = G images x wpi warps.  Thread tau of an image owns start word column j = tau % Wc and
-//   the T start rows y0 .. y0+T-1, y0 = (tau / Wc) * T.  All warps of a CTA walk the same item.
+// eval kernel, version 2: register strips on octant views.
+//   CTA = G images x wpi warps; every warp of the CTA walks the same work item = (program item, row band,
+//   strip band) on the same phase plane.  Lane = start row inside a block of 32 rows, warp = (strip, row
+//   block): a thread owns the TX x-adjacent start words [strip*TX, strip*TX+TX) of TY start rows (32 apart).
+//   It keeps the TX+1 words of the CURRENT path row in registers (R), so a node that stays in the same row
+//   and word column costs TX x (SHF + LOP3) and no load at all; a node that changes row reloads TX+1 words
+//   (odd row stride: the 32 lanes hit 32 different banks).  Saved masks of the depth-first walk live in
+//   registers too (NS slots, warp-uniform switch).
 // ---------------------------------------------------------------------------------------------
-template <int T>
-__global__ void __launch_bounds__(1024) eval_kernel_v1(const EvalParams p) {
+#define LPF_SLOT_CASES(OP) OP(0) OP(1) OP(2) OP(3) OP(4) OP(5) OP(6) OP(7) OP(8) OP(9)
+
+template <int TX, int TY, int NS>
+__global__ void __launch_bounds__(256, 2) eval_kernel_v2(const EvalParams p) {
+  constexpr int T = TX * TY;
   extern __shared__ __align__(128) uint32_t smem[];
   __shared__ __align__(8) uint64_t bar;
   __shared__ unsigned int s_work;
@@ -91,19 +114,13 @@ __global__ void __launch_bounds__(1024) eval_kernel_v1(const EvalParams p) {
   const Geom& g = p.g;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int img_local = warp / g.wpi;
-  const int tau = (warp % g.wpi) * 32 + lane;
-  const bool active = tau < g.tpi;
-  const int tau_c = active ? tau : 0;
-  const int j = tau_c % g.Wc;
-  const int y0 = (tau_c / g.Wc) * T;
-  const uint32_t* base = smem + (size_t)img_local * g.img_words + y0 * g.stride + j + g.CL;
+  const int ww = warp - img_local * g.wpi;
+  const int strip_l = ww % g.SB, rblk = ww / g.SB;
+  const int row0 = rblk * 32 * TY + lane;               // band-local start row of ty = 0
 
-  uint32_t colmask = 0xffffffffu;                     // start pixels x = 32 j + k < W
-  if (32 * j + 32 > g.W) colmask = (g.W - 32 * j >= 32) ? 0xffffffffu : ((1u << (g.W - 32 * j)) - 1u);
-  if (!active) colmask = 0u;
-
-  uint32_t stack[MAX_SLOTS][T];
   uint32_t M[T];
+  uint32_t R[TY][TX + 1];
+  uint32_t stk[NS][T];
 
   if (tid == 0) {
     mbar_init(&bar, 1);
@@ -111,75 +128,124 @@ __global__ void __launch_bounds__(1024) eval_kernel_v1(const EvalParams p) {
   }
   __syncthreads();
   unsigned parity = 0;
-  const unsigned total_work = (unsigned)p.n_items * (unsigned)p.n_groups;
+  const unsigned total_work = (unsigned)p.n_work * (unsigned)p.n_gp;
   const int groups_per_plane = p.Bpad / g.G;
-  const unsigned img_bytes = (unsigned)g.img_words * 4u * (unsigned)g.G;
 
   for (;;) {
     if (tid == 0) s_work = atomicAdd(p.counter, 1u);
-    __syncthreads();                 // everybody is also done reading the previous image
+    __syncthreads();                 // everybody is also done reading the previous band
     const unsigned work = s_work;
     if (work >= total_work) break;
-    const int item = (int)(work / (unsigned)p.n_groups);    // big items first, over all groups
-    const int gp = (int)(work % (unsigned)p.n_groups);
+    const int wi = (int)(work / (unsigned)p.n_gp);          // big items first, over all groups
+    const int gp = (int)(work - (unsigned)wi * (unsigned)p.n_gp);
     const int plane = gp / groups_per_plane;
-    const int b0 = (gp % groups_per_plane) * g.G;
+    const int b0 = (gp - plane * groups_per_plane) * g.G;
+    const int4 wk = __ldg(p.work + wi);
+    const int o = wk.z & 15, sband = wk.z >> 4, band = wk.w;
+    const ViewGeom& v = g.v[o];
+    const int stride = v.stride;
     if (tid == 0) {
-      mbar_expect_tx(&bar, img_bytes);
-      tma_bulk_g2s(smem, p.packed + ((size_t)plane * p.Bpad + b0) * g.img_words, img_bytes, &bar);
+      const unsigned bytes = (unsigned)v.band_words * 4u;
+      mbar_expect_tx(&bar, bytes * (unsigned)g.G);
+      const uint32_t* src = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b0 * v.view_words +
+                            (size_t)band * g.band_rows * stride;
+      for (int gi = 0; gi < g.G; ++gi)
+        tma_bulk_g2s(smem + (size_t)gi * v.band_words, src + (size_t)gi * v.view_words, bytes, &bar);
     }
+    // per-item thread geometry (the octant decides the view size)
+    const int strip = sband * g.SB + strip_l;
+    const bool active = strip < v.n_strips;
+    const uint32_t* base = smem + (size_t)img_local * v.band_words + row0 * stride + (active ? strip : 0) * TX;
+    const int b_img = b0 + img_local;
+    unsigned long long* cnt = p.counts + ((size_t)b_img * p.n_phase + plane) * (size_t)p.S * p.S;
+    const bool store = (lane == 0) && (b_img < p.B);
     mbar_wait(&bar, parity);
     parity ^= 1u;
     __syncthreads();                 // s_work may be rewritten only after everyone has read it
 
-    const int b_img = b0 + img_local;
-    unsigned long long* cnt = p.counts + ((size_t)b_img * p.n_phase + plane) * (size_t)p.S * p.S;
-    const long long e0 = p.items[2 * item], e1 = e0 + p.items[2 * item + 1];
-    for (long long e = e0; e < e1; ++e) {
-      const uint64_t ent = __ldg(p.entries + e);
-      const uint32_t x = (uint32_t)ent, yw = (uint32_t)(ent >> 32);
-      const int sh = x & E_SH_MASK;
-      const int col = (int)((x >> E_COL_SHIFT) & E_COL_MASK) - E_COL_BIAS;
-      const int b = (x >> E_B_SHIFT) & E_B_MASK;
-      if (x & E_INIT) {
+    const long long e0 = wk.x, e1 = e0 + wk.y;
+    uint2 ent = __ldg(p.entries + e0);
+    for (long long e = e0; e < e1;) {
+      const uint2 nxt = __ldg(p.entries + e + 1);           // the entry array is padded by one
+      const uint32_t x = ent.x;
+      long long ne = e + 1;
+      if (x & (E_INIT | E_RESTORE)) {
+        if (x & E_INIT) {
 #pragma unroll
-        for (int t = 0; t < T; ++t) M[t] = (y0 + t < g.H) ? colmask : 0u;
-      } else if (x & E_RESTORE) {
-        const int rs = (yw >> E_RSLOT_SHIFT) & E_SLOT_MASK;
+          for (int ty = 0; ty < TY; ++ty) {
+            const bool rowok = active && (band * g.band_rows + row0 + ty * 32 < v.Hv);
 #pragma unroll
-        for (int t = 0; t < T; ++t) M[t] = stack[rs][t];
-      }
-      const uint32_t* rp = base + b * g.stride + col;
-#pragma unroll
-      for (int t = 0; t < T; ++t) {
-        const uint32_t lo = rp[t * g.stride], hi = rp[t * g.stride + 1];
-        M[t] &= __funnelshift_r(lo, hi, sh);
-      }
-      if (x & E_TERMINAL) {
-        int c = 0;
-#pragma unroll
-        for (int t = 0; t < T; ++t) c += __popc(M[t]);
-        c = __reduce_add_sync(0xffffffffu, c);
-        if (c != 0) {
-          if (lane == 0 && b_img < p.B) atomicAdd(cnt + (yw & E_CIDX_MASK), (unsigned long long)c);
-        } else if (p.prune) {
-          e += p.skip[e];            // paper's "enhanced" rule: nothing below can count
-          continue;
+            for (int t = 0; t < TX; ++t) {
+              const int nb = v.Wv - 32 * (strip * TX + t);   // start pixels x' < Wv only
+              const uint32_t cm = nb >= 32 ? 0xffffffffu : (nb <= 0 ? 0u : ((1u << nb) - 1u));
+              M[ty * TX + t] = rowok ? cm : 0u;
+            }
+          }
+        } else {
+          switch ((ent.y >> E_RSLOT_SHIFT) & E_SLOT_MASK) {
+#define LPF_RESTORE(s)                                                             \
+  case s:                                                                          \
+    if (s < NS) {                                                                  \
+      _Pragma("unroll") for (int t = 0; t < T; ++t) M[t] = stk[s < NS ? s : 0][t]; \
+    }                                                                              \
+    break;
+            LPF_SLOT_CASES(LPF_RESTORE)
+#undef LPF_RESTORE
+            default: break;
+          }
         }
       }
-      if (x & E_SAVE) {
-        const int ss = (yw >> E_SSLOT_SHIFT) & E_SLOT_MASK;
+      if (x & E_RELOAD) {
+        const uint32_t* rp = base + (x >> E_OFF_SHIFT);
 #pragma unroll
-        for (int t = 0; t < T; ++t) stack[ss][t] = M[t];
+        for (int ty = 0; ty < TY; ++ty)
+#pragma unroll
+          for (int i = 0; i <= TX; ++i) R[ty][i] = rp[ty * 32 * stride + i];
       }
+#pragma unroll
+      for (int ty = 0; ty < TY; ++ty)
+#pragma unroll
+        for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __funnelshift_r(R[ty][t], R[ty][t + 1], x);
+      if (x & (E_TERMINAL | E_SAVE)) {
+        if (x & E_TERMINAL) {
+          int c = 0;
+#pragma unroll
+          for (int t = 0; t < T; ++t) c += __popc(M[t]);
+          c = __reduce_add_sync(0xffffffffu, c);
+          if (c != 0) {
+            if (store) atomicAdd(cnt + (ent.y & E_CIDX_MASK), (unsigned long long)c);
+          } else if (p.prune) {          // paper's "enhanced" rule: nothing below can count
+            ne += __ldg(p.skip + e);
+            ent = __ldg(p.entries + ne);
+            e = ne;
+            continue;
+          }
+        }
+        if (x & E_SAVE) {
+          switch ((ent.y >> E_SSLOT_SHIFT) & E_SLOT_MASK) {
+#define LPF_SAVE(s)                                                                \
+  case s:                                                                          \
+    if (s < NS) {                                                                  \
+      _Pragma("unroll") for (int t = 0; t < T; ++t) stk[s < NS ? s : 0][t] = M[t]; \
+    }                                                                              \
+    break;
+            LPF_SLOT_CASES(LPF_SAVE)
+#undef LPF_SAVE
+            default: break;
+          }
+        }
+      }
+      ent = nxt;
+      e = ne;
     }
   }
 }
 
-template __global__ void eval_kernel_v1<4>(const EvalParams);
-template __global__ void eval_kernel_v1<8>(const EvalParams);
-template __global__ void eval_kernel_v1<16>(const EvalParams);
-
+typedef void (*eval_fn)(const EvalParams);
+static eval_fn eval_fn_for(int TX, int NS) {
+  if (TX == 8) return NS <= 6 ? eval_kernel_v2<8, 1, 6> : eval_kernel_v2<8, 1, 10>;
+  return NS <= 6 ? eval_kernel_v2<4, 2, 6> : eval_kernel_v2<4, 2, 10>;
+}
 // ---------------------------------------------------------------------------------------------
 // mirror: counts[-v] = counts[v] for v in D.  n_arrays = B * n_phase arrays of S*S.
 // ---------------------------------------------------------------------------------------------
@@ -310,32 +376,23 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v1(const uint8_t* __res
 // ---------------------------------------------------------------------------------------------
 cudaError_t launch_pack(const uint8_t* images, uint32_t* packed, const Geom& g, int B, int Bpad, int n_phase,
                         int phase0, unsigned int* counter, int n_sm, cudaStream_t st) {
-  const long long total = (long long)n_phase * Bpad * g.img_words;
+  const long long total = (long long)n_phase * g.plane_words;
   long long blocks = (total + 7) / 8;
-  if (blocks > (long long)n_sm * 16) blocks = (long long)n_sm * 16;
+  if (blocks > (long long)n_sm * 32) blocks = (long long)n_sm * 32;
   if (blocks < 1) blocks = 1;
   pack_kernel<<<(unsigned)blocks, 256, 0, st>>>(images, packed, g, B, Bpad, n_phase, phase0, counter);
   return cudaGetLastError();
 }
 
-typedef void (*eval_fn)(const EvalParams);
-static eval_fn eval_fn_for(int T) {
-  switch (T) {
-    case 4: return eval_kernel_v1<4>;
-    case 8: return eval_kernel_v1<8>;
-    default: return eval_kernel_v1<16>;
-  }
-}
-
-cudaError_t eval_occupancy(int T, int threads, size_t smem, int* blocks_per_sm) {
-  eval_fn f = eval_fn_for(T);
+cudaError_t eval_occupancy(int TX, int NS, int threads, size_t smem, int* blocks_per_sm) {
+  eval_fn f = eval_fn_for(TX, NS);
   cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, f, threads, smem);
 }
 
-cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st) {
-  eval_fn f = eval_fn_for(p.g.T);
+cudaError_t launch_eval(const EvalParams& p, int NS, int grid, int threads, size_t smem, cudaStream_t st) {
+  eval_fn f = eval_fn_for(p.g.TX, NS);
   f<<<grid, threads, smem, st>>>(p);
   return cudaGetLastError();
 }

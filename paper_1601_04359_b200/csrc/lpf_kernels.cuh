@@ -1,40 +1,55 @@
-// lpf_kernels.cuh -- launch parameter blocks shared by lpf_kernels.cu and lpf_api.cu.
+// lpf_kernels.cuh -- geometry and launch parameter blocks shared by lpf_paths.cpp (host geometry),
+// lpf_kernels.cu and lpf_api.cu.  Plain structs, no CUDA types.
 #pragma once
 #include <cstdint>
+#include <vector_types.h>
 
 namespace lpf {
 
-// Geometry of one packed image in HBM / shared memory.
-//   word (r, i), r in [0, rows), i in [0, stride): bit k holds [ I[r mod H][(32 (i - CL) + k) mod W] == phase ]
-//   rows   = Hpad + m            Hpad = ceil(H / T) * T   (start rows padded to whole threads)
-//   stride = Wc + CL + CR (+pad) Wc = ceil(W / 32), CL = ceil(m / 32), CR = floor(m / 32) + 1
+// One octant view of one image in HBM / shared memory.
+//   word (r, i), r in [0, rows), i in [0, stride): bit k holds [ view(x' = (32 i + k) mod Wv, y' = r mod Hv) == phase ]
+//   rows = n_bands * band_rows + m (periodic halo below), stride = n_strips * TX + m / 32 + 1, made odd
+struct ViewGeom {
+  int Hv, Wv;        // view height (rows) and width (pixels): octants 0,3: H,W; octants 1,2: W,H
+  int Wc;            // ceil(Wv / 32) words that hold start pixels
+  int n_strips;      // ceil(Wc / TX) strips of TX words per row
+  int stride;        // words per packed row
+  int n_bands;       // ceil(Hv / band_rows) bands of start rows
+  int band_words;    // (band_rows + m) * stride rounded up to a multiple of 4: one band in shared memory
+  int view_words;    // whole packed view of one image, multiple of 4
+  long long packed_off;   // word offset of this octant's [Bpad][view_words] block inside one phase plane
+};
+
 struct Geom {
   int H, W, m;
-  int T;            // start rows per thread
-  int Wc;           // start word columns
-  int CL;           // halo words on the left
-  int stride;       // words per packed row
-  int rows;         // packed rows
-  int img_words;    // rows * stride rounded up to a multiple of 4 (16-byte TMA granule)
-  int tpi;          // threads per image = Wc * ceil(H / T)
-  int wpi;          // warps per image
-  int G;            // images per CTA
+  int TX, TY;        // thread tile: TX adjacent words x TY start rows (32 rows apart)
+  int band_rows;     // start rows per work item, multiple of 32 * TY
+  int SB;            // strips per work item (<= 8)
+  int wpi;           // warps per image band = SB * band_rows / (32 TY)
+  int G;             // images per CTA
+  int threads;       // G * wpi * 32
+  int smem_bytes;    // G * max band_words * 4
+  ViewGeom v[4];
+  long long plane_words;  // words of one phase plane: Bpad * sum_o view_words
 };
+
+// host: pick the geometry for (m, H, W, B); false if one band does not fit in shared memory
+bool choose_geom(int m, int H, int W, int B, int max_smem, Geom* out);
 
 struct EvalParams {
   Geom g;
-  const uint64_t* entries;
+  const uint2* entries;
   const uint32_t* skip;
-  const int64_t* items;       // [n_items][2]
-  int n_items;
-  int n_groups;               // ceil(B / G) * n_phase
+  const int4* work;           // [n_work] = first entry, count, octant | strip band << 4, row band; big first
+  int n_work;
+  int n_gp;                   // ceil(B / G) * n_phase (image group x phase plane)
   int B;
   int n_phase;                // 1 or 2 phase planes in `packed`
-  const uint32_t* packed;     // [n_phase][Bpad][img_words], Bpad = ceil(B / G) * G
+  const uint32_t* packed;     // [n_phase][4 octants][Bpad][view_words]
   int Bpad;
   unsigned long long* counts; // [B][n_phase][S][S]
   int S;                      // 2m + 1
-  unsigned int* counter;      // dynamic work-item counter, zeroed by the pack kernel
+  unsigned int* counter;      // dynamic work counter, zeroed by the pack kernel
   int prune;
 };
 

@@ -1,10 +1,11 @@
 // lpf_paths.cpp -- host side of liblpf.so: paper "step 1".
 //   * closed-form Bresenham rasteriser for the canonical half D (Eq. 13)
-//   * prefix trie over all P_v, |dx|,|dy| <= m
-//   * partition of the trie into work items and linearisation into the node program that
+//   * prefix tries over all P_v, |dx|,|dy| <= m, one per octant in that octant's view coordinates
+//   * partition of the tries into work items and linearisation into the node program that
 //     the eval kernel interprets
 // No CUDA calls here.  Shares nothing with oracle/ (which rasterises incrementally).
 #include <algorithm>
+#include <array>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -37,12 +38,32 @@ int canonical_path(int dx, int dy, int16_t* xy) {
   return n + 1;
 }
 
+// inserts the pixel list xy[1..len-1] (already in the trie's coordinates) below the root
+static void trie_insert(std::vector<Node>& nd, const int16_t* xy, int len) {
+  int cur = 0;
+  for (int k = 1; k < len; ++k) {
+    const int16_t a = xy[2 * k], b = xy[2 * k + 1];
+    int c = nd[cur].first_child;
+    while (c >= 0 && !(nd[c].a == a && nd[c].b == b)) c = nd[c].next_sibling;
+    if (c < 0) {
+      c = (int)nd.size();
+      nd.push_back(Node{a, b, cur, -1, nd[cur].first_child, 1, nd[cur].depth + 1, 0});
+      nd[cur].first_child = c;
+    }
+    cur = c;
+  }
+  nd[cur].terminal = 1;
+}
+
 static void build_trie(lpf_paths* p) {
   const int m = p->m;
-  std::vector<Node>& nd = p->nodes;
-  nd.clear();
-  nd.push_back(Node{0, 0, -1, -1, -1, 1, 0, 0});
-  std::vector<int16_t> xy(2 * (size_t)(m + 1));
+  std::vector<Node> all;   // one trie over D in image coordinates: only its size is kept (lpf_paths_info)
+  all.push_back(Node{0, 0, -1, -1, -1, 1, 0, 0});
+  for (int o = 0; o < 4; ++o) {
+    p->oct[o].clear();
+    p->oct[o].push_back(Node{0, 0, -1, -1, -1, 1, 0, 0});
+  }
+  std::vector<int16_t> xy(2 * (size_t)(m + 1)), vxy(2 * (size_t)(m + 1));
   p->n_half = 0;
   p->sum_len = 0;
   for (int dy = 0; dy <= m; ++dy)
@@ -51,61 +72,58 @@ static void build_trie(lpf_paths* p) {
       const int len = canonical_path(dx, dy, xy.data());
       p->n_half += 1;
       p->sum_len += len;
-      int cur = 0;
-      for (int k = 1; k < len; ++k) {
-        const int16_t a = xy[2 * k], b = xy[2 * k + 1];
-        int c = nd[cur].first_child;
-        while (c >= 0 && !(nd[c].a == a && nd[c].b == b)) c = nd[c].next_sibling;
-        if (c < 0) {
-          c = (int)nd.size();
-          nd.push_back(Node{a, b, cur, -1, nd[cur].first_child, 1, nd[cur].depth + 1, 0});
-          nd[cur].first_child = c;
-        }
-        cur = c;
+      trie_insert(all, xy.data(), len);
+      const int o = octant_of(dx, dy);
+      for (int k = 0; k < len; ++k) {
+        int av, bv;
+        to_view(o, xy[2 * k], xy[2 * k + 1], &av, &bv);
+        vxy[2 * k] = (int16_t)av;
+        vxy[2 * k + 1] = (int16_t)bv;
       }
-      nd[cur].terminal = 1;
+      trie_insert(p->oct[o], vxy.data(), len);
     }
+  p->n_trie_nodes = (int64_t)all.size();
   // children are created after their parent, so a reverse sweep accumulates subtree sizes
-  for (int i = (int)nd.size() - 1; i > 0; --i) nd[nd[i].parent].size += nd[i].size;
+  for (int o = 0; o < 4; ++o) {
+    std::vector<Node>& nd = p->oct[o];
+    for (int i = (int)nd.size() - 1; i > 0; --i) nd[nd[i].parent].size += nd[i].size;
+  }
 }
 
 // ---- program emission ----------------------------------------------------------------------
 
-static inline uint64_t make_entry(int m, int a, int b, uint32_t flags, int rslot, int sslot) {
-  const uint32_t sh = (uint32_t)(a & 31);
-  const uint32_t col = (uint32_t)((a >> 5) + E_COL_BIAS);   // arithmetic shift: floor(a / 32)
-  const uint32_t x = sh | (col << E_COL_SHIFT) | ((uint32_t)b << E_B_SHIFT) | flags;
-  const uint32_t cidx = (uint32_t)((b + m) * (2 * m + 1) + (a + m));
-  const uint32_t y = cidx | ((uint32_t)rslot << E_RSLOT_SHIFT) | ((uint32_t)sslot << E_SSLOT_SHIFT);
-  return (uint64_t)x | ((uint64_t)y << 32);
-}
-
 struct Emitter {
-  const lpf_paths* p;
+  int m, o, stride;
   const std::vector<Node>& nd;
   const std::vector<uint8_t>& cut;      // node is the root of a piece
   const std::vector<int32_t>& psize;    // nodes of the subtree that stay in the node's own piece
   Program& out;
   int max_slots = 0;
 
-  uint32_t step_flags(int node, int prev) const {   // ADV / RELOAD of a direct descent prev -> node
-    uint32_t f = 0;
-    if (nd[node].b == nd[prev].b + 1) f |= E_ADV;
-    if ((nd[node].a >> 5) != (nd[prev].a >> 5)) f |= E_RELOAD;
-    return f;
+  // prev: the node whose row strip is in the registers when this entry runs (-1: none)
+  uint64_t entry(int node, uint32_t flags, int prev, int rslot, int sslot) const {
+    const int a = nd[node].a, b = nd[node].b;      // view coordinates: a >= 0, 0 <= b <= a
+    const bool direct = !(flags & (E_RESTORE | E_INIT));
+    if (!direct || prev < 0 || nd[prev].b != b || (nd[prev].a >> 5) != (a >> 5)) flags |= E_RELOAD;
+    const uint32_t off = (uint32_t)(b * stride + (a >> 5));
+    const uint32_t x = (uint32_t)(a & 31) | flags | (off << E_OFF_SHIFT);
+    int ia, ib;
+    from_view(o, a, b, &ia, &ib);
+    const uint32_t cidx = (uint32_t)((ib + m) * (2 * m + 1) + (ia + m));
+    const uint32_t y = cidx | ((uint32_t)rslot << E_RSLOT_SHIFT) | ((uint32_t)sslot << E_SSLOT_SHIFT);
+    return (uint64_t)x | ((uint64_t)y << 32);
   }
 
   // emits `node` and the part of its subtree inside the piece. src: 0 direct, 1 restore(rslot), 2 init.
-  void emit(int node, int src, int rslot, int depth_slots) {
+  void emit(int node, int src, int rslot, int depth_slots, bool count_it) {
     std::vector<int> kids;
     for (int c = nd[node].first_child; c >= 0; c = nd[c].next_sibling)
       if (!cut[c]) kids.push_back(c);
     // heaviest child last: its descent frees the slot, so live slots <= log2(piece size) + 1
     std::stable_sort(kids.begin(), kids.end(), [&](int x, int y) { return psize[x] < psize[y]; });
-    uint32_t flags = nd[node].terminal ? E_TERMINAL : 0u;
+    uint32_t flags = (nd[node].terminal && count_it) ? E_TERMINAL : 0u;
     if (src == 1) flags |= E_RESTORE;
     if (src == 2) flags |= E_INIT;
-    if (src == 0) flags |= step_flags(node, nd[node].parent);
     int sslot = 0;
     if (kids.size() >= 2) {
       flags |= E_SAVE;
@@ -113,17 +131,17 @@ struct Emitter {
       max_slots = std::max(max_slots, depth_slots + 1);
     }
     const size_t at = out.entries.size();
-    out.entries.push_back(make_entry(p->m, nd[node].a, nd[node].b, flags, rslot, sslot));
+    out.entries.push_back(entry(node, flags, nd[node].parent, rslot, sslot));
     out.skip.push_back(0);
     for (size_t i = 0; i < kids.size(); ++i) {
       if (kids.size() == 1) {
-        emit(kids[i], 0, 0, depth_slots);
+        emit(kids[i], 0, 0, depth_slots, true);
       } else if (i == 0) {
-        emit(kids[i], 0, 0, depth_slots + 1);
+        emit(kids[i], 0, 0, depth_slots + 1, true);
       } else if (i + 1 < kids.size()) {
-        emit(kids[i], 1, sslot, depth_slots + 1);
+        emit(kids[i], 1, sslot, depth_slots + 1, true);
       } else {
-        emit(kids[i], 1, sslot, depth_slots);      // last child: the slot is free again
+        emit(kids[i], 1, sslot, depth_slots, true);      // last child: the slot is free again
       }
     }
     out.skip[at] = (uint32_t)(out.entries.size() - at - 1);
@@ -131,48 +149,54 @@ struct Emitter {
 };
 
 static void sort_items(Program& pr) {
-  const size_t n = pr.items.size() / 2;
-  std::vector<std::pair<int64_t, int64_t>> v(n);
-  for (size_t i = 0; i < n; ++i) v[i] = {pr.items[2 * i], pr.items[2 * i + 1]};
-  std::stable_sort(v.begin(), v.end(), [](const std::pair<int64_t, int64_t>& a,
-                                          const std::pair<int64_t, int64_t>& b) { return a.second > b.second; });
-  for (size_t i = 0; i < n; ++i) {
-    pr.items[2 * i] = v[i].first;
-    pr.items[2 * i + 1] = v[i].second;
-  }
+  const size_t n = pr.items.size() / 4;
+  std::vector<std::array<int64_t, 4>> v(n);
+  for (size_t i = 0; i < n; ++i)
+    v[i] = {pr.items[4 * i], pr.items[4 * i + 1], pr.items[4 * i + 2], pr.items[4 * i + 3]};
+  std::stable_sort(v.begin(), v.end(),
+                   [](const std::array<int64_t, 4>& a, const std::array<int64_t, 4>& b) { return a[1] > b[1]; });
+  for (size_t i = 0; i < n; ++i)
+    for (int k = 0; k < 4; ++k) pr.items[4 * i + k] = v[i][k];
+}
+
+static void push_item(Program& pr, int64_t first, int o) {
+  pr.items.push_back(first);
+  pr.items.push_back((int64_t)pr.entries.size() - first);
+  pr.items.push_back(o);
+  pr.items.push_back(0);
 }
 
 static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
-  const std::vector<Node>& nd = p->nodes;
-  const int N = (int)nd.size();
-  std::vector<uint8_t> cut(N, 0);
-  std::vector<int32_t> psize(N, 1);
-  // greedy bottom-up partition: a node whose residual subtree reaches piece_nodes starts a piece
-  for (int i = N - 1; i > 0; --i) {
-    if (piece_nodes > 0 && psize[i] >= piece_nodes) cut[i] = 1;
-    else psize[nd[i].parent] += psize[i];
-  }
-  cut[0] = 1;
-  Emitter em{p, nd, cut, psize, pr};
-  std::vector<int> chain;
-  for (int r = 0; r < N; ++r) {
-    if (!cut[r]) continue;
-    const int64_t first = (int64_t)pr.entries.size();
-    // chain root -> parent(r): recomputed per item, never counted, never saved
-    chain.clear();
-    for (int u = nd[r].parent; u >= 0; u = nd[u].parent) chain.push_back(u);
-    std::reverse(chain.begin(), chain.end());
-    for (size_t i = 0; i < chain.size(); ++i) {
-      const int u = chain[i];
-      const uint32_t f = (i == 0) ? E_INIT : em.step_flags(u, chain[i - 1]);
-      pr.entries.push_back(make_entry(p->m, nd[u].a, nd[u].b, f, 0, 0));
-      pr.skip.push_back(0);
+  for (int o = 0; o < 4; ++o) {
+    const std::vector<Node>& nd = p->oct[o];
+    const int N = (int)nd.size();
+    std::vector<uint8_t> cut(N, 0);
+    std::vector<int32_t> psize(N, 1);
+    // greedy bottom-up partition: a node whose residual subtree reaches piece_nodes starts a piece
+    for (int i = N - 1; i > 0; --i) {
+      if (piece_nodes > 0 && psize[i] >= piece_nodes) cut[i] = 1;
+      else psize[nd[i].parent] += psize[i];
     }
-    em.emit(r, chain.empty() ? 2 : 0, 0, 0);
-    pr.items.push_back(first);
-    pr.items.push_back((int64_t)pr.entries.size() - first);
+    cut[0] = 1;
+    Emitter em{p->m, o, pr.stride[o], nd, cut, psize, pr};
+    std::vector<int> chain;
+    for (int r = 0; r < N; ++r) {
+      if (!cut[r]) continue;
+      if (r == 0 && o != 0 && psize[0] == 1) continue;   // v = 0 is counted in octant 0 only
+      const int64_t first = (int64_t)pr.entries.size();
+      // chain root -> parent(r): recomputed per item, never counted, never saved
+      chain.clear();
+      for (int u = nd[r].parent; u >= 0; u = nd[u].parent) chain.push_back(u);
+      std::reverse(chain.begin(), chain.end());
+      for (size_t i = 0; i < chain.size(); ++i) {
+        pr.entries.push_back(em.entry(chain[i], i == 0 ? E_INIT : 0u, i == 0 ? -1 : chain[i - 1], 0, 0));
+        pr.skip.push_back(0);
+      }
+      em.emit(r, chain.empty() ? 2 : 0, 0, 0, !(r == 0 && o != 0));
+      push_item(pr, first, o);
+    }
+    pr.n_slots = std::max(pr.n_slots, em.max_slots);
   }
-  pr.n_slots = em.max_slots;
   sort_items(pr);
 }
 
@@ -180,43 +204,47 @@ static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
 static void build_chain_program(lpf_paths* p, int piece_nodes, Program& pr) {
   const int m = p->m;
   std::vector<int16_t> xy(2 * (size_t)(m + 1));
-  int64_t first = 0;
-  for (int dy = 0; dy <= m; ++dy)
-    for (int dx = -m; dx <= m; ++dx) {
-      if (!in_half(dx, dy)) continue;
-      const int len = canonical_path(dx, dy, xy.data());
-      for (int k = 0; k < len; ++k) {
-        uint32_t f = (k == 0) ? E_INIT : 0u;
-        if (k > 0) {
-          if (xy[2 * k + 1] == xy[2 * k - 1] + 1) f |= E_ADV;
-          if ((xy[2 * k] >> 5) != (xy[2 * k - 2] >> 5)) f |= E_RELOAD;
+  for (int o = 0; o < 4; ++o) {
+    int64_t first = (int64_t)pr.entries.size();
+    const int stride = pr.stride[o];
+    for (int dy = 0; dy <= m; ++dy)
+      for (int dx = -m; dx <= m; ++dx) {
+        if (!in_half(dx, dy) || octant_of(dx, dy) != o) continue;
+        const int len = canonical_path(dx, dy, xy.data());
+        int pa = 0, pb = 0;
+        for (int k = 0; k < len; ++k) {
+          int a, b;
+          to_view(o, xy[2 * k], xy[2 * k + 1], &a, &b);
+          uint32_t f = (k == 0) ? (E_INIT | E_RELOAD) : 0u;
+          if (k > 0 && (b != pb || (a >> 5) != (pa >> 5))) f |= E_RELOAD;
+          if (k == len - 1) f |= E_TERMINAL;
+          const uint32_t off = (uint32_t)(b * stride + (a >> 5));
+          const uint32_t x = (uint32_t)(a & 31) | f | (off << E_OFF_SHIFT);
+          const uint32_t cidx = (uint32_t)((dy + m) * (2 * m + 1) + (dx + m));
+          pr.entries.push_back((uint64_t)x | ((uint64_t)cidx << 32));
+          pr.skip.push_back(0);
+          pa = a;
+          pb = b;
         }
-        if (k == len - 1) f |= E_TERMINAL;
-        pr.entries.push_back(make_entry(m, xy[2 * k], xy[2 * k + 1], f, 0, 0));
-        pr.skip.push_back(0);
+        if (piece_nodes > 0 && (int64_t)pr.entries.size() - first >= piece_nodes) {
+          push_item(pr, first, o);
+          first = (int64_t)pr.entries.size();
+        }
       }
-      const int64_t cur = (int64_t)pr.entries.size();
-      if (piece_nodes > 0 && cur - first >= piece_nodes) {
-        pr.items.push_back(first);
-        pr.items.push_back(cur - first);
-        first = cur;
-      }
-    }
-  const int64_t cur = (int64_t)pr.entries.size();
-  if (cur > first) {
-    pr.items.push_back(first);
-    pr.items.push_back(cur - first);
+    if ((int64_t)pr.entries.size() > first) push_item(pr, first, o);
   }
   pr.n_slots = 0;
   sort_items(pr);
 }
 
-Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags) {
+Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12) {
   if (piece_nodes < 0) piece_nodes = 0;
-  const std::pair<int, unsigned> key(piece_nodes, flags & LPF_NO_TRIE);
+  const std::tuple<int, unsigned, int, int> key(piece_nodes, flags & LPF_NO_TRIE, stride03, stride12);
   auto it = p->programs.find(key);
   if (it != p->programs.end()) return it->second;
   Program& pr = p->programs[key];
+  pr.stride[0] = pr.stride[3] = stride03;
+  pr.stride[1] = pr.stride[2] = stride12;
   if (flags & LPF_NO_TRIE) build_chain_program(p, piece_nodes, pr);
   else build_trie_program(p, piece_nodes, pr);
   return pr;
@@ -229,6 +257,66 @@ int build_host_table(lpf_paths* p) {
     return LPF_E_NOMEM;
   }
   return LPF_OK;
+}
+
+}  // namespace lpf
+
+// ---- geometry (host only) ---------------------------------------------
+
+#include "lpf_kernels.cuh"
+
+namespace lpf {
+
+bool choose_geom(int m, int H, int W, int B, int max_smem, Geom* out) {
+  Geom g;
+  std::memset(&g, 0, sizeof(g));
+  g.H = H; g.W = W; g.m = m;
+  const int wc_max = (std::max(H, W) + 31) / 32;
+  g.TX = wc_max >= 8 ? 8 : 4;
+  g.TY = 8 / g.TX;
+  const int rows_per_warp = 32 * g.TY;
+  int strips_max = 0, hv_max = 0;
+  for (int o = 0; o < 4; ++o) {
+    ViewGeom& v = g.v[o];
+    const bool tr = (o == 1 || o == 2);
+    v.Hv = tr ? W : H;
+    v.Wv = tr ? H : W;
+    v.Wc = (v.Wv + 31) / 32;
+    v.n_strips = (v.Wc + g.TX - 1) / g.TX;
+    v.stride = v.n_strips * g.TX + m / 32 + 1;
+    if (!(v.stride & 1)) v.stride += 1;          // odd: 32 consecutive rows of one column hit 32 banks
+    strips_max = std::max(strips_max, v.n_strips);
+    hv_max = std::max(hv_max, v.Hv);
+  }
+  int row_blocks = std::max(1, 8 / strips_max);
+  const int max_blocks = (hv_max + rows_per_warp - 1) / rows_per_warp;
+  row_blocks = std::min(row_blocks, max_blocks);
+  for (;;) {
+    g.band_rows = rows_per_warp * row_blocks;
+    g.SB = std::min(strips_max, 8);
+    g.wpi = g.SB * row_blocks;
+    int bw_max = 0;
+    for (int o = 0; o < 4; ++o) {
+      ViewGeom& v = g.v[o];
+      v.n_bands = (v.Hv + g.band_rows - 1) / g.band_rows;
+      v.band_words = ((g.band_rows + m) * v.stride + 3) / 4 * 4;
+      v.view_words = ((v.n_bands * g.band_rows + m) * v.stride + 3) / 4 * 4 + 4;
+      bw_max = std::max(bw_max, v.band_words);
+    }
+    if (g.wpi <= 32 && (size_t)bw_max * 4 + 1024 <= (size_t)max_smem) {
+      int G = std::max(1, 8 / g.wpi);
+      G = std::min(G, std::max(B, 1));
+      G = (int)std::min<size_t>((size_t)G, ((size_t)max_smem - 1024) / ((size_t)bw_max * 4));
+      g.G = std::max(G, 1);
+      g.threads = g.G * g.wpi * 32;
+      g.smem_bytes = g.G * bw_max * 4;
+      break;
+    }
+    if (row_blocks == 1) return false;
+    row_blocks /= 2;
+  }
+  *out = g;
+  return true;
 }
 
 }  // namespace lpf
@@ -251,10 +339,11 @@ extern "C" int lpf_paths_info(const lpf_paths* p, int64_t* n_half_vectors, int64
   if (!p) return LPF_E_INVAL;
   if (n_half_vectors) *n_half_vectors = p->n_half;
   if (sum_path_len) *sum_path_len = p->sum_len;
-  if (n_trie_nodes) *n_trie_nodes = (int64_t)p->nodes.size();
+  if (n_trie_nodes) *n_trie_nodes = p->n_trie_nodes;
   if (max_depth) {
     int d = 0;
-    for (const lpf::Node& n : p->nodes) d = std::max(d, (int)n.depth);
+    for (int o = 0; o < 4; ++o)
+      for (const lpf::Node& n : p->oct[o]) d = std::max(d, (int)n.depth);
     *max_depth = d;
   }
   return LPF_OK;
@@ -281,15 +370,19 @@ extern "C" int lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, in
   return LPF_OK;
 }
 
-extern "C" int lpf_paths_program(lpf_paths* p, int piece_nodes, unsigned flags, uint64_t* entries,
-                                 int64_t cap_entries, int64_t* n_entries, int64_t* items,
-                                 int64_t cap_items, int64_t* n_items, int* n_slots) {
-  if (!p || !n_entries || !n_items || !n_slots) return LPF_E_INVAL;
+extern "C" int lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, unsigned flags, uint64_t* entries,
+                                 int64_t cap_entries, int64_t* n_entries, int64_t* items, int64_t cap_items,
+                                 int64_t* n_items, int* n_slots, int* strides) {
+  if (!p || !n_entries || !n_items || !n_slots || !strides) return LPF_E_INVAL;
+  if (H < 1 || W < 1 || p->m > std::min(H, W) - 1) return LPF_E_INVAL;
+  lpf::Geom g;
+  if (!lpf::choose_geom(p->m, H, W, 1, p->max_smem > 0 ? p->max_smem : 232448, &g)) return LPF_E_UNSUPPORTED;
   try {
-    lpf::Program& pr = lpf::get_program(p, piece_nodes, flags);
+    lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride);
     *n_entries = (int64_t)pr.entries.size();
-    *n_items = (int64_t)pr.items.size() / 2;
+    *n_items = (int64_t)pr.items.size() / 4;
     *n_slots = pr.n_slots;
+    for (int o = 0; o < 4; ++o) strides[o] = pr.stride[o];
     if (entries) {
       if (cap_entries < *n_entries) return LPF_E_INVAL;
       std::memcpy(entries, pr.entries.data(), sizeof(uint64_t) * pr.entries.size());

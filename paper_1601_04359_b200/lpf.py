@@ -58,7 +58,7 @@ def load() -> ctypes.CDLL:
     lib.lpf_paths_info.restype = I
     lib.lpf_paths_get.argtypes = [VP, I, I, VP, I, PI]
     lib.lpf_paths_get.restype = I
-    lib.lpf_paths_program.argtypes = [VP, I, U, VP, I64, PI64, VP, I64, PI64, PI]
+    lib.lpf_paths_program.argtypes = [VP, I, I, I, U, VP, I64, PI64, VP, I64, PI64, PI, PI]
     lib.lpf_paths_program.restype = I
     lib.lpf_eval.argtypes = [VP, VP, I, I, I, I, VP, U, VP]
     lib.lpf_eval.restype = I
@@ -141,18 +141,19 @@ def lpf_paths_get(p: Paths, dx: int, dy: int) -> np.ndarray:
     return xy[: n.value]
 
 
-def lpf_paths_program(p: Paths, piece_nodes: int = 0, flags: int = 0):
-    """(entries uint64 [n], items int64 [k, 2], n_slots) of the linearised walk program."""
+def lpf_paths_program(p: Paths, H: int, W: int, piece_nodes: int = 0, flags: int = 0):
+    """(entries uint64 [n], items int64 [k, 4], n_slots, strides [4]) of the linearised walk program."""
     lib = load()
     ne, ni, ns = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int()
-    _check(lib.lpf_paths_program(p.handle, int(piece_nodes), int(flags), None, 0, ctypes.byref(ne), None, 0,
-                                 ctypes.byref(ni), ctypes.byref(ns)), "lpf_paths_program")
+    strides = (ctypes.c_int * 4)()
+    _check(lib.lpf_paths_program(p.handle, int(H), int(W), int(piece_nodes), int(flags), None, 0, ctypes.byref(ne),
+                                 None, 0, ctypes.byref(ni), ctypes.byref(ns), strides), "lpf_paths_program")
     entries = np.zeros(ne.value, dtype=np.uint64)
-    items = np.zeros((ni.value, 2), dtype=np.int64)
-    _check(lib.lpf_paths_program(p.handle, int(piece_nodes), int(flags), entries.ctypes.data, ne.value,
-                                 ctypes.byref(ne), items.ctypes.data, ni.value, ctypes.byref(ni),
-                                 ctypes.byref(ns)), "lpf_paths_program")
-    return entries, items, ns.value
+    items = np.zeros((ni.value, 4), dtype=np.int64)
+    _check(lib.lpf_paths_program(p.handle, int(H), int(W), int(piece_nodes), int(flags), entries.ctypes.data,
+                                 ne.value, ctypes.byref(ne), items.ctypes.data, ni.value, ctypes.byref(ni),
+                                 ctypes.byref(ns), strides), "lpf_paths_program")
+    return entries, items, ns.value, [int(v) for v in strides]
 
 
 # ---- device entry points (torch tensors in, torch tensors out) -------------------------------
@@ -273,7 +274,7 @@ def lpf_last_launch_info(p: Paths) -> dict:
     lib = load()
     out = (ctypes.c_int64 * 8)()
     _check(lib.lpf_last_launch_info(p.handle, out), "lpf_last_launch_info")
-    keys = ("kernels", "work_items", "program_entries", "grid", "block", "smem_bytes", "T", "G")
+    keys = ("kernels", "work_items", "program_entries", "grid", "block", "smem_bytes", "tile", "G")
     return dict(zip(keys, [int(v) for v in out]))
 
 

@@ -93,27 +93,32 @@ def test_closed_form_rasteriser_equals_oracle_incremental_form(m):
 def _decode(entries):
     x = (entries & np.uint64(0xffffffff)).astype(np.int64)
     y = (entries >> np.uint64(32)).astype(np.int64)
-    sh = x & 31
-    col = ((x >> 5) & 63) - 16
-    a = col * 32 + sh
-    b = (x >> 11) & 1023
-    return dict(a=a, b=b, terminal=(x >> 21) & 1, save=(x >> 22) & 1, restore=(x >> 23) & 1,
-                init=(x >> 24) & 1, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 63, sslot=(y >> 26) & 63)
+    return dict(sh=x & 31, reload=(x >> 5) & 1, terminal=(x >> 6) & 1, save=(x >> 7) & 1, restore=(x >> 8) & 1,
+                init=(x >> 9) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 15, sslot=(y >> 24) & 15)
 
 
-@pytest.mark.parametrize("m,piece,flags", [(5, 0, 0), (12, 16, 0), (33, 256, 0), (12, 0, lpf.LPF_NO_TRIE),
-                                           (12, 64, lpf.LPF_NO_TRIE)])
-def test_program_walk_reproduces_every_canonical_path_once(m, piece, flags):
+def _from_view(o, a, b):
+    # inverse of the octant view transforms documented in include/lpf.h (lpf_paths_program)
+    return [(a, b), (b, a), (-b, a), (-a, b)][o]
+
+
+@pytest.mark.parametrize("m,H,W,piece,flags", [(5, 8, 8, 0, 0), (12, 40, 100, 16, 0), (33, 64, 64, 256, 0),
+                                               (70, 300, 128, 512, 0), (12, 13, 13, 0, lpf.LPF_NO_TRIE),
+                                               (12, 64, 32, 64, lpf.LPF_NO_TRIE)])
+def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags):
     """Interpret the node program on the host with a stack of pixel lists instead of masks:
-    every terminal must be reached exactly once with exactly the pixel list P_v."""
+    every terminal must be reached exactly once with exactly the pixel list P_v, and the row-strip
+    reload flag must be set whenever the row or word column differs from the previous entry."""
     p = lpf.lpf_build_paths(m, -1)
-    entries, items, n_slots = lpf.lpf_paths_program(p, piece, flags)
+    entries, items, n_slots, strides = lpf.lpf_paths_program(p, H, W, piece, flags)
     d = _decode(entries)
     S = 2 * m + 1
     seen = {}
     covered = np.zeros(len(entries), dtype=bool)
-    for first, cnt in items:
-        cur, stack = None, {}
+    assert n_slots <= 10
+    for first, cnt, o, _ in items:
+        cur, stack, held = None, {}, None
+        assert strides[o] % 2 == 1
         for e in range(first, first + cnt):
             assert not covered[e]
             covered[e] = True
@@ -122,7 +127,13 @@ def test_program_walk_reproduces_every_canonical_path_once(m, piece, flags):
             elif d["restore"][e]:
                 cur = list(stack[int(d["rslot"][e])])
             assert cur is not None
-            cur = cur + [(int(d["a"][e]), int(d["b"][e]))]
+            bv, col = divmod(int(d["off"][e]), strides[o])
+            av = col * 32 + int(d["sh"][e])
+            assert 0 <= bv <= av <= m
+            if d["reload"][e]:
+                held = (bv, col)
+            assert held == (bv, col), "stale row strip"
+            cur = cur + [_from_view(o, av, bv)]
             if d["terminal"][e]:
                 cidx = int(d["cidx"][e])
                 dy, dx = cidx // S - m, cidx % S - m
@@ -130,7 +141,7 @@ def test_program_walk_reproduces_every_canonical_path_once(m, piece, flags):
                 assert (dx, dy) not in seen
                 seen[(dx, dy)] = cur
             if d["save"][e]:
-                assert int(d["sslot"][e]) < n_slots
+                assert int(d["sslot"][e]) < max(n_slots, 1)
                 stack[int(d["sslot"][e])] = list(cur)
     assert covered.all()
     assert len(seen) == 2 * m * m + 2 * m + 1
