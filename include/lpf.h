@@ -128,7 +128,7 @@ int  lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, int H, int W
 
 /* Counters of the most recent lpf_eval / lpf_eval_both on this object (host values known at
  * launch time): kernels launched, work items, program entries walked per image-phase, grid,
- * block, dynamic shared memory bytes, thread tile code (100 TX + 10 TY + slots % 10), images per CTA.
+ * block, dynamic shared memory bytes, thread tile code (1000 TX + 100 TY + mask-stack slots), images per CTA.
  * out = host int64[8]. */
 int  lpf_last_launch_info(const lpf_paths* p, int64_t* out8);
 
@@ -138,6 +138,11 @@ int  lpf_last_launch_info(const lpf_paths* p, int64_t* out8);
  * the most recent eval kernel in milliseconds.  INVAL if no timed eval has been issued. */
 int  lpf_set_timing(lpf_paths* p, int enable);
 int  lpf_last_eval_kernel_ms(lpf_paths* p, float* ms);
+
+/* Tuning hook: overrides the thread tile of the eval kernel -- TX x-adjacent words x
+ * TY start rows per thread, (TX,TY) in {(4,2),(8,1),(4,4),(8,2),(16,1)}, and the warps per CTA (1..8) -- for the
+ * following lpf_eval calls on this object; 0 = automatic choice.  Never changes a count.  INVAL otherwise. */
+int  lpf_set_tile(lpf_paths* p, int tx, int ty, int cta_warps);
 
 #ifdef __cplusplus
 }

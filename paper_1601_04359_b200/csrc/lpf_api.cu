@@ -50,9 +50,10 @@ static void free_program(Program& pr) {
 // uploads the program (once) and the work list expanded over (row band, strip band) of each octant
 static int upload_program(Program& pr, const Geom& g) {
   if (!pr.d_entries) {
-    LPF_CUDA(cudaMalloc(&pr.d_entries, sizeof(uint64_t) * (pr.entries.size() + 1)));   // +1: the walker prefetches
+    // +64: the walker fetches 32 entries per warp, one chunk ahead
+    LPF_CUDA(cudaMalloc(&pr.d_entries, sizeof(uint64_t) * (pr.entries.size() + 64)));
     LPF_CUDA(cudaMalloc(&pr.d_skip, sizeof(uint32_t) * std::max<size_t>(pr.skip.size(), 1)));
-    LPF_CUDA(cudaMemset(pr.d_entries, 0, sizeof(uint64_t) * (pr.entries.size() + 1)));
+    LPF_CUDA(cudaMemset(pr.d_entries, 0, sizeof(uint64_t) * (pr.entries.size() + 64)));
     LPF_CUDA(cudaMemcpy(pr.d_entries, pr.entries.data(), sizeof(uint64_t) * pr.entries.size(), cudaMemcpyHostToDevice));
     LPF_CUDA(cudaMemcpy(pr.d_skip, pr.skip.data(), sizeof(uint32_t) * pr.skip.size(), cudaMemcpyHostToDevice));
   }
@@ -140,8 +141,8 @@ namespace lpf {
 
 cudaError_t launch_pack(const uint8_t* images, uint32_t* packed, const Geom& g, int B, int Bpad, int n_phase,
                         int phase0, unsigned int* counter, int n_sm, cudaStream_t st);
-cudaError_t eval_occupancy(int TX, int NS, int threads, size_t smem, int* blocks_per_sm);
-cudaError_t launch_eval(const EvalParams& p, int NS, int grid, int threads, size_t smem, cudaStream_t st);
+cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem, int* blocks_per_sm);
+cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st);
 cudaError_t launch_mirror(unsigned long long* counts, int S, long long n_arrays, int n_sm, cudaStream_t st);
 cudaError_t launch_objective(const long long* counts, const long long* target, int B, long long K,
                              unsigned long long* sse, int n_sm, cudaStream_t st);
@@ -161,7 +162,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   if (!dg.ok) return LPF_E_CUDA;
   cudaStream_t st = (cudaStream_t)stream;
   Geom g;
-  if (!choose_geom(p->m, H, W, B, p->max_smem, &g)) return LPF_E_UNSUPPORTED;
+  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, &g)) return LPF_E_UNSUPPORTED;
   const int Bpad = (B + g.G - 1) / g.G * g.G;
   long long off = 0;
   int work_per_item = 0;                           // (row band x strip band) pairs summed over the octants / 4
@@ -191,15 +192,17 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
     } catch (const std::bad_alloc&) {
       return LPF_E_NOMEM;
     }
-    if (pr->n_slots <= 10) break;
+    if (pr->n_slots <= STACK_SLOTS_BUDGET) break;
     if (q <= 64) return LPF_E_UNSUPPORTED;
   }
-  const int NS = pr->n_slots <= 6 ? 6 : 10;
+  if (pr->entries.size() >= (size_t)1 << 30) return LPF_E_UNSUPPORTED;
   int rc = upload_program(*pr, g);
   if (rc != LPF_OK) return rc;
 
+  const bool prune = (flags & LPF_PRUNE) != 0;
+  const size_t smem_total = (size_t)g.smem_bytes + (size_t)g.threads * (pr->n_slots * g.TX * g.TY + 1) * 4;
   int occ = 0;
-  LPF_CUDA(eval_occupancy(g.TX, NS, g.threads, (size_t)g.smem_bytes, &occ));
+  LPF_CUDA(eval_occupancy(g.TX, g.TY, prune, g.threads, smem_total, &occ));
   if (occ < 1) return LPF_E_UNSUPPORTED;
   const int resident = p->n_sm * occ;
 
@@ -228,7 +231,8 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   ep.counts = (unsigned long long*)counts;
   ep.S = S;
   ep.counter = p->d_counter;
-  ep.prune = (flags & LPF_PRUNE) ? 1 : 0;
+  ep.prune = prune ? 1 : 0;
+  ep.n_slots = pr->n_slots;
   const long long total_work = (long long)ep.n_work * n_gp;
   if (total_work >= (1ll << 32)) return LPF_E_UNSUPPORTED;
   const int grid = (int)std::min<long long>(total_work, resident);
@@ -239,7 +243,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
     }
     LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_start, st));
   }
-  LPF_CUDA(launch_eval(ep, NS, grid, g.threads, (size_t)g.smem_bytes, st));
+  LPF_CUDA(launch_eval(ep, grid, g.threads, smem_total, st));
   if (p->timing) LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_stop, st));
   LPF_CUDA(launch_mirror((unsigned long long*)counts, S, (long long)B * n_phase, p->n_sm, st));
 
@@ -248,8 +252,8 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   p->last_info[2] = (int64_t)pr->entries.size();         // program entries (all four octants)
   p->last_info[3] = grid;
   p->last_info[4] = g.threads;
-  p->last_info[5] = (int64_t)g.smem_bytes;
-  p->last_info[6] = g.TX * 100 + g.TY * 10 + NS % 10;    // thread tile TX, TY and mask slots (6 or 10 -> 0)
+  p->last_info[5] = (int64_t)smem_total;
+  p->last_info[6] = g.TX * 1000 + g.TY * 100 + pr->n_slots;   // thread tile TX, TY and mask-stack slots
   p->last_info[7] = g.G;
   return LPF_OK;
 }
@@ -269,6 +273,15 @@ extern "C" int lpf_eval_both(lpf_paths* p, const uint8_t* images, int B, int H, 
 extern "C" int lpf_set_timing(lpf_paths* p, int enable) {
   if (!p || p->device < 0) return LPF_E_INVAL;
   p->timing = enable ? 1 : 0;
+  return LPF_OK;
+}
+
+extern "C" int lpf_set_tile(lpf_paths* p, int tx, int ty, int cta_warps) {
+  if (!p) return LPF_E_INVAL;
+  const bool known = (tx == 0 && ty == 0) || (tx == 4 && ty == 2) || (tx == 8 && ty == 1) || (tx == 4 && ty == 4) ||
+                     (tx == 8 && ty == 2) || (tx == 16 && ty == 1);
+  if (!known || cta_warps < 0 || cta_warps > 8) return LPF_E_INVAL;
+  p->tile_tx = tx; p->tile_ty = ty; p->cta_warps = cta_warps;
   return LPF_OK;
 }
 

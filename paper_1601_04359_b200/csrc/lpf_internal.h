@@ -69,7 +69,6 @@ constexpr int E_SSLOT_SHIFT = 24;
 constexpr uint32_t E_SLOT_MASK = 15u;
 
 constexpr int MAX_M = 511;
-constexpr int MAX_SLOTS = 12;   // mask-stack slots the kernels provide per thread
 
 struct Node {
   int16_t a, b;          // pixel offset of this node (last pixel of the prefix), view coordinates
@@ -122,6 +121,7 @@ struct lpf_paths {
   size_t io_out_bytes = 0;
   void* io_stream = nullptr;
   // lpf_set_timing: CUDA events recorded around the eval kernel alone
+  int tile_tx = 0, tile_ty = 0, cta_warps = 0;   // lpf_set_tile overrides (0 = automatic)
   int timing = 0;
   void* ev_start = nullptr;
   void* ev_stop = nullptr;

@@ -1,7 +1,7 @@
 // lpf_kernels.cu -- CUDA kernels of liblpf.so (sm_100a).
 //   pack_kernel       uint8 image -> bit planes, 32 px / word, four octant views per image, each with
 //                     its periodic halo laid out exactly as the eval kernel wants it in shared memory (a2)
-//   eval_kernel<..>   the hot loop: walk the node program with a running AND mask (a3), POPC +
+//   eval_kernel_v3<.> the hot loop: walk the node program with a running AND mask (a3), POPC +
 //                     warp reduce at terminals (a4), optional zero-mask pruning (a5)
 //   mirror_kernel     counts[-v] = counts[v] (a6)
 //   objective_kernel  sum (c - t)^2 per image (a8, Eq. 14/19)
@@ -93,20 +93,23 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, unsigne
 }
 
 // ---------------------------------------------------------------------------------------------
-// eval kernel, version 2: register strips on octant views.
+// eval kernel, version 3: register strips on octant views, lean interpreter.
 //   CTA = G images x wpi warps; every warp of the CTA walks the same work item = (program item, row band,
 //   strip band) on the same phase plane.  Lane = start row inside a block of 32 rows, warp = (strip, row
 //   block): a thread owns the TX x-adjacent start words [strip*TX, strip*TX+TX) of TY start rows (32 apart).
 //   It keeps the TX+1 words of the CURRENT path row in registers (R), so a node that stays in the same row
 //   and word column costs TX x (SHF + LOP3) and no load at all; a node that changes row reloads TX+1 words
-//   (odd row stride: the 32 lanes hit 32 different banks).  Saved masks of the depth-first walk live in
-//   registers too (NS slots, warp-uniform switch).
+//   (odd row stride: the 32 lanes hit 32 different banks).
+//   Program fetch: each warp loads 32 entries at a time, one per lane (one coalesced 256 B request, issued a
+//   whole chunk ahead), and broadcasts them node by node with SHFL; the high word (count index, slots) is
+//   fetched only by the rare entries that need it.
+//   Saved masks of the depth-first walk live in shared memory (saves/restores are ~2.6 % of the nodes each),
+//   one private odd-pitched column per thread, so the hot loop carries no stack registers.
 // ---------------------------------------------------------------------------------------------
-#define LPF_SLOT_CASES(OP) OP(0) OP(1) OP(2) OP(3) OP(4) OP(5) OP(6) OP(7) OP(8) OP(9)
-
-template <int TX, int TY, int NS>
-__global__ void __launch_bounds__(256, 2) eval_kernel_v2(const EvalParams p) {
+template <int TX, int TY, bool PRUNE>
+__global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
   constexpr int T = TX * TY;
+  constexpr unsigned FULL = 0xffffffffu;
   extern __shared__ __align__(128) uint32_t smem[];
   __shared__ __align__(8) uint64_t bar;
   __shared__ unsigned int s_work;
@@ -117,10 +120,10 @@ __global__ void __launch_bounds__(256, 2) eval_kernel_v2(const EvalParams p) {
   const int ww = warp - img_local * g.wpi;
   const int strip_l = ww % g.SB, rblk = ww / g.SB;
   const int row0 = rblk * 32 * TY + lane;               // band-local start row of ty = 0
+  uint32_t* const stk = smem + g.stack_off + tid * (p.n_slots * T + 1);
 
   uint32_t M[T];
   uint32_t R[TY][TX + 1];
-  uint32_t stk[NS][T];
 
   if (tid == 0) {
     mbar_init(&bar, 1);
@@ -155,7 +158,9 @@ __global__ void __launch_bounds__(256, 2) eval_kernel_v2(const EvalParams p) {
     // per-item thread geometry (the octant decides the view size)
     const int strip = sband * g.SB + strip_l;
     const bool active = strip < v.n_strips;
-    const uint32_t* base = smem + (size_t)img_local * v.band_words + row0 * stride + (active ? strip : 0) * TX;
+    const char* base =
+        (const char*)(smem + (size_t)img_local * v.band_words + row0 * stride + (active ? strip : 0) * TX);
+    const int rowstep = 32 * stride * 4;                     // bytes between the TY start rows of a thread
     const int b_img = b0 + img_local;
     unsigned long long* cnt = p.counts + ((size_t)b_img * p.n_phase + plane) * (size_t)p.S * p.S;
     const bool store = (lane == 0) && (b_img < p.B);
@@ -163,88 +168,94 @@ __global__ void __launch_bounds__(256, 2) eval_kernel_v2(const EvalParams p) {
     parity ^= 1u;
     __syncthreads();                 // s_work may be rewritten only after everyone has read it
 
-    const long long e0 = wk.x, e1 = e0 + wk.y;
-    uint2 ent = __ldg(p.entries + e0);
-    for (long long e = e0; e < e1;) {
-      const uint2 nxt = __ldg(p.entries + e + 1);           // the entry array is padded by one
-      const uint32_t x = ent.x;
-      long long ne = e + 1;
-      if (x & (E_INIT | E_RESTORE)) {
-        if (x & E_INIT) {
+    int e = wk.x;
+    const int e1 = e + wk.y;
+    uint2 cur = __ldg(p.entries + e + lane);                 // the entry array is padded by 64
+    while (e < e1) {
+      const uint2 nxt = __ldg(p.entries + e + 32 + lane);
+      const int n = min(32, e1 - e);
+      int jump = -1;
+      uint32_t x = __shfl_sync(FULL, cur.x, 0);
+#pragma unroll 1
+      for (int i = 0; i < n; ++i) {
+        const uint32_t xn = __shfl_sync(FULL, cur.x, i + 1);
+        if (x & (E_INIT | E_RESTORE)) {
+          if (x & E_INIT) {
 #pragma unroll
-          for (int ty = 0; ty < TY; ++ty) {
-            const bool rowok = active && (band * g.band_rows + row0 + ty * 32 < v.Hv);
+            for (int ty = 0; ty < TY; ++ty) {
+              const bool rowok = active && (band * g.band_rows + row0 + ty * 32 < v.Hv);
 #pragma unroll
-            for (int t = 0; t < TX; ++t) {
-              const int nb = v.Wv - 32 * (strip * TX + t);   // start pixels x' < Wv only
-              const uint32_t cm = nb >= 32 ? 0xffffffffu : (nb <= 0 ? 0u : ((1u << nb) - 1u));
-              M[ty * TX + t] = rowok ? cm : 0u;
+              for (int t = 0; t < TX; ++t) {
+                const int nb = v.Wv - 32 * (strip * TX + t);   // start pixels x' < Wv only
+                const uint32_t cm = nb >= 32 ? 0xffffffffu : (nb <= 0 ? 0u : ((1u << nb) - 1u));
+                M[ty * TX + t] = rowok ? cm : 0u;
+              }
             }
-          }
-        } else {
-          switch ((ent.y >> E_RSLOT_SHIFT) & E_SLOT_MASK) {
-#define LPF_RESTORE(s)                                                             \
-  case s:                                                                          \
-    if (s < NS) {                                                                  \
-      _Pragma("unroll") for (int t = 0; t < T; ++t) M[t] = stk[s < NS ? s : 0][t]; \
-    }                                                                              \
-    break;
-            LPF_SLOT_CASES(LPF_RESTORE)
-#undef LPF_RESTORE
-            default: break;
+          } else {
+            const uint32_t y = __shfl_sync(FULL, cur.y, i);
+            const uint32_t* s = stk + ((y >> E_RSLOT_SHIFT) & E_SLOT_MASK) * T;
+#pragma unroll
+            for (int t = 0; t < T; ++t) M[t] = s[t];
           }
         }
-      }
-      if (x & E_RELOAD) {
-        const uint32_t* rp = base + (x >> E_OFF_SHIFT);
+        if (x & E_RELOAD) {
+          const char* rp = base + (x >> (E_OFF_SHIFT - 2));   // bits 10, 11 are zero: byte offset
+#pragma unroll
+          for (int ty = 0; ty < TY; ++ty)
+#pragma unroll
+            for (int k = 0; k <= TX; ++k) R[ty][k] = *(const uint32_t*)(rp + ty * rowstep + 4 * k);
+        }
 #pragma unroll
         for (int ty = 0; ty < TY; ++ty)
 #pragma unroll
-          for (int i = 0; i <= TX; ++i) R[ty][i] = rp[ty * 32 * stride + i];
-      }
+          for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __funnelshift_r(R[ty][t], R[ty][t + 1], x);
+        if (x & (E_TERMINAL | E_SAVE)) {
+          const uint32_t y = __shfl_sync(FULL, cur.y, i);
+          if (x & E_SAVE) {
+            uint32_t* s = stk + ((y >> E_SSLOT_SHIFT) & E_SLOT_MASK) * T;
 #pragma unroll
-      for (int ty = 0; ty < TY; ++ty)
+            for (int t = 0; t < T; ++t) s[t] = M[t];
+          }
+          if (x & E_TERMINAL) {
+            int c = 0;
 #pragma unroll
-        for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __funnelshift_r(R[ty][t], R[ty][t + 1], x);
-      if (x & (E_TERMINAL | E_SAVE)) {
-        if (x & E_TERMINAL) {
-          int c = 0;
-#pragma unroll
-          for (int t = 0; t < T; ++t) c += __popc(M[t]);
-          c = __reduce_add_sync(0xffffffffu, c);
-          if (c != 0) {
-            if (store) atomicAdd(cnt + (ent.y & E_CIDX_MASK), (unsigned long long)c);
-          } else if (p.prune) {          // paper's "enhanced" rule: nothing below can count
-            ne += __ldg(p.skip + e);
-            ent = __ldg(p.entries + ne);
-            e = ne;
-            continue;
+            for (int t = 0; t < T; ++t) c += __popc(M[t]);
+            c = __reduce_add_sync(FULL, c);
+            if (c != 0) {
+              if (store) atomicAdd(cnt + (y & E_CIDX_MASK), (unsigned long long)c);
+            } else if (PRUNE) {          // paper's "enhanced" rule: nothing below can count
+              const int sk = (int)__ldg(p.skip + e + i);
+              if (sk) {
+                jump = e + i + 1 + sk;
+                break;
+              }
+            }
           }
         }
-        if (x & E_SAVE) {
-          switch ((ent.y >> E_SSLOT_SHIFT) & E_SLOT_MASK) {
-#define LPF_SAVE(s)                                                                \
-  case s:                                                                          \
-    if (s < NS) {                                                                  \
-      _Pragma("unroll") for (int t = 0; t < T; ++t) stk[s < NS ? s : 0][t] = M[t]; \
-    }                                                                              \
-    break;
-            LPF_SLOT_CASES(LPF_SAVE)
-#undef LPF_SAVE
-            default: break;
-          }
-        }
+        x = xn;
       }
-      ent = nxt;
-      e = ne;
+      if (PRUNE && jump >= 0) {
+        e = jump;
+        if (e < e1) cur = __ldg(p.entries + e + lane);
+      } else {
+        e += 32;
+        cur = nxt;
+      }
     }
   }
 }
 
 typedef void (*eval_fn)(const EvalParams);
-static eval_fn eval_fn_for(int TX, int NS) {
-  if (TX == 8) return NS <= 6 ? eval_kernel_v2<8, 1, 6> : eval_kernel_v2<8, 1, 10>;
-  return NS <= 6 ? eval_kernel_v2<4, 2, 6> : eval_kernel_v2<4, 2, 10>;
+static eval_fn eval_fn_for(int TX, int TY, bool prune) {
+#define LPF_PICK(tx, ty) \
+  if (TX == tx && TY == ty) return prune ? eval_kernel_v3<tx, ty, true> : eval_kernel_v3<tx, ty, false>;
+  LPF_PICK(4, 2)
+  LPF_PICK(8, 1)
+  LPF_PICK(4, 4)
+  LPF_PICK(8, 2)
+  LPF_PICK(16, 1)
+#undef LPF_PICK
+  return nullptr;
 }
 // ---------------------------------------------------------------------------------------------
 // mirror: counts[-v] = counts[v] for v in D.  n_arrays = B * n_phase arrays of S*S.
@@ -384,15 +395,17 @@ cudaError_t launch_pack(const uint8_t* images, uint32_t* packed, const Geom& g, 
   return cudaGetLastError();
 }
 
-cudaError_t eval_occupancy(int TX, int NS, int threads, size_t smem, int* blocks_per_sm) {
-  eval_fn f = eval_fn_for(TX, NS);
+cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem, int* blocks_per_sm) {
+  eval_fn f = eval_fn_for(TX, TY, prune);
+  if (!f) return cudaErrorInvalidValue;
   cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, f, threads, smem);
 }
 
-cudaError_t launch_eval(const EvalParams& p, int NS, int grid, int threads, size_t smem, cudaStream_t st) {
-  eval_fn f = eval_fn_for(p.g.TX, NS);
+cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st) {
+  eval_fn f = eval_fn_for(p.g.TX, p.g.TY, p.prune != 0);
+  if (!f) return cudaErrorInvalidValue;
   f<<<grid, threads, smem, st>>>(p);
   return cudaGetLastError();
 }

@@ -267,13 +267,19 @@ int build_host_table(lpf_paths* p) {
 
 namespace lpf {
 
-bool choose_geom(int m, int H, int W, int B, int max_smem, Geom* out) {
+bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, Geom* out) {
   Geom g;
   std::memset(&g, 0, sizeof(g));
   g.H = H; g.W = W; g.m = m;
   const int wc_max = (std::max(H, W) + 31) / 32;
-  g.TX = wc_max >= 8 ? 8 : 4;
-  g.TY = 8 / g.TX;
+  if (tx > 0 && ty > 0) {
+    g.TX = tx; g.TY = ty;
+  } else {                                       // thread tile of 8 words
+    g.TX = wc_max >= 8 ? 8 : 4;
+    g.TY = 8 / g.TX;
+  }
+  const int T = g.TX * g.TY;
+  if (cta_warps < 1 || cta_warps > 8) cta_warps = 8;
   const int rows_per_warp = 32 * g.TY;
   int strips_max = 0, hv_max = 0;
   for (int o = 0; o < 4; ++o) {
@@ -288,12 +294,14 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, Geom* out) {
     strips_max = std::max(strips_max, v.n_strips);
     hv_max = std::max(hv_max, v.Hv);
   }
-  int row_blocks = std::max(1, 8 / strips_max);
+  g.SB = std::min(strips_max, cta_warps);
+  int row_blocks = std::max(1, cta_warps / g.SB);
   const int max_blocks = (hv_max + rows_per_warp - 1) / rows_per_warp;
   row_blocks = std::min(row_blocks, max_blocks);
+  // shared memory: G bands + one mask-stack column of (slots * T + 1) words per thread
+  const size_t stack_per_thread = (size_t)(STACK_SLOTS_BUDGET * T + 1) * 4;
   for (;;) {
     g.band_rows = rows_per_warp * row_blocks;
-    g.SB = std::min(strips_max, 8);
     g.wpi = g.SB * row_blocks;
     int bw_max = 0;
     for (int o = 0; o < 4; ++o) {
@@ -303,13 +311,15 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, Geom* out) {
       v.view_words = ((v.n_bands * g.band_rows + m) * v.stride + 3) / 4 * 4 + 4;
       bw_max = std::max(bw_max, v.band_words);
     }
-    if (g.wpi <= 32 && (size_t)bw_max * 4 + 1024 <= (size_t)max_smem) {
-      int G = std::max(1, 8 / g.wpi);
+    const size_t per_image = (size_t)bw_max * 4 + (size_t)g.wpi * 32 * stack_per_thread;
+    if (per_image + 1024 <= (size_t)max_smem) {
+      int G = std::max(1, cta_warps / g.wpi);
       G = std::min(G, std::max(B, 1));
-      G = (int)std::min<size_t>((size_t)G, ((size_t)max_smem - 1024) / ((size_t)bw_max * 4));
+      G = (int)std::min<size_t>((size_t)G, ((size_t)max_smem - 1024) / per_image);
       g.G = std::max(G, 1);
       g.threads = g.G * g.wpi * 32;
       g.smem_bytes = g.G * bw_max * 4;
+      g.stack_off = g.G * bw_max;
       break;
     }
     if (row_blocks == 1) return false;
@@ -376,7 +386,8 @@ extern "C" int lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, un
   if (!p || !n_entries || !n_items || !n_slots || !strides) return LPF_E_INVAL;
   if (H < 1 || W < 1 || p->m > std::min(H, W) - 1) return LPF_E_INVAL;
   lpf::Geom g;
-  if (!lpf::choose_geom(p->m, H, W, 1, p->max_smem > 0 ? p->max_smem : 232448, &g)) return LPF_E_UNSUPPORTED;
+  if (!lpf::choose_geom(p->m, H, W, 1, p->max_smem > 0 ? p->max_smem : 232448, p->tile_tx, p->tile_ty, p->cta_warps, &g))
+    return LPF_E_UNSUPPORTED;
   try {
     lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride);
     *n_entries = (int64_t)pr.entries.size();

@@ -21,6 +21,7 @@ EXPORTS = (
     "lpf_strerror", "lpf_last_cuda_error", "lpf_build_paths", "lpf_free_paths", "lpf_paths_info",
     "lpf_paths_get", "lpf_paths_program", "lpf_eval", "lpf_eval_both", "lpf_objective",
     "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
+    "lpf_set_tile",
 )
 
 _lib = None
@@ -76,6 +77,8 @@ def load() -> ctypes.CDLL:
     lib.lpf_set_timing.restype = I
     lib.lpf_last_eval_kernel_ms.argtypes = [VP, ctypes.POINTER(ctypes.c_float)]
     lib.lpf_last_eval_kernel_ms.restype = I
+    lib.lpf_set_tile.argtypes = [VP, I, I, I]
+    lib.lpf_set_tile.restype = I
     _lib = lib
     return lib
 
@@ -280,6 +283,11 @@ def lpf_last_launch_info(p: Paths) -> dict:
 
 def lpf_set_timing(p: Paths, enable: bool) -> None:
     _check(load().lpf_set_timing(p.handle, int(bool(enable))), "lpf_set_timing")
+
+
+def lpf_set_tile(p: Paths, tx: int = 0, ty: int = 0, cta_warps: int = 0) -> None:
+    """Tuning hook: thread tile (TX words x TY rows) and warps per CTA of the eval kernel; 0 = automatic."""
+    _check(load().lpf_set_tile(p.handle, int(tx), int(ty), int(cta_warps)), "lpf_set_tile")
 
 
 def lpf_last_eval_kernel_ms(p: Paths) -> float:
