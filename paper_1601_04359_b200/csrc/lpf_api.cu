@@ -200,7 +200,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   if (rc != LPF_OK) return rc;
 
   const bool prune = (flags & LPF_PRUNE) != 0;
-  const size_t smem_total = (size_t)g.smem_bytes + (size_t)g.threads * (pr->n_slots * g.TX * g.TY + 1) * 4;
+  const size_t smem_total = (size_t)g.smem_bytes;
   int occ = 0;
   LPF_CUDA(eval_occupancy(g.TX, g.TY, prune, g.threads, smem_total, &occ));
   if (occ < 1) return LPF_E_UNSUPPORTED;

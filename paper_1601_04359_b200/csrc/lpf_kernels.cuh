@@ -28,15 +28,14 @@ struct Geom {
   int wpi;           // warps per image band = SB * band_rows / (32 TY)
   int G;             // images per CTA
   int threads;       // G * wpi * 32
-  int smem_bytes;    // G * max band_words * 4 (the mask stacks follow: threads * (slots * T + 1) words)
-  int stack_off;     // word offset of the mask stacks in dynamic shared memory
+  int smem_bytes;    // G * max band_words * 4
   ViewGeom v[4];
   long long plane_words;  // words of one phase plane: Bpad * sum_o view_words
 };
 
 // host: pick the geometry for (m, H, W, B); false if one band does not fit in shared memory
 //   tx, ty > 0 override the thread tile; cta_warps (1..8) the warps per CTA
-constexpr int STACK_SLOTS_BUDGET = 8;   // mask-stack slots the geometry reserves shared memory for
+constexpr int STACK_SLOTS_BUDGET = 8;   // mask-stack slots per thread (local memory, T words each)
 bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, Geom* out);
 
 struct EvalParams {

@@ -274,11 +274,10 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int c
   const int wc_max = (std::max(H, W) + 31) / 32;
   if (tx > 0 && ty > 0) {
     g.TX = tx; g.TY = ty;
-  } else {                                       // thread tile of 8 words
-    g.TX = wc_max >= 8 ? 8 : 4;
-    g.TY = 8 / g.TX;
+  } else {                                       // thread tile of 16 words
+    g.TX = wc_max >= 16 ? 16 : (wc_max >= 8 ? 8 : 4);
+    g.TY = 16 / g.TX;
   }
-  const int T = g.TX * g.TY;
   if (cta_warps < 1 || cta_warps > 8) cta_warps = 8;
   const int rows_per_warp = 32 * g.TY;
   int strips_max = 0, hv_max = 0;
@@ -298,8 +297,6 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int c
   int row_blocks = std::max(1, cta_warps / g.SB);
   const int max_blocks = (hv_max + rows_per_warp - 1) / rows_per_warp;
   row_blocks = std::min(row_blocks, max_blocks);
-  // shared memory: G bands + one mask-stack column of (slots * T + 1) words per thread
-  const size_t stack_per_thread = (size_t)(STACK_SLOTS_BUDGET * T + 1) * 4;
   for (;;) {
     g.band_rows = rows_per_warp * row_blocks;
     g.wpi = g.SB * row_blocks;
@@ -311,7 +308,7 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int c
       v.view_words = ((v.n_bands * g.band_rows + m) * v.stride + 3) / 4 * 4 + 4;
       bw_max = std::max(bw_max, v.band_words);
     }
-    const size_t per_image = (size_t)bw_max * 4 + (size_t)g.wpi * 32 * stack_per_thread;
+    const size_t per_image = (size_t)bw_max * 4;     // shared memory holds the G bands only
     if (per_image + 1024 <= (size_t)max_smem) {
       int G = std::max(1, cta_warps / g.wpi);
       G = std::min(G, std::max(B, 1));
@@ -319,7 +316,6 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int c
       g.G = std::max(G, 1);
       g.threads = g.G * g.wpi * 32;
       g.smem_bytes = g.G * bw_max * 4;
-      g.stack_off = g.G * bw_max;
       break;
     }
     if (row_blocks == 1) return false;
