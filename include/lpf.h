@@ -80,7 +80,8 @@ int  lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, int cap, int
  * into connected pieces of about `piece_nodes` nodes (<= 0: one piece per octant); each piece is one item =
  * the chain from the root to the piece root followed by the piece in depth-first order.  flags: 0 or LPF_NO_TRIE.
  *   entries  host [cap_entries] uint64 (may be NULL to query sizes); low word: bits 0-4 a' & 31, bit 5 reload,
- *            6 terminal, 7 save, 8 restore, 9 init, bits 12-31 b' * stride + (a' >> 5); high word: bits 0-19
+ *            6 terminal, 7 save, 8 restore, 9 init, 10 pair (own mask never needed, next entry is the direct child),
+ *            bits 12-31 b' * stride + (a' >> 5); high word: bits 0-19
  *            (dy+m)*(2m+1) + (dx+m) in IMAGE coordinates, 20-23 restore slot, 24-27 save slot
  *   items    host [cap_items][4] int64 = (first entry, number of entries, octant, 0) (may be NULL)
  *   strides  host int[4]: words per packed row of each octant view (decodes b', a' >> 5)

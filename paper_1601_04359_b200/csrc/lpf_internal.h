@@ -51,6 +51,8 @@ inline void from_view(int o, int av, int bv, int* a, int* b) {
 //   [ 7] SAVE        copy the running mask to stack slot sslot (node has >= 2 children in its piece)
 //   [ 8] RESTORE     parent mask comes from stack slot rslot (not from the previous entry)
 //   [ 9] INIT        parent mask is "every valid start pixel" (first entry of a work item / chain)
+//   [10] PAIR        this node's own mask is never needed (not TERMINAL, not SAVE) and the next entry is its
+//                    direct child: the walker fuses both windows into one 3-input AND (M & W1 & W2)
 //   [12..31] off     = b' * stride + (a' >> 5), word offset of the window in the packed view
 // high word y:
 //   [ 0..19] cidx    = (dy + m) * (2m + 1) + (dx + m), index into counts[2m+1][2m+1] (image coordinates)
@@ -62,6 +64,7 @@ constexpr uint32_t E_TERMINAL = 1u << 6;
 constexpr uint32_t E_SAVE = 1u << 7;
 constexpr uint32_t E_RESTORE = 1u << 8;
 constexpr uint32_t E_INIT = 1u << 9;
+constexpr uint32_t E_PAIR = 1u << 10;
 constexpr int E_OFF_SHIFT = 12;
 constexpr uint32_t E_CIDX_MASK = (1u << 20) - 1u;
 constexpr int E_RSLOT_SHIFT = 20;

@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
       uint32_t x = __shfl_sync(FULL, cur.x, 0);
 #pragma unroll 1
       for (int i = 0; i < n; ++i) {
-        const uint32_t xn = __shfl_sync(FULL, cur.x, i + 1);
+        uint32_t xn = __shfl_sync(FULL, cur.x, i + 1);
         if (x & (E_INIT | E_RESTORE)) {
           if (x & E_INIT) {
 #pragma unroll
@@ -200,16 +200,40 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
           }
         }
         if (x & E_RELOAD) {
-          const char* rp = base + (x >> (E_OFF_SHIFT - 2));   // bits 10, 11 are zero: byte offset
+          const char* rp = base + ((x >> (E_OFF_SHIFT - 2)) & ~3u);
 #pragma unroll
           for (int ty = 0; ty < TY; ++ty)
 #pragma unroll
             for (int k = 0; k <= TX; ++k) R[ty][k] = *(const uint32_t*)(rp + ty * rowstep + 4 * k);
         }
+        if ((x & E_PAIR) && i + 1 < n) {
+          // this node's mask is never needed on its own: fold its window and its child's into one 3-input AND
+          uint32_t Wp[T];
 #pragma unroll
-        for (int ty = 0; ty < TY; ++ty)
+          for (int ty = 0; ty < TY; ++ty)
 #pragma unroll
-          for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __funnelshift_r(R[ty][t], R[ty][t + 1], x);
+            for (int t = 0; t < TX; ++t) Wp[ty * TX + t] = __funnelshift_r(R[ty][t], R[ty][t + 1], x);
+          x = xn;
+          ++i;
+          xn = __shfl_sync(FULL, cur.x, i + 1);
+          if (x & E_RELOAD) {
+            const char* rp = base + ((x >> (E_OFF_SHIFT - 2)) & ~3u);
+#pragma unroll
+            for (int ty = 0; ty < TY; ++ty)
+#pragma unroll
+              for (int k = 0; k <= TX; ++k) R[ty][k] = *(const uint32_t*)(rp + ty * rowstep + 4 * k);
+          }
+#pragma unroll
+          for (int ty = 0; ty < TY; ++ty)
+#pragma unroll
+            for (int t = 0; t < TX; ++t)
+              M[ty * TX + t] &= Wp[ty * TX + t] & __funnelshift_r(R[ty][t], R[ty][t + 1], x);
+        } else {
+#pragma unroll
+          for (int ty = 0; ty < TY; ++ty)
+#pragma unroll
+            for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __funnelshift_r(R[ty][t], R[ty][t + 1], x);
+        }
         if (x & (E_TERMINAL | E_SAVE)) {
           const uint32_t y = __shfl_sync(FULL, cur.y, i);
           if (x & E_SAVE) {

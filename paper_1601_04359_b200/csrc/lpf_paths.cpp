@@ -159,7 +159,17 @@ static void sort_items(Program& pr) {
     for (int k = 0; k < 4; ++k) pr.items[4 * i + k] = v[i][k];
 }
 
+// marks the entries whose mask is never needed on its own and whose successor is a direct child (E_PAIR)
+static void mark_pairs(Program& pr, int64_t first) {
+  const int64_t end = (int64_t)pr.entries.size();
+  for (int64_t k = first; k + 1 < end; ++k) {
+    const uint32_t x = (uint32_t)pr.entries[k], xn = (uint32_t)pr.entries[k + 1];
+    if (!(x & (E_TERMINAL | E_SAVE)) && !(xn & (E_INIT | E_RESTORE))) pr.entries[k] |= E_PAIR;
+  }
+}
+
 static void push_item(Program& pr, int64_t first, int o) {
+  mark_pairs(pr, first);
   pr.items.push_back(first);
   pr.items.push_back((int64_t)pr.entries.size() - first);
   pr.items.push_back(o);

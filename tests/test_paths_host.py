@@ -94,7 +94,7 @@ def _decode(entries):
     x = (entries & np.uint64(0xffffffff)).astype(np.int64)
     y = (entries >> np.uint64(32)).astype(np.int64)
     return dict(sh=x & 31, reload=(x >> 5) & 1, terminal=(x >> 6) & 1, save=(x >> 7) & 1, restore=(x >> 8) & 1,
-                init=(x >> 9) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 15, sslot=(y >> 24) & 15)
+                init=(x >> 9) & 1, pair=(x >> 10) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 15, sslot=(y >> 24) & 15)
 
 
 def _from_view(o, a, b):
@@ -115,7 +115,7 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
     S = 2 * m + 1
     seen = {}
     covered = np.zeros(len(entries), dtype=bool)
-    assert n_slots <= 10
+    assert n_slots <= 8
     for first, cnt, o, _ in items:
         cur, stack, held = None, {}, None
         assert strides[o] % 2 == 1
@@ -143,6 +143,10 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
             if d["save"][e]:
                 assert int(d["sslot"][e]) < max(n_slots, 1)
                 stack[int(d["sslot"][e])] = list(cur)
+            # PAIR: this node's own mask is never needed and the next entry of the item continues from it
+            want_pair = (not d["terminal"][e] and not d["save"][e] and e + 1 < first + cnt
+                         and not d["init"][e + 1] and not d["restore"][e + 1])
+            assert bool(d["pair"][e]) == bool(want_pair)
     assert covered.all()
     assert len(seen) == 2 * m * m + 2 * m + 1
     for (dx, dy), pix in seen.items():
