@@ -26,6 +26,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 from paper_1601_04359_b200 import inputs  # noqa: E402  (seeded generators only; no method arithmetic)
+from paper_1601_04359_b200 import dist as lpf_dist  # noqa: E402  (rank plumbing: seeds, max over ranks)
 
 METRIC = "segment tests/sec (start-pixel x vector)"
 UNIT = "segment tests/s"
@@ -44,7 +45,7 @@ WORKLOADS = {
 def make_images(w, rank):
     """Synthetic images of the workload for this rank (rank r offsets the seed by 100000 r)."""
     c = w["cfg"]
-    off = 100000 * rank
+    off = lpf_dist.rank_seed_offset(rank)
     if c == 2:
         return inputs.disks(256, 256, 8.0, 0.30, inputs.seed_for(2) + off)[None], None
     if c == 3:
@@ -254,11 +255,8 @@ def main():
             torch.cuda.synchronize()
             e2e_s = (time.perf_counter() - t0) / k
             e2e = {"seconds_per_step": e2e_s, "h2d": int(h_in.numel()), "d2h": int(h_out.numel() * 8)}
-        t = torch.tensor([total_ms, float(np.mean(kernel_ms)), e2e["seconds_per_step"] if e2e else 0.0],
-                         dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, kern_ms, e2e_s = (float(v) for v in t.cpu())
+        total_ms, kern_ms, e2e_s = lpf_dist.max_over_ranks(
+            [total_ms, float(np.mean(kernel_ms)), e2e["seconds_per_step"] if e2e else 0.0], device="cuda")
         lpf.lpf_free_paths(p)
         return dict(total_ms=total_ms, kernel_ms=kern_ms, e2e_s=e2e_s, e2e=e2e, info=info, launch=launch,
                     launches_per_step=launches_per_step, clocks=clocks, imgs=imgs, wall=wall)
