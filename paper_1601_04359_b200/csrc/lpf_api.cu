@@ -139,7 +139,7 @@ extern "C" void lpf_free_paths(lpf_paths* p) {
 
 namespace lpf {
 
-cudaError_t launch_pack(const uint8_t* images, uint32_t* packed, const Geom& g, int B, int Bpad, int n_phase,
+cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed, const Geom& g, int B, int n_phase,
                         int phase0, unsigned int* counter, int n_sm, cudaStream_t st);
 cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem, int* blocks_per_sm);
 cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st);
@@ -206,7 +206,10 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   if (occ < 1) return LPF_E_UNSUPPORTED;
   const int resident = p->n_sm * occ;
 
-  const size_t need = (size_t)n_phase * (size_t)g.plane_words * 4;
+  // workspace: the packed octant views, then the compact row-major / column-major bit images of stage 1
+  const size_t views_bytes = (size_t)n_phase * (size_t)g.plane_words * 4;
+  const size_t base_words = (size_t)n_phase * B * ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32));
+  const size_t need = views_bytes + base_words * 4;
   if (need > p->packed_bytes) {
     if (p->d_packed) { LPF_CUDA(cudaStreamSynchronize(st)); cudaFree(p->d_packed); p->d_packed = nullptr; p->packed_bytes = 0; }
     LPF_CUDA(cudaMalloc(&p->d_packed, need));
@@ -215,7 +218,8 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
 
   const int S = 2 * p->m + 1;
   LPF_CUDA(cudaMemsetAsync(counts, 0, sizeof(int64_t) * (size_t)B * n_phase * S * S, st));
-  LPF_CUDA(launch_pack(images, p->d_packed, g, B, Bpad, n_phase, phase0, p->d_counter, p->n_sm, st));
+  LPF_CUDA(launch_pack(images, p->d_packed + views_bytes / 4, p->d_packed, g, B, n_phase, phase0, p->d_counter,
+                       p->n_sm, st));
 
   EvalParams ep;
   ep.g = g;
@@ -247,7 +251,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   if (p->timing) LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_stop, st));
   LPF_CUDA(launch_mirror((unsigned long long*)counts, S, (long long)B * n_phase, p->n_sm, st));
 
-  p->last_info[0] = 3;                                   // kernels launched (pack, eval, mirror)
+  p->last_info[0] = 4;                                   // kernels launched (pack base, pack views, eval, mirror)
   p->last_info[1] = total_work;
   p->last_info[2] = (int64_t)pr->entries.size();         // program entries (all four octants)
   p->last_info[3] = grid;

@@ -1,6 +1,7 @@
 // lpf_kernels.cu -- CUDA kernels of liblpf.so (sm_100a).
-//   pack_kernel       uint8 image -> bit planes, 32 px / word, four octant views per image, each with
-//                     its periodic halo laid out exactly as the eval kernel wants it in shared memory (a2)
+//   pack_base_kernel  uint8 image -> row-major and column-major bit images, 32 px / word, one coalesced pass
+//   pack_views_kernel the four octant views per image, each with its periodic halo laid out exactly as the
+//                     eval kernel wants it in shared memory (a2)
 //   eval_kernel_v3<.> the hot loop: walk the node program with a running AND mask (a3), POPC +
 //                     warp reduce at terminals (a4), optional zero-mask pruning (a5)
 //   mirror_kernel     counts[-v] = counts[v] (a6)
@@ -8,24 +9,86 @@
 //   swap_delta_kernel per-proposal count deltas (a9)
 #include <cuda_runtime.h>
 
+#include <algorithm>
+
 #include "lpf_internal.h"
 #include "lpf_kernels.cuh"
 
 namespace lpf {
 
 // ---------------------------------------------------------------------------------------------
-// bit-pack + halo + octant views.  One warp per output word: lane k tests one pixel, __ballot_sync
-// packs.  Also zeroes the work counter for the eval kernel that follows on the same stream.
-//   view o of image I (lpf_internal.h): 0: I[y'][x']  1: I[x'][y']  2: I[x'][-y' mod W]  3: I[y'][-x' mod W]
+// bit-pack, stage 1: uint8 image -> two compact bit images per phase plane, from ONE coalesced pass.
+//   One warp per 32 x 32 pixel tile: lane k reads byte (y0 + j, x0 + k) for j = 0..31 (32 coalesced row
+//   segments).  Row words come from __ballot_sync (bit k of Brow[y][x0/32] = [I[y][x0+k] == phase]); every
+//   lane also assembles its own COLUMN word (bit j of Bcol[x][y0/32] = [I[y0+j][x] == phase]), so the
+//   transposed octant views never read the image with a stride.
+//   base layout per plane and image: Brow [H][Wc] then Bcol [W][Hc]   (Wc = ceil(W/32), Hc = ceil(H/32))
+// Also zeroes the work counter of the eval kernel that follows on the same stream.
 // ---------------------------------------------------------------------------------------------
-__global__ void pack_kernel(const uint8_t* __restrict__ images, uint32_t* __restrict__ packed, Geom g, int B,
-                            int Bpad, int n_phase, int phase0, unsigned int* counter) {
+__global__ void __launch_bounds__(256) pack_base_kernel(const uint8_t* __restrict__ images,
+                                                        uint32_t* __restrict__ base, int B, int H, int W,
+                                                        int n_phase, int phase0, unsigned int* counter) {
   if (blockIdx.x == 0 && threadIdx.x == 0) *counter = 0u;
   const int lane = threadIdx.x & 31;
+  const int Wc = (W + 31) >> 5, Hc = (H + 31) >> 5;
+  const long long img_words = (long long)H * Wc + (long long)W * Hc;
+  const long long tiles = (long long)B * Hc * Wc;
   const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+  for (long long t = warp; t < tiles; t += nwarps) {
+    const int b = (int)(t / (Hc * Wc));
+    const int rem = (int)(t - (long long)b * Hc * Wc);
+    const int ty = rem / Wc, tx = rem - ty * Wc;
+    const int x = tx * 32 + lane;
+    const uint8_t* src = images + ((size_t)b * H + (size_t)ty * 32) * W + x;
+    unsigned col0 = 0, col1 = 0, row0 = 0, row1 = 0;
+#pragma unroll 8
+    for (int j = 0; j < 32; ++j) {
+      const int y = ty * 32 + j;
+      int v = 255;
+      if (x < W && y < H) v = src[(size_t)j * W];
+      const bool b0 = n_phase == 2 ? (v == 0) : (v == phase0);
+      const bool b1 = n_phase == 2 && (v == 1);
+      const unsigned r0 = __ballot_sync(0xffffffffu, b0);
+      const unsigned r1 = __ballot_sync(0xffffffffu, b1);
+      if (lane == j) { row0 = r0; row1 = r1; }
+      col0 |= (unsigned)b0 << j;
+      col1 |= (unsigned)b1 << j;
+    }
+    uint32_t* o0 = base + (size_t)b * img_words;
+    const int y = ty * 32 + lane;
+    if (y < H) o0[(size_t)y * Wc + tx] = row0;
+    if (x < W) o0[(size_t)H * Wc + (size_t)x * Hc + ty] = col0;
+    if (n_phase == 2) {
+      uint32_t* o1 = o0 + (size_t)B * img_words;
+      if (y < H) o1[(size_t)y * Wc + tx] = row1;
+      if (x < W) o1[(size_t)H * Wc + (size_t)x * Hc + ty] = col1;
+    }
+  }
+}
+
+// 32 consecutive view pixels x' = xs .. xs+31 (no wrap inside) of one source row of `words` words
+__device__ __forceinline__ uint32_t window32(const uint32_t* __restrict__ row, int words, int xs) {
+  const int w = xs >> 5;
+  const uint32_t lo = row[w];
+  const uint32_t hi = (w + 1 < words) ? row[w + 1] : 0u;
+  return __funnelshift_r(lo, hi, xs & 31);
+}
+
+// ---------------------------------------------------------------------------------------------
+// bit-pack, stage 2: the four octant views with their periodic halo, one thread per output word.
+//   view o of image I (lpf_internal.h): 0: I[y'][x']  1: I[x'][y']  2: I[x'][-y' mod W]  3: I[y'][-x' mod W]
+//   word (r, i) of a view holds x' = (32 i + k) mod Wv, y' = r mod Hv.  Views 0 and 3 read Brow, views 1 and 2
+//   read Bcol; a word whose 32 pixels do not wrap is one funnel shift of two base words (view 3: of the
+//   bit-reversed pair), the others are gathered bit by bit.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restrict__ base,
+                                                         uint32_t* __restrict__ packed, Geom g, int B, int n_phase) {
+  const int Wc = (g.W + 31) >> 5, Hc = (g.H + 31) >> 5;
+  const long long img_words = (long long)g.H * Wc + (long long)g.W * Hc;
   const long long total = (long long)n_phase * g.plane_words;
-  for (long long w = warp; w < total; w += nwarps) {
+  for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < total;
+       w += (long long)gridDim.x * blockDim.x) {
     const int plane = (int)(w / g.plane_words);
     const long long wp = w - (long long)plane * g.plane_words;
     int o = 0;
@@ -38,22 +101,40 @@ __global__ void pack_kernel(const uint8_t* __restrict__ images, uint32_t* __rest
     const int idx = (int)(rem - (long long)b * v.view_words);
     const int r = idx / v.stride, i = idx - r * v.stride;
     const int rows = v.n_bands * g.band_rows + g.m;
-    bool bit = false;
+    uint32_t word = 0;
     if (b < B && r < rows) {
       const int yv = r % v.Hv;
-      const int xv = (32 * i + lane) % v.Wv;
-      int x, y;
-      switch (o) {
-        case 0: x = xv; y = yv; break;
-        case 1: x = yv; y = xv; break;
-        case 2: x = yv ? g.W - yv : 0; y = xv; break;
-        default: x = xv ? g.W - xv : 0; y = yv; break;
+      const int x0 = (32 * i) % v.Wv;
+      const uint32_t* bimg = base + ((size_t)plane * B + b) * img_words;
+      // source row of this view row: views 0, 3: image row yv (Brow); view 1: image column yv; view 2: column -yv
+      const uint32_t* srow;
+      int words;
+      if (o == 0 || o == 3) { srow = bimg + (size_t)yv * Wc; words = Wc; }
+      else {
+        const int c = (o == 1) ? yv : (yv ? g.W - yv : 0);
+        srow = bimg + (size_t)g.H * Wc + (size_t)c * Hc;
+        words = Hc;
       }
-      const int phase = (n_phase == 2) ? plane : phase0;
-      bit = images[((size_t)b * g.H + y) * g.W + x] == (uint8_t)phase;
+      if (o != 3) {
+        if (x0 + 32 <= v.Wv) word = window32(srow, words, x0);
+        else
+          for (int k = 0; k < 32; ++k) {
+            const int xs = (x0 + k) % v.Wv;
+            word |= ((srow[xs >> 5] >> (xs & 31)) & 1u) << k;
+          }
+      } else {
+        // bit k = source bit (Wv - x0 - k) mod Wv: for 1 <= x0 and x0 + 31 <= Wv the sources are the 32
+        // consecutive pixels Wv - x0 - 31 .. Wv - x0 in descending order
+        if (x0 >= 1 && x0 + 31 <= v.Wv) word = __brev(window32(srow, words, v.Wv - x0 - 31));
+        else
+          for (int k = 0; k < 32; ++k) {
+            const int xv = (x0 + k) % v.Wv;
+            const int xs = xv ? v.Wv - xv : 0;
+            word |= ((srow[xs >> 5] >> (xs & 31)) & 1u) << k;
+          }
+      }
     }
-    const unsigned word = __ballot_sync(0xffffffffu, bit);
-    if (lane == 0) packed[w] = word;
+    packed[w] = word;
   }
 }
 
@@ -410,13 +491,18 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v1(const uint8_t* __res
 // ---------------------------------------------------------------------------------------------
 // host launch wrappers (called from lpf_api.cu)
 // ---------------------------------------------------------------------------------------------
-cudaError_t launch_pack(const uint8_t* images, uint32_t* packed, const Geom& g, int B, int Bpad, int n_phase,
+cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed, const Geom& g, int B, int n_phase,
                         int phase0, unsigned int* counter, int n_sm, cudaStream_t st) {
+  const long long tiles = (long long)B * ((g.H + 31) / 32) * ((g.W + 31) / 32);
+  long long blocks = (tiles + 7) / 8;
+  blocks = std::max(1ll, std::min(blocks, (long long)n_sm * 16));
+  pack_base_kernel<<<(unsigned)blocks, 256, 0, st>>>(images, base, B, g.H, g.W, n_phase, phase0, counter);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
   const long long total = (long long)n_phase * g.plane_words;
-  long long blocks = (total + 7) / 8;
-  if (blocks > (long long)n_sm * 32) blocks = (long long)n_sm * 32;
-  if (blocks < 1) blocks = 1;
-  pack_kernel<<<(unsigned)blocks, 256, 0, st>>>(images, packed, g, B, Bpad, n_phase, phase0, counter);
+  blocks = (total + 255) / 256;
+  blocks = std::max(1ll, std::min(blocks, (long long)n_sm * 32));
+  pack_views_kernel<<<(unsigned)blocks, 256, 0, st>>>(base, packed, g, B, n_phase);
   return cudaGetLastError();
 }
 
