@@ -123,9 +123,8 @@ extern "C" void lpf_free_paths(lpf_paths* p) {
     for (auto& kv : p->programs) free_program(kv.second);
     if (p->d_packed) cudaFree(p->d_packed);
     if (p->d_counter) cudaFree(p->d_counter);
-    if (p->d_path_xy) cudaFree(p->d_path_xy);
-    if (p->d_path_off) cudaFree(p->d_path_off);
-    if (p->d_vecs) cudaFree(p->d_vecs);
+    if (p->d_swap_rec) cudaFree(p->d_swap_rec);
+    if (p->d_swap_bits) cudaFree(p->d_swap_bits);
     if (p->d_io_in) cudaFree(p->d_io_in);
     if (p->d_io_out) cudaFree(p->d_io_out);
     if (p->io_stream) cudaStreamDestroy((cudaStream_t)p->io_stream);
@@ -146,9 +145,9 @@ cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem,
 cudaError_t launch_mirror(unsigned long long* counts, int S, long long n_arrays, int n_sm, cudaStream_t st);
 cudaError_t launch_objective(const long long* counts, const long long* target, int B, long long K,
                              unsigned long long* sse, int n_sm, cudaStream_t st);
-cudaError_t launch_swap_delta(const uint8_t* image, int H, int W, int m, int phase, const int* pairs, long long n,
-                              const int16_t* path_xy, const int* path_off, const int16_t* vecs, int n_half,
-                              int* delta, cudaStream_t st);
+cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W, int m, int phase, const int* pairs,
+                              long long n, const int32_t* rec, int n_nodes, int* delta, unsigned int* counter,
+                              int n_sm, cudaStream_t st);
 
 static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, int n_phase, int phase0,
                      int64_t* counts, unsigned flags, void* stream) {
@@ -319,32 +318,15 @@ extern "C" int lpf_objective(const int64_t* counts, const int64_t* target, int B
 
 namespace lpf {
 
-// flattened canonical paths for the swap-delta kernel, built on first use
-static int ensure_path_table(lpf_paths* p) {
-  if (p->d_path_xy) return LPF_OK;
-  const int m = p->m;
+// node records of the image-coordinate trie for the swap-delta kernel, built and uploaded on first use
+static int ensure_swap_table(lpf_paths* p) {
+  if (p->d_swap_rec) return LPF_OK;
   try {
-    std::vector<int16_t> xy((size_t)p->sum_len * 2), vecs((size_t)p->n_half * 2), tmp(2 * (size_t)(m + 1));
-    std::vector<int32_t> off((size_t)p->n_half + 1);
-    size_t at = 0, v = 0;
-    for (int dy = 0; dy <= m; ++dy)
-      for (int dx = -m; dx <= m; ++dx) {
-        if (!in_half(dx, dy)) continue;
-        const int len = canonical_path(dx, dy, tmp.data());
-        off[v] = (int32_t)at;
-        vecs[2 * v] = (int16_t)dx;
-        vecs[2 * v + 1] = (int16_t)dy;
-        std::memcpy(&xy[2 * at], tmp.data(), sizeof(int16_t) * 2 * (size_t)len);
-        at += (size_t)len;
-        ++v;
-      }
-    off[v] = (int32_t)at;
-    LPF_CUDA(cudaMalloc(&p->d_path_xy, sizeof(int16_t) * xy.size()));
-    LPF_CUDA(cudaMalloc(&p->d_path_off, sizeof(int32_t) * off.size()));
-    LPF_CUDA(cudaMalloc(&p->d_vecs, sizeof(int16_t) * vecs.size()));
-    LPF_CUDA(cudaMemcpy(p->d_path_xy, xy.data(), sizeof(int16_t) * xy.size(), cudaMemcpyHostToDevice));
-    LPF_CUDA(cudaMemcpy(p->d_path_off, off.data(), sizeof(int32_t) * off.size(), cudaMemcpyHostToDevice));
-    LPF_CUDA(cudaMemcpy(p->d_vecs, vecs.data(), sizeof(int16_t) * vecs.size(), cudaMemcpyHostToDevice));
+    std::vector<int32_t> rec;
+    build_swap_records(p, rec);
+    if ((int64_t)rec.size() != 4 * p->n_trie_nodes) return LPF_E_INVAL;
+    LPF_CUDA(cudaMalloc(&p->d_swap_rec, sizeof(int32_t) * rec.size()));
+    LPF_CUDA(cudaMemcpy(p->d_swap_rec, rec.data(), sizeof(int32_t) * rec.size(), cudaMemcpyHostToDevice));
   } catch (const std::bad_alloc&) {
     return LPF_E_NOMEM;
   }
@@ -362,12 +344,21 @@ extern "C" int lpf_swap_delta(lpf_paths* p, const uint8_t* image, int H, int W, 
   if (n == 0) return LPF_OK;
   DeviceGuard dg(p->device);
   if (!dg.ok) return LPF_E_CUDA;
-  const size_t smem = (size_t)2 * H * ((W + 31) / 32) * 4;
-  if (smem > (size_t)p->max_smem) return LPF_E_UNSUPPORTED;
-  int rc = ensure_path_table(p);
+  // the base bit image and eight warp stacks of 8 KB live in shared memory; node indices are 24-bit
+  const size_t smem = (size_t)H * ((W + 31) / 32) * 4 + 8 + 8 * 1024 * 8;
+  if (smem + 2048 > (size_t)p->max_smem || p->n_trie_nodes >= (1 << 24)) return LPF_E_UNSUPPORTED;
+  int rc = ensure_swap_table(p);
   if (rc != LPF_OK) return rc;
-  LPF_CUDA(launch_swap_delta(image, H, W, p->m, phase, pairs, (long long)n, p->d_path_xy, p->d_path_off, p->d_vecs,
-                             (int)p->n_half, delta, (cudaStream_t)stream));
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t bits_bytes = ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32)) * 4;
+  if (bits_bytes > p->swap_bits_bytes) {
+    if (p->d_swap_bits) { LPF_CUDA(cudaStreamSynchronize(st)); cudaFree(p->d_swap_bits); p->d_swap_bits = nullptr; }
+    p->swap_bits_bytes = 0;
+    LPF_CUDA(cudaMalloc(&p->d_swap_bits, bits_bytes));
+    p->swap_bits_bytes = bits_bytes;
+  }
+  LPF_CUDA(launch_swap_delta(image, p->d_swap_bits, H, W, p->m, phase, pairs, (long long)n, p->d_swap_rec,
+                             (int)p->n_trie_nodes, delta, p->d_counter + 1, p->n_sm, st));
   return LPF_OK;
 }
 

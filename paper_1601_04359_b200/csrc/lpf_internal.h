@@ -113,10 +113,10 @@ struct lpf_paths {
   uint32_t* d_packed = nullptr;
   size_t packed_bytes = 0;
   unsigned int* d_counter = nullptr;
-  // swap-delta path table: canonical paths, flattened (built lazily)
-  int16_t* d_path_xy = nullptr;      // [sum_len][2]
-  int32_t* d_path_off = nullptr;     // [n_half + 1]
-  int16_t* d_vecs = nullptr;         // [n_half][2] = dx, dy of each canonical vector
+  // swap-delta node records: the image-coordinate trie in preorder, 16 bytes per node (built lazily)
+  int32_t* d_swap_rec = nullptr;     // [n_trie_nodes][4]
+  uint32_t* d_swap_bits = nullptr;   // packed base image of the last lpf_swap_delta call (grown on demand)
+  size_t swap_bits_bytes = 0;
   // device staging buffers of lpf_eval_host (grown on demand) and its private stream
   void* d_io_in = nullptr;
   size_t io_in_bytes = 0;
@@ -136,6 +136,9 @@ namespace lpf {
 // closed-form rasteriser: P_v for v in the canonical half (lpf_paths.cpp)
 int canonical_path(int dx, int dy, int16_t* xy);
 inline bool in_half(int dx, int dy) { return dy > 0 || (dy == 0 && dx >= 0); }
+
+// the image-coordinate trie in preorder for lpf_swap_delta (lpf_paths.cpp)
+void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec);
 
 // builds (or returns the cached) program for (piece_nodes, flags, view strides); host side only
 Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride01, int stride12);

@@ -6,7 +6,7 @@
 //                     warp reduce at terminals (a4), optional zero-mask pruning (a5)
 //   mirror_kernel     counts[-v] = counts[v] (a6)
 //   objective_kernel  sum (c - t)^2 per image (a8, Eq. 14/19)
-//   swap_delta_kernel per-proposal count deltas (a9)
+//   swap_delta_kernel_v3 + swap_mirror_kernel  per-proposal count deltas (a9)
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -407,84 +407,221 @@ __global__ void objective_kernel(const long long* __restrict__ counts, const lon
 }
 
 // ---------------------------------------------------------------------------------------------
-// swap delta, version 1.  One CTA per proposal.
-//   Bit plane Bp of the base image in shared memory (no halo, modular addressing), and a second
-//   copy Bq with the two bits exchanged.  If the two bits are equal nothing changes.  Otherwise let
-//   u be the pixel whose bit becomes 1 and w the one whose bit becomes 0:
-//     delta(v) = #{k : segment started at u - P_v[k] lies in phase in I'}   (it contains u)
-//              - #{k : segment started at w - P_v[k] lies in phase in I }   (it contains w)
-//   Warp per vector of D, lane per candidate k; the other half is the mirror delta(-v) = delta(v).
+// swap delta, version 3.
+//   For one proposal let u be the pixel whose bit becomes 1 and w the one whose bit becomes 0:
+//     delta(v) = #{segments of vector v that contain u and lie in phase in I'}
+//              - #{segments of vector v that contain w and lie in phase in I }
+//   A segment of v that has pixel px at path position k starts at s = px - P_v[k]; P_v[0..k] is a trie node N, so
+//   the candidates are exactly the pairs (trie node N, terminal D in the subtree of N) with start s_N = px - o_N.
+//   (A) lane per node N: the prefix root -> N must be in phase from s_N.  The parent's pixel is one of the 8
+//       neighbours of px (register mask lookup: most nodes stop there); the other ancestors' pixels are stepped
+//       backwards with Bresenham error arithmetic on a vector that runs through N -- no loads but the image bits.
+//   (B) the subtree of every surviving (N, start) is explored by the whole warp from a per-warp stack in shared
+//       memory: a lane pops one node, tests its pixel, counts it if it is a terminal, and pushes its next sibling
+//       (always) and its first child (if the pixel is in phase).  A dead prefix kills every vector below it at once.
+//   CTA = SW proposals (node records are fetched once for all of them); image bits in shared memory.
+//   delta must be zero on entry; only the canonical half is written (swap_mirror_kernel fills the rest).
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ bool seg_in_phase(const uint32_t* plane, int Wc, int H, int W, const short2* path,
-                                             int len, int sx, int sy) {
-  for (int jx = 0; jx < len; ++jx) {
-    const short2 o = path[jx];
-    int x = sx + o.x, y = sy + o.y;
-    x += (x < 0) ? W : 0;
-    x -= (x >= W) ? W : 0;
-    y += (y < 0) ? H : 0;
-    y -= (y >= H) ? H : 0;
-    if (!((plane[y * Wc + (x >> 5)] >> (x & 31)) & 1u)) return false;
-  }
-  return true;
+constexpr int SWAP_SW = 8;          // proposals per CTA
+constexpr int SWAP_STACK = 1024;    // items per warp stack (8 bytes each)
+
+__device__ __forceinline__ int wrap_coord(int x, int n) {
+  x += (x < 0) ? n : 0;
+  x -= (x >= n) ? n : 0;
+  return x;
 }
 
-__global__ void __launch_bounds__(256) swap_delta_kernel_v1(const uint8_t* __restrict__ image, int H, int W, int m,
-                                                             int phase, const int* __restrict__ pairs,
-                                                             const short2* __restrict__ path_xy,
-                                                             const int* __restrict__ path_off,
-                                                             const short2* __restrict__ vecs, int n_half,
+struct SwapPass {                   // one (proposal, pixel) pass, in shared memory
+  int px, py;                       // the swapped pixel the segments must contain
+  int ox, oy;                       // pixel that reads as out of phase in this pass (w in I'), or -1
+  unsigned nb;                      // in-phase bits of the 8 neighbours px - step, by step code
+  int sign;                         // +1: u on I', -1: w on I
+  int slot;                         // proposal index inside the CTA
+};
+
+__global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __restrict__ bits, int H, int W, int m,
+                                                             const int* __restrict__ pairs, long long n,
+                                                             const int4* __restrict__ rec, int n_nodes,
                                                              int* __restrict__ delta) {
   extern __shared__ __align__(16) uint32_t sm[];
+  __shared__ SwapPass s_pass[2 * SWAP_SW];
+  __shared__ int s_n;
   const int Wc = (W + 31) >> 5;
-  uint32_t* P0 = sm;                  // base image plane
-  uint32_t* P1 = sm + H * Wc;         // plane after the swap
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
-  const long long sw = blockIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint32_t* P = sm;                                                   // [H][Wc] bits of the base image I
+  uint2* stk = (uint2*)(sm + ((H * Wc + 1) & ~1)) + (size_t)warp * SWAP_STACK;
   const int S = 2 * m + 1;
-  int* out = delta + sw * (long long)S * S;
-  const int xp = pairs[4 * sw], yp = pairs[4 * sw + 1], xq = pairs[4 * sw + 2], yq = pairs[4 * sw + 3];
-  const bool ok = xp >= 0 && xp < W && xq >= 0 && xq < W && yp >= 0 && yp < H && yq >= 0 && yq < H;
-  for (int w = warp; w < H * Wc; w += nw) {
-    const int y = w / Wc, x = (w - y * Wc) * 32 + lane;
-    const bool bit = (x < W) && image[(size_t)y * W + x] == (uint8_t)phase;
-    const unsigned v = __ballot_sync(0xffffffffu, bit);
-    if (lane == 0) { P0[w] = v; P1[w] = v; }
-  }
+  const long long K = (long long)S * S;
+  for (int i = tid; i < H * Wc; i += blockDim.x) P[i] = bits[i];
   __syncthreads();
-  int bp = 0, bq = 0;
-  if (ok) {
-    bp = (P0[yp * Wc + (xp >> 5)] >> (xp & 31)) & 1;
-    bq = (P0[yq * Wc + (xq >> 5)] >> (xq & 31)) & 1;
-  }
-  if (!ok || bp == bq) {              // nothing changes for this phase
-    for (int k = tid; k < S * S; k += blockDim.x) out[k] = 0;
-    return;
-  }
-  __syncthreads();
-  if (tid == 0) {                     // exchange the two bits in P1
-    P1[yp * Wc + (xp >> 5)] ^= 1u << (xp & 31);
-    P1[yq * Wc + (xq >> 5)] ^= 1u << (xq & 31);
-  }
-  __syncthreads();
-  const int ux = bp ? xq : xp, uy = bp ? yq : yp;   // bit 0 -> 1
-  const int wx = bp ? xp : xq, wy = bp ? yp : yq;   // bit 1 -> 0
-  for (int v = warp; v < n_half; v += nw) {
-    const int off = path_off[v], len = path_off[v + 1] - off;
-    const short2* path = path_xy + off;
-    int d = 0;
-    for (int c = lane; c < 2 * len; c += 32) {
-      const int k = (c < len) ? c : c - len;
-      const short2 o = path[k];
-      if (c < len) d += seg_in_phase(P1, Wc, H, W, path, len, ux - o.x, uy - o.y) ? 1 : 0;
-      else d -= seg_in_phase(P0, Wc, H, W, path, len, wx - o.x, wy - o.y) ? 1 : 0;
+  if (tid == 0) {
+    int cnt = 0;
+    for (int j = 0; j < SWAP_SW; ++j) {
+      const long long sw = (long long)blockIdx.x * SWAP_SW + j;
+      if (sw >= n) break;
+      const int xp = pairs[4 * sw], yp = pairs[4 * sw + 1], xq = pairs[4 * sw + 2], yq = pairs[4 * sw + 3];
+      const bool ok = xp >= 0 && xp < W && xq >= 0 && xq < W && yp >= 0 && yp < H && yq >= 0 && yq < H;
+      if (!ok) continue;
+      const int bp = (P[yp * Wc + (xp >> 5)] >> (xp & 31)) & 1, bq = (P[yq * Wc + (xq >> 5)] >> (xq & 31)) & 1;
+      if (bp == bq) continue;                              // nothing changes for this phase
+      const int ux = bp ? xq : xp, uy = bp ? yq : yp;      // bit 0 -> 1
+      const int wx = bp ? xp : xq, wy = bp ? yp : yq;      // bit 1 -> 0
+      for (int pass = 0; pass < 2; ++pass) {
+        SwapPass sp;
+        sp.px = pass ? wx : ux; sp.py = pass ? wy : uy;
+        sp.ox = pass ? -1 : wx; sp.oy = pass ? -1 : wy;
+        sp.nb = 0;
+        for (int code = 0; code < 9; ++code) {
+          const int x = wrap_coord(sp.px - (code / 3 - 1), W), y = wrap_coord(sp.py - (code % 3 - 1), H);
+          unsigned bit = (P[y * Wc + (x >> 5)] >> (x & 31)) & 1u;
+          if (x == sp.ox && y == sp.oy) bit = 0;
+          sp.nb |= bit << code;
+        }
+        sp.sign = pass ? -1 : 1;
+        sp.slot = j;
+        s_pass[cnt++] = sp;
+      }
     }
-    d = __reduce_add_sync(0xffffffffu, d);
-    if (lane == 0) {
-      const short2 vv = vecs[v];
-      out[(vv.y + m) * S + (vv.x + m)] = d;
-      out[(-vv.y + m) * S + (-vv.x + m)] = d;
+    s_n = cnt;
+  }
+  __syncthreads();
+  const int np = s_n;
+  if (np == 0) return;
+  int* const out0 = delta + (long long)blockIdx.x * SWAP_SW * K;
+  const unsigned lt = (1u << lane) - 1u;
+  int top = 0;                                             // warp-uniform: items on this warp's stack
+
+  for (int N0 = warp * 32; N0 < n_nodes; N0 += blockDim.x) {
+    const int N = N0 + lane;
+    int4 rN = make_int4(0, 0, 0, 0);
+    if (N < n_nodes) rN = __ldg(rec + N);
+    const int oNx = (short)(rN.x & 0xffff), oNy = rN.x >> 16;
+    const int codeN = (rN.w >> 20) & 15;
+    const int d = max(abs(oNx), abs(oNy));                 // depth of N
+    // Bresenham state of the representative vector at position d (reading D2, closed form)
+    const int vx = (short)(rN.y & 0xffff), vy = rN.y >> 16;
+    const int ax = abs(vx), ay = abs(vy);
+    const bool xmaj = ax >= ay;
+    const int nn = xmaj ? ax : ay, mn = xmaj ? ay : ax;
+    const int sxs = (vx > 0) - (vx < 0), sys = (vy > 0) - (vy < 0);
+    const int q0 = xmaj ? abs(oNy) : abs(oNx);
+    const int e0 = 2 * d * mn + nn - 2 * nn * q0;
+    for (int q = 0; q < np; ++q) {
+      const unsigned nb = s_pass[q].nb;
+      bool alive = (N < n_nodes) && (d == 0 || ((nb >> codeN) & 1u));
+      if (!__any_sync(0xffffffffu, alive)) continue;       // typical for u: an isolated pixel kills all 32 at once
+      const int ox = s_pass[q].ox, oy = s_pass[q].oy;
+      const int sx = wrap_coord(s_pass[q].px - oNx, W), sy = wrap_coord(s_pass[q].py - oNy, H);
+      if (alive && d >= 2)                                 // the far end first: a long prefix usually dies at its start
+        alive = ((P[sy * Wc + (sx >> 5)] >> (sx & 31)) & 1u) && !(sx == ox && sy == oy);
+      if (alive) {
+        // (A) ancestors at positions d-2 .. 1 (d-1 was the neighbour test, 0 the start), stepping the error term backwards
+        int e = e0, qq = q0;
+        for (int k = d - 1; k >= 1; --k) {
+          e -= 2 * mn;
+          if (e < 0) { e += 2 * nn; --qq; }
+          if (k == d - 1) continue;
+          const int ax_ = xmaj ? sxs * k : sxs * qq, ay_ = xmaj ? sys * qq : sys * k;
+          const int x = wrap_coord(sx + ax_, W), y = wrap_coord(sy + ay_, H);
+          if (!((P[y * Wc + (x >> 5)] >> (x & 31)) & 1u) || (x == ox && y == oy)) { alive = false; break; }
+        }
+      }
+      int* const out = out0 + (long long)s_pass[q].slot * K;
+      const int sign = s_pass[q].sign;
+      if (alive && (rN.w & 0xFFFFF) != 0xFFFFF) atomicAdd(out + (rN.w & 0xFFFFF), sign);
+      // (B) push the first child of every survivor, then drain the warp stack
+      const bool push = alive && rN.z > 1;
+      const unsigned pm = __ballot_sync(0xffffffffu, push);
+      if (push)                                            // the stack is empty here (drained per pass)
+        stk[__popc(pm & lt)] =
+            make_uint2((unsigned)(N + 1) | ((unsigned)q << 24), (unsigned)sx | ((unsigned)sy << 16));
+      top = __popc(pm);
+      __syncwarp();
+      while (top > 0) {
+        const int take = min(top, 32);
+        uint2 it = make_uint2(0, 0);
+        if (lane < take) it = stk[top - 1 - lane];
+        top -= take;
+        __syncwarp();
+        bool p_sib = false, p_child = false;
+        int i = 0;
+        if (lane < take) {
+          i = (int)(it.x & 0xFFFFFF);
+          const int qi = (int)(it.x >> 24);
+          const int4 r = __ldg(rec + i);
+          const int isx = (int)(it.y & 0xffff), isy = (int)(it.y >> 16);
+          const int x = wrap_coord(isx + (short)(r.x & 0xffff), W), y = wrap_coord(isy + (r.x >> 16), H);
+          const bool in = ((P[y * Wc + (x >> 5)] >> (x & 31)) & 1u) && !(x == s_pass[qi].ox && y == s_pass[qi].oy);
+          if (in && (r.w & 0xFFFFF) != 0xFFFFF)
+            atomicAdd(out0 + (long long)s_pass[qi].slot * K + (r.w & 0xFFFFF), s_pass[qi].sign);
+          p_sib = (r.w >> 24) & 1;
+          p_child = in && r.z > 1;
+          if (p_sib) it.x += (unsigned)r.z;                // next sibling = i + subtree size
+        }
+        const unsigned ms = __ballot_sync(0xffffffffu, p_sib);
+        const unsigned mc = __ballot_sync(0xffffffffu, p_child);
+        const int ns = __popc(ms), nc = __popc(mc);
+        if (top + ns + nc > SWAP_STACK) {
+          // the stack cannot take this batch: every lane walks its own item's remainder serially (rare)
+          if (lane < take) {
+            const int qi = (int)(it.x >> 24);                // it.x may already point at the sibling: undo
+            const int isx = (int)(it.y & 0xffff), isy = (int)(it.y >> 16);
+            const int4 r0 = __ldg(rec + i);
+            // serial preorder scan of: the subtree of i below i (if in phase), then all later siblings' subtrees
+            int j = p_child ? i + 1 : i + r0.z;
+            // end of the scan: the parent's subtree end is unknown here, so follow sibling flags
+            bool more = true;
+            int cur_top = i;                                  // the sibling-level node whose subtree is scanned
+            int4 rt = r0;
+            while (more) {
+              const int end = cur_top + rt.z;
+              while (j < end) {
+                const int4 r = __ldg(rec + j);
+                const int x = wrap_coord(isx + (short)(r.x & 0xffff), W), y = wrap_coord(isy + (r.x >> 16), H);
+                const bool in = ((P[y * Wc + (x >> 5)] >> (x & 31)) & 1u) &&
+                                !(x == s_pass[qi].ox && y == s_pass[qi].oy);
+                if (in) {
+                  if ((r.w & 0xFFFFF) != 0xFFFFF)
+                    atomicAdd(out0 + (long long)s_pass[qi].slot * K + (r.w & 0xFFFFF), s_pass[qi].sign);
+                  ++j;
+                } else {
+                  j += r.z;
+                }
+              }
+              more = (rt.w >> 24) & 1;
+              if (more) {                                     // move to the next sibling: test it like any node
+                cur_top = end;
+                rt = __ldg(rec + cur_top);
+                const int x = wrap_coord(isx + (short)(rt.x & 0xffff), W), y = wrap_coord(isy + (rt.x >> 16), H);
+                const bool in = ((P[y * Wc + (x >> 5)] >> (x & 31)) & 1u) &&
+                                !(x == s_pass[qi].ox && y == s_pass[qi].oy);
+                if (in && (rt.w & 0xFFFFF) != 0xFFFFF)
+                  atomicAdd(out0 + (long long)s_pass[qi].slot * K + (rt.w & 0xFFFFF), s_pass[qi].sign);
+                j = in ? cur_top + 1 : cur_top + rt.z;
+              }
+            }
+          }
+        } else {
+          if (p_sib) stk[top + __popc(ms & lt)] = it;
+          if (p_child) stk[top + ns + __popc(mc & lt)] = make_uint2((unsigned)(i + 1) | (it.x & 0xFF000000u), it.y);
+          top += ns + nc;
+        }
+        __syncwarp();
+      }
     }
+  }
+}
+
+// delta(-v) = delta(v) (Eq. 12): fills the half outside D of every [S][S] array
+__global__ void swap_mirror_kernel(int* __restrict__ delta, int S, long long n_arrays) {
+  const long long K = (long long)S * S;
+  const long long half = K / 2;                            // indices below the centre are outside D
+  const long long total = n_arrays * half;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total;
+       i += (long long)gridDim.x * blockDim.x) {
+    const long long arr = i / half;
+    const long long k = i - arr * half;
+    delta[arr * K + k] = delta[arr * K + (K - 1 - k)];
   }
 }
 
@@ -546,19 +683,27 @@ cudaError_t launch_objective(const long long* counts, const long long* target, i
   return cudaGetLastError();
 }
 
-cudaError_t launch_swap_delta(const uint8_t* image, int H, int W, int m, int phase, const int* pairs, long long n,
-                              const int16_t* path_xy, const int* path_off, const int16_t* vecs, int n_half,
-                              int* delta, cudaStream_t st) {
-  const size_t smem = (size_t)2 * H * ((W + 31) / 32) * 4;
-  cudaError_t e = cudaFuncSetAttribute(swap_delta_kernel_v1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W, int m, int phase, const int* pairs,
+                              long long n, const int32_t* rec, int n_nodes, int* delta, unsigned int* counter,
+                              int n_sm, cudaStream_t st) {
+  const int Wc = (W + 31) / 32, Hc = (H + 31) / 32;
+  const size_t smem = (size_t)((H * Wc + 1) & ~1) * 4 + (size_t)8 * SWAP_STACK * 8;
+  cudaError_t e = cudaFuncSetAttribute(swap_delta_kernel_v3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   const long long S2 = (long long)(2 * m + 1) * (2 * m + 1);
-  for (long long s0 = 0; s0 < n; s0 += (1ll << 30)) {
-    const long long cnt = (n - s0 < (1ll << 30)) ? (n - s0) : (1ll << 30);
-    swap_delta_kernel_v1<<<(unsigned)cnt, 256, smem, st>>>(image, H, W, m, phase, pairs + 4 * s0,
-                                                          (const short2*)path_xy, path_off, (const short2*)vecs,
-                                                          n_half, delta + s0 * S2);
+  e = cudaMemsetAsync(delta, 0, sizeof(int) * (size_t)n * S2, st);
+  if (e != cudaSuccess) return e;
+  // stage 1 of the bit-pack gives the row-major bit image of the base image (the column-major half is unused)
+  pack_base_kernel<<<(unsigned)std::max(1, (Hc * Wc + 7) / 8), 256, 0, st>>>(image, bits, 1, H, W, 1, phase, counter);
+  const long long ctas = (n + SWAP_SW - 1) / SWAP_SW;
+  for (long long c0 = 0; c0 < ctas; c0 += (1ll << 30)) {
+    const long long cnt = std::min(ctas - c0, 1ll << 30);
+    const long long s0 = c0 * SWAP_SW;
+    swap_delta_kernel_v3<<<(unsigned)cnt, 256, smem, st>>>(bits, H, W, m, pairs + 4 * s0, n - s0, (const int4*)rec,
+                                                          n_nodes, delta + s0 * S2);
   }
+  long long blocks = std::min<long long>((n * (S2 / 2) + 255) / 256, (long long)n_sm * 16);
+  swap_mirror_kernel<<<(unsigned)std::max(1ll, blocks), 256, 0, st>>>(delta, 2 * m + 1, n);
   return cudaGetLastError();
 }
 

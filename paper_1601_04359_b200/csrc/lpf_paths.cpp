@@ -90,6 +90,56 @@ static void build_trie(lpf_paths* p) {
   }
 }
 
+// ---- swap-delta node records ----------------------------------------
+// The single prefix trie over D in IMAGE coordinates, in depth-first preorder; one 16-byte record per node:
+//   [0] (a & 0xffff) | (b << 16)    pixel offset of the node
+//   [1] (dx & 0xffff) | (dy << 16)  a canonical vector whose path runs through the node (its prefix IS the chain
+//                                   root -> node, so the ancestors' pixels follow from Bresenham arithmetic)
+//   [2] nodes in the subtree, self included (first child = index + 1, next sibling = index + [2])
+//   [3] bits 0-19: (b+m)(2m+1)+(a+m) if the prefix is a whole path P_v, else 0xFFFFF; bits 20-23: 3 (sa+1) + (sb+1)
+//       for the step (sa, sb) from the parent; bit 24: the node has a next sibling
+void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec) {
+  const int m = p->m;
+  std::vector<Node> nd;
+  nd.push_back(Node{0, 0, -1, -1, -1, 1, 0, 0});
+  std::vector<int16_t> xy(2 * (size_t)(m + 1));
+  for (int dy = 0; dy <= m; ++dy)
+    for (int dx = -m; dx <= m; ++dx) {
+      if (!in_half(dx, dy)) continue;
+      trie_insert(nd, xy.data(), canonical_path(dx, dy, xy.data()));
+    }
+  const size_t N = nd.size();
+  std::vector<int32_t> rep(N, 0);           // representative vector, packed; children are created after parents
+  for (int i = (int)N - 1; i >= 0; --i) {
+    if (nd[i].terminal) rep[i] = (int32_t)(((uint32_t)(uint16_t)nd[i].a) | ((uint32_t)(uint16_t)nd[i].b << 16));
+    if (i > 0) {
+      nd[nd[i].parent].size += nd[i].size;
+      if (!nd[nd[i].parent].terminal) rep[nd[i].parent] = rep[i];
+    }
+  }
+  rec.assign(4 * N, 0);
+  std::vector<std::pair<int, int>> stack{{0, 0}};   // (trie index, has next sibling)
+  int32_t at = 0;
+  std::vector<int> kids;
+  while (!stack.empty()) {
+    const int u = stack.back().first, sib = stack.back().second;
+    stack.pop_back();
+    const int par = nd[u].parent;
+    int step = 4;
+    if (par >= 0) step = 3 * (nd[u].a - nd[par].a + 1) + (nd[u].b - nd[par].b + 1);
+    const uint32_t cidx = nd[u].terminal ? (uint32_t)((nd[u].b + m) * (2 * m + 1) + (nd[u].a + m)) : 0xFFFFFu;
+    rec[4 * (size_t)at + 0] = (int32_t)(((uint32_t)(uint16_t)nd[u].a) | ((uint32_t)(uint16_t)nd[u].b << 16));
+    rec[4 * (size_t)at + 1] = rep[u];
+    rec[4 * (size_t)at + 2] = nd[u].size;
+    rec[4 * (size_t)at + 3] = (int32_t)(cidx | ((uint32_t)step << 20) | ((uint32_t)sib << 24));
+    ++at;
+    kids.clear();
+    for (int c = nd[u].first_child; c >= 0; c = nd[c].next_sibling) kids.push_back(c);
+    // popped in reverse push order: the first pushed child is emitted last and has no next sibling
+    for (size_t k = 0; k < kids.size(); ++k) stack.push_back({kids[k], k == 0 ? 0 : 1});
+  }
+}
+
 // ---- program emission ----------------------------------------------------------------------
 
 struct Emitter {
