@@ -109,7 +109,7 @@ def oracle_sample(w, imgs, seconds_hint, rng_seed=0, n_vec=None):
     m = w["m"]
     rng = np.random.default_rng(rng_seed)
     if n_vec is None:
-        n_vec = {2: 6000, 3: 1500, 4: 20000}[w["cfg"]]
+        n_vec = {2: 24000, 3: 6000, 4: 80000}[w["cfg"]]      # about 15 s on 16 cores
     vecs = rng.integers(-m, m + 1, size=(n_vec, 2))
     img = imgs[0]
     t0 = time.perf_counter()
@@ -261,6 +261,28 @@ def main():
         return dict(total_ms=total_ms, kernel_ms=kern_ms, e2e_s=e2e_s, e2e=e2e, info=info, launch=launch,
                     launches_per_step=launches_per_step, clocks=clocks, imgs=imgs, wall=wall)
 
+    def measure_swaps(n=20000):
+        """config 5: n independent two-pixel swap proposals on the 256x256 disk image, m = 64, phase 1."""
+        img = inputs.config_image(5)
+        pairs = inputs.config5_pairs(img, 2 * n)
+        p5 = lpf.lpf_build_paths(64, local_rank)
+        info5 = lpf.lpf_paths_info(p5)
+        d_img = torch.from_numpy(img[None]).cuda()
+        d_pairs = torch.from_numpy(pairs).cuda()
+        out = torch.empty((n, 129, 129), dtype=torch.int32, device="cuda")
+        lpf.lpf_swap_delta(p5, d_img, 1, d_pairs[:n], out=out)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        lpf.lpf_swap_delta(p5, d_img, 1, d_pairs[n:], out=out)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        lpf.lpf_free_paths(p5)
+        cand = 2 * (2 * info5["sum_path_len"] - 1)          # candidate (start, vector) tests per swap, SURVEY 8 a9
+        return {"swaps": n, "ms": ms, "swaps_per_s": n / (ms * 1e-3), "candidate_tests_per_s": n * cand / (ms * 1e-3),
+                "d2d_bytes_out": int(out.numel() * 4)}
+
     r = measure(w, args.steps, args.warmup, True)
     tests_per_step = nominal_tests(w) * world
     value = tests_per_step * args.steps / (r["total_ms"] * 1e-3)
@@ -276,6 +298,10 @@ def main():
     sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     peak_ops = SM_COUNT * ALU_LANES_PER_CLK_PER_SM * sm_max_mhz * 1e6
     achieved = alg_ops / (r["kernel_ms"] * 1e-3)
+    measured = lpf.lpf_alu_peak(local_rank) if rank == 0 else None     # live LOP3 / SHF / pair-pattern / POPC rates
+    # dram__bytes_read.sum + dram__bytes_write.sum of one eval-kernel launch, from the committed ncu --set full
+    # capture of this command (profiles/r01_v4_eval_kernel_full.csv: 42.55 MB + 15.11 MB); config 3, no flags only
+    traffic = 57.66e6 if (args.workload == "cfg3" and not args.flags) else None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": r["total_ms"] / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -285,7 +311,11 @@ def main():
                    "timing": "sum of per-step CUDA-event times on the launch stream, max over ranks",
                    "launch": r["launch"]},
         "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_ops / 1e12, "unit": "T int-op/s",
-                     "frac": achieved / peak_ops, "traffic": None,
+                     "frac": achieved / peak_ops, "traffic": traffic,
+                     "peak_measured": None if measured is None else
+                     {"lop3": measured["lop3"] / 1e12, "shf": measured["shf"] / 1e12,
+                      "shf_shf_lop3": measured["pair"] / 1e12, "popc": measured["popc"] / 1e12,
+                      "unit": "T int-op/s", "how": "lpf_alu_peak: 8 register-only chains per thread, all SMs, live"},
                      "kernel": "eval_kernel", "kernel_ms": r["kernel_ms"], "algorithmic_ops_per_launch": alg_ops,
                      "peak_source": "derived: 148 SM x 64 alu lanes/clk x %.0f MHz (sm_max_mhz of MEASURED_PEAKS.json)"
                                     % sm_max_mhz,
@@ -308,6 +338,7 @@ def main():
             extra[name] = {"value": nominal_tests(wl) * k / (rr["total_ms"] * 1e-3), "unit": UNIT,
                            "ms_per_step": rr["total_ms"] / k, "kernel_ms": rr["kernel_ms"],
                            "roofline_frac": ops / (rr["kernel_ms"] * 1e-3) / peak_ops}
+        extra["cfg5"] = measure_swaps()
         line["other_workloads"] = extra
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         tests, dt, cores, what = oracle_sample(w, r["imgs"], 20)

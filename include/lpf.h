@@ -140,6 +140,12 @@ int  lpf_last_launch_info(const lpf_paths* p, int64_t* out8);
 int  lpf_set_timing(lpf_paths* p, int enable);
 int  lpf_last_eval_kernel_ms(lpf_paths* p, float* ms);
 
+/* Measurement hook: runs a few milliseconds of register-only
+ * integer instructions on every SM of `device` (synchronous, default stream) and returns the measured thread-level
+ * instruction rates in ops/s: out4 = { LOP3, SHF.R.W, the eval kernel's SHF+SHF+LOP3 pair pattern, POPC }.
+ * It is the measured counterpart of the derived peak bench.py reports against; it touches no lpf_paths state. */
+int  lpf_alu_peak(int device, double* out4);
+
 /* Tuning hook: overrides the thread tile of the eval kernel -- TX x-adjacent words x
  * TY start rows per thread, (TX,TY) in {(4,2),(8,1),(4,4),(8,2),(16,1)}, and the warps per CTA (1..8) -- for the
  * following lpf_eval calls on this object; 0 = automatic choice.  Never changes a count.  INVAL otherwise. */

@@ -21,7 +21,7 @@ EXPORTS = (
     "lpf_strerror", "lpf_last_cuda_error", "lpf_build_paths", "lpf_free_paths", "lpf_paths_info",
     "lpf_paths_get", "lpf_paths_program", "lpf_eval", "lpf_eval_both", "lpf_objective",
     "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
-    "lpf_set_tile",
+    "lpf_set_tile", "lpf_alu_peak",
 )
 
 _lib = None
@@ -77,6 +77,8 @@ def load() -> ctypes.CDLL:
     lib.lpf_set_timing.restype = I
     lib.lpf_last_eval_kernel_ms.argtypes = [VP, ctypes.POINTER(ctypes.c_float)]
     lib.lpf_last_eval_kernel_ms.restype = I
+    lib.lpf_alu_peak.argtypes = [I, ctypes.POINTER(ctypes.c_double)]
+    lib.lpf_alu_peak.restype = I
     lib.lpf_set_tile.argtypes = [VP, I, I, I]
     lib.lpf_set_tile.restype = I
     _lib = lib
@@ -283,6 +285,13 @@ def lpf_last_launch_info(p: Paths) -> dict:
 
 def lpf_set_timing(p: Paths, enable: bool) -> None:
     _check(load().lpf_set_timing(p.handle, int(bool(enable))), "lpf_set_timing")
+
+
+def lpf_alu_peak(device: int = 0) -> dict:
+    """Measured thread-level integer instruction rates (ops/s) of the device: LOP3, SHF, SHF+SHF+LOP3, POPC."""
+    out = (ctypes.c_double * 4)()
+    _check(load().lpf_alu_peak(int(device), out), "lpf_alu_peak")
+    return dict(zip(("lop3", "shf", "pair", "popc"), [float(v) for v in out]))
 
 
 def lpf_set_tile(p: Paths, tx: int = 0, ty: int = 0, cta_warps: int = 0) -> None:
