@@ -305,7 +305,7 @@ def main():
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": r["total_ms"] / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "u32 bit-planes (u8 pixels in, int64 counts out)", "data": "synthetic",
+        "dtype": "u32", "data": "synthetic",
         "config": {"workload": args.workload_desc, "images_per_gpu": w["B"], "flags": args.flags or "none",
                    "l2": "flushed with a 256 MiB memset between timed steps",
                    "timing": "sum of per-step CUDA-event times on the launch stream, max over ranks",

@@ -174,15 +174,15 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   work_per_item = std::max(1, work_per_item / 4);
   const int n_gp = (Bpad / g.G) * n_phase;
 
-  // work items: about 16 per resident CTA, pieces of 512 .. 16384 trie nodes; fewer mask slots than the
+  // work items: about 20 per resident CTA (measured optimum on configs 2-4), pieces of 256 .. 16384 trie nodes; fewer mask slots than the
   // kernel provides (a smaller piece needs fewer)
   const int resident_guess = p->n_sm * 2;
   long long n_nodes = 0;
   for (int o = 0; o < 4; ++o) n_nodes += (long long)p->oct[o].size();
-  const long long want_items = std::max<long long>(1, 16ll * resident_guess / ((long long)n_gp * work_per_item));
+  const long long want_items = std::max<long long>(1, 32ll * resident_guess / ((long long)n_gp * work_per_item));
   long long piece = n_nodes / want_items;
-  piece = std::max<long long>(512, std::min<long long>(piece, 16384));
-  int q = 512;
+  piece = std::max<long long>(256, std::min<long long>(piece, 16384));
+  int q = 256;
   while (q * 2 <= piece) q *= 2;                   // quantised so that nearby shapes share one cached program
   Program* pr = nullptr;
   for (;; q /= 2) {
