@@ -145,6 +145,82 @@ def run_reference(args, w, rank, world):
     print(json.dumps(line))
 
 
+TAB1_SIZES = (10, 20, 50, 100, 200, 500)
+# paper's Tab. 1, standard / enhanced GPU seconds on a Quadro 4000, both phases; context only
+TAB1_PAPER = {"chess": {10: (2.4e-3, 2.4e-3), 20: (11.9e-3, 11.1e-3), 50: (0.15, 0.10), 100: (2.1, 0.26),
+                        200: (32.6, 2.0), 500: (318.4, 16.3)},
+              "squares": {10: (2.5e-3, 2.5e-3), 20: (12.9e-3, 12.5e-3), 50: (0.16, 0.13), 100: (2.5, 1.7),
+                          200: (41.9, 20.8), 500: (411.6, 205.1)}}
+
+
+def run_tab1(lpf, torch, device, out_dir):
+    """Tab. 1-shaped study: one evaluation of the ENTIRE L2 (all segments up to
+    W-1, H-1, i.e. m = size - 1) for both phases, standard and enhanced (LPF_PRUNE), on the two morphologies the
+    paper describes in words: chess with 10x10 px fields and a suspension of 4x4 px squares (its volume fraction is
+    not printed; 0.20 here).  Times: eval kernel alone, whole device step, and the paper's quantity -- host image in,
+    host counts out (Alg. 2 lines 6-21) -- through lpf_eval_host, mean of 5 after one warm-up.  Every cell is checked
+    bit-exactly against the CPU oracle on 200 random vectors per phase.  Returns a list of row dicts."""
+    from oracle import lpf_oracle as orc
+    rows = []
+    for size in TAB1_SIZES:
+        m = size - 1
+        p = lpf.lpf_build_paths(m, device)                    # paper step 1: untimed
+        lpf.lpf_set_timing(p, True)
+        for morph in ("chess", "squares"):
+            img = inputs.chess(size, size, 10) if morph == "chess" else \
+                inputs.squares(size, size, 4, 0.20, inputs.seed_for(6, size))
+            d_img = torch.from_numpy(img[None]).cuda()
+            h_in = torch.from_numpy(img[None].copy()).pin_memory()
+            S = 2 * m + 1
+            h_out = torch.empty((1, 2, S, S), dtype=torch.int64).pin_memory()
+            rng = np.random.default_rng(size)
+            vecs = rng.integers(-m, m + 1, size=(200, 2))
+            row = {"morphology": morph, "size": size, "segments": 2 * m * m + 2 * m + 1,
+                   "paper_gpu_s": TAB1_PAPER[morph][size]}
+            for name, flags in (("standard", 0), ("enhanced", lpf.LPF_PRUNE)):
+                out = lpf.lpf_eval_both(p, d_img, flags)
+                torch.cuda.synchronize()
+                c = out.cpu().numpy()[0]
+                for phase in (0, 1):
+                    want, _ = orc.counts_list(img, phase, vecs)
+                    got = c[phase][vecs[:, 1] + m, vecs[:, 0] + m]
+                    if not np.array_equal(got, want):
+                        raise AssertionError("tab1: %s %d %s phase %d differs from the oracle" % (morph, size, name, phase))
+                ker, dev_ms = [], []
+                for _ in range(5):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    lpf.lpf_eval_both(p, d_img, flags, out=out)
+                    e1.record()
+                    torch.cuda.synchronize()
+                    dev_ms.append(e0.elapsed_time(e1))
+                    ker.append(lpf.lpf_last_eval_kernel_ms(p))
+                lpf.lpf_eval_host(p, h_in, -1, h_out, flags)
+                t0 = time.perf_counter()
+                for _ in range(5):
+                    lpf.lpf_eval_host(p, h_in, -1, h_out, flags)
+                e2e = (time.perf_counter() - t0) / 5
+                row[name] = {"kernel_ms": float(np.mean(ker)), "device_ms": float(np.mean(dev_ms)), "e2e_s": e2e}
+            rows.append(row)
+            print("tab1 %-8s %4d  std %.3f ms  enh %.3f ms  e2e %.3f / %.3f ms" % (
+                morph, size, row["standard"]["device_ms"], row["enhanced"]["device_ms"],
+                1e3 * row["standard"]["e2e_s"], 1e3 * row["enhanced"]["e2e_s"]), file=sys.stderr, flush=True)
+        lpf.lpf_free_paths(p)
+    os.makedirs(out_dir, exist_ok=True)
+    with open(os.path.join(out_dir, "tab1.json"), "w") as f:
+        json.dump(rows, f, indent=1)
+    with open(os.path.join(out_dir, "tab1.md"), "w") as f:
+        f.write("| morphology | size | segments | std kernel ms | std e2e ms | enh kernel ms | enh e2e ms | "
+                "paper GPU std s | paper GPU enh s | e2e speed-up std | enh |\n|---|---|---|---|---|---|---|---|---|---|---|\n")
+        for r in rows:
+            ps, pe = r["paper_gpu_s"]
+            f.write("| %s | %d | %d | %.3f | %.3f | %.3f | %.3f | %g | %g | %.0fx | %.0fx |\n" % (
+                r["morphology"], r["size"], r["segments"], r["standard"]["kernel_ms"], 1e3 * r["standard"]["e2e_s"],
+                r["enhanced"]["kernel_ms"], 1e3 * r["enhanced"]["e2e_s"], ps, pe,
+                ps / r["standard"]["e2e_s"], pe / r["enhanced"]["e2e_s"]))
+    return rows
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -155,6 +231,9 @@ def main():
     ap.add_argument("--flags", default="")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the secondary workloads in the same JSON line")
+    ap.add_argument("--tab1", action="store_true",
+                    help="also run the Tab. 1-shaped size study (chess / 4x4 squares, 10..500 px, m = size - 1) and "
+                         "write gpurun_out/tab1.{json,md}")
     args = ap.parse_args()
     w = WORKLOADS[args.workload]
     rank = int(os.environ.get("RANK", "0"))
@@ -344,6 +423,9 @@ def main():
         tests, dt, cores, what = oracle_sample(w, r["imgs"], 20)
         line["cpu_baseline"] = {"value": tests / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what,
                                 "seconds": dt}
+    if args.tab1 and rank == 0 and world == 1:
+        rows = run_tab1(lpf, torch, local_rank, os.path.join(ROOT, "gpurun_out"))
+        line["tab1"] = {"rows": len(rows), "written_to": "gpurun_out/tab1.json, gpurun_out/tab1.md"}
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

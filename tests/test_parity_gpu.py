@@ -74,6 +74,25 @@ def test_ragged_shapes_both_phases_all_flags(H, W, m):
             assert np.array_equal(got, want), (phase, flags)
 
 
+@pytest.mark.parametrize("size", [50, 200])
+def test_tab1_morphologies_entire_domain(size):
+    """The paper's Tab. 1 workloads: chess with 10x10 px fields and 4x4 px squares, ALL segments up to
+    (W-1, H-1) (m = size - 1, widths that are not multiples of 32), standard and enhanced, sampled vectors."""
+    m = size - 1
+    rng = np.random.default_rng(size)
+    vecs = rng.integers(-m, m + 1, size=(150, 2))
+    for img in (inputs.chess(size, size, 10), inputs.squares(size, size, 4, 0.20, inputs.seed_for(6, size))):
+        for flags in (0, lpf.LPF_PRUNE):
+            both = lpf.lpf_eval_both(paths(m), dev(img[None]), flags)
+            torch.cuda.synchronize()
+            c = both.cpu().numpy()[0]
+            for phase in (0, 1):
+                want, _ = orc.counts_list(img, phase, vecs)
+                assert np.array_equal(c[phase][vecs[:, 1] + m, vecs[:, 0] + m], want)
+                assert c[phase][m, m] == int((img == phase).sum())
+                assert np.array_equal(c[phase], c[phase][::-1, ::-1])
+
+
 def test_degenerate_images():
     H, W, m = 48, 80, 20
     S = 2 * m + 1
