@@ -32,6 +32,9 @@
  * paths/image in tests/golden/, stripes and run-length closed forms, scipy erosion,
  * numpy FFT autocorrelation for |P_v| = 2 (Eq. 6/7), brute force by whole-array
  * roll-and-AND on tiny images, Eq. 10/12 invariants, Bernoulli statistics.
+ * lpf_oracle_counts_masked (L2~): all-ones mask = lpf_oracle_counts_list, additivity over disjoint
+ * masks, one-pixel masks vs the definition.  lpf_oracle_s2_counts (Eq. 6): numpy FFT form of Eq. 7, S2(0) = phase
+ * count, point symmetry, equality with the lineal-path counts for the 8 neighbours (|P_v| = 2).
  * Parity with the AUTHORS' numbers is unpinned: the paper prints no L2 value.
  *
  * Build:  gcc -O2 -fopenmp -shared -fPIC -o liblpf_oracle.so lpf_oracle.c
@@ -251,6 +254,50 @@ void lpf_oracle_swap_delta_local(const uint8_t *img, int H, int W, int phase, in
             delta[(size_t)(dy + m) * S + (dx + m)] = d;
         }
     free(img2); free(xy); free(sxs); free(sys);
+}
+
+/* L2~ of PAPER.md:160-164 (Monte-Carlo / N-position approximation, used in Eq. 14): the segments are compared with
+ * the image only at the start pixels whose mask byte is non-zero; out[i] = number of those starts at which segment
+ * vecs[i] lies in phase.  (L2~ = out / N with N = number of selected positions; the caller divides.)  Plain loops. */
+void lpf_oracle_counts_masked(const uint8_t *img, const uint8_t *mask, int H, int W, int phase,
+                              const int32_t *vecs, int64_t n, int64_t *out)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        int dx = vecs[2 * i], dy = vecs[2 * i + 1];
+        int cap = imax_(iabs_(dx), iabs_(dy)) + 1;
+        int16_t *xy = (int16_t *)malloc(sizeof(int16_t) * 2 * (size_t)cap);
+        int len = lpf_oracle_path(dx, dy, xy);
+        int64_t hits = 0;
+        for (int y = 0; y < H; ++y)
+            for (int x = 0; x < W; ++x) {
+                if (!mask[(size_t)y * W + x]) continue;          /* not a selected position */
+                int pix;
+                for (pix = 0; pix < len; ++pix) {
+                    int xx = pmod_(x + xy[2 * pix], W), yy = pmod_(y + xy[2 * pix + 1], H);
+                    if (img[(size_t)yy * W + xx] != phase) break;
+                }
+                if (pix == len) ++hits;
+            }
+        out[i] = hits;
+        free(xy);
+    }
+}
+
+/* Two-point probability S2 of Eq. 6, un-normalised: for every v = (dx,dy) of the template
+ *   out[dy+m][dx+m] = #{ (x1,y1) : chi(x1,y1) = 1 and chi((x1+dx)%W, (y1+dy)%H) = 1 },  chi = [byte == phase];
+ * S2 = out / (W*H).  The double sum of Eq. 6 written out; no FFT here (the FFT form, Eq. 7, is a PIN in the tests). */
+void lpf_oracle_s2_counts(const uint8_t *img, int H, int W, int phase, int m, int64_t *out)
+{
+    int S = 2 * m + 1;
+    for (int dy = -m; dy <= m; ++dy)
+        for (int dx = -m; dx <= m; ++dx) {
+            int64_t hits = 0;
+            for (int y1 = 0; y1 < H; ++y1)
+                for (int x1 = 0; x1 < W; ++x1)
+                    if (img[(size_t)y1 * W + x1] == phase &&
+                        img[(size_t)pmod_(y1 + dy, H) * W + pmod_(x1 + dx, W)] == phase) ++hits;
+            out[(size_t)(dy + m) * S + (dx + m)] = hits;
+        }
 }
 
 int lpf_oracle_max_threads(void)

@@ -54,6 +54,10 @@ def _load():
         lib.lpf_oracle_swap_delta_full.restype = I
         lib.lpf_oracle_swap_delta_local.argtypes = [c_u8p, I, I, I, I, I, I, I, I, c_i32p]
         lib.lpf_oracle_swap_delta_local.restype = None
+        lib.lpf_oracle_counts_masked.argtypes = [c_u8p, c_u8p, I, I, I, c_i32p, ctypes.c_int64, c_i64p]
+        lib.lpf_oracle_counts_masked.restype = None
+        lib.lpf_oracle_s2_counts.argtypes = [c_u8p, I, I, I, I, c_i64p]
+        lib.lpf_oracle_s2_counts.restype = None
         lib.lpf_oracle_max_threads.argtypes = []
         lib.lpf_oracle_max_threads.restype = I
         _lib = lib
@@ -106,6 +110,28 @@ def counts(image, phase: int, m: int, full_template: bool = False, threads: int 
     out = np.zeros((S, S), dtype=np.int64)
     _load().lpf_oracle_counts(_p(a, ctypes.c_uint8), a.shape[0], a.shape[1], int(phase), int(m),
                               _p(out, ctypes.c_int64), int(bool(full_template)), int(threads))
+    return out
+
+
+def counts_masked(image, mask, phase: int, vecs) -> np.ndarray:
+    """L2~ counts: hits of each vector over the start pixels with mask != 0."""
+    a = _img(image)
+    k = np.ascontiguousarray(mask, dtype=np.uint8)
+    assert k.shape == a.shape
+    v = np.ascontiguousarray(vecs, dtype=np.int32).reshape(-1, 2)
+    out = np.zeros(v.shape[0], dtype=np.int64)
+    _load().lpf_oracle_counts_masked(_p(a, ctypes.c_uint8), _p(k, ctypes.c_uint8), a.shape[0], a.shape[1], int(phase),
+                                     _p(v, ctypes.c_int32), v.shape[0], _p(out, ctypes.c_int64))
+    return out
+
+
+def s2_counts(image, phase: int, m: int) -> np.ndarray:
+    """Un-normalised two-point probability of Eq. 6: int64 [2m+1, 2m+1], index [dy+m, dx+m]."""
+    a = _img(image)
+    S = 2 * int(m) + 1
+    out = np.zeros((S, S), dtype=np.int64)
+    _load().lpf_oracle_s2_counts(_p(a, ctypes.c_uint8), a.shape[0], a.shape[1], int(phase), int(m),
+                                 _p(out, ctypes.c_int64))
     return out
 
 
