@@ -50,6 +50,11 @@ extern "C" {
 #define LPF_NO_TRIE  2u   /* one chain per path P_v (no prefix sharing): the "one-path-per-warp" design
                              variant, kept for the measurement in DESIGN.md. Same counts. */
 
+#define LPF_S2       4u   /* two-point probability instead of the lineal path: only the two END pixels of every
+                             segment are tested, counts[v] = #{x : I[x] and I[x+v] in phase} = W*H*S2(v), Eq. 6
+                             (PAPER.md:99); same kernels, a program of 2-pixel "paths".  Exact integers (the paper's
+                             FFT form, Eq. 7, is floating point). */
+
 typedef struct lpf_paths lpf_paths;   /* opaque: path table + prefix trie + device programs for one m */
 
 const char* lpf_strerror(int code);
@@ -78,7 +83,7 @@ int  lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, int cap, int
  * (DESIGN.md "Node program").  Every v in D is walked in one of four octant VIEWS of the image (transposed /
  * flipped so that the path is x-major with a' >= 0, 0 <= b' <= a'); each octant has its own prefix trie, cut
  * into connected pieces of about `piece_nodes` nodes (<= 0: one piece per octant); each piece is one item =
- * the chain from the root to the piece root followed by the piece in depth-first order.  flags: 0 or LPF_NO_TRIE.
+ * the chain from the root to the piece root followed by the piece in depth-first order.  flags: 0, LPF_NO_TRIE or LPF_S2.
  *   entries  host [cap_entries] uint64 (may be NULL to query sizes); low word: bits 0-4 a' & 31, bit 5 reload,
  *            6 terminal, 7 save, 8 restore, 9 init, 10 pair (own mask never needed, next entry is the direct child),
  *            bits 12-31 b' * stride + (a' >> 5); high word: bits 0-19
@@ -101,6 +106,17 @@ int  lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, unsigned fla
  * and D stops at W-1,H-1: PAPER.md:154), UNSUPPORTED, NOMEM, CUDA. */
 int  lpf_eval(lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase,
               int64_t* counts, unsigned flags, void* stream);
+
+/* Monte-Carlo / N-position approximation L2~ (used in Eq. 14): the segments are compared with the
+ * image only at the selected start positions.
+ *   start_mask dev uint8 [H][W], shared by the whole batch: a start pixel is selected iff its byte is non-zero
+ *   phase      0 | 1: counts dev int64 [B][2m+1][2m+1];  -1: both phases, counts dev int64 [B][2][2m+1][2m+1]
+ * counts[v] for v in D (Eq. 13) = number of selected starts at which P_v lies in phase (L2~ = counts / N, the caller
+ * divides by its N); the half outside D repeats it point-symmetrically, as the descriptor is stored in the paper
+ * -- with a proper subset of starts the definition itself is not symmetric (reading S16).
+ * A mask of all non-zero bytes gives exactly lpf_eval.  Same errors as lpf_eval. */
+int  lpf_eval_masked(lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase, const uint8_t* start_mask,
+                     int64_t* counts, unsigned flags, void* stream);
 
 /* Both phases in one call: counts dev int64 [B][2][2m+1][2m+1], index [b][phase][dy+m][dx+m]. */
 int  lpf_eval_both(lpf_paths* p, const uint8_t* images, int B, int H, int W,

@@ -150,13 +150,13 @@ cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W
                               int n_sm, cudaStream_t st);
 
 static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, int n_phase, int phase0,
-                     int64_t* counts, unsigned flags, void* stream) {
+                     int64_t* counts, unsigned flags, void* stream, const uint8_t* start_mask = nullptr) {
   if (!p || !images || !counts) return LPF_E_INVAL;
   if (p->device < 0) return LPF_E_INVAL;
   if (B < 1 || H < 1 || W < 1) return LPF_E_INVAL;
   if (n_phase == 1 && phase0 != 0 && phase0 != 1) return LPF_E_INVAL;
   if (p->m > std::min(H, W) - 1) return LPF_E_INVAL;
-  if (flags & ~(LPF_PRUNE | LPF_NO_TRIE)) return LPF_E_INVAL;
+  if (flags & ~(LPF_PRUNE | LPF_NO_TRIE | LPF_S2)) return LPF_E_INVAL;
   DeviceGuard dg(p->device);
   if (!dg.ok) return LPF_E_CUDA;
   cudaStream_t st = (cudaStream_t)stream;
@@ -183,6 +183,10 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   long long piece = n_nodes / want_items;
   piece = std::max<long long>(256, std::min<long long>(piece, 16384));
   int q = 256;
+  if (flags & LPF_S2) {                            // S2 items are lists of vectors, not trie pieces
+    piece = std::max<long long>(32, std::min<long long>(p->n_half / want_items, 4096));
+    q = 32;
+  }
   while (q * 2 <= piece) q *= 2;                   // quantised so that nearby shapes share one cached program
   Program* pr = nullptr;
   for (;; q /= 2) {
@@ -208,7 +212,17 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   // workspace: the packed octant views, then the compact row-major / column-major bit images of stage 1
   const size_t views_bytes = (size_t)n_phase * (size_t)g.plane_words * 4;
   const size_t base_words = (size_t)n_phase * B * ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32));
-  const size_t need = views_bytes + base_words * 4;
+  // ... and, for lpf_eval_masked, the views and the base bit images of the start mask (one image, one plane)
+  Geom gm = g;
+  size_t mask_views_bytes = 0, mask_base_bytes = 0;
+  if (start_mask) {
+    long long moff = 0;
+    for (int o = 0; o < 4; ++o) { gm.v[o].packed_off = moff; moff += gm.v[o].view_words; }
+    gm.plane_words = moff;
+    mask_views_bytes = (size_t)moff * 4;
+    mask_base_bytes = ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32)) * 4;
+  }
+  const size_t need = views_bytes + base_words * 4 + mask_views_bytes + mask_base_bytes;
   if (need > p->packed_bytes) {
     if (p->d_packed) { LPF_CUDA(cudaStreamSynchronize(st)); cudaFree(p->d_packed); p->d_packed = nullptr; p->packed_bytes = 0; }
     LPF_CUDA(cudaMalloc(&p->d_packed, need));
@@ -219,6 +233,9 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   LPF_CUDA(cudaMemsetAsync(counts, 0, sizeof(int64_t) * (size_t)B * n_phase * S * S, st));
   LPF_CUDA(launch_pack(images, p->d_packed + views_bytes / 4, p->d_packed, g, B, n_phase, phase0, p->d_counter,
                        p->n_sm, st));
+  uint32_t* const d_mask = p->d_packed + views_bytes / 4 + base_words;
+  if (start_mask)                                  // "phase" -1: a start pixel is selected iff its byte is non-zero
+    LPF_CUDA(launch_pack(start_mask, d_mask + mask_views_bytes / 4, d_mask, gm, 1, 1, -1, p->d_counter, p->n_sm, st));
 
   EvalParams ep;
   ep.g = g;
@@ -236,6 +253,8 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   ep.counter = p->d_counter;
   ep.prune = prune ? 1 : 0;
   ep.n_slots = pr->n_slots;
+  ep.mask = start_mask ? d_mask : nullptr;
+  for (int o = 0; o < 4; ++o) ep.mask_off[o] = gm.v[o].packed_off;
   const long long total_work = (long long)ep.n_work * n_gp;
   if (total_work >= (1ll << 32)) return LPF_E_UNSUPPORTED;
   const int grid = (int)std::min<long long>(total_work, resident);
@@ -250,7 +269,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   if (p->timing) LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_stop, st));
   LPF_CUDA(launch_mirror((unsigned long long*)counts, S, (long long)B * n_phase, p->n_sm, st));
 
-  p->last_info[0] = 4;                                   // kernels launched (pack base, pack views, eval, mirror)
+  p->last_info[0] = start_mask ? 6 : 4;                  // kernels launched (pack base, pack views, eval, mirror)
   p->last_info[1] = total_work;
   p->last_info[2] = (int64_t)pr->entries.size();         // program entries (all four octants)
   p->last_info[3] = grid;
@@ -271,6 +290,13 @@ extern "C" int lpf_eval(lpf_paths* p, const uint8_t* images, int B, int H, int W
 extern "C" int lpf_eval_both(lpf_paths* p, const uint8_t* images, int B, int H, int W, int64_t* counts,
                              unsigned flags, void* stream) {
   return lpf::eval_impl(p, images, B, H, W, 2, 0, counts, flags, stream);
+}
+
+extern "C" int lpf_eval_masked(lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase,
+                               const uint8_t* start_mask, int64_t* counts, unsigned flags, void* stream) {
+  if (!start_mask || phase < -1 || phase > 1) return LPF_E_INVAL;
+  return phase < 0 ? lpf::eval_impl(p, images, B, H, W, 2, 0, counts, flags, stream, start_mask)
+                   : lpf::eval_impl(p, images, B, H, W, 1, phase, counts, flags, stream, start_mask);
 }
 
 extern "C" int lpf_set_timing(lpf_paths* p, int enable) {

@@ -47,7 +47,7 @@ __global__ void __launch_bounds__(256) pack_base_kernel(const uint8_t* __restric
       const int y = ty * 32 + j;
       int v = 255;
       if (x < W && y < H) v = src[(size_t)j * W];
-      const bool b0 = n_phase == 2 ? (v == 0) : (v == phase0);
+      const bool b0 = n_phase == 2 ? (v == 0) : (phase0 < 0 ? (v != 0 && x < W && y < H) : (v == phase0));
       const bool b1 = n_phase == 2 && (v == 1);
       const unsigned r0 = __ballot_sync(0xffffffffu, b0);
       const unsigned r1 = __ballot_sync(0xffffffffu, b1);
@@ -271,6 +271,12 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
                 const int nb = v.Wv - 32 * (strip * TX + t);   // start pixels x' < Wv only
                 const uint32_t cm = nb >= 32 ? 0xffffffffu : (nb <= 0 ? 0u : ((1u << nb) - 1u));
                 M[ty * TX + t] = rowok ? cm : 0u;
+              }
+              if (p.mask != nullptr && rowok) {                  // L2~: only the selected start pixels
+                const uint32_t* mw = p.mask + p.mask_off[o] +
+                                     (size_t)(band * g.band_rows + row0 + ty * 32) * stride + strip * TX;
+#pragma unroll
+                for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __ldg(mw + t);
               }
             }
           } else {

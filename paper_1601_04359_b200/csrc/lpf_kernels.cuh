@@ -54,6 +54,8 @@ struct EvalParams {
   unsigned int* counter;      // dynamic work counter, zeroed by the pack kernel
   int prune;
   int n_slots;                // mask-stack slots of the program (<= STACK_SLOTS_BUDGET)
+  const uint32_t* mask;       // lpf_eval_masked: packed views of the start mask (one image), or nullptr
+  long long mask_off[4];      // word offset of each octant view inside `mask`
 };
 
 }  // namespace lpf

@@ -297,15 +297,67 @@ static void build_chain_program(lpf_paths* p, int piece_nodes, Program& pr) {
   sort_items(pr);
 }
 
+// LPF_S2: two-point probability (Eq. 6).  Every vector is a 2-pixel "path" {0, v}: the root window is
+// saved once per item and every vector restores it, ANDs the window at v and counts.  Items of about piece_nodes vectors.
+static void build_s2_program(lpf_paths* p, int piece_nodes, Program& pr) {
+  const int m = p->m;
+  if (piece_nodes <= 0) piece_nodes = 1 << 30;
+  for (int o = 0; o < 4; ++o) {
+    const int stride = pr.stride[o];
+    int64_t first = -1;
+    int in_item = 0;
+    bool zero_done = false;
+    for (int dy = 0; dy <= m; ++dy)
+      for (int dx = -m; dx <= m; ++dx) {
+        if (!in_half(dx, dy) || octant_of(dx, dy) != o) continue;
+        if (first < 0) {                                   // open an item: the root pixel, saved in slot 0
+          first = (int64_t)pr.entries.size();
+          uint32_t x = E_INIT | E_RELOAD | E_SAVE;
+          const bool count_zero = (o == 0 && !zero_done);  // v = 0 is counted once, in octant 0
+          if (count_zero) { x |= E_TERMINAL; zero_done = true; }
+          const uint32_t cidx0 = (uint32_t)(m * (2 * m + 1) + m);
+          pr.entries.push_back((uint64_t)x | ((uint64_t)cidx0 << 32));
+          pr.skip.push_back(0);
+          in_item = 0;
+        }
+        if (dx == 0 && dy == 0) continue;
+        int a, b;
+        to_view(o, dx, dy, &a, &b);
+        const uint32_t off = (uint32_t)(b * stride + (a >> 5));
+        const uint32_t x = (uint32_t)(a & 31) | E_RESTORE | E_RELOAD | E_TERMINAL | (off << E_OFF_SHIFT);
+        const uint32_t cidx = (uint32_t)((dy + m) * (2 * m + 1) + (dx + m));
+        pr.entries.push_back((uint64_t)x | ((uint64_t)cidx << 32));   // restore slot 0, save slot unused
+        pr.skip.push_back(0);
+        if (++in_item >= piece_nodes) {
+          pr.items.push_back(first);
+          pr.items.push_back((int64_t)pr.entries.size() - first);
+          pr.items.push_back(o);
+          pr.items.push_back(0);
+          first = -1;
+        }
+      }
+    if (first >= 0) {
+      pr.items.push_back(first);
+      pr.items.push_back((int64_t)pr.entries.size() - first);
+      pr.items.push_back(o);
+      pr.items.push_back(0);
+    }
+  }
+  pr.n_slots = 1;
+  sort_items(pr);
+}
+
 Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12) {
   if (piece_nodes < 0) piece_nodes = 0;
-  const std::tuple<int, unsigned, int, int> key(piece_nodes, flags & LPF_NO_TRIE, stride03, stride12);
+  const unsigned kind = (flags & LPF_S2) ? LPF_S2 : (flags & LPF_NO_TRIE);
+  const std::tuple<int, unsigned, int, int> key(piece_nodes, kind, stride03, stride12);
   auto it = p->programs.find(key);
   if (it != p->programs.end()) return it->second;
   Program& pr = p->programs[key];
   pr.stride[0] = pr.stride[3] = stride03;
   pr.stride[1] = pr.stride[2] = stride12;
-  if (flags & LPF_NO_TRIE) build_chain_program(p, piece_nodes, pr);
+  if (flags & LPF_S2) build_s2_program(p, piece_nodes, pr);
+  else if (flags & LPF_NO_TRIE) build_chain_program(p, piece_nodes, pr);
   else build_trie_program(p, piece_nodes, pr);
   return pr;
 }

@@ -15,13 +15,13 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "liblpf.so")
 
 LPF_OK, LPF_E_INVAL, LPF_E_NOMEM, LPF_E_CUDA, LPF_E_UNSUPPORTED = 0, -1, -2, -3, -4
-LPF_PRUNE, LPF_NO_TRIE = 1, 2
+LPF_PRUNE, LPF_NO_TRIE, LPF_S2 = 1, 2, 4
 
 EXPORTS = (
     "lpf_strerror", "lpf_last_cuda_error", "lpf_build_paths", "lpf_free_paths", "lpf_paths_info",
     "lpf_paths_get", "lpf_paths_program", "lpf_eval", "lpf_eval_both", "lpf_objective",
     "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
-    "lpf_set_tile", "lpf_alu_peak",
+    "lpf_set_tile", "lpf_alu_peak", "lpf_eval_masked",
 )
 
 _lib = None
@@ -65,6 +65,8 @@ def load() -> ctypes.CDLL:
     lib.lpf_eval.restype = I
     lib.lpf_eval_both.argtypes = [VP, VP, I, I, I, VP, U, VP]
     lib.lpf_eval_both.restype = I
+    lib.lpf_eval_masked.argtypes = [VP, VP, I, I, I, I, VP, VP, U, VP]
+    lib.lpf_eval_masked.restype = I
     lib.lpf_objective.argtypes = [VP, VP, I, I64, VP, VP]
     lib.lpf_objective.restype = I
     lib.lpf_swap_delta.argtypes = [VP, VP, I, I, I, VP, I64, VP, VP]
@@ -212,6 +214,25 @@ def lpf_eval_both(p: Paths, images, flags: int = 0, out=None, stream=None):
     assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() == B * 2 * S * S
     _check(lib.lpf_eval_both(p.handle, images.data_ptr(), B, H, W, out.data_ptr(), int(flags),
                              _stream_ptr(stream)), "lpf_eval_both")
+    return out
+
+
+def lpf_eval_masked(p: Paths, images, phase: int, start_mask, flags: int = 0, out=None, stream=None):
+    """L2~ counts over the selected start pixels (start_mask uint8 [H, W], non-zero = selected); phase 0 | 1 gives
+    int64 [B, 2m+1, 2m+1], phase -1 both phases [B, 2, 2m+1, 2m+1]."""
+    torch = _torch()
+    lib = load()
+    images = _dev_images(images, 3)
+    B, H, W = images.shape
+    assert start_mask.is_cuda and start_mask.dtype == torch.uint8 and tuple(start_mask.shape) == (H, W)
+    start_mask = start_mask.contiguous()
+    S = 2 * p.m + 1
+    shape = (B, 2, S, S) if phase < 0 else (B, S, S)
+    if out is None:
+        out = torch.empty(shape, dtype=torch.int64, device=images.device)
+    assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() == int(np.prod(shape))
+    _check(lib.lpf_eval_masked(p.handle, images.data_ptr(), B, H, W, int(phase), start_mask.data_ptr(),
+                               out.data_ptr(), int(flags), _stream_ptr(stream)), "lpf_eval_masked")
     return out
 
 

@@ -262,3 +262,76 @@ def test_eval_host_end_to_end_entry():
     assert np.array_equal(got[0], orc.counts(img, 1, 16))
     both = lpf.lpf_eval_host(paths(16), img, -1)
     assert np.array_equal(both[0, 0], orc.counts(img, 0, 16))
+
+
+# ---- S2 (LPF_S2, Eq. 6) and masked L2~ (lpf_eval_masked) -------------------------------------
+
+@pytest.mark.parametrize("H,W,m", [(1, 1, 0), (3, 5, 2), (12, 9, 8), (33, 31, 30), (40, 70, 39), (96, 128, 63)])
+def test_s2_counts_bit_exact(H, W, m):
+    rng = np.random.default_rng(7 * H + W)
+    img = (rng.random((H, W)) < 0.55).astype(np.uint8)
+    img[rng.random((H, W)) < 0.03] = 5
+    for phase in (0, 1):
+        want = orc.s2_counts(img, phase, m)
+        for flags in (lpf.LPF_S2, lpf.LPF_S2 | lpf.LPF_PRUNE):
+            got = gpu_counts(img, phase, m, flags)[0]
+            assert np.array_equal(got, want), (phase, flags)
+    both = lpf.lpf_eval_both(paths(m), dev(img[None]), lpf.LPF_S2).cpu().numpy()[0]
+    assert np.array_equal(both[0], orc.s2_counts(img, 0, m)) and np.array_equal(both[1], orc.s2_counts(img, 1, m))
+
+
+def test_s2_config2_size_against_fft_form():
+    """Full config-2 size: the exact integer S2 counts equal the rounded FFT autocorrelation of Eq. 7."""
+    img = inputs.config_image(2)
+    m = 128
+    got = gpu_counts(img, 1, m, lpf.LPF_S2)[0]
+    chi = (img == 1).astype(np.float64)
+    F = np.fft.fft2(chi)
+    corr = np.rint(np.fft.ifft2(F * np.conj(F)).real).astype(np.int64)
+    idx = (np.arange(-m, m + 1)) % 256
+    assert np.array_equal(got, corr[np.ix_((-np.arange(-m, m + 1)) % 256, (-np.arange(-m, m + 1)) % 256)])
+    assert idx.size == 2 * m + 1
+
+
+@pytest.mark.parametrize("H,W,m", [(2, 2, 1), (12, 9, 8), (31, 33, 12), (64, 96, 20), (65, 129, 64)])
+def test_masked_eval_matches_oracle_on_canonical_half(H, W, m):
+    rng = np.random.default_rng(H + 31 * W)
+    img = (rng.random((H, W)) < 0.8).astype(np.uint8)
+    mask = (rng.random((H, W)) < 0.3).astype(np.uint8) * rng.integers(1, 255, size=(H, W)).astype(np.uint8)
+    p = paths(m)
+    vecs = np.array([(dx, dy) for dy in range(0, m + 1) for dx in range(-m, m + 1)
+                     if orc.in_half(dx, dy)], dtype=np.int32)
+    if len(vecs) > 400:
+        vecs = vecs[rng.choice(len(vecs), 400, replace=False)]
+    for phase in (0, 1):
+        want = orc.counts_masked(img, mask, phase, vecs)
+        for flags in (0, lpf.LPF_PRUNE, lpf.LPF_NO_TRIE):
+            got = lpf.lpf_eval_masked(p, dev(img[None]), phase, dev(mask), flags).cpu().numpy()[0]
+            assert np.array_equal(got[vecs[:, 1] + m, vecs[:, 0] + m], want), (phase, flags)
+            assert np.array_equal(got, got[::-1, ::-1])       # the half outside D repeats D (reading S16)
+            assert got[m, m] == int(((img == phase) & (mask != 0)).sum())
+    # all positions selected: exactly lpf_eval; both phases in one call
+    ones = np.full((H, W), 200, dtype=np.uint8)
+    full = lpf.lpf_eval_both(p, dev(img[None])).cpu().numpy()
+    got = lpf.lpf_eval_masked(p, dev(img[None]), -1, dev(ones)).cpu().numpy()
+    assert np.array_equal(got, full)
+    # no position selected
+    assert not lpf.lpf_eval_masked(p, dev(img[None]), 1, dev(np.zeros((H, W), np.uint8))).cpu().numpy().any()
+
+
+def test_masked_batch_and_s2_combination():
+    rng = np.random.default_rng(5)
+    H, W, m = 48, 64, 17
+    imgs = (rng.random((5, H, W)) < 0.7).astype(np.uint8)
+    mask = (rng.random((H, W)) < 0.5).astype(np.uint8)
+    p = paths(m)
+    got = lpf.lpf_eval_masked(p, dev(imgs), 1, dev(mask)).cpu().numpy()
+    vecs = np.array([(3, 0), (0, 5), (-4, 9), (17, 17), (-17, 1), (7, 2)], dtype=np.int32)
+    for b in range(5):
+        assert np.array_equal(got[b][vecs[:, 1] + m, vecs[:, 0] + m], orc.counts_masked(imgs[b], mask, 1, vecs))
+    # masked two-point counts: start pixel selected and in phase, end pixel in phase
+    s2m = lpf.lpf_eval_masked(p, dev(imgs[:1]), 1, dev(mask), lpf.LPF_S2).cpu().numpy()[0]
+    chi = imgs[0] == 1
+    for dx, dy in vecs:
+        want = int((chi & (mask != 0) & np.roll(chi, (-dy, -dx), axis=(0, 1))).sum())
+        assert s2m[dy + m, dx + m] == want
