@@ -35,10 +35,14 @@
  * lpf_oracle_counts_masked (L2~): all-ones mask = lpf_oracle_counts_list, additivity over disjoint
  * masks, one-pixel masks vs the definition.  lpf_oracle_s2_counts (Eq. 6): numpy FFT form of Eq. 7, S2(0) = phase
  * count, point symmetry, equality with the lineal-path counts for the 8 neighbours (|P_v| = 2).
+ * lpf_oracle_anneal (Alg. 3): volume fractions preserved, E tracked = Eq. 19 of the final image re-evaluated, a huge
+ * T accepts every move (final image = all swaps applied, temperature levels = floor(N / s_max)), a tiny T never lets E
+ * grow, the local-delta form equals the literal re-evaluation form decision by decision.
  * Parity with the AUTHORS' numbers is unpinned: the paper prints no L2 value.
  *
  * Build:  gcc -O2 -fopenmp -shared -fPIC -o liblpf_oracle.so lpf_oracle.c
  */
+#include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
@@ -298,6 +302,98 @@ void lpf_oracle_s2_counts(const uint8_t *img, int H, int W, int phase, int m, in
                         img[(size_t)pmod_(y1 + dy, H) * W + pmod_(x1 + dx, W)] == phase) ++hits;
             out[(size_t)(dy + m) * S + (dx + m)] = hits;
         }
+}
+
+/* Simulated annealing, Alg. 3 with Tab. 2's parameters as arguments, on the integer
+ * descriptor.  Readings (the listing is garbled):
+ *   A1  one counter n runs over all N proposals (printed: "while c < N_step" although c is reset inside); c and s are
+ *       the per-temperature counters, s is incremented on acceptance (missing in the listing)
+ *   A2  T_mult = (T_min/T_max)^(s_max/N)  (printed exponent "succ_max/N_step")
+ *   A3  the error is minimised: accept iff u < exp((SDP - SDQ)/T) (the printed sign is a maximiser's), evaluated as
+ *       ln u < (E_P - E_Q) / ((W*H)^2 * T) with ln u given by the caller: only IEEE * and / are left
+ *   A4  SD error = Eq. 19 summed over D (Eq. 13) and over the requested phases, on L = count/(W*H):
+ *       e = E/(W*H)^2,  E = sum_phases sum_{v in D} (t_v - c_v)^2  (exact integer)
+ *   A5  modify(P) = exchange the bytes of the two pixels of proposal k (given by the caller); a pair
+ *       of equal bytes is the identity move (SDQ = SDP: accepted like any other move with no change of error)
+ *   phase: 0 | 1 = that phase only, -1 = both (target / counts hold [phase 0][phase 1] then).
+ *   use_local = 0: SDQ = evaluate(Q) from scratch, Alg. 3 line 10 literally;  1: counts(Q) = counts(P) + the
+ *   local swap delta (pinned to the literal form in the tests; for sizes the literal form cannot reach).
+ * img is modified in place; counts_out [n_ph][S][S] = descriptor of the final image (full template, mirrored);
+ * stats = { proposals done, accepted, temperature levels finished, final T, final E }; accept_log[N] (may be NULL)
+ * gets 1 for every accepted proposal. */
+static uint64_t half_sse_(const int64_t *c, const int64_t *t, int m)
+{
+    int S = 2 * m + 1;
+    uint64_t e = 0;
+    for (int dy = 0; dy <= m; ++dy)
+        for (int dx = -m; dx <= m; ++dx) {
+            if (!lpf_oracle_in_half(dx, dy)) continue;
+            int64_t d = t[(size_t)(dy + m) * S + (dx + m)] - c[(size_t)(dy + m) * S + (dx + m)];
+            e += (uint64_t)(d * d);
+        }
+    return e;
+}
+
+void lpf_oracle_anneal(uint8_t *img, int H, int W, int phase, int m, const int64_t *target,
+                       const int32_t *pairs, const double *log_u, int64_t N,
+                       double T_max, double T_min, int64_t c_max, int64_t s_max, int use_local,
+                       int64_t *counts_out, double *stats, uint8_t *accept_log)
+{
+    int S = 2 * m + 1;
+    size_t K = (size_t)S * S;
+    int n_ph = phase < 0 ? 2 : 1;
+    int64_t *cP = counts_out;                                  /* descriptor of P */
+    int64_t *cQ = (int64_t *)malloc(sizeof(int64_t) * K * n_ph);
+    int32_t *dl = (int32_t *)malloc(sizeof(int32_t) * K);
+    for (int i = 0; i < n_ph; ++i)                             /* line 2: SDP = evaluate(P) */
+        lpf_oracle_counts(img, H, W, phase < 0 ? i : phase, m, cP + K * i, 0, 0);
+    uint64_t EP = 0;
+    for (int i = 0; i < n_ph; ++i) EP += half_sse_(cP + K * i, target + K * i, m);
+    double T = T_max;                                          /* line 3 */
+    double T_mult = pow(T_min / T_max, (double)s_max / (double)N);   /* line 4, reading A2 */
+    double wh2 = (double)W * (double)H * (double)W * (double)H;
+    int64_t n = 0, accepted = 0, levels = 0;
+    while (n < N) {                                            /* line 5, reading A1 */
+        int64_t c = 0, s = 0;                                  /* line 6 */
+        while (c < c_max && s < s_max && n < N) {              /* line 7 */
+            c = c + 1;                                         /* line 8 */
+            int xp = pairs[4 * n], yp = pairs[4 * n + 1], xq = pairs[4 * n + 2], yq = pairs[4 * n + 3];
+            /* line 9: Q = modify(P) */
+            uint8_t bp = img[(size_t)yp * W + xp], bq = img[(size_t)yq * W + xq];
+            if (use_local) {
+                for (int i = 0; i < n_ph; ++i) {
+                    lpf_oracle_swap_delta_local(img, H, W, phase < 0 ? i : phase, m, xp, yp, xq, yq, dl);
+                    for (size_t k = 0; k < K; ++k) cQ[K * i + k] = cP[K * i + k] + dl[k];
+                }
+                img[(size_t)yp * W + xp] = bq; img[(size_t)yq * W + xq] = bp;
+            } else {
+                img[(size_t)yp * W + xp] = bq; img[(size_t)yq * W + xq] = bp;
+                for (int i = 0; i < n_ph; ++i)                 /* line 10: SDQ = evaluate(Q) */
+                    lpf_oracle_counts(img, H, W, phase < 0 ? i : phase, m, cQ + K * i, 0, 0);
+            }
+            uint64_t EQ = 0;
+            for (int i = 0; i < n_ph; ++i) EQ += half_sse_(cQ + K * i, target + K * i, m);
+            double num = (double)((int64_t)EP - (int64_t)EQ);  /* exact: |E| < 2^53 */
+            double den = wh2 * T;
+            int acc = log_u[n] < num / den;                    /* line 11, reading A3 */
+            if (acc) {                                         /* lines 12-13: P = Q, SDP = SDQ */
+                memcpy(cP, cQ, sizeof(int64_t) * K * n_ph);
+                EP = EQ;
+                s = s + 1;
+                ++accepted;
+            } else {                                           /* undo the modification */
+                img[(size_t)yp * W + xp] = bp; img[(size_t)yq * W + xq] = bq;
+            }
+            if (accept_log) accept_log[n] = (uint8_t)acc;
+            ++n;
+        }
+        if (c >= c_max || s >= s_max) {                        /* the temperature level is complete */
+            T = T * T_mult;                                    /* line 17 */
+            ++levels;
+        }
+    }
+    stats[0] = (double)n; stats[1] = (double)accepted; stats[2] = (double)levels; stats[3] = T; stats[4] = (double)EP;
+    free(cQ); free(dl);
 }
 
 int lpf_oracle_max_threads(void)

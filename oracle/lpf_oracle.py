@@ -26,7 +26,7 @@ def build(force: bool = False) -> str:
     if stale:
         tmp = _LIB + ".tmp.%d" % os.getpid()
         subprocess.check_call(["gcc", "-O2", "-std=c99", "-fopenmp", "-shared", "-fPIC",
-                               "-o", tmp, _SRC])
+                               "-o", tmp, _SRC, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -58,6 +58,10 @@ def _load():
         lib.lpf_oracle_counts_masked.restype = None
         lib.lpf_oracle_s2_counts.argtypes = [c_u8p, I, I, I, I, c_i64p]
         lib.lpf_oracle_s2_counts.restype = None
+        lib.lpf_oracle_anneal.argtypes = [c_u8p, I, I, I, I, c_i64p, c_i32p, ctypes.POINTER(ctypes.c_double),
+                                          ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int64,
+                                          ctypes.c_int64, I, c_i64p, ctypes.POINTER(ctypes.c_double), c_u8p]
+        lib.lpf_oracle_anneal.restype = None
         lib.lpf_oracle_max_threads.argtypes = []
         lib.lpf_oracle_max_threads.restype = I
         _lib = lib
@@ -133,6 +137,38 @@ def s2_counts(image, phase: int, m: int) -> np.ndarray:
     _load().lpf_oracle_s2_counts(_p(a, ctypes.c_uint8), a.shape[0], a.shape[1], int(phase), int(m),
                                  _p(out, ctypes.c_int64))
     return out
+
+
+def anneal(image, phase: int, m: int, target, pairs, log_u, T_max: float, T_min: float, c_max: int, s_max: int,
+           use_local: bool = False):
+    """Alg. 3.  Returns (final image, counts [n_ph, S, S], stats dict, accept log uint8 [N])."""
+    a = _img(image).copy()
+    S = 2 * int(m) + 1
+    n_ph = 2 if phase < 0 else 1
+    t = np.ascontiguousarray(target, dtype=np.int64).reshape(n_ph, S, S)
+    pr = np.ascontiguousarray(pairs, dtype=np.int32).reshape(-1, 4)
+    lu = np.ascontiguousarray(log_u, dtype=np.float64)
+    assert lu.shape[0] == pr.shape[0]
+    counts_out = np.zeros((n_ph, S, S), dtype=np.int64)
+    stats = np.zeros(5, dtype=np.float64)
+    log = np.zeros(pr.shape[0], dtype=np.uint8)
+    _load().lpf_oracle_anneal(_p(a, ctypes.c_uint8), a.shape[0], a.shape[1], int(phase), int(m), _p(t, ctypes.c_int64),
+                              _p(pr, ctypes.c_int32), _p(lu, ctypes.c_double), pr.shape[0], float(T_max), float(T_min),
+                              int(c_max), int(s_max), int(bool(use_local)), _p(counts_out, ctypes.c_int64),
+                              _p(stats, ctypes.c_double), _p(log, ctypes.c_uint8))
+    keys = ("steps", "accepted", "levels", "T", "E")
+    return a, counts_out, dict(zip(keys, [float(v) for v in stats])), log
+
+
+def half_sse(c, t, m: int) -> int:
+    """Eq. 19 over D (reading A4): sum over the canonical half of (t - c)^2, exact; numpy, for the tests."""
+    c = np.asarray(c, dtype=np.int64)
+    t = np.asarray(t, dtype=np.int64)
+    S = 2 * int(m) + 1
+    k = np.arange(S * S).reshape(S, S)
+    half = k >= (m * S + m)
+    d = (t - c)[..., half]
+    return int((d * d).sum())
 
 
 def sse(c, t) -> int:

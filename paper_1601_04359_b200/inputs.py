@@ -116,6 +116,18 @@ def swap_pairs(image: np.ndarray, n: int, seed: int) -> np.ndarray:
     return np.stack([zx[ip], zy[ip], ox[iq], oy[iq]], axis=1).astype(np.int32)
 
 
+def anneal_proposals(H: int, W: int, n: int, seed: int):
+    """Inputs of the annealing loop (Alg. 3): n proposals of two uniformly drawn pixels, int32 [n, 4] =
+    (x_p, y_p, x_q, y_q), and ln(u) of n uniform random numbers u in [0, 1) for the Metropolis rule (float64; -inf for u = 0).
+    Both sides receive these arrays; neither draws random numbers itself."""
+    rng = np.random.default_rng(seed)
+    pairs = np.stack([rng.integers(0, W, n), rng.integers(0, H, n), rng.integers(0, W, n), rng.integers(0, H, n)],
+                     axis=1).astype(np.int32)
+    with np.errstate(divide="ignore"):
+        log_u = np.log(rng.random(n))
+    return pairs, log_u
+
+
 # --- the five BASELINE.json configs -------------------------------------------------
 
 CONFIGS = {
