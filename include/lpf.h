@@ -138,6 +138,23 @@ int  lpf_objective(const int64_t* counts, const int64_t* target, int B, int64_t 
 int  lpf_swap_delta(lpf_paths* p, const uint8_t* image, int H, int W, int phase,
                     const int32_t* pairs, int64_t n, int32_t* delta, void* stream);
 
+/* Simulated annealing of Alg. 3 with the two-pixel swap and the least-square
+ * error of Eq. 19 on the lineal path descriptor; Tab. 2's parameters are arguments.  Readings A1-A5 of
+ * the garbled listing are listed in DESIGN.md "Annealing readings".  The chain is exactly the sequential one:
+ * proposal k exchanges the bytes of pixels (x_p,y_p), (x_q,y_q) = pairs[k]; it is accepted iff
+ * log_u[k] < (E_P - E_Q) / ((W*H)^2 * T), E = sum over the phases and v in D of (target - counts)^2; a pair of equal
+ * bytes (or out of range) is the identity move; T *= (T_min/T_max)^(s_max/N) whenever c_max proposals or s_max
+ * acceptances were seen at the current temperature.  Batches of consecutive proposals are evaluated speculatively in
+ * parallel (lpf_swap_delta) and decided in order on the device.
+ *   image dev uint8 [H][W], modified in place      phase 0 | 1 | -1 (both: target/counts are [2][2m+1][2m+1])
+ *   target dev int64 [n_ph][2m+1][2m+1]            pairs dev int32 [N][4], log_u dev double [N] (ln of uniforms in [0,1))
+ *   counts dev int64 [n_ph][2m+1][2m+1]: descriptor of the final image      accept_log dev uint8 [N] or NULL
+ *   stats5 HOST double[5] = { proposals done, accepted, temperature levels completed, final T, final E }
+ * Synchronous: returns when the chain is finished.  Errors as lpf_eval / lpf_swap_delta. */
+int  lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase, const int64_t* target, const int32_t* pairs,
+                const double* log_u, int64_t N, double T_max, double T_min, int64_t c_max, int64_t s_max,
+                int64_t* counts, uint8_t* accept_log, double* stats5, void* stream);
+
 /* HOST-buffer convenience used by the end-to-end measurement: copies `images` (host, pinned or
  * not) to the device, runs lpf_eval(_both if phase < 0), copies counts back, synchronises. */
 int  lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, int H, int W, int phase,

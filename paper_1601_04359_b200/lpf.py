@@ -21,7 +21,7 @@ EXPORTS = (
     "lpf_strerror", "lpf_last_cuda_error", "lpf_build_paths", "lpf_free_paths", "lpf_paths_info",
     "lpf_paths_get", "lpf_paths_program", "lpf_eval", "lpf_eval_both", "lpf_objective",
     "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
-    "lpf_set_tile", "lpf_alu_peak", "lpf_eval_masked",
+    "lpf_set_tile", "lpf_alu_peak", "lpf_eval_masked", "lpf_anneal",
 )
 
 _lib = None
@@ -67,6 +67,9 @@ def load() -> ctypes.CDLL:
     lib.lpf_eval_both.restype = I
     lib.lpf_eval_masked.argtypes = [VP, VP, I, I, I, I, VP, VP, U, VP]
     lib.lpf_eval_masked.restype = I
+    lib.lpf_anneal.argtypes = [VP, VP, I, I, I, VP, VP, VP, I64, ctypes.c_double, ctypes.c_double, I64, I64, VP, VP,
+                               ctypes.POINTER(ctypes.c_double), VP]
+    lib.lpf_anneal.restype = I
     lib.lpf_objective.argtypes = [VP, VP, I, I64, VP, VP]
     lib.lpf_objective.restype = I
     lib.lpf_swap_delta.argtypes = [VP, VP, I, I, I, VP, I64, VP, VP]
@@ -234,6 +237,33 @@ def lpf_eval_masked(p: Paths, images, phase: int, start_mask, flags: int = 0, ou
     _check(lib.lpf_eval_masked(p.handle, images.data_ptr(), B, H, W, int(phase), start_mask.data_ptr(),
                                out.data_ptr(), int(flags), _stream_ptr(stream)), "lpf_eval_masked")
     return out
+
+
+def lpf_anneal(p: Paths, image, phase: int, target, pairs, log_u, T_max: float, T_min: float, c_max: int, s_max: int,
+               accept_log=None, stream=None):
+    """Alg. 3 on the device.  image: CUDA uint8 [H, W], modified in place.  Returns (counts int64 [n_ph, S, S], stats)."""
+    torch = _torch()
+    lib = load()
+    assert image.is_cuda and image.dtype == torch.uint8 and image.dim() == 2 and image.is_contiguous()
+    H, W = image.shape
+    S = 2 * p.m + 1
+    n_ph = 2 if phase < 0 else 1
+    target = target.contiguous()
+    pairs = pairs.contiguous()
+    log_u = log_u.contiguous()
+    assert target.is_cuda and target.dtype == torch.int64 and target.numel() == n_ph * S * S
+    assert pairs.is_cuda and pairs.dtype == torch.int32 and pairs.dim() == 2 and pairs.shape[1] == 4
+    assert log_u.is_cuda and log_u.dtype == torch.float64 and log_u.numel() == pairs.shape[0]
+    if accept_log is not None:
+        assert accept_log.is_cuda and accept_log.dtype == torch.uint8 and accept_log.numel() == pairs.shape[0]
+    counts = torch.empty((n_ph, S, S), dtype=torch.int64, device=image.device)
+    stats = (ctypes.c_double * 5)()
+    _check(lib.lpf_anneal(p.handle, image.data_ptr(), H, W, int(phase), target.data_ptr(), pairs.data_ptr(),
+                          log_u.data_ptr(), pairs.shape[0], float(T_max), float(T_min), int(c_max), int(s_max),
+                          counts.data_ptr(), accept_log.data_ptr() if accept_log is not None else None, stats,
+                          _stream_ptr(stream)), "lpf_anneal")
+    keys = ("steps", "accepted", "levels", "T", "E")
+    return counts, dict(zip(keys, [float(v) for v in stats]))
 
 
 def lpf_objective(counts, target, out=None, stream=None):

@@ -335,3 +335,60 @@ def test_masked_batch_and_s2_combination():
     for dx, dy in vecs:
         want = int((chi & (mask != 0) & np.roll(chi, (-dy, -dx), axis=(0, 1))).sum())
         assert s2m[dy + m, dx + m] == want
+
+
+# ---- simulated annealing (lpf_anneal, Alg. 3) ---------------------------------------------------------------
+
+def _anneal_case(H, W, m, phase, seed, N):
+    rng = np.random.default_rng(seed)
+    target_img = inputs.squares(H, W, 3, 0.35, seed)
+    start = target_img.flatten()
+    rng.shuffle(start)
+    start = start.reshape(H, W)
+    phases = (0, 1) if phase < 0 else (phase,)
+    target = np.stack([orc.counts(target_img, ph, m) for ph in phases])
+    pairs, log_u = inputs.anneal_proposals(H, W, N, seed + 1)
+    E0 = sum(orc.half_sse(orc.counts(start, ph, m), target[i], m) for i, ph in enumerate(phases))
+    return start, target, pairs, log_u, E0
+
+
+@pytest.mark.parametrize("H,W,m,phase,N,c_max,s_max,use_local", [
+    (12, 10, 5, 1, 150, 15, 5, False),          # literal oracle (re-evaluates everything per proposal)
+    (12, 10, 5, -1, 150, 15, 5, False),
+    (24, 40, 11, 0, 600, 60, 12, True),
+    (33, 31, 16, -1, 400, 40, 9, True),
+])
+def test_anneal_chain_is_decision_for_decision_the_oracles(H, W, m, phase, N, c_max, s_max, use_local):
+    start, target, pairs, log_u, E0 = _anneal_case(H, W, m, phase, 100 + H, N)
+    T_max = 2.0 * E0 / (H * W) ** 2 / 50
+    w_img, w_counts, w_st, w_log = orc.anneal(start, phase, m, target, pairs, log_u, T_max, 0.01 * T_max, c_max, s_max,
+                                              use_local=use_local)
+    d_img = dev(start)
+    d_log = torch.zeros(N, dtype=torch.uint8, device="cuda")
+    counts, st = lpf.lpf_anneal(paths(m), d_img, phase, dev(target), dev(pairs), dev(log_u), T_max, 0.01 * T_max,
+                                c_max, s_max, accept_log=d_log)
+    assert np.array_equal(d_log.cpu().numpy(), w_log)                  # every Metropolis decision
+    assert np.array_equal(d_img.cpu().numpy(), w_img)
+    assert np.array_equal(counts.cpu().numpy(), w_counts)
+    assert st == w_st                                                  # steps, accepted, levels, final T (bitwise), E
+    assert 0 < w_log.sum() < N
+
+
+def test_anneal_limits_and_identity_moves():
+    H, W, m, N = 16, 16, 7, 200
+    start, target, pairs, log_u, _ = _anneal_case(H, W, m, 1, 77, N)
+    pairs[5] = (3, 3, 3, 3)                                            # same pixel: identity move, accepted
+    # huge temperature: every proposal accepted, final image = all swaps applied
+    d_img = dev(start)
+    counts, st = lpf.lpf_anneal(paths(m), d_img, 1, dev(target), dev(pairs), dev(log_u), 1e300, 1e300, 50, 7)
+    want = start.copy()
+    for xp, yp, xq, yq in pairs:
+        want[yp, xp], want[yq, xq] = want[yq, xq], want[yp, xp]
+    assert np.array_equal(d_img.cpu().numpy(), want)
+    assert st["steps"] == N and st["accepted"] == N and st["levels"] == N // 7
+    assert np.array_equal(counts.cpu().numpy()[0], orc.counts(want, 1, m))
+    assert st["E"] == orc.half_sse(orc.counts(want, 1, m), target[0], m)
+    # N = 0: nothing happens, the descriptor of the start image comes back
+    d_img = dev(start)
+    counts, st = lpf.lpf_anneal(paths(m), d_img, 1, dev(target), dev(pairs[:0]), dev(log_u[:0]), 1.0, 0.01, 5, 5)
+    assert st["steps"] == 0 and np.array_equal(counts.cpu().numpy()[0], orc.counts(start, 1, m))
