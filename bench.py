@@ -362,6 +362,40 @@ def main():
         return {"swaps": n, "ms": ms, "swaps_per_s": n / (ms * 1e-3), "candidate_tests_per_s": n * cand / (ms * 1e-3),
                 "d2d_bytes_out": int(out.numel() * 4)}
 
+    def measure_anneal(n=20000):
+        """Alg. 3 (lpf_anneal) on the paper's compression setting: target = descriptor of a 100x100
+        suspension of 4x4 squares, start = its pixels shuffled, both phases, m = 49, Tab. 2 ratios for c_max, s_max."""
+        H = W = 100
+        m = 49
+        tgt_img = inputs.squares(H, W, 4, 0.20, inputs.seed_for(7))
+        start = tgt_img.flatten()
+        np.random.default_rng(inputs.seed_for(7, 1)).shuffle(start)
+        pairs, log_u = inputs.anneal_proposals(H, W, n, inputs.seed_for(7, 2))
+        pa = lpf.lpf_build_paths(m, local_rank)
+        target = lpf.lpf_eval_both(pa, torch.from_numpy(tgt_img[None]).cuda())[0].clone()
+        d_img = torch.from_numpy(start.reshape(1, H, W).copy()).cuda()
+        c0 = lpf.lpf_eval_both(pa, d_img)[0]
+        half = torch.arange((2 * m + 1) ** 2, device="cuda").reshape(2 * m + 1, 2 * m + 1) >= (m * (2 * m + 1) + m)
+        E0 = float((((target - c0)[:, half]) ** 2).sum())
+        # T_max so that a typical worsening move is accepted with probability 1/2 at the start (Tab. 2: "s/c = 0.5"):
+        # pilot of 256 proposals against the start image
+        d_pairs = torch.from_numpy(pairs).cuda()
+        dE = torch.zeros(256, dtype=torch.int64, device="cuda")
+        for ph in (0, 1):
+            dl = lpf.lpf_swap_delta(pa, d_img, ph, d_pairs[:256]).to(torch.int64)[:, half]
+            dd = (target[ph] - c0[ph])[half]
+            dE += (dl * dl - 2 * dd[None] * dl).sum(dim=1)
+        worse = dE[dE > 0].double()
+        T_max = float(worse.mean()) / (H * W) ** 2 / np.log(2.0) if worse.numel() else 1.0
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        _, st = lpf.lpf_anneal(pa, d_img[0], -1, target, d_pairs, torch.from_numpy(log_u).cuda(),
+                               T_max, 0.01 * T_max, max(1, n // 10), max(1, n // 100))
+        dt = time.perf_counter() - t0
+        lpf.lpf_free_paths(pa)
+        return {"proposals": n, "seconds": dt, "proposals_per_s": n / dt, "accepted": st["accepted"],
+                "E_start": E0, "E_end": st["E"], "levels": st["levels"], "T_max": T_max}
+
     r = measure(w, args.steps, args.warmup, True)
     tests_per_step = nominal_tests(w) * world
     value = tests_per_step * args.steps / (r["total_ms"] * 1e-3)
@@ -418,6 +452,7 @@ def main():
                            "ms_per_step": rr["total_ms"] / k, "kernel_ms": rr["kernel_ms"],
                            "roofline_frac": ops / (rr["kernel_ms"] * 1e-3) / peak_ops}
         extra["cfg5"] = measure_swaps()
+        extra["anneal"] = measure_anneal()
         line["other_workloads"] = extra
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         tests, dt, cores, what = oracle_sample(w, r["imgs"], 20)

@@ -497,10 +497,13 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
   const unsigned lt = (1u << lane) - 1u;
   int top = 0;                                             // warp-uniform: items on this warp's stack
 
-  for (int N0 = warp * 32; N0 < n_nodes; N0 += blockDim.x) {
+  // blockIdx.y slices the node range, so that a small batch of proposals still fills the chip
+  const int slice = (n_nodes + gridDim.y - 1) / gridDim.y;
+  const int n_begin = blockIdx.y * slice, n_end = min(n_nodes, n_begin + slice);
+  for (int N0 = n_begin + warp * 32; N0 < n_end; N0 += blockDim.x) {
     const int N = N0 + lane;
     int4 rN = make_int4(0, 0, 0, 0);
-    if (N < n_nodes) rN = __ldg(rec + N);
+    if (N < n_end) rN = __ldg(rec + N);
     const int oNx = (short)(rN.x & 0xffff), oNy = rN.x >> 16;
     const int codeN = (rN.w >> 20) & 15;
     const int d = max(abs(oNx), abs(oNy));                 // depth of N
@@ -514,7 +517,7 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
     const int e0 = 2 * d * mn + nn - 2 * nn * q0;
     for (int q = 0; q < np; ++q) {
       const unsigned nb = s_pass[q].nb;
-      bool alive = (N < n_nodes) && (d == 0 || ((nb >> codeN) & 1u));
+      bool alive = (N < n_end) && (d == 0 || ((nb >> codeN) & 1u));
       if (!__any_sync(0xffffffffu, alive)) continue;       // typical for u: an isolated pixel kills all 32 at once
       const int ox = s_pass[q].ox, oy = s_pass[q].oy;
       const int sx = wrap_coord(s_pass[q].px - oNx, W), sy = wrap_coord(s_pass[q].py - oNy, H);
@@ -705,7 +708,9 @@ cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W
   for (long long c0 = 0; c0 < ctas; c0 += (1ll << 30)) {
     const long long cnt = std::min(ctas - c0, 1ll << 30);
     const long long s0 = c0 * SWAP_SW;
-    swap_delta_kernel_v3<<<(unsigned)cnt, 256, smem, st>>>(bits, H, W, m, pairs + 4 * s0, n - s0, (const int4*)rec,
+    // node slices: about two CTAs per SM in total, at least 256 nodes per slice
+    const int slices = (int)std::max(1ll, std::min<long long>({(2ll * n_sm + cnt - 1) / cnt, (n_nodes + 255) / 256, 65535ll}));
+    swap_delta_kernel_v3<<<dim3((unsigned)cnt, (unsigned)slices), 256, smem, st>>>(bits, H, W, m, pairs + 4 * s0, n - s0, (const int4*)rec,
                                                           n_nodes, delta + s0 * S2);
   }
   long long blocks = std::min<long long>((n * (S2 / 2) + 255) / 256, (long long)n_sm * 16);
