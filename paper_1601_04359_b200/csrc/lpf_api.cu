@@ -370,13 +370,14 @@ extern "C" int lpf_swap_delta(lpf_paths* p, const uint8_t* image, int H, int W, 
   if (n == 0) return LPF_OK;
   DeviceGuard dg(p->device);
   if (!dg.ok) return LPF_E_CUDA;
-  // the base bit image and eight warp stacks of 8 KB live in shared memory; node indices are 24-bit
-  const size_t smem = (size_t)H * ((W + 31) / 32) * 4 + 8 + 8 * 1024 * 8;
+  // the padded base bit image (halo of m pixels) and eight warp stacks of 4 KB live in shared memory; 24-bit node indices
+  const size_t padded_words = (size_t)(H + 2 * p->m) * ((W + 2 * p->m + 31) / 32);
+  const size_t smem = padded_words * 4 + 8 + 8 * 512 * 8;
   if (smem + 2048 > (size_t)p->max_smem || p->n_trie_nodes >= (1 << 24)) return LPF_E_UNSUPPORTED;
   int rc = ensure_swap_table(p);
   if (rc != LPF_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  const size_t bits_bytes = ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32)) * 4;
+  const size_t bits_bytes = ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32) + padded_words) * 4;
   if (bits_bytes > p->swap_bits_bytes) {
     if (p->d_swap_bits) { LPF_CUDA(cudaStreamSynchronize(st)); cudaFree(p->d_swap_bits); p->d_swap_bits = nullptr; }
     p->swap_bits_bytes = 0;

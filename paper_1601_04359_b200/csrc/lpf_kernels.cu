@@ -428,8 +428,32 @@ __global__ void objective_kernel(const long long* __restrict__ counts, const lon
 //   CTA = SW proposals (node records are fetched once for all of them); image bits in shared memory.
 //   delta must be zero on entry; only the canonical half is written (swap_mirror_kernel fills the rest).
 // ---------------------------------------------------------------------------------------------
+// the base bit image with a periodic halo of m pixels on every side: bit (X, Y) of the padded image, X in
+// [0, W + 2m), Y in [0, H + 2m), is pixel ((X - m) mod W, (Y - m) mod H).  One thread per output word.  With it a
+// segment that starts inside the image never needs a modulo.
+__global__ void pack_padded_kernel(const uint32_t* __restrict__ brow, uint32_t* __restrict__ padded, int H, int W,
+                                   int m) {
+  const int Wc = (W + 31) >> 5, PWc = (W + 2 * m + 31) >> 5, PH = H + 2 * m;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < PH * PWc; i += gridDim.x * blockDim.x) {
+    const int Y = i / PWc, wi = i - Y * PWc;
+    int y = (Y - m) % H;
+    y += y < 0 ? H : 0;
+    const uint32_t* srow = brow + (size_t)y * Wc;
+    int x0 = (32 * wi - m) % W;
+    x0 += x0 < 0 ? W : 0;
+    uint32_t word = 0;
+    if (x0 + 32 <= W) word = window32(srow, Wc, x0);
+    else
+      for (int k = 0; k < 32; ++k) {
+        const int xs = (x0 + k) % W;
+        word |= ((srow[xs >> 5] >> (xs & 31)) & 1u) << k;
+      }
+    padded[i] = word;
+  }
+}
+
 constexpr int SWAP_SW = 8;          // proposals per CTA
-constexpr int SWAP_STACK = 1024;    // items per warp stack (8 bytes each)
+constexpr int SWAP_STACK = 512;     // items per warp stack (8 bytes each)
 
 __device__ __forceinline__ int wrap_coord(int x, int n) {
   x += (x < 0) ? n : 0;
@@ -452,13 +476,18 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
   extern __shared__ __align__(16) uint32_t sm[];
   __shared__ SwapPass s_pass[2 * SWAP_SW];
   __shared__ int s_n;
-  const int Wc = (W + 31) >> 5;
+  const int PWc = (W + 2 * m + 31) >> 5, PH = H + 2 * m;                // padded bit image: halo of m pixels all round
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  uint32_t* P = sm;                                                   // [H][Wc] bits of the base image I
-  uint2* stk = (uint2*)(sm + ((H * Wc + 1) & ~1)) + (size_t)warp * SWAP_STACK;
+  uint32_t* P = sm;                                                   // [PH][PWc] bits of the base image I
+  uint2* stk = (uint2*)(sm + ((PH * PWc + 1) & ~1)) + (size_t)warp * SWAP_STACK;
+  // pixel (x, y), x in [-m, W + m), y in [-m, H + m)
+  auto pbit = [&](int x, int y) -> unsigned {
+    const int X = x + m;
+    return (P[(y + m) * PWc + (X >> 5)] >> (X & 31)) & 1u;
+  };
   const int S = 2 * m + 1;
   const long long K = (long long)S * S;
-  for (int i = tid; i < H * Wc; i += blockDim.x) P[i] = bits[i];
+  for (int i = tid; i < PH * PWc; i += blockDim.x) P[i] = bits[i];
   __syncthreads();
   if (tid == 0) {
     int cnt = 0;
@@ -468,7 +497,7 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
       const int xp = pairs[4 * sw], yp = pairs[4 * sw + 1], xq = pairs[4 * sw + 2], yq = pairs[4 * sw + 3];
       const bool ok = xp >= 0 && xp < W && xq >= 0 && xq < W && yp >= 0 && yp < H && yq >= 0 && yq < H;
       if (!ok) continue;
-      const int bp = (P[yp * Wc + (xp >> 5)] >> (xp & 31)) & 1, bq = (P[yq * Wc + (xq >> 5)] >> (xq & 31)) & 1;
+      const int bp = (int)pbit(xp, yp), bq = (int)pbit(xq, yq);
       if (bp == bq) continue;                              // nothing changes for this phase
       const int ux = bp ? xq : xp, uy = bp ? yq : yp;      // bit 0 -> 1
       const int wx = bp ? xp : xq, wy = bp ? yp : yq;      // bit 1 -> 0
@@ -479,7 +508,7 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
         sp.nb = 0;
         for (int code = 0; code < 9; ++code) {
           const int x = wrap_coord(sp.px - (code / 3 - 1), W), y = wrap_coord(sp.py - (code % 3 - 1), H);
-          unsigned bit = (P[y * Wc + (x >> 5)] >> (x & 31)) & 1u;
+          unsigned bit = pbit(x, y);
           if (x == sp.ox && y == sp.oy) bit = 0;
           sp.nb |= bit << code;
         }
@@ -522,17 +551,31 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
       const int ox = s_pass[q].ox, oy = s_pass[q].oy;
       const int sx = wrap_coord(s_pass[q].px - oNx, W), sy = wrap_coord(s_pass[q].py - oNy, H);
       if (alive && d >= 2)                                 // the far end first: a long prefix usually dies at its start
-        alive = ((P[sy * Wc + (sx >> 5)] >> (sx & 31)) & 1u) && !(sx == ox && sy == oy);
+        alive = pbit(sx, sy) && !(sx == ox && sy == oy);
       if (alive) {
         // (A) ancestors at positions d-2 .. 1 (d-1 was the neighbour test, 0 the start), stepping the error term backwards
         int e = e0, qq = q0;
-        for (int k = d - 1; k >= 1; --k) {
-          e -= 2 * mn;
-          if (e < 0) { e += 2 * nn; --qq; }
-          if (k == d - 1) continue;
-          const int ax_ = xmaj ? sxs * k : sxs * qq, ay_ = xmaj ? sys * qq : sys * k;
-          const int x = wrap_coord(sx + ax_, W), y = wrap_coord(sy + ay_, H);
-          if (!((P[y * Wc + (x >> 5)] >> (x & 31)) & 1u) || (x == ox && y == oy)) { alive = false; break; }
+        if (ox < 0) {
+          // fast walk (the w pass on I: nothing to mask): one linear bit index into the padded image, no modulo
+          const int PW = PWc * 32;
+          const int dmaj = xmaj ? sxs : sys * PW, dmin = xmaj ? sys * PW : sxs;
+          int L = (sy + m + oNy) * PW + (sx + m + oNx);      // pixel px itself (position d)
+          for (int k = d - 1; k >= 1; --k) {
+            e -= 2 * mn;
+            L -= dmaj;
+            if (e < 0) { e += 2 * nn; L -= dmin; }
+            if (k == d - 1) continue;
+            if (!((P[L >> 5] >> (L & 31)) & 1u)) { alive = false; break; }
+          }
+        } else {
+          for (int k = d - 1; k >= 1; --k) {
+            e -= 2 * mn;
+            if (e < 0) { e += 2 * nn; --qq; }
+            if (k == d - 1) continue;
+            const int ax_ = xmaj ? sxs * k : sxs * qq, ay_ = xmaj ? sys * qq : sys * k;
+            const int x = wrap_coord(sx + ax_, W), y = wrap_coord(sy + ay_, H);
+            if (!pbit(x, y) || (x == ox && y == oy)) { alive = false; break; }
+          }
         }
       }
       int* const out = out0 + (long long)s_pass[q].slot * K;
@@ -560,7 +603,7 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
           const int4 r = __ldg(rec + i);
           const int isx = (int)(it.y & 0xffff), isy = (int)(it.y >> 16);
           const int x = wrap_coord(isx + (short)(r.x & 0xffff), W), y = wrap_coord(isy + (r.x >> 16), H);
-          const bool in = ((P[y * Wc + (x >> 5)] >> (x & 31)) & 1u) && !(x == s_pass[qi].ox && y == s_pass[qi].oy);
+          const bool in = pbit(x, y) && !(x == s_pass[qi].ox && y == s_pass[qi].oy);
           if (in && (r.w & 0xFFFFF) != 0xFFFFF)
             atomicAdd(out0 + (long long)s_pass[qi].slot * K + (r.w & 0xFFFFF), s_pass[qi].sign);
           p_sib = (r.w >> 24) & 1;
@@ -587,7 +630,7 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
               while (j < end) {
                 const int4 r = __ldg(rec + j);
                 const int x = wrap_coord(isx + (short)(r.x & 0xffff), W), y = wrap_coord(isy + (r.x >> 16), H);
-                const bool in = ((P[y * Wc + (x >> 5)] >> (x & 31)) & 1u) &&
+                const bool in = pbit(x, y) &&
                                 !(x == s_pass[qi].ox && y == s_pass[qi].oy);
                 if (in) {
                   if ((r.w & 0xFFFFF) != 0xFFFFF)
@@ -602,7 +645,7 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
                 cur_top = end;
                 rt = __ldg(rec + cur_top);
                 const int x = wrap_coord(isx + (short)(rt.x & 0xffff), W), y = wrap_coord(isy + (rt.x >> 16), H);
-                const bool in = ((P[y * Wc + (x >> 5)] >> (x & 31)) & 1u) &&
+                const bool in = pbit(x, y) &&
                                 !(x == s_pass[qi].ox && y == s_pass[qi].oy);
                 if (in && (rt.w & 0xFFFFF) != 0xFFFFF)
                   atomicAdd(out0 + (long long)s_pass[qi].slot * K + (rt.w & 0xFFFFF), s_pass[qi].sign);
@@ -696,7 +739,9 @@ cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W
                               long long n, const int32_t* rec, int n_nodes, int* delta, unsigned int* counter,
                               int n_sm, cudaStream_t st) {
   const int Wc = (W + 31) / 32, Hc = (H + 31) / 32;
-  const size_t smem = (size_t)((H * Wc + 1) & ~1) * 4 + (size_t)8 * SWAP_STACK * 8;
+  const int PWc = (W + 2 * m + 31) / 32, PH = H + 2 * m;
+  const size_t smem = (size_t)((PH * PWc + 1) & ~1) * 4 + (size_t)8 * SWAP_STACK * 8;
+  uint32_t* const padded = bits + (size_t)H * Wc + (size_t)W * Hc;
   cudaError_t e = cudaFuncSetAttribute(swap_delta_kernel_v3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   const long long S2 = (long long)(2 * m + 1) * (2 * m + 1);
@@ -704,13 +749,14 @@ cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W
   if (e != cudaSuccess) return e;
   // stage 1 of the bit-pack gives the row-major bit image of the base image (the column-major half is unused)
   pack_base_kernel<<<(unsigned)std::max(1, (Hc * Wc + 7) / 8), 256, 0, st>>>(image, bits, 1, H, W, 1, phase, counter);
+  pack_padded_kernel<<<(unsigned)std::max(1, std::min((PH * PWc + 255) / 256, n_sm * 8)), 256, 0, st>>>(bits, padded, H, W, m);
   const long long ctas = (n + SWAP_SW - 1) / SWAP_SW;
   for (long long c0 = 0; c0 < ctas; c0 += (1ll << 30)) {
     const long long cnt = std::min(ctas - c0, 1ll << 30);
     const long long s0 = c0 * SWAP_SW;
     // node slices: about two CTAs per SM in total, at least 256 nodes per slice
     const int slices = (int)std::max(1ll, std::min<long long>({(2ll * n_sm + cnt - 1) / cnt, (n_nodes + 255) / 256, 65535ll}));
-    swap_delta_kernel_v3<<<dim3((unsigned)cnt, (unsigned)slices), 256, smem, st>>>(bits, H, W, m, pairs + 4 * s0, n - s0, (const int4*)rec,
+    swap_delta_kernel_v3<<<dim3((unsigned)cnt, (unsigned)slices), 256, smem, st>>>(padded, H, W, m, pairs + 4 * s0, n - s0, (const int4*)rec,
                                                           n_nodes, delta + s0 * S2);
   }
   long long blocks = std::min<long long>((n * (S2 / 2) + 255) / 256, (long long)n_sm * 16);
