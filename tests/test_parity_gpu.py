@@ -392,3 +392,23 @@ def test_anneal_limits_and_identity_moves():
     d_img = dev(start)
     counts, st = lpf.lpf_anneal(paths(m), d_img, 1, dev(target), dev(pairs[:0]), dev(log_u[:0]), 1.0, 0.01, 5, 5)
     assert st["steps"] == 0 and np.array_equal(counts.cpu().numpy()[0], orc.counts(start, 1, m))
+
+
+@pytest.mark.parametrize("H,W,m", [(64, 4640, 20), (4640, 40, 33), (1024, 1024, 40)])
+def test_large_and_very_elongated_images(H, W, m):
+    """More than 8 strips of 16 words per row (several strip bands per work item) in the direct and in the
+    transposed views, and a megapixel image; sampled vectors, both phases, all flags."""
+    rng = np.random.default_rng(H + W)
+    img = (rng.random((H, W)) < 0.93).astype(np.uint8)
+    vecs = rng.integers(-m, m + 1, size=(120, 2))
+    vecs[:4] = [(0, 0), (m, m), (-m, m), (m, 0)]
+    for flags in (0, lpf.LPF_PRUNE, lpf.LPF_NO_TRIE, lpf.LPF_S2):
+        both = lpf.lpf_eval_both(paths(m), dev(img[None]), flags).cpu().numpy()[0]
+        for phase in (0, 1):
+            if flags & lpf.LPF_S2:
+                chi = img == phase
+                want = np.array([int((chi & np.roll(chi, (-dy, -dx), axis=(0, 1))).sum()) for dx, dy in vecs])
+            else:
+                want, _ = orc.counts_list(img, phase, vecs)
+            assert np.array_equal(both[phase][vecs[:, 1] + m, vecs[:, 0] + m], want), (flags, phase)
+            assert np.array_equal(both[phase], both[phase][::-1, ::-1])
