@@ -134,7 +134,9 @@ int  lpf_objective(const int64_t* counts, const int64_t* target, int B, int64_t 
  * the bytes of pixels p_i and q_i exchanged.  Only segments through p or q are re-tested.
  *   image dev uint8 [H][W]; pairs dev int32 [n][4] = x_p, y_p, x_q, y_q; delta dev int32 [n][2m+1][2m+1].
  * Pairs are range-checked on the device; an out-of-range pair yields an all-zero delta and the
- * call still returns LPF_OK (no host sync) -- validate on the host if needed. */
+ * call still returns LPF_OK (no host sync) -- validate on the host if needed.
+ * UNSUPPORTED when the bit image with its halo of m pixels, (H+2m) x ceil((W+2m)/32) words, plus 32 KB of warp stacks
+ * does not fit the shared memory of one block, or when the trie has 2^24 nodes or more (m > ~380). */
 int  lpf_swap_delta(lpf_paths* p, const uint8_t* image, int H, int W, int phase,
                     const int32_t* pairs, int64_t n, int32_t* delta, void* stream);
 

@@ -412,3 +412,24 @@ def test_large_and_very_elongated_images(H, W, m):
                 want, _ = orc.counts_list(img, phase, vecs)
             assert np.array_equal(both[phase][vecs[:, 1] + m, vecs[:, 0] + m], want), (flags, phase)
             assert np.array_equal(both[phase], both[phase][::-1, ::-1])
+
+
+def test_maximum_template_m511():
+    """The largest template the library takes (m = 511 = MAX_M, 1023 x 1023 vectors, 4e7 program entries) on a
+    512 x 512 image: sampled vectors against the oracle, Eq. 10 and Eq. 12; m = 512 is refused."""
+    m, H, W = 511, 512, 512
+    img = inputs.gaussian_field(H, W, 12.0, 0.40, inputs.seed_for(3, 7))
+    p = lpf.lpf_build_paths(m, 0)
+    try:
+        got = lpf.lpf_eval(p, dev(img[None]), 1).cpu().numpy()[0]
+    finally:
+        lpf.lpf_free_paths(p)
+    rng = np.random.default_rng(511)
+    vecs = rng.integers(-m, m + 1, size=(200, 2))
+    vecs[:6] = [(0, 0), (m, m), (-m, m), (m, 0), (0, m), (-m, 1)]
+    want, _ = orc.counts_list(img, 1, vecs)
+    assert np.array_equal(got[vecs[:, 1] + m, vecs[:, 0] + m], want)
+    assert got[m, m] == int(img.sum()) and np.array_equal(got, got[::-1, ::-1])
+    with pytest.raises(lpf.LpfError) as ei:
+        lpf.lpf_build_paths(512, 0)
+    assert ei.value.code == lpf.LPF_E_UNSUPPORTED
