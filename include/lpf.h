@@ -55,6 +55,9 @@ extern "C" {
                              (PAPER.md:99); same kernels, a program of 2-pixel "paths".  Exact integers (the paper's
                              FFT form, Eq. 7, is floating point). */
 
+#define LPF_NO_E2    8u   /* measurement: walk every node on the plain bit plane (no eroded plane E2 = row & row >> 1,
+                             DESIGN.md "E2 plane").  Same counts. */
+
 typedef struct lpf_paths lpf_paths;   /* opaque: path table + prefix trie + device programs for one m */
 
 const char* lpf_strerror(int code);
@@ -83,13 +86,16 @@ int  lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, int cap, int
  * (DESIGN.md "Node program").  Every v in D is walked in one of four octant VIEWS of the image (transposed /
  * flipped so that the path is x-major with a' >= 0, 0 <= b' <= a'); each octant has its own prefix trie, cut
  * into connected pieces of about `piece_nodes` nodes (<= 0: one piece per octant); each piece is one item =
- * the chain from the root to the piece root followed by the piece in depth-first order.  flags: 0, LPF_NO_TRIE or LPF_S2.
+ * the chain from the root to the piece root followed by the piece in depth-first order.  flags: 0, LPF_NO_TRIE, LPF_S2, LPF_NO_E2.
  *   entries  host [cap_entries] uint64 (may be NULL to query sizes); low word: bits 0-4 a' & 31, bit 5 reload,
  *            6 terminal, 7 save, 8 restore, 9 init, 10 pair (own mask never needed, next entry is the direct child),
  *            bits 12-31 b' * stride + (a' >> 5); high word: bits 0-19
  *            (dy+m)*(2m+1) + (dx+m) in IMAGE coordinates, 20-23 restore slot, 24-27 save slot
  *   items    host [cap_items][4] int64 = (first entry, number of entries, octant, 0) (may be NULL)
- *   strides  host int[4]: words per packed row of each octant view (decodes b', a' >> 5)
+ *            bit 11 (E2): the entry stands for this node AND its direct child (a'+1, b'), walked on the eroded plane
+ *            whose word offset strides[4+o] is included in bits 12-31; terminal / save / count index are the child's
+ *   strides  host int[8]: [0..3] words per packed row of each octant view (decodes b', a' >> 5), [4..7] word offset
+ *            of the E2 plane of each view in shared memory (0 if the program has no E2 entries)
  * *n_entries / *n_items / *n_slots (mask-stack slots the program needs) are always written.
  * Octants (view coordinates a', b' from image coordinates a, b): 0: dx>=0, dy<=dx (a,b); 1: dx>=0, dy>dx (b,a);
  * 2: dx<0, dy>-dx (b,-a); 3: dx<0, dy<=-dx (-a,b). */

@@ -156,12 +156,13 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   if (B < 1 || H < 1 || W < 1) return LPF_E_INVAL;
   if (n_phase == 1 && phase0 != 0 && phase0 != 1) return LPF_E_INVAL;
   if (p->m > std::min(H, W) - 1) return LPF_E_INVAL;
-  if (flags & ~(LPF_PRUNE | LPF_NO_TRIE | LPF_S2)) return LPF_E_INVAL;
+  if (flags & ~(LPF_PRUNE | LPF_NO_TRIE | LPF_S2 | LPF_NO_E2)) return LPF_E_INVAL;
   DeviceGuard dg(p->device);
   if (!dg.ok) return LPF_E_CUDA;
   cudaStream_t st = (cudaStream_t)stream;
   Geom g;
-  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, &g)) return LPF_E_UNSUPPORTED;
+  const bool use_e2 = !(flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2));     // the E2 plane serves the trie program
+  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, use_e2, &g)) return LPF_E_UNSUPPORTED;
   const int Bpad = (B + g.G - 1) / g.G * g.G;
   long long off = 0;
   int work_per_item = 0;                           // (row band x strip band) pairs summed over the octants / 4
@@ -191,7 +192,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   Program* pr = nullptr;
   for (;; q /= 2) {
     try {
-      pr = &get_program(p, q, flags, g.v[0].stride, g.v[1].stride);
+      pr = &get_program(p, q, flags, g.v[0].stride, g.v[1].stride, g.v[0].e2_band_off, g.v[1].e2_band_off);
     } catch (const std::bad_alloc&) {
       return LPF_E_NOMEM;
     }

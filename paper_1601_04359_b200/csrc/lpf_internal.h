@@ -53,6 +53,9 @@ inline void from_view(int o, int av, int bv, int* a, int* b) {
 //   [ 9] INIT        parent mask is "every valid start pixel" (first entry of a work item / chain)
 //   [10] PAIR        this node's own mask is never needed (not TERMINAL, not SAVE) and the next entry is its
 //                    direct child: the walker fuses both windows into one 3-input AND (M & W1 & W2)
+//   [11] E2          the entry stands for TWO nodes, this one and its direct child (a'+1, b') in the same word column:
+//                    its window is read from the eroded plane E2 = row & (row >> 1), whose word offset is already
+//                    added to `off`; TERMINAL, SAVE and cidx are the child's
 //   [12..31] off     = b' * stride + (a' >> 5), word offset of the window in the packed view
 // high word y:
 //   [ 0..19] cidx    = (dy + m) * (2m + 1) + (dx + m), index into counts[2m+1][2m+1] (image coordinates)
@@ -65,6 +68,7 @@ constexpr uint32_t E_SAVE = 1u << 7;
 constexpr uint32_t E_RESTORE = 1u << 8;
 constexpr uint32_t E_INIT = 1u << 9;
 constexpr uint32_t E_PAIR = 1u << 10;
+constexpr uint32_t E_E2 = 1u << 11;
 constexpr int E_OFF_SHIFT = 12;
 constexpr uint32_t E_CIDX_MASK = (1u << 20) - 1u;
 constexpr int E_RSLOT_SHIFT = 20;
@@ -89,6 +93,7 @@ struct Program {         // one linearisation of the four octant tries for one s
   std::vector<int64_t> items;          // [n_items][4] = first entry, count, octant, 0; sorted by count, descending
   int n_slots = 0;
   int stride[4] = {0, 0, 0, 0};
+  int e2_off[4] = {0, 0, 0, 0};        // word offset of the E2 plane of each view in shared memory (0: none)
   uint64_t* d_entries = nullptr;
   uint32_t* d_skip = nullptr;
   int32_t* d_work = nullptr;           // expanded (item x band) list, see lpf_api.cu
@@ -107,8 +112,8 @@ struct lpf_paths {
   int64_t sum_len = 0;
   int64_t n_trie_nodes = 0;          // distinct prefixes of all P_v, v in D (one trie, image coordinates)
   std::vector<lpf::Node> oct[4];     // per-octant prefix tries in view coordinates; [0] = root (0,0)
-  // key: (piece_nodes, flags & LPF_NO_TRIE, stride0, stride1)   (stride2 = stride1, stride3 = stride0)
-  std::map<std::tuple<int, unsigned, int, int>, lpf::Program> programs;
+  // key: (piece_nodes, program kind, stride0, stride1, E2 offset 0, E2 offset 1)   (views 3, 2 as views 0, 1)
+  std::map<std::tuple<int, unsigned, int, int, int, int>, lpf::Program> programs;
   // device workspace (grown on demand)
   uint32_t* d_packed = nullptr;
   size_t packed_bytes = 0;
@@ -141,6 +146,7 @@ inline bool in_half(int dx, int dy) { return dy > 0 || (dy == 0 && dx >= 0); }
 void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec);
 
 // builds (or returns the cached) program for (piece_nodes, flags, view strides); host side only
-Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride01, int stride12);
+Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int e2off03,
+                     int e2off12);
 
 }  // namespace lpf

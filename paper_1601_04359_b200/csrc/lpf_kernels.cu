@@ -75,6 +75,29 @@ __device__ __forceinline__ uint32_t window32(const uint32_t* __restrict__ row, i
   return __funnelshift_r(lo, hi, xs & 31);
 }
 
+// word i of one view row: 32 view pixels x' = (32 i + k) mod Wv read from the source row (views 0-2 in order, view 3
+// mirrored: bit k = source pixel (Wv - x') mod Wv)
+__device__ __forceinline__ uint32_t view_word(const uint32_t* __restrict__ srow, int words, int o, int Wv, int i) {
+  const int x0 = (32 * i) % Wv;
+  uint32_t word = 0;
+  if (o != 3) {
+    if (x0 + 32 <= Wv) return window32(srow, words, x0);
+    for (int k = 0; k < 32; ++k) {
+      const int xs = (x0 + k) % Wv;
+      word |= ((srow[xs >> 5] >> (xs & 31)) & 1u) << k;
+    }
+  } else {
+    // for 1 <= x0 and x0 + 31 <= Wv the sources are the 32 consecutive pixels Wv - x0 - 31 .. Wv - x0, descending
+    if (x0 >= 1 && x0 + 31 <= Wv) return __brev(window32(srow, words, Wv - x0 - 31));
+    for (int k = 0; k < 32; ++k) {
+      const int xv = (x0 + k) % Wv;
+      const int xs = xv ? Wv - xv : 0;
+      word |= ((srow[xs >> 5] >> (xs & 31)) & 1u) << k;
+    }
+  }
+  return word;
+}
+
 // ---------------------------------------------------------------------------------------------
 // bit-pack, stage 2: the four octant views with their periodic halo, one thread per output word.
 //   view o of image I (lpf_internal.h): 0: I[y'][x']  1: I[x'][y']  2: I[x'][-y' mod W]  3: I[y'][-x' mod W]
@@ -99,12 +122,14 @@ __global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restr
     const long long rem = wp - v.packed_off;
     const int b = (int)(rem / v.view_words);
     const int idx = (int)(rem - (long long)b * v.view_words);
-    const int r = idx / v.stride, i = idx - r * v.stride;
+    // plain view first, then (if enabled) the eroded view E2 = word & (word >> 1 across the word boundary)
+    const bool e2 = v.e2_view_off > 0 && idx >= v.e2_view_off;
+    const int idx1 = e2 ? idx - v.e2_view_off : idx;
+    const int r = idx1 / v.stride, i = idx1 - r * v.stride;
     const int rows = v.n_bands * g.band_rows + g.m;
     uint32_t word = 0;
     if (b < B && r < rows) {
       const int yv = r % v.Hv;
-      const int x0 = (32 * i) % v.Wv;
       const uint32_t* bimg = base + ((size_t)plane * B + b) * img_words;
       // source row of this view row: views 0, 3: image row yv (Brow); view 1: image column yv; view 2: column -yv
       const uint32_t* srow;
@@ -115,23 +140,10 @@ __global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restr
         srow = bimg + (size_t)g.H * Wc + (size_t)c * Hc;
         words = Hc;
       }
-      if (o != 3) {
-        if (x0 + 32 <= v.Wv) word = window32(srow, words, x0);
-        else
-          for (int k = 0; k < 32; ++k) {
-            const int xs = (x0 + k) % v.Wv;
-            word |= ((srow[xs >> 5] >> (xs & 31)) & 1u) << k;
-          }
-      } else {
-        // bit k = source bit (Wv - x0 - k) mod Wv: for 1 <= x0 and x0 + 31 <= Wv the sources are the 32
-        // consecutive pixels Wv - x0 - 31 .. Wv - x0 in descending order
-        if (x0 >= 1 && x0 + 31 <= v.Wv) word = __brev(window32(srow, words, v.Wv - x0 - 31));
-        else
-          for (int k = 0; k < 32; ++k) {
-            const int xv = (x0 + k) % v.Wv;
-            const int xs = xv ? v.Wv - xv : 0;
-            word |= ((srow[xs >> 5] >> (xs & 31)) & 1u) << k;
-          }
+      word = view_word(srow, words, o, v.Wv, i);
+      if (e2) {
+        const uint32_t next = (i + 1 < v.stride) ? view_word(srow, words, o, v.Wv, i + 1) : 0u;
+        word &= __funnelshift_r(word, next, 1);
       }
     }
     packed[w] = word;
@@ -231,17 +243,21 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
     const int stride = v.stride;
     if (tid == 0) {
       const unsigned bytes = (unsigned)v.band_words * 4u;
-      mbar_expect_tx(&bar, bytes * (unsigned)g.G);
+      mbar_expect_tx(&bar, bytes * (unsigned)g.G * (v.e2_band_off ? 2u : 1u));
       const uint32_t* src = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b0 * v.view_words +
                             (size_t)band * g.band_rows * stride;
-      for (int gi = 0; gi < g.G; ++gi)
-        tma_bulk_g2s(smem + (size_t)gi * v.band_words, src + (size_t)gi * v.view_words, bytes, &bar);
+      for (int gi = 0; gi < g.G; ++gi) {
+        tma_bulk_g2s(smem + (size_t)gi * v.band_pitch, src + (size_t)gi * v.view_words, bytes, &bar);
+        if (v.e2_band_off)          // the eroded plane E2 of the same band, right behind the plain one
+          tma_bulk_g2s(smem + (size_t)gi * v.band_pitch + v.e2_band_off,
+                       src + (size_t)gi * v.view_words + v.e2_view_off, bytes, &bar);
+      }
     }
     // per-item thread geometry (the octant decides the view size)
     const int strip = sband * g.SB + strip_l;
     const bool active = strip < v.n_strips;
     const char* base =
-        (const char*)(smem + (size_t)img_local * v.band_words + row0 * stride + (active ? strip : 0) * TX);
+        (const char*)(smem + (size_t)img_local * v.band_pitch + row0 * stride + (active ? strip : 0) * TX);
     const int rowstep = 32 * stride * 4;                     // bytes between the TY start rows of a thread
     const int b_img = b0 + img_local;
     unsigned long long* cnt = p.counts + ((size_t)b_img * p.n_phase + plane) * (size_t)p.S * p.S;

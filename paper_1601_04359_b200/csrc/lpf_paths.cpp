@@ -142,36 +142,62 @@ void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec) {
 
 // ---- program emission ----------------------------------------------------------------------
 
+struct Held {            // the row strip that is in the registers when an entry runs
+  int b = -1, col = -1, plane = -1;
+};
+
 struct Emitter {
   int m, o, stride;
+  int e2_off;                           // word offset of the E2 plane of this view in shared memory (0: no E2 plane)
   const std::vector<Node>& nd;
   const std::vector<uint8_t>& cut;      // node is the root of a piece
   const std::vector<int32_t>& psize;    // nodes of the subtree that stay in the node's own piece
   Program& out;
   int max_slots = 0;
 
-  // prev: the node whose row strip is in the registers when this entry runs (-1: none)
-  uint64_t entry(int node, uint32_t flags, int prev, int rslot, int sslot) const {
-    const int a = nd[node].a, b = nd[node].b;      // view coordinates: a >= 0, 0 <= b <= a
+  // `head` and its direct child in the same row and word column can be walked as ONE entry on the eroded plane
+  // E2 = row & (row >> 1): the window of E2 at head's shift is the AND of the two windows
+  bool mergeable(int head, int child) const {
+    return e2_off > 0 && nd[head].b == nd[child].b && (nd[head].a >> 5) == (nd[child].a >> 5);
+  }
+
+  // one entry: the window of `head` (on the E2 plane if e2: then it also covers head's child `tail`); TERMINAL / SAVE
+  // and the count index are those of `tail`.  *held is updated to what the entry leaves in the registers.
+  uint64_t entry(int head, int tail, bool e2, uint32_t flags, Held* held, int rslot, int sslot) const {
+    const int a = nd[head].a, b = nd[head].b;      // view coordinates: a >= 0, 0 <= b <= a
     const bool direct = !(flags & (E_RESTORE | E_INIT));
-    if (!direct || prev < 0 || nd[prev].b != b || (nd[prev].a >> 5) != (a >> 5)) flags |= E_RELOAD;
-    const uint32_t off = (uint32_t)(b * stride + (a >> 5));
-    const uint32_t x = (uint32_t)(a & 31) | flags | (off << E_OFF_SHIFT);
+    const int plane = e2 ? 1 : 0;
+    if (!direct || held->b != b || held->col != (a >> 5) || held->plane != plane) flags |= E_RELOAD;
+    held->b = b; held->col = a >> 5; held->plane = plane;
+    const uint32_t off = (uint32_t)(b * stride + (a >> 5) + (e2 ? e2_off : 0));
+    const uint32_t x = (uint32_t)(a & 31) | flags | (e2 ? E_E2 : 0u) | (off << E_OFF_SHIFT);
     int ia, ib;
-    from_view(o, a, b, &ia, &ib);
+    from_view(o, nd[tail].a, nd[tail].b, &ia, &ib);
     const uint32_t cidx = (uint32_t)((ib + m) * (2 * m + 1) + (ia + m));
     const uint32_t y = cidx | ((uint32_t)rslot << E_RSLOT_SHIFT) | ((uint32_t)sslot << E_SSLOT_SHIFT);
     return (uint64_t)x | ((uint64_t)y << 32);
   }
 
-  // emits `node` and the part of its subtree inside the piece. src: 0 direct, 1 restore(rslot), 2 init.
-  void emit(int node, int src, int rslot, int depth_slots, bool count_it) {
-    std::vector<int> kids;
+  void kids_of(int node, std::vector<int>* kids) const {
+    kids->clear();
     for (int c = nd[node].first_child; c >= 0; c = nd[c].next_sibling)
-      if (!cut[c]) kids.push_back(c);
+      if (!cut[c]) kids->push_back(c);
     // heaviest child last: its descent frees the slot, so live slots <= log2(piece size) + 1
-    std::stable_sort(kids.begin(), kids.end(), [&](int x, int y) { return psize[x] < psize[y]; });
-    uint32_t flags = (nd[node].terminal && count_it) ? E_TERMINAL : 0u;
+    std::stable_sort(kids->begin(), kids->end(), [&](int x, int y) { return psize[x] < psize[y]; });
+  }
+
+  // emits `node` and the part of its subtree inside the piece. src: 0 direct, 1 restore(rslot), 2 init.
+  void emit(int node, int src, int rslot, int depth_slots, bool count_it, Held held) {
+    std::vector<int> kids;
+    kids_of(node, &kids);
+    int tail = node;
+    bool term = nd[node].terminal && count_it;
+    if (kids.size() == 1 && !term && mergeable(node, kids[0])) {   // node's own mask is never needed: fold the child in
+      tail = kids[0];
+      term = nd[tail].terminal;
+      kids_of(tail, &kids);
+    }
+    uint32_t flags = term ? E_TERMINAL : 0u;
     if (src == 1) flags |= E_RESTORE;
     if (src == 2) flags |= E_INIT;
     int sslot = 0;
@@ -181,17 +207,17 @@ struct Emitter {
       max_slots = std::max(max_slots, depth_slots + 1);
     }
     const size_t at = out.entries.size();
-    out.entries.push_back(entry(node, flags, nd[node].parent, rslot, sslot));
+    out.entries.push_back(entry(node, tail, tail != node, flags, &held, rslot, sslot));
     out.skip.push_back(0);
     for (size_t i = 0; i < kids.size(); ++i) {
       if (kids.size() == 1) {
-        emit(kids[i], 0, 0, depth_slots, true);
+        emit(kids[i], 0, 0, depth_slots, true, held);
       } else if (i == 0) {
-        emit(kids[i], 0, 0, depth_slots + 1, true);
+        emit(kids[i], 0, 0, depth_slots + 1, true, held);
       } else if (i + 1 < kids.size()) {
-        emit(kids[i], 1, sslot, depth_slots + 1, true);
+        emit(kids[i], 1, sslot, depth_slots + 1, true, held);
       } else {
-        emit(kids[i], 1, sslot, depth_slots, true);      // last child: the slot is free again
+        emit(kids[i], 1, sslot, depth_slots, true, held);      // last child: the slot is free again
       }
     }
     out.skip[at] = (uint32_t)(out.entries.size() - at - 1);
@@ -238,7 +264,7 @@ static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
       else psize[nd[i].parent] += psize[i];
     }
     cut[0] = 1;
-    Emitter em{p->m, o, pr.stride[o], nd, cut, psize, pr};
+    Emitter em{p->m, o, pr.stride[o], pr.e2_off[o], nd, cut, psize, pr};
     std::vector<int> chain;
     for (int r = 0; r < N; ++r) {
       if (!cut[r]) continue;
@@ -248,11 +274,14 @@ static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
       chain.clear();
       for (int u = nd[r].parent; u >= 0; u = nd[u].parent) chain.push_back(u);
       std::reverse(chain.begin(), chain.end());
-      for (size_t i = 0; i < chain.size(); ++i) {
-        pr.entries.push_back(em.entry(chain[i], i == 0 ? E_INIT : 0u, i == 0 ? -1 : chain[i - 1], 0, 0));
+      Held held;
+      for (size_t i = 0; i < chain.size();) {
+        const bool e2 = i + 1 < chain.size() && em.mergeable(chain[i], chain[i + 1]);
+        pr.entries.push_back(em.entry(chain[i], e2 ? chain[i + 1] : chain[i], e2, i == 0 ? E_INIT : 0u, &held, 0, 0));
         pr.skip.push_back(0);
+        i += e2 ? 2 : 1;
       }
-      em.emit(r, chain.empty() ? 2 : 0, 0, 0, !(r == 0 && o != 0));
+      em.emit(r, chain.empty() ? 2 : 0, 0, 0, !(r == 0 && o != 0), held);
       push_item(pr, first, o);
     }
     pr.n_slots = std::max(pr.n_slots, em.max_slots);
@@ -347,15 +376,19 @@ static void build_s2_program(lpf_paths* p, int piece_nodes, Program& pr) {
   sort_items(pr);
 }
 
-Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12) {
+Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int e2off03,
+                     int e2off12) {
   if (piece_nodes < 0) piece_nodes = 0;
   const unsigned kind = (flags & LPF_S2) ? LPF_S2 : (flags & LPF_NO_TRIE);
-  const std::tuple<int, unsigned, int, int> key(piece_nodes, kind, stride03, stride12);
+  if (kind != 0) e2off03 = e2off12 = 0;                    // the E2 plane serves the trie program only
+  const std::tuple<int, unsigned, int, int, int, int> key(piece_nodes, kind, stride03, stride12, e2off03, e2off12);
   auto it = p->programs.find(key);
   if (it != p->programs.end()) return it->second;
   Program& pr = p->programs[key];
   pr.stride[0] = pr.stride[3] = stride03;
   pr.stride[1] = pr.stride[2] = stride12;
+  pr.e2_off[0] = pr.e2_off[3] = e2off03;
+  pr.e2_off[1] = pr.e2_off[2] = e2off12;
   if (flags & LPF_S2) build_s2_program(p, piece_nodes, pr);
   else if (flags & LPF_NO_TRIE) build_chain_program(p, piece_nodes, pr);
   else build_trie_program(p, piece_nodes, pr);
@@ -379,7 +412,7 @@ int build_host_table(lpf_paths* p) {
 
 namespace lpf {
 
-bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, Geom* out) {
+bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2, Geom* out) {
   Geom g;
   std::memset(&g, 0, sizeof(g));
   g.H = H; g.W = W; g.m = m;
@@ -417,8 +450,12 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int c
       ViewGeom& v = g.v[o];
       v.n_bands = (v.Hv + g.band_rows - 1) / g.band_rows;
       v.band_words = ((g.band_rows + m) * v.stride + 3) / 4 * 4;
-      v.view_words = ((v.n_bands * g.band_rows + m) * v.stride + 3) / 4 * 4 + 4;
-      bw_max = std::max(bw_max, v.band_words);
+      const int plain_view = ((v.n_bands * g.band_rows + m) * v.stride + 3) / 4 * 4 + 4;
+      v.band_pitch = use_e2 ? 2 * v.band_words : v.band_words;
+      v.e2_band_off = use_e2 ? v.band_words : 0;
+      v.view_words = use_e2 ? 2 * plain_view : plain_view;
+      v.e2_view_off = use_e2 ? plain_view : 0;
+      bw_max = std::max(bw_max, v.band_pitch);
     }
     const size_t per_image = (size_t)bw_max * 4;     // shared memory holds the G bands only
     if (per_image + 1024 <= (size_t)max_smem) {
@@ -494,14 +531,16 @@ extern "C" int lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, un
   if (!p || !n_entries || !n_items || !n_slots || !strides) return LPF_E_INVAL;
   if (H < 1 || W < 1 || p->m > std::min(H, W) - 1) return LPF_E_INVAL;
   lpf::Geom g;
-  if (!lpf::choose_geom(p->m, H, W, 1, p->max_smem > 0 ? p->max_smem : 232448, p->tile_tx, p->tile_ty, p->cta_warps, &g))
+  if (!lpf::choose_geom(p->m, H, W, 1, p->max_smem > 0 ? p->max_smem : 232448, p->tile_tx, p->tile_ty, p->cta_warps,
+                        !(flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)), &g))
     return LPF_E_UNSUPPORTED;
   try {
-    lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride);
+    lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride, g.v[0].e2_band_off,
+                                        g.v[1].e2_band_off);
     *n_entries = (int64_t)pr.entries.size();
     *n_items = (int64_t)pr.items.size() / 4;
     *n_slots = pr.n_slots;
-    for (int o = 0; o < 4; ++o) strides[o] = pr.stride[o];
+    for (int o = 0; o < 4; ++o) { strides[o] = pr.stride[o]; strides[4 + o] = pr.e2_off[o]; }
     if (entries) {
       if (cap_entries < *n_entries) return LPF_E_INVAL;
       std::memcpy(entries, pr.entries.data(), sizeof(uint64_t) * pr.entries.size());

@@ -15,7 +15,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "liblpf.so")
 
 LPF_OK, LPF_E_INVAL, LPF_E_NOMEM, LPF_E_CUDA, LPF_E_UNSUPPORTED = 0, -1, -2, -3, -4
-LPF_PRUNE, LPF_NO_TRIE, LPF_S2 = 1, 2, 4
+LPF_PRUNE, LPF_NO_TRIE, LPF_S2, LPF_NO_E2 = 1, 2, 4, 8
 
 EXPORTS = (
     "lpf_strerror", "lpf_last_cuda_error", "lpf_build_paths", "lpf_free_paths", "lpf_paths_info",
@@ -152,10 +152,11 @@ def lpf_paths_get(p: Paths, dx: int, dy: int) -> np.ndarray:
 
 
 def lpf_paths_program(p: Paths, H: int, W: int, piece_nodes: int = 0, flags: int = 0):
-    """(entries uint64 [n], items int64 [k, 4], n_slots, strides [4]) of the linearised walk program."""
+    """(entries uint64 [n], items int64 [k, 4], n_slots, strides [8]: row strides of the 4 views, then their E2 plane
+    word offsets) of the linearised walk program."""
     lib = load()
     ne, ni, ns = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int()
-    strides = (ctypes.c_int * 4)()
+    strides = (ctypes.c_int * 8)()
     _check(lib.lpf_paths_program(p.handle, int(H), int(W), int(piece_nodes), int(flags), None, 0, ctypes.byref(ne),
                                  None, 0, ctypes.byref(ni), ctypes.byref(ns), strides), "lpf_paths_program")
     entries = np.zeros(ne.value, dtype=np.uint64)

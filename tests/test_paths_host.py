@@ -94,7 +94,7 @@ def _decode(entries):
     x = (entries & np.uint64(0xffffffff)).astype(np.int64)
     y = (entries >> np.uint64(32)).astype(np.int64)
     return dict(sh=x & 31, reload=(x >> 5) & 1, terminal=(x >> 6) & 1, save=(x >> 7) & 1, restore=(x >> 8) & 1,
-                init=(x >> 9) & 1, pair=(x >> 10) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 15, sslot=(y >> 24) & 15)
+                init=(x >> 9) & 1, pair=(x >> 10) & 1, e2=(x >> 11) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 15, sslot=(y >> 24) & 15)
 
 
 def _from_view(o, a, b):
@@ -104,7 +104,8 @@ def _from_view(o, a, b):
 
 @pytest.mark.parametrize("m,H,W,piece,flags", [(5, 8, 8, 0, 0), (12, 40, 100, 16, 0), (33, 64, 64, 256, 0),
                                                (70, 300, 128, 512, 0), (12, 13, 13, 0, lpf.LPF_NO_TRIE),
-                                               (12, 64, 32, 64, lpf.LPF_NO_TRIE)])
+                                               (12, 64, 32, 64, lpf.LPF_NO_TRIE), (33, 64, 64, 256, lpf.LPF_NO_E2),
+                                               (40, 41, 97, 64, lpf.LPF_NO_E2)])
 def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags):
     """Interpret the node program on the host with a stack of pixel lists instead of masks:
     every terminal must be reached exactly once with exactly the pixel list P_v, and the row-strip
@@ -127,13 +128,19 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
             elif d["restore"][e]:
                 cur = list(stack[int(d["rslot"][e])])
             assert cur is not None
-            bv, col = divmod(int(d["off"][e]), strides[o])
+            e2 = bool(d["e2"][e])
+            if e2:
+                assert strides[4 + o] > 0 and not (flags & (lpf.LPF_NO_E2 | lpf.LPF_NO_TRIE))
+            bv, col = divmod(int(d["off"][e]) - (strides[4 + o] if e2 else 0), strides[o])
             av = col * 32 + int(d["sh"][e])
             assert 0 <= bv <= av <= m
             if d["reload"][e]:
-                held = (bv, col)
-            assert held == (bv, col), "stale row strip"
+                held = (bv, col, e2)
+            assert held == (bv, col, e2), "stale row strip"
             cur = cur + [_from_view(o, av, bv)]
+            if e2:                                           # the entry also stands for the child (a'+1, b'), same word
+                assert (av + 1) >> 5 == col and av + 1 <= m
+                cur = cur + [_from_view(o, av + 1, bv)]
             if d["terminal"][e]:
                 cidx = int(d["cidx"][e])
                 dy, dx = cidx // S - m, cidx % S - m
@@ -149,6 +156,8 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
             assert bool(d["pair"][e]) == bool(want_pair)
     assert covered.all()
     assert len(seen) == 2 * m * m + 2 * m + 1
+    if not (flags & (lpf.LPF_NO_E2 | lpf.LPF_NO_TRIE)):
+        assert d["e2"].sum() > len(entries) // 8            # the eroded plane really carries a share of the nodes
     for (dx, dy), pix in seen.items():
         assert orc.in_half(dx, dy)
         assert pix == [tuple(int(t) for t in r) for r in orc.path(dx, dy)], (dx, dy)
