@@ -412,7 +412,29 @@ int build_host_table(lpf_paths* p) {
 
 namespace lpf {
 
+static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2,
+                              Geom* out);
+
 bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2, Geom* out) {
+  if (cta_warps >= 1 && cta_warps <= 8) return choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cta_warps, use_e2, out);
+  // automatic CTA size: the one that keeps the most warps resident per SM (shared memory is the limiter: a CTA of
+  // several small images needs the same bytes per warp whatever its size, so smaller CTAs quantise better)
+  int best_warps = -1;
+  for (int cw = 8; cw >= 2; cw /= 2) {
+    Geom g;
+    if (!choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cw, use_e2, &g)) continue;
+    const int per_sm = std::min(32, (max_smem + 1024) / (g.smem_bytes + 1024));
+    const int warps = std::min(64, per_sm * (g.threads / 32));
+    if (warps > best_warps + best_warps / 8) {         // a smaller CTA must win by more than 12 %
+      best_warps = warps;
+      *out = g;
+    }
+  }
+  return best_warps > 0;
+}
+
+static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2,
+                              Geom* out) {
   Geom g;
   std::memset(&g, 0, sizeof(g));
   g.H = H; g.W = W; g.m = m;
