@@ -415,22 +415,42 @@ namespace lpf {
 static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2,
                               Geom* out);
 
-bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2, Geom* out) {
+static int resident_warps(const Geom& g, int max_smem) {
+  const int per_sm = std::min(32, (max_smem + 1024) / (g.smem_bytes + 1024));
+  return std::min(64, per_sm * (g.threads / 32));
+}
+
+// one plane layout (with or without E2); automatic CTA size: the one that keeps the most warps resident per SM
+// (shared memory is the limiter: a CTA of several small images needs the same bytes per warp whatever its size, so
+// smaller CTAs quantise better)
+static bool choose_geom_plane(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2,
+                              Geom* out) {
   if (cta_warps >= 1 && cta_warps <= 8) return choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cta_warps, use_e2, out);
-  // automatic CTA size: the one that keeps the most warps resident per SM (shared memory is the limiter: a CTA of
-  // several small images needs the same bytes per warp whatever its size, so smaller CTAs quantise better)
   int best_warps = -1;
   for (int cw = 8; cw >= 2; cw /= 2) {
     Geom g;
     if (!choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cw, use_e2, &g)) continue;
-    const int per_sm = std::min(32, (max_smem + 1024) / (g.smem_bytes + 1024));
-    const int warps = std::min(64, per_sm * (g.threads / 32));
+    const int warps = resident_warps(g, max_smem);
     if (warps > best_warps + best_warps / 8) {         // a smaller CTA must win by more than 12 %
       best_warps = warps;
       *out = g;
     }
   }
   return best_warps > 0;
+}
+
+// use_e2 = "the E2 plane is allowed": it doubles the shared memory of a band, which pays (measured, DESIGN.md "E2
+// plane") as long as at least 12 warps stay resident per SM; templates that are large against the image (m close to
+// H: the halo dominates the band) fall back to the plain plane.
+bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2, Geom* out) {
+  if (use_e2) {
+    Geom g;
+    if (choose_geom_plane(m, H, W, B, max_smem, tx, ty, cta_warps, true, &g) && resident_warps(g, max_smem) >= 12) {
+      *out = g;
+      return true;
+    }
+  }
+  return choose_geom_plane(m, H, W, B, max_smem, tx, ty, cta_warps, false, out);
 }
 
 static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2,
