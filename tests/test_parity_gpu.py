@@ -433,3 +433,27 @@ def test_maximum_template_m511():
     with pytest.raises(lpf.LpfError) as ei:
         lpf.lpf_build_paths(512, 0)
     assert ei.value.code == lpf.LPF_E_UNSUPPORTED
+
+
+def test_hypothesis_generated_small_cases():
+    """Random small shapes, template sizes, fill fractions, batch sizes and flags (hypothesis, derandomised):
+    full-template bit-exact parity of lpf_eval / lpf_eval_both with the oracle."""
+    from hypothesis import given, settings, strategies as st
+
+    @settings(max_examples=250, deadline=None, derandomize=True)
+    @given(st.integers(1, 48), st.integers(1, 70), st.floats(0.05, 0.98), st.integers(0, 2 ** 31 - 1),
+           st.sampled_from([0, lpf.LPF_PRUNE, lpf.LPF_NO_TRIE, lpf.LPF_NO_E2, lpf.LPF_PRUNE | lpf.LPF_NO_E2]),
+           st.integers(1, 3), st.data())
+    def check(H, W, fill, seed, flags, B, data):
+        m = data.draw(st.integers(0, min(H, W) - 1))
+        rng = np.random.default_rng(seed)
+        imgs = (rng.random((B, H, W)) < fill).astype(np.uint8)
+        both = lpf.lpf_eval_both(paths(m), dev(imgs), flags).cpu().numpy()
+        one = lpf.lpf_eval(paths(m), dev(imgs), 1, flags).cpu().numpy()
+        for b in range(B):
+            for phase in (0, 1):
+                want = orc.counts(imgs[b], phase, m, full_template=(H * W <= 600))
+                assert np.array_equal(both[b, phase], want), (H, W, m, flags, b, phase)
+            assert np.array_equal(one[b], both[b, 1])
+
+    check()
