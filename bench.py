@@ -115,7 +115,7 @@ def oracle_sample(w, imgs, seconds_hint, rng_seed=0, n_vec=None):
     t0 = time.perf_counter()
     cores = 1
     for phase in ((0, 1) if w["n_phase"] == 2 else (1,)):
-        _, cores = orc.counts_list(img, phase, vecs)
+        _, cores = orc.counts_list(img, phase, vecs, threads=os.cpu_count() or 1)   # all host cores, whatever OMP_NUM_THREADS torchrun set
     dt = time.perf_counter() - t0
     tests = n_vec * w["H"] * w["W"] * w["n_phase"]
     what = "%d random template vectors x all %dx%d start pixels x %d phase(s) of image 0" % (
