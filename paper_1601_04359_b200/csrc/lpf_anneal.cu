@@ -192,8 +192,8 @@ extern "C" int lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase,
     K = std::min(K, K_max);
     for (int rep = 0; rep < 8 && rc == LPF_OK && e == cudaSuccess; ++rep) {
       anneal_gather_kernel<<<(K + 63) / 64, 64, 0, st>>>(pairs, N, d_state, d_batch, K);
-      for (int i = 0; i < n_ph && rc == LPF_OK; ++i)             // Q = modify(P), SDQ = evaluate(Q): lines 9-10
-        rc = lpf_swap_delta(p, image, H, W, phase < 0 ? i : phase, d_batch, K, d_delta + i * ph_stride, stream);
+      // Q = modify(P), SDQ = evaluate(Q): lines 9-10 (both phases in one pass over the trie if asked)
+      rc = swap_delta_impl(p, image, H, W, phase, d_batch, K, d_delta, ph_stride, stream);
       if (rc != LPF_OK) break;
       anneal_de_kernel<<<K, 256, 0, st>>>(d_delta, ph_stride, (const long long*)counts, (const long long*)target, S,
                                           n_ph, d_dE);

@@ -146,8 +146,8 @@ cudaError_t launch_mirror(unsigned long long* counts, int S, long long n_arrays,
 cudaError_t launch_objective(const long long* counts, const long long* target, int B, long long K,
                              unsigned long long* sse, int n_sm, cudaStream_t st);
 cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W, int m, int phase, const int* pairs,
-                              long long n, const int32_t* rec, int n_nodes, int* delta, unsigned int* counter,
-                              int n_sm, cudaStream_t st);
+                              long long n, const int32_t* rec, int n_nodes, int* delta, long long plane_stride,
+                              unsigned int* counter, int n_sm, cudaStream_t st);
 
 static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, int n_phase, int phase0,
                      int64_t* counts, unsigned flags, void* stream, const uint8_t* start_mask = nullptr) {
@@ -362,23 +362,29 @@ static int ensure_swap_table(lpf_paths* p) {
 
 }  // namespace lpf
 
-extern "C" int lpf_swap_delta(lpf_paths* p, const uint8_t* image, int H, int W, int phase, const int32_t* pairs,
-                              int64_t n, int32_t* delta, void* stream) {
+namespace lpf {
+
+// phase 0 | 1: delta [n][S][S] of that phase;  phase < 0: both phases in one pass over the trie, phase k written at
+// delta + k * plane_stride (used by lpf_anneal)
+int swap_delta_impl(lpf_paths* p, const uint8_t* image, int H, int W, int phase, const int32_t* pairs, int64_t n,
+                    int32_t* delta, int64_t plane_stride, void* stream) {
   if (!p || !image || !pairs || !delta) return LPF_E_INVAL;
   if (p->device < 0 || H < 1 || W < 1 || n < 0) return LPF_E_INVAL;
-  if (phase != 0 && phase != 1) return LPF_E_INVAL;
+  if (phase < -1 || phase > 1) return LPF_E_INVAL;
   if (p->m > std::min(H, W) - 1) return LPF_E_INVAL;
   if (n == 0) return LPF_OK;
   DeviceGuard dg(p->device);
   if (!dg.ok) return LPF_E_CUDA;
-  // the padded base bit image (halo of m pixels) and eight warp stacks of 4 KB live in shared memory; 24-bit node indices
-  const size_t padded_words = (size_t)(H + 2 * p->m) * ((W + 2 * p->m + 31) / 32);
+  const int n_planes = phase < 0 ? 2 : 1;
+  // the padded base bit image(s) (halo of m pixels) and eight warp stacks of 4 KB live in shared memory; 24-bit node indices
+  const size_t padded_words = (size_t)n_planes * (H + 2 * p->m) * ((W + 2 * p->m + 31) / 32);
   const size_t smem = padded_words * 4 + 8 + 8 * 512 * 8;
   if (smem + 2048 > (size_t)p->max_smem || p->n_trie_nodes >= (1 << 24)) return LPF_E_UNSUPPORTED;
   int rc = ensure_swap_table(p);
   if (rc != LPF_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  const size_t bits_bytes = ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32) + padded_words) * 4;
+  const size_t bits_bytes =
+      (n_planes * ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32)) + padded_words) * 4;
   if (bits_bytes > p->swap_bits_bytes) {
     if (p->d_swap_bits) { LPF_CUDA(cudaStreamSynchronize(st)); cudaFree(p->d_swap_bits); p->d_swap_bits = nullptr; }
     p->swap_bits_bytes = 0;
@@ -386,8 +392,16 @@ extern "C" int lpf_swap_delta(lpf_paths* p, const uint8_t* image, int H, int W, 
     p->swap_bits_bytes = bits_bytes;
   }
   LPF_CUDA(launch_swap_delta(image, p->d_swap_bits, H, W, p->m, phase, pairs, (long long)n, p->d_swap_rec,
-                             (int)p->n_trie_nodes, delta, p->d_counter + 1, p->n_sm, st));
+                             (int)p->n_trie_nodes, delta, (long long)plane_stride, p->d_counter + 1, p->n_sm, st));
   return LPF_OK;
+}
+
+}  // namespace lpf
+
+extern "C" int lpf_swap_delta(lpf_paths* p, const uint8_t* image, int H, int W, int phase, const int32_t* pairs,
+                              int64_t n, int32_t* delta, void* stream) {
+  if (phase != 0 && phase != 1) return LPF_E_INVAL;
+  return lpf::swap_delta_impl(p, image, H, W, phase, pairs, n, delta, 0, stream);
 }
 
 // ---- host-buffer convenience (end-to-end measurement) ---------------------------------------------

@@ -142,6 +142,10 @@ namespace lpf {
 int canonical_path(int dx, int dy, int16_t* xy);
 inline bool in_half(int dx, int dy) { return dy > 0 || (dy == 0 && dx >= 0); }
 
+// lpf_swap_delta for one phase (0 | 1) or for both in one pass (phase < 0: phase k at delta + k * plane_stride); lpf_api.cu
+int swap_delta_impl(lpf_paths* p, const uint8_t* image, int H, int W, int phase, const int32_t* pairs, int64_t n,
+                    int32_t* delta, int64_t plane_stride, void* stream);
+
 // the image-coordinate trie in preorder for lpf_swap_delta (lpf_paths.cpp)
 void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec);
 

@@ -448,8 +448,10 @@ __global__ void objective_kernel(const long long* __restrict__ counts, const lon
 // [0, W + 2m), Y in [0, H + 2m), is pixel ((X - m) mod W, (Y - m) mod H).  One thread per output word.  With it a
 // segment that starts inside the image never needs a modulo.
 __global__ void pack_padded_kernel(const uint32_t* __restrict__ brow, uint32_t* __restrict__ padded, int H, int W,
-                                   int m) {
+                                   int m, long long brow_plane_stride) {
   const int Wc = (W + 31) >> 5, PWc = (W + 2 * m + 31) >> 5, PH = H + 2 * m;
+  brow += blockIdx.y * brow_plane_stride;                  // one phase plane per blockIdx.y
+  padded += (size_t)blockIdx.y * PH * PWc;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < PH * PWc; i += gridDim.x * blockDim.x) {
     const int Y = i / PWc, wi = i - Y * PWc;
     int y = (Y - m) % H;
@@ -482,28 +484,31 @@ struct SwapPass {                   // one (proposal, pixel) pass, in shared mem
   int ox, oy;                       // pixel that reads as out of phase in this pass (w in I'), or -1
   unsigned nb;                      // in-phase bits of the 8 neighbours px - step, by step code
   int sign;                         // +1: u on I', -1: w on I
-  int slot;                         // proposal index inside the CTA
+  int pbase;                        // word offset of this pass's phase plane in the shared-memory bit images
+  long long out_off;                // offset of this pass's [S][S] delta array from the CTA's first one
 };
 
 __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __restrict__ bits, int H, int W, int m,
                                                              const int* __restrict__ pairs, long long n,
                                                              const int4* __restrict__ rec, int n_nodes,
-                                                             int* __restrict__ delta) {
+                                                             int* __restrict__ delta, int n_planes,
+                                                             long long plane_stride) {
   extern __shared__ __align__(16) uint32_t sm[];
-  __shared__ SwapPass s_pass[2 * SWAP_SW];
+  __shared__ SwapPass s_pass[4 * SWAP_SW];                            // (proposal, phase plane, pixel)
   __shared__ int s_n;
   const int PWc = (W + 2 * m + 31) >> 5, PH = H + 2 * m;                // padded bit image: halo of m pixels all round
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  uint32_t* P = sm;                                                   // [PH][PWc] bits of the base image I
-  uint2* stk = (uint2*)(sm + ((PH * PWc + 1) & ~1)) + (size_t)warp * SWAP_STACK;
-  // pixel (x, y), x in [-m, W + m), y in [-m, H + m)
-  auto pbit = [&](int x, int y) -> unsigned {
+  uint32_t* P = sm;                                                   // [n_planes][PH][PWc] bits of the base image I
+  const int plane_words = PH * PWc;
+  uint2* stk = (uint2*)(sm + ((n_planes * plane_words + 1) & ~1)) + (size_t)warp * SWAP_STACK;
+  // pixel (x, y) of the plane at Pq, x in [-m, W + m), y in [-m, H + m)
+  auto pbit = [&](const uint32_t* Pq, int x, int y) -> unsigned {
     const int X = x + m;
-    return (P[(y + m) * PWc + (X >> 5)] >> (X & 31)) & 1u;
+    return (Pq[(y + m) * PWc + (X >> 5)] >> (X & 31)) & 1u;
   };
   const int S = 2 * m + 1;
   const long long K = (long long)S * S;
-  for (int i = tid; i < PH * PWc; i += blockDim.x) P[i] = bits[i];
+  for (int i = tid; i < n_planes * plane_words; i += blockDim.x) P[i] = bits[i];
   __syncthreads();
   if (tid == 0) {
     int cnt = 0;
@@ -513,24 +518,28 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
       const int xp = pairs[4 * sw], yp = pairs[4 * sw + 1], xq = pairs[4 * sw + 2], yq = pairs[4 * sw + 3];
       const bool ok = xp >= 0 && xp < W && xq >= 0 && xq < W && yp >= 0 && yp < H && yq >= 0 && yq < H;
       if (!ok) continue;
-      const int bp = (int)pbit(xp, yp), bq = (int)pbit(xq, yq);
-      if (bp == bq) continue;                              // nothing changes for this phase
-      const int ux = bp ? xq : xp, uy = bp ? yq : yp;      // bit 0 -> 1
-      const int wx = bp ? xp : xq, wy = bp ? yp : yq;      // bit 1 -> 0
-      for (int pass = 0; pass < 2; ++pass) {
-        SwapPass sp;
-        sp.px = pass ? wx : ux; sp.py = pass ? wy : uy;
-        sp.ox = pass ? -1 : wx; sp.oy = pass ? -1 : wy;
-        sp.nb = 0;
-        for (int code = 0; code < 9; ++code) {
-          const int x = wrap_coord(sp.px - (code / 3 - 1), W), y = wrap_coord(sp.py - (code % 3 - 1), H);
-          unsigned bit = pbit(x, y);
-          if (x == sp.ox && y == sp.oy) bit = 0;
-          sp.nb |= bit << code;
+      for (int pl = 0; pl < n_planes; ++pl) {
+        const uint32_t* Pq = P + pl * plane_words;
+        const int bp = (int)pbit(Pq, xp, yp), bq = (int)pbit(Pq, xq, yq);
+        if (bp == bq) continue;                            // nothing changes for this phase
+        const int ux = bp ? xq : xp, uy = bp ? yq : yp;    // bit 0 -> 1
+        const int wx = bp ? xp : xq, wy = bp ? yp : yq;    // bit 1 -> 0
+        for (int pass = 0; pass < 2; ++pass) {
+          SwapPass sp;
+          sp.px = pass ? wx : ux; sp.py = pass ? wy : uy;
+          sp.ox = pass ? -1 : wx; sp.oy = pass ? -1 : wy;
+          sp.nb = 0;
+          for (int code = 0; code < 9; ++code) {
+            const int x = wrap_coord(sp.px - (code / 3 - 1), W), y = wrap_coord(sp.py - (code % 3 - 1), H);
+            unsigned bit = pbit(Pq, x, y);
+            if (x == sp.ox && y == sp.oy) bit = 0;
+            sp.nb |= bit << code;
+          }
+          sp.sign = pass ? -1 : 1;
+          sp.pbase = pl * plane_words;
+          sp.out_off = (long long)pl * plane_stride + (long long)j * K;
+          s_pass[cnt++] = sp;
         }
-        sp.sign = pass ? -1 : 1;
-        sp.slot = j;
-        s_pass[cnt++] = sp;
       }
     }
     s_n = cnt;
@@ -562,12 +571,13 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
     const int e0 = 2 * d * mn + nn - 2 * nn * q0;
     for (int q = 0; q < np; ++q) {
       const unsigned nb = s_pass[q].nb;
+      const uint32_t* Pq = P + s_pass[q].pbase;
       bool alive = (N < n_end) && (d == 0 || ((nb >> codeN) & 1u));
       if (!__any_sync(0xffffffffu, alive)) continue;       // typical for u: an isolated pixel kills all 32 at once
       const int ox = s_pass[q].ox, oy = s_pass[q].oy;
       const int sx = wrap_coord(s_pass[q].px - oNx, W), sy = wrap_coord(s_pass[q].py - oNy, H);
       if (alive && d >= 2)                                 // the far end first: a long prefix usually dies at its start
-        alive = pbit(sx, sy) && !(sx == ox && sy == oy);
+        alive = pbit(Pq, sx, sy) && !(sx == ox && sy == oy);
       if (alive) {
         // (A) ancestors at positions d-2 .. 1 (d-1 was the neighbour test, 0 the start), stepping the error term backwards
         int e = e0, qq = q0;
@@ -581,7 +591,7 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
             L -= dmaj;
             if (e < 0) { e += 2 * nn; L -= dmin; }
             if (k == d - 1) continue;
-            if (!((P[L >> 5] >> (L & 31)) & 1u)) { alive = false; break; }
+            if (!((Pq[L >> 5] >> (L & 31)) & 1u)) { alive = false; break; }
           }
         } else {
           for (int k = d - 1; k >= 1; --k) {
@@ -590,11 +600,11 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
             if (k == d - 1) continue;
             const int ax_ = xmaj ? sxs * k : sxs * qq, ay_ = xmaj ? sys * qq : sys * k;
             const int x = wrap_coord(sx + ax_, W), y = wrap_coord(sy + ay_, H);
-            if (!pbit(x, y) || (x == ox && y == oy)) { alive = false; break; }
+            if (!pbit(Pq, x, y) || (x == ox && y == oy)) { alive = false; break; }
           }
         }
       }
-      int* const out = out0 + (long long)s_pass[q].slot * K;
+      int* const out = out0 + s_pass[q].out_off;
       const int sign = s_pass[q].sign;
       if (alive && (rN.w & 0xFFFFF) != 0xFFFFF) atomicAdd(out + (rN.w & 0xFFFFF), sign);
       // (B) push the first child of every survivor, then drain the warp stack
@@ -619,9 +629,9 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
           const int4 r = __ldg(rec + i);
           const int isx = (int)(it.y & 0xffff), isy = (int)(it.y >> 16);
           const int x = wrap_coord(isx + (short)(r.x & 0xffff), W), y = wrap_coord(isy + (r.x >> 16), H);
-          const bool in = pbit(x, y) && !(x == s_pass[qi].ox && y == s_pass[qi].oy);
+          const bool in = pbit(P + s_pass[qi].pbase, x, y) && !(x == s_pass[qi].ox && y == s_pass[qi].oy);
           if (in && (r.w & 0xFFFFF) != 0xFFFFF)
-            atomicAdd(out0 + (long long)s_pass[qi].slot * K + (r.w & 0xFFFFF), s_pass[qi].sign);
+            atomicAdd(out0 + s_pass[qi].out_off + (r.w & 0xFFFFF), s_pass[qi].sign);
           p_sib = (r.w >> 24) & 1;
           p_child = in && r.z > 1;
           if (p_sib) it.x += (unsigned)r.z;                // next sibling = i + subtree size
@@ -646,11 +656,11 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
               while (j < end) {
                 const int4 r = __ldg(rec + j);
                 const int x = wrap_coord(isx + (short)(r.x & 0xffff), W), y = wrap_coord(isy + (r.x >> 16), H);
-                const bool in = pbit(x, y) &&
+                const bool in = pbit(P + s_pass[qi].pbase, x, y) &&
                                 !(x == s_pass[qi].ox && y == s_pass[qi].oy);
                 if (in) {
                   if ((r.w & 0xFFFFF) != 0xFFFFF)
-                    atomicAdd(out0 + (long long)s_pass[qi].slot * K + (r.w & 0xFFFFF), s_pass[qi].sign);
+                    atomicAdd(out0 + s_pass[qi].out_off + (r.w & 0xFFFFF), s_pass[qi].sign);
                   ++j;
                 } else {
                   j += r.z;
@@ -661,10 +671,10 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
                 cur_top = end;
                 rt = __ldg(rec + cur_top);
                 const int x = wrap_coord(isx + (short)(rt.x & 0xffff), W), y = wrap_coord(isy + (rt.x >> 16), H);
-                const bool in = pbit(x, y) &&
+                const bool in = pbit(P + s_pass[qi].pbase, x, y) &&
                                 !(x == s_pass[qi].ox && y == s_pass[qi].oy);
                 if (in && (rt.w & 0xFFFFF) != 0xFFFFF)
-                  atomicAdd(out0 + (long long)s_pass[qi].slot * K + (rt.w & 0xFFFFF), s_pass[qi].sign);
+                  atomicAdd(out0 + s_pass[qi].out_off + (rt.w & 0xFFFFF), s_pass[qi].sign);
                 j = in ? cur_top + 1 : cur_top + rt.z;
               }
             }
@@ -751,32 +761,41 @@ cudaError_t launch_objective(const long long* counts, const long long* target, i
   return cudaGetLastError();
 }
 
+// phase 0 | 1: one plane, delta [n][S][S];  phase < 0: both planes, phase k at delta + k * plane_stride
 cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W, int m, int phase, const int* pairs,
-                              long long n, const int32_t* rec, int n_nodes, int* delta, unsigned int* counter,
-                              int n_sm, cudaStream_t st) {
+                              long long n, const int32_t* rec, int n_nodes, int* delta, long long plane_stride,
+                              unsigned int* counter, int n_sm, cudaStream_t st) {
+  const int n_planes = phase < 0 ? 2 : 1;
   const int Wc = (W + 31) / 32, Hc = (H + 31) / 32;
   const int PWc = (W + 2 * m + 31) / 32, PH = H + 2 * m;
-  const size_t smem = (size_t)((PH * PWc + 1) & ~1) * 4 + (size_t)8 * SWAP_STACK * 8;
-  uint32_t* const padded = bits + (size_t)H * Wc + (size_t)W * Hc;
+  const size_t smem = (size_t)((n_planes * PH * PWc + 1) & ~1) * 4 + (size_t)8 * SWAP_STACK * 8;
+  const long long img_words = (long long)H * Wc + (long long)W * Hc;
+  uint32_t* const padded = bits + (size_t)n_planes * img_words;
   cudaError_t e = cudaFuncSetAttribute(swap_delta_kernel_v3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   const long long S2 = (long long)(2 * m + 1) * (2 * m + 1);
-  e = cudaMemsetAsync(delta, 0, sizeof(int) * (size_t)n * S2, st);
-  if (e != cudaSuccess) return e;
-  // stage 1 of the bit-pack gives the row-major bit image of the base image (the column-major half is unused)
-  pack_base_kernel<<<(unsigned)std::max(1, (Hc * Wc + 7) / 8), 256, 0, st>>>(image, bits, 1, H, W, 1, phase, counter);
-  pack_padded_kernel<<<(unsigned)std::max(1, std::min((PH * PWc + 255) / 256, n_sm * 8)), 256, 0, st>>>(bits, padded, H, W, m);
+  for (int pl = 0; pl < n_planes; ++pl) {
+    e = cudaMemsetAsync(delta + pl * plane_stride, 0, sizeof(int) * (size_t)n * S2, st);
+    if (e != cudaSuccess) return e;
+  }
+  // stage 1 of the bit-pack gives the row-major bit image(s) of the base image (the column-major half is unused)
+  pack_base_kernel<<<(unsigned)std::max(1, (Hc * Wc + 7) / 8), 256, 0, st>>>(image, bits, 1, H, W, n_planes,
+                                                                             phase < 0 ? 0 : phase, counter);
+  pack_padded_kernel<<<dim3((unsigned)std::max(1, std::min((PH * PWc + 255) / 256, n_sm * 8)), (unsigned)n_planes), 256,
+                       0, st>>>(bits, padded, H, W, m, img_words);
   const long long ctas = (n + SWAP_SW - 1) / SWAP_SW;
   for (long long c0 = 0; c0 < ctas; c0 += (1ll << 30)) {
     const long long cnt = std::min(ctas - c0, 1ll << 30);
     const long long s0 = c0 * SWAP_SW;
     // node slices: about two CTAs per SM in total, at least 256 nodes per slice
-    const int slices = (int)std::max(1ll, std::min<long long>({(2ll * n_sm + cnt - 1) / cnt, (n_nodes + 255) / 256, 65535ll}));
-    swap_delta_kernel_v3<<<dim3((unsigned)cnt, (unsigned)slices), 256, smem, st>>>(padded, H, W, m, pairs + 4 * s0, n - s0, (const int4*)rec,
-                                                          n_nodes, delta + s0 * S2);
+    const int slices =
+        (int)std::max(1ll, std::min<long long>({(2ll * n_sm + cnt - 1) / cnt, (n_nodes + 255) / 256, 65535ll}));
+    swap_delta_kernel_v3<<<dim3((unsigned)cnt, (unsigned)slices), 256, smem, st>>>(
+        padded, H, W, m, pairs + 4 * s0, n - s0, (const int4*)rec, n_nodes, delta + s0 * S2, n_planes, plane_stride);
   }
-  long long blocks = std::min<long long>((n * (S2 / 2) + 255) / 256, (long long)n_sm * 16);
-  swap_mirror_kernel<<<(unsigned)std::max(1ll, blocks), 256, 0, st>>>(delta, 2 * m + 1, n);
+  const long long blocks = std::max(1ll, std::min<long long>((n * (S2 / 2) + 255) / 256, (long long)n_sm * 16));
+  for (int pl = 0; pl < n_planes; ++pl)
+    swap_mirror_kernel<<<(unsigned)blocks, 256, 0, st>>>(delta + pl * plane_stride, 2 * m + 1, n);
   return cudaGetLastError();
 }
 
