@@ -573,7 +573,7 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
       const unsigned nb = s_pass[q].nb;
       const uint32_t* Pq = P + s_pass[q].pbase;
       bool alive = (N < n_end) && (d == 0 || ((nb >> codeN) & 1u));
-      if (!__any_sync(0xffffffffu, alive)) continue;       // typical for u: an isolated pixel kills all 32 at once
+      if (__any_sync(0xffffffffu, alive)) {                // (not so: typical for u, an isolated pixel kills all 32 at once)
       const int ox = s_pass[q].ox, oy = s_pass[q].oy;
       const int sx = wrap_coord(s_pass[q].px - oNx, W), sy = wrap_coord(s_pass[q].py - oNy, H);
       if (alive && d >= 2)                                 // the far end first: a long prefix usually dies at its start
@@ -610,11 +610,15 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
       // (B) push the first child of every survivor, then drain the warp stack
       const bool push = alive && rN.z > 1;
       const unsigned pm = __ballot_sync(0xffffffffu, push);
-      if (push)                                            // the stack is empty here (drained per pass)
-        stk[__popc(pm & lt)] =
+      if (push)
+        stk[top + __popc(pm & lt)] =
             make_uint2((unsigned)(N + 1) | ((unsigned)q << 24), (unsigned)sx | ((unsigned)sy << 16));
-      top = __popc(pm);
+      top += __popc(pm);
       __syncwarp();
+      }
+      // the survivors of all passes are explored together (the depth of the live region is paid once, not once
+      // per pass); the stack is drained early only when the next 32 pushes might not fit
+      if (top <= SWAP_STACK - 32 && q + 1 < np) continue;
       while (top > 0) {
         const int take = min(top, 32);
         uint2 it = make_uint2(0, 0);
