@@ -454,6 +454,14 @@ def main():
             extra[name] = {"value": nominal_tests(wl) * k / (rr["total_ms"] * 1e-3), "unit": UNIT,
                            "ms_per_step": rr["total_ms"] / k, "kernel_ms": rr["kernel_ms"],
                            "roofline_frac": ops / (rr["kernel_ms"] * 1e-3) / peak_ops}
+        # the design variants the north star asks to compare, eval kernel alone on the headline workload
+        variants = {}
+        for vname, vflags in (("trie_pair_e2", 0), ("trie_no_e2", lpf.LPF_NO_E2), ("trie_prune", lpf.LPF_PRUNE),
+                              ("one_chain_per_path", lpf.LPF_NO_TRIE)):
+            flags_saved, flags = flags, vflags
+            variants[vname + "_kernel_ms"] = measure(w, 3, 1, False)["kernel_ms"]
+            flags = flags_saved
+        extra["variants_" + args.workload] = variants
         extra["cfg5"] = measure_swaps()
         extra["anneal"] = measure_anneal()
         line["other_workloads"] = extra
