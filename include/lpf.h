@@ -93,7 +93,8 @@ int  lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, int cap, int
  *            (dy+m)*(2m+1) + (dx+m) in IMAGE coordinates, 20-23 restore slot, 24-27 save slot
  *   items    host [cap_items][4] int64 = (first entry, number of entries, octant, 0) (may be NULL)
  *            bit 11 (E2): the entry stands for this node AND its direct child (a'+1, b'), walked on the eroded plane
- *            whose word offset strides[4+o] is included in bits 12-31; terminal / save / count index are the child's
+ *            whose word offset strides[4+o] is included in bits 12-31; terminal / save / count index are the child's;
+ *            with bit 28 of the high word the entry is ONE node read as E2 at (a'-1, b') (the extra pixel is its parent's)
  *   strides  host int[8]: [0..3] words per packed row of each octant view (decodes b', a' >> 5), [4..7] word offset
  *            of the E2 plane of each view in shared memory (0 if the program has no E2 entries)
  * *n_entries / *n_items / *n_slots (mask-stack slots the program needs) are always written.

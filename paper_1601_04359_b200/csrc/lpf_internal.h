@@ -61,6 +61,7 @@ inline void from_view(int o, int av, int bv, int* a, int* b) {
 //   [ 0..19] cidx    = (dy + m) * (2m + 1) + (dx + m), index into counts[2m+1][2m+1] (image coordinates)
 //   [20..23] rslot
 //   [24..27] sslot
+//   [28] BACK        (with E2) the entry is a single node read as E2 at (a'-1, b'): the extra pixel is its parent's
 constexpr uint32_t E_SH_MASK = 31u;
 constexpr uint32_t E_RELOAD = 1u << 5;
 constexpr uint32_t E_TERMINAL = 1u << 6;
@@ -69,6 +70,7 @@ constexpr uint32_t E_RESTORE = 1u << 8;
 constexpr uint32_t E_INIT = 1u << 9;
 constexpr uint32_t E_PAIR = 1u << 10;
 constexpr uint32_t E_E2 = 1u << 11;
+constexpr uint32_t E_BACK_HI = 1u << 28;   // high word: an E2 entry of ONE node, window one pixel to the left (for tests)
 constexpr int E_OFF_SHIFT = 12;
 constexpr uint32_t E_CIDX_MASK = (1u << 20) - 1u;
 constexpr int E_RSLOT_SHIFT = 20;

@@ -161,20 +161,30 @@ struct Emitter {
     return e2_off > 0 && nd[head].b == nd[child].b && (nd[head].a >> 5) == (nd[child].a >> 5);
   }
 
-  // one entry: the window of `head` (on the E2 plane if e2: then it also covers head's child `tail`); TERMINAL / SAVE
-  // and the count index are those of `tail`.  *held is updated to what the entry leaves in the registers.
-  uint64_t entry(int head, int tail, bool e2, uint32_t flags, Held* held, int rslot, int sslot) const {
-    const int a = nd[head].a, b = nd[head].b;      // view coordinates: a >= 0, 0 <= b <= a
+  // A single node whose parent lies in the same row and word column can ALSO be read from the E2 plane, one pixel
+  // to the left: E2 at (a-1, b) is pixel (a-1, b) -- the parent's, already in the mask -- AND pixel (a, b).  That keeps
+  // a whole same-row run on one plane (no strip reload for a plane change inside the run).
+  bool backward_ok(int node) const {
+    const int par = nd[node].parent;
+    return e2_off > 0 && par >= 0 && nd[par].b == nd[node].b && (nd[node].a & 31) != 0;
+  }
+
+  // one entry: the window of `head` (on the E2 plane if e2: then it also covers head's child `tail`, or, if back, the
+  // window starts one pixel to the left of the single node head == tail); TERMINAL / SAVE and the count index are those
+  // of `tail`.  *held is updated to what the entry leaves in the registers.
+  uint64_t entry(int head, int tail, bool e2, bool back, uint32_t flags, Held* held, int rslot, int sslot) const {
+    const int a = nd[head].a - (back ? 1 : 0), b = nd[head].b;      // view coordinates: a >= 0, 0 <= b <= a
     const bool direct = !(flags & (E_RESTORE | E_INIT));
-    const int plane = e2 ? 1 : 0;
+    const int plane = (e2 || back) ? 1 : 0;
     if (!direct || held->b != b || held->col != (a >> 5) || held->plane != plane) flags |= E_RELOAD;
     held->b = b; held->col = a >> 5; held->plane = plane;
-    const uint32_t off = (uint32_t)(b * stride + (a >> 5) + (e2 ? e2_off : 0));
-    const uint32_t x = (uint32_t)(a & 31) | flags | (e2 ? E_E2 : 0u) | (off << E_OFF_SHIFT);
+    const uint32_t off = (uint32_t)(b * stride + (a >> 5) + (plane ? e2_off : 0));
+    const uint32_t x = (uint32_t)(a & 31) | flags | (plane ? E_E2 : 0u) | (off << E_OFF_SHIFT);
     int ia, ib;
     from_view(o, nd[tail].a, nd[tail].b, &ia, &ib);
     const uint32_t cidx = (uint32_t)((ib + m) * (2 * m + 1) + (ia + m));
-    const uint32_t y = cidx | ((uint32_t)rslot << E_RSLOT_SHIFT) | ((uint32_t)sslot << E_SSLOT_SHIFT);
+    const uint32_t y = cidx | ((uint32_t)rslot << E_RSLOT_SHIFT) | ((uint32_t)sslot << E_SSLOT_SHIFT) |
+                       (back ? E_BACK_HI : 0u);
     return (uint64_t)x | ((uint64_t)y << 32);
   }
 
@@ -207,7 +217,8 @@ struct Emitter {
       max_slots = std::max(max_slots, depth_slots + 1);
     }
     const size_t at = out.entries.size();
-    out.entries.push_back(entry(node, tail, tail != node, flags, &held, rslot, sslot));
+    const bool back = tail == node && src != 2 && backward_ok(node);
+    out.entries.push_back(entry(node, tail, tail != node, back, flags, &held, rslot, sslot));
     out.skip.push_back(0);
     for (size_t i = 0; i < kids.size(); ++i) {
       if (kids.size() == 1) {
@@ -277,7 +288,9 @@ static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
       Held held;
       for (size_t i = 0; i < chain.size();) {
         const bool e2 = i + 1 < chain.size() && em.mergeable(chain[i], chain[i + 1]);
-        pr.entries.push_back(em.entry(chain[i], e2 ? chain[i + 1] : chain[i], e2, i == 0 ? E_INIT : 0u, &held, 0, 0));
+        const bool back = !e2 && i > 0 && em.backward_ok(chain[i]);
+        pr.entries.push_back(
+            em.entry(chain[i], e2 ? chain[i + 1] : chain[i], e2, back, i == 0 ? E_INIT : 0u, &held, 0, 0));
         pr.skip.push_back(0);
         i += e2 ? 2 : 1;
       }

@@ -94,7 +94,7 @@ def _decode(entries):
     x = (entries & np.uint64(0xffffffff)).astype(np.int64)
     y = (entries >> np.uint64(32)).astype(np.int64)
     return dict(sh=x & 31, reload=(x >> 5) & 1, terminal=(x >> 6) & 1, save=(x >> 7) & 1, restore=(x >> 8) & 1,
-                init=(x >> 9) & 1, pair=(x >> 10) & 1, e2=(x >> 11) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 15, sslot=(y >> 24) & 15)
+                init=(x >> 9) & 1, pair=(x >> 10) & 1, e2=(x >> 11) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 15, sslot=(y >> 24) & 15, back=(y >> 28) & 1)
 
 
 def _from_view(o, a, b):
@@ -137,10 +137,16 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
             if d["reload"][e]:
                 held = (bv, col, e2)
             assert held == (bv, col, e2), "stale row strip"
-            cur = cur + [_from_view(o, av, bv)]
-            if e2:                                           # the entry also stands for the child (a'+1, b'), same word
+            if e2 and d["back"][e]:                          # single node read one pixel to the left: the parent's pixel
+                assert cur and cur[-1] == _from_view(o, av, bv) and not d["init"][e]
                 assert (av + 1) >> 5 == col and av + 1 <= m
                 cur = cur + [_from_view(o, av + 1, bv)]
+            else:
+                assert not d["back"][e]
+                cur = cur + [_from_view(o, av, bv)]
+                if e2:                                       # the entry also stands for the child (a'+1, b'), same word
+                    assert (av + 1) >> 5 == col and av + 1 <= m
+                    cur = cur + [_from_view(o, av + 1, bv)]
             if d["terminal"][e]:
                 cidx = int(d["cidx"][e])
                 dy, dx = cidx // S - m, cidx % S - m
