@@ -161,7 +161,8 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   if (!dg.ok) return LPF_E_CUDA;
   cudaStream_t st = (cudaStream_t)stream;
   Geom g;
-  const bool use_e2 = !(flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2));     // the E2 plane serves the trie program
+  // the eroded planes serve the trie program; m = 0 has nothing but the root, which only the plain program counts
+  const bool use_e2 = !(flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)) && p->m >= 1;
   if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, use_e2, &g)) return LPF_E_UNSUPPORTED;
   const int Bpad = (B + g.G - 1) / g.G * g.G;
   long long off = 0;

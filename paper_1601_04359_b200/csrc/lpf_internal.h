@@ -70,7 +70,9 @@ constexpr uint32_t E_RESTORE = 1u << 8;
 constexpr uint32_t E_INIT = 1u << 9;
 constexpr uint32_t E_PAIR = 1u << 10;
 constexpr uint32_t E_E2 = 1u << 11;
-constexpr uint32_t E_BACK_HI = 1u << 28;   // high word: an E2 entry of ONE node, window one pixel to the left (for tests)
+constexpr uint32_t E_BACK_HI = 1u << 28;
+constexpr uint32_t E_D2_HI = 1u << 29;        // high word: the entry reads the D2 plane (pixel & lower-right neighbour)
+constexpr uint32_t E_ROOTCOUNT_HI = 1u << 30; // high word, INIT entries of the eroded program: count v = 0 here   // high word: an E2 entry of ONE node, window one pixel to the left (for tests)
 constexpr int E_OFF_SHIFT = 12;
 constexpr uint32_t E_CIDX_MASK = (1u << 20) - 1u;
 constexpr int E_RSLOT_SHIFT = 20;

@@ -122,28 +122,38 @@ __global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restr
     const long long rem = wp - v.packed_off;
     const int b = (int)(rem / v.view_words);
     const int idx = (int)(rem - (long long)b * v.view_words);
-    // plain view first, then (if enabled) the eroded view E2 = word & (word >> 1 across the word boundary)
-    const bool e2 = v.e2_view_off > 0 && idx >= v.e2_view_off;
-    const int idx1 = e2 ? idx - v.e2_view_off : idx;
+    // plain view first, then (if enabled) the two eroded views: E2 = pixel & right neighbour, D2 = pixel & lower-right
+    // neighbour (both across word boundaries)
+    const int which = v.e2_view_off > 0 ? idx / v.e2_view_off : 0;        // 0 plain, 1 E2, 2 D2
+    const int idx1 = idx - which * v.e2_view_off;
     const int r = idx1 / v.stride, i = idx1 - r * v.stride;
     const int rows = v.n_bands * g.band_rows + g.m;
     uint32_t word = 0;
-    if (b < B && r < rows) {
-      const int yv = r % v.Hv;
+    if (b < B && r < rows && which < 3) {
       const uint32_t* bimg = base + ((size_t)plane * B + b) * img_words;
-      // source row of this view row: views 0, 3: image row yv (Brow); view 1: image column yv; view 2: column -yv
-      const uint32_t* srow;
-      int words;
-      if (o == 0 || o == 3) { srow = bimg + (size_t)yv * Wc; words = Wc; }
-      else {
+      // source row of a view row: views 0, 3: image row yv (Brow); view 1: image column yv; view 2: column -yv
+      auto source_row = [&](int rr, int* words) -> const uint32_t* {
+        const int yv = rr % v.Hv;
+        if (o == 0 || o == 3) { *words = Wc; return bimg + (size_t)yv * Wc; }
         const int c = (o == 1) ? yv : (yv ? g.W - yv : 0);
-        srow = bimg + (size_t)g.H * Wc + (size_t)c * Hc;
-        words = Hc;
-      }
+        *words = Hc;
+        return bimg + (size_t)g.H * Wc + (size_t)c * Hc;
+      };
+      int words;
+      const uint32_t* srow = source_row(r, &words);
       word = view_word(srow, words, o, v.Wv, i);
-      if (e2) {
+      if (which == 1) {
         const uint32_t next = (i + 1 < v.stride) ? view_word(srow, words, o, v.Wv, i + 1) : 0u;
         word &= __funnelshift_r(word, next, 1);
+      } else if (which == 2) {
+        uint32_t below = 0;
+        if (r + 1 < rows) {
+          const uint32_t* s1 = source_row(r + 1, &words);
+          const uint32_t lo = view_word(s1, words, o, v.Wv, i);
+          const uint32_t hi = (i + 1 < v.stride) ? view_word(s1, words, o, v.Wv, i + 1) : 0u;
+          below = __funnelshift_r(lo, hi, 1);
+        }
+        word &= below;
       }
     }
     packed[w] = word;
@@ -247,10 +257,13 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
       const uint32_t* src = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b0 * v.view_words +
                             (size_t)band * g.band_rows * stride;
       for (int gi = 0; gi < g.G; ++gi) {
-        tma_bulk_g2s(smem + (size_t)gi * v.band_pitch, src + (size_t)gi * v.view_words, bytes, &bar);
-        if (v.e2_band_off)          // the eroded plane E2 of the same band, right behind the plain one
+        if (v.e2_band_off) {        // eroded mode: shared memory holds the E2 and the D2 band, the plain view stays in HBM
+          tma_bulk_g2s(smem + (size_t)gi * v.band_pitch, src + (size_t)gi * v.view_words + v.e2_view_off, bytes, &bar);
           tma_bulk_g2s(smem + (size_t)gi * v.band_pitch + v.e2_band_off,
-                       src + (size_t)gi * v.view_words + v.e2_view_off, bytes, &bar);
+                       src + (size_t)gi * v.view_words + 2 * (size_t)v.e2_view_off, bytes, &bar);
+        } else {
+          tma_bulk_g2s(smem + (size_t)gi * v.band_pitch, src + (size_t)gi * v.view_words, bytes, &bar);
+        }
       }
     }
     // per-item thread geometry (the octant decides the view size)
@@ -288,12 +301,27 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
                 const uint32_t cm = nb >= 32 ? 0xffffffffu : (nb <= 0 ? 0u : ((1u << nb) - 1u));
                 M[ty * TX + t] = rowok ? cm : 0u;
               }
+              if (v.e2_band_off && rowok) {                      // eroded mode: the root pixel comes from the plain view in HBM
+                const uint32_t* pw = p.packed + (size_t)plane * g.plane_words + v.packed_off +
+                                     (size_t)b_img * v.view_words +
+                                     (size_t)(band * g.band_rows + row0 + ty * 32) * stride + strip * TX;
+#pragma unroll
+                for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __ldg(pw + t);
+              }
               if (p.mask != nullptr && rowok) {                  // L2~: only the selected start pixels
                 const uint32_t* mw = p.mask + p.mask_off[o] +
                                      (size_t)(band * g.band_rows + row0 + ty * 32) * stride + strip * TX;
 #pragma unroll
                 for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __ldg(mw + t);
               }
+            }
+            const uint32_t yi = __shfl_sync(FULL, cur.y, i);
+            if (yi & E_ROOTCOUNT_HI) {   // eroded mode has no entry for the root: v = 0 is counted here, once per image
+              int c = 0;
+#pragma unroll
+              for (int t = 0; t < T; ++t) c += __popc(M[t]);
+              c = __reduce_add_sync(FULL, c);
+              if (c != 0 && store) atomicAdd(cnt + (size_t)(p.S / 2) * p.S + p.S / 2, (unsigned long long)c);
             }
           } else {
             const uint32_t y = __shfl_sync(FULL, cur.y, i);

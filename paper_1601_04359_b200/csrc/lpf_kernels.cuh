@@ -16,10 +16,10 @@ struct ViewGeom {
   int stride;        // words per packed row
   int n_bands;       // ceil(Hv / band_rows) bands of start rows
   int band_words;    // (band_rows + m) * stride rounded up to a multiple of 4: one band (one plane) in shared memory
-  int band_pitch;    // words per image in shared memory: band_words, or 2 * band_words with the E2 plane behind it
-  int e2_band_off;   // word offset of the E2 plane inside one image's shared-memory block (0: no E2 plane)
-  int view_words;    // whole packed block of one image (plain view, then the E2 view if enabled), multiple of 4
-  int e2_view_off;   // word offset of the E2 view inside that block (0: none)
+  int band_pitch;    // words per image in shared memory: band_words (plain mode) or 2 * band_words (eroded mode)
+  int e2_band_off;   // eroded mode: shared memory holds the E2 band at 0 and the D2 band at this offset; 0: plain mode
+  int view_words;    // whole packed block of one image: plain view, then (eroded mode) the E2 and the D2 view
+  int e2_view_off;   // eroded mode: the E2 view starts here, the D2 view at twice this; 0: plain mode
   long long packed_off;   // word offset of this octant's [Bpad][view_words] block inside one phase plane
 };
 
@@ -39,7 +39,8 @@ struct Geom {
 // host: pick the geometry for (m, H, W, B); false if one band does not fit in shared memory
 //   tx, ty > 0 override the thread tile; cta_warps (1..8) the warps per CTA
 constexpr int STACK_SLOTS_BUDGET = 8;   // mask-stack slots per thread (local memory, T words each)
-//   use_e2: also keep the eroded plane E2 = row & (row >> 1) of every view
+//   use_e2: eroded mode allowed: shared memory holds E2 = pixel & right neighbour and D2 = pixel & lower-right
+//   neighbour instead of the plain plane
 bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2, Geom* out);
 
 struct EvalParams {

@@ -146,46 +146,53 @@ struct Held {            // the row strip that is in the registers when an entry
   int b = -1, col = -1, plane = -1;
 };
 
+// Emits the entries of one octant.  Two program styles:
+//   plain mode  (d2_off == 0): one entry per node, window read from the plain bit plane
+//   eroded mode (d2_off  > 0): shared memory holds E2 = pixel & right neighbour (at word offset 0) and D2 = pixel &
+//     lower-right neighbour (at d2_off) instead of the plain plane.  Every path step is (+1, 0) or (+1, +1), so
+//       - a node whose own mask is never needed and its only child are ONE entry (window of E2 or D2 at the node),
+//       - any other node is read "backwards": the window of E2 / D2 at its PARENT covers the parent's pixel, which
+//         is already in the mask, and its own;
+//     the root has no entry: INIT loads the plain word of the start pixels from HBM, every child of the root starts
+//     with INIT, and v = 0 is counted by the INIT entry that carries E_ROOTCOUNT_HI.
 struct Emitter {
   int m, o, stride;
-  int e2_off;                           // word offset of the E2 plane of this view in shared memory (0: no E2 plane)
+  int d2_off;
   const std::vector<Node>& nd;
   const std::vector<uint8_t>& cut;      // node is the root of a piece
   const std::vector<int32_t>& psize;    // nodes of the subtree that stay in the node's own piece
   Program& out;
+  bool* root_pending;                   // v = 0 still has to be attached to an INIT entry (octant 0, eroded mode)
   int max_slots = 0;
 
-  // `head` and its direct child in the same row and word column can be walked as ONE entry on the eroded plane
-  // E2 = row & (row >> 1): the window of E2 at head's shift is the AND of the two windows
-  bool mergeable(int head, int child) const {
-    return e2_off > 0 && nd[head].b == nd[child].b && (nd[head].a >> 5) == (nd[child].a >> 5);
-  }
+  bool eroded() const { return d2_off > 0; }
 
-  // A single node whose parent lies in the same row and word column can ALSO be read from the E2 plane, one pixel
-  // to the left: E2 at (a-1, b) is pixel (a-1, b) -- the parent's, already in the mask -- AND pixel (a, b).  That keeps
-  // a whole same-row run on one plane (no strip reload for a plane change inside the run).
-  bool backward_ok(int node) const {
-    const int par = nd[node].parent;
-    return e2_off > 0 && par >= 0 && nd[par].b == nd[node].b && (nd[node].a & 31) != 0;
-  }
-
-  // one entry: the window of `head` (on the E2 plane if e2: then it also covers head's child `tail`, or, if back, the
-  // window starts one pixel to the left of the single node head == tail); TERMINAL / SAVE and the count index are those
-  // of `tail`.  *held is updated to what the entry leaves in the registers.
-  uint64_t entry(int head, int tail, bool e2, bool back, uint32_t flags, Held* held, int rslot, int sslot) const {
-    const int a = nd[head].a - (back ? 1 : 0), b = nd[head].b;      // view coordinates: a >= 0, 0 <= b <= a
+  // window at view pixel (a, b) on plane 0 plain / 1 E2 / 2 D2; TERMINAL / SAVE / count index belong to node `tail`
+  uint64_t entry(int a, int b, int plane, bool back, int tail, uint32_t flags, Held* held, int rslot, int sslot) const {
     const bool direct = !(flags & (E_RESTORE | E_INIT));
-    const int plane = (e2 || back) ? 1 : 0;
     if (!direct || held->b != b || held->col != (a >> 5) || held->plane != plane) flags |= E_RELOAD;
     held->b = b; held->col = a >> 5; held->plane = plane;
-    const uint32_t off = (uint32_t)(b * stride + (a >> 5) + (plane ? e2_off : 0));
+    const uint32_t off = (uint32_t)(b * stride + (a >> 5) + (plane == 2 ? d2_off : 0));
     const uint32_t x = (uint32_t)(a & 31) | flags | (plane ? E_E2 : 0u) | (off << E_OFF_SHIFT);
     int ia, ib;
     from_view(o, nd[tail].a, nd[tail].b, &ia, &ib);
     const uint32_t cidx = (uint32_t)((ib + m) * (2 * m + 1) + (ia + m));
-    const uint32_t y = cidx | ((uint32_t)rslot << E_RSLOT_SHIFT) | ((uint32_t)sslot << E_SSLOT_SHIFT) |
-                       (back ? E_BACK_HI : 0u);
+    uint32_t y = cidx | ((uint32_t)rslot << E_RSLOT_SHIFT) | ((uint32_t)sslot << E_SSLOT_SHIFT) |
+                 (back ? E_BACK_HI : 0u) | (plane == 2 ? E_D2_HI : 0u);
+    if ((flags & E_INIT) && root_pending && *root_pending) {
+      y |= E_ROOTCOUNT_HI;
+      *root_pending = false;
+    }
     return (uint64_t)x | ((uint64_t)y << 32);
+  }
+
+  // the entry of `node` alone (backward window in eroded mode) or, if `child` >= 0, of node and child merged
+  uint64_t node_entry(int node, int child, uint32_t flags, Held* held, int rslot, int sslot) const {
+    if (!eroded()) return entry(nd[node].a, nd[node].b, 0, false, node, flags, held, rslot, sslot);
+    if (child >= 0)
+      return entry(nd[node].a, nd[node].b, nd[child].b == nd[node].b ? 1 : 2, false, child, flags, held, rslot, sslot);
+    const int par = nd[node].parent;                 // >= 0: the root has no entry in eroded mode
+    return entry(nd[par].a, nd[par].b, nd[par].b == nd[node].b ? 1 : 2, true, node, flags, held, rslot, sslot);
   }
 
   void kids_of(int node, std::vector<int>* kids) const {
@@ -200,12 +207,12 @@ struct Emitter {
   void emit(int node, int src, int rslot, int depth_slots, bool count_it, Held held) {
     std::vector<int> kids;
     kids_of(node, &kids);
-    int tail = node;
+    int child = -1;
     bool term = nd[node].terminal && count_it;
-    if (kids.size() == 1 && !term && mergeable(node, kids[0])) {   // node's own mask is never needed: fold the child in
-      tail = kids[0];
-      term = nd[tail].terminal;
-      kids_of(tail, &kids);
+    if (eroded() && kids.size() == 1 && !term) {     // node's own mask is never needed: fold the only child in
+      child = kids[0];
+      term = nd[child].terminal;
+      kids_of(child, &kids);
     }
     uint32_t flags = term ? E_TERMINAL : 0u;
     if (src == 1) flags |= E_RESTORE;
@@ -217,8 +224,7 @@ struct Emitter {
       max_slots = std::max(max_slots, depth_slots + 1);
     }
     const size_t at = out.entries.size();
-    const bool back = tail == node && src != 2 && backward_ok(node);
-    out.entries.push_back(entry(node, tail, tail != node, back, flags, &held, rslot, sslot));
+    out.entries.push_back(node_entry(node, child, flags, &held, rslot, sslot));
     out.skip.push_back(0);
     for (size_t i = 0; i < kids.size(); ++i) {
       if (kids.size() == 1) {
@@ -275,26 +281,34 @@ static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
       else psize[nd[i].parent] += psize[i];
     }
     cut[0] = 1;
-    Emitter em{p->m, o, pr.stride[o], pr.e2_off[o], nd, cut, psize, pr};
-    std::vector<int> chain;
+    bool root_pending = (o == 0) && pr.e2_off[o] > 0;      // eroded mode only: plain mode has a root entry
+    Emitter em{p->m, o, pr.stride[o], pr.e2_off[o], nd, cut, psize, pr, &root_pending};
+    std::vector<int> chain, kids;
     for (int r = 0; r < N; ++r) {
       if (!cut[r]) continue;
-      if (r == 0 && o != 0 && psize[0] == 1) continue;   // v = 0 is counted in octant 0 only
       const int64_t first = (int64_t)pr.entries.size();
-      // chain root -> parent(r): recomputed per item, never counted, never saved
+      if (em.eroded() && r == 0) {
+        // the root piece: the root has no entry, each of its children in the piece starts from INIT
+        em.kids_of(0, &kids);
+        for (int c : kids) em.emit(c, 2, 0, 0, true, Held());
+        if (pr.entries.size() > (size_t)first) push_item(pr, first, o);
+        continue;
+      }
+      if (r == 0 && o != 0 && psize[0] == 1) continue;   // plain mode: v = 0 is counted in octant 0 only
+      // chain root -> parent(r): recomputed per item, never counted, never saved (eroded mode: without the root)
       chain.clear();
       for (int u = nd[r].parent; u >= 0; u = nd[u].parent) chain.push_back(u);
       std::reverse(chain.begin(), chain.end());
       Held held;
-      for (size_t i = 0; i < chain.size();) {
-        const bool e2 = i + 1 < chain.size() && em.mergeable(chain[i], chain[i + 1]);
-        const bool back = !e2 && i > 0 && em.backward_ok(chain[i]);
-        pr.entries.push_back(
-            em.entry(chain[i], e2 ? chain[i + 1] : chain[i], e2, back, i == 0 ? E_INIT : 0u, &held, 0, 0));
+      bool started = false;
+      for (size_t i = em.eroded() ? 1 : 0; i < chain.size();) {
+        const bool merge = em.eroded() && i + 1 < chain.size();
+        pr.entries.push_back(em.node_entry(chain[i], merge ? chain[i + 1] : -1, started ? 0u : E_INIT, &held, 0, 0));
         pr.skip.push_back(0);
-        i += e2 ? 2 : 1;
+        started = true;
+        i += merge ? 2 : 1;
       }
-      em.emit(r, chain.empty() ? 2 : 0, 0, 0, !(r == 0 && o != 0), held);
+      em.emit(r, started ? 0 : 2, 0, 0, !(r == 0 && o != 0), held);
       push_item(pr, first, o);
     }
     pr.n_slots = std::max(pr.n_slots, em.max_slots);
@@ -508,7 +522,7 @@ static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, 
       const int plain_view = ((v.n_bands * g.band_rows + m) * v.stride + 3) / 4 * 4 + 4;
       v.band_pitch = use_e2 ? 2 * v.band_words : v.band_words;
       v.e2_band_off = use_e2 ? v.band_words : 0;
-      v.view_words = use_e2 ? 2 * plain_view : plain_view;
+      v.view_words = use_e2 ? 3 * plain_view : plain_view;     // eroded mode packs plain | E2 | D2
       v.e2_view_off = use_e2 ? plain_view : 0;
       bw_max = std::max(bw_max, v.band_pitch);
     }
@@ -587,7 +601,7 @@ extern "C" int lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, un
   if (H < 1 || W < 1 || p->m > std::min(H, W) - 1) return LPF_E_INVAL;
   lpf::Geom g;
   if (!lpf::choose_geom(p->m, H, W, 1, p->max_smem > 0 ? p->max_smem : 232448, p->tile_tx, p->tile_ty, p->cta_warps,
-                        !(flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)), &g))
+                        !(flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)) && p->m >= 1, &g))
     return LPF_E_UNSUPPORTED;
   try {
     lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride, g.v[0].e2_band_off,

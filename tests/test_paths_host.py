@@ -94,7 +94,8 @@ def _decode(entries):
     x = (entries & np.uint64(0xffffffff)).astype(np.int64)
     y = (entries >> np.uint64(32)).astype(np.int64)
     return dict(sh=x & 31, reload=(x >> 5) & 1, terminal=(x >> 6) & 1, save=(x >> 7) & 1, restore=(x >> 8) & 1,
-                init=(x >> 9) & 1, pair=(x >> 10) & 1, e2=(x >> 11) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 15, sslot=(y >> 24) & 15, back=(y >> 28) & 1)
+                init=(x >> 9) & 1, pair=(x >> 10) & 1, e2=(x >> 11) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 15, sslot=(y >> 24) & 15, back=(y >> 28) & 1,
+                d2=(y >> 29) & 1, rootcount=(y >> 30) & 1)
 
 
 def _from_view(o, a, b):
@@ -120,33 +121,39 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
     for first, cnt, o, _ in items:
         cur, stack, held = None, {}, None
         assert strides[o] % 2 == 1
+        eroded = strides[4 + o] > 0                          # shared memory holds E2 and D2 instead of the plain plane
+        if eroded:
+            assert not (flags & (lpf.LPF_NO_E2 | lpf.LPF_NO_TRIE))
         for e in range(first, first + cnt):
             assert not covered[e]
             covered[e] = True
             if d["init"][e]:
-                cur = []
+                cur = [(0, 0)] if eroded else []             # eroded mode: INIT loads the root pixel from the plain view
+                if d["rootcount"][e]:
+                    assert eroded and o == 0 and (0, 0) not in seen
+                    seen[(0, 0)] = [(0, 0)]
             elif d["restore"][e]:
                 cur = list(stack[int(d["rslot"][e])])
-            assert cur is not None
-            e2 = bool(d["e2"][e])
-            if e2:
-                assert strides[4 + o] > 0 and not (flags & (lpf.LPF_NO_E2 | lpf.LPF_NO_TRIE))
-            bv, col = divmod(int(d["off"][e]) - (strides[4 + o] if e2 else 0), strides[o])
+            assert cur is not None and not (d["rootcount"][e] and not d["init"][e])
+            plane = (2 if d["d2"][e] else 1) if d["e2"][e] else 0
+            assert (plane > 0) == eroded
+            bv, col = divmod(int(d["off"][e]) - (strides[4 + o] if plane == 2 else 0), strides[o])
             av = col * 32 + int(d["sh"][e])
             assert 0 <= bv <= av <= m
             if d["reload"][e]:
-                held = (bv, col, e2)
-            assert held == (bv, col, e2), "stale row strip"
-            if e2 and d["back"][e]:                          # single node read one pixel to the left: the parent's pixel
-                assert cur and cur[-1] == _from_view(o, av, bv) and not d["init"][e]
-                assert (av + 1) >> 5 == col and av + 1 <= m
-                cur = cur + [_from_view(o, av + 1, bv)]
-            else:
+                held = (bv, col, plane)
+            assert held == (bv, col, plane), "stale row strip"
+            if plane == 0:
                 assert not d["back"][e]
                 cur = cur + [_from_view(o, av, bv)]
-                if e2:                                       # the entry also stands for the child (a'+1, b'), same word
-                    assert (av + 1) >> 5 == col and av + 1 <= m
-                    cur = cur + [_from_view(o, av + 1, bv)]
+            else:
+                second = (av + 1, bv) if plane == 1 else (av + 1, bv + 1)    # E2: right neighbour, D2: lower right
+                assert second[1] <= second[0] <= m
+                if d["back"][e]:                             # one node, read at its parent: the first pixel is old
+                    assert cur[-1] == _from_view(o, av, bv)
+                else:                                        # a node whose mask is never needed and its only child
+                    cur = cur + [_from_view(o, av, bv)]
+                cur = cur + [_from_view(o, *second)]
             if d["terminal"][e]:
                 cidx = int(d["cidx"][e])
                 dy, dx = cidx // S - m, cidx % S - m
@@ -162,8 +169,8 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
             assert bool(d["pair"][e]) == bool(want_pair)
     assert covered.all()
     assert len(seen) == 2 * m * m + 2 * m + 1
-    if not (flags & (lpf.LPF_NO_E2 | lpf.LPF_NO_TRIE)):
-        assert d["e2"].sum() > len(entries) // 8            # the eroded plane really carries a share of the nodes
+    if not (flags & (lpf.LPF_NO_E2 | lpf.LPF_NO_TRIE)) and m >= 1:
+        assert d["e2"].all() and d["d2"].any() and (~d["d2"].astype(bool)).any()   # the default program is the eroded one
     for (dx, dy), pix in seen.items():
         assert orc.in_half(dx, dy)
         assert pix == [tuple(int(t) for t in r) for r in orc.path(dx, dy)], (dx, dy)
