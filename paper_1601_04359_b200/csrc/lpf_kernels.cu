@@ -282,6 +282,37 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
     int e = wk.x;
     const int e1 = e + wk.y;
     uint2 cur = __ldg(p.entries + e + lane);                 // the entry array is padded by 64
+    // Every item begins with its only INIT entry: the parent mask is "every valid start pixel" (of the selected ones
+    // for L2~; in eroded mode AND the plain word of the start pixels themselves, i.e. the root pixel, from HBM).
+#pragma unroll
+    for (int ty = 0; ty < TY; ++ty) {
+      const bool rowok = active && (band * g.band_rows + row0 + ty * 32 < v.Hv);
+#pragma unroll
+      for (int t = 0; t < TX; ++t) {
+        const int nb = v.Wv - 32 * (strip * TX + t);         // start pixels x' < Wv only
+        const uint32_t cm = nb >= 32 ? 0xffffffffu : (nb <= 0 ? 0u : ((1u << nb) - 1u));
+        M[ty * TX + t] = rowok ? cm : 0u;
+      }
+      if (v.e2_band_off && rowok) {
+        const uint32_t* pw = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b_img * v.view_words +
+                             (size_t)(band * g.band_rows + row0 + ty * 32) * stride + strip * TX;
+#pragma unroll
+        for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __ldg(pw + t);
+      }
+      if (p.mask != nullptr && rowok) {                      // L2~: only the selected start pixels
+        const uint32_t* mw =
+            p.mask + p.mask_off[o] + (size_t)(band * g.band_rows + row0 + ty * 32) * stride + strip * TX;
+#pragma unroll
+        for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __ldg(mw + t);
+      }
+    }
+    if (__shfl_sync(FULL, cur.y, 0) & E_ROOTCOUNT_HI) {      // eroded mode has no entry for the root: v = 0 is counted here
+      int c = 0;
+#pragma unroll
+      for (int t = 0; t < T; ++t) c += __popc(M[t]);
+      c = __reduce_add_sync(FULL, c);
+      if (c != 0 && store) atomicAdd(cnt + (size_t)(p.S / 2) * p.S + p.S / 2, (unsigned long long)c);
+    }
     while (e < e1) {
       const uint2 nxt = __ldg(p.entries + e + 32 + lane);
       const int n = min(32, e1 - e);
@@ -290,45 +321,11 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
 #pragma unroll 1
       for (int i = 0; i < n; ++i) {
         uint32_t xn = __shfl_sync(FULL, cur.x, i + 1);
-        if (x & (E_INIT | E_RESTORE)) {
-          if (x & E_INIT) {
+        if (x & E_RESTORE) {
+          const uint32_t y = __shfl_sync(FULL, cur.y, i);
+          const uint32_t* s = stk + ((y >> E_RSLOT_SHIFT) & E_SLOT_MASK) * T;
 #pragma unroll
-            for (int ty = 0; ty < TY; ++ty) {
-              const bool rowok = active && (band * g.band_rows + row0 + ty * 32 < v.Hv);
-#pragma unroll
-              for (int t = 0; t < TX; ++t) {
-                const int nb = v.Wv - 32 * (strip * TX + t);   // start pixels x' < Wv only
-                const uint32_t cm = nb >= 32 ? 0xffffffffu : (nb <= 0 ? 0u : ((1u << nb) - 1u));
-                M[ty * TX + t] = rowok ? cm : 0u;
-              }
-              if (v.e2_band_off && rowok) {                      // eroded mode: the root pixel comes from the plain view in HBM
-                const uint32_t* pw = p.packed + (size_t)plane * g.plane_words + v.packed_off +
-                                     (size_t)b_img * v.view_words +
-                                     (size_t)(band * g.band_rows + row0 + ty * 32) * stride + strip * TX;
-#pragma unroll
-                for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __ldg(pw + t);
-              }
-              if (p.mask != nullptr && rowok) {                  // L2~: only the selected start pixels
-                const uint32_t* mw = p.mask + p.mask_off[o] +
-                                     (size_t)(band * g.band_rows + row0 + ty * 32) * stride + strip * TX;
-#pragma unroll
-                for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __ldg(mw + t);
-              }
-            }
-            const uint32_t yi = __shfl_sync(FULL, cur.y, i);
-            if (yi & E_ROOTCOUNT_HI) {   // eroded mode has no entry for the root: v = 0 is counted here, once per image
-              int c = 0;
-#pragma unroll
-              for (int t = 0; t < T; ++t) c += __popc(M[t]);
-              c = __reduce_add_sync(FULL, c);
-              if (c != 0 && store) atomicAdd(cnt + (size_t)(p.S / 2) * p.S + p.S / 2, (unsigned long long)c);
-            }
-          } else {
-            const uint32_t y = __shfl_sync(FULL, cur.y, i);
-            const uint32_t* s = stk + ((y >> E_RSLOT_SHIFT) & E_SLOT_MASK) * T;
-#pragma unroll
-            for (int t = 0; t < T; ++t) M[t] = s[t];
-          }
+          for (int t = 0; t < T; ++t) M[t] = s[t];
         }
         if (x & E_RELOAD) {
           const char* rp = base + ((x >> (E_OFF_SHIFT - 2)) & ~3u);

@@ -290,8 +290,11 @@ static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
       if (em.eroded() && r == 0) {
         // the root piece: the root has no entry, each of its children in the piece starts from INIT
         em.kids_of(0, &kids);
-        for (int c : kids) em.emit(c, 2, 0, 0, true, Held());
-        if (pr.entries.size() > (size_t)first) push_item(pr, first, o);
+        for (int c : kids) {                               // INIT is only ever the first entry of an item
+          const int64_t f = (int64_t)pr.entries.size();
+          em.emit(c, 2, 0, 0, true, Held());
+          push_item(pr, f, o);
+        }
         continue;
       }
       if (r == 0 && o != 0 && psize[0] == 1) continue;   // plain mode: v = 0 is counted in octant 0 only
@@ -316,40 +319,50 @@ static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
   sort_items(pr);
 }
 
-// LPF_NO_TRIE: one chain per path, no sharing ("one-path-per-warp" variant of the north star)
+// LPF_NO_TRIE: one chain per path, no sharing ("one-path-per-warp" variant of the north star).  An item opens with the
+// root pixel (its only INIT entry, saved in slot 0); every path restores that mask and walks its pixels 1..n.
 static void build_chain_program(lpf_paths* p, int piece_nodes, Program& pr) {
   const int m = p->m;
   std::vector<int16_t> xy(2 * (size_t)(m + 1));
+  const uint32_t cidx0 = (uint32_t)(m * (2 * m + 1) + m);
   for (int o = 0; o < 4; ++o) {
-    int64_t first = (int64_t)pr.entries.size();
+    int64_t first = -1;
+    bool zero_done = false;
     const int stride = pr.stride[o];
     for (int dy = 0; dy <= m; ++dy)
       for (int dx = -m; dx <= m; ++dx) {
         if (!in_half(dx, dy) || octant_of(dx, dy) != o) continue;
+        if (first < 0) {                                   // open an item: the root pixel, saved in slot 0
+          first = (int64_t)pr.entries.size();
+          uint32_t x = E_INIT | E_RELOAD | E_SAVE;
+          if (o == 0 && !zero_done) { x |= E_TERMINAL; zero_done = true; }   // v = 0 is counted once
+          pr.entries.push_back((uint64_t)x | ((uint64_t)cidx0 << 32));
+          pr.skip.push_back(0);
+        }
         const int len = canonical_path(dx, dy, xy.data());
         int pa = 0, pb = 0;
-        for (int k = 0; k < len; ++k) {
+        for (int k = 1; k < len; ++k) {
           int a, b;
           to_view(o, xy[2 * k], xy[2 * k + 1], &a, &b);
-          uint32_t f = (k == 0) ? (E_INIT | E_RELOAD) : 0u;
-          if (k > 0 && (b != pb || (a >> 5) != (pa >> 5))) f |= E_RELOAD;
+          uint32_t f = (k == 1) ? (E_RESTORE | E_RELOAD) : 0u;
+          if (k > 1 && (b != pb || (a >> 5) != (pa >> 5))) f |= E_RELOAD;
           if (k == len - 1) f |= E_TERMINAL;
           const uint32_t off = (uint32_t)(b * stride + (a >> 5));
           const uint32_t x = (uint32_t)(a & 31) | f | (off << E_OFF_SHIFT);
           const uint32_t cidx = (uint32_t)((dy + m) * (2 * m + 1) + (dx + m));
-          pr.entries.push_back((uint64_t)x | ((uint64_t)cidx << 32));
+          pr.entries.push_back((uint64_t)x | ((uint64_t)cidx << 32));   // restore slot 0
           pr.skip.push_back(0);
           pa = a;
           pb = b;
         }
         if (piece_nodes > 0 && (int64_t)pr.entries.size() - first >= piece_nodes) {
           push_item(pr, first, o);
-          first = (int64_t)pr.entries.size();
+          first = -1;
         }
       }
-    if ((int64_t)pr.entries.size() > first) push_item(pr, first, o);
+    if (first >= 0) push_item(pr, first, o);
   }
-  pr.n_slots = 0;
+  pr.n_slots = 1;
   sort_items(pr);
 }
 

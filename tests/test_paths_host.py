@@ -127,6 +127,7 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
         for e in range(first, first + cnt):
             assert not covered[e]
             covered[e] = True
+            assert bool(d["init"][e]) == (e == first)        # the kernel initialises the mask once, at the item's start
             if d["init"][e]:
                 cur = [(0, 0)] if eroded else []             # eroded mode: INIT loads the root pixel from the plain view
                 if d["rootcount"][e]:
