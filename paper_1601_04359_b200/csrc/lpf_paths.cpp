@@ -479,18 +479,23 @@ static bool choose_geom_plane(int m, int H, int W, int B, int max_smem, int tx, 
   return best_warps > 0;
 }
 
-// use_e2 = "the E2 plane is allowed": it doubles the shared memory of a band, which pays (measured, DESIGN.md "E2
-// plane") as long as at least 12 warps stay resident per SM; templates that are large against the image (m close to
-// H: the halo dominates the band) fall back to the plain plane.
+// use_e2 = "the eroded program is allowed": its two planes double the shared memory of a band; templates that are
+// large against the image (m close to H: the halo dominates the band) can lose too much residency and then fall
+// back to the plain plane.
 bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2, Geom* out) {
-  if (use_e2) {
-    Geom g;
-    if (choose_geom_plane(m, H, W, B, max_smem, tx, ty, cta_warps, true, &g) && resident_warps(g, max_smem) >= 12) {
-      *out = g;
+  Geom plain, eroded;
+  const bool ok_plain = choose_geom_plane(m, H, W, B, max_smem, tx, ty, cta_warps, false, &plain);
+  if (use_e2 && choose_geom_plane(m, H, W, B, max_smem, tx, ty, cta_warps, true, &eroded)) {
+    // measured: the eroded program wins with 16 resident warps against 24 and with 8
+    // against 16, and loses with 8 against 24
+    const int we = resident_warps(eroded, max_smem), wp = ok_plain ? resident_warps(plain, max_smem) : 0;
+    if (we >= 12 || 2 * we >= wp) {
+      *out = eroded;
       return true;
     }
   }
-  return choose_geom_plane(m, H, W, B, max_smem, tx, ty, cta_warps, false, out);
+  if (ok_plain) *out = plain;
+  return ok_plain;
 }
 
 static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2,
