@@ -55,8 +55,9 @@ extern "C" {
                              (PAPER.md:99); same kernels, a program of 2-pixel "paths".  Exact integers (the paper's
                              FFT form, Eq. 7, is floating point). */
 
-#define LPF_NO_E2    8u   /* measurement: walk every node on the plain bit plane (no eroded plane E2 = row & row >> 1,
-                             DESIGN.md "E2 plane").  Same counts. */
+#define LPF_NO_E2    8u   /* measurement: walk every node on the plain bit plane instead of the two eroded planes
+                             (pixel & right neighbour, pixel & lower-right neighbour).
+                             Same counts. */
 
 typedef struct lpf_paths lpf_paths;   /* opaque: path table + prefix trie + device programs for one m */
 
@@ -92,11 +93,14 @@ int  lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, int cap, int
  *            bits 12-31 b' * stride + (a' >> 5); high word: bits 0-19
  *            (dy+m)*(2m+1) + (dx+m) in IMAGE coordinates, 20-23 restore slot, 24-27 save slot
  *   items    host [cap_items][4] int64 = (first entry, number of entries, octant, 0) (may be NULL)
- *            bit 11 (E2): the entry stands for this node AND its direct child (a'+1, b'), walked on the eroded plane
- *            whose word offset strides[4+o] is included in bits 12-31; terminal / save / count index are the child's;
- *            with bit 28 of the high word the entry is ONE node read as E2 at (a'-1, b') (the extra pixel is its parent's)
+ *            bit 11: the window is read from an eroded plane (eroded program: every entry).  High word bit 29 chooses
+ *            D2 = pixel & lower-right neighbour (else E2 = pixel & right neighbour); the window then covers TWO path
+ *            pixels: the entry's node and its only child (terminal / save / count index are the child's), or, with
+ *            high word bit 28, the node's parent -- already in the mask -- and the node.  The eroded program has no
+ *            entry for the root: the kernel starts every item (its first and only INIT entry) from the plain word of
+ *            the start pixels, and counts v = 0 at the INIT entry that carries high word bit 30.
  *   strides  host int[8]: [0..3] words per packed row of each octant view (decodes b', a' >> 5), [4..7] word offset
- *            of the E2 plane of each view in shared memory (0 if the program has no E2 entries)
+ *            of the D2 plane of each view in shared memory (E2 sits at 0; all 0 for the plain program)
  * *n_entries / *n_items / *n_slots (mask-stack slots the program needs) are always written.
  * Octants (view coordinates a', b' from image coordinates a, b): 0: dx>=0, dy<=dx (a,b); 1: dx>=0, dy>dx (b,a);
  * 2: dx<0, dy>-dx (b,-a); 3: dx<0, dy<=-dx (-a,b). */
