@@ -413,8 +413,8 @@ def main():
     achieved = alg_ops / (r["kernel_ms"] * 1e-3)
     measured = lpf.lpf_alu_peak(local_rank) if rank == 0 else None     # live LOP3 / SHF / pair-pattern / POPC rates
     # dram__bytes_read.sum + dram__bytes_write.sum of one eval-kernel launch, from the committed ncu --set full
-    # capture of this command (profiles/r01_v5_eval_kernel_full.csv: 29.99 MB + 1.32 MB); config 3, no flags only
-    traffic = 31.31e6 if (args.workload == "cfg3" and not args.flags) else None
+    # capture of this command (profiles/r01_v6_eval_kernel_full.csv: 24.07 MB + 1.02 MB); config 3, no flags only
+    traffic = 25.10e6 if (args.workload == "cfg3" and not args.flags) else None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": r["total_ms"] / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -434,8 +434,8 @@ def main():
                                     % sm_max_mhz,
                      "kernel_share_of_step": r["kernel_ms"] * args.steps / r["total_ms"],
                      "note": "algorithmic ops = SURVEY 8(d): 2 per word-node + 2 per word-terminal; the kernel executes fewer "
-                             "(3-input AND pair fusion, eroded E2 plane: DESIGN.md), so frac can exceed 1; ncu of this "
-                             "command: alu pipe 65 %, shared-memory wavefronts 75 % of peak (profiles/r01_v5_eval_kernel.md)"},
+                             "(3-input AND pair fusion, eroded planes E2/D2: DESIGN.md), so frac can exceed 1; ncu of this "
+                             "command: alu pipe 66 %, shared-memory wavefronts 73 % of peak (profiles/r01_v6_eval_kernel.md)"},
         "e2e": {"value": tests_per_step / r["e2e_s"], "unit": UNIT, "h2d_bytes_per_step": r["e2e"]["h2d"],
                 "d2h_bytes_per_step": r["e2e"]["d2h"]},
         "gpu_launches": r["launches_per_step"] * args.steps,

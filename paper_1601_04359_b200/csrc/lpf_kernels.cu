@@ -109,27 +109,29 @@ __global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restr
                                                          uint32_t* __restrict__ packed, Geom g, int B, int n_phase) {
   const int Wc = (g.W + 31) >> 5, Hc = (g.H + 31) >> 5;
   const long long img_words = (long long)g.H * Wc + (long long)g.W * Hc;
-  const long long total = (long long)n_phase * g.plane_words;
-  for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < total;
-       w += (long long)gridDim.x * blockDim.x) {
-    const int plane = (int)(w / g.plane_words);
-    const long long wp = w - (long long)plane * g.plane_words;
+  // one thread per word POSITION (r, i) of a view: it writes the plain word and, in eroded mode, the E2 and the D2
+  // word of the same position (E2 = pixel & right neighbour, D2 = pixel & lower-right neighbour, across word and
+  // row boundaries), from the four plain words (r, i), (r, i+1), (r+1, i), (r+1, i+1)
+  const int np = g.v[0].e2_view_off > 0 ? 3 : 1;
+  const long long units_per_plane = g.plane_words / np;
+  const long long total = (long long)n_phase * units_per_plane;
+  for (long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x; u < total;
+       u += (long long)gridDim.x * blockDim.x) {
+    const int plane = (int)(u / units_per_plane);
+    const long long up = u - (long long)plane * units_per_plane;
     int o = 0;
 #pragma unroll
     for (int k = 1; k < 4; ++k)
-      if (wp >= g.v[k].packed_off) o = k;
+      if (up >= g.v[k].packed_off / np) o = k;
     const ViewGeom& v = g.v[o];
-    const long long rem = wp - v.packed_off;
-    const int b = (int)(rem / v.view_words);
-    const int idx = (int)(rem - (long long)b * v.view_words);
-    // plain view first, then (if enabled) the two eroded views: E2 = pixel & right neighbour, D2 = pixel & lower-right
-    // neighbour (both across word boundaries)
-    const int which = v.e2_view_off > 0 ? idx / v.e2_view_off : 0;        // 0 plain, 1 E2, 2 D2
-    const int idx1 = idx - which * v.e2_view_off;
-    const int r = idx1 / v.stride, i = idx1 - r * v.stride;
+    const int pv = v.view_words / np;                          // words of one plane of one image
+    const long long rem = up - v.packed_off / np;
+    const int b = (int)(rem / pv);
+    const int idx = (int)(rem - (long long)b * pv);
+    const int r = idx / v.stride, i = idx - r * v.stride;
     const int rows = v.n_bands * g.band_rows + g.m;
-    uint32_t word = 0;
-    if (b < B && r < rows && which < 3) {
+    uint32_t w00 = 0, e2 = 0, d2 = 0;
+    if (b < B && r < rows) {
       const uint32_t* bimg = base + ((size_t)plane * B + b) * img_words;
       // source row of a view row: views 0, 3: image row yv (Brow); view 1: image column yv; view 2: column -yv
       auto source_row = [&](int rr, int* words) -> const uint32_t* {
@@ -140,23 +142,26 @@ __global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restr
         return bimg + (size_t)g.H * Wc + (size_t)c * Hc;
       };
       int words;
-      const uint32_t* srow = source_row(r, &words);
-      word = view_word(srow, words, o, v.Wv, i);
-      if (which == 1) {
-        const uint32_t next = (i + 1 < v.stride) ? view_word(srow, words, o, v.Wv, i + 1) : 0u;
-        word &= __funnelshift_r(word, next, 1);
-      } else if (which == 2) {
-        uint32_t below = 0;
+      const uint32_t* s0 = source_row(r, &words);
+      w00 = view_word(s0, words, o, v.Wv, i);
+      if (np == 3) {
+        const bool more = i + 1 < v.stride;
+        const uint32_t w01 = more ? view_word(s0, words, o, v.Wv, i + 1) : 0u;
+        e2 = w00 & __funnelshift_r(w00, w01, 1);
         if (r + 1 < rows) {
           const uint32_t* s1 = source_row(r + 1, &words);
-          const uint32_t lo = view_word(s1, words, o, v.Wv, i);
-          const uint32_t hi = (i + 1 < v.stride) ? view_word(s1, words, o, v.Wv, i + 1) : 0u;
-          below = __funnelshift_r(lo, hi, 1);
+          const uint32_t w10 = view_word(s1, words, o, v.Wv, i);
+          const uint32_t w11 = more ? view_word(s1, words, o, v.Wv, i + 1) : 0u;
+          d2 = w00 & __funnelshift_r(w10, w11, 1);
         }
-        word &= below;
       }
     }
-    packed[w] = word;
+    uint32_t* dst = packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b * v.view_words + idx;
+    dst[0] = w00;
+    if (np == 3) {
+      dst[v.e2_view_off] = e2;
+      dst[2 * (size_t)v.e2_view_off] = d2;
+    }
   }
 }
 
@@ -743,7 +748,7 @@ cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed,
   pack_base_kernel<<<(unsigned)blocks, 256, 0, st>>>(images, base, B, g.H, g.W, n_phase, phase0, counter);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  const long long total = (long long)n_phase * g.plane_words;
+  const long long total = (long long)n_phase * g.plane_words / (g.v[0].e2_view_off > 0 ? 3 : 1);
   blocks = (total + 255) / 256;
   blocks = std::max(1ll, std::min(blocks, (long long)n_sm * 32));
   pack_views_kernel<<<(unsigned)blocks, 256, 0, st>>>(base, packed, g, B, n_phase);
