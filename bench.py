@@ -102,7 +102,7 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_sample(w, imgs, seconds_hint, rng_seed=0, n_vec=None):
+def oracle_sample(w, imgs, seconds_hint, rng_seed=0, n_vec=None, threads=None):
     """The oracle as it stands on a bounded sample of the workload: a random subset of template vectors
     (all start pixels, all phases of the workload) on the first image. Returns (tests, seconds, cores, what)."""
     from oracle import lpf_oracle as orc
@@ -115,7 +115,8 @@ def oracle_sample(w, imgs, seconds_hint, rng_seed=0, n_vec=None):
     t0 = time.perf_counter()
     cores = 1
     for phase in ((0, 1) if w["n_phase"] == 2 else (1,)):
-        _, cores = orc.counts_list(img, phase, vecs, threads=os.cpu_count() or 1)   # all host cores, whatever OMP_NUM_THREADS torchrun set
+        # all host cores by default, whatever OMP_NUM_THREADS torchrun set
+        _, cores = orc.counts_list(img, phase, vecs, threads=threads or os.cpu_count() or 1)
     dt = time.perf_counter() - t0
     tests = n_vec * w["H"] * w["W"] * w["n_phase"]
     what = "%d random template vectors x all %dx%d start pixels x %d phase(s) of image 0" % (
@@ -469,6 +470,9 @@ def main():
         tests, dt, cores, what = oracle_sample(w, r["imgs"], 20)
         line["cpu_baseline"] = {"value": tests / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what,
                                 "seconds": dt}
+        # the paper's CPU column is sequential (one core): the same oracle on one thread, smaller sample
+        t1, d1, c1, w1 = oracle_sample(w, r["imgs"], 5, n_vec={2: 800, 3: 200, 4: 2500}[w["cfg"]], threads=1)
+        line["cpu_baseline"]["one_thread"] = {"value": t1 / d1, "cores": c1, "sample": w1, "seconds": d1}
     if args.tab1 and rank == 0 and world == 1:
         rows = run_tab1(lpf, torch, local_rank, os.path.join(ROOT, "gpurun_out"))
         line["tab1"] = {"rows": len(rows), "written_to": "gpurun_out/tab1.json, gpurun_out/tab1.md"}
