@@ -1,7 +1,7 @@
 // lpf_kernels.cu -- CUDA kernels of liblpf.so (sm_100a).
 //   pack_base_kernel  uint8 image -> row-major and column-major bit images, 32 px / word, one coalesced pass
-//   pack_views_kernel the four octant views per image, each with its periodic halo laid out exactly as the
-//                     eval kernel wants it in shared memory (a2)
+//   pack_views_kernel the four octant views per image (plain, and the eroded planes E2 / D2), each with its periodic
+//                     halo laid out exactly as the eval kernel wants it in shared memory (a2)
 //   eval_kernel_v3<.> the hot loop: walk the node program with a running AND mask (a3), POPC +
 //                     warp reduce at terminals (a4), optional zero-mask pruning (a5)
 //   mirror_kernel     counts[-v] = counts[v] (a6)
@@ -214,6 +214,10 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, unsigne
 //   Saved masks of the depth-first walk live in LOCAL memory (saves/restores are ~2.6 % of the nodes each;
 //   the lines stay in L1), so the hot loop carries no stack registers and shared memory holds only the
 //   bands: 4-5 CTAs per SM instead of 2 (measured: config 3 15.4 -> 11.6 ms against a shared-memory stack).
+//   The kernel does not know about planes: in eroded mode shared memory holds the E2 and
+//   the D2 band instead of the plain one, an entry's offset field already points into the right plane, and one
+//   window then covers two path pixels.  PAIR entries fold their window into the next entry's 3-input AND.
+//   The mask of an item is initialised once, before the loop (INIT is only ever an item's first entry).
 // ---------------------------------------------------------------------------------------------
 template <int TX, int TY, bool PRUNE>
 __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
