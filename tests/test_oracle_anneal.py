@@ -77,4 +77,79 @@ def test_local_delta_form_equals_literal_form(phase):
     b = orc.anneal(start, phase, m, target, pairs, log_u, T_max, 0.01 * T_max, 15, 5, use_local=True)
     assert np.array_equal(a[3], b[3]) and np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and a[2] == b[2]
     assert 0 < a[3].sum() < N                                   # the run exercised accept and reject
-    assert a[2]["E"] <= E0 or True
+
+
+# ---- the Metropolis rule at FINITE temperature (Alg. 3 line 11; reading A3) ----------
+# The expected decision never comes from the oracle's annealing code: E_P and E_Q are Python-integer sums over the
+# canonical half D (Eq. 13 / Eq. 19) of descriptors of numpy-built images, the threshold is the exact rational
+# (E_P - E_Q) / ((W*H)^2 * T), and ln u is placed a relative 1e-9 on either side of it.  A dropped (W*H)^2, W^4 in its
+# place, T^2, the full-array error instead of the half, or a flipped sign moves the threshold by far more than that.
+
+def _half_E(img, target, phases, m):
+    """Eq. 19 over D and the phases, exact Python integers, from descriptors of `img` (not from the annealing code)."""
+    E = 0
+    for i, ph in enumerate(phases):
+        c = orc.counts(img, ph, m)
+        for dy in range(0, m + 1):
+            for dx in range(-m, m + 1):
+                if dy > 0 or dx >= 0:                           # D of Eq. 13 (PAPER.md:154)
+                    d = int(target[i][dy + m, dx + m]) - int(c[dy + m, dx + m])
+                    E += d * d
+    return E
+
+
+def _swapped(img, pair):
+    xp, yp, xq, yq = (int(v) for v in pair)
+    q = img.copy()
+    q[yp, xp], q[yq, xq] = img[yq, xq], img[yp, xp]             # x indexes columns, y rows (reading S2)
+    return q
+
+
+@pytest.mark.parametrize("H,W,m,phase,T", [(6, 9, 3, 1, 0.37), (9, 6, 4, -1, 2.5e-3), (5, 8, 4, 0, 11.0)])
+def test_metropolis_threshold_at_finite_temperature(H, W, m, phase, T):
+    from fractions import Fraction
+    start, target, pairs, _, phases = _setup(H, W, m, phase, 31 + H, 40)
+    seen_worse = seen_better = 0
+    for pr in pairs:
+        if start[pr[1], pr[0]] == start[pr[3], pr[2]]:
+            continue                                            # identity move: E_P = E_Q, threshold 0
+        E_P = _half_E(start, target, phases, m)
+        E_Q = _half_E(_swapped(start, pr), target, phases, m)
+        if E_P == E_Q:
+            continue
+        r = Fraction(E_P - E_Q, (W * H) ** 2) / Fraction(T)     # exact: T is a binary rational
+        seen_worse += E_Q > E_P
+        seen_better += E_Q < E_P
+        for rel, want in ((1e-9, r < 0), (-1e-9, r > 0)):       # ln u = r (1 + rel): below r iff rel has the sign of -r
+            lu = float(r) * (1.0 + rel)
+            want_acc = Fraction(lu) < r
+            assert want_acc == want
+            _, _, st, log = orc.anneal(start, phase, m, target, pr[None], np.array([lu]), T, T, 5, 5)
+            assert bool(log[0]) == want_acc, (pr, E_P, E_Q, lu)
+            assert st["accepted"] == int(want_acc) and st["E"] == (E_Q if want_acc else E_P)
+    assert seen_worse >= 3 and seen_better >= 3                 # both signs of the threshold were exercised
+
+
+def test_metropolis_threshold_follows_the_temperature_schedule():
+    """Second proposal of a chain with c_max = 1: the level ends after the first, so T = T_max * T_mult (Alg. 3
+    lines 4 and 17, reading A2) enters the second threshold."""
+    from fractions import Fraction
+    H, W, m, phase = 7, 10, 4, -1
+    start, target, pairs, _, phases = _setup(H, W, m, phase, 77, 60)
+    T_max, T_min, s_max, N = 0.8, 0.05, 3, 2
+    T2 = T_max * (T_min / T_max) ** (s_max / N)
+    done = 0
+    for k in range(0, 58):
+        two = pairs[k:k + 2]
+        P1 = _swapped(start, two[0])                            # the first proposal is always accepted (ln u = -inf)
+        E_P, E_Q = _half_E(P1, target, phases, m), _half_E(_swapped(P1, two[1]), target, phases, m)
+        if E_P == E_Q:
+            continue
+        r = Fraction(E_P - E_Q, (W * H) ** 2) / Fraction(T2)
+        for rel in (1e-9, -1e-9):
+            lu = float(r) * (1.0 + rel)
+            _, _, st, log = orc.anneal(start, phase, m, target, two, np.array([-np.inf, lu]), T_max, T_min, 1, s_max)
+            assert bool(log[0]) and bool(log[1]) == (Fraction(lu) < r)
+            assert st["levels"] == 2 and st["T"] == T2 * (T_min / T_max) ** (s_max / N)
+        done += 1
+    assert done >= 20

@@ -69,3 +69,27 @@ def test_swap_pairs_generator_contract():
     pr = inputs.swap_pairs(img, 500, 6)
     assert pr.shape == (500, 4) and pr.dtype == np.int32
     assert np.all(img[pr[:, 1], pr[:, 0]] == 0) and np.all(img[pr[:, 3], pr[:, 2]] == 1)
+
+
+def test_swap_delta_full_pixel_convention_against_numpy_built_image():
+    """(x_p, y_p) addresses column x_p of row y_p (reading S2; Eq. 6 `x%W, y%H`): the oracle's delta equals
+    counts(I') - counts(I) with I' built here with numpy indexing, on a NON-square image and a pair whose transposed
+    reading (x <-> y) is in range too and gives a different answer."""
+    H, W, m = 7, 11, 5
+    img = inputs.bernoulli(H, W, 0.6, 4242)
+    zeros = [(x, y) for y in range(H) for x in range(W) if img[y, x] == 0 and x < H and y < W and x != y]
+    ones = [(x, y) for y in range(H) for x in range(W) if img[y, x] == 1 and x < H and y < W and x != y]
+    checked = 0
+    for (xp, yp), (xq, yq) in zip(zeros[:6], ones[:6]):
+        q = img.copy()
+        q[yp, xp], q[yq, xq] = img[yq, xq], img[yp, xp]
+        tr = img.copy()                                          # the transposed (wrong) reading of the same pair
+        tr[xp, yp], tr[xq, yq] = img[xq, yq], img[xp, yp]
+        for phase in (0, 1):
+            want = orc.counts(q, phase, m, full_template=True) - orc.counts(img, phase, m, full_template=True)
+            wrong = orc.counts(tr, phase, m, full_template=True) - orc.counts(img, phase, m, full_template=True)
+            got = orc.swap_delta_full(img, phase, m, (xp, yp, xq, yq))
+            assert np.array_equal(got, want)
+            assert np.array_equal(orc.swap_delta_local(img, phase, m, (xp, yp, xq, yq)), want)
+            checked += not np.array_equal(want, wrong)
+    assert checked >= 6                                          # the cases do tell the two readings apart
