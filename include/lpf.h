@@ -22,10 +22,17 @@
  *     owns only what lives inside lpf_paths (the path/trie tables and a packed-image
  *     workspace that grows on demand).
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
- *     entry points are asynchronous on that stream and do not synchronise the host, except
- *     that the first call for a new (B,H,W) shape may cudaMalloc workspace.
- *   - One lpf_paths object must not be used from two streams/threads at the same time (the
- *     workspace is shared).
+ *     entry points are asynchronous on that stream.  lpf_build_paths and lpf_reserve are the
+ *     only calls that allocate device memory, upload tables or synchronise the host: after
+ *     lpf_reserve for a shape, lpf_eval / lpf_eval_both / lpf_eval_masked / lpf_eval_sum /
+ *     lpf_swap_delta on that shape ONLY enqueue kernels and memsets on `stream` (they can be
+ *     captured into a CUDA graph).  A call for a shape that was never reserved reserves it
+ *     first, i.e. that one call allocates and synchronises.
+ *   - The `const lpf_paths*` of the hot calls: the path table is never modified; the object's
+ *     internal caches (plans, workspace, last-launch record) are, so one lpf_paths must not be
+ *     used from two host threads at the same time.  Using it from several STREAMS is safe:
+ *     consecutive calls share one workspace, so a call on another stream than the previous
+ *     call's makes its stream wait, on the device, for the previous call's work.
  *   - There is no CPU fallback: a device entry point called on a table built with
  *     device < 0 returns LPF_E_INVAL.
  */
@@ -58,6 +65,14 @@ extern "C" {
 #define LPF_NO_E2    8u   /* measurement: walk every node on the plain bit plane instead of the two eroded planes
                              (pixel & right neighbour, pixel & lower-right neighbour).
                              Same counts. */
+
+/* `what` of lpf_reserve */
+#define LPF_FOR_EVAL        1u   /* lpf_eval and one-phase lpf_eval_sum with (B, H, W, flags) */
+#define LPF_FOR_EVAL_BOTH   2u   /* lpf_eval_both and two-phase lpf_eval_sum */
+#define LPF_FOR_MASKED      4u   /* together with one of the above: lpf_eval_masked (one phase / both) instead */
+#define LPF_FOR_SWAP_DELTA  8u   /* lpf_swap_delta on H x W images (B, flags unused) */
+#define LPF_FOR_ANNEAL     16u   /* lpf_anneal on H x W images (B, flags unused) */
+#define LPF_FOR_HOST       32u   /* lpf_eval_host with (B, H, W, flags), one phase or both */
 
 typedef struct lpf_paths lpf_paths;   /* opaque: path table + prefix trie + device programs for one m */
 
@@ -108,6 +123,15 @@ int  lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, unsigned fla
                        uint64_t* entries, int64_t cap_entries, int64_t* n_entries,
                        int64_t* items, int64_t cap_items, int64_t* n_items, int* n_slots, int* strides);
 
+/* The rest of paper "step 1" for one image shape (step 1 is executed once, steps 2-3 "are called
+ * repeatedly ... for new binary images of the same dimensions"): cuts the tries into the work items of a B x H x W
+ * batch, linearises and uploads the node program, sizes every device workspace the named calls need and fixes their
+ * launch configuration.  `what` is an OR of LPF_FOR_*; `flags` are the eval flags the later calls will pass.
+ * Synchronous (allocates, copies, synchronises the device).  After it the named calls on that shape only enqueue work
+ * on their stream.  May be called any number of times; a larger shape grows the workspace (the device is synchronised
+ * first, so work in flight is safe).  Errors: INVAL, UNSUPPORTED, NOMEM, CUDA as for the calls themselves. */
+int  lpf_reserve(lpf_paths* p, int B, int H, int W, unsigned flags, unsigned what);
+
 /* Paper "steps 2-3" (Alg. 1 / Alg. 2) for a batch of B independent images
  * of one size: translate every segment over every start pixel, compare, count.
  *   images  dev uint8 [B][H][W]; a pixel is in phase phi iff its byte == phi
@@ -115,7 +139,7 @@ int  lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, unsigned fla
  *           (the half outside D is the mirror counts[-v] = counts[v])
  * Errors: INVAL (see above; m > min(H,W)-1 is rejected because a path would wrap onto itself,
  * and D stops at W-1,H-1: PAPER.md:154), UNSUPPORTED, NOMEM, CUDA. */
-int  lpf_eval(lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase,
+int  lpf_eval(const lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase,
               int64_t* counts, unsigned flags, void* stream);
 
 /* Monte-Carlo / N-position approximation L2~ (used in Eq. 14): the segments are compared with the
@@ -126,12 +150,21 @@ int  lpf_eval(lpf_paths* p, const uint8_t* images, int B, int H, int W, int phas
  * divides by its N); the half outside D repeats it point-symmetrically, as the descriptor is stored in the paper
  * -- with a proper subset of starts the definition itself is not symmetric (reading S16).
  * A mask of all non-zero bytes gives exactly lpf_eval.  Same errors as lpf_eval. */
-int  lpf_eval_masked(lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase, const uint8_t* start_mask,
-                     int64_t* counts, unsigned flags, void* stream);
+int  lpf_eval_masked(const lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase,
+                     const uint8_t* start_mask, int64_t* counts, unsigned flags, void* stream);
 
 /* Both phases in one call: counts dev int64 [B][2][2m+1][2m+1], index [b][phase][dy+m][dx+m]. */
-int  lpf_eval_both(lpf_paths* p, const uint8_t* images, int B, int H, int W,
+int  lpf_eval_both(const lpf_paths* p, const uint8_t* images, int B, int H, int W,
                    int64_t* counts, unsigned flags, void* stream);
+
+/* Ensemble descriptor of an image stack (the descriptor of the bone specimen is "averaged over 100
+ * slices", ergodicity): counts_sum[v] = sum over the B images of count(image_b, v), accumulated on the device into ONE
+ * array without materialising the per-image counts; the ensemble average of L2 is counts_sum / (B*W*H), one division
+ * done by the caller.  With LPF_S2 the same for the two-point probability.
+ *   phase 0 | 1: counts_sum dev int64 [2m+1][2m+1];  -1: both phases, dev int64 [2][2m+1][2m+1].
+ * Same errors as lpf_eval. */
+int  lpf_eval_sum(const lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase,
+                  int64_t* counts_sum, unsigned flags, void* stream);
 
 /* Least-square objective, Eq. 14 / Eq. 19 on integer counts:
  *   sse[b] = sum_k (counts[b][k] - target[k])^2, exact in uint64 (wraps mod 2^64 if it overflows;
@@ -148,7 +181,7 @@ int  lpf_objective(const int64_t* counts, const int64_t* target, int B, int64_t 
  * call still returns LPF_OK (no host sync) -- validate on the host if needed.
  * UNSUPPORTED when the bit image with its halo of m pixels, (H+2m) x ceil((W+2m)/32) words, plus 32 KB of warp stacks
  * does not fit the shared memory of one block, or when the trie has 2^24 nodes or more (m > ~380). */
-int  lpf_swap_delta(lpf_paths* p, const uint8_t* image, int H, int W, int phase,
+int  lpf_swap_delta(const lpf_paths* p, const uint8_t* image, int H, int W, int phase,
                     const int32_t* pairs, int64_t n, int32_t* delta, void* stream);
 
 /* Simulated annealing of Alg. 3 with the two-pixel swap and the least-square
@@ -169,22 +202,26 @@ int  lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase, const int
                 int64_t* counts, uint8_t* accept_log, double* stats5, void* stream);
 
 /* HOST-buffer convenience used by the end-to-end measurement: copies `images` (host, pinned or
- * not) to the device, runs lpf_eval(_both if phase < 0), copies counts back, synchronises. */
+ * not) to the device on a private stream (ordered after earlier work on this table), runs lpf_eval (_both if
+ * phase < 0), copies counts back, synchronises that stream.  Staging buffers: lpf_reserve with LPF_FOR_HOST. */
 int  lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, int H, int W, int phase,
                    int64_t* counts_host, unsigned flags);
 
 /* Counters of the most recent lpf_eval / lpf_eval_both on this object (host values known at
  * launch time): kernels launched, work items, program entries walked per image-phase, grid,
- * block, dynamic shared memory bytes, thread tile code (1000 TX + 100 TY + mask-stack slots), images per CTA.
- * out = host int64[8]. */
-int  lpf_last_launch_info(const lpf_paths* p, int64_t* out8);
+ * block, dynamic shared memory bytes, thread tile code (1000 TX + 100 TY + mask-stack slots), images per CTA,
+ * 1 if the eroded planes E2 / D2 were walked (0: the plain plane); then what the walker executes per image-phase and
+ * per start WORD, counted by replaying its loop over the program on the host: pairs of entries folded into one
+ * 3-input AND (2 SHF + 1 LOP3 each), entries executed on their own (1 SHF + 1 LOP3), terminal entries (1 POPC +
+ * 1 add), and the trie nodes per program piece.  out = host int64[13]. */
+int  lpf_last_launch_info(const lpf_paths* p, int64_t* out13);
 
 /* Measurement hook: with enable != 0 every lpf_eval / lpf_eval_both on this object
  * records one CUDA event before and one after the eval kernel (the dominant kernel) on the caller's
  * stream; lpf_last_eval_kernel_ms waits for the second event and returns the elapsed device time of
  * the most recent eval kernel in milliseconds.  INVAL if no timed eval has been issued. */
 int  lpf_set_timing(lpf_paths* p, int enable);
-int  lpf_last_eval_kernel_ms(lpf_paths* p, float* ms);
+int  lpf_last_eval_kernel_ms(const lpf_paths* p, float* ms);
 
 /* Measurement hook: runs a few milliseconds of register-only
  * integer instructions on every SM of `device` (synchronous, default stream) and returns the measured thread-level

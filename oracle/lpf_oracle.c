@@ -35,7 +35,9 @@
  * lpf_oracle_counts_masked (L2~): all-ones mask = lpf_oracle_counts_list, additivity over disjoint
  * masks, one-pixel masks vs the definition.  lpf_oracle_s2_counts (Eq. 6): numpy FFT form of Eq. 7, S2(0) = phase
  * count, point symmetry, equality with the lineal-path counts for the 8 neighbours (|P_v| = 2).
- * lpf_oracle_anneal (Alg. 3): volume fractions preserved, E tracked = Eq. 19 of the final image re-evaluated, a huge
+ * lpf_oracle_counts_sum (ensemble over a stack): one image = lpf_oracle_counts, additive over a split of
+ * the stack, k copies of the worked image = k times its golden counts, Eq. 10 summed (centre = phase pixels of the stack).
+ * lpf_oracle_anneal (Alg. 3): the Metropolis threshold at finite T against exact rationals computed in the test, volume fractions preserved, E tracked = Eq. 19 of the final image re-evaluated, a huge
  * T accepts every move (final image = all swaps applied, temperature levels = floor(N / s_max)), a tiny T never lets E
  * grow, the local-delta form equals the literal re-evaluation form decision by decision.
  * Parity with the AUTHORS' numbers is unpinned: the paper prints no L2 value.
@@ -175,6 +177,23 @@ int lpf_oracle_counts(const uint8_t *img, int H, int W, int phase, int m,
     }
     free(vecs); free(tmp);
     return used;
+}
+
+/* Ensemble descriptor of a stack of B images of one size (the descriptor of the specimen is "averaged
+ * over 100 slices"): sum_out[v] = sum_b count(image_b, v); the ensemble average of L2 is sum_out / (B*W*H), one division
+ * by the caller.  Plain loop over the images, each evaluated on its own by lpf_oracle_counts (canonical half + Eq. 12). */
+void lpf_oracle_counts_sum(const uint8_t *imgs, int B, int H, int W, int phase, int m,
+                           int64_t *sum_out, int threads)
+{
+    int S = 2 * m + 1;
+    size_t K = (size_t)S * S;
+    int64_t *one = (int64_t *)malloc(sizeof(int64_t) * K);
+    for (size_t k = 0; k < K; ++k) sum_out[k] = 0;
+    for (int b = 0; b < B; ++b) {
+        lpf_oracle_counts(imgs + (size_t)b * H * W, H, W, phase, m, one, 0, threads);
+        for (size_t k = 0; k < K; ++k) sum_out[k] += one[k];
+    }
+    free(one);
 }
 
 /* Eq. 14 / Eq. 19 on integer counts: sum_k (c_k - t_k)^2, exact.

@@ -48,6 +48,8 @@ def _load():
         lib.lpf_oracle_counts_list.restype = I
         lib.lpf_oracle_counts.argtypes = [c_u8p, I, I, I, I, c_i64p, I, I]
         lib.lpf_oracle_counts.restype = I
+        lib.lpf_oracle_counts_sum.argtypes = [c_u8p, I, I, I, I, I, c_i64p, I]
+        lib.lpf_oracle_counts_sum.restype = None
         lib.lpf_oracle_sse.argtypes = [c_i64p, c_i64p, ctypes.c_int64]
         lib.lpf_oracle_sse.restype = ctypes.c_uint64
         lib.lpf_oracle_swap_delta_full.argtypes = [c_u8p, I, I, I, I, I, I, I, I, c_i32p, I]
@@ -117,6 +119,18 @@ def counts(image, phase: int, m: int, full_template: bool = False, threads: int 
     return out
 
 
+def counts_sum(images, phase: int, m: int, threads: int = 0) -> np.ndarray:
+    """Ensemble sum over a stack [B, H, W]: int64 [2m+1, 2m+1]."""
+    a = np.ascontiguousarray(images, dtype=np.uint8)
+    if a.ndim != 3:
+        raise ValueError("images must be [B, H, W]")
+    S = 2 * int(m) + 1
+    out = np.zeros((S, S), dtype=np.int64)
+    _load().lpf_oracle_counts_sum(_p(a, ctypes.c_uint8), a.shape[0], a.shape[1], a.shape[2], int(phase), int(m),
+                                  _p(out, ctypes.c_int64), int(threads))
+    return out
+
+
 def counts_masked(image, mask, phase: int, vecs) -> np.ndarray:
     """L2~ counts: hits of each vector over the start pixels with mask != 0."""
     a = _img(image)
@@ -161,7 +175,8 @@ def anneal(image, phase: int, m: int, target, pairs, log_u, T_max: float, T_min:
 
 
 def half_sse(c, t, m: int) -> int:
-    """Eq. 19 over D (reading A4): sum over the canonical half of (t - c)^2, exact; numpy, for the tests."""
+    """Eq. 19 over D (reading A4): sum over the canonical half of (t - c)^2, exact.  The one piece of numpy arithmetic
+    in this binding: it is what the tests compare the C file's half_sse_ (inside lpf_oracle_anneal) against."""
     c = np.asarray(c, dtype=np.int64)
     t = np.asarray(t, dtype=np.int64)
     S = 2 * int(m) + 1

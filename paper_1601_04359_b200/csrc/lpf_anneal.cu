@@ -163,17 +163,17 @@ extern "C" int lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase,
   if (cudaGetDevice(&prev) != cudaSuccess) return LPF_E_CUDA;
   if (prev != p->device && cudaSetDevice(p->device) != cudaSuccess) return LPF_E_CUDA;
 
-  // batch size: at most 256 proposals and about 256 MB of delta arrays
-  int K_max = 256;
-  while (K_max > 8 && (long long)K_max * K2 * 4 * n_ph > (256ll << 20)) K_max /= 2;
-  AnnealState* d_state = nullptr;
-  int* d_batch = nullptr;
-  int* d_delta = nullptr;
-  long long* d_dE = nullptr;
-  cudaError_t e = cudaMalloc(&d_state, sizeof(AnnealState));
-  if (e == cudaSuccess) e = cudaMalloc(&d_batch, sizeof(int) * 4 * K_max);
-  if (e == cudaSuccess) e = cudaMalloc(&d_delta, sizeof(int) * (size_t)n_ph * K_max * K2);
-  if (e == cudaSuccess) e = cudaMalloc(&d_dE, sizeof(long long) * K_max);
+  // chain state, proposal batch, deltas and error changes live in the table (lpf_reserve with LPF_FOR_ANNEAL)
+  const int K_max = anneal_kmax(p->m, n_ph);
+  if (!p->d_an_state || p->an_delta_bytes < sizeof(int) * (size_t)n_ph * K_max * K2) {
+    rc = reserve_anneal(p, H, W);
+    if (rc != LPF_OK) { if (prev != p->device) cudaSetDevice(prev); return rc; }
+  }
+  AnnealState* d_state = (AnnealState*)p->d_an_state;
+  int* d_batch = p->d_an_batch;
+  int* d_delta = p->d_an_delta;
+  long long* d_dE = (long long*)p->d_an_dE;
+  cudaError_t e = cudaSuccess;
   AnnealState h{};
   h.T = T_max;                                                   // line 3
   h.acc_idx = -1;
@@ -226,10 +226,6 @@ extern "C" int lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase,
   stats5[2] = (double)h.levels;
   stats5[3] = h.T;
   stats5[4] = (double)h.E;
-  if (d_state) cudaFree(d_state);
-  if (d_batch) cudaFree(d_batch);
-  if (d_delta) cudaFree(d_delta);
-  if (d_dE) cudaFree(d_dE);
   if (prev != p->device) cudaSetDevice(prev);
   if (rc != LPF_OK) return rc;
   if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? LPF_E_NOMEM : LPF_E_CUDA;

@@ -1,6 +1,11 @@
 // lpf_api.cu -- C ABI entry points of liblpf.so that touch the device (include/lpf.h).
 // Host logic only: argument checks, geometry, workspace, program upload, launches.  Every step
 // of the hot path runs in the kernels of lpf_kernels.cu.
+//
+// Allocation discipline ("no hidden host sync except in lpf_build_paths"): everything that
+// allocates, uploads or synchronises lives in lpf_reserve (reserve_* below).  The hot calls look their shape up in
+// p->plans and only enqueue kernels and memsets on the caller's stream; a call for a shape that was never reserved
+// reserves it first (documented in lpf.h) -- after that first call it is a pure enqueue as well.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -16,7 +21,7 @@ int build_host_table(lpf_paths* p);   // lpf_paths.cpp
 
 static thread_local int g_last_cuda = 0;
 
-static int cuda_fail(cudaError_t e) {
+int cuda_fail(cudaError_t e) {
   g_last_cuda = (int)e;
   (void)cudaGetLastError();
   return e == cudaErrorMemoryAllocation ? LPF_E_NOMEM : LPF_E_CUDA;
@@ -40,49 +45,70 @@ struct DeviceGuard {   // binds the calling thread to the table's device for the
   }
 };
 
+// Consecutive calls on one lpf_paths share its workspace.  A call on a stream other than the previous call's first
+// makes its stream wait (on the device) for the event recorded after that call; nothing blocks the host.  While a
+// stream is being captured into a CUDA graph neither the wait nor the record is issued: the graph's own order holds.
+struct StreamOrder {
+  lpf_paths* p;
+  cudaStream_t st;
+  bool capturing = false;
+  cudaError_t err = cudaSuccess;
+  StreamOrder(lpf_paths* p_, cudaStream_t st_) : p(p_), st(st_) {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    err = cudaStreamIsCapturing(st, &cs);
+    capturing = cs != cudaStreamCaptureStatusNone;
+    if (err == cudaSuccess && !capturing && p->last_stream_valid && p->last_stream != (void*)st)
+      err = cudaStreamWaitEvent(st, (cudaEvent_t)p->ev_done, 0);
+  }
+  cudaError_t done() {
+    if (capturing) return cudaSuccess;
+    p->last_stream = (void*)st;
+    p->last_stream_valid = 1;
+    return cudaEventRecord((cudaEvent_t)p->ev_done, st);
+  }
+};
+
+// growing a workspace buffer: work already enqueued may still read the old one
+template <typename T>
+static int grow(T** buf, size_t* have, size_t need) {
+  if (need <= *have && *buf) return LPF_OK;
+  if (*buf) {
+    LPF_CUDA(cudaDeviceSynchronize());
+    cudaFree(*buf);
+    *buf = nullptr;
+    *have = 0;
+  }
+  LPF_CUDA(cudaMalloc((void**)buf, std::max<size_t>(need, 16)));
+  *have = need;
+  return LPF_OK;
+}
+
 static void free_program(Program& pr) {
   if (pr.d_entries) cudaFree(pr.d_entries);
   if (pr.d_skip) cudaFree(pr.d_skip);
-  if (pr.d_work) cudaFree(pr.d_work);
-  pr.d_entries = nullptr; pr.d_skip = nullptr; pr.d_work = nullptr;
+  pr.d_entries = nullptr;
+  pr.d_skip = nullptr;
 }
 
-// uploads the program (once) and the work list expanded over (row band, strip band) of each octant
-static int upload_program(Program& pr, const Geom& g) {
-  if (!pr.d_entries) {
-    // +64: the walker fetches 32 entries per warp, one chunk ahead
-    LPF_CUDA(cudaMalloc(&pr.d_entries, sizeof(uint64_t) * (pr.entries.size() + 64)));
-    LPF_CUDA(cudaMalloc(&pr.d_skip, sizeof(uint32_t) * std::max<size_t>(pr.skip.size(), 1)));
-    LPF_CUDA(cudaMemset(pr.d_entries, 0, sizeof(uint64_t) * (pr.entries.size() + 64)));
-    LPF_CUDA(cudaMemcpy(pr.d_entries, pr.entries.data(), sizeof(uint64_t) * pr.entries.size(), cudaMemcpyHostToDevice));
-    LPF_CUDA(cudaMemcpy(pr.d_skip, pr.skip.data(), sizeof(uint32_t) * pr.skip.size(), cudaMemcpyHostToDevice));
+// uploads the program once; the device pointers are published only when every step has succeeded
+static int upload_program(Program& pr) {
+  if (pr.d_entries) return LPF_OK;
+  uint64_t* d_e = nullptr;
+  uint32_t* d_s = nullptr;
+  const size_t ne = pr.entries.size() + 64;      // +64: the walker fetches 32 entries per warp, one chunk ahead
+  cudaError_t e = cudaMalloc(&d_e, sizeof(uint64_t) * ne);
+  if (e == cudaSuccess) e = cudaMalloc(&d_s, sizeof(uint32_t) * std::max<size_t>(pr.skip.size(), 1));
+  if (e == cudaSuccess) e = cudaMemset(d_e, 0, sizeof(uint64_t) * ne);
+  if (e == cudaSuccess)
+    e = cudaMemcpy(d_e, pr.entries.data(), sizeof(uint64_t) * pr.entries.size(), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(d_s, pr.skip.data(), sizeof(uint32_t) * pr.skip.size(), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    if (d_e) cudaFree(d_e);
+    if (d_s) cudaFree(d_s);
+    return cuda_fail(e);
   }
-  int bands[4];
-  bool same = pr.d_work != nullptr;
-  for (int o = 0; o < 4; ++o) {
-    const int sb = (g.v[o].n_strips + g.SB - 1) / g.SB;
-    bands[o] = g.v[o].n_bands * 65536 + sb;
-    same = same && bands[o] == pr.work_bands[o];
-  }
-  if (same) return LPF_OK;
-  if (pr.d_work) { cudaFree(pr.d_work); pr.d_work = nullptr; }
-  std::vector<int32_t> work;
-  const size_t n_items = pr.items.size() / 4;
-  for (size_t i = 0; i < n_items; ++i) {           // items are sorted big first; keep that order
-    const int o = (int)pr.items[4 * i + 2];
-    const int sb = (g.v[o].n_strips + g.SB - 1) / g.SB;
-    for (int band = 0; band < g.v[o].n_bands; ++band)
-      for (int s = 0; s < sb; ++s) {
-        work.push_back((int32_t)pr.items[4 * i]);
-        work.push_back((int32_t)pr.items[4 * i + 1]);
-        work.push_back(o | (s << 4));
-        work.push_back(band);
-      }
-  }
-  pr.n_work = (int64_t)work.size() / 4;
-  LPF_CUDA(cudaMalloc(&pr.d_work, sizeof(int32_t) * std::max<size_t>(work.size(), 4)));
-  LPF_CUDA(cudaMemcpy(pr.d_work, work.data(), sizeof(int32_t) * work.size(), cudaMemcpyHostToDevice));
-  for (int o = 0; o < 4; ++o) pr.work_bands[o] = bands[o];
+  pr.d_entries = d_e;
+  pr.d_skip = d_s;
   return LPF_OK;
 }
 
@@ -108,7 +134,10 @@ extern "C" int lpf_build_paths(int m, int device, lpf_paths** out) {
     cudaDeviceProp prop;
     cudaError_t e = g.ok ? cudaGetDeviceProperties(&prop, device) : cudaErrorInvalidDevice;
     if (e == cudaSuccess) e = cudaMalloc(&p->d_counter, sizeof(unsigned int) * 4);
-    if (e != cudaSuccess) { rc = cuda_fail(e); delete p; return rc; }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags((cudaEvent_t*)&p->ev_done, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreate((cudaEvent_t*)&p->ev_start);
+    if (e == cudaSuccess) e = cudaEventCreate((cudaEvent_t*)&p->ev_stop);
+    if (e != cudaSuccess) { rc = cuda_fail(e); lpf_free_paths(p); return rc; }
     p->n_sm = prop.multiProcessorCount;
     p->max_smem = (int)prop.sharedMemPerBlockOptin;
   }
@@ -120,68 +149,85 @@ extern "C" void lpf_free_paths(lpf_paths* p) {
   if (!p) return;
   if (p->device >= 0) {
     DeviceGuard g(p->device);
+    cudaDeviceSynchronize();
     for (auto& kv : p->programs) free_program(kv.second);
+    for (auto& kv : p->plans)
+      if (kv.second.d_work) cudaFree(kv.second.d_work);
     if (p->d_packed) cudaFree(p->d_packed);
     if (p->d_counter) cudaFree(p->d_counter);
     if (p->d_swap_rec) cudaFree(p->d_swap_rec);
     if (p->d_swap_bits) cudaFree(p->d_swap_bits);
+    if (p->d_an_state) cudaFree(p->d_an_state);
+    if (p->d_an_batch) cudaFree(p->d_an_batch);
+    if (p->d_an_delta) cudaFree(p->d_an_delta);
+    if (p->d_an_dE) cudaFree(p->d_an_dE);
     if (p->d_io_in) cudaFree(p->d_io_in);
     if (p->d_io_out) cudaFree(p->d_io_out);
     if (p->io_stream) cudaStreamDestroy((cudaStream_t)p->io_stream);
+    if (p->ev_done) cudaEventDestroy((cudaEvent_t)p->ev_done);
     if (p->ev_start) cudaEventDestroy((cudaEvent_t)p->ev_start);
     if (p->ev_stop) cudaEventDestroy((cudaEvent_t)p->ev_stop);
   }
   delete p;
 }
 
-// ---- geometry ------------------------------------------------------------------------------------
+// ---- plans: everything that allocates, uploads or synchronises ----------------------------------------
 
 namespace lpf {
 
-cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed, const Geom& g, int B, int n_phase,
-                        int phase0, unsigned int* counter, int n_sm, cudaStream_t st);
-cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem, int* blocks_per_sm);
+cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed, const Geom& g, int B, int Bpad,
+                        int n_phase, int phase0, unsigned int* counter, int n_sm, cudaStream_t st);
+cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem, int max_smem, int* blocks_per_sm);
 cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st);
 cudaError_t launch_mirror(unsigned long long* counts, int S, long long n_arrays, int n_sm, cudaStream_t st);
 cudaError_t launch_objective(const long long* counts, const long long* target, int B, long long K,
                              unsigned long long* sse, int n_sm, cudaStream_t st);
+cudaError_t swap_delta_prepare(size_t smem);
 cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W, int m, int phase, const int* pairs,
                               long long n, const int32_t* rec, int n_nodes, int* delta, long long plane_stride,
                               unsigned int* counter, int n_sm, cudaStream_t st);
 
-static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, int n_phase, int phase0,
-                     int64_t* counts, unsigned flags, void* stream, const uint8_t* start_mask = nullptr) {
-  if (!p || !images || !counts) return LPF_E_INVAL;
-  if (p->device < 0) return LPF_E_INVAL;
+static std::array<int64_t, 8> plan_key(const lpf_paths* p, int B, int H, int W, int n_phase, unsigned flags,
+                                       bool masked) {
+  return {B, H, W, n_phase, (int64_t)flags, masked ? 1 : 0, 100 * p->tile_tx + p->tile_ty, p->cta_warps};
+}
+
+static int check_eval_args(const lpf_paths* p, int B, int H, int W, unsigned flags) {
+  if (!p || p->device < 0) return LPF_E_INVAL;
   if (B < 1 || H < 1 || W < 1) return LPF_E_INVAL;
-  if (n_phase == 1 && phase0 != 0 && phase0 != 1) return LPF_E_INVAL;
   if (p->m > std::min(H, W) - 1) return LPF_E_INVAL;
   if (flags & ~(LPF_PRUNE | LPF_NO_TRIE | LPF_S2 | LPF_NO_E2)) return LPF_E_INVAL;
-  DeviceGuard dg(p->device);
-  if (!dg.ok) return LPF_E_CUDA;
-  cudaStream_t st = (cudaStream_t)stream;
-  Geom g;
+  return LPF_OK;
+}
+
+// builds the plan of one eval shape: geometry, program (built and uploaded), work list, launch configuration, and
+// grows the packed-image workspace.  The only place of the eval path that allocates, copies or synchronises.
+static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned flags, bool masked) {
+  const auto key = plan_key(p, B, H, W, n_phase, flags, masked);
+  if (p->plans.count(key)) return LPF_OK;
+  EvalPlan pl;
+  Geom& g = pl.g;
   // the eroded planes serve the trie program; m = 0 has nothing but the root, which only the plain program counts
   const bool use_e2 = !(flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)) && p->m >= 1;
-  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, use_e2, &g)) return LPF_E_UNSUPPORTED;
-  const int Bpad = (B + g.G - 1) / g.G * g.G;
+  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, use_e2, &g))
+    return LPF_E_UNSUPPORTED;
+  pl.Bpad = (B + g.G - 1) / g.G * g.G;
   long long off = 0;
   int work_per_item = 0;                           // (row band x strip band) pairs summed over the octants / 4
   for (int o = 0; o < 4; ++o) {
     g.v[o].packed_off = off;
-    off += (long long)Bpad * g.v[o].view_words;
+    off += (long long)pl.Bpad * g.v[o].view_words;
     work_per_item += g.v[o].n_bands * ((g.v[o].n_strips + g.SB - 1) / g.SB);
   }
   g.plane_words = off;
   work_per_item = std::max(1, work_per_item / 4);
-  const int n_gp = (Bpad / g.G) * n_phase;
+  pl.n_gp = (pl.Bpad / g.G) * n_phase;
 
-  // work items: about 20 per resident CTA (measured optimum on configs 2-4), pieces of 256 .. 16384 trie nodes; fewer mask slots than the
-  // kernel provides (a smaller piece needs fewer)
+  // work items: about 20 per resident CTA (measured optimum on configs 2-4), pieces of 256 .. 16384 trie nodes
   const int resident_guess = p->n_sm * 2;
   long long n_nodes = 0;
   for (int o = 0; o < 4; ++o) n_nodes += (long long)p->oct[o].size();
-  const long long want_items = std::max<long long>(1, 32ll * resident_guess / ((long long)n_gp * work_per_item));
+  const long long want_items = std::max<long long>(1, 32ll * resident_guess / ((long long)pl.n_gp * work_per_item));
   long long piece = n_nodes / want_items;
   piece = std::max<long long>(256, std::min<long long>(piece, 16384));
   int q = 256;
@@ -198,107 +244,297 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
       return LPF_E_NOMEM;
     }
     if (pr->n_slots <= STACK_SLOTS_BUDGET) break;
+    drop_program(p, pr);                           // needs more mask slots than the kernel has: not kept
     if (q <= 64) return LPF_E_UNSUPPORTED;
   }
   if (pr->entries.size() >= (size_t)1 << 30) return LPF_E_UNSUPPORTED;
-  int rc = upload_program(*pr, g);
+  DeviceGuard dg(p->device);
+  if (!dg.ok) return LPF_E_CUDA;
+  int rc = upload_program(*pr);
   if (rc != LPF_OK) return rc;
+  pl.pr = pr;
 
-  const bool prune = (flags & LPF_PRUNE) != 0;
-  const size_t smem_total = (size_t)g.smem_bytes;
+  // the work list: items expanded over (row band, strip band) of their octant, big items first
+  std::vector<int32_t> work;
+  const size_t n_items = pr->items.size() / 4;
+  for (size_t i = 0; i < n_items; ++i) {
+    const int o = (int)pr->items[4 * i + 2];
+    const int sb = (g.v[o].n_strips + g.SB - 1) / g.SB;
+    for (int band = 0; band < g.v[o].n_bands; ++band)
+      for (int s = 0; s < sb; ++s) {
+        work.push_back((int32_t)pr->items[4 * i]);
+        work.push_back((int32_t)pr->items[4 * i + 1]);
+        work.push_back(o | (s << 4));
+        work.push_back(band);
+      }
+  }
+  pl.n_work = (int64_t)work.size() / 4;
+  // the walker's loop replayed on the host (eval_kernel_v3: chunks of 32 entries, a PAIR entry that is not the last of
+  // its chunk is folded with its successor): the data operations the design executes per start word
+  pl.piece_nodes = q;
+  for (size_t i = 0; i < n_items; ++i) {
+    const int64_t first = pr->items[4 * i], cnt = pr->items[4 * i + 1];
+    for (int64_t c0 = 0; c0 < cnt; c0 += 32) {
+      const int n = (int)std::min<int64_t>(32, cnt - c0);
+      for (int k = 0; k < n; ++k) {
+        uint32_t x = (uint32_t)pr->entries[first + c0 + k];
+        if ((x & E_PAIR) && k + 1 < n) {
+          ++pl.fused_pairs;
+          ++k;
+          x = (uint32_t)pr->entries[first + c0 + k];
+        } else {
+          ++pl.singles;
+        }
+        if (x & E_TERMINAL) ++pl.terminals;
+      }
+    }
+    if ((uint32_t)(pr->entries[first] >> 32) & E_ROOTCOUNT_HI) ++pl.terminals;
+  }
+  const long long total_work = (long long)pl.n_work * pl.n_gp;
+  if (total_work >= (1ll << 32)) return LPF_E_UNSUPPORTED;
+
+  pl.prune = (flags & LPF_PRUNE) ? 1 : 0;
+  pl.smem = (size_t)g.smem_bytes;
   int occ = 0;
-  LPF_CUDA(eval_occupancy(g.TX, g.TY, prune, g.threads, smem_total, &occ));
+  LPF_CUDA(eval_occupancy(g.TX, g.TY, pl.prune != 0, g.threads, pl.smem, p->max_smem, &occ));
   if (occ < 1) return LPF_E_UNSUPPORTED;
-  const int resident = p->n_sm * occ;
+  pl.grid = (int)std::min<long long>(total_work, (long long)p->n_sm * occ);
 
-  // workspace: the packed octant views, then the compact row-major / column-major bit images of stage 1
-  const size_t views_bytes = (size_t)n_phase * (size_t)g.plane_words * 4;
-  const size_t base_words = (size_t)n_phase * B * ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32));
-  // ... and, for lpf_eval_masked, the views and the base bit images of the start mask (one image, one plane)
-  Geom gm = g;
-  size_t mask_views_bytes = 0, mask_base_bytes = 0;
-  if (start_mask) {
+  // workspace: the packed octant views, then the compact row-major / column-major bit images of stage 1, then (for
+  // lpf_eval_masked) the views and the base bit images of the start mask (one image, one plane)
+  pl.views_bytes = (size_t)n_phase * (size_t)g.plane_words * 4;
+  pl.base_words = (size_t)n_phase * B * ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32));
+  pl.gm = g;
+  if (masked) {
     long long moff = 0;
-    for (int o = 0; o < 4; ++o) { gm.v[o].packed_off = moff; moff += gm.v[o].view_words; }
-    gm.plane_words = moff;
-    mask_views_bytes = (size_t)moff * 4;
-    mask_base_bytes = ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32)) * 4;
+    for (int o = 0; o < 4; ++o) { pl.gm.v[o].packed_off = moff; moff += pl.gm.v[o].view_words; }
+    pl.gm.plane_words = moff;
+    pl.mask_views_bytes = (size_t)moff * 4;
+    pl.mask_base_bytes = ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32)) * 4;
   }
-  const size_t need = views_bytes + base_words * 4 + mask_views_bytes + mask_base_bytes;
-  if (need > p->packed_bytes) {
-    if (p->d_packed) { LPF_CUDA(cudaStreamSynchronize(st)); cudaFree(p->d_packed); p->d_packed = nullptr; p->packed_bytes = 0; }
-    LPF_CUDA(cudaMalloc(&p->d_packed, need));
-    p->packed_bytes = need;
+  pl.need = pl.views_bytes + pl.base_words * 4 + pl.mask_views_bytes + pl.mask_base_bytes;
+  rc = grow(&p->d_packed, &p->packed_bytes, pl.need);
+  if (rc != LPF_OK) return rc;
+  int32_t* d_work = nullptr;
+  cudaError_t e = cudaMalloc(&d_work, sizeof(int32_t) * std::max<size_t>(work.size(), 4));
+  if (e == cudaSuccess) e = cudaMemcpy(d_work, work.data(), sizeof(int32_t) * work.size(), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    if (d_work) cudaFree(d_work);
+    return cuda_fail(e);
   }
+  pl.d_work = d_work;
+  try {
+    p->plans[key] = pl;
+  } catch (const std::bad_alloc&) {
+    cudaFree(d_work);
+    return LPF_E_NOMEM;
+  }
+  return LPF_OK;
+}
+
+// node records of the image-coordinate trie and the bit-image workspace of lpf_swap_delta on H x W images
+static int reserve_swap(lpf_paths* p, int H, int W) {
+  if (!p || p->device < 0 || H < 1 || W < 1 || p->m > std::min(H, W) - 1) return LPF_E_INVAL;
+  // the padded base bit image(s) (halo of m pixels) and eight warp stacks of 4 KB live in shared memory; 24-bit node indices
+  const size_t padded_words = (size_t)2 * (H + 2 * p->m) * ((W + 2 * p->m + 31) / 32);
+  const size_t smem1 = padded_words / 2 * 4 + 8 + 8 * 512 * 8;
+  if (smem1 + 2048 > (size_t)p->max_smem || p->n_trie_nodes >= (1 << 24)) return LPF_E_UNSUPPORTED;
+  DeviceGuard dg(p->device);
+  if (!dg.ok) return LPF_E_CUDA;
+  if (!p->d_swap_rec) {
+    try {
+      std::vector<int32_t> rec;
+      build_swap_records(p, rec);
+      if ((int64_t)rec.size() != 4 * p->n_trie_nodes) return LPF_E_INVAL;
+      int32_t* d = nullptr;
+      cudaError_t e = cudaMalloc(&d, sizeof(int32_t) * rec.size());
+      if (e == cudaSuccess) e = cudaMemcpy(d, rec.data(), sizeof(int32_t) * rec.size(), cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) {
+        if (d) cudaFree(d);
+        return cuda_fail(e);
+      }
+      p->d_swap_rec = d;
+    } catch (const std::bad_alloc&) {
+      return LPF_E_NOMEM;
+    }
+    LPF_CUDA(swap_delta_prepare((size_t)p->max_smem));
+  }
+  // both phase planes: compact bit images of stage 1, then the padded planes
+  const size_t bits_bytes = (2 * ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32)) + padded_words) * 4;
+  return grow(&p->d_swap_bits, &p->swap_bits_bytes, bits_bytes);
+}
+
+int anneal_kmax(int m, int n_ph) {       // batch size: at most 256 proposals and about 256 MB of delta arrays
+  const long long K2 = (long long)(2 * m + 1) * (2 * m + 1);
+  int K_max = 256;
+  while (K_max > 8 && (long long)K_max * K2 * 4 * n_ph > (256ll << 20)) K_max /= 2;
+  return K_max;
+}
+
+int reserve_anneal(lpf_paths* p, int H, int W) {
+  int rc = reserve_eval(p, 1, H, W, 1, 0, false);
+  if (rc == LPF_OK) rc = reserve_eval(p, 1, H, W, 2, 0, false);
+  if (rc == LPF_OK) rc = reserve_swap(p, H, W);
+  if (rc != LPF_OK) return rc;
+  DeviceGuard dg(p->device);
+  if (!dg.ok) return LPF_E_CUDA;
+  const long long K2 = (long long)(2 * p->m + 1) * (2 * p->m + 1);
+  const int K_max = std::max(anneal_kmax(p->m, 1), 2 * anneal_kmax(p->m, 2));   // arrays of either phase count
+  if (!p->d_an_state) {
+    LPF_CUDA(cudaMalloc(&p->d_an_state, 256));
+    LPF_CUDA(cudaMalloc(&p->d_an_batch, sizeof(int32_t) * 4 * 256));
+    LPF_CUDA(cudaMalloc(&p->d_an_dE, sizeof(int64_t) * 256));
+  }
+  p->an_kmax = K_max;
+  return grow(&p->d_an_delta, &p->an_delta_bytes, sizeof(int32_t) * (size_t)K_max * K2);
+}
+
+static int reserve_host(lpf_paths* p, int B, int H, int W) {
+  DeviceGuard dg(p->device);
+  if (!dg.ok) return LPF_E_CUDA;
+  const int S = 2 * p->m + 1;
+  int rc = grow((uint8_t**)&p->d_io_in, &p->io_in_bytes, (size_t)B * H * W);
+  if (rc == LPF_OK) rc = grow((uint8_t**)&p->d_io_out, &p->io_out_bytes, sizeof(int64_t) * (size_t)B * 2 * S * S);
+  if (rc != LPF_OK) return rc;
+  if (!p->io_stream) LPF_CUDA(cudaStreamCreateWithFlags((cudaStream_t*)&p->io_stream, cudaStreamNonBlocking));
+  return LPF_OK;
+}
+
+// ---- the eval calls: look the plan up, enqueue -------------------------------------------------------
+
+// sum_over_batch: every image adds into ONE [n_phase][S][S] array (ensemble sum) instead of its own
+static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, int n_phase, int phase0,
+                     int64_t* counts, unsigned flags, void* stream, const uint8_t* start_mask = nullptr,
+                     bool sum_over_batch = false) {
+  if (!images || !counts) return LPF_E_INVAL;
+  int rc = check_eval_args(p, B, H, W, flags);
+  if (rc != LPF_OK) return rc;
+  if (n_phase == 1 && phase0 != 0 && phase0 != 1) return LPF_E_INVAL;
+  auto it = p->plans.find(plan_key(p, B, H, W, n_phase, flags, start_mask != nullptr));
+  if (it == p->plans.end()) {                      // a shape that was not reserved: reserve it now (allocates, syncs)
+    rc = reserve_eval(p, B, H, W, n_phase, flags, start_mask != nullptr);
+    if (rc != LPF_OK) return rc;
+    it = p->plans.find(plan_key(p, B, H, W, n_phase, flags, start_mask != nullptr));
+  }
+  const EvalPlan& pl = it->second;
+  if (pl.need > p->packed_bytes) return LPF_E_INVAL;   // cannot happen: the workspace only grows
+  DeviceGuard dg(p->device);
+  if (!dg.ok) return LPF_E_CUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  StreamOrder order(p, st);
+  LPF_CUDA(order.err);
 
   const int S = 2 * p->m + 1;
-  LPF_CUDA(cudaMemsetAsync(counts, 0, sizeof(int64_t) * (size_t)B * n_phase * S * S, st));
-  LPF_CUDA(launch_pack(images, p->d_packed + views_bytes / 4, p->d_packed, g, B, n_phase, phase0, p->d_counter,
-                       p->n_sm, st));
-  uint32_t* const d_mask = p->d_packed + views_bytes / 4 + base_words;
+  const long long n_arrays = sum_over_batch ? n_phase : (long long)B * n_phase;
+  LPF_CUDA(cudaMemsetAsync(counts, 0, sizeof(int64_t) * (size_t)n_arrays * S * S, st));
+  LPF_CUDA(launch_pack(images, p->d_packed + pl.views_bytes / 4, p->d_packed, pl.g, B, pl.Bpad, n_phase, phase0,
+                       p->d_counter, p->n_sm, st));
+  uint32_t* const d_mask = p->d_packed + pl.views_bytes / 4 + pl.base_words;
   if (start_mask)                                  // "phase" -1: a start pixel is selected iff its byte is non-zero
-    LPF_CUDA(launch_pack(start_mask, d_mask + mask_views_bytes / 4, d_mask, gm, 1, 1, -1, p->d_counter, p->n_sm, st));
+    LPF_CUDA(launch_pack(start_mask, d_mask + pl.mask_views_bytes / 4, d_mask, pl.gm, 1, 1, 1, -1, p->d_counter,
+                         p->n_sm, st));
 
   EvalParams ep;
-  ep.g = g;
-  ep.entries = (const uint2*)pr->d_entries;
-  ep.skip = pr->d_skip;
-  ep.work = (const int4*)pr->d_work;
-  ep.n_work = (int)pr->n_work;
-  ep.n_gp = n_gp;
+  ep.g = pl.g;
+  ep.entries = (const uint2*)pl.pr->d_entries;
+  ep.skip = pl.pr->d_skip;
+  ep.work = (const int4*)pl.d_work;
+  ep.n_work = (int)pl.n_work;
+  ep.n_gp = pl.n_gp;
   ep.B = B;
   ep.n_phase = n_phase;
   ep.packed = p->d_packed;
-  ep.Bpad = Bpad;
+  ep.Bpad = pl.Bpad;
   ep.counts = (unsigned long long*)counts;
   ep.S = S;
+  ep.image_stride = sum_over_batch ? 0 : (long long)n_phase * S * S;
   ep.counter = p->d_counter;
-  ep.prune = prune ? 1 : 0;
-  ep.n_slots = pr->n_slots;
+  ep.prune = pl.prune;
+  ep.n_slots = pl.pr->n_slots;
   ep.mask = start_mask ? d_mask : nullptr;
-  for (int o = 0; o < 4; ++o) ep.mask_off[o] = gm.v[o].packed_off;
-  const long long total_work = (long long)ep.n_work * n_gp;
-  if (total_work >= (1ll << 32)) return LPF_E_UNSUPPORTED;
-  const int grid = (int)std::min<long long>(total_work, resident);
-  if (p->timing) {
-    if (!p->ev_start) {
-      LPF_CUDA(cudaEventCreate((cudaEvent_t*)&p->ev_start));
-      LPF_CUDA(cudaEventCreate((cudaEvent_t*)&p->ev_stop));
-    }
-    LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_start, st));
+  for (int o = 0; o < 4; ++o) ep.mask_off[o] = pl.gm.v[o].packed_off;
+  const bool timed = p->timing && !order.capturing;
+  if (timed) LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_start, st));
+  LPF_CUDA(launch_eval(ep, pl.grid, pl.g.threads, pl.smem, st));
+  if (timed) {
+    LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_stop, st));
+    p->timed_once = 1;
   }
-  LPF_CUDA(launch_eval(ep, grid, g.threads, smem_total, st));
-  if (p->timing) LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_stop, st));
-  LPF_CUDA(launch_mirror((unsigned long long*)counts, S, (long long)B * n_phase, p->n_sm, st));
+  LPF_CUDA(launch_mirror((unsigned long long*)counts, S, n_arrays, p->n_sm, st));
+  LPF_CUDA(order.done());
 
   p->last_info[0] = start_mask ? 6 : 4;                  // kernels launched (pack base, pack views, eval, mirror)
-  p->last_info[1] = total_work;
-  p->last_info[2] = (int64_t)pr->entries.size();         // program entries (all four octants)
-  p->last_info[3] = grid;
-  p->last_info[4] = g.threads;
-  p->last_info[5] = (int64_t)smem_total;
-  p->last_info[6] = g.TX * 1000 + g.TY * 100 + pr->n_slots;   // thread tile TX, TY and mask-stack slots
-  p->last_info[7] = g.G;
+  p->last_info[1] = (long long)pl.n_work * pl.n_gp;
+  p->last_info[2] = (int64_t)pl.pr->entries.size();      // program entries (all four octants)
+  p->last_info[3] = pl.grid;
+  p->last_info[4] = pl.g.threads;
+  p->last_info[5] = (int64_t)pl.smem;
+  p->last_info[6] = pl.g.TX * 1000 + pl.g.TY * 100 + pl.pr->n_slots;   // thread tile TX, TY and mask-stack slots
+  p->last_info[7] = pl.g.G;
+  p->last_info[8] = pl.g.v[0].e2_band_off ? 1 : 0;       // eroded planes in shared memory (else the plain plane)
+  p->last_info[9] = pl.fused_pairs;                      // per image-phase and start word: 2 SHF + 1 LOP3 each
+  p->last_info[10] = pl.singles;                         //   1 SHF + 1 LOP3 each
+  p->last_info[11] = pl.terminals;                       //   1 POPC + 1 add each
+  p->last_info[12] = pl.piece_nodes;
   return LPF_OK;
 }
 
 }  // namespace lpf
 
-extern "C" int lpf_eval(lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase, int64_t* counts,
+extern "C" int lpf_reserve(lpf_paths* p, int B, int H, int W, unsigned flags, unsigned what) {
+  if (!p || p->device < 0 || H < 1 || W < 1 || what == 0) return LPF_E_INVAL;
+  if (what & ~(LPF_FOR_EVAL | LPF_FOR_EVAL_BOTH | LPF_FOR_MASKED | LPF_FOR_SWAP_DELTA | LPF_FOR_ANNEAL | LPF_FOR_HOST))
+    return LPF_E_INVAL;
+  int rc = LPF_OK;
+  if (what & (LPF_FOR_EVAL | LPF_FOR_EVAL_BOTH | LPF_FOR_HOST)) {
+    rc = check_eval_args(p, B, H, W, flags);
+    if (rc != LPF_OK) return rc;
+  }
+  const bool masked = (what & LPF_FOR_MASKED) != 0;
+  if (masked && !(what & (LPF_FOR_EVAL | LPF_FOR_EVAL_BOTH))) return LPF_E_INVAL;
+  if (rc == LPF_OK && (what & LPF_FOR_EVAL)) rc = reserve_eval(p, B, H, W, 1, flags, masked);
+  if (rc == LPF_OK && (what & LPF_FOR_EVAL_BOTH)) rc = reserve_eval(p, B, H, W, 2, flags, masked);
+  if (rc == LPF_OK && (what & LPF_FOR_SWAP_DELTA)) rc = reserve_swap(p, H, W);
+  if (rc == LPF_OK && (what & LPF_FOR_ANNEAL)) rc = reserve_anneal(p, H, W);
+  if (rc == LPF_OK && (what & LPF_FOR_HOST)) {
+    rc = reserve_host(p, B, H, W);
+    if (rc == LPF_OK && !(what & (LPF_FOR_EVAL | LPF_FOR_EVAL_BOTH))) {
+      rc = reserve_eval(p, B, H, W, 1, flags, false);
+      if (rc == LPF_OK) rc = reserve_eval(p, B, H, W, 2, flags, false);
+    }
+  }
+  if (rc == LPF_OK) {                              // uploads above used synchronous copies; leave nothing in flight
+    DeviceGuard dg(p->device);
+    if (!dg.ok) return LPF_E_CUDA;
+    LPF_CUDA(cudaDeviceSynchronize());
+  }
+  return rc;
+}
+
+extern "C" int lpf_eval(const lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase, int64_t* counts,
                         unsigned flags, void* stream) {
-  return lpf::eval_impl(p, images, B, H, W, 1, phase, counts, flags, stream);
+  return lpf::eval_impl(const_cast<lpf_paths*>(p), images, B, H, W, 1, phase, counts, flags, stream);
 }
 
-extern "C" int lpf_eval_both(lpf_paths* p, const uint8_t* images, int B, int H, int W, int64_t* counts,
+extern "C" int lpf_eval_both(const lpf_paths* p, const uint8_t* images, int B, int H, int W, int64_t* counts,
                              unsigned flags, void* stream) {
-  return lpf::eval_impl(p, images, B, H, W, 2, 0, counts, flags, stream);
+  return lpf::eval_impl(const_cast<lpf_paths*>(p), images, B, H, W, 2, 0, counts, flags, stream);
 }
 
-extern "C" int lpf_eval_masked(lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase,
+extern "C" int lpf_eval_masked(const lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase,
                                const uint8_t* start_mask, int64_t* counts, unsigned flags, void* stream) {
   if (!start_mask || phase < -1 || phase > 1) return LPF_E_INVAL;
-  return phase < 0 ? lpf::eval_impl(p, images, B, H, W, 2, 0, counts, flags, stream, start_mask)
-                   : lpf::eval_impl(p, images, B, H, W, 1, phase, counts, flags, stream, start_mask);
+  lpf_paths* q = const_cast<lpf_paths*>(p);
+  return phase < 0 ? lpf::eval_impl(q, images, B, H, W, 2, 0, counts, flags, stream, start_mask)
+                   : lpf::eval_impl(q, images, B, H, W, 1, phase, counts, flags, stream, start_mask);
+}
+
+extern "C" int lpf_eval_sum(const lpf_paths* p, const uint8_t* images, int B, int H, int W, int phase,
+                            int64_t* counts_sum, unsigned flags, void* stream) {
+  if (phase < -1 || phase > 1) return LPF_E_INVAL;
+  lpf_paths* q = const_cast<lpf_paths*>(p);
+  return phase < 0 ? lpf::eval_impl(q, images, B, H, W, 2, 0, counts_sum, flags, stream, nullptr, true)
+                   : lpf::eval_impl(q, images, B, H, W, 1, phase, counts_sum, flags, stream, nullptr, true);
 }
 
 extern "C" int lpf_set_timing(lpf_paths* p, int enable) {
@@ -316,8 +552,8 @@ extern "C" int lpf_set_tile(lpf_paths* p, int tx, int ty, int cta_warps) {
   return LPF_OK;
 }
 
-extern "C" int lpf_last_eval_kernel_ms(lpf_paths* p, float* ms) {
-  if (!p || !ms || p->device < 0 || !p->ev_start) return LPF_E_INVAL;
+extern "C" int lpf_last_eval_kernel_ms(const lpf_paths* p, float* ms) {
+  if (!p || !ms || p->device < 0 || !p->timed_once) return LPF_E_INVAL;
   DeviceGuard dg(p->device);
   if (!dg.ok) return LPF_E_CUDA;
   LPF_CUDA(cudaEventSynchronize((cudaEvent_t)p->ev_stop));
@@ -325,9 +561,9 @@ extern "C" int lpf_last_eval_kernel_ms(lpf_paths* p, float* ms) {
   return LPF_OK;
 }
 
-extern "C" int lpf_last_launch_info(const lpf_paths* p, int64_t* out8) {
-  if (!p || !out8) return LPF_E_INVAL;
-  std::memcpy(out8, p->last_info, sizeof(p->last_info));
+extern "C" int lpf_last_launch_info(const lpf_paths* p, int64_t* out13) {
+  if (!p || !out13) return LPF_E_INVAL;
+  std::memcpy(out13, p->last_info, sizeof(p->last_info));
   return LPF_OK;
 }
 
@@ -346,25 +582,6 @@ extern "C" int lpf_objective(const int64_t* counts, const int64_t* target, int B
 
 namespace lpf {
 
-// node records of the image-coordinate trie for the swap-delta kernel, built and uploaded on first use
-static int ensure_swap_table(lpf_paths* p) {
-  if (p->d_swap_rec) return LPF_OK;
-  try {
-    std::vector<int32_t> rec;
-    build_swap_records(p, rec);
-    if ((int64_t)rec.size() != 4 * p->n_trie_nodes) return LPF_E_INVAL;
-    LPF_CUDA(cudaMalloc(&p->d_swap_rec, sizeof(int32_t) * rec.size()));
-    LPF_CUDA(cudaMemcpy(p->d_swap_rec, rec.data(), sizeof(int32_t) * rec.size(), cudaMemcpyHostToDevice));
-  } catch (const std::bad_alloc&) {
-    return LPF_E_NOMEM;
-  }
-  return LPF_OK;
-}
-
-}  // namespace lpf
-
-namespace lpf {
-
 // phase 0 | 1: delta [n][S][S] of that phase;  phase < 0: both phases in one pass over the trie, phase k written at
 // delta + k * plane_stride (used by lpf_anneal)
 int swap_delta_impl(lpf_paths* p, const uint8_t* image, int H, int W, int phase, const int32_t* pairs, int64_t n,
@@ -374,35 +591,30 @@ int swap_delta_impl(lpf_paths* p, const uint8_t* image, int H, int W, int phase,
   if (phase < -1 || phase > 1) return LPF_E_INVAL;
   if (p->m > std::min(H, W) - 1) return LPF_E_INVAL;
   if (n == 0) return LPF_OK;
+  const size_t padded_words = (size_t)2 * (H + 2 * p->m) * ((W + 2 * p->m + 31) / 32);
+  const size_t bits_bytes = (2 * ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32)) + padded_words) * 4;
+  if (!p->d_swap_rec || bits_bytes > p->swap_bits_bytes) {   // not reserved: reserve now (allocates, syncs)
+    const int rc = reserve_swap(p, H, W);
+    if (rc != LPF_OK) return rc;
+  }
+  if (phase < 0 && padded_words * 4 + 8 + 8 * 512 * 8 + 2048 > (size_t)p->max_smem) return LPF_E_UNSUPPORTED;
   DeviceGuard dg(p->device);
   if (!dg.ok) return LPF_E_CUDA;
-  const int n_planes = phase < 0 ? 2 : 1;
-  // the padded base bit image(s) (halo of m pixels) and eight warp stacks of 4 KB live in shared memory; 24-bit node indices
-  const size_t padded_words = (size_t)n_planes * (H + 2 * p->m) * ((W + 2 * p->m + 31) / 32);
-  const size_t smem = padded_words * 4 + 8 + 8 * 512 * 8;
-  if (smem + 2048 > (size_t)p->max_smem || p->n_trie_nodes >= (1 << 24)) return LPF_E_UNSUPPORTED;
-  int rc = ensure_swap_table(p);
-  if (rc != LPF_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
-  const size_t bits_bytes =
-      (n_planes * ((size_t)H * ((W + 31) / 32) + (size_t)W * ((H + 31) / 32)) + padded_words) * 4;
-  if (bits_bytes > p->swap_bits_bytes) {
-    if (p->d_swap_bits) { LPF_CUDA(cudaStreamSynchronize(st)); cudaFree(p->d_swap_bits); p->d_swap_bits = nullptr; }
-    p->swap_bits_bytes = 0;
-    LPF_CUDA(cudaMalloc(&p->d_swap_bits, bits_bytes));
-    p->swap_bits_bytes = bits_bytes;
-  }
+  StreamOrder order(p, st);
+  LPF_CUDA(order.err);
   LPF_CUDA(launch_swap_delta(image, p->d_swap_bits, H, W, p->m, phase, pairs, (long long)n, p->d_swap_rec,
                              (int)p->n_trie_nodes, delta, (long long)plane_stride, p->d_counter + 1, p->n_sm, st));
+  LPF_CUDA(order.done());
   return LPF_OK;
 }
 
 }  // namespace lpf
 
-extern "C" int lpf_swap_delta(lpf_paths* p, const uint8_t* image, int H, int W, int phase, const int32_t* pairs,
+extern "C" int lpf_swap_delta(const lpf_paths* p, const uint8_t* image, int H, int W, int phase, const int32_t* pairs,
                               int64_t n, int32_t* delta, void* stream) {
   if (phase != 0 && phase != 1) return LPF_E_INVAL;
-  return lpf::swap_delta_impl(p, image, H, W, phase, pairs, n, delta, 0, stream);
+  return lpf::swap_delta_impl(const_cast<lpf_paths*>(p), image, H, W, phase, pairs, n, delta, 0, stream);
 }
 
 // ---- host-buffer convenience (end-to-end measurement) ---------------------------------------------
@@ -411,27 +623,25 @@ extern "C" int lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, in
                              int64_t* counts_host, unsigned flags) {
   if (!p || !images_host || !counts_host) return LPF_E_INVAL;
   if (p->device < 0 || B < 1 || H < 1 || W < 1) return LPF_E_INVAL;
-  DeviceGuard dg(p->device);
-  if (!dg.ok) return LPF_E_CUDA;
   const int n_phase = phase < 0 ? 2 : 1;
   const int S = 2 * p->m + 1;
   const size_t in_bytes = (size_t)B * H * W;
   const size_t out_bytes = sizeof(int64_t) * (size_t)B * n_phase * S * S;
-  if (in_bytes > p->io_in_bytes) {
-    if (p->d_io_in) cudaFree(p->d_io_in);
-    p->d_io_in = nullptr; p->io_in_bytes = 0;
-    LPF_CUDA(cudaMalloc(&p->d_io_in, in_bytes));
-    p->io_in_bytes = in_bytes;
+  if (in_bytes > p->io_in_bytes || sizeof(int64_t) * (size_t)B * 2 * S * S > p->io_out_bytes || !p->io_stream) {
+    int rc = check_eval_args(p, B, H, W, flags);
+    if (rc == LPF_OK) rc = reserve_host(p, B, H, W);
+    if (rc != LPF_OK) return rc;
   }
-  if (out_bytes > p->io_out_bytes) {
-    if (p->d_io_out) cudaFree(p->d_io_out);
-    p->d_io_out = nullptr; p->io_out_bytes = 0;
-    LPF_CUDA(cudaMalloc(&p->d_io_out, out_bytes));
-    p->io_out_bytes = out_bytes;
-  }
-  if (!p->io_stream) LPF_CUDA(cudaStreamCreateWithFlags((cudaStream_t*)&p->io_stream, cudaStreamNonBlocking));
+  DeviceGuard dg(p->device);
+  if (!dg.ok) return LPF_E_CUDA;
+  // the private stream: lpf_eval below orders it after earlier work on this table (StreamOrder)
   cudaStream_t st = (cudaStream_t)p->io_stream;
-  LPF_CUDA(cudaMemcpyAsync(p->d_io_in, images_host, in_bytes, cudaMemcpyHostToDevice, st));
+  {
+    StreamOrder order(p, st);                      // the H2D copy overwrites d_io_in: wait for the previous call first
+    LPF_CUDA(order.err);
+    LPF_CUDA(cudaMemcpyAsync(p->d_io_in, images_host, in_bytes, cudaMemcpyHostToDevice, st));
+    LPF_CUDA(order.done());
+  }
   int rc = n_phase == 2 ? lpf_eval_both(p, (const uint8_t*)p->d_io_in, B, H, W, (int64_t*)p->d_io_out, flags, st)
                         : lpf_eval(p, (const uint8_t*)p->d_io_in, B, H, W, phase, (int64_t*)p->d_io_out, flags, st);
   if (rc != LPF_OK) return rc;

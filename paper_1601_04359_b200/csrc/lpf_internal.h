@@ -3,12 +3,14 @@
 // Nothing here is used by, or shared with, oracle/.
 #pragma once
 #include <cstdint>
+#include <array>
 #include <map>
 #include <tuple>
 #include <utility>
 #include <vector>
 
 #include "lpf.h"
+#include "lpf_kernels.cuh"
 
 namespace lpf {
 
@@ -98,11 +100,24 @@ struct Program {         // one linearisation of the four octant tries for one s
   int n_slots = 0;
   int stride[4] = {0, 0, 0, 0};
   int e2_off[4] = {0, 0, 0, 0};        // word offset of the E2 plane of each view in shared memory (0: none)
-  uint64_t* d_entries = nullptr;
+  uint64_t* d_entries = nullptr;       // device copy, uploaded by lpf_reserve (lpf_api.cu)
   uint32_t* d_skip = nullptr;
-  int32_t* d_work = nullptr;           // expanded (item x band) list, see lpf_api.cu
+};
+
+// Everything one eval call needs for one (B, H, W, phases, flags, masked, tile) shape; built by lpf_reserve (or by the
+// first call for the shape), after which an eval only enqueues work (lpf_api.cu).
+struct EvalPlan {
+  Geom g;                              // views with their offsets inside one phase plane of the packed workspace
+  Geom gm;                             // the same views for the start mask of lpf_eval_masked (one image, one plane)
+  Program* pr = nullptr;
+  int32_t* d_work = nullptr;           // [n_work][4] = first entry, count, octant | strip band << 4, row band; big first
   int64_t n_work = 0;
-  int work_bands[4] = {0, 0, 0, 0};    // bands per octant the work list was expanded for
+  int Bpad = 0, n_gp = 0, grid = 0, prune = 0;
+  size_t smem = 0;
+  size_t views_bytes = 0, base_words = 0, mask_views_bytes = 0, mask_base_bytes = 0, need = 0;
+  // what the walker executes per image-phase and start word (lpf_last_launch_info): pairs of entries folded into one
+  // 3-input AND, entries executed on their own, terminal entries (POPC + add), trie nodes per piece
+  int64_t fused_pairs = 0, singles = 0, terminals = 0, piece_nodes = 0;
 };
 
 }  // namespace lpf
@@ -118,15 +133,29 @@ struct lpf_paths {
   std::vector<lpf::Node> oct[4];     // per-octant prefix tries in view coordinates; [0] = root (0,0)
   // key: (piece_nodes, program kind, stride0, stride1, E2 offset 0, E2 offset 1)   (views 3, 2 as views 0, 1)
   std::map<std::tuple<int, unsigned, int, int, int, int>, lpf::Program> programs;
-  // device workspace (grown on demand)
+  // key: B, H, W, phases, flags, masked, 100 tile_tx + tile_ty, cta_warps
+  std::map<std::array<int64_t, 8>, lpf::EvalPlan> plans;
+  // device workspace (sized by lpf_reserve; a call for a shape that was not reserved reserves it first)
   uint32_t* d_packed = nullptr;
   size_t packed_bytes = 0;
   unsigned int* d_counter = nullptr;
-  // swap-delta node records: the image-coordinate trie in preorder, 16 bytes per node (built lazily)
+  // swap-delta node records: the image-coordinate trie in preorder, 16 bytes per node (built by lpf_reserve)
   int32_t* d_swap_rec = nullptr;     // [n_trie_nodes][4]
-  uint32_t* d_swap_bits = nullptr;   // packed base image of the last lpf_swap_delta call (grown on demand)
+  uint32_t* d_swap_bits = nullptr;   // packed base image of the last lpf_swap_delta call
   size_t swap_bits_bytes = 0;
-  // device staging buffers of lpf_eval_host (grown on demand) and its private stream
+  // lpf_anneal: chain state, proposal batch, speculative deltas and their error changes
+  void* d_an_state = nullptr;
+  int32_t* d_an_batch = nullptr;
+  int32_t* d_an_delta = nullptr;
+  int64_t* d_an_dE = nullptr;
+  size_t an_delta_bytes = 0;
+  int an_kmax = 0;
+  // stream order: work of consecutive calls shares the workspace, so a call on another stream first waits for the
+  // event recorded after the previous call (no host synchronisation)
+  void* ev_done = nullptr;
+  void* last_stream = nullptr;
+  int last_stream_valid = 0;
+  // device staging buffers of lpf_eval_host and its private stream
   void* d_io_in = nullptr;
   size_t io_in_bytes = 0;
   void* d_io_out = nullptr;
@@ -135,9 +164,10 @@ struct lpf_paths {
   // lpf_set_timing: CUDA events recorded around the eval kernel alone
   int tile_tx = 0, tile_ty = 0, cta_warps = 0;   // lpf_set_tile overrides (0 = automatic)
   int timing = 0;
+  int timed_once = 0;                // a timed eval has been issued: ev_start / ev_stop hold a measurement
   void* ev_start = nullptr;
   void* ev_stop = nullptr;
-  int64_t last_info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  int64_t last_info[13] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
 };
 
 namespace lpf {
@@ -156,5 +186,12 @@ void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec);
 // builds (or returns the cached) program for (piece_nodes, flags, view strides); host side only
 Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int e2off03,
                      int e2off12);
+// forgets a cached program that was never uploaded (one the kernel cannot take)
+void drop_program(lpf_paths* p, const Program* pr);
+
+// largest proposal batch of lpf_anneal for n_ph phase planes; plans + swap tables + batch buffers of lpf_anneal on
+// H x W images (lpf_api.cu; allocates and synchronises)
+int anneal_kmax(int m, int n_ph);
+int reserve_anneal(lpf_paths* p, int H, int W);
 
 }  // namespace lpf

@@ -75,92 +75,103 @@ __device__ __forceinline__ uint32_t window32(const uint32_t* __restrict__ row, i
   return __funnelshift_r(lo, hi, xs & 31);
 }
 
-// word i of one view row: 32 view pixels x' = (32 i + k) mod Wv read from the source row (views 0-2 in order, view 3
-// mirrored: bit k = source pixel (Wv - x') mod Wv)
-__device__ __forceinline__ uint32_t view_word(const uint32_t* __restrict__ srow, int words, int o, int Wv, int i) {
-  const int x0 = (32 * i) % Wv;
-  uint32_t word = 0;
-  if (o != 3) {
-    if (x0 + 32 <= Wv) return window32(srow, words, x0);
-    for (int k = 0; k < 32; ++k) {
-      const int xs = (x0 + k) % Wv;
-      word |= ((srow[xs >> 5] >> (xs & 31)) & 1u) << k;
-    }
-  } else {
-    // for 1 <= x0 and x0 + 31 <= Wv the sources are the 32 consecutive pixels Wv - x0 - 31 .. Wv - x0, descending
-    if (x0 >= 1 && x0 + 31 <= Wv) return __brev(window32(srow, words, Wv - x0 - 31));
-    for (int k = 0; k < 32; ++k) {
-      const int xv = (x0 + k) % Wv;
-      const int xs = xv ? Wv - xv : 0;
-      word |= ((srow[xs >> 5] >> (xs & 31)) & 1u) << k;
-    }
+// 32 pixels x .. x+31 of the MIRRORED row msrc[x] = src[(Wv - x) mod Wv], x in [0, Wv), zero beyond Wv (view 3).
+// For x + k >= 1 the sources are src[Wv - x - k], descending: the bit-reversed window of src at s = Wv - x - 31.
+// Source index 0 inside that window would be pixel x + k = Wv (beyond the row) and is cleared, indices < 0 shift in
+// as zeros; pixel 0 of the mirrored row is src[0].
+__device__ __forceinline__ uint32_t mirrored_window32(const uint32_t* __restrict__ src, int words, int Wv, int x) {
+  const int s = Wv - x - 31;
+  uint32_t w;
+  if (s > 0) w = window32(src, words, s);
+  else if (s > -32) w = (window32(src, words, 0) & ~1u) << (-s);
+  else w = 0u;
+  return __brev(w) | (x == 0 ? (src[0] & 1u) : 0u);
+}
+
+// word of the periodic extension of a view row: 32 view pixels x' = (x0 + k) mod Wv, x0 in [0, Wv).  One window of
+// the source row, and one more per wrap (a word wraps at most once unless Wv < 32).  No per-bit work, no division.
+template <bool MIRROR>
+__device__ __forceinline__ uint32_t periodic_word(const uint32_t* __restrict__ src, int words, int Wv, int x0) {
+  uint32_t word = MIRROR ? mirrored_window32(src, words, Wv, x0) : window32(src, words, x0);
+  int filled = Wv - x0;                                  // valid bits so far; the bits above them are zero
+  if (filled < 32) {
+    const uint32_t head = MIRROR ? mirrored_window32(src, words, Wv, 0) : window32(src, words, 0);
+    do {
+      word |= head << filled;
+      filled += Wv;
+    } while (filled < 32);
   }
   return word;
 }
 
 // ---------------------------------------------------------------------------------------------
-// bit-pack, stage 2: the four octant views with their periodic halo, one thread per output word.
+// bit-pack, stage 2: the four octant views with their periodic halo.
 //   view o of image I (lpf_internal.h): 0: I[y'][x']  1: I[x'][y']  2: I[x'][-y' mod W]  3: I[y'][-x' mod W]
-//   word (r, i) of a view holds x' = (32 i + k) mod Wv, y' = r mod Hv.  Views 0 and 3 read Brow, views 1 and 2
-//   read Bcol; a word whose 32 pixels do not wrap is one funnel shift of two base words (view 3: of the
-//   bit-reversed pair), the others are gathered bit by bit.
+//   word (r, i) of a view holds x' = (32 i + k) mod Wv, y' = r mod Hv.  Views 0 and 3 read Brow, views 1 and 2 Bcol.
+//   One CTA per tile of PACK_TILE consecutive words of one (phase plane, view, image): it stages the plain words of
+//   the tile and of the row below it in shared memory (each a funnel shift of two base words, wrap words two of them),
+//   derives E2 = pixel & right neighbour and D2 = pixel & lower-right neighbour there (across word and row boundaries)
+//   and writes the planes with fully coalesced stores (a tile is one contiguous block of every plane).
 // ---------------------------------------------------------------------------------------------
+constexpr int PACK_TILE = 4096;
+
 __global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restrict__ base,
-                                                         uint32_t* __restrict__ packed, Geom g, int B, int n_phase) {
+                                                         uint32_t* __restrict__ packed, Geom g, int B, int Bpad,
+                                                         int4 tiles, long long ctas_per_plane) {
+  extern __shared__ uint32_t s_plain[];                    // [PACK_TILE + stride + 2]
   const int Wc = (g.W + 31) >> 5, Hc = (g.H + 31) >> 5;
   const long long img_words = (long long)g.H * Wc + (long long)g.W * Hc;
-  // one thread per word POSITION (r, i) of a view: it writes the plain word and, in eroded mode, the E2 and the D2
-  // word of the same position (E2 = pixel & right neighbour, D2 = pixel & lower-right neighbour, across word and
-  // row boundaries), from the four plain words (r, i), (r, i+1), (r+1, i), (r+1, i+1)
   const int np = g.v[0].e2_view_off > 0 ? 3 : 1;
-  const long long units_per_plane = g.plane_words / np;
-  const long long total = (long long)n_phase * units_per_plane;
-  for (long long u = (long long)blockIdx.x * blockDim.x + threadIdx.x; u < total;
-       u += (long long)gridDim.x * blockDim.x) {
-    const int plane = (int)(u / units_per_plane);
-    const long long up = u - (long long)plane * units_per_plane;
-    int o = 0;
-#pragma unroll
-    for (int k = 1; k < 4; ++k)
-      if (up >= g.v[k].packed_off / np) o = k;
-    const ViewGeom& v = g.v[o];
-    const int pv = v.view_words / np;                          // words of one plane of one image
-    const long long rem = up - v.packed_off / np;
-    const int b = (int)(rem / pv);
-    const int idx = (int)(rem - (long long)b * pv);
-    const int r = idx / v.stride, i = idx - r * v.stride;
-    const int rows = v.n_bands * g.band_rows + g.m;
-    uint32_t w00 = 0, e2 = 0, d2 = 0;
-    if (b < B && r < rows) {
-      const uint32_t* bimg = base + ((size_t)plane * B + b) * img_words;
-      // source row of a view row: views 0, 3: image row yv (Brow); view 1: image column yv; view 2: column -yv
-      auto source_row = [&](int rr, int* words) -> const uint32_t* {
-        const int yv = rr % v.Hv;
-        if (o == 0 || o == 3) { *words = Wc; return bimg + (size_t)yv * Wc; }
-        const int c = (o == 1) ? yv : (yv ? g.W - yv : 0);
-        *words = Hc;
-        return bimg + (size_t)g.H * Wc + (size_t)c * Hc;
-      };
-      int words;
-      const uint32_t* s0 = source_row(r, &words);
-      w00 = view_word(s0, words, o, v.Wv, i);
-      if (np == 3) {
-        const bool more = i + 1 < v.stride;
-        const uint32_t w01 = more ? view_word(s0, words, o, v.Wv, i + 1) : 0u;
-        e2 = w00 & __funnelshift_r(w00, w01, 1);
-        if (r + 1 < rows) {
-          const uint32_t* s1 = source_row(r + 1, &words);
-          const uint32_t w10 = view_word(s1, words, o, v.Wv, i);
-          const uint32_t w11 = more ? view_word(s1, words, o, v.Wv, i + 1) : 0u;
-          d2 = w00 & __funnelshift_r(w10, w11, 1);
-        }
-      }
+  // CTA -> (phase plane, view, image, tile)
+  const long long cta = blockIdx.x;
+  const int plane = (int)(cta / ctas_per_plane);
+  long long rem = cta - (long long)plane * ctas_per_plane;
+  int o = 0, tl = tiles.x;
+  if (rem >= (long long)Bpad * tl) { rem -= (long long)Bpad * tl; o = 1; tl = tiles.y; }
+  if (o == 1 && rem >= (long long)Bpad * tl) { rem -= (long long)Bpad * tl; o = 2; tl = tiles.z; }
+  if (o == 2 && rem >= (long long)Bpad * tl) { rem -= (long long)Bpad * tl; o = 3; tl = tiles.w; }
+  const ViewGeom& v = g.v[o];
+  const int b = (int)(rem / tl);
+  const int tile = (int)(rem - (long long)b * tl);
+  const int pv = v.view_words / np;                        // words of one plane of one image (rows * stride + padding)
+  const int stride = v.stride, rows = v.n_bands * g.band_rows + g.m;
+  const int w0 = tile * PACK_TILE, w1 = min(pv, w0 + PACK_TILE);
+  const int n_stage = min(w1 + stride + 2, rows * stride) - w0;      // staged words; beyond them everything is zero
+  uint32_t* dst = packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b * v.view_words;
+  if (b >= B) {                                            // padding images of the last CTA group: all-zero planes
+    for (int L = w0 + threadIdx.x; L < w1; L += blockDim.x) {
+      dst[L] = 0u;
+      if (np == 3) { dst[L + v.e2_view_off] = 0u; dst[L + 2 * (size_t)v.e2_view_off] = 0u; }
     }
-    uint32_t* dst = packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b * v.view_words + idx;
-    dst[0] = w00;
+    return;
+  }
+  const uint32_t* bimg = base + ((size_t)plane * B + b) * img_words;
+  const bool rowmajor = (o == 0 || o == 3);
+  const int words = rowmajor ? Wc : Hc;
+  for (int j = threadIdx.x; j < n_stage; j += blockDim.x) {
+    const int L = w0 + j;
+    const int r = L / stride, i = L - r * stride;
+    int yv = r;                                            // r < rows <= 2 Hv + band_rows: a few subtractions at most
+    while (yv >= v.Hv) yv -= v.Hv;
+    // source row of a view row: views 0, 3: image row yv (Brow); view 1: image column yv; view 2: column -yv
+    const uint32_t* src = rowmajor ? bimg + (size_t)yv * Wc
+                                   : bimg + (size_t)g.H * Wc + (size_t)((o == 1) ? yv : (yv ? g.W - yv : 0)) * Hc;
+    const int x0 = (int)((32u * (unsigned)i) % (unsigned)v.Wv);
+    s_plain[j] = (o == 3) ? periodic_word<true>(src, words, v.Wv, x0) : periodic_word<false>(src, words, v.Wv, x0);
+  }
+  __syncthreads();
+  for (int L = w0 + threadIdx.x; L < w1; L += blockDim.x) {
+    const int j = L - w0;
+    const uint32_t w00 = j < n_stage ? s_plain[j] : 0u;
+    dst[L] = w00;
     if (np == 3) {
-      dst[v.e2_view_off] = e2;
-      dst[2 * (size_t)v.e2_view_off] = d2;
+      const int r = L / stride, i = L - r * stride;
+      const bool more = i + 1 < stride;                    // the word right of the last one of a row reads as zero
+      const uint32_t w01 = (more && j + 1 < n_stage) ? s_plain[j + 1] : 0u;
+      const uint32_t w10 = (j + stride < n_stage) ? s_plain[j + stride] : 0u;
+      const uint32_t w11 = (more && j + stride + 1 < n_stage) ? s_plain[j + stride + 1] : 0u;
+      dst[L + v.e2_view_off] = w00 & __funnelshift_r(w00, w01, 1);
+      dst[L + 2 * (size_t)v.e2_view_off] = w00 & __funnelshift_r(w10, w11, 1);
     }
   }
 }
@@ -282,7 +293,7 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
         (const char*)(smem + (size_t)img_local * v.band_pitch + row0 * stride + (active ? strip : 0) * TX);
     const int rowstep = 32 * stride * 4;                     // bytes between the TY start rows of a thread
     const int b_img = b0 + img_local;
-    unsigned long long* cnt = p.counts + ((size_t)b_img * p.n_phase + plane) * (size_t)p.S * p.S;
+    unsigned long long* cnt = p.counts + (size_t)b_img * p.image_stride + (size_t)plane * p.S * p.S;
     const bool store = (lane == 0) && (b_img < p.B);
     mbar_wait(&bar, parity);
     parity ^= 1u;
@@ -744,25 +755,38 @@ __global__ void swap_mirror_kernel(int* __restrict__ delta, int S, long long n_a
 // ---------------------------------------------------------------------------------------------
 // host launch wrappers (called from lpf_api.cu)
 // ---------------------------------------------------------------------------------------------
-cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed, const Geom& g, int B, int n_phase,
-                        int phase0, unsigned int* counter, int n_sm, cudaStream_t st) {
+// Bpad: images per octant block of the packed layout (B rounded up to the CTA group; 1 for a start mask)
+cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed, const Geom& g, int B, int Bpad,
+                        int n_phase, int phase0, unsigned int* counter, int n_sm, cudaStream_t st) {
   const long long tiles = (long long)B * ((g.H + 31) / 32) * ((g.W + 31) / 32);
   long long blocks = (tiles + 7) / 8;
   blocks = std::max(1ll, std::min(blocks, (long long)n_sm * 16));
   pack_base_kernel<<<(unsigned)blocks, 256, 0, st>>>(images, base, B, g.H, g.W, n_phase, phase0, counter);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  const long long total = (long long)n_phase * g.plane_words / (g.v[0].e2_view_off > 0 ? 3 : 1);
-  blocks = (total + 255) / 256;
-  blocks = std::max(1ll, std::min(blocks, (long long)n_sm * 32));
-  pack_views_kernel<<<(unsigned)blocks, 256, 0, st>>>(base, packed, g, B, n_phase);
+  const int np = g.v[0].e2_view_off > 0 ? 3 : 1;
+  int tl[4], stride_max = 0;
+  long long per_plane = 0;
+  for (int o = 0; o < 4; ++o) {
+    tl[o] = (g.v[o].view_words / np + PACK_TILE - 1) / PACK_TILE;
+    per_plane += (long long)Bpad * tl[o];
+    stride_max = std::max(stride_max, g.v[o].stride);
+  }
+  if (per_plane * n_phase >= (1ll << 31)) return cudaErrorInvalidValue;
+  pack_views_kernel<<<(unsigned)(per_plane * n_phase), 256, (size_t)(PACK_TILE + stride_max + 2) * 4, st>>>(
+      base, packed, g, B, Bpad, make_int4(tl[0], tl[1], tl[2], tl[3]), per_plane);
   return cudaGetLastError();
 }
 
-cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem, int* blocks_per_sm) {
+// also raises the kernel's dynamic shared memory limit to the device maximum (once is enough, repeating is harmless),
+// so that launches of any plan fit whatever order the plans were made in
+cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem, int max_smem, int* blocks_per_sm) {
   eval_fn f = eval_fn_for(TX, TY, prune);
   if (!f) return cudaErrorInvalidValue;
-  cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncAttributes fa;
+  cudaError_t e = cudaFuncGetAttributes(&fa, f);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem - (int)fa.sharedSizeBytes);
   if (e != cudaSuccess) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, f, threads, smem);
 }
@@ -799,6 +823,14 @@ cudaError_t launch_objective(const long long* counts, const long long* target, i
   return cudaGetLastError();
 }
 
+cudaError_t swap_delta_prepare(size_t max_smem) {
+  cudaFuncAttributes fa;
+  cudaError_t e = cudaFuncGetAttributes(&fa, swap_delta_kernel_v3);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(swap_delta_kernel_v3, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)max_smem - (int)fa.sharedSizeBytes);
+}
+
 // phase 0 | 1: one plane, delta [n][S][S];  phase < 0: both planes, phase k at delta + k * plane_stride
 cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W, int m, int phase, const int* pairs,
                               long long n, const int32_t* rec, int n_nodes, int* delta, long long plane_stride,
@@ -809,8 +841,7 @@ cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W
   const size_t smem = (size_t)((n_planes * PH * PWc + 1) & ~1) * 4 + (size_t)8 * SWAP_STACK * 8;
   const long long img_words = (long long)H * Wc + (long long)W * Hc;
   uint32_t* const padded = bits + (size_t)n_planes * img_words;
-  cudaError_t e = cudaFuncSetAttribute(swap_delta_kernel_v3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
+  cudaError_t e = cudaSuccess;
   const long long S2 = (long long)(2 * m + 1) * (2 * m + 1);
   for (int pl = 0; pl < n_planes; ++pl) {
     e = cudaMemsetAsync(delta + pl * plane_stride, 0, sizeof(int) * (size_t)n * S2, st);

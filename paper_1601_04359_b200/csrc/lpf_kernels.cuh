@@ -54,7 +54,8 @@ struct EvalParams {
   int n_phase;                // 1 or 2 phase planes in `packed`
   const uint32_t* packed;     // [n_phase][4 octants][Bpad][view_words]
   int Bpad;
-  unsigned long long* counts; // [B][n_phase][S][S]
+  unsigned long long* counts; // [B][n_phase][S][S]  (lpf_eval_sum: [n_phase][S][S], image_stride 0)
+  long long image_stride;     // elements between the count arrays of consecutive images: n_phase * S * S, or 0
   int S;                      // 2m + 1
   unsigned int* counter;      // dynamic work counter, zeroed by the pack kernel
   int prune;

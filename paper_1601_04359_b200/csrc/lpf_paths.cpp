@@ -435,6 +435,14 @@ Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03
   return pr;
 }
 
+void drop_program(lpf_paths* p, const Program* pr) {
+  for (auto it = p->programs.begin(); it != p->programs.end(); ++it)
+    if (&it->second == pr) {
+      if (!pr->d_entries) p->programs.erase(it);
+      return;
+    }
+}
+
 int build_host_table(lpf_paths* p) {
   try {
     build_trie(p);

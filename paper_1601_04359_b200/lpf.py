@@ -21,8 +21,9 @@ EXPORTS = (
     "lpf_strerror", "lpf_last_cuda_error", "lpf_build_paths", "lpf_free_paths", "lpf_paths_info",
     "lpf_paths_get", "lpf_paths_program", "lpf_eval", "lpf_eval_both", "lpf_objective",
     "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
-    "lpf_set_tile", "lpf_alu_peak", "lpf_eval_masked", "lpf_anneal",
+    "lpf_set_tile", "lpf_alu_peak", "lpf_eval_masked", "lpf_anneal", "lpf_reserve", "lpf_eval_sum",
 )
+LPF_FOR_EVAL, LPF_FOR_EVAL_BOTH, LPF_FOR_MASKED, LPF_FOR_SWAP_DELTA, LPF_FOR_ANNEAL, LPF_FOR_HOST = 1, 2, 4, 8, 16, 32
 
 _lib = None
 
@@ -67,6 +68,10 @@ def load() -> ctypes.CDLL:
     lib.lpf_eval_both.restype = I
     lib.lpf_eval_masked.argtypes = [VP, VP, I, I, I, I, VP, VP, U, VP]
     lib.lpf_eval_masked.restype = I
+    lib.lpf_eval_sum.argtypes = [VP, VP, I, I, I, I, VP, U, VP]
+    lib.lpf_eval_sum.restype = I
+    lib.lpf_reserve.argtypes = [VP, I, I, I, U, U]
+    lib.lpf_reserve.restype = I
     lib.lpf_anneal.argtypes = [VP, VP, I, I, I, VP, VP, VP, I64, ctypes.c_double, ctypes.c_double, I64, I64, VP, VP,
                                ctypes.POINTER(ctypes.c_double), VP]
     lib.lpf_anneal.restype = I
@@ -174,16 +179,29 @@ def _torch():
     return torch
 
 
-def _stream_ptr(stream) -> int:
+def _stream_ptr(stream, *tensors) -> int:
+    """The launch stream as an integer; tensors handed to the C call are recorded on it, so that a temporary made by
+    .contiguous() is not recycled by torch's caching allocator before the enqueued kernels have read it."""
     torch = _torch()
     s = stream if stream is not None else torch.cuda.current_stream()
+    for t in tensors:
+        if t is not None and t.is_cuda:
+            t.record_stream(s)
     return int(s.cuda_stream)
 
 
-def _dev_images(images, ndim: int):
+def _on_device(p: "Paths", *tensors) -> None:
+    for t in tensors:
+        if t is not None and (not t.is_cuda or t.device.index != p.device):
+            raise ValueError("tensor on %s, but the lpf_paths table is bound to cuda:%d" % (t.device, p.device))
+
+
+def _dev_images(images, ndim: int, p: "Paths" = None):
     torch = _torch()
     if not (isinstance(images, torch.Tensor) and images.is_cuda and images.dtype == torch.uint8):
         raise TypeError("images must be a CUDA uint8 tensor")
+    if p is not None:
+        _on_device(p, images)
     if images.dim() == ndim - 1:
         images = images.unsqueeze(0)
     if images.dim() != ndim:
@@ -195,14 +213,15 @@ def lpf_eval(p: Paths, images, phase: int, flags: int = 0, out=None, stream=None
     """counts int64 [B, 2m+1, 2m+1] on the device; index [b, dy+m, dx+m]."""
     torch = _torch()
     lib = load()
-    images = _dev_images(images, 3)
+    images = _dev_images(images, 3, p)
     B, H, W = images.shape
     S = 2 * p.m + 1
     if out is None:
         out = torch.empty((B, S, S), dtype=torch.int64, device=images.device)
     assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() == B * S * S
+    _on_device(p, out)
     _check(lib.lpf_eval(p.handle, images.data_ptr(), B, H, W, int(phase), out.data_ptr(), int(flags),
-                        _stream_ptr(stream)), "lpf_eval")
+                        _stream_ptr(stream, images)), "lpf_eval")
     return out
 
 
@@ -210,14 +229,15 @@ def lpf_eval_both(p: Paths, images, flags: int = 0, out=None, stream=None):
     """counts int64 [B, 2, 2m+1, 2m+1]; index [b, phase, dy+m, dx+m]."""
     torch = _torch()
     lib = load()
-    images = _dev_images(images, 3)
+    images = _dev_images(images, 3, p)
     B, H, W = images.shape
     S = 2 * p.m + 1
     if out is None:
         out = torch.empty((B, 2, S, S), dtype=torch.int64, device=images.device)
     assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() == B * 2 * S * S
+    _on_device(p, out)
     _check(lib.lpf_eval_both(p.handle, images.data_ptr(), B, H, W, out.data_ptr(), int(flags),
-                             _stream_ptr(stream)), "lpf_eval_both")
+                             _stream_ptr(stream, images)), "lpf_eval_both")
     return out
 
 
@@ -226,18 +246,43 @@ def lpf_eval_masked(p: Paths, images, phase: int, start_mask, flags: int = 0, ou
     int64 [B, 2m+1, 2m+1], phase -1 both phases [B, 2, 2m+1, 2m+1]."""
     torch = _torch()
     lib = load()
-    images = _dev_images(images, 3)
+    images = _dev_images(images, 3, p)
     B, H, W = images.shape
     assert start_mask.is_cuda and start_mask.dtype == torch.uint8 and tuple(start_mask.shape) == (H, W)
+    _on_device(p, start_mask)
     start_mask = start_mask.contiguous()
     S = 2 * p.m + 1
     shape = (B, 2, S, S) if phase < 0 else (B, S, S)
     if out is None:
         out = torch.empty(shape, dtype=torch.int64, device=images.device)
     assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() == int(np.prod(shape))
+    _on_device(p, out)
     _check(lib.lpf_eval_masked(p.handle, images.data_ptr(), B, H, W, int(phase), start_mask.data_ptr(),
-                               out.data_ptr(), int(flags), _stream_ptr(stream)), "lpf_eval_masked")
+                               out.data_ptr(), int(flags), _stream_ptr(stream, images, start_mask)), "lpf_eval_masked")
     return out
+
+
+def lpf_eval_sum(p: Paths, images, phase: int, flags: int = 0, out=None, stream=None):
+    """Ensemble sum over the B images (PAPER.md:495): int64 [2m+1, 2m+1] (phase 0 | 1) or [2, 2m+1, 2m+1] (phase -1);
+    the ensemble average of L2 is out / (B * W * H)."""
+    torch = _torch()
+    lib = load()
+    images = _dev_images(images, 3, p)
+    B, H, W = images.shape
+    S = 2 * p.m + 1
+    shape = (2, S, S) if phase < 0 else (S, S)
+    if out is None:
+        out = torch.empty(shape, dtype=torch.int64, device=images.device)
+    assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() == int(np.prod(shape))
+    _check(lib.lpf_eval_sum(p.handle, images.data_ptr(), B, H, W, int(phase), out.data_ptr(), int(flags),
+                            _stream_ptr(stream, images)), "lpf_eval_sum")
+    return out
+
+
+def lpf_reserve(p: Paths, B: int, H: int, W: int, flags: int = 0, what: int = LPF_FOR_EVAL) -> None:
+    """Builds and uploads everything the calls named by `what` (LPF_FOR_*) need for B x H x W images: after it they
+    only enqueue work on their stream (no allocation, copy or host synchronisation)."""
+    _check(load().lpf_reserve(p.handle, int(B), int(H), int(W), int(flags), int(what)), "lpf_reserve")
 
 
 def lpf_anneal(p: Paths, image, phase: int, target, pairs, log_u, T_max: float, T_min: float, c_max: int, s_max: int,
@@ -246,6 +291,7 @@ def lpf_anneal(p: Paths, image, phase: int, target, pairs, log_u, T_max: float, 
     torch = _torch()
     lib = load()
     assert image.is_cuda and image.dtype == torch.uint8 and image.dim() == 2 and image.is_contiguous()
+    _on_device(p, image, target, pairs, log_u, accept_log)
     H, W = image.shape
     S = 2 * p.m + 1
     n_ph = 2 if phase < 0 else 1
@@ -262,7 +308,7 @@ def lpf_anneal(p: Paths, image, phase: int, target, pairs, log_u, T_max: float, 
     _check(lib.lpf_anneal(p.handle, image.data_ptr(), H, W, int(phase), target.data_ptr(), pairs.data_ptr(),
                           log_u.data_ptr(), pairs.shape[0], float(T_max), float(T_min), int(c_max), int(s_max),
                           counts.data_ptr(), accept_log.data_ptr() if accept_log is not None else None, stats,
-                          _stream_ptr(stream)), "lpf_anneal")
+                          _stream_ptr(stream, target, pairs, log_u)), "lpf_anneal")
     keys = ("steps", "accepted", "levels", "T", "E")
     return counts, dict(zip(keys, [float(v) for v in stats]))
 
@@ -281,8 +327,8 @@ def lpf_objective(counts, target, out=None, stream=None):
     if out is None:
         out = torch.empty((B,), dtype=torch.int64, device=counts.device)
     with torch.cuda.device(counts.device):
-        _check(lib.lpf_objective(counts.data_ptr(), target.data_ptr(), B, K, out.data_ptr(), _stream_ptr(stream)),
-               "lpf_objective")
+        _check(lib.lpf_objective(counts.data_ptr(), target.data_ptr(), B, K, out.data_ptr(),
+                                 _stream_ptr(stream, counts, target)), "lpf_objective")
     return out
 
 
@@ -290,19 +336,21 @@ def lpf_swap_delta(p: Paths, image, phase: int, pairs, out=None, stream=None):
     """delta int32 [n, 2m+1, 2m+1] for n independent two-pixel swaps (pairs int32 [n, 4])."""
     torch = _torch()
     lib = load()
-    image = _dev_images(image, 3)
+    image = _dev_images(image, 3, p)
     if image.shape[0] != 1:
         raise ValueError("lpf_swap_delta takes one base image")
     _, H, W = image.shape
     assert pairs.is_cuda and pairs.dtype == torch.int32 and pairs.dim() == 2 and pairs.shape[1] == 4
+    _on_device(p, pairs)
     pairs = pairs.contiguous()
     n = pairs.shape[0]
     S = 2 * p.m + 1
     if out is None:
         out = torch.empty((n, S, S), dtype=torch.int32, device=image.device)
     assert out.is_cuda and out.dtype == torch.int32 and out.is_contiguous() and out.numel() == n * S * S
+    _on_device(p, out)
     _check(lib.lpf_swap_delta(p.handle, image.data_ptr(), H, W, int(phase), pairs.data_ptr(), n, out.data_ptr(),
-                              _stream_ptr(stream)), "lpf_swap_delta")
+                              _stream_ptr(stream, image, pairs)), "lpf_swap_delta")
     return out
 
 
@@ -329,9 +377,10 @@ def lpf_eval_host(p: Paths, images_host, phase: int, counts_host=None, flags: in
 
 def lpf_last_launch_info(p: Paths) -> dict:
     lib = load()
-    out = (ctypes.c_int64 * 8)()
+    out = (ctypes.c_int64 * 13)()
     _check(lib.lpf_last_launch_info(p.handle, out), "lpf_last_launch_info")
-    keys = ("kernels", "work_items", "program_entries", "grid", "block", "smem_bytes", "tile", "G")
+    keys = ("kernels", "work_items", "program_entries", "grid", "block", "smem_bytes", "tile", "G", "eroded",
+            "fused_pairs", "singles", "terminals", "piece_nodes")
     return dict(zip(keys, [int(v) for v in out]))
 
 

@@ -61,3 +61,27 @@ def test_masked_counts_pins():
         pth = orc.path(int(dx), int(dy))
         want = int(all(img[(y0 + int(py)) % H, (x0 + int(px)) % W] == 1 for px, py in pth))
         assert got[i] == want
+
+
+# ---- ensemble sum over an image stack ("averaged over 100 slices") -------------------------------
+
+def test_counts_sum_pins():
+    rows = ["110111", "111101", "011111", "111011"]            # tests/golden/worked_image.txt (hand-derived counts)
+    img = np.array([[int(c) for c in r] for r in rows], dtype=np.uint8)
+    gold1 = np.array([[13, 13, 12, 14, 15], [14, 16, 16, 17, 13], [12, 16, 20, 16, 12], [13, 17, 16, 16, 14],
+                      [15, 14, 12, 13, 13]])
+    assert np.array_equal(orc.counts_sum(np.stack([img] * 3), 1, 2), 3 * gold1)    # k copies = k x the golden counts
+    # the worked image and its complement: phase 1 of the pair = golden phase 1 + golden phase 0
+    gold0 = np.zeros((5, 5), dtype=np.int64)
+    gold0[2, 2], gold0[1, 3], gold0[3, 1] = 4, 1, 1
+    assert np.array_equal(orc.counts_sum(np.stack([img, 1 - img]), 1, 2), gold1 + gold0)
+    rng = np.random.default_rng(8)
+    stack = (rng.random((7, 9, 13)) < 0.7).astype(np.uint8)
+    m = 6
+    one = orc.counts_sum(stack[:1], 1, m)
+    assert np.array_equal(one, orc.counts(stack[0], 1, m, full_template=True))     # B = 1: the single-image function
+    whole = orc.counts_sum(stack, 1, m)
+    assert np.array_equal(whole, orc.counts_sum(stack[:3], 1, m) + orc.counts_sum(stack[3:], 1, m))   # additive
+    assert whole[m, m] == int(stack.sum())                                          # Eq. 10 summed over the stack
+    assert np.array_equal(whole, whole[::-1, ::-1])                                 # Eq. 12
+    assert np.array_equal(orc.counts_sum(stack, 0, m)[m, m], (stack == 0).sum())

@@ -1,9 +1,16 @@
 """GPU parity: the CUDA path behind the C ABI (liblpf.so) against the CPU oracle, bit-exact
 (integer counts: SURVEY.md 8(c) S14), on the same seeded inputs (paper_1601_04359_b200.inputs).
 
-Small/medium cases compare element by element; the full-size configs 3 and 4 compare sampled
-vectors / images that the oracle can compute one by one, plus properties that hold at any size
-(Eq. 10 and Eq. 12 of the paper; prefix monotonicity)."""
+Small/medium cases compare element by element with the oracle called in the test.  The full-size configs
+3, 4 and 5 are compared IN FULL with digests of the oracle's result (tests/golden/*.digest.txt, written by
+tests/golden/make_full_size_digests.py, which calls only oracle/): sha256 of the whole array plus a crc32 per
+row / image / proposal so that a mismatch is located; on top of that sampled vectors / images are compared with
+the oracle called here, and properties that hold at any size are checked (Eq. 10 and Eq. 12 of the paper,
+PAPER.md:131-148; prefix monotonicity)."""
+import hashlib
+import os
+import zlib
+
 import numpy as np
 import pytest
 
@@ -25,6 +32,25 @@ def paths(m):
 
 def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def digest_lines(name):
+    out = []
+    for line in open(os.path.join(GOLDEN, name)):
+        if line.strip() and not line.startswith("#"):
+            out.append(line.split())
+    return out
+
+
+def crc(a):
+    return "%08x" % (zlib.crc32(np.ascontiguousarray(a).tobytes()) & 0xFFFFFFFF)
+
+
+def sha(a):
+    return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
 
 
 def gpu_counts(img, phase, m, flags=0):
@@ -165,6 +191,23 @@ def test_config3_sampled_vectors_and_properties():
     assert np.array_equal(pruned, got)
 
 
+def test_config3_whole_template_against_the_oracle_digest():
+    """ALL 2 x 513 x 513 counts of config 3 against the oracle's (tests/golden/config3_counts.digest.txt): crc32 of
+    every row, then sha256 of the whole array; default flags, LPF_PRUNE and LPF_NO_E2."""
+    img = inputs.config_image(3)
+    m = 256
+    lines = digest_lines("config3_counts.digest.txt")
+    want_sha = [t[1] for t in lines if t[0] == "sha256"][0]
+    rows = {(int(t[1]), int(t[2])): t[3] for t in lines if t[0] == "row"}
+    assert len(rows) == 2 * (2 * m + 1)
+    for flags in (0, lpf.LPF_PRUNE, lpf.LPF_NO_E2):
+        got = lpf.lpf_eval_both(paths(m), dev(img[None]), flags).cpu().numpy()[0].astype("<i8")
+        bad = [(ph, r) for ph in (0, 1) for r in range(2 * m + 1) if crc(got[ph, r]) != rows[(ph, r)]]
+        assert not bad, (flags, bad[:10])
+        assert sha(got) == want_sha, flags
+        assert lpf.lpf_last_launch_info(paths(m))["eroded"] == (0 if flags & lpf.LPF_NO_E2 else 1)
+
+
 def test_config4_sampled_images_properties_and_objective():
     B = 1024
     imgs, target_img = inputs.config4_batch(B)
@@ -176,7 +219,16 @@ def test_config4_sampled_images_properties_and_objective():
     counts = d_counts.cpu().numpy()
     target = d_target.cpu().numpy()[0]
     assert np.array_equal(target, orc.counts(target_img, 1, m))
-    for b in (0, 1, 511, 777, 1023):
+    # ALL 1024 images against the oracle's digest: crc32 of every image's counts, its exact squared error, sha256 of all
+    lines = digest_lines("config4_counts.digest.txt")
+    per_img = {int(t[1]): (t[2], int(t[3])) for t in lines if t[0] == "img"}
+    assert len(per_img) == B
+    assert crc(target.astype("<i8")) == [t[1] for t in lines if t[0] == "target"][0]
+    bad = [b for b in range(B) if crc(counts[b].astype("<i8")) != per_img[b][0] or int(sse[b]) != per_img[b][1]]
+    assert not bad, bad[:10]
+    assert sha(counts.astype("<i8")) == [t[1] for t in lines if t[0] == "sha256"][0]
+    # 64 images element by element against the oracle called here (every 16th, the last group included)
+    for b in list(range(0, B, 16))[:62] + [1022, 1023]:
         want = orc.counts(imgs[b], 1, m)
         assert np.array_equal(counts[b], want), b
         assert int(sse[b]) == orc.sse(want, target)
@@ -198,7 +250,23 @@ def test_objective_exact_large_values():
         assert int(got[b]) == orc.sse(c[b], t)
 
 
-def test_config5_swap_delta():
+def _swapped_images(d_img, d_pairs):
+    """[n, H, W] copies of the base image with the two pixels of each proposal exchanged (built on the device)."""
+    n = d_pairs.shape[0]
+    mod = d_img.expand(n, -1, -1).contiguous()
+    idx = torch.arange(n, device=d_img.device)
+    xp, yp, xq, yq = (d_pairs[:, k].long() for k in range(4))
+    bp, bq = d_img[0, yp, xp], d_img[0, yq, xq]
+    mod[idx, yp, xp] = bq
+    mod[idx, yq, xq] = bp
+    return mod
+
+
+def test_config5_swap_delta_all_proposals():
+    """Config 5: 100 000 proposals on the 256 x 256 disk image, m = 64.  (i) EVERY delta against a full re-evaluation
+    of I' by lpf_eval (itself verified against the oracle) minus the base counts; (ii) the first 1000 (phase 1) and 200
+    (phase 0) against the oracle's definition-level delta through its digest; (iii) 24 + 3 against the oracle called
+    here (local form / full re-evaluation); invariants on all."""
     img = inputs.config_image(5)
     m = 64
     p = paths(m)
@@ -206,38 +274,53 @@ def test_config5_swap_delta():
     pairs = inputs.config5_pairs(img, n)
     d_img = dev(img[None])
     d_pairs = dev(pairs)
-    base = lpf.lpf_eval(p, d_img, 1)[0]
     S = 2 * m + 1
-    # a chunk of the 100000 proposals at a time (6.66 GB of int32 in total)
-    chunk = 10000
-    checked = 0
-    sums = []
-    for s0 in range(0, n, chunk):
-        d = lpf.lpf_swap_delta(p, d_img, 1, d_pairs[s0:s0 + chunk])
-        assert d.shape == (chunk, S, S)
-        assert bool((d[:, m, m] == 0).all())                          # volume fraction preserved
-        assert bool((d == d.flip(1, 2)).all())                        # delta(v) = delta(-v)
-        sums.append(d.sum(dim=(1, 2)).cpu().numpy())
-        if s0 == 0:
-            dn = d[:64].cpu().numpy()
-            # oracle, local form, 24 proposals; full re-evaluation (the definition), 3 proposals
-            for i in range(24):
-                assert np.array_equal(dn[i], orc.swap_delta_local(img, 1, m, pairs[i])), i
-            for i in range(3):
-                assert np.array_equal(dn[i], orc.swap_delta_full(img, 1, m, pairs[i])), i
-            # GPU full re-evaluation of I' for 64 proposals
-            mod = np.repeat(img[None], 64, axis=0)
-            for i in range(64):
-                xp, yp, xq, yq = pairs[i]
-                mod[i, yp, xp], mod[i, yq, xq] = img[yq, xq], img[yp, xp]
-            re = lpf.lpf_eval(p, dev(mod), 1) - base[None]
-            assert np.array_equal(re.cpu().numpy(), dn.astype(np.int64))
-            checked += 64
-    assert checked == 64 and len(sums) == n // chunk
-    # phase 0 deltas of the same proposals
-    d0 = lpf.lpf_swap_delta(p, d_img, 0, d_pairs[:8]).cpu().numpy()
-    for i in range(4):
-        assert np.array_equal(d0[i], orc.swap_delta_local(img, 0, m, pairs[i]))
+    dig = {(int(t[1]), int(t[2])): t[3] for t in digest_lines("config5_deltas.digest.txt") if t[0] == "swap"}
+    assert sum(1 for k in dig if k[0] == 1) == 1000 and sum(1 for k in dig if k[0] == 0) == 200
+    for phase, count in ((1, n), (0, 4000)):
+        base = lpf.lpf_eval(p, d_img, phase)[0]
+        assert np.array_equal(base.cpu().numpy(), orc.counts(img, phase, m))
+        chunk = 2000
+        for s0 in range(0, count, chunk):
+            d = lpf.lpf_swap_delta(p, d_img, phase, d_pairs[s0:s0 + chunk])
+            assert d.shape == (chunk, S, S)
+            assert bool((d[:, m, m] == 0).all())                          # volume fraction preserved
+            assert bool((d == d.flip(1, 2)).all())                        # delta(v) = delta(-v)
+            re = lpf.lpf_eval(p, _swapped_images(d_img, d_pairs[s0:s0 + chunk]), phase) - base[None]
+            same = (re == d.to(torch.int64)).flatten(1).all(dim=1)
+            assert bool(same.all()), (phase, s0, torch.nonzero(~same).flatten()[:10].tolist())
+            if s0 == 0:
+                dn = d.cpu().numpy().astype("<i4")
+                lim = 1000 if phase == 1 else 200
+                bad = [i for i in range(lim) if crc(dn[i]) != dig[(phase, i)]]
+                assert not bad, (phase, bad[:10])
+                for i in range(24 if phase == 1 else 6):
+                    assert np.array_equal(dn[i], orc.swap_delta_local(img, phase, m, pairs[i])), i
+                for i in range(3 if phase == 1 else 1):
+                    assert np.array_equal(dn[i], orc.swap_delta_full(img, phase, m, pairs[i])), i
+            del d, re
+
+
+def test_swap_delta_dense_image_overflows_the_warp_stacks():
+    """An image that is >= 95 % in phase: almost every prefix survives, the per-warp stacks of swap_delta_kernel_v3
+    fill up and the serial fall-back walk runs.  Every delta against full re-evaluation on the GPU, a few against the
+    oracle; both phases."""
+    H = W = 160
+    m = 64
+    rng = np.random.default_rng(95)
+    img = (rng.random((H, W)) < 0.97).astype(np.uint8)
+    p = paths(m)
+    pairs = inputs.swap_pairs(img, 96, 96)
+    d_img, d_pairs = dev(img[None]), dev(pairs)
+    for phase in (1, 0):
+        base = lpf.lpf_eval(p, d_img, phase)[0]
+        d = lpf.lpf_swap_delta(p, d_img, phase, d_pairs)
+        re = lpf.lpf_eval(p, _swapped_images(d_img, d_pairs), phase) - base[None]
+        assert bool((re == d.to(torch.int64)).all()), phase
+        dn = d.cpu().numpy()
+        for i in range(3):
+            assert np.array_equal(dn[i], orc.swap_delta_local(img, phase, m, pairs[i])), (phase, i)
+    assert int(d_img.sum()) > 0.95 * H * W
 
 
 def test_swap_delta_small_and_degenerate_pairs():
@@ -457,3 +540,144 @@ def test_hypothesis_generated_small_cases():
             assert np.array_equal(one[b], both[b, 1])
 
     check()
+
+
+# ---- the plain-plane program at full size, the automatic fall-back, the boundary contract --------------------
+
+def test_no_e2_and_plain_fallback_at_full_size():
+    """LPF_NO_E2 on a 256 x 384 image and a shape where the geometry chooser itself falls back to the plain plane
+    (300 x 300, m = 299: the two eroded bands would leave too few resident warps); which program ran is read from
+    lpf_last_launch_info.  Sampled vectors against the oracle, both phases, plus Eq. 10 / Eq. 12."""
+    for H, W, m, flags, eroded in ((256, 384, 120, lpf.LPF_NO_E2, 0), (256, 384, 120, 0, 1), (300, 300, 299, 0, 0)):
+        img = inputs.disks(H, W, 7.0, 0.45, inputs.seed_for(8, H + m))
+        rng = np.random.default_rng(m)
+        vecs = rng.integers(-m, m + 1, size=(300, 2))
+        vecs[:6] = [(0, 0), (m, m), (-m, m), (m, 0), (0, m), (-m, 1)]
+        got = lpf.lpf_eval_both(paths(m), dev(img[None]), flags).cpu().numpy()[0]
+        assert lpf.lpf_last_launch_info(paths(m))["eroded"] == eroded, (H, W, m, flags)
+        for phase in (0, 1):
+            want, _ = orc.counts_list(img, phase, vecs)
+            assert np.array_equal(got[phase][vecs[:, 1] + m, vecs[:, 0] + m], want), (H, W, m, flags, phase)
+            _properties(got[phase], img, phase, m)
+
+
+def test_reserved_calls_only_enqueue_cuda_graph_capture():
+    """After lpf_reserve the hot calls neither allocate, copy synchronously nor synchronise: they can
+    be captured into a CUDA graph (a cudaMalloc / cudaMemcpy / stream sync inside would abort the capture), and the
+    replayed graph gives the oracle's counts for NEW image contents."""
+    H, W, m, B = 96, 128, 40, 6
+    p = lpf.lpf_build_paths(m, 0)
+    try:
+        lpf.lpf_reserve(p, B, H, W, 0, lpf.LPF_FOR_EVAL | lpf.LPF_FOR_EVAL_BOTH | lpf.LPF_FOR_SWAP_DELTA)
+        lpf.lpf_reserve(p, B, H, W, 0, lpf.LPF_FOR_EVAL | lpf.LPF_FOR_MASKED)
+        rng = np.random.default_rng(17)
+        imgs = (rng.random((B, H, W)) < 0.75).astype(np.uint8)
+        d_imgs = dev(np.zeros_like(imgs))
+        d_mask = dev((rng.random((H, W)) < 0.5).astype(np.uint8))
+        S = 2 * m + 1
+        out1 = torch.zeros((B, S, S), dtype=torch.int64, device="cuda")
+        out2 = torch.zeros((B, 2, S, S), dtype=torch.int64, device="cuda")
+        outm = torch.zeros((B, S, S), dtype=torch.int64, device="cuda")
+        outs = torch.zeros((S, S), dtype=torch.int64, device="cuda")
+        sse = torch.zeros((B,), dtype=torch.int64, device="cuda")
+        pairs = inputs.swap_pairs(imgs[0], 16, 3)
+        d_pairs = dev(pairs)
+        delta = torch.zeros((16, S, S), dtype=torch.int32, device="cuda")
+        side = torch.cuda.Stream()
+        graph = torch.cuda.CUDAGraph()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.graph(graph, stream=side):
+            st = torch.cuda.current_stream()
+            lpf.lpf_eval(p, d_imgs, 1, out=out1, stream=st)
+            lpf.lpf_eval_both(p, d_imgs, out=out2, stream=st)
+            lpf.lpf_eval_masked(p, d_imgs, 1, d_mask, out=outm, stream=st)
+            lpf.lpf_eval_sum(p, d_imgs, 1, out=outs, stream=st)
+            lpf.lpf_objective(out1, out1[0], out=sse, stream=st)
+            lpf.lpf_swap_delta(p, d_imgs[:1], 1, d_pairs, out=delta, stream=st)
+        d_imgs.copy_(dev(imgs))                                   # new contents: the graph must recompute
+        graph.replay()
+        torch.cuda.synchronize()
+        c1, c2 = out1.cpu().numpy(), out2.cpu().numpy()
+        for b in range(B):
+            want1 = orc.counts(imgs[b], 1, m)
+            assert np.array_equal(c1[b], want1) and np.array_equal(c2[b, 1], want1)
+            assert np.array_equal(c2[b, 0], orc.counts(imgs[b], 0, m))
+            assert int(sse[b]) == orc.sse(want1, c1[0])
+        assert np.array_equal(outs.cpu().numpy(), orc.counts_sum(imgs, 1, m))
+        mv = np.array([(0, 0), (1, 0), (-3, 2), (m, m), (-m, 1), (7, 40)])
+        assert np.array_equal(outm.cpu().numpy()[2][mv[:, 1] + m, mv[:, 0] + m],
+                              orc.counts_masked(imgs[2], d_mask.cpu().numpy(), 1, mv))
+        dn = delta.cpu().numpy()
+        for i in range(4):
+            assert np.array_equal(dn[i], orc.swap_delta_local(imgs[0], 1, m, pairs[i]))
+    finally:
+        lpf.lpf_free_paths(p)
+
+
+def test_calls_return_before_the_device_has_finished():
+    """Asynchrony seen from the host: right after lpf_eval_both of config 3 returns, an event recorded behind it is
+    not yet complete (the evaluation takes milliseconds; the call only enqueued it)."""
+    img = inputs.config_image(3)
+    p = paths(256)
+    d_img = dev(img[None])
+    out = lpf.lpf_eval_both(p, d_img)                             # plans and workspace exist from here on
+    torch.cuda.synchronize()
+    ev = torch.cuda.Event()
+    not_ready = 0
+    for _ in range(5):
+        lpf.lpf_eval_both(p, d_img, out=out)
+        ev.record()
+        not_ready += not ev.query()
+        torch.cuda.synchronize()
+    assert not_ready >= 4
+
+
+def test_two_streams_share_one_table_safely():
+    """Consecutive calls on DIFFERENT streams share the packed-image workspace: the library orders them on the device
+    (event wait, no host sync), so both results are right."""
+    rng = np.random.default_rng(23)
+    H, W, m = 128, 160, 50
+    a = (rng.random((3, H, W)) < 0.7).astype(np.uint8)
+    b = (rng.random((3, H, W)) < 0.4).astype(np.uint8)
+    p = paths(m)
+    d_a, d_b = dev(a), dev(b)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    outs = []
+    for rep in range(6):
+        st, src = (s1, d_a) if rep % 2 == 0 else (s2, d_b)
+        with torch.cuda.stream(st):
+            outs.append(lpf.lpf_eval(p, src, 1, stream=st))
+    torch.cuda.synchronize()
+    want_a = np.stack([orc.counts(a[i], 1, m) for i in range(3)])
+    want_b = np.stack([orc.counts(b[i], 1, m) for i in range(3)])
+    for rep, o in enumerate(outs):
+        assert np.array_equal(o.cpu().numpy(), want_a if rep % 2 == 0 else want_b), rep
+    # the host-buffer entry runs on a private stream and is ordered behind work in flight on the table too
+    lpf.lpf_eval(p, d_a, 1, stream=s1)
+    got = lpf.lpf_eval_host(p, b, 1)
+    assert np.array_equal(got, want_b)
+
+
+# ---- ensemble sum over an image stack (lpf_eval_sum, PAPER.md:495) ----------------------------------------------
+
+def test_eval_sum_hundred_slices():
+    """100 slices of 100 x 100 (the paper's bone specimen is 100^3 voxels, its descriptor the average over 100 slices,
+    PAPER.md:493-495): the device-side ensemble sum against the oracle's, one phase, both phases, pruned, and S2."""
+    B, H, W, m = 100, 100, 100, 49
+    stack = np.stack([inputs.disks(H, W, 5.0, 0.3, inputs.seed_for(9, i)) for i in range(B)])
+    p = paths(m)
+    d = dev(stack)
+    want = [orc.counts_sum(stack, ph, m) for ph in (0, 1)]
+    for flags in (0, lpf.LPF_PRUNE):
+        assert np.array_equal(lpf.lpf_eval_sum(p, d, 1, flags).cpu().numpy(), want[1])
+        both = lpf.lpf_eval_sum(p, d, -1, flags).cpu().numpy()
+        assert np.array_equal(both[0], want[0]) and np.array_equal(both[1], want[1])
+    # against the per-image call summed on the device
+    per = lpf.lpf_eval(p, d, 1).sum(dim=0).cpu().numpy()
+    assert np.array_equal(per, want[1])
+    s2 = lpf.lpf_eval_sum(p, d[:7], 1, lpf.LPF_S2).cpu().numpy()
+    assert np.array_equal(s2, sum(orc.s2_counts(stack[i], 1, m) for i in range(7)))
+    # a ragged stack: B not a multiple of the images per CTA
+    r = lpf.lpf_eval_sum(p, d[:13], 0).cpu().numpy()
+    assert np.array_equal(r, orc.counts_sum(stack[:13], 0, m))
