@@ -61,6 +61,52 @@ def nominal_tests(w):
     return w["B"] * w["n_phase"] * w["H"] * w["W"] * S * S
 
 
+def survey_ops(w, info):
+    """SURVEY.md 8(d)'s op model: per image-phase Nw * (2 * trie nodes + 2 * half vectors) -- (SHF + LOP3) per word-node,
+    (POPC + add) per word-terminal.  The design needs fewer (below), so this is kept as a secondary figure only."""
+    nw = w["H"] * w["W"] // 32
+    return w["B"] * w["n_phase"] * nw * (2 * info["n_trie_nodes"] + 2 * info["n_half_vectors"])
+
+
+def design_ops(w, launch):
+    """Data operations the DESIGN executes at minimum, from the program that was actually uploaded (replayed on the host
+    by the library, lpf_last_launch_info): per image-phase and per start word, a fused pair of entries costs 2 SHF + 1
+    LOP3, an entry on its own 1 SHF + 1 LOP3, a terminal 1 POPC + 1 add.  Times the H*W/32 start words of an image
+    (not the padded strips), images and phases.  Overhead instructions (loads, entry decode, reductions) are not counted:
+    this is the numerator of a utilisation, so it is <= the ALU pipe's executed count."""
+    nw = w["H"] * w["W"] // 32
+    per_word = 3 * launch["fused_pairs"] + 2 * launch["singles"] + 2 * launch["terminals"]
+    return w["B"] * w["n_phase"] * nw * per_word
+
+
+def csrc_digest():
+    """sha256 over the CUDA/C++ sources and the public header: the key of profiles/capture_index.csv, so that ncu
+    figures are only quoted for the kernels they were captured from."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_1601_04359_b200", "csrc")
+    for name in sorted(os.listdir(csrc)) + [os.path.join("..", "..", "include", "lpf.h")]:
+        with open(os.path.join(csrc, name), "rb") as f:
+            h.update(name.encode() + b"\0" + f.read())
+    return h.hexdigest()[:16]
+
+
+def capture_lookup(workload, flags):
+    """ncu figures of the eval kernel for (these sources, workload, flags) from profiles/capture_index.csv, or None."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "capture_index.csv")
+    if not os.path.exists(path):
+        return None
+    key = csrc_digest()
+    for row in csv.DictReader(open(path)):
+        if row["csrc_sha256"] == key and row["workload"] == workload and row["flags"] == (flags or "none"):
+            out = {k: float(row[k]) for k in ("alu_pipe_pct", "smem_wavefront_pct", "issue_active_pct",
+                                              "dram_read_bytes", "dram_write_bytes", "gpu_time_us")}
+            out["source"] = row["source"]
+            return out
+    return None
+
+
 class ClockSampler(threading.Thread):
     """nvidia-smi clocks/throttle reasons sampled during the timed region (B200_PROFILING.md)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -222,6 +268,59 @@ def run_tab1(lpf, torch, device, out_dir):
     return rows
 
 
+FIG7_N = (100, 200, 500, 1000, 2000, 4000, 6000, 8000, 9000, 9500, 10000)
+
+
+def run_fig7(lpf, torch, device, out_dir):
+    """Fig. 7-shaped study: error of the N-position approximation L2~ of the
+    lineal path function against the exact L2, Eq. 14: e = sum over D of (L2 - L2~)^2, as a function of the number N of
+    start positions, drawn as a random N-combination WITHOUT repetition, on three 100 x 100 images (the paper's three
+    are not in the container: a chess board with 10 px fields, a suspension of 4 x 4 squares and a disk model stand in),
+    entire domain (m = 99), both phases.  L2 = counts / (W H), L2~ = masked counts / N.  e must be exactly 0 at
+    N = W H.  One point per image is re-checked against the CPU oracle in the run."""
+    from oracle import lpf_oracle as orc
+    H = W = 100
+    m = 99
+    S = 2 * m + 1
+    p = lpf.lpf_build_paths(m, device)
+    lpf.lpf_reserve(p, 1, H, W, 0, lpf.LPF_FOR_EVAL_BOTH)
+    lpf.lpf_reserve(p, 1, H, W, 0, lpf.LPF_FOR_EVAL_BOTH | lpf.LPF_FOR_MASKED)
+    half = (torch.arange(S * S, device="cuda") >= m * S + m).reshape(S, S)        # D of Eq. 13
+    images = {"chess 10 px": inputs.chess(H, W, 10), "squares 4 px, 0.20": inputs.squares(H, W, 4, 0.20, inputs.seed_for(6, 100)),
+              "disks r = 8, 0.45": inputs.disks(H, W, 8.0, 0.45, inputs.seed_for(10))}
+    rows = []
+    for name, img in images.items():
+        d_img = torch.from_numpy(img[None]).cuda()
+        exact = lpf.lpf_eval_both(p, d_img)[0].double() / (W * H)
+        rng = np.random.default_rng(inputs.seed_for(10, 1))
+        order = rng.permutation(H * W)                        # nested N-combinations without repetition
+        for N in FIG7_N:
+            mask = np.zeros(H * W, dtype=np.uint8)
+            mask[order[:N]] = 1
+            d_mask = torch.from_numpy(mask.reshape(H, W)).cuda()
+            got = lpf.lpf_eval_masked(p, d_img, -1, d_mask)[0]
+            err = (((exact - got.double() / N) ** 2) * half).sum(dim=(1, 2)).cpu().numpy()
+            rows.append({"image": name, "N": N, "e_phase0": float(err[0]), "e_phase1": float(err[1])})
+            if N == 1000:                                     # spot check of the masked counts against the oracle
+                vecs = rng.integers(-m, m + 1, size=(60, 2))
+                vecs = np.array([v if (v[1] > 0 or (v[1] == 0 and v[0] >= 0)) else -v for v in vecs])
+                for ph in (0, 1):
+                    want = orc.counts_masked(img, mask.reshape(H, W), ph, vecs)
+                    if not np.array_equal(got[ph].cpu().numpy()[vecs[:, 1] + m, vecs[:, 0] + m], want):
+                        raise AssertionError("fig7: masked counts differ from the oracle (%s, phase %d)" % (name, ph))
+        if rows[-1]["e_phase0"] != 0.0 or rows[-1]["e_phase1"] != 0.0:
+            raise AssertionError("fig7: the error at N = WH is not zero")
+    lpf.lpf_free_paths(p)
+    os.makedirs(out_dir, exist_ok=True)
+    with open(os.path.join(out_dir, "fig7.json"), "w") as f:
+        json.dump(rows, f, indent=1)
+    with open(os.path.join(out_dir, "fig7.md"), "w") as f:
+        f.write("| image (100 x 100, m = 99) | N | e(L2, phase 0) | e(L2, phase 1) |\n|---|---|---|---|\n")
+        for r in rows:
+            f.write("| %s | %d | %.4e | %.4e |\n" % (r["image"], r["N"], r["e_phase0"], r["e_phase1"]))
+    return rows
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -230,6 +329,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--flags", default="")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank evaluates its own full workload; strong (cfg4) = the ONE batch of 1024 "
+                         "images is split over the ranks (PAPER.md:353) and the count slices are all-gathered")
+    ap.add_argument("--fig7", action="store_true",
+                    help="also run the Fig. 7-shaped study of the N-position approximation (PAPER.md:160-172) and write "
+                         "gpurun_out/fig7.{json,md}")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the secondary workloads in the same JSON line")
     ap.add_argument("--tab1", action="store_true",
@@ -268,21 +373,30 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
-    def measure(wl, steps, warmup, with_e2e):
-        """Times `steps` steps of workload wl. Returns dict of results for this rank (max over ranks applied)."""
-        imgs, target_img = make_images(wl, rank)
+    def measure(wl, steps, warmup, with_e2e, strong=False):
+        """Times `steps` steps of workload wl. Returns dict of results for this rank (max over ranks applied).
+        strong: all ranks hold the same batch, rank r evaluates the images lpf_dist.shard_range(B, r, world) and the
+        per-rank count slices are all-gathered (the one collective of the split path) inside the timed region."""
+        strong = strong and world > 1 and wl["B"] >= world
+        imgs, target_img = make_images(wl, 0 if strong else rank)
+        b0, b1 = lpf_dist.shard_range(wl["B"], rank, world) if strong else (0, wl["B"])
+        imgs = imgs[b0:b1]
+        B_loc = b1 - b0
         p = lpf.lpf_build_paths(wl["m"], local_rank)      # paper step 1: untimed (PAPER.md:312)
         info = lpf.lpf_paths_info(p)
         d_imgs = torch.from_numpy(imgs).cuda()
         Sw = 2 * wl["m"] + 1
-        shape = (wl["B"], 2, Sw, Sw) if wl["n_phase"] == 2 else (wl["B"], Sw, Sw)
+        shape = (B_loc, 2, Sw, Sw) if wl["n_phase"] == 2 else (B_loc, Sw, Sw)
         d_counts = torch.empty(shape, dtype=torch.int64, device="cuda")
+        d_all = lpf_dist.gather_buffer(d_counts, wl["B"], world) if strong else None
         d_target = d_sse = None
         if target_img is not None:
             d_target = lpf.lpf_eval(p, torch.from_numpy(target_img[None]).cuda(), 1)[0].clone()
-            d_sse = torch.empty((wl["B"],), dtype=torch.int64, device="cuda")
+            d_sse = torch.empty((B_loc,), dtype=torch.int64, device="cuda")
         flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
         stream = torch.cuda.current_stream()
+        lpf.lpf_reserve(p, B_loc, wl["H"], wl["W"], flags,
+                        (lpf.LPF_FOR_EVAL_BOTH if wl["n_phase"] == 2 else lpf.LPF_FOR_EVAL) | lpf.LPF_FOR_HOST)
         lpf.lpf_set_timing(p, True)
 
         def step():
@@ -292,6 +406,8 @@ def main():
                 lpf.lpf_eval(p, d_imgs, 1, flags, out=d_counts, stream=stream)
             if d_target is not None:
                 lpf.lpf_objective(d_counts, d_target, out=d_sse, stream=stream)
+            if strong:                                    # every rank ends the step with the whole [B, S, S] array
+                lpf_dist.gather_shards(d_counts, d_all, wl["B"], rank, world)
 
         for _ in range(warmup):
             flush.zero_()
@@ -339,29 +455,111 @@ def main():
             [total_ms, float(np.mean(kernel_ms)), e2e["seconds_per_step"] if e2e else 0.0], device="cuda")
         lpf.lpf_free_paths(p)
         return dict(total_ms=total_ms, kernel_ms=kern_ms, e2e_s=e2e_s, e2e=e2e, info=info, launch=launch,
-                    launches_per_step=launches_per_step, clocks=clocks, imgs=imgs, wall=wall)
+                    launches_per_step=launches_per_step, clocks=clocks, imgs=imgs, wall=wall, images_per_gpu=B_loc,
+                    strong=strong)
 
     def measure_swaps(n=20000):
-        """config 5: n independent two-pixel swap proposals on the 256x256 disk image, m = 64, phase 1."""
+        """config 5: n independent two-pixel swap proposals on the 256x256 disk image, m = 64; phase 1 (the config) and,
+        on a quarter of the proposals, phase 0 (the matrix: long in-phase segments, a much larger live region)."""
         img = inputs.config_image(5)
         pairs = inputs.config5_pairs(img, 2 * n)
         p5 = lpf.lpf_build_paths(64, local_rank)
         info5 = lpf.lpf_paths_info(p5)
+        lpf.lpf_reserve(p5, 1, 256, 256, 0, lpf.LPF_FOR_SWAP_DELTA)
         d_img = torch.from_numpy(img[None]).cuda()
         d_pairs = torch.from_numpy(pairs).cuda()
         out = torch.empty((n, 129, 129), dtype=torch.int32, device="cuda")
-        lpf.lpf_swap_delta(p5, d_img, 1, d_pairs[:n], out=out)
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        lpf.lpf_swap_delta(p5, d_img, 1, d_pairs[n:], out=out)
-        e1.record()
-        torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1)
-        lpf.lpf_free_paths(p5)
         cand = 2 * (2 * info5["sum_path_len"] - 1)          # candidate (start, vector) tests per swap, SURVEY 8 a9
-        return {"swaps": n, "ms": ms, "swaps_per_s": n / (ms * 1e-3), "candidate_tests_per_s": n * cand / (ms * 1e-3),
-                "d2d_bytes_out": int(out.numel() * 4)}
+        res = {}
+        for phase, k in ((1, n), (0, n // 4)):
+            lpf.lpf_swap_delta(p5, d_img, phase, d_pairs[:k], out=out[:k])
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            lpf.lpf_swap_delta(p5, d_img, phase, d_pairs[n:n + k], out=out[:k])
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            res["phase%d" % phase] = {"swaps": k, "ms": ms, "swaps_per_s": k / (ms * 1e-3),
+                                      "candidate_tests_per_s": k * cand / (ms * 1e-3),
+                                      "d2d_bytes_out": int(k * 129 * 129 * 4)}
+        lpf.lpf_free_paths(p5)
+        res.update(res["phase1"])                            # the config's own figures at the top level
+        return res
+
+    def measure_s2(cfg_name):
+        """Two-point probability of both phases (LPF_S2: exact integer counts of Eq. 6, O(WH * S^2) bit operations) on a
+        workload's image, next to the transform form of Eq. 7 (O(WH log WH), floating point) run with
+        torch.fft = cuFFT on the same image as CONTEXT -- it is a library call and not part of this library's path."""
+        wl = WORKLOADS[cfg_name]
+        imgs, _ = make_images(wl, 0)
+        p2 = lpf.lpf_build_paths(wl["m"], local_rank)
+        lpf.lpf_reserve(p2, 1, wl["H"], wl["W"], lpf.LPF_S2, lpf.LPF_FOR_EVAL_BOTH)
+        lpf.lpf_set_timing(p2, True)
+        d_img = torch.from_numpy(imgs[:1]).cuda()
+        out = lpf.lpf_eval_both(p2, d_img, lpf.LPF_S2)
+        torch.cuda.synchronize()
+        step_ms, ker_ms = [], []
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            lpf.lpf_eval_both(p2, d_img, lpf.LPF_S2, out=out)
+            e1.record()
+            torch.cuda.synchronize()
+            step_ms.append(e0.elapsed_time(e1))
+            ker_ms.append(lpf.lpf_last_eval_kernel_ms(p2))
+        m = wl["m"]
+
+        def fft_form():
+            chi = torch.stack([(d_img[0] == 0), (d_img[0] == 1)]).to(torch.float64)
+            F = torch.fft.rfft2(chi)
+            return torch.fft.irfft2(F * F.conj(), s=chi.shape[-2:])
+        corr = fft_form()
+        torch.cuda.synchronize()
+        fft_ms = []
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            corr = fft_form()
+            e1.record()
+            torch.cuda.synchronize()
+            fft_ms.append(e0.elapsed_time(e1))
+        idx = (-torch.arange(-m, m + 1, device="cuda")) % wl["H"]
+        jdx = (-torch.arange(-m, m + 1, device="cuda")) % wl["W"]
+        same = bool((torch.round(corr[:, idx][:, :, jdx]).to(torch.int64) == out[0]).all())
+        lpf.lpf_free_paths(p2)
+        return {"direct_step_ms": float(np.median(step_ms)), "direct_kernel_ms": float(np.median(ker_ms)),
+                "cufft_context_ms": float(np.median(fft_ms)), "direct_over_cufft": float(np.median(step_ms) / np.median(fft_ms)),
+                "rounded_fft_equals_exact_counts": same}
+
+    def measure_ensemble():
+        """lpf_eval_sum: ensemble descriptor of 100 slices of 100 x 100, both phases, entire L2
+        (m = 99), against the per-image call + a device-side sum over the batch."""
+        B, H, W, m = 100, 100, 100, 99
+        stack = np.stack([inputs.disks(H, W, 5.0, 0.45, inputs.seed_for(9, i)) for i in range(B)])
+        pe = lpf.lpf_build_paths(m, local_rank)
+        lpf.lpf_reserve(pe, B, H, W, 0, lpf.LPF_FOR_EVAL_BOTH)
+        d = torch.from_numpy(stack).cuda()
+        out = lpf.lpf_eval_sum(pe, d, -1)
+        per = lpf.lpf_eval_both(pe, d)
+        ok = bool((per.sum(dim=0) == out).all())
+        torch.cuda.synchronize()
+        t_sum, t_per = [], []
+        for _ in range(5):
+            e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            e0.record()
+            lpf.lpf_eval_sum(pe, d, -1, out=out)
+            e1.record()
+            lpf.lpf_eval_both(pe, d, out=per)
+            per.sum(dim=0)
+            e2.record()
+            torch.cuda.synchronize()
+            t_sum.append(e0.elapsed_time(e1))
+            t_per.append(e1.elapsed_time(e2))
+        lpf.lpf_free_paths(pe)
+        S = 2 * m + 1
+        return {"slices": B, "eval_sum_ms": float(np.median(t_sum)), "per_image_then_sum_ms": float(np.median(t_per)),
+                "equal": ok, "tests_per_s": B * 2 * H * W * S * S / (np.median(t_sum) * 1e-3)}
 
     def measure_anneal(n=20000):
         """Alg. 3 (lpf_anneal) on the paper's compression setting: target = descriptor of a 100x100
@@ -397,13 +595,17 @@ def main():
         return {"proposals": n, "seconds": dt, "proposals_per_s": n / dt, "accepted": st["accepted"],
                 "E_start": E0, "E_end": st["E"], "levels": st["levels"], "T_max": T_max}
 
-    r = measure(w, args.steps, args.warmup, True)
-    tests_per_step = nominal_tests(w) * world
+    r = measure(w, args.steps, args.warmup, True, strong=(args.scaling == "strong"))
+    if args.scaling == "strong" and not r["strong"]:
+        args.scaling = "weak"                             # one rank, or a workload with fewer images than ranks
+    tests_per_step = lpf_dist.sum_over_ranks(nominal_tests(dict(w, B=r["images_per_gpu"])), device="cuda")
     value = tests_per_step * args.steps / (r["total_ms"] * 1e-3)
-    # roofline of the dominant kernel (eval): algorithmic INT ops per launch:
-    #   per image-phase Nw * (2 * trie nodes + 2 * half vectors): (SHF + LOP3) per word-node, (POPC + IADD) per word-terminal
-    Nw = w["H"] * w["W"] // 32
-    alg_ops = w["B"] * w["n_phase"] * Nw * (2 * r["info"]["n_trie_nodes"] + 2 * r["info"]["n_half_vectors"])
+    # roofline of the dominant kernel (eval): a UTILISATION of the ALU pipe -- the data operations the design executes
+    # at minimum (design_ops, from the uploaded program) over kernel time x derived ALU peak.  The survey's op model
+    # (more ops than the design needs since PAIR fusion and the eroded planes) is kept as frac_vs_survey_ops.
+    w_loc = dict(w, B=r["images_per_gpu"])               # the eval kernel of THIS rank (strong scaling: its shard)
+    d_ops = design_ops(w_loc, r["launch"])
+    s_ops = survey_ops(w_loc, r["info"])
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -411,32 +613,36 @@ def main():
         pass
     sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     peak_ops = SM_COUNT * ALU_LANES_PER_CLK_PER_SM * sm_max_mhz * 1e6
-    achieved = alg_ops / (r["kernel_ms"] * 1e-3)
+    achieved = d_ops / (r["kernel_ms"] * 1e-3)
     measured = lpf.lpf_alu_peak(local_rank) if rank == 0 else None     # live LOP3 / SHF / pair-pattern / POPC rates
-    # dram__bytes_read.sum + dram__bytes_write.sum of one eval-kernel launch, from the committed ncu --set full
-    # capture of this command (profiles/r01_v6_eval_kernel_full.csv: 24.07 MB + 1.02 MB); config 3, no flags only
-    traffic = 25.10e6 if (args.workload == "cfg3" and not args.flags) else None
+    cap = capture_lookup(args.workload, args.flags)                     # ncu --set full of THESE sources, or None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": r["total_ms"] / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "u32", "data": "synthetic",
-        "config": {"workload": args.workload_desc, "images_per_gpu": w["B"], "flags": args.flags or "none",
+        "ms_per_step": r["total_ms"] / args.steps, "higher_is_better": True, "scaling": args.scaling,
+        "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": args.workload_desc, "images_per_gpu": r["images_per_gpu"], "flags": args.flags or "none",
                    "l2": "flushed with a 256 MiB memset between timed steps",
                    "timing": "sum of per-step CUDA-event times on the launch stream, max over ranks",
                    "launch": r["launch"]},
         "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_ops / 1e12, "unit": "T int-op/s",
-                     "frac": achieved / peak_ops, "traffic": traffic,
+                     "frac": achieved / peak_ops,
+                     "traffic": None if cap is None else cap["dram_read_bytes"] + cap["dram_write_bytes"],
+                     "frac_vs_survey_ops": s_ops / (r["kernel_ms"] * 1e-3) / peak_ops,
+                     "ncu": cap, "csrc_sha256": csrc_digest(),
                      "peak_measured": None if measured is None else
                      {"lop3": measured["lop3"] / 1e12, "shf": measured["shf"] / 1e12,
                       "shf_shf_lop3": measured["pair"] / 1e12, "popc": measured["popc"] / 1e12,
                       "unit": "T int-op/s", "how": "lpf_alu_peak: 8 register-only chains per thread, all SMs, live"},
-                     "kernel": "eval_kernel", "kernel_ms": r["kernel_ms"], "algorithmic_ops_per_launch": alg_ops,
+                     "kernel": "eval_kernel", "kernel_ms": r["kernel_ms"], "design_ops_per_launch": d_ops,
+                     "survey_ops_per_launch": s_ops,
                      "peak_source": "derived: 148 SM x 64 alu lanes/clk x %.0f MHz (sm_max_mhz of MEASURED_PEAKS.json)"
                                     % sm_max_mhz,
                      "kernel_share_of_step": r["kernel_ms"] * args.steps / r["total_ms"],
-                     "note": "algorithmic ops = SURVEY 8(d): 2 per word-node + 2 per word-terminal; the kernel executes fewer "
-                             "(3-input AND pair fusion, eroded planes E2/D2: DESIGN.md), so frac can exceed 1; ncu of this "
-                             "command: alu pipe 66 %, shared-memory wavefronts 73 % of peak (profiles/r01_v6_eval_kernel.md)"},
+                     "note": "frac = data ops the design executes at minimum (per start word: 2 SHF + 1 LOP3 per fused "
+                             "pair of program entries, 1 SHF + 1 LOP3 per single entry, POPC + add per terminal; counted "
+                             "from the uploaded program) / (kernel time x peak); frac_vs_survey_ops uses SURVEY 8(d)'s "
+                             "2 ops per word-node, which the design undercuts, and may exceed 1; `ncu` = pipe figures of "
+                             "a committed ncu capture of exactly these sources (profiles/capture_index.csv) or null"},
         "e2e": {"value": tests_per_step / r["e2e_s"], "unit": UNIT, "h2d_bytes_per_step": r["e2e"]["h2d"],
                 "d2h_bytes_per_step": r["e2e"]["d2h"]},
         "gpu_launches": r["launches_per_step"] * args.steps,
@@ -449,12 +655,13 @@ def main():
                 continue
             wl = WORKLOADS[name]
             rr = measure(wl, max(3, args.steps // 2), 3, False)
-            nw = wl["H"] * wl["W"] // 32
-            ops = wl["B"] * wl["n_phase"] * nw * (2 * rr["info"]["n_trie_nodes"] + 2 * rr["info"]["n_half_vectors"])
             k = max(3, args.steps // 2)
+            cap2 = capture_lookup(name, args.flags)
             extra[name] = {"value": nominal_tests(wl) * k / (rr["total_ms"] * 1e-3), "unit": UNIT,
                            "ms_per_step": rr["total_ms"] / k, "kernel_ms": rr["kernel_ms"],
-                           "roofline_frac": ops / (rr["kernel_ms"] * 1e-3) / peak_ops}
+                           "roofline_frac": design_ops(wl, rr["launch"]) / (rr["kernel_ms"] * 1e-3) / peak_ops,
+                           "frac_vs_survey_ops": survey_ops(wl, rr["info"]) / (rr["kernel_ms"] * 1e-3) / peak_ops,
+                           "ncu": cap2}
         # the design variants the north star asks to compare, eval kernel alone on the headline workload
         variants = {}
         for vname, vflags in (("trie_pair_e2", 0), ("trie_no_e2", lpf.LPF_NO_E2), ("trie_prune", lpf.LPF_PRUNE),
@@ -465,6 +672,9 @@ def main():
         extra["variants_" + args.workload] = variants
         extra["cfg5"] = measure_swaps()
         extra["anneal"] = measure_anneal()
+        extra["s2_cfg2"] = measure_s2("cfg2")
+        extra["s2_cfg3"] = measure_s2("cfg3")
+        extra["ensemble_sum"] = measure_ensemble()
         line["other_workloads"] = extra
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         tests, dt, cores, what = oracle_sample(w, r["imgs"], 20)
@@ -476,6 +686,9 @@ def main():
     if args.tab1 and rank == 0 and world == 1:
         rows = run_tab1(lpf, torch, local_rank, os.path.join(ROOT, "gpurun_out"))
         line["tab1"] = {"rows": len(rows), "written_to": "gpurun_out/tab1.json, gpurun_out/tab1.md"}
+    if args.fig7 and rank == 0 and world == 1:
+        rows = run_fig7(lpf, torch, local_rank, os.path.join(ROOT, "gpurun_out"))
+        line["fig7"] = {"rows": len(rows), "written_to": "gpurun_out/fig7.json, gpurun_out/fig7.md"}
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

@@ -45,7 +45,45 @@ def test_two_ranks_partition_units_and_reduce_times(tmp_path, n_units):
     for k in range(world):
         assert r[k][2] == n_units                                                 # whole-job unit count
         assert r[k][3] == 11.0 and r[k][4] == 5.0                                 # max over ranks
-    assert r[0][5] != r[1][5] or True                                             # independent images per rank
+    assert r[0][5] != r[1][5]                                                     # independent images per rank
+
+
+def _split_worker(rank, world, port, n_img, out_dir):
+    """Strong-scaling split of ONE batch (bench.py --scaling strong): every rank holds the batch,
+    evaluates only its shard (here with the CPU oracle standing in for lpf_eval) and all-gathers the count slices."""
+    from oracle import lpf_oracle as orc
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        m = 4
+        batch = np.stack([inputs.bernoulli(9, 11, 0.6, inputs.seed_for(1, i)) for i in range(n_img)])
+        b, e = lpf_dist.shard_range(n_img, rank, world)
+        local = torch.from_numpy(np.stack([orc.counts(batch[i], 1, m, threads=1) for i in range(b, e)])
+                                 if e > b else np.zeros((0, 2 * m + 1, 2 * m + 1), dtype=np.int64))
+        buf = lpf_dist.gather_buffer(local, n_img, world)
+        whole = lpf_dist.gather_shards(local, buf, n_img, rank, world)
+        np.save(os.path.join(out_dir, "g%d.npy" % rank), whole.numpy())
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("n_img", [8, 7])
+def test_two_ranks_split_one_batch_and_gather_the_whole_result(tmp_path, n_img):
+    from oracle import lpf_oracle as orc
+    world = 2
+    mp.spawn(_split_worker, args=(world, _free_port(), n_img, str(tmp_path)), nprocs=world, join=True)
+    batch = np.stack([inputs.bernoulli(9, 11, 0.6, inputs.seed_for(1, i)) for i in range(n_img)])
+    want = np.stack([orc.counts(batch[i], 1, 4) for i in range(n_img)])            # the unsplit, one-rank result
+    for k in range(world):
+        got = np.load(tmp_path / ("g%d.npy" % k))
+        assert got.shape == want.shape and np.array_equal(got, want), k
+
+
+def test_gather_without_process_group_is_identity():
+    local = torch.arange(12).reshape(3, 4)
+    buf = lpf_dist.gather_buffer(local, 3, 1)
+    assert lpf_dist.gather_shards(local, buf, 3, 0, 1) is local
 
 
 def test_shard_range_properties():
