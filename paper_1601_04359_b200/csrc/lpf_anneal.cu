@@ -1,18 +1,27 @@
 // lpf_anneal.cu -- simulated annealing of Alg. 3 on the device.
 // The chain itself is sequential (one proposal, one Metropolis decision at a time); what is parallel is the
-// EVALUATION: a batch of K consecutive proposals is evaluated speculatively against the current image with
-// lpf_swap_delta, the decisions are then taken in order by one thread, the first accepted proposal is applied and the
-// proposals after it are thrown away and re-evaluated in the next batch -- so the result is exactly the sequential
-// chain, whatever K is.  The host never sees a decision: it only reads the progress counter every few batches.
+// EVALUATION: a batch of K consecutive proposals is evaluated speculatively against the current image by the swap-delta
+// kernel (which reads them straight from the caller's proposal list at the device-resident progress counter), the
+// decisions are then taken in order by one thread, the first accepted proposal is applied and the proposals after it
+// are thrown away and re-evaluated in the next batch -- so the result is exactly the sequential chain, whatever K is.
+// The whole chain runs in ONE cooperative launch (anneal_chain_kernel): the host never sees a decision, it reads the
+// final state when the chain is finished.
 // Readings A1-A5 of the garbled listing are those of DESIGN.md "Annealing readings" (the oracle states them too).
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
 #include <cmath>
 
 #include "lpf_internal.h"
+#include "lpf_swap.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace lpf {
+
+cudaError_t launch_swap_bits(const uint8_t* image, uint32_t* bits, int H, int W, int m, int phase,
+                             unsigned int* counter, int n_sm, cudaStream_t st, uint32_t** padded_out);
 
 struct AnnealState {
   long long next;        // proposals consumed so far (reading A1: the one counter that runs to N)
@@ -21,7 +30,9 @@ struct AnnealState {
   long long E;           // Eq. 19 over D and the requested phases on integer counts (reading A4), exact
   double T;
   int acc_idx;           // index inside the current batch of the accepted proposal, or -1
-  int pad;
+  int ticket;            // blocks of anneal_decide_kernel that have delivered their dE
+  int acc_pair[4];       // the accepted proposal's pixels (x_p, y_p, x_q, y_q) if it exchanged two bytes, else -1
+  int acc_bytes[2];      // ... and the bytes that are at p and at q after the exchange
 };
 
 // E of the start image: sum over the canonical half of (t - c)^2, all phases.  One block.
@@ -44,99 +55,218 @@ __global__ void anneal_e0_kernel(const long long* __restrict__ counts, const lon
   if (threadIdx.x == 0) st->E = red[0];
 }
 
-// the next K proposals, or (-1,-1,-1,-1) past the end (lpf_swap_delta gives those an all-zero delta)
-__global__ void anneal_gather_kernel(const int* __restrict__ pairs, long long N, const AnnealState* st,
-                                     int* __restrict__ batch, int K) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= K) return;
-  const long long idx = st->next + j;
-#pragma unroll
-  for (int t = 0; t < 4; ++t) batch[4 * j + t] = idx < N ? pairs[4 * idx + t] : -1;
-}
+struct AnnealArgs {
+  AnnealState* state;
+  const uint32_t* padded;      // [n_ph] padded bit planes of the START image (lpf_swap.cuh layout)
+  int H, W, m, phase, n_ph;
+  const int* pairs;            // [N][4]
+  const double* log_u;         // [N]
+  long long N;
+  const int4* rec;             // swap-delta node records
+  int n_nodes;
+  int* delta;                  // [n_ph][K_max][S][S], zero on entry and again on exit
+  long long ph_stride;
+  int K_max;
+  long long* dE;               // [K_max], zero on entry
+  long long* counts;           // [n_ph][S][S]: descriptor of P
+  const long long* target;
+  uint8_t* image;
+  uint8_t* accept_log;
+  double wh2, T_mult;
+  long long c_max, s_max;
+};
 
-// dE[j] = E(Q_j) - E(P) = sum_phases sum_{v in D} [ (t - c - delta)^2 - (t - c)^2 ], exact.  One block per proposal.
-__global__ void anneal_de_kernel(const int* __restrict__ delta, long long ph_stride,
-                                 const long long* __restrict__ counts, const long long* __restrict__ target, int S,
-                                 int n_ph, long long* __restrict__ dE) {
-  const long long K = (long long)S * S, c0 = K / 2;
-  const int j = blockIdx.x;
-  long long s = 0;
-  for (int ph = 0; ph < n_ph; ++ph) {
-    const int* dl = delta + ph * ph_stride + (long long)j * K;
-    for (long long k = c0 + threadIdx.x; k < K; k += blockDim.x) {
-      const long long dv = dl[k];
-      if (dv != 0) {
-        const long long d = target[ph * K + k] - counts[ph * K + k];
-        s += dv * dv - 2 * d * dv;
+__device__ __forceinline__ long long ld_cg(const long long* p) { return __ldcg(p); }
+
+// The whole chain in ONE cooperative launch (one CTA set resident on every SM, grid-wide barriers between the phases of
+// a batch): the padded bit planes of the current image stay in every CTA's shared memory and are patched after an
+// acceptance; nothing goes back to the host until the chain is finished.  Per batch of K proposals:
+//   (A) Q = modify(P), SDQ = evaluate(Q) for proposals next .. next + K - 1, speculatively against P: swap_delta_unit
+//       on (proposal, node slice) units spread over the grid  (Alg. 3 lines 9-10)
+//   (B) dE[j] = E(Q_j) - E(P) = sum_phases sum_{v in D} [ (t - c - delta)^2 - (t - c)^2 ], exact, by (proposal, chunk)
+//       units; the CTA that finishes LAST takes the decisions in order -- lines 7-17 -- up to and including the first
+//       accepted proposal, whose two bytes it exchanges (P = Q)
+//   (C) SDP = SDQ: the accepted proposal's delta is added to the descriptor (both halves), every delta is zeroed
+//       again, every CTA patches its bit planes.
+// The proposals after an accepted one saw a stale image: they are not consumed and come back in the next batch, so
+// the chain is exactly the sequential one for any K; K follows the acceptance rate (about three expected acceptances
+// per batch).  Memory that other CTAs write during the launch (state, delta, dE, counts) is read with ld.global.cg.
+__global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
+  cg::grid_group grid = cg::this_grid();
+  extern __shared__ __align__(16) uint32_t sm[];
+  __shared__ SwapShared sh;
+  __shared__ long long s_red[8];
+  __shared__ long long s_dE[256];
+  __shared__ double s_lu[256];
+  __shared__ int s_last;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int H = a.H, W = a.W, m = a.m, n_ph = a.n_ph;
+  const int PWc = (W + 2 * m + 31) >> 5, PH = H + 2 * m;
+  const int plane_words = PH * PWc;
+  uint2* stk = (uint2*)(sm + ((n_ph * plane_words + 1) & ~1));
+  for (int i = tid; i < n_ph * plane_words; i += blockDim.x) sm[i] = a.padded[i];
+  const int S = 2 * m + 1;
+  const long long K2 = (long long)S * S, c0 = K2 / 2, half = K2 - c0;
+  const long long per_prop = n_ph * half;                       // elements of D over the phases
+  const int n_chunks = (int)((per_prop + 1023) / 1024);
+  int K = min(16, a.K_max);
+  long long win_next = 0, win_acc = 0;
+  for (int batch = 0;; ++batch) {
+    const long long next = ld_cg(&a.state->next);
+    if (next >= a.N) break;
+    // ---- (A)
+    const int n_slices = max(1, min((int)gridDim.x / K, (a.n_nodes + 255) / 256));
+    for (int unit = blockIdx.x; unit < K * n_slices; unit += gridDim.x) {
+      const int j = unit / n_slices, slice = unit - j * n_slices;
+      swap_delta_unit(sm, stk, sh, H, W, m, a.pairs, a.N, next + j, a.rec, a.n_nodes, a.delta + (long long)j * K2, n_ph,
+                      a.ph_stride, 1, slice, n_slices);
+    }
+    grid.sync();
+    // ---- (B)
+    for (int unit = blockIdx.x; unit < K * n_chunks; unit += gridDim.x) {
+      const int j = unit / n_chunks, chunk = unit - j * n_chunks;
+      long long s = 0;
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const long long i = (long long)chunk * 1024 + r * 256 + tid;
+        if (i < per_prop) {
+          const long long ph = i / half, k = c0 + (i - ph * half);
+          const long long dv = __ldcg(a.delta + ph * a.ph_stride + (long long)j * K2 + k);
+          if (dv != 0) {
+            const long long d = a.target[ph * K2 + k] - ld_cg(a.counts + ph * K2 + k);
+            s += dv * dv - 2 * d * dv;
+          }
+        }
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+      __syncthreads();
+      if (lane == 0) s_red[warp] = s;
+      __syncthreads();
+      if (tid == 0) {
+        long long t = 0;
+        for (int w8 = 0; w8 < 8; ++w8) t += s_red[w8];
+        if (t != 0) atomicAdd((unsigned long long*)(a.dE + j), (unsigned long long)t);
       }
     }
-  }
-  __shared__ long long red[256];
-  red[threadIdx.x] = s;
-  __syncthreads();
-  for (int o = 128; o > 0; o >>= 1) {
-    if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+    if (tid == 0) {
+      __threadfence();
+      s_last = (atomicAdd(&a.state->ticket, 1) == (int)gridDim.x - 1);
+    }
     __syncthreads();
-  }
-  if (threadIdx.x == 0) dE[j] = red[0];
-}
-
-// Alg. 3 lines 7-17 for the proposals of this batch, in order, up to and including the first accepted one.
-__global__ void anneal_decide_kernel(AnnealState* state, const long long* __restrict__ dE,
-                                     const double* __restrict__ log_u, long long N, int K, double wh2, double T_mult,
-                                     long long c_max, long long s_max, const int* __restrict__ batch,
-                                     uint8_t* image, int H, int W, uint8_t* accept_log) {
-  if (threadIdx.x != 0 || blockIdx.x != 0) return;
-  AnnealState st = *state;
-  int acc_idx = -1;
-  long long consumed = 0;
-  for (int j = 0; j < K; ++j) {
-    const long long idx = st.next + j;
-    if (idx >= N) break;
-    ++consumed;
-    st.c += 1;                                                  // line 8
-    const double num = (double)(-dE[j]);                        // E_P - E_Q, exact
-    const double den = wh2 * st.T;
-    const bool acc = log_u[idx] < num / den;                    // line 11, reading A3
-    if (accept_log) accept_log[idx] = acc ? 1 : 0;
-    if (acc) {                                                  // lines 12-13
-      st.s += 1;
-      st.accepted += 1;
-      st.E += dE[j];
-      acc_idx = j;
+    if (s_last) {                                                // every dE[j] of this batch is complete
+      __threadfence();
+      if (tid < K) {
+        s_dE[tid] = ld_cg(a.dE + tid);
+        a.dE[tid] = 0;
+        s_lu[tid] = (next + tid < a.N) ? a.log_u[next + tid] : 0.0;
+      }
+      __syncthreads();
+      if (tid == 0) {
+        AnnealState st;
+        st.next = next;
+        st.c = ld_cg(&a.state->c); st.s = ld_cg(&a.state->s);
+        st.accepted = ld_cg(&a.state->accepted); st.levels = ld_cg(&a.state->levels);
+        st.E = ld_cg(&a.state->E);
+        st.T = __longlong_as_double(ld_cg((const long long*)&a.state->T));
+        int acc_idx = -1;
+        long long consumed = 0;
+        for (int jj = 0; jj < K; ++jj) {
+          const long long idx = next + jj;
+          if (idx >= a.N) break;
+          ++consumed;
+          st.c += 1;                                            // line 8
+          const long long de = s_dE[jj];
+          const double num = (double)(-de);                     // E_P - E_Q, exact
+          const double den = a.wh2 * st.T;
+          const bool acc = s_lu[jj] < num / den;                // line 11, reading A3
+          if (a.accept_log) a.accept_log[idx] = acc ? 1 : 0;
+          if (acc) {                                            // lines 12-13
+            st.s += 1;
+            st.accepted += 1;
+            st.E += de;
+            acc_idx = jj;
+          }
+          if (st.c >= a.c_max || st.s >= a.s_max) {             // the temperature level is complete: line 17
+            st.T = st.T * a.T_mult;
+            st.levels += 1;
+            st.c = 0;
+            st.s = 0;
+          }
+          if (acc) break;                                       // the later proposals saw a stale image
+        }
+        st.acc_idx = acc_idx;
+        st.acc_pair[0] = st.acc_pair[1] = st.acc_pair[2] = st.acc_pair[3] = -1;
+        st.acc_bytes[0] = st.acc_bytes[1] = 0;
+        if (acc_idx >= 0) {                                     // P = Q: exchange the two bytes (reading A5)
+          const long long idx = next + acc_idx;
+          const int xp = a.pairs[4 * idx], yp = a.pairs[4 * idx + 1], xq = a.pairs[4 * idx + 2],
+                    yq = a.pairs[4 * idx + 3];
+          if (xp >= 0 && xp < W && xq >= 0 && xq < W && yp >= 0 && yp < H && yq >= 0 && yq < H) {
+            volatile uint8_t* img = a.image;
+            const uint8_t bp = img[(size_t)yp * W + xp], bq = img[(size_t)yq * W + xq];
+            img[(size_t)yp * W + xp] = bq;
+            img[(size_t)yq * W + xq] = bp;
+            st.acc_pair[0] = xp; st.acc_pair[1] = yp; st.acc_pair[2] = xq; st.acc_pair[3] = yq;
+            st.acc_bytes[0] = bq; st.acc_bytes[1] = bp;         // the bytes now at p and at q
+          }
+        }
+        st.next = next + consumed;
+        st.ticket = 0;
+        *a.state = st;
+      }
     }
-    if (st.c >= c_max || st.s >= s_max) {                       // the temperature level is complete: line 17
-      st.T = st.T * T_mult;
-      st.levels += 1;
-      st.c = 0;
-      st.s = 0;
+    grid.sync();
+    // ---- (C)
+    const int acc_idx = __ldcg(&a.state->acc_idx);
+    for (int unit = blockIdx.x; unit < K * n_chunks; unit += gridDim.x) {
+      const int j = unit / n_chunks, chunk = unit - j * n_chunks;
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const long long i = (long long)chunk * 1024 + r * 256 + tid;
+        if (i < per_prop) {
+          const long long ph = i / half, k = c0 + (i - ph * half);
+          int* dp = a.delta + ph * a.ph_stride + (long long)j * K2 + k;
+          const int dv = __ldcg(dp);
+          if (dv != 0) {
+            if (j == acc_idx) {
+              const long long nv = ld_cg(a.counts + ph * K2 + k) + dv;
+              a.counts[ph * K2 + k] = nv;
+              a.counts[ph * K2 + (K2 - 1 - k)] = nv;                     // count(-v) = count(v); v = 0 never changes
+            }
+            *dp = 0;
+          }
+        }
+      }
     }
-    if (acc) break;                                             // the later proposals saw a stale image
-  }
-  st.next += consumed;
-  st.acc_idx = acc_idx;
-  *state = st;
-  if (acc_idx >= 0) {                                           // P = Q: exchange the two bytes (reading A5)
-    const int xp = batch[4 * acc_idx], yp = batch[4 * acc_idx + 1], xq = batch[4 * acc_idx + 2],
-              yq = batch[4 * acc_idx + 3];
-    if (xp >= 0 && xp < W && xq >= 0 && xq < W && yp >= 0 && yp < H && yq >= 0 && yq < H) {
-      const uint8_t bp = image[(size_t)yp * W + xp], bq = image[(size_t)yq * W + xq];
-      image[(size_t)yp * W + xp] = bq;
-      image[(size_t)yq * W + xq] = bp;
+    if (acc_idx >= 0 && tid < 18 * n_ph) {                       // the two exchanged pixels, every periodic replica
+      const int ph = tid / 18, r = tid % 18, which = r / 9, rep = r % 9;
+      const int x = __ldcg(&a.state->acc_pair[2 * which]), y = __ldcg(&a.state->acc_pair[2 * which + 1]);
+      if (x >= 0) {
+        const int X = x + m + (rep / 3 - 1) * W, Y = y + m + (rep % 3 - 1) * H;
+        if (X >= 0 && X < W + 2 * m && Y >= 0 && Y < PH) {
+          const int want = (a.phase < 0) ? ph : a.phase;
+          uint32_t* wp = sm + (size_t)ph * plane_words + (size_t)Y * PWc + (X >> 5);
+          const uint32_t bit = 1u << (X & 31);
+          if (__ldcg(&a.state->acc_bytes[which]) == want) atomicOr(wp, bit); else atomicAnd(wp, ~bit);
+        }
+      }
     }
-  }
-}
-
-// SDP = SDQ: counts += delta of the accepted proposal (the delta arrays are full templates, mirrored)
-__global__ void anneal_apply_kernel(const AnnealState* state, const int* __restrict__ delta, long long ph_stride,
-                                    long long* __restrict__ counts, int S, int n_ph) {
-  const int j = state->acc_idx;
-  if (j < 0) return;
-  const long long K = (long long)S * S;
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < (long long)n_ph * K;
-       i += (long long)gridDim.x * blockDim.x) {
-    const long long ph = i / K, k = i - ph * K;
-    counts[i] += delta[ph * ph_stride + (long long)j * K + k];
+    // batch size for the next rounds: about three expected acceptances per batch, revised every 16 batches
+    if ((batch & 15) == 15) {
+      const long long nx = ld_cg(&a.state->next), ac = ld_cg(&a.state->accepted);
+      const long long dn = nx - win_next, da = ac - win_acc;
+      win_next = nx;
+      win_acc = ac;
+      if (dn > 0) {
+        const double rate = (double)max(1ll, da) / (double)dn;
+        const int want = (int)fmin(256.0, fmax(8.0, 3.0 / rate));
+        K = 8;
+        while (K < want) K *= 2;
+        K = min(K, a.K_max);
+      }
+    }
+    grid.sync();
   }
 }
 
@@ -170,7 +300,6 @@ extern "C" int lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase,
     if (rc != LPF_OK) { if (prev != p->device) cudaSetDevice(prev); return rc; }
   }
   AnnealState* d_state = (AnnealState*)p->d_an_state;
-  int* d_batch = p->d_an_batch;
   int* d_delta = p->d_an_delta;
   long long* d_dE = (long long*)p->d_an_dE;
   cudaError_t e = cudaSuccess;
@@ -179,42 +308,42 @@ extern "C" int lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase,
   h.acc_idx = -1;
   const double T_mult = N > 0 ? std::pow(T_min / T_max, (double)s_max / (double)N) : 1.0;   // line 4, reading A2
   const double wh2 = (double)W * (double)H * (double)W * (double)H;
+  const long long ph_stride = (long long)K_max * K2;
+  // the chain's workspace: state, zeroed delta arrays, the padded bit planes of the start image (kept up to date by
+  // anneal_apply_kernel from then on), E of the start image
+  uint32_t* padded = nullptr;
   if (e == cudaSuccess) e = cudaMemcpyAsync(d_state, &h, sizeof(h), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_delta, 0, sizeof(int) * (size_t)n_ph * K_max * K2, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_dE, 0, sizeof(long long) * 256, st);
+  if (e == cudaSuccess)
+    e = launch_swap_bits(image, p->d_swap_bits, H, W, p->m, phase, p->d_counter + 1, p->n_sm, st, &padded);
   if (e == cudaSuccess) {
     anneal_e0_kernel<<<1, 256, 0, st>>>((const long long*)counts, (const long long*)target, S, n_ph, d_state);
     e = cudaGetLastError();
   }
-  const long long ph_stride = (long long)K_max * K2;
-  int K = 16;
-  long long last_next = 0, last_acc = 0;
   rc = LPF_OK;
-  while (e == cudaSuccess && rc == LPF_OK && h.next < N) {
-    K = std::min(K, K_max);
-    for (int rep = 0; rep < 8 && rc == LPF_OK && e == cudaSuccess; ++rep) {
-      anneal_gather_kernel<<<(K + 63) / 64, 64, 0, st>>>(pairs, N, d_state, d_batch, K);
-      // Q = modify(P), SDQ = evaluate(Q): lines 9-10 (both phases in one pass over the trie if asked)
-      rc = swap_delta_impl(p, image, H, W, phase, d_batch, K, d_delta, ph_stride, stream);
-      if (rc != LPF_OK) break;
-      anneal_de_kernel<<<K, 256, 0, st>>>(d_delta, ph_stride, (const long long*)counts, (const long long*)target, S,
-                                          n_ph, d_dE);
-      anneal_decide_kernel<<<1, 32, 0, st>>>(d_state, d_dE, log_u, N, K, wh2, T_mult, c_max, s_max, d_batch, image,
-                                             H, W, accept_log);
-      anneal_apply_kernel<<<std::max(1, std::min(p->n_sm * 4, (int)((n_ph * K2 + 255) / 256))), 256, 0, st>>>(
-          d_state, d_delta, ph_stride, (long long*)counts, S, n_ph);
-      e = cudaGetLastError();
-    }
-    if (e != cudaSuccess || rc != LPF_OK) break;
-    e = cudaMemcpyAsync(&h, d_state, sizeof(h), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    // batch size for the next rounds: about three expected acceptances per batch
-    const long long dn = h.next - last_next, da = h.accepted - last_acc;
-    last_next = h.next;
-    last_acc = h.accepted;
-    if (dn > 0) {
-      const double rate = std::max(1.0, (double)da) / (double)dn;
-      int want = (int)std::min(256.0, std::max(8.0, 3.0 / rate));
-      K = 8;
-      while (K < want) K *= 2;
+  if (e == cudaSuccess && N > 0) {
+    // the whole chain: one cooperative launch, as many CTAs as are resident at once
+    const size_t smem = (size_t)((n_ph * (H + 2 * p->m) * ((W + 2 * p->m + 31) / 32) + 1) & ~1) * 4 +
+                        (size_t)8 * SWAP_STACK * 8;
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, anneal_chain_kernel);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(anneal_chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               p->max_smem - (int)fa.sharedSizeBytes);
+    int occ = 0;
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, anneal_chain_kernel, 256, smem);
+    if (e == cudaSuccess && occ < 1) rc = LPF_E_UNSUPPORTED;
+    if (e == cudaSuccess && rc == LPF_OK) {
+      AnnealArgs a;
+      a.state = d_state; a.padded = padded; a.H = H; a.W = W; a.m = p->m; a.phase = phase; a.n_ph = n_ph;
+      a.pairs = pairs; a.log_u = log_u; a.N = N; a.rec = (const int4*)p->d_swap_rec; a.n_nodes = (int)p->n_trie_nodes;
+      a.delta = d_delta; a.ph_stride = ph_stride; a.K_max = K_max; a.dE = d_dE; a.counts = (long long*)counts;
+      a.target = (const long long*)target; a.image = image; a.accept_log = accept_log; a.wh2 = wh2; a.T_mult = T_mult;
+      a.c_max = c_max; a.s_max = s_max;
+      void* args[] = {&a};
+      e = cudaLaunchCooperativeKernel((const void*)anneal_chain_kernel, dim3((unsigned)(occ * p->n_sm)), dim3(256),
+                                      args, smem, st);
     }
   }
   if (e == cudaSuccess && rc == LPF_OK) {

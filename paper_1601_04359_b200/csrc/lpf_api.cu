@@ -158,7 +158,6 @@ extern "C" void lpf_free_paths(lpf_paths* p) {
     if (p->d_swap_rec) cudaFree(p->d_swap_rec);
     if (p->d_swap_bits) cudaFree(p->d_swap_bits);
     if (p->d_an_state) cudaFree(p->d_an_state);
-    if (p->d_an_batch) cudaFree(p->d_an_batch);
     if (p->d_an_delta) cudaFree(p->d_an_delta);
     if (p->d_an_dE) cudaFree(p->d_an_dE);
     if (p->d_io_in) cudaFree(p->d_io_in);
@@ -382,7 +381,6 @@ int reserve_anneal(lpf_paths* p, int H, int W) {
   const int K_max = std::max(anneal_kmax(p->m, 1), 2 * anneal_kmax(p->m, 2));   // arrays of either phase count
   if (!p->d_an_state) {
     LPF_CUDA(cudaMalloc(&p->d_an_state, 256));
-    LPF_CUDA(cudaMalloc(&p->d_an_batch, sizeof(int32_t) * 4 * 256));
     LPF_CUDA(cudaMalloc(&p->d_an_dE, sizeof(int64_t) * 256));
   }
   p->an_kmax = K_max;

@@ -143,9 +143,8 @@ struct lpf_paths {
   int32_t* d_swap_rec = nullptr;     // [n_trie_nodes][4]
   uint32_t* d_swap_bits = nullptr;   // packed base image of the last lpf_swap_delta call
   size_t swap_bits_bytes = 0;
-  // lpf_anneal: chain state, proposal batch, speculative deltas and their error changes
+  // lpf_anneal: chain state, speculative deltas and their error changes
   void* d_an_state = nullptr;
-  int32_t* d_an_batch = nullptr;
   int32_t* d_an_delta = nullptr;
   int64_t* d_an_dE = nullptr;
   size_t an_delta_bytes = 0;

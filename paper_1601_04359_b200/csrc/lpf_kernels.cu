@@ -13,6 +13,7 @@
 
 #include "lpf_internal.h"
 #include "lpf_kernels.cuh"
+#include "lpf_swap.cuh"
 
 namespace lpf {
 
@@ -474,20 +475,7 @@ __global__ void objective_kernel(const long long* __restrict__ counts, const lon
 }
 
 // ---------------------------------------------------------------------------------------------
-// swap delta, version 3.
-//   For one proposal let u be the pixel whose bit becomes 1 and w the one whose bit becomes 0:
-//     delta(v) = #{segments of vector v that contain u and lie in phase in I'}
-//              - #{segments of vector v that contain w and lie in phase in I }
-//   A segment of v that has pixel px at path position k starts at s = px - P_v[k]; P_v[0..k] is a trie node N, so
-//   the candidates are exactly the pairs (trie node N, terminal D in the subtree of N) with start s_N = px - o_N.
-//   (A) lane per node N: the prefix root -> N must be in phase from s_N.  The parent's pixel is one of the 8
-//       neighbours of px (register mask lookup: most nodes stop there); the other ancestors' pixels are stepped
-//       backwards with Bresenham error arithmetic on a vector that runs through N -- no loads but the image bits.
-//   (B) the subtree of every surviving (N, start) is explored by the whole warp from a per-warp stack in shared
-//       memory: a lane pops one node, tests its pixel, counts it if it is a terminal, and pushes its next sibling
-//       (always) and its first child (if the pixel is in phase).  A dead prefix kills every vector below it at once.
-//   CTA = SW proposals (node records are fetched once for all of them); image bits in shared memory.
-//   delta must be zero on entry; only the canonical half is written (swap_mirror_kernel fills the rest).
+// swap delta, version 3: the device code is in lpf_swap.cuh.
 // ---------------------------------------------------------------------------------------------
 // the base bit image with a periodic halo of m pixels on every side: bit (X, Y) of the padded image, X in
 // [0, W + 2m), Y in [0, H + 2m), is pixel ((X - m) mod W, (Y - m) mod H).  One thread per output word.  With it a
@@ -515,228 +503,23 @@ __global__ void pack_padded_kernel(const uint32_t* __restrict__ brow, uint32_t* 
   }
 }
 
-constexpr int SWAP_SW = 8;          // proposals per CTA
-constexpr int SWAP_STACK = 512;     // items per warp stack (8 bytes each)
-
-__device__ __forceinline__ int wrap_coord(int x, int n) {
-  x += (x < 0) ? n : 0;
-  x -= (x >= n) ? n : 0;
-  return x;
-}
-
-struct SwapPass {                   // one (proposal, pixel) pass, in shared memory
-  int px, py;                       // the swapped pixel the segments must contain
-  int ox, oy;                       // pixel that reads as out of phase in this pass (w in I'), or -1
-  unsigned nb;                      // in-phase bits of the 8 neighbours px - step, by step code
-  int sign;                         // +1: u on I', -1: w on I
-  int pbase;                        // word offset of this pass's phase plane in the shared-memory bit images
-  long long out_off;                // offset of this pass's [S][S] delta array from the CTA's first one
-};
-
+// CTA = sw proposals (1 .. SWAP_SW: 8 when there are many proposals -- the node records are fetched once for all of
+// them -- fewer for a small batch, so that its passes run in parallel CTAs instead of one after the other) x one node
+// slice (gridDim.y slices, so that a small batch still fills the chip); image bits in shared memory.
+// delta must be zero on entry; only the canonical half is written (swap_mirror_kernel fills the rest).
 __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __restrict__ bits, int H, int W, int m,
                                                              const int* __restrict__ pairs, long long n,
                                                              const int4* __restrict__ rec, int n_nodes,
                                                              int* __restrict__ delta, int n_planes,
-                                                             long long plane_stride) {
+                                                             long long plane_stride, int sw) {
   extern __shared__ __align__(16) uint32_t sm[];
-  __shared__ SwapPass s_pass[4 * SWAP_SW];                            // (proposal, phase plane, pixel)
-  __shared__ int s_n;
-  const int PWc = (W + 2 * m + 31) >> 5, PH = H + 2 * m;                // padded bit image: halo of m pixels all round
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  uint32_t* P = sm;                                                   // [n_planes][PH][PWc] bits of the base image I
-  const int plane_words = PH * PWc;
-  uint2* stk = (uint2*)(sm + ((n_planes * plane_words + 1) & ~1)) + (size_t)warp * SWAP_STACK;
-  // pixel (x, y) of the plane at Pq, x in [-m, W + m), y in [-m, H + m)
-  auto pbit = [&](const uint32_t* Pq, int x, int y) -> unsigned {
-    const int X = x + m;
-    return (Pq[(y + m) * PWc + (X >> 5)] >> (X & 31)) & 1u;
-  };
-  const int S = 2 * m + 1;
-  const long long K = (long long)S * S;
-  for (int i = tid; i < n_planes * plane_words; i += blockDim.x) P[i] = bits[i];
-  __syncthreads();
-  if (tid == 0) {
-    int cnt = 0;
-    for (int j = 0; j < SWAP_SW; ++j) {
-      const long long sw = (long long)blockIdx.x * SWAP_SW + j;
-      if (sw >= n) break;
-      const int xp = pairs[4 * sw], yp = pairs[4 * sw + 1], xq = pairs[4 * sw + 2], yq = pairs[4 * sw + 3];
-      const bool ok = xp >= 0 && xp < W && xq >= 0 && xq < W && yp >= 0 && yp < H && yq >= 0 && yq < H;
-      if (!ok) continue;
-      for (int pl = 0; pl < n_planes; ++pl) {
-        const uint32_t* Pq = P + pl * plane_words;
-        const int bp = (int)pbit(Pq, xp, yp), bq = (int)pbit(Pq, xq, yq);
-        if (bp == bq) continue;                            // nothing changes for this phase
-        const int ux = bp ? xq : xp, uy = bp ? yq : yp;    // bit 0 -> 1
-        const int wx = bp ? xp : xq, wy = bp ? yp : yq;    // bit 1 -> 0
-        for (int pass = 0; pass < 2; ++pass) {
-          SwapPass sp;
-          sp.px = pass ? wx : ux; sp.py = pass ? wy : uy;
-          sp.ox = pass ? -1 : wx; sp.oy = pass ? -1 : wy;
-          sp.nb = 0;
-          for (int code = 0; code < 9; ++code) {
-            const int x = wrap_coord(sp.px - (code / 3 - 1), W), y = wrap_coord(sp.py - (code % 3 - 1), H);
-            unsigned bit = pbit(Pq, x, y);
-            if (x == sp.ox && y == sp.oy) bit = 0;
-            sp.nb |= bit << code;
-          }
-          sp.sign = pass ? -1 : 1;
-          sp.pbase = pl * plane_words;
-          sp.out_off = (long long)pl * plane_stride + (long long)j * K;
-          s_pass[cnt++] = sp;
-        }
-      }
-    }
-    s_n = cnt;
-  }
-  __syncthreads();
-  const int np = s_n;
-  if (np == 0) return;
-  int* const out0 = delta + (long long)blockIdx.x * SWAP_SW * K;
-  const unsigned lt = (1u << lane) - 1u;
-  int top = 0;                                             // warp-uniform: items on this warp's stack
-
-  // blockIdx.y slices the node range, so that a small batch of proposals still fills the chip
-  const int slice = (n_nodes + gridDim.y - 1) / gridDim.y;
-  const int n_begin = blockIdx.y * slice, n_end = min(n_nodes, n_begin + slice);
-  for (int N0 = n_begin + warp * 32; N0 < n_end; N0 += blockDim.x) {
-    const int N = N0 + lane;
-    int4 rN = make_int4(0, 0, 0, 0);
-    if (N < n_end) rN = __ldg(rec + N);
-    const int oNx = (short)(rN.x & 0xffff), oNy = rN.x >> 16;
-    const int codeN = (rN.w >> 20) & 15;
-    const int d = max(abs(oNx), abs(oNy));                 // depth of N
-    // Bresenham state of the representative vector at position d (reading D2, closed form)
-    const int vx = (short)(rN.y & 0xffff), vy = rN.y >> 16;
-    const int ax = abs(vx), ay = abs(vy);
-    const bool xmaj = ax >= ay;
-    const int nn = xmaj ? ax : ay, mn = xmaj ? ay : ax;
-    const int sxs = (vx > 0) - (vx < 0), sys = (vy > 0) - (vy < 0);
-    const int q0 = xmaj ? abs(oNy) : abs(oNx);
-    const int e0 = 2 * d * mn + nn - 2 * nn * q0;
-    for (int q = 0; q < np; ++q) {
-      const unsigned nb = s_pass[q].nb;
-      const uint32_t* Pq = P + s_pass[q].pbase;
-      bool alive = (N < n_end) && (d == 0 || ((nb >> codeN) & 1u));
-      if (__any_sync(0xffffffffu, alive)) {                // (not so: typical for u, an isolated pixel kills all 32 at once)
-      const int ox = s_pass[q].ox, oy = s_pass[q].oy;
-      const int sx = wrap_coord(s_pass[q].px - oNx, W), sy = wrap_coord(s_pass[q].py - oNy, H);
-      if (alive && d >= 2)                                 // the far end first: a long prefix usually dies at its start
-        alive = pbit(Pq, sx, sy) && !(sx == ox && sy == oy);
-      if (alive) {
-        // (A) ancestors at positions d-2 .. 1 (d-1 was the neighbour test, 0 the start), stepping the error term backwards
-        int e = e0, qq = q0;
-        if (ox < 0) {
-          // fast walk (the w pass on I: nothing to mask): one linear bit index into the padded image, no modulo
-          const int PW = PWc * 32;
-          const int dmaj = xmaj ? sxs : sys * PW, dmin = xmaj ? sys * PW : sxs;
-          int L = (sy + m + oNy) * PW + (sx + m + oNx);      // pixel px itself (position d)
-          for (int k = d - 1; k >= 1; --k) {
-            e -= 2 * mn;
-            L -= dmaj;
-            if (e < 0) { e += 2 * nn; L -= dmin; }
-            if (k == d - 1) continue;
-            if (!((Pq[L >> 5] >> (L & 31)) & 1u)) { alive = false; break; }
-          }
-        } else {
-          for (int k = d - 1; k >= 1; --k) {
-            e -= 2 * mn;
-            if (e < 0) { e += 2 * nn; --qq; }
-            if (k == d - 1) continue;
-            const int ax_ = xmaj ? sxs * k : sxs * qq, ay_ = xmaj ? sys * qq : sys * k;
-            const int x = wrap_coord(sx + ax_, W), y = wrap_coord(sy + ay_, H);
-            if (!pbit(Pq, x, y) || (x == ox && y == oy)) { alive = false; break; }
-          }
-        }
-      }
-      int* const out = out0 + s_pass[q].out_off;
-      const int sign = s_pass[q].sign;
-      if (alive && (rN.w & 0xFFFFF) != 0xFFFFF) atomicAdd(out + (rN.w & 0xFFFFF), sign);
-      // (B) push the first child of every survivor, then drain the warp stack
-      const bool push = alive && rN.z > 1;
-      const unsigned pm = __ballot_sync(0xffffffffu, push);
-      if (push)
-        stk[top + __popc(pm & lt)] =
-            make_uint2((unsigned)(N + 1) | ((unsigned)q << 24), (unsigned)sx | ((unsigned)sy << 16));
-      top += __popc(pm);
-      __syncwarp();
-      }
-      // the survivors of all passes are explored together (the depth of the live region is paid once, not once
-      // per pass); the stack is drained early only when the next 32 pushes might not fit
-      if (top <= SWAP_STACK - 32 && q + 1 < np) continue;
-      while (top > 0) {
-        const int take = min(top, 32);
-        uint2 it = make_uint2(0, 0);
-        if (lane < take) it = stk[top - 1 - lane];
-        top -= take;
-        __syncwarp();
-        bool p_sib = false, p_child = false;
-        int i = 0;
-        if (lane < take) {
-          i = (int)(it.x & 0xFFFFFF);
-          const int qi = (int)(it.x >> 24);
-          const int4 r = __ldg(rec + i);
-          const int isx = (int)(it.y & 0xffff), isy = (int)(it.y >> 16);
-          const int x = wrap_coord(isx + (short)(r.x & 0xffff), W), y = wrap_coord(isy + (r.x >> 16), H);
-          const bool in = pbit(P + s_pass[qi].pbase, x, y) && !(x == s_pass[qi].ox && y == s_pass[qi].oy);
-          if (in && (r.w & 0xFFFFF) != 0xFFFFF)
-            atomicAdd(out0 + s_pass[qi].out_off + (r.w & 0xFFFFF), s_pass[qi].sign);
-          p_sib = (r.w >> 24) & 1;
-          p_child = in && r.z > 1;
-          if (p_sib) it.x += (unsigned)r.z;                // next sibling = i + subtree size
-        }
-        const unsigned ms = __ballot_sync(0xffffffffu, p_sib);
-        const unsigned mc = __ballot_sync(0xffffffffu, p_child);
-        const int ns = __popc(ms), nc = __popc(mc);
-        if (top + ns + nc > SWAP_STACK) {
-          // the stack cannot take this batch: every lane walks its own item's remainder serially (rare)
-          if (lane < take) {
-            const int qi = (int)(it.x >> 24);                // it.x may already point at the sibling: undo
-            const int isx = (int)(it.y & 0xffff), isy = (int)(it.y >> 16);
-            const int4 r0 = __ldg(rec + i);
-            // serial preorder scan of: the subtree of i below i (if in phase), then all later siblings' subtrees
-            int j = p_child ? i + 1 : i + r0.z;
-            // end of the scan: the parent's subtree end is unknown here, so follow sibling flags
-            bool more = true;
-            int cur_top = i;                                  // the sibling-level node whose subtree is scanned
-            int4 rt = r0;
-            while (more) {
-              const int end = cur_top + rt.z;
-              while (j < end) {
-                const int4 r = __ldg(rec + j);
-                const int x = wrap_coord(isx + (short)(r.x & 0xffff), W), y = wrap_coord(isy + (r.x >> 16), H);
-                const bool in = pbit(P + s_pass[qi].pbase, x, y) &&
-                                !(x == s_pass[qi].ox && y == s_pass[qi].oy);
-                if (in) {
-                  if ((r.w & 0xFFFFF) != 0xFFFFF)
-                    atomicAdd(out0 + s_pass[qi].out_off + (r.w & 0xFFFFF), s_pass[qi].sign);
-                  ++j;
-                } else {
-                  j += r.z;
-                }
-              }
-              more = (rt.w >> 24) & 1;
-              if (more) {                                     // move to the next sibling: test it like any node
-                cur_top = end;
-                rt = __ldg(rec + cur_top);
-                const int x = wrap_coord(isx + (short)(rt.x & 0xffff), W), y = wrap_coord(isy + (rt.x >> 16), H);
-                const bool in = pbit(P + s_pass[qi].pbase, x, y) &&
-                                !(x == s_pass[qi].ox && y == s_pass[qi].oy);
-                if (in && (rt.w & 0xFFFFF) != 0xFFFFF)
-                  atomicAdd(out0 + s_pass[qi].out_off + (rt.w & 0xFFFFF), s_pass[qi].sign);
-                j = in ? cur_top + 1 : cur_top + rt.z;
-              }
-            }
-          }
-        } else {
-          if (p_sib) stk[top + __popc(ms & lt)] = it;
-          if (p_child) stk[top + ns + __popc(mc & lt)] = make_uint2((unsigned)(i + 1) | (it.x & 0xFF000000u), it.y);
-          top += ns + nc;
-        }
-        __syncwarp();
-      }
-    }
-  }
+  __shared__ SwapShared sh;
+  const int plane_words = (H + 2 * m) * ((W + 2 * m + 31) >> 5);
+  uint2* stk = (uint2*)(sm + ((n_planes * plane_words + 1) & ~1));
+  for (int i = threadIdx.x; i < n_planes * plane_words; i += blockDim.x) sm[i] = bits[i];
+  const long long S2 = (long long)(2 * m + 1) * (2 * m + 1);
+  swap_delta_unit(sm, stk, sh, H, W, m, pairs, n, (long long)blockIdx.x * sw, rec, n_nodes,
+                  delta + (long long)blockIdx.x * sw * S2, n_planes, plane_stride, sw, blockIdx.y, gridDim.y);
 }
 
 // delta(-v) = delta(v) (Eq. 12): fills the half outside D of every [S][S] array
@@ -831,37 +614,64 @@ cudaError_t swap_delta_prepare(size_t max_smem) {
                               (int)max_smem - (int)fa.sharedSizeBytes);
 }
 
+// the padded bit planes of the base image for the swap-delta kernel: stage 1 of the bit-pack gives the row-major bit
+// image(s) (the column-major half is unused), pack_padded_kernel adds the periodic halo of m pixels.
+// bits: [n_planes compact images][n_planes padded planes]; returns the padded planes through *padded.
+cudaError_t launch_swap_bits(const uint8_t* image, uint32_t* bits, int H, int W, int m, int phase,
+                             unsigned int* counter, int n_sm, cudaStream_t st, uint32_t** padded_out) {
+  const int n_planes = phase < 0 ? 2 : 1;
+  const int Wc = (W + 31) / 32, Hc = (H + 31) / 32;
+  const int PWc = (W + 2 * m + 31) / 32, PH = H + 2 * m;
+  const long long img_words = (long long)H * Wc + (long long)W * Hc;
+  uint32_t* const padded = bits + (size_t)n_planes * img_words;
+  pack_base_kernel<<<(unsigned)std::max(1, (Hc * Wc + 7) / 8), 256, 0, st>>>(image, bits, 1, H, W, n_planes,
+                                                                             phase < 0 ? 0 : phase, counter);
+  pack_padded_kernel<<<dim3((unsigned)std::max(1, std::min((PH * PWc + 255) / 256, n_sm * 8)), (unsigned)n_planes), 256,
+                       0, st>>>(bits, padded, H, W, m, img_words);
+  *padded_out = padded;
+  return cudaGetLastError();
+}
+
+// the swap-delta kernel alone on the n_launch proposals of `pairs`: delta must be zero, only the canonical half is written
+static cudaError_t launch_swap_core(const uint32_t* padded, int H, int W, int m, int n_planes, const int* pairs,
+                                    long long n_launch, const int32_t* rec, int n_nodes, int* delta,
+                                    long long plane_stride, int n_sm, cudaStream_t st) {
+  const int PWc = (W + 2 * m + 31) / 32, PH = H + 2 * m;
+  const size_t smem = (size_t)((n_planes * PH * PWc + 1) & ~1) * 4 + (size_t)8 * SWAP_STACK * 8;
+  const long long S2 = (long long)(2 * m + 1) * (2 * m + 1);
+  // proposals per CTA: 8 for big batches; a small batch is spread over about four CTAs per SM instead
+  int sw = SWAP_SW;
+  while (sw > 1 && (n_launch + sw - 1) / sw < 4ll * n_sm) sw /= 2;
+  const long long ctas = (n_launch + sw - 1) / sw;
+  for (long long c0 = 0; c0 < ctas; c0 += (1ll << 30)) {
+    const long long cnt = std::min(ctas - c0, 1ll << 30);
+    const long long s0 = c0 * sw;
+    // node slices: about four CTAs per SM in total, at least 256 nodes per slice
+    const int slices =
+        (int)std::max(1ll, std::min<long long>({(4ll * n_sm + cnt - 1) / cnt, (n_nodes + 255) / 256, 65535ll}));
+    swap_delta_kernel_v3<<<dim3((unsigned)cnt, (unsigned)slices), 256, smem, st>>>(
+        padded, H, W, m, pairs + 4 * s0, n_launch - s0, (const int4*)rec, n_nodes, delta + s0 * S2, n_planes,
+        plane_stride, sw);
+  }
+  return cudaGetLastError();
+}
+
 // phase 0 | 1: one plane, delta [n][S][S];  phase < 0: both planes, phase k at delta + k * plane_stride
 cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W, int m, int phase, const int* pairs,
                               long long n, const int32_t* rec, int n_nodes, int* delta, long long plane_stride,
                               unsigned int* counter, int n_sm, cudaStream_t st) {
   const int n_planes = phase < 0 ? 2 : 1;
-  const int Wc = (W + 31) / 32, Hc = (H + 31) / 32;
-  const int PWc = (W + 2 * m + 31) / 32, PH = H + 2 * m;
-  const size_t smem = (size_t)((n_planes * PH * PWc + 1) & ~1) * 4 + (size_t)8 * SWAP_STACK * 8;
-  const long long img_words = (long long)H * Wc + (long long)W * Hc;
-  uint32_t* const padded = bits + (size_t)n_planes * img_words;
-  cudaError_t e = cudaSuccess;
   const long long S2 = (long long)(2 * m + 1) * (2 * m + 1);
+  cudaError_t e = cudaSuccess;
   for (int pl = 0; pl < n_planes; ++pl) {
     e = cudaMemsetAsync(delta + pl * plane_stride, 0, sizeof(int) * (size_t)n * S2, st);
     if (e != cudaSuccess) return e;
   }
-  // stage 1 of the bit-pack gives the row-major bit image(s) of the base image (the column-major half is unused)
-  pack_base_kernel<<<(unsigned)std::max(1, (Hc * Wc + 7) / 8), 256, 0, st>>>(image, bits, 1, H, W, n_planes,
-                                                                             phase < 0 ? 0 : phase, counter);
-  pack_padded_kernel<<<dim3((unsigned)std::max(1, std::min((PH * PWc + 255) / 256, n_sm * 8)), (unsigned)n_planes), 256,
-                       0, st>>>(bits, padded, H, W, m, img_words);
-  const long long ctas = (n + SWAP_SW - 1) / SWAP_SW;
-  for (long long c0 = 0; c0 < ctas; c0 += (1ll << 30)) {
-    const long long cnt = std::min(ctas - c0, 1ll << 30);
-    const long long s0 = c0 * SWAP_SW;
-    // node slices: about two CTAs per SM in total, at least 256 nodes per slice
-    const int slices =
-        (int)std::max(1ll, std::min<long long>({(2ll * n_sm + cnt - 1) / cnt, (n_nodes + 255) / 256, 65535ll}));
-    swap_delta_kernel_v3<<<dim3((unsigned)cnt, (unsigned)slices), 256, smem, st>>>(
-        padded, H, W, m, pairs + 4 * s0, n - s0, (const int4*)rec, n_nodes, delta + s0 * S2, n_planes, plane_stride);
-  }
+  uint32_t* padded = nullptr;
+  e = launch_swap_bits(image, bits, H, W, m, phase, counter, n_sm, st, &padded);
+  if (e != cudaSuccess) return e;
+  e = launch_swap_core(padded, H, W, m, n_planes, pairs, n, rec, n_nodes, delta, plane_stride, n_sm, st);
+  if (e != cudaSuccess) return e;
   const long long blocks = std::max(1ll, std::min<long long>((n * (S2 / 2) + 255) / 256, (long long)n_sm * 16));
   for (int pl = 0; pl < n_planes; ++pl)
     swap_mirror_kernel<<<(unsigned)blocks, 256, 0, st>>>(delta + pl * plane_stride, 2 * m + 1, n);

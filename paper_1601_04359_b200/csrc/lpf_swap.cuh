@@ -1,0 +1,249 @@
+// lpf_swap.cuh -- device code of the swap-delta evaluation,
+// shared by swap_delta_kernel_v3 (lpf_kernels.cu) and the persistent annealing kernel (lpf_anneal.cu).
+//   For one proposal let u be the pixel whose bit becomes 1 and w the one whose bit becomes 0:
+//     delta(v) = #{segments of vector v that contain u and lie in phase in I'}
+//              - #{segments of vector v that contain w and lie in phase in I }
+//   A segment of v that has pixel px at path position k starts at s = px - P_v[k]; P_v[0..k] is a trie node N, so
+//   the candidates are exactly the pairs (trie node N, terminal D in the subtree of N) with start s_N = px - o_N.
+//   (A) lane per node N: the prefix root -> N must be in phase from s_N.  The parent's pixel is one of the 8
+//       neighbours of px (register mask lookup: most nodes stop there); the other ancestors' pixels are stepped
+//       backwards with Bresenham error arithmetic on a vector that runs through N -- no loads but the image bits.
+//   (B) the subtrees of all surviving (N, start) are explored by the whole CTA from one stack in shared memory: a
+//       thread pops one node, tests its pixel, counts it if it is a terminal, and pushes its next sibling (always)
+//       and its first child (if the pixel is in phase).  A dead prefix kills every vector below it at once.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+namespace lpf {
+
+constexpr int SWAP_SW = 8;          // proposals per CTA
+constexpr int SWAP_STACK = 512;     // items per warp stack (8 bytes each)
+
+__device__ __forceinline__ int wrap_coord(int x, int n) {
+  x += (x < 0) ? n : 0;
+  x -= (x >= n) ? n : 0;
+  return x;
+}
+
+struct SwapPass {                   // one (proposal, pixel) pass, in shared memory
+  int px, py;                       // the swapped pixel the segments must contain
+  int ox, oy;                       // pixel that reads as out of phase in this pass (w in I'), or -1
+  unsigned nb;                      // in-phase bits of the 8 neighbours px - step, by step code
+  int sign;                         // +1: u on I', -1: w on I
+  int pbase;                        // word offset of this pass's phase plane in the shared-memory bit images
+  long long out_off;                // offset of this pass's [S][S] delta array from the CTA's first one
+};
+
+struct SwapShared {                 // per-CTA scratch of swap_delta_unit
+  SwapPass pass[4 * SWAP_SW];       // (proposal, phase plane, pixel)
+  int n;                            // passes
+  int top;                          // items on the CTA's stack (may run past its capacity: see swap_delta_unit)
+};
+
+// One unit of swap-delta work of a CTA of 256 threads: the proposals pairs[first_prop .. first_prop + sw) (those below
+// n; sw <= SWAP_SW) against node slice `slice` of `n_slices` equal slices of the trie.  Adds into out0 [sw][S][S]
+// (canonical half only; plane k at + k * plane_stride), which must have been zeroed.
+//   P    shared memory: [n_planes][H + 2m][ceil((W + 2m) / 32)] bits of the base image with its halo of m pixels
+//   stk  shared memory: the CTA's stack of 8 * SWAP_STACK items (8 bytes each)
+__device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, SwapShared& sh, int H, int W, int m,
+                                                const int* __restrict__ pairs, long long n, long long first_prop,
+                                                const int4* __restrict__ rec, int n_nodes, int* __restrict__ out0,
+                                                int n_planes, long long plane_stride, int sw, int slice,
+                                                int n_slices) {
+  const int PWc = (W + 2 * m + 31) >> 5, PH = H + 2 * m;                // padded bit image: halo of m pixels all round
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int plane_words = PH * PWc;
+  // pixel (x, y) of the plane at Pq, x in [-m, W + m), y in [-m, H + m)
+  auto pbit = [&](const uint32_t* Pq, int x, int y) -> unsigned {
+    const int X = x + m;
+    return (Pq[(y + m) * PWc + (X >> 5)] >> (X & 31)) & 1u;
+  };
+  const int S = 2 * m + 1;
+  const long long K = (long long)S * S;
+  __syncthreads();                                        // the previous unit of this CTA is finished with sh
+  if (tid == 0) { sh.n = 0; sh.top = 0; }
+  __syncthreads();
+  // one thread per (proposal of this CTA, phase plane): its two passes (u on I', w on I) go to the next free slots
+  if (tid < sw * n_planes) {
+    const int j = tid / n_planes, pl = tid - j * n_planes;
+    const long long swi = first_prop + j;
+    if (swi < n) {
+      const int xp = pairs[4 * swi], yp = pairs[4 * swi + 1], xq = pairs[4 * swi + 2], yq = pairs[4 * swi + 3];
+      const bool ok = xp >= 0 && xp < W && xq >= 0 && xq < W && yp >= 0 && yp < H && yq >= 0 && yq < H;
+      const uint32_t* Pq = P + pl * plane_words;
+      const int bp = ok ? (int)pbit(Pq, xp, yp) : 0, bq = ok ? (int)pbit(Pq, xq, yq) : 0;
+      if (bp != bq) {                                        // otherwise nothing changes for this phase
+        const int ux = bp ? xq : xp, uy = bp ? yq : yp;      // bit 0 -> 1
+        const int wx = bp ? xp : xq, wy = bp ? yp : yq;      // bit 1 -> 0
+        const int slot = atomicAdd(&sh.n, 2);
+        for (int pass = 0; pass < 2; ++pass) {
+          SwapPass sp;
+          sp.px = pass ? wx : ux; sp.py = pass ? wy : uy;
+          sp.ox = pass ? -1 : wx; sp.oy = pass ? -1 : wy;
+          sp.nb = 0;
+          for (int code = 0; code < 9; ++code) {
+            const int x = wrap_coord(sp.px - (code / 3 - 1), W), y = wrap_coord(sp.py - (code % 3 - 1), H);
+            unsigned bit = pbit(Pq, x, y);
+            if (x == sp.ox && y == sp.oy) bit = 0;
+            sp.nb |= bit << code;
+          }
+          sp.sign = pass ? -1 : 1;
+          sp.pbase = pl * plane_words;
+          sp.out_off = (long long)pl * plane_stride + (long long)j * K;
+          sh.pass[slot + pass] = sp;
+        }
+      }
+    }
+  }
+  __syncthreads();
+  const int np = sh.n;
+  if (np == 0) return;
+  const unsigned lt = (1u << lane) - 1u;
+  constexpr int CAP = 8 * SWAP_STACK;                      // the CTA's stack: the eight warp stacks as one
+  constexpr unsigned DUMMY = 0xFFFFFFFFu;                  // a reserved slot that was not filled
+  // test node i of pass qi from start (isx, isy): in phase?  counts it if it is a whole path
+  auto visit = [&](int i, int qi, int isx, int isy, const int4& r) -> bool {
+    const int x = wrap_coord(isx + (short)(r.x & 0xffff), W), y = wrap_coord(isy + (r.x >> 16), H);
+    const bool in = pbit(P + sh.pass[qi].pbase, x, y) && !(x == sh.pass[qi].ox && y == sh.pass[qi].oy);
+    if (in && (r.w & 0xFFFFF) != 0xFFFFF) atomicAdd(out0 + sh.pass[qi].out_off + (r.w & 0xFFFFF), sh.pass[qi].sign);
+    return in;
+  };
+  // serial fall-backs for a full stack (rare): the preorder range [j, end) with dead subtrees skipped; node `cur`, its
+  // later siblings and everything below them
+  auto scan_range = [&](int j, int end, int qi, int isx, int isy) {
+    while (j < end) {
+      const int4 r = __ldg(rec + j);
+      j += visit(j, qi, isx, isy, r) ? 1 : r.z;
+    }
+  };
+  auto scan_siblings = [&](int cur, int qi, int isx, int isy) {
+    for (;;) {
+      const int4 r = __ldg(rec + cur);
+      if (visit(cur, qi, isx, isy, r)) scan_range(cur + 1, cur + r.z, qi, isx, isy);
+      if (!((r.w >> 24) & 1)) break;
+      cur += r.z;
+    }
+  };
+  // reserves cnt slots of the CTA's stack for this warp and returns the first; slots at or beyond CAP do not exist:
+  // their owners walk their items serially instead, and the stack top is clamped before the next pop
+  auto reserve = [&](int cnt) -> int {
+    int base = 0;
+    if (lane == 0) base = atomicAdd(&sh.top, cnt);
+    return __shfl_sync(0xffffffffu, base, 0);
+  };
+
+  // the node range is sliced, so that a small batch of proposals still fills the chip
+  const int slice_nodes = (n_nodes + n_slices - 1) / n_slices;
+  const int n_begin = slice * slice_nodes, n_end = min(n_nodes, n_begin + slice_nodes);
+  const int n_iter = (n_end - n_begin + (int)blockDim.x - 1) / (int)blockDim.x;
+  for (int itn = 0; itn < n_iter; ++itn) {
+    const int N = n_begin + itn * blockDim.x + tid;
+    int4 rN = make_int4(0, 0, 0, 0);
+    if (N < n_end) rN = __ldg(rec + N);
+    const int oNx = (short)(rN.x & 0xffff), oNy = rN.x >> 16;
+    const int codeN = (rN.w >> 20) & 15;
+    const int d = max(abs(oNx), abs(oNy));                 // depth of N
+    // Bresenham state of the representative vector at position d (reading D2, closed form)
+    const int vx = (short)(rN.y & 0xffff), vy = rN.y >> 16;
+    const int ax = abs(vx), ay = abs(vy);
+    const bool xmaj = ax >= ay;
+    const int nn = xmaj ? ax : ay, mn = xmaj ? ay : ax;
+    const int sxs = (vx > 0) - (vx < 0), sys = (vy > 0) - (vy < 0);
+    const int q0 = xmaj ? abs(oNy) : abs(oNx);
+    const int e0 = 2 * d * mn + nn - 2 * nn * q0;
+    for (int q = 0; q < np; ++q) {
+      const unsigned nb = sh.pass[q].nb;
+      const uint32_t* Pq = P + sh.pass[q].pbase;
+      bool alive = (N < n_end) && (d == 0 || ((nb >> codeN) & 1u));
+      if (!__any_sync(0xffffffffu, alive)) continue;       // typical for u: an isolated pixel kills all 32 at once
+      const int ox = sh.pass[q].ox, oy = sh.pass[q].oy;
+      const int sx = wrap_coord(sh.pass[q].px - oNx, W), sy = wrap_coord(sh.pass[q].py - oNy, H);
+      if (alive && d >= 2)                                 // the far end first: a long prefix usually dies at its start
+        alive = pbit(Pq, sx, sy) && !(sx == ox && sy == oy);
+      if (alive) {
+        // (A) ancestors at positions d-2 .. 1 (d-1 was the neighbour test, 0 the start), stepping the error term backwards
+        int e = e0, qq = q0;
+        if (ox < 0) {
+          // fast walk (the w pass on I: nothing to mask): one linear bit index into the padded image, no modulo
+          const int PW = PWc * 32;
+          const int dmaj = xmaj ? sxs : sys * PW, dmin = xmaj ? sys * PW : sxs;
+          int L = (sy + m + oNy) * PW + (sx + m + oNx);      // pixel px itself (position d)
+          for (int k = d - 1; k >= 1; --k) {
+            e -= 2 * mn;
+            L -= dmaj;
+            if (e < 0) { e += 2 * nn; L -= dmin; }
+            if (k == d - 1) continue;
+            if (!((Pq[L >> 5] >> (L & 31)) & 1u)) { alive = false; break; }
+          }
+        } else {
+          for (int k = d - 1; k >= 1; --k) {
+            e -= 2 * mn;
+            if (e < 0) { e += 2 * nn; --qq; }
+            if (k == d - 1) continue;
+            const int ax_ = xmaj ? sxs * k : sxs * qq, ay_ = xmaj ? sys * qq : sys * k;
+            const int x = wrap_coord(sx + ax_, W), y = wrap_coord(sy + ay_, H);
+            if (!pbit(Pq, x, y) || (x == ox && y == oy)) { alive = false; break; }
+          }
+        }
+      }
+      if (alive && (rN.w & 0xFFFFF) != 0xFFFFF) atomicAdd(out0 + sh.pass[q].out_off + (rN.w & 0xFFFFF), sh.pass[q].sign);
+      // (B) the first child of every survivor goes on the CTA's stack
+      const bool push = alive && rN.z > 1;
+      const unsigned pm = __ballot_sync(0xffffffffu, push);
+      if (pm) {
+        const int pos = reserve(__popc(pm)) + __popc(pm & lt);
+        if (push) {
+          if (pos < CAP) stk[pos] = make_uint2((unsigned)(N + 1) | ((unsigned)q << 24), (unsigned)sx | ((unsigned)sy << 16));
+          else scan_siblings(N + 1, q, sx, sy);
+        }
+      }
+    }
+    // The survivors of all passes and of all warps are explored together, by the whole CTA (a deep live region is
+    // paid once, and a big one is shared by eight warps): now, if the stack is half full or the slice is finished.
+    if (!__syncthreads_or(itn + 1 == n_iter || sh.top > CAP / 2)) continue;   // one decision for the whole CTA
+    for (;;) {
+      const int n = min(sh.top, CAP);                      // slots beyond CAP were never written: their owners scanned
+      if (n == 0) break;
+      const int take = min(n, (int)blockDim.x);
+      uint2 it = make_uint2(DUMMY, 0);
+      if (tid < take) it = stk[n - 1 - tid];
+      __syncthreads();                                     // every thread has read top and its item
+      if (tid == 0) sh.top = n - take;
+      __syncthreads();
+      bool p_sib = false, p_child = false;
+      int i = 0, qi = 0, isx = 0, isy = 0, size_i = 0;
+      if (it.x != DUMMY) {
+        i = (int)(it.x & 0xFFFFFF);
+        qi = (int)(it.x >> 24);
+        isx = (int)(it.y & 0xffff);
+        isy = (int)(it.y >> 16);
+        const int4 r = __ldg(rec + i);
+        size_i = r.z;
+        p_child = visit(i, qi, isx, isy, r) && r.z > 1;
+        p_sib = (r.w >> 24) & 1;
+        if (p_sib) it.x += (unsigned)r.z;                  // next sibling = i + subtree size
+      }
+      const unsigned ms = __ballot_sync(0xffffffffu, p_sib);
+      const unsigned mc = __ballot_sync(0xffffffffu, p_child);
+      const int ns = __popc(ms), nc = __popc(mc);
+      if (ns + nc) {
+        const int base = reserve(ns + nc);
+        if (base + ns + nc <= CAP) {
+          if (p_sib) stk[base + __popc(ms & lt)] = it;
+          if (p_child) stk[base + ns + __popc(mc & lt)] = make_uint2((unsigned)(i + 1) | (it.x & 0xFF000000u), it.y);
+        } else {
+          // the stack cannot take this warp's pushes: every lane walks the remainder of its own item serially, and
+          // the part of the reservation that lies inside the stack is marked unused
+          for (int k = base + lane; k < min(base + ns + nc, CAP); k += 32) stk[k] = make_uint2(DUMMY, 0);
+          if (p_child) scan_range(i + 1, i + size_i, qi, isx, isy);
+          if (p_sib) scan_siblings(i + size_i, qi, isx, isy);
+        }
+      }
+      __syncthreads();                                     // all pushes of this round are in
+    }
+  }
+}
+
+}  // namespace lpf
