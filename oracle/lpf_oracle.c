@@ -37,6 +37,9 @@
  * count, point symmetry, equality with the lineal-path counts for the 8 neighbours (|P_v| = 2).
  * lpf_oracle_counts_sum (ensemble over a stack): one image = lpf_oracle_counts, additive over a split of
  * the stack, k copies of the worked image = k times its golden counts, Eq. 10 summed (centre = phase pixels of the stack).
+ * lpf_oracle_splitmix64 / lpf_oracle_propose (modification operator, reading A7): the published SplitMix64 test vectors;
+ * every generated pair has different bytes and (policy 2) two interfacial pixels, checked with numpy; uniform over the
+ * qualifying pixels (chi-square); the generating chain = the list chain fed with the generated pairs.
  * lpf_oracle_anneal (Alg. 3): the Metropolis threshold at finite T against exact rationals computed in the test, volume fractions preserved, E tracked = Eq. 19 of the final image re-evaluated, a huge
  * T accepts every move (final image = all swaps applied, temperature levels = floor(N / s_max)), a tiny T never lets E
  * grow, the local-delta form equals the literal re-evaluation form decision by decision.
@@ -353,10 +356,65 @@ static uint64_t half_sse_(const int64_t *c, const int64_t *t, int m)
     return e;
 }
 
-void lpf_oracle_anneal(uint8_t *img, int H, int W, int phase, int m, const int64_t *target,
-                       const int32_t *pairs, const double *log_u, int64_t N,
-                       double T_max, double T_min, int64_t c_max, int64_t s_max, int use_local,
-                       int64_t *counts_out, double *stats, uint8_t *accept_log)
+/* Modification operator of Alg. 3 line 9, generated from the CURRENT image ("interchanging two
+ * randomly chosen pixels from different phases ... Very simple acceleration employed in our implementation consists in
+ * a random selection of interfacial pixels").  The paper does not say how the pixels are drawn; reading A7 of DESIGN.md:
+ *   random words: the counter-based generator SplitMix64 (Steele, Lea, Flood 2014; Vigna's splitmix64.c): the n-th
+ *     output for `seed` is mix(seed + n * 0x9E3779B97F4A7C15); proposal k, attempt t (0..63), side s (0: p, 1: q) uses
+ *     n = 1 + 2 * (64 k + t) + s;  a word u gives the pixel x = ((u >> 32) * W) >> 32, y = ((u & 0xffffffff) * H) >> 32
+ *   policy 1 (opposite):    p = attempt 0 of side 0 (any pixel); q = the first attempt of side 1 whose byte differs from p's
+ *   policy 2 (interfacial): p = the first attempt of side 0 that is interfacial; q = the first attempt of side 1 that is
+ *     interfacial and whose byte differs from p's.  A pixel is interfacial iff one of its 4 periodic neighbours
+ *     (x+-1, y), (x, y+-1) has a different byte.
+ *   no attempt qualifies (64 tried): q = p, the identity move (reading A5).
+ * Rejection from uniform draws = uniform over the qualifying pixels. */
+uint64_t lpf_oracle_splitmix64(uint64_t seed, uint64_t n)
+{
+    uint64_t z = seed + n * 0x9E3779B97F4A7C15ULL;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+
+static int interfacial_(const uint8_t *img, int H, int W, int x, int y)
+{
+    uint8_t b = img[(size_t)y * W + x];
+    return img[(size_t)y * W + pmod_(x + 1, W)] != b || img[(size_t)y * W + pmod_(x - 1, W)] != b ||
+           img[(size_t)pmod_(y + 1, H) * W + x] != b || img[(size_t)pmod_(y - 1, H) * W + x] != b;
+}
+
+void lpf_oracle_propose(const uint8_t *img, int H, int W, int policy, uint64_t seed, int64_t k, int32_t *pair)
+{
+    int px = -1, py = -1, qx = -1, qy = -1;
+    for (int t = 0; t < 64 && px < 0; ++t) {
+        uint64_t u = lpf_oracle_splitmix64(seed, 1 + 2 * (64 * (uint64_t)k + (uint64_t)t));
+        int x = (int)(((u >> 32) * (uint64_t)W) >> 32), y = (int)(((u & 0xffffffffULL) * (uint64_t)H) >> 32);
+        if (policy == 1 || interfacial_(img, H, W, x, y)) { px = x; py = y; }
+    }
+    if (px < 0) {                                   /* no interfacial pixel met: attempt 0 of side 0, identity move */
+        uint64_t u = lpf_oracle_splitmix64(seed, 1 + 2 * (64 * (uint64_t)k));
+        px = (int)(((u >> 32) * (uint64_t)W) >> 32); py = (int)(((u & 0xffffffffULL) * (uint64_t)H) >> 32);
+        pair[0] = px; pair[1] = py; pair[2] = px; pair[3] = py;
+        return;
+    }
+    for (int t = 0; t < 64 && qx < 0; ++t) {
+        uint64_t u = lpf_oracle_splitmix64(seed, 1 + 2 * (64 * (uint64_t)k + (uint64_t)t) + 1);
+        int x = (int)(((u >> 32) * (uint64_t)W) >> 32), y = (int)(((u & 0xffffffffULL) * (uint64_t)H) >> 32);
+        if (img[(size_t)y * W + x] != img[(size_t)py * W + px] && (policy == 1 || interfacial_(img, H, W, x, y))) {
+            qx = x; qy = y;
+        }
+    }
+    if (qx < 0) { qx = px; qy = py; }
+    pair[0] = px; pair[1] = py; pair[2] = qx; pair[3] = qy;
+}
+
+/* policy 0: proposal n is pairs[n] (given); policy 1 | 2: it is generated from the current image by lpf_oracle_propose
+ * and written to pairs_out[n] (may be NULL) */
+static void anneal_core_(uint8_t *img, int H, int W, int phase, int m, const int64_t *target,
+                         const int32_t *pairs, const double *log_u, int64_t N,
+                         double T_max, double T_min, int64_t c_max, int64_t s_max, int use_local,
+                         int64_t *counts_out, double *stats, uint8_t *accept_log,
+                         int policy, uint64_t seed, int32_t *pairs_out)
 {
     int S = 2 * m + 1;
     size_t K = (size_t)S * S;
@@ -376,7 +434,14 @@ void lpf_oracle_anneal(uint8_t *img, int H, int W, int phase, int m, const int64
         int64_t c = 0, s = 0;                                  /* line 6 */
         while (c < c_max && s < s_max && n < N) {              /* line 7 */
             c = c + 1;                                         /* line 8 */
-            int xp = pairs[4 * n], yp = pairs[4 * n + 1], xq = pairs[4 * n + 2], yq = pairs[4 * n + 3];
+            int32_t gen[4];
+            if (policy != 0) {                                 /* line 9: the operator draws its pixels from P */
+                lpf_oracle_propose(img, H, W, policy, seed, n, gen);
+                if (pairs_out) memcpy(pairs_out + 4 * n, gen, sizeof(gen));
+            } else {
+                memcpy(gen, pairs + 4 * n, sizeof(gen));
+            }
+            int xp = gen[0], yp = gen[1], xq = gen[2], yq = gen[3];
             /* line 9: Q = modify(P) */
             uint8_t bp = img[(size_t)yp * W + xp], bq = img[(size_t)yq * W + xq];
             if (use_local) {
@@ -413,6 +478,26 @@ void lpf_oracle_anneal(uint8_t *img, int H, int W, int phase, int m, const int64
     }
     stats[0] = (double)n; stats[1] = (double)accepted; stats[2] = (double)levels; stats[3] = T; stats[4] = (double)EP;
     free(cQ); free(dl);
+}
+
+void lpf_oracle_anneal(uint8_t *img, int H, int W, int phase, int m, const int64_t *target,
+                       const int32_t *pairs, const double *log_u, int64_t N,
+                       double T_max, double T_min, int64_t c_max, int64_t s_max, int use_local,
+                       int64_t *counts_out, double *stats, uint8_t *accept_log)
+{
+    anneal_core_(img, H, W, phase, m, target, pairs, log_u, N, T_max, T_min, c_max, s_max, use_local,
+                 counts_out, stats, accept_log, 0, 0, NULL);
+}
+
+/* Alg. 3 with the modification operator drawing its own pixels (policy 1 | 2 above); pairs_out[N][4] receives the
+ * proposal that was decided at every step. */
+void lpf_oracle_anneal_generate(uint8_t *img, int H, int W, int phase, int m, const int64_t *target,
+                                int policy, uint64_t seed, int32_t *pairs_out, const double *log_u, int64_t N,
+                                double T_max, double T_min, int64_t c_max, int64_t s_max, int use_local,
+                                int64_t *counts_out, double *stats, uint8_t *accept_log)
+{
+    anneal_core_(img, H, W, phase, m, target, NULL, log_u, N, T_max, T_min, c_max, s_max, use_local,
+                 counts_out, stats, accept_log, policy, seed, pairs_out);
 }
 
 int lpf_oracle_max_threads(void)

@@ -64,6 +64,15 @@ def _load():
                                           ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int64,
                                           ctypes.c_int64, I, c_i64p, ctypes.POINTER(ctypes.c_double), c_u8p]
         lib.lpf_oracle_anneal.restype = None
+        lib.lpf_oracle_splitmix64.argtypes = [ctypes.c_uint64, ctypes.c_uint64]
+        lib.lpf_oracle_splitmix64.restype = ctypes.c_uint64
+        lib.lpf_oracle_propose.argtypes = [c_u8p, I, I, I, ctypes.c_uint64, ctypes.c_int64, c_i32p]
+        lib.lpf_oracle_propose.restype = None
+        lib.lpf_oracle_anneal_generate.argtypes = [c_u8p, I, I, I, I, c_i64p, I, ctypes.c_uint64, c_i32p,
+                                                   ctypes.POINTER(ctypes.c_double), ctypes.c_int64, ctypes.c_double,
+                                                   ctypes.c_double, ctypes.c_int64, ctypes.c_int64, I, c_i64p,
+                                                   ctypes.POINTER(ctypes.c_double), c_u8p]
+        lib.lpf_oracle_anneal_generate.restype = None
         lib.lpf_oracle_max_threads.argtypes = []
         lib.lpf_oracle_max_threads.restype = I
         _lib = lib
@@ -172,6 +181,42 @@ def anneal(image, phase: int, m: int, target, pairs, log_u, T_max: float, T_min:
                               _p(stats, ctypes.c_double), _p(log, ctypes.c_uint8))
     keys = ("steps", "accepted", "levels", "T", "E")
     return a, counts_out, dict(zip(keys, [float(v) for v in stats])), log
+
+
+def splitmix64(seed: int, n: int) -> int:
+    """n-th output (n = 1, 2, ...) of SplitMix64 seeded with `seed`."""
+    return int(_load().lpf_oracle_splitmix64(int(seed) & (2 ** 64 - 1), int(n)))
+
+
+def propose(image, policy: int, seed: int, k: int) -> np.ndarray:
+    """The pair (x_p, y_p, x_q, y_q) the modification operator draws for proposal k from `image` (reading A7)."""
+    a = _img(image)
+    pair = np.zeros(4, dtype=np.int32)
+    _load().lpf_oracle_propose(_p(a, ctypes.c_uint8), a.shape[0], a.shape[1], int(policy), int(seed) & (2 ** 64 - 1),
+                               int(k), _p(pair, ctypes.c_int32))
+    return pair
+
+
+def anneal_generate(image, phase: int, m: int, target, policy: int, seed: int, log_u, T_max: float, T_min: float,
+                    c_max: int, s_max: int, use_local: bool = False):
+    """Alg. 3 with generated proposals.  Returns (final image, counts, stats, accept log, pairs decided int32 [N, 4])."""
+    a = _img(image).copy()
+    S = 2 * int(m) + 1
+    n_ph = 2 if phase < 0 else 1
+    t = np.ascontiguousarray(target, dtype=np.int64).reshape(n_ph, S, S)
+    lu = np.ascontiguousarray(log_u, dtype=np.float64)
+    N = lu.shape[0]
+    counts_out = np.zeros((n_ph, S, S), dtype=np.int64)
+    stats = np.zeros(5, dtype=np.float64)
+    log = np.zeros(N, dtype=np.uint8)
+    pairs = np.zeros((N, 4), dtype=np.int32)
+    _load().lpf_oracle_anneal_generate(_p(a, ctypes.c_uint8), a.shape[0], a.shape[1], int(phase), int(m),
+                                       _p(t, ctypes.c_int64), int(policy), int(seed) & (2 ** 64 - 1),
+                                       _p(pairs, ctypes.c_int32), _p(lu, ctypes.c_double), N, float(T_max), float(T_min),
+                                       int(c_max), int(s_max), int(bool(use_local)), _p(counts_out, ctypes.c_int64),
+                                       _p(stats, ctypes.c_double), _p(log, ctypes.c_uint8))
+    keys = ("steps", "accepted", "levels", "T", "E")
+    return a, counts_out, dict(zip(keys, [float(v) for v in stats])), log, pairs
 
 
 def half_sse(c, t, m: int) -> int:

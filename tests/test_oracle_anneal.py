@@ -153,3 +153,78 @@ def test_metropolis_threshold_follows_the_temperature_schedule():
             assert st["levels"] == 2 and st["T"] == T2 * (T_min / T_max) ** (s_max / N)
         done += 1
     assert done >= 20
+
+
+# ---- the modification operator drawing its own pixels (reading A7) ------------------
+
+def test_splitmix64_published_vectors():
+    """Reference outputs of Vigna's splitmix64.c for seed 1234567 (also the Rosetta Code task's expected values) and
+    the well-known first output for seed 0."""
+    want = [6457827717110365317, 3203168211198807973, 9817491932198370423, 4593380528125082431, 16408922859458223821]
+    assert [orc.splitmix64(1234567, n) for n in range(1, 6)] == want
+    assert orc.splitmix64(0, 1) == 0xE220A8397B1DCDAF
+
+
+def _interfacial(img):
+    return ((img != np.roll(img, 1, 0)) | (img != np.roll(img, -1, 0)) | (img != np.roll(img, 1, 1)) |
+            (img != np.roll(img, -1, 1)))
+
+
+@pytest.mark.parametrize("policy", [1, 2])
+def test_proposals_have_the_policy_properties_and_are_uniform(policy):
+    H, W = 11, 14                                               # non-square: a transposed pixel would leave the image
+    img = inputs.squares(H, W, 3, 0.4, 77)
+    inter = _interfacial(img)
+    n = 6000
+    pr = np.array([orc.propose(img, policy, 99, k) for k in range(n)])
+    xp, yp, xq, yq = pr.T
+    assert np.all((0 <= xp) & (xp < W) & (0 <= yp) & (yp < H) & (0 <= xq) & (xq < W) & (0 <= yq) & (yq < H))
+    assert np.all(img[yp, xp] != img[yq, xq])                   # "two ... pixels from different phases"
+    if policy == 2:
+        assert inter[yp, xp].all() and inter[yq, xq].all()      # "random selection of interfacial pixels"
+    # p is uniform over the qualifying pixels; q uniform over the qualifying pixels of the other byte, given p's byte
+    ok_p = inter if policy == 2 else np.ones_like(inter)
+    cnt = np.zeros((H, W))
+    np.add.at(cnt, (yp, xp), 1)
+    exp = n / ok_p.sum()
+    chi2 = (((cnt - exp) ** 2)[ok_p] / exp).sum()
+    assert cnt[~ok_p].sum() == 0 and chi2 < ok_p.sum() + 6 * np.sqrt(2 * ok_p.sum())
+    for b in (0, 1):
+        sel = img[yp, xp] == b
+        ok_q = ok_p & (img != b)
+        cq = np.zeros((H, W))
+        np.add.at(cq, (yq[sel], xq[sel]), 1)
+        e = sel.sum() / ok_q.sum()
+        assert cq[~ok_q].sum() == 0 and (((cq - e) ** 2)[ok_q] / e).sum() < ok_q.sum() + 6 * np.sqrt(2 * ok_q.sum())
+    # the random words are the documented ones: proposal k, attempt 0, side 0 is SplitMix64 output 1 + 128 k
+    if policy == 1:
+        for k in (0, 1, 17):
+            u = orc.splitmix64(99, 1 + 128 * k)
+            assert (xp[k], yp[k]) == (((u >> 32) * W) >> 32, ((u & 0xffffffff) * H) >> 32)
+
+
+def test_no_qualifying_pixel_gives_the_identity_move():
+    img = np.ones((6, 9), dtype=np.uint8)                        # one phase only: nothing to exchange
+    for policy in (1, 2):
+        pr = orc.propose(img, policy, 5, 3)
+        assert (pr[0], pr[1]) == (pr[2], pr[3])
+
+
+@pytest.mark.parametrize("policy,phase", [(1, 1), (2, -1)])
+def test_generating_chain_equals_the_list_chain_on_its_own_proposals(policy, phase):
+    """Every decided proposal was drawn from the image of that moment (replayed here with numpy), and feeding the
+    decided proposals back as a LIST reproduces the chain (the list chain is pinned above)."""
+    H, W, m, N = 10, 12, 5, 160
+    start, target, _, log_u, _ = _setup(H, W, m, phase, 41, N)
+    E0 = _half_E(start, target, (0, 1) if phase < 0 else (phase,), m)
+    T_max = 2.0 * E0 / (H * W) ** 2 / 50
+    img, counts, st, log, pairs = orc.anneal_generate(start, phase, m, target, policy, 2024, log_u, T_max, 0.01 * T_max,
+                                                      16, 5)
+    cur = start.copy()
+    for k in range(N):
+        assert np.array_equal(pairs[k], orc.propose(cur, policy, 2024, k)), k
+        if log[k]:
+            cur = _swapped(cur, pairs[k])
+    assert np.array_equal(cur, img) and 0 < log.sum() < N
+    a = orc.anneal(start, phase, m, target, pairs, log_u, T_max, 0.01 * T_max, 16, 5)
+    assert np.array_equal(a[0], img) and np.array_equal(a[1], counts) and a[2] == st and np.array_equal(a[3], log)
