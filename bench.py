@@ -571,6 +571,7 @@ def main():
         np.random.default_rng(inputs.seed_for(7, 1)).shuffle(start)
         pairs, log_u = inputs.anneal_proposals(H, W, n, inputs.seed_for(7, 2))
         pa = lpf.lpf_build_paths(m, local_rank)
+        lpf.lpf_reserve(pa, 1, H, W, 0, lpf.LPF_FOR_ANNEAL)
         target = lpf.lpf_eval_both(pa, torch.from_numpy(tgt_img[None]).cuda())[0].clone()
         d_img = torch.from_numpy(start.reshape(1, H, W).copy()).cuda()
         c0 = lpf.lpf_eval_both(pa, d_img)[0]
@@ -591,9 +592,18 @@ def main():
         _, st = lpf.lpf_anneal(pa, d_img[0], -1, target, d_pairs, torch.from_numpy(log_u).cuda(),
                                T_max, 0.01 * T_max, max(1, n // 10), max(1, n // 100))
         dt = time.perf_counter() - t0
+        # the paper's own operator: interfacial pixels of different phases, drawn on the device (lpf_anneal_generate)
+        d_img2 = torch.from_numpy(start.reshape(H, W).copy()).cuda()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        _, st2, _ = lpf.lpf_anneal_generate(pa, d_img2, -1, target, lpf.LPF_PROPOSE_INTERFACIAL, inputs.seed_for(7, 3),
+                                            torch.from_numpy(log_u).cuda(), T_max, 0.01 * T_max, max(1, n // 10),
+                                            max(1, n // 100))
+        dt2 = time.perf_counter() - t0
         lpf.lpf_free_paths(pa)
         return {"proposals": n, "seconds": dt, "proposals_per_s": n / dt, "accepted": st["accepted"],
-                "E_start": E0, "E_end": st["E"], "levels": st["levels"], "T_max": T_max}
+                "E_start": E0, "E_end": st["E"], "levels": st["levels"], "T_max": T_max,
+                "interfacial_operator": {"proposals_per_s": n / dt2, "accepted": st2["accepted"], "E_end": st2["E"]}}
 
     r = measure(w, args.steps, args.warmup, True, strong=(args.scaling == "strong"))
     if args.scaling == "strong" and not r["strong"]:

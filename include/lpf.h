@@ -191,7 +191,8 @@ int  lpf_swap_delta(const lpf_paths* p, const uint8_t* image, int H, int W, int 
  * log_u[k] < (E_P - E_Q) / ((W*H)^2 * T), E = sum over the phases and v in D of (target - counts)^2; a pair of equal
  * bytes (or out of range) is the identity move; T *= (T_min/T_max)^(s_max/N) whenever c_max proposals or s_max
  * acceptances were seen at the current temperature.  Batches of consecutive proposals are evaluated speculatively in
- * parallel (lpf_swap_delta) and decided in order on the device.
+ * parallel (the swap-delta evaluation) and decided in order on the device; the whole chain is ONE cooperative kernel
+ * launch (workspace: lpf_reserve with LPF_FOR_ANNEAL).
  *   image dev uint8 [H][W], modified in place      phase 0 | 1 | -1 (both: target/counts are [2][2m+1][2m+1])
  *   target dev int64 [n_ph][2m+1][2m+1]            pairs dev int32 [N][4], log_u dev double [N] (ln of uniforms in [0,1))
  *   counts dev int64 [n_ph][2m+1][2m+1]: descriptor of the final image      accept_log dev uint8 [N] or NULL
@@ -200,6 +201,24 @@ int  lpf_swap_delta(const lpf_paths* p, const uint8_t* image, int H, int W, int 
 int  lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase, const int64_t* target, const int32_t* pairs,
                 const double* log_u, int64_t N, double T_max, double T_min, int64_t c_max, int64_t s_max,
                 int64_t* counts, uint8_t* accept_log, double* stats5, void* stream);
+
+/* lpf_anneal with the modification operator drawing its own pixels from the current image ("two
+ * randomly chosen pixels from different phases"; "a random selection of interfacial pixels", the acceleration the paper
+ * uses).  The paper does not say how they are drawn; reading A7: proposal k, attempt t = 0..63, side s (0: p,
+ * 1: q) uses output n = 1 + 2 (64 k + t) + s of SplitMix64 seeded with `seed`; a word u gives the pixel
+ * x = ((u >> 32) * W) >> 32, y = ((u & 0xffffffff) * H) >> 32.
+ *   LPF_PROPOSE_OPPOSITE:    p = attempt 0 of side 0; q = the first attempt of side 1 whose byte differs from p's
+ *   LPF_PROPOSE_INTERFACIAL: p = the first interfacial attempt of side 0; q = the first interfacial attempt of side 1
+ *                            whose byte differs from p's (interfacial: one of the 4 periodic neighbours has another byte)
+ *   nothing qualifies: q = p, the identity move.
+ *   pairs_out dev int32 [N][4]: the proposal decided at every step (written by the device; required)
+ * Everything else as lpf_anneal (log_u stays an input: the logarithm is not bit-reproducible across libraries). */
+#define LPF_PROPOSE_OPPOSITE    1
+#define LPF_PROPOSE_INTERFACIAL 2
+int  lpf_anneal_generate(lpf_paths* p, uint8_t* image, int H, int W, int phase, const int64_t* target, int policy,
+                         uint64_t seed, int32_t* pairs_out, const double* log_u, int64_t N, double T_max, double T_min,
+                         int64_t c_max, int64_t s_max, int64_t* counts, uint8_t* accept_log, double* stats5,
+                         void* stream);
 
 /* HOST-buffer convenience used by the end-to-end measurement: copies `images` (host, pinned or
  * not) to the device on a private stream (ordered after earlier work on this table), runs lpf_eval (_both if

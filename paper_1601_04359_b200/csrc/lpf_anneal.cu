@@ -59,7 +59,10 @@ struct AnnealArgs {
   AnnealState* state;
   const uint32_t* padded;      // [n_ph] padded bit planes of the START image (lpf_swap.cuh layout)
   int H, W, m, phase, n_ph;
-  const int* pairs;            // [N][4]
+  const int* pairs;            // [N][4] the proposals (policy 0: the caller's list; else = pairs_out)
+  int* pairs_out;              // policy 1 | 2: [N][4], every proposal is written here when it is generated
+  int policy;                  // 0: list; 1: opposite bytes; 2: opposite bytes, both interfacial (reading A7)
+  unsigned long long seed;
   const double* log_u;         // [N]
   long long N;
   const int4* rec;             // swap-delta node records
@@ -77,6 +80,57 @@ struct AnnealArgs {
 };
 
 __device__ __forceinline__ long long ld_cg(const long long* p) { return __ldcg(p); }
+
+// n-th output of SplitMix64 for `seed` (Steele, Lea, Flood 2014): the counter-based generator of reading A7
+__device__ __forceinline__ unsigned long long splitmix64(unsigned long long seed, unsigned long long n) {
+  unsigned long long z = seed + n * 0x9E3779B97F4A7C15ull;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+// The modification operator drawing its own pixels from the CURRENT image (reading A7),
+// by one warp: lane t tries attempts t and t + 32 of a side, the first qualifying attempt wins (ballot).  The image
+// bytes are read with ld.global.cg: the deciding thread of an earlier batch may have exchanged two of them.
+//   policy 1: p = attempt 0 (any pixel), q = first attempt with another byte
+//   policy 2: p = first interfacial attempt, q = first interfacial attempt with another byte
+//   nothing qualifies in 64 attempts: q = p (identity move).  Every lane returns the same pair.
+__device__ __forceinline__ int4 propose_pair(const uint8_t* image, int H, int W, int policy, unsigned long long seed,
+                                             long long k, int lane) {
+  auto byte_at = [&](int x, int y) -> int { return __ldcg(image + (size_t)y * W + x); };
+  auto wrap = [](int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); };
+  int px = -1, py = -1, qx = -1, qy = -1, bp = -1;
+  for (int side = 0; side < 2; ++side) {
+    for (int round = 0; round < 2; ++round) {
+      const int t = lane + 32 * round;
+      const unsigned long long u = splitmix64(seed, 1ull + 2ull * (64ull * (unsigned long long)k + t) + side);
+      const int x = (int)(((u >> 32) * (unsigned long long)W) >> 32);
+      const int y = (int)(((u & 0xffffffffull) * (unsigned long long)H) >> 32);
+      const int b = byte_at(x, y);
+      bool ok = side == 0 || b != bp;
+      if (policy == 2 && ok)
+        ok = byte_at(wrap(x + 1, W), y) != b || byte_at(wrap(x - 1, W), y) != b || byte_at(x, wrap(y + 1, H)) != b ||
+             byte_at(x, wrap(y - 1, H)) != b;
+      if (policy == 1 && side == 0) ok = (t == 0);
+      const unsigned hit = __ballot_sync(0xffffffffu, ok);
+      if (hit) {
+        const int src = __ffs(hit) - 1;
+        const int wx = __shfl_sync(0xffffffffu, x, src), wy = __shfl_sync(0xffffffffu, y, src);
+        if (side == 0) { px = wx; py = wy; bp = __shfl_sync(0xffffffffu, b, src); }
+        else { qx = wx; qy = wy; }
+        break;
+      }
+    }
+    if (side == 0 && px < 0) {                               // no interfacial pixel met: attempt 0, identity move
+      const unsigned long long u = splitmix64(seed, 1ull + 2ull * (64ull * (unsigned long long)k));
+      px = (int)(((u >> 32) * (unsigned long long)W) >> 32);
+      py = (int)(((u & 0xffffffffull) * (unsigned long long)H) >> 32);
+      return make_int4(px, py, px, py);
+    }
+  }
+  if (qx < 0) { qx = px; qy = py; }
+  return make_int4(px, py, qx, qy);
+}
 
 // The whole chain in ONE cooperative launch (one CTA set resident on every SM, grid-wide barriers between the phases of
 // a batch): the padded bit planes of the current image stay in every CTA's shared memory and are patched after an
@@ -99,6 +153,7 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
   __shared__ long long s_dE[256];
   __shared__ double s_lu[256];
   __shared__ int s_last;
+  __shared__ int s_pair[4];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int H = a.H, W = a.W, m = a.m, n_ph = a.n_ph;
   const int PWc = (W + 2 * m + 31) >> 5, PH = H + 2 * m;
@@ -118,8 +173,26 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
     const int n_slices = max(1, min((int)gridDim.x / K, (a.n_nodes + 255) / 256));
     for (int unit = blockIdx.x; unit < K * n_slices; unit += gridDim.x) {
       const int j = unit / n_slices, slice = unit - j * n_slices;
-      swap_delta_unit(sm, stk, sh, H, W, m, a.pairs, a.N, next + j, a.rec, a.n_nodes, a.delta + (long long)j * K2, n_ph,
-                      a.ph_stride, 1, slice, n_slices);
+      if (next + j >= a.N) continue;
+      if (a.policy == 0) {
+        swap_delta_unit(sm, stk, sh, H, W, m, a.pairs, a.N, next + j, a.rec, a.n_nodes, a.delta + (long long)j * K2,
+                        n_ph, a.ph_stride, 1, slice, n_slices);
+      } else {                                               // Q = modify(P): the operator draws its pixels from P
+        __syncthreads();                                     // the previous unit is finished with s_pair
+        if (warp == 0) {
+          const int4 pr = propose_pair(a.image, H, W, a.policy, a.seed, next + j, lane);
+          if (lane == 0) {
+            s_pair[0] = pr.x; s_pair[1] = pr.y; s_pair[2] = pr.z; s_pair[3] = pr.w;
+            if (slice == 0) {                                // for the decisions and for the caller
+              int* po = a.pairs_out + 4 * (next + j);
+              po[0] = pr.x; po[1] = pr.y; po[2] = pr.z; po[3] = pr.w;
+            }
+          }
+        }
+        __syncthreads();
+        swap_delta_unit(sm, stk, sh, H, W, m, s_pair, 1, 0, a.rec, a.n_nodes, a.delta + (long long)j * K2, n_ph,
+                        a.ph_stride, 1, slice, n_slices);
+      }
     }
     grid.sync();
     // ---- (B)
@@ -200,8 +273,8 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
         st.acc_bytes[0] = st.acc_bytes[1] = 0;
         if (acc_idx >= 0) {                                     // P = Q: exchange the two bytes (reading A5)
           const long long idx = next + acc_idx;
-          const int xp = a.pairs[4 * idx], yp = a.pairs[4 * idx + 1], xq = a.pairs[4 * idx + 2],
-                    yq = a.pairs[4 * idx + 3];
+          const int xp = __ldcg(a.pairs + 4 * idx), yp = __ldcg(a.pairs + 4 * idx + 1),
+                    xq = __ldcg(a.pairs + 4 * idx + 2), yq = __ldcg(a.pairs + 4 * idx + 3);
           if (xp >= 0 && xp < W && xq >= 0 && xq < W && yp >= 0 && yp < H && yq >= 0 && yq < H) {
             volatile uint8_t* img = a.image;
             const uint8_t bp = img[(size_t)yp * W + xp], bq = img[(size_t)yq * W + xq];
@@ -274,10 +347,10 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
 
 using namespace lpf;
 
-extern "C" int lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase, const int64_t* target,
-                          const int32_t* pairs, const double* log_u, int64_t N, double T_max, double T_min,
-                          int64_t c_max, int64_t s_max, int64_t* counts, uint8_t* accept_log, double* stats5,
-                          void* stream) {
+static int anneal_impl(lpf_paths* p, uint8_t* image, int H, int W, int phase, const int64_t* target,
+                       const int32_t* pairs, int policy, uint64_t seed, int32_t* pairs_out, const double* log_u,
+                       int64_t N, double T_max, double T_min, int64_t c_max, int64_t s_max, int64_t* counts,
+                       uint8_t* accept_log, double* stats5, void* stream) {
   if (!p || !image || !target || !counts || !stats5 || (N > 0 && (!pairs || !log_u))) return LPF_E_INVAL;
   if (p->device < 0 || N < 0 || phase < -1 || phase > 1 || c_max < 1 || s_max < 1) return LPF_E_INVAL;
   if (!(T_max > 0.0) || !(T_min > 0.0)) return LPF_E_INVAL;
@@ -337,7 +410,7 @@ extern "C" int lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase,
     if (e == cudaSuccess && rc == LPF_OK) {
       AnnealArgs a;
       a.state = d_state; a.padded = padded; a.H = H; a.W = W; a.m = p->m; a.phase = phase; a.n_ph = n_ph;
-      a.pairs = pairs; a.log_u = log_u; a.N = N; a.rec = (const int4*)p->d_swap_rec; a.n_nodes = (int)p->n_trie_nodes;
+      a.pairs = pairs; a.pairs_out = pairs_out; a.policy = policy; a.seed = seed; a.log_u = log_u; a.N = N; a.rec = (const int4*)p->d_swap_rec; a.n_nodes = (int)p->n_trie_nodes;
       a.delta = d_delta; a.ph_stride = ph_stride; a.K_max = K_max; a.dE = d_dE; a.counts = (long long*)counts;
       a.target = (const long long*)target; a.image = image; a.accept_log = accept_log; a.wh2 = wh2; a.T_mult = T_mult;
       a.c_max = c_max; a.s_max = s_max;
@@ -359,4 +432,22 @@ extern "C" int lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase,
   if (rc != LPF_OK) return rc;
   if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? LPF_E_NOMEM : LPF_E_CUDA;
   return LPF_OK;
+}
+
+extern "C" int lpf_anneal(lpf_paths* p, uint8_t* image, int H, int W, int phase, const int64_t* target,
+                          const int32_t* pairs, const double* log_u, int64_t N, double T_max, double T_min,
+                          int64_t c_max, int64_t s_max, int64_t* counts, uint8_t* accept_log, double* stats5,
+                          void* stream) {
+  return anneal_impl(p, image, H, W, phase, target, pairs, 0, 0, nullptr, log_u, N, T_max, T_min, c_max, s_max, counts,
+                     accept_log, stats5, stream);
+}
+
+extern "C" int lpf_anneal_generate(lpf_paths* p, uint8_t* image, int H, int W, int phase, const int64_t* target,
+                                   int policy, uint64_t seed, int32_t* pairs_out, const double* log_u, int64_t N,
+                                   double T_max, double T_min, int64_t c_max, int64_t s_max, int64_t* counts,
+                                   uint8_t* accept_log, double* stats5, void* stream) {
+  if (policy != LPF_PROPOSE_OPPOSITE && policy != LPF_PROPOSE_INTERFACIAL) return LPF_E_INVAL;
+  if (N > 0 && !pairs_out) return LPF_E_INVAL;
+  return anneal_impl(p, image, H, W, phase, target, pairs_out, policy, seed, pairs_out, log_u, N, T_max, T_min, c_max,
+                     s_max, counts, accept_log, stats5, stream);
 }

@@ -53,7 +53,7 @@ __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, S
                                                 int n_planes, long long plane_stride, int sw, int slice,
                                                 int n_slices) {
   const int PWc = (W + 2 * m + 31) >> 5, PH = H + 2 * m;                // padded bit image: halo of m pixels all round
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31;
   const int plane_words = PH * PWc;
   // pixel (x, y) of the plane at Pq, x in [-m, W + m), y in [-m, H + m)
   auto pbit = [&](const uint32_t* Pq, int x, int y) -> unsigned {

@@ -22,7 +22,9 @@ EXPORTS = (
     "lpf_paths_get", "lpf_paths_program", "lpf_eval", "lpf_eval_both", "lpf_objective",
     "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
     "lpf_set_tile", "lpf_alu_peak", "lpf_eval_masked", "lpf_anneal", "lpf_reserve", "lpf_eval_sum",
+    "lpf_anneal_generate",
 )
+LPF_PROPOSE_OPPOSITE, LPF_PROPOSE_INTERFACIAL = 1, 2
 LPF_FOR_EVAL, LPF_FOR_EVAL_BOTH, LPF_FOR_MASKED, LPF_FOR_SWAP_DELTA, LPF_FOR_ANNEAL, LPF_FOR_HOST = 1, 2, 4, 8, 16, 32
 
 _lib = None
@@ -75,6 +77,9 @@ def load() -> ctypes.CDLL:
     lib.lpf_anneal.argtypes = [VP, VP, I, I, I, VP, VP, VP, I64, ctypes.c_double, ctypes.c_double, I64, I64, VP, VP,
                                ctypes.POINTER(ctypes.c_double), VP]
     lib.lpf_anneal.restype = I
+    lib.lpf_anneal_generate.argtypes = [VP, VP, I, I, I, VP, I, ctypes.c_uint64, VP, VP, I64, ctypes.c_double,
+                                        ctypes.c_double, I64, I64, VP, VP, ctypes.POINTER(ctypes.c_double), VP]
+    lib.lpf_anneal_generate.restype = I
     lib.lpf_objective.argtypes = [VP, VP, I, I64, VP, VP]
     lib.lpf_objective.restype = I
     lib.lpf_swap_delta.argtypes = [VP, VP, I, I, I, VP, I64, VP, VP]
@@ -311,6 +316,36 @@ def lpf_anneal(p: Paths, image, phase: int, target, pairs, log_u, T_max: float, 
                           _stream_ptr(stream, target, pairs, log_u)), "lpf_anneal")
     keys = ("steps", "accepted", "levels", "T", "E")
     return counts, dict(zip(keys, [float(v) for v in stats]))
+
+
+def lpf_anneal_generate(p: Paths, image, phase: int, target, policy: int, seed: int, log_u, T_max: float, T_min: float,
+                        c_max: int, s_max: int, accept_log=None, stream=None):
+    """Alg. 3 with the modification operator drawing its own pixels (LPF_PROPOSE_OPPOSITE / LPF_PROPOSE_INTERFACIAL).
+    Returns (counts int64 [n_ph, S, S], stats, pairs int32 [N, 4]: the proposal decided at every step)."""
+    torch = _torch()
+    lib = load()
+    assert image.is_cuda and image.dtype == torch.uint8 and image.dim() == 2 and image.is_contiguous()
+    _on_device(p, image, target, log_u, accept_log)
+    H, W = image.shape
+    S = 2 * p.m + 1
+    n_ph = 2 if phase < 0 else 1
+    target = target.contiguous()
+    log_u = log_u.contiguous()
+    N = log_u.numel()
+    assert target.is_cuda and target.dtype == torch.int64 and target.numel() == n_ph * S * S
+    assert log_u.is_cuda and log_u.dtype == torch.float64
+    if accept_log is not None:
+        assert accept_log.is_cuda and accept_log.dtype == torch.uint8 and accept_log.numel() == N
+    counts = torch.empty((n_ph, S, S), dtype=torch.int64, device=image.device)
+    pairs = torch.zeros((max(N, 1), 4), dtype=torch.int32, device=image.device)
+    stats = (ctypes.c_double * 5)()
+    _check(lib.lpf_anneal_generate(p.handle, image.data_ptr(), H, W, int(phase), target.data_ptr(), int(policy),
+                                   int(seed) & (2 ** 64 - 1), pairs.data_ptr(), log_u.data_ptr(), N, float(T_max),
+                                   float(T_min), int(c_max), int(s_max), counts.data_ptr(),
+                                   accept_log.data_ptr() if accept_log is not None else None, stats,
+                                   _stream_ptr(stream, target, log_u)), "lpf_anneal_generate")
+    keys = ("steps", "accepted", "levels", "T", "E")
+    return counts, dict(zip(keys, [float(v) for v in stats])), pairs[:N]
 
 
 def lpf_objective(counts, target, out=None, stream=None):

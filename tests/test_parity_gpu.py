@@ -457,6 +457,28 @@ def test_anneal_chain_is_decision_for_decision_the_oracles(H, W, m, phase, N, c_
     assert 0 < w_log.sum() < N
 
 
+@pytest.mark.parametrize("H,W,m,phase,policy,N", [(24, 40, 11, 1, 1, 500), (33, 31, 16, -1, 2, 400),
+                                                   (20, 26, 9, 0, 2, 600), (100, 100, 20, -1, 2, 300)])
+def test_anneal_with_generated_proposals_is_the_oracles_chain(H, W, m, phase, policy, N):
+    """lpf_anneal_generate: the modification operator draws its own pixels from the current image on the device
+    (opposite phases / interfacial, reading A7): proposals, decisions, final image, descriptor and statistics are the
+    oracle's."""
+    start, target, _, log_u, E0 = _anneal_case(H, W, m, phase, 300 + H, N)
+    T_max = 2.0 * E0 / (H * W) ** 2 / 50
+    c_max, s_max = max(1, N // 10), max(1, N // 40)
+    w_img, w_counts, w_st, w_log, w_pairs = orc.anneal_generate(start, phase, m, target, policy, 777, log_u, T_max,
+                                                               0.01 * T_max, c_max, s_max, use_local=True)
+    d_img = dev(start)
+    d_log = torch.zeros(N, dtype=torch.uint8, device="cuda")
+    counts, st, pairs = lpf.lpf_anneal_generate(paths(m), d_img, phase, dev(target), policy, 777, dev(log_u), T_max,
+                                                0.01 * T_max, c_max, s_max, accept_log=d_log)
+    assert np.array_equal(pairs.cpu().numpy(), w_pairs)
+    assert np.array_equal(d_log.cpu().numpy(), w_log)
+    assert np.array_equal(d_img.cpu().numpy(), w_img)
+    assert np.array_equal(counts.cpu().numpy(), w_counts)
+    assert st == w_st and 0 < w_log.sum() < N
+
+
 def test_anneal_limits_and_identity_moves():
     H, W, m, N = 16, 16, 7, 200
     start, target, pairs, log_u, _ = _anneal_case(H, W, m, 1, 77, N)
