@@ -337,6 +337,8 @@ def main():
                          "gpurun_out/fig7.{json,md}")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the secondary workloads in the same JSON line")
+    ap.add_argument("--leg", default="", choices=["", "cfg5", "anneal", "s2", "ensemble"],
+                    help="run ONE secondary leg alone and print its JSON (used for the ncu captures under profiles/)")
     ap.add_argument("--tab1", action="store_true",
                     help="also run the Tab. 1-shaped size study (chess / 4x4 squares, 10..500 px, m = size - 1) and "
                          "write gpurun_out/tab1.{json,md}")
@@ -605,6 +607,11 @@ def main():
                 "E_start": E0, "E_end": st["E"], "levels": st["levels"], "T_max": T_max,
                 "interfacial_operator": {"proposals_per_s": n / dt2, "accepted": st2["accepted"], "E_end": st2["E"]}}
 
+    if args.leg:
+        out = {"cfg5": measure_swaps, "anneal": measure_anneal, "ensemble": measure_ensemble,
+               "s2": lambda: {"cfg2": measure_s2("cfg2"), "cfg3": measure_s2("cfg3")}}[args.leg]()
+        print(json.dumps({"leg": args.leg, "result": out}))
+        return
     r = measure(w, args.steps, args.warmup, True, strong=(args.scaling == "strong"))
     if args.scaling == "strong" and not r["strong"]:
         args.scaling = "weak"                             # one rank, or a workload with fewer images than ranks
