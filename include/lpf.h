@@ -253,6 +253,13 @@ int  lpf_alu_peak(int device, double* out4);
  * following lpf_eval calls on this object; 0 = automatic choice.  Never changes a count.  INVAL otherwise. */
 int  lpf_set_tile(lpf_paths* p, int tx, int ty, int cta_warps);
 
+/* Tuning hook: a CTA of the eval kernel is n_teams teams that share the row bands it holds in
+ * shared memory; every team walks its own work unit (the segments are distributed, the image is shared).
+ * n_teams = 1..32 fixes the number for the following lpf_reserve / lpf_eval calls on this object (shapes whose CTA would
+ * exceed 1024 threads are refused, LPF_E_UNSUPPORTED), 0 = automatic (the count that keeps the most warps resident).
+ * Never changes a count.  INVAL otherwise. */
+int  lpf_set_teams(lpf_paths* p, int n_teams);
+
 #ifdef __cplusplus
 }
 #endif

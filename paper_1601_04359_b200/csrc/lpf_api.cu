@@ -188,7 +188,8 @@ cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W
 
 static std::array<int64_t, 8> plan_key(const lpf_paths* p, int B, int H, int W, int n_phase, unsigned flags,
                                        bool masked) {
-  return {B, H, W, n_phase, (int64_t)flags, masked ? 1 : 0, 100 * p->tile_tx + p->tile_ty, p->cta_warps};
+  return {B, H, W, n_phase, (int64_t)flags, masked ? 1 : 0, 100 * p->tile_tx + p->tile_ty,
+          p->cta_warps + 100 * p->n_teams};
 }
 
 static int check_eval_args(const lpf_paths* p, int B, int H, int W, unsigned flags) {
@@ -222,11 +223,33 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   work_per_item = std::max(1, work_per_item / 4);
   pl.n_gp = (pl.Bpad / g.G) * n_phase;
 
-  // work items: about 20 per resident CTA (measured optimum on configs 2-4), pieces of 256 .. 16384 trie nodes
-  const int resident_guess = p->n_sm * 2;
+  DeviceGuard dg(p->device);
+  if (!dg.ok) return LPF_E_CUDA;
+  // teams per CTA: a CTA of NT teams shares its bands in shared memory, every team walks its own work unit.  Shared
+  // memory per CTA does not grow with NT, so NT is the one that keeps the most warps resident (fewest teams on a tie).
+  pl.prune = (flags & LPF_PRUNE) ? 1 : 0;
+  pl.smem = (size_t)g.smem_bytes;
+  int occ = 0;
+  {
+    int best_warps = 0;
+    g.NT = 1;
+    for (int nt = 1; nt * g.threads <= EVAL_CTA_MAX_THREADS; ++nt) {
+      if (p->n_teams > 0 && nt != p->n_teams) continue;
+      int o_nt = 0;
+      LPF_CUDA(eval_occupancy(g.TX, g.TY, pl.prune != 0, nt * g.threads, pl.smem, p->max_smem, &o_nt));
+      const int warps = o_nt * nt * (g.threads / 32);
+      if (warps > best_warps) { best_warps = warps; g.NT = nt; occ = o_nt; }
+    }
+    if (best_warps < 1) return LPF_E_UNSUPPORTED;
+  }
+
+  // work units: about 20 chunks of NT units per resident CTA (measured optimum on configs 2-4), pieces of
+  // 256 .. 16384 trie nodes, and at least 2 NT pieces per octant so that the teams of a CTA find work on one band
+  const int resident_guess = p->n_sm * std::max(occ, 1);
   long long n_nodes = 0;
   for (int o = 0; o < 4; ++o) n_nodes += (long long)p->oct[o].size();
-  const long long want_items = std::max<long long>(1, 32ll * resident_guess / ((long long)pl.n_gp * work_per_item));
+  const long long want_items =
+      std::max<long long>({1, 20ll * g.NT * resident_guess / ((long long)pl.n_gp * work_per_item), 8ll * g.NT});
   long long piece = n_nodes / want_items;
   piece = std::max<long long>(256, std::min<long long>(piece, 16384));
   int q = 256;
@@ -247,27 +270,40 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
     if (q <= 64) return LPF_E_UNSUPPORTED;
   }
   if (pr->entries.size() >= (size_t)1 << 30) return LPF_E_UNSUPPORTED;
-  DeviceGuard dg(p->device);
-  if (!dg.ok) return LPF_E_CUDA;
   int rc = upload_program(*pr);
   if (rc != LPF_OK) return rc;
   pl.pr = pr;
 
-  // the work list: items expanded over (row band, strip band) of their octant, big items first
+  // the work list: items expanded over the strip bands of their octant are the units of one (octant, row band); the
+  // units of a key, big first, are cut into chunks of NT (the last one padded with empty units), big chunks first
   std::vector<int32_t> work;
-  const size_t n_items = pr->items.size() / 4;
-  for (size_t i = 0; i < n_items; ++i) {
-    const int o = (int)pr->items[4 * i + 2];
-    const int sb = (g.v[o].n_strips + g.SB - 1) / g.SB;
-    for (int band = 0; band < g.v[o].n_bands; ++band)
-      for (int s = 0; s < sb; ++s) {
-        work.push_back((int32_t)pr->items[4 * i]);
-        work.push_back((int32_t)pr->items[4 * i + 1]);
-        work.push_back(o | (s << 4));
-        work.push_back(band);
+  {
+    const size_t n_items = pr->items.size() / 4;
+    std::vector<std::array<int32_t, 4>> chunks_first;      // first unit of every chunk (sort key) + position
+    std::vector<std::array<int32_t, 4>> units, all;
+    for (int o = 0; o < 4; ++o)
+      for (int band = 0; band < g.v[o].n_bands; ++band) {
+        units.clear();
+        const int sb = (g.v[o].n_strips + g.SB - 1) / g.SB;
+        for (size_t i = 0; i < n_items; ++i) {             // items are sorted by size, descending
+          if ((int)pr->items[4 * i + 2] != o) continue;
+          for (int s = 0; s < sb; ++s)
+            units.push_back({(int32_t)pr->items[4 * i], (int32_t)pr->items[4 * i + 1], o | (s << 4), band});
+        }
+        while (units.size() % (size_t)g.NT) units.push_back({0, 0, o, band});
+        for (size_t u = 0; u < units.size(); u += (size_t)g.NT) {
+          chunks_first.push_back({units[u][1], (int32_t)(all.size() / (size_t)g.NT), 0, 0});
+          for (int t = 0; t < g.NT; ++t) all.push_back(units[u + t]);
+        }
       }
+    std::stable_sort(chunks_first.begin(), chunks_first.end(),
+                     [](const std::array<int32_t, 4>& a, const std::array<int32_t, 4>& b) { return a[0] > b[0]; });
+    for (const auto& c : chunks_first)
+      for (int t = 0; t < g.NT; ++t)
+        for (int k = 0; k < 4; ++k) work.push_back(all[(size_t)c[1] * g.NT + t][k]);
   }
-  pl.n_work = (int64_t)work.size() / 4;
+  pl.n_chunks = (int64_t)work.size() / 4 / g.NT;
+  const size_t n_items = pr->items.size() / 4;
   // the walker's loop replayed on the host (eval_kernel_v3: chunks of 32 entries, a PAIR entry that is not the last of
   // its chunk is folded with its successor): the data operations the design executes per start word
   pl.piece_nodes = q;
@@ -289,14 +325,8 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
     }
     if ((uint32_t)(pr->entries[first] >> 32) & E_ROOTCOUNT_HI) ++pl.terminals;
   }
-  const long long total_work = (long long)pl.n_work * pl.n_gp;
+  const long long total_work = (long long)pl.n_chunks * pl.n_gp;
   if (total_work >= (1ll << 32)) return LPF_E_UNSUPPORTED;
-
-  pl.prune = (flags & LPF_PRUNE) ? 1 : 0;
-  pl.smem = (size_t)g.smem_bytes;
-  int occ = 0;
-  LPF_CUDA(eval_occupancy(g.TX, g.TY, pl.prune != 0, g.threads, pl.smem, p->max_smem, &occ));
-  if (occ < 1) return LPF_E_UNSUPPORTED;
   pl.grid = (int)std::min<long long>(total_work, (long long)p->n_sm * occ);
 
   // workspace: the packed octant views, then the compact row-major / column-major bit images of stage 1, then (for
@@ -437,7 +467,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   ep.entries = (const uint2*)pl.pr->d_entries;
   ep.skip = pl.pr->d_skip;
   ep.work = (const int4*)pl.d_work;
-  ep.n_work = (int)pl.n_work;
+  ep.n_chunks = (int)pl.n_chunks;
   ep.n_gp = pl.n_gp;
   ep.B = B;
   ep.n_phase = n_phase;
@@ -453,7 +483,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   for (int o = 0; o < 4; ++o) ep.mask_off[o] = pl.gm.v[o].packed_off;
   const bool timed = p->timing && !order.capturing;
   if (timed) LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_start, st));
-  LPF_CUDA(launch_eval(ep, pl.grid, pl.g.threads, pl.smem, st));
+  LPF_CUDA(launch_eval(ep, pl.grid, pl.g.NT * pl.g.threads, pl.smem, st));
   if (timed) {
     LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_stop, st));
     p->timed_once = 1;
@@ -462,10 +492,10 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   LPF_CUDA(order.done());
 
   p->last_info[0] = start_mask ? 6 : 4;                  // kernels launched (pack base, pack views, eval, mirror)
-  p->last_info[1] = (long long)pl.n_work * pl.n_gp;
+  p->last_info[1] = (long long)pl.n_chunks * pl.n_gp;    // chunks of NT work units x (image group, phase plane)
   p->last_info[2] = (int64_t)pl.pr->entries.size();      // program entries (all four octants)
   p->last_info[3] = pl.grid;
-  p->last_info[4] = pl.g.threads;
+  p->last_info[4] = pl.g.NT * pl.g.threads;              // CTA = NT teams
   p->last_info[5] = (int64_t)pl.smem;
   p->last_info[6] = pl.g.TX * 1000 + pl.g.TY * 100 + pl.pr->n_slots;   // thread tile TX, TY and mask-stack slots
   p->last_info[7] = pl.g.G;
@@ -547,6 +577,12 @@ extern "C" int lpf_set_tile(lpf_paths* p, int tx, int ty, int cta_warps) {
                      (tx == 8 && ty == 2) || (tx == 16 && ty == 1);
   if (!known || cta_warps < 0 || cta_warps > 8) return LPF_E_INVAL;
   p->tile_tx = tx; p->tile_ty = ty; p->cta_warps = cta_warps;
+  return LPF_OK;
+}
+
+extern "C" int lpf_set_teams(lpf_paths* p, int n_teams) {
+  if (!p || n_teams < 0 || n_teams > EVAL_CTA_MAX_THREADS / 32) return LPF_E_INVAL;
+  p->n_teams = n_teams;
   return LPF_OK;
 }
 

@@ -110,8 +110,8 @@ struct EvalPlan {
   Geom g;                              // views with their offsets inside one phase plane of the packed workspace
   Geom gm;                             // the same views for the start mask of lpf_eval_masked (one image, one plane)
   Program* pr = nullptr;
-  int32_t* d_work = nullptr;           // [n_work][4] = first entry, count, octant | strip band << 4, row band; big first
-  int64_t n_work = 0;
+  int32_t* d_work = nullptr;           // [n_chunks][NT][4] = first entry, count, octant | strip band << 4, row band
+  int64_t n_chunks = 0;
   int Bpad = 0, n_gp = 0, grid = 0, prune = 0;
   size_t smem = 0;
   size_t views_bytes = 0, base_words = 0, mask_views_bytes = 0, mask_base_bytes = 0, need = 0;
@@ -162,6 +162,7 @@ struct lpf_paths {
   void* io_stream = nullptr;
   // lpf_set_timing: CUDA events recorded around the eval kernel alone
   int tile_tx = 0, tile_ty = 0, cta_warps = 0;   // lpf_set_tile overrides (0 = automatic)
+  int n_teams = 0;                   // teams per CTA override (0 = automatic)
   int timing = 0;
   int timed_once = 0;                // a timed eval has been issued: ev_start / ev_stop hold a measurement
   void* ev_start = nullptr;

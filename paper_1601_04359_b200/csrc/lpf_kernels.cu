@@ -17,6 +17,7 @@
 
 namespace lpf {
 
+
 // ---------------------------------------------------------------------------------------------
 // bit-pack, stage 1: uint8 image -> two compact bit images per phase plane, from ONE coalesced pass.
 //   One warp per 32 x 32 pixel tile: lane k reads byte (y0 + j, x0 + k) for j = 0..31 (32 coalesced row
@@ -231,8 +232,13 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, unsigne
 //   window then covers two path pixels.  PAIR entries fold their window into the next entry's 3-input AND.
 //   The mask of an item is initialised once, before the loop (INIT is only ever an item's first entry).
 // ---------------------------------------------------------------------------------------------
+// 64 registers per thread: CTAs of up to 1024 threads, 32 warps resident per SM (measured against 72 registers and 24
+// warps: config 3 5.33 vs 5.38 ms, config 4 3.67 vs 3.76 ms; the few spilled words sit next to the mask stack in L1)
+#ifndef LPF_EVAL_ATTR
+#define LPF_EVAL_ATTR __maxnreg__(64)
+#endif
 template <int TX, int TY, bool PRUNE>
-__global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
+__global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
   constexpr int T = TX * TY;
   constexpr unsigned FULL = 0xffffffffu;
   extern __shared__ __align__(128) uint32_t smem[];
@@ -240,9 +246,13 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
   __shared__ unsigned int s_work;
 
   const Geom& g = p.g;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int img_local = warp / g.wpi;
-  const int ww = warp - img_local * g.wpi;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // provably warp-uniform: the team's unit stays in uniform registers
+  const int team_warps = g.G * g.wpi;
+  const int team = warp / team_warps;                   // teams walk different items on the same bands
+  const int wteam = warp - team * team_warps;
+  const int img_local = wteam / g.wpi;
+  const int ww = wteam - img_local * g.wpi;
   const int strip_l = ww % g.SB, rblk = ww / g.SB;
   const int row0 = rblk * 32 * TY + lane;               // band-local start row of ty = 0
   uint32_t stk[STACK_SLOTS_BUDGET * T];
@@ -256,7 +266,7 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
   }
   __syncthreads();
   unsigned parity = 0;
-  const unsigned total_work = (unsigned)p.n_work * (unsigned)p.n_gp;
+  const unsigned total_work = (unsigned)p.n_chunks * (unsigned)p.n_gp;
   const int groups_per_plane = p.Bpad / g.G;
 
   for (;;) {
@@ -264,11 +274,11 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
     __syncthreads();                 // everybody is also done reading the previous band
     const unsigned work = s_work;
     if (work >= total_work) break;
-    const int wi = (int)(work / (unsigned)p.n_gp);          // big items first, over all groups
-    const int gp = (int)(work - (unsigned)wi * (unsigned)p.n_gp);
+    const int ci = (int)(work / (unsigned)p.n_gp);          // big chunks first, over all groups
+    const int gp = (int)(work - (unsigned)ci * (unsigned)p.n_gp);
     const int plane = gp / groups_per_plane;
     const int b0 = (gp - plane * groups_per_plane) * g.G;
-    const int4 wk = __ldg(p.work + wi);
+    const int4 wk = __ldg(p.work + (size_t)ci * g.NT + team);   // the units of a chunk share octant and row band
     const int o = wk.z & 15, sband = wk.z >> 4, band = wk.w;
     const ViewGeom& v = g.v[o];
     const int stride = v.stride;
@@ -300,6 +310,7 @@ __global__ void __launch_bounds__(256) eval_kernel_v3(const EvalParams p) {
     parity ^= 1u;
     __syncthreads();                 // s_work may be rewritten only after everyone has read it
 
+    if (wk.y == 0) continue;         // padding unit of a partial chunk: this team idles (the band is still shared)
     int e = wk.x;
     const int e1 = e + wk.y;
     uint2 cur = __ldg(p.entries + e + lane);                 // the entry array is padded by 64

@@ -30,7 +30,8 @@ struct Geom {
   int SB;            // strips per work item (<= 8)
   int wpi;           // warps per image band = SB * band_rows / (32 TY)
   int G;             // images per CTA
-  int threads;       // G * wpi * 32
+  int NT;            // teams per CTA: every team (G * wpi warps) walks its own work unit on the CTA's shared bands
+  int threads;       // threads of one team: G * wpi * 32 (the CTA has NT times as many)
   int smem_bytes;    // G * max band_words * 4
   ViewGeom v[4];
   long long plane_words;  // words of one phase plane: Bpad * sum_o view_words
@@ -38,6 +39,7 @@ struct Geom {
 
 // host: pick the geometry for (m, H, W, B); false if one band does not fit in shared memory
 //   tx, ty > 0 override the thread tile; cta_warps (1..8) the warps per CTA
+constexpr int EVAL_CTA_MAX_THREADS = 1024;  // a CTA of NT teams (the eval kernel is compiled for 64 registers per thread)
 constexpr int STACK_SLOTS_BUDGET = 8;   // mask-stack slots per thread (local memory, T words each)
 //   use_e2: eroded mode allowed: shared memory holds E2 = pixel & right neighbour and D2 = pixel & lower-right
 //   neighbour instead of the plain plane
@@ -47,8 +49,9 @@ struct EvalParams {
   Geom g;
   const uint2* entries;
   const uint32_t* skip;
-  const int4* work;           // [n_work] = first entry, count, octant | strip band << 4, row band; big first
-  int n_work;
+  const int4* work;           // [n_chunks][NT] units = first entry, count (0: padding), octant | strip band << 4,
+                              // row band; the NT units of a chunk share octant and row band; big chunks first
+  int n_chunks;
   int n_gp;                   // ceil(B / G) * n_phase (image group x phase plane)
   int B;
   int n_phase;                // 1 or 2 phase planes in `packed`

@@ -22,7 +22,7 @@ EXPORTS = (
     "lpf_paths_get", "lpf_paths_program", "lpf_eval", "lpf_eval_both", "lpf_objective",
     "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
     "lpf_set_tile", "lpf_alu_peak", "lpf_eval_masked", "lpf_anneal", "lpf_reserve", "lpf_eval_sum",
-    "lpf_anneal_generate",
+    "lpf_anneal_generate", "lpf_set_teams",
 )
 LPF_PROPOSE_OPPOSITE, LPF_PROPOSE_INTERFACIAL = 1, 2
 LPF_FOR_EVAL, LPF_FOR_EVAL_BOTH, LPF_FOR_MASKED, LPF_FOR_SWAP_DELTA, LPF_FOR_ANNEAL, LPF_FOR_HOST = 1, 2, 4, 8, 16, 32
@@ -96,6 +96,8 @@ def load() -> ctypes.CDLL:
     lib.lpf_alu_peak.restype = I
     lib.lpf_set_tile.argtypes = [VP, I, I, I]
     lib.lpf_set_tile.restype = I
+    lib.lpf_set_teams.argtypes = [VP, I]
+    lib.lpf_set_teams.restype = I
     _lib = lib
     return lib
 
@@ -433,6 +435,10 @@ def lpf_alu_peak(device: int = 0) -> dict:
 def lpf_set_tile(p: Paths, tx: int = 0, ty: int = 0, cta_warps: int = 0) -> None:
     """Tuning hook: thread tile (TX words x TY rows) and warps per CTA of the eval kernel; 0 = automatic."""
     _check(load().lpf_set_tile(p.handle, int(tx), int(ty), int(cta_warps)), "lpf_set_tile")
+
+
+def lpf_set_teams(p: Paths, n_teams: int = 0) -> None:
+    _check(load().lpf_set_teams(p.handle, int(n_teams)), "lpf_set_teams")
 
 
 def lpf_last_eval_kernel_ms(p: Paths) -> float:
