@@ -62,8 +62,8 @@ extern "C" {
                              (PAPER.md:99); same kernels, a program of 2-pixel "paths".  Exact integers (the paper's
                              FFT form, Eq. 7, is floating point). */
 
-#define LPF_NO_E2    8u   /* measurement: walk every node on the plain bit plane instead of the two eroded planes
-                             (pixel & right neighbour, pixel & lower-right neighbour).
+#define LPF_NO_E2    8u   /* measurement: walk every node on the plain bit plane instead of the eroded planes (one
+                             plane per K-step pattern of a path, K + 1 pixels per window).
                              Same counts. */
 
 /* `what` of lpf_reserve */
@@ -104,18 +104,19 @@ int  lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, int cap, int
  * into connected pieces of about `piece_nodes` nodes (<= 0: one piece per octant); each piece is one item =
  * the chain from the root to the piece root followed by the piece in depth-first order.  flags: 0, LPF_NO_TRIE, LPF_S2, LPF_NO_E2.
  *   entries  host [cap_entries] uint64 (may be NULL to query sizes); low word: bits 0-4 a' & 31, bit 5 reload,
- *            6 terminal, 7 save, 8 restore, 9 init, 10 pair (own mask never needed, next entry is the direct child),
- *            bits 12-31 b' * stride + (a' >> 5); high word: bits 0-19
- *            (dy+m)*(2m+1) + (dx+m) in IMAGE coordinates, 20-23 restore slot, 24-27 save slot
+ *            6 terminal, 7 save, 8 restore, 9 init, 10 pair (own mask never needed, the next entry continues from it),
+ *            bits 12-31 b' * stride + (a' >> 5) (+ q * band_words); high word: bits 0-19
+ *            (dy+m)*(2m+1) + (dx+m) in IMAGE coordinates, 20-22 restore slot, 23-25 save slot, 26-28 q, 29-30 back.
+ *            bit 11: the window is read from an eroded plane (program of level K >= 1: every entry).  Plane q holds,
+ *            at (a', b'), the AND of the K + 1 pixels (a' + j, b' + s_1 + .. + s_j), j = 0..K, s_j = bit j-1 of q --
+ *            K + 1 consecutive pixels of a first-octant path.  The first `back` of them are nodes that are already in
+ *            the mask, the others are the nodes of this entry; terminal / save / count index are the last one's.
+ *            At level K no window ends above depth K: every item starts (its first and only init entry) with the
+ *            window root .. depth K, and the vectors shorter than that are counted by a separate small kernel.
  *   items    host [cap_items][4] int64 = (first entry, number of entries, octant, 0) (may be NULL)
- *            bit 11: the window is read from an eroded plane (eroded program: every entry).  High word bit 29 chooses
- *            D2 = pixel & lower-right neighbour (else E2 = pixel & right neighbour); the window then covers TWO path
- *            pixels: the entry's node and its only child (terminal / save / count index are the child's), or, with
- *            high word bit 28, the node's parent -- already in the mask -- and the node.  The eroded program has no
- *            entry for the root: the kernel starts every item (its first and only INIT entry) from the plain word of
- *            the start pixels, and counts v = 0 at the INIT entry that carries high word bit 30.
- *   strides  host int[8]: [0..3] words per packed row of each octant view (decodes b', a' >> 5), [4..7] word offset
- *            of the D2 plane of each view in shared memory (E2 sits at 0; all 0 for the plain program)
+ *   strides  host int[9]: [0..3] words per packed row of each octant view (decodes b', a' >> 5), [4..7] words of one
+ *            eroded band of each view in shared memory (plane q sits at q times that; 0 for the plain program),
+ *            [8] the level K of the program (0: plain)
  * *n_entries / *n_items / *n_slots (mask-stack slots the program needs) are always written.
  * Octants (view coordinates a', b' from image coordinates a, b): 0: dx>=0, dy<=dx (a,b); 1: dx>=0, dy>dx (b,a);
  * 2: dx<0, dy>-dx (b,-a); 3: dx<0, dy<=-dx (-a,b). */
@@ -227,13 +228,14 @@ int  lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, int H, int W
                    int64_t* counts_host, unsigned flags);
 
 /* Counters of the most recent lpf_eval / lpf_eval_both on this object (host values known at
- * launch time): kernels launched, work items, program entries walked per image-phase, grid,
- * block, dynamic shared memory bytes, thread tile code (1000 TX + 100 TY + mask-stack slots), images per CTA,
- * 1 if the eroded planes E2 / D2 were walked (0: the plain plane); then what the walker executes per image-phase and
+ * launch time): kernels launched, work chunks (NT units each) x (image group, phase), program entries walked per
+ * image-phase, grid, block, dynamic shared memory bytes, thread tile code (1000 TX + 100 TY + mask-stack slots), images
+ * per team, the erosion level K of the program (0: the plain plane); then what the walker executes per image-phase and
  * per start WORD, counted by replaying its loop over the program on the host: pairs of entries folded into one
  * 3-input AND (2 SHF + 1 LOP3 each), entries executed on their own (1 SHF + 1 LOP3), terminal entries (1 POPC +
- * 1 add), and the trie nodes per program piece.  out = host int64[13]. */
-int  lpf_last_launch_info(const lpf_paths* p, int64_t* out13);
+ * 1 add), the trie nodes per program piece; the teams per CTA, the CTAs resident per SM, and the vectors shorter than K
+ * that the small extra kernel counts.  out = host int64[16]. */
+int  lpf_last_launch_info(const lpf_paths* p, int64_t* out16);
 
 /* Measurement hook: with enable != 0 every lpf_eval / lpf_eval_both on this object
  * records one CUDA event before and one after the eval kernel (the dominant kernel) on the caller's
@@ -252,6 +254,12 @@ int  lpf_alu_peak(int device, double* out4);
  * TY start rows per thread, (TX,TY) in {(4,2),(8,1),(4,4),(8,2),(16,1)}, and the warps per CTA (1..8) -- for the
  * following lpf_eval calls on this object; 0 = automatic choice.  Never changes a count.  INVAL otherwise. */
 int  lpf_set_tile(lpf_paths* p, int tx, int ty, int cta_warps);
+
+/* Tuning hook: caps the erosion level of the programs built for the following
+ * lpf_reserve / lpf_eval / lpf_paths_program calls on this object: 0..3, or -1 = automatic (the default).  Level K
+ * keeps 2^K planes per row band in shared memory; the highest level that fits and keeps enough warps resident is the
+ * fastest.  LPF_NO_E2 is level 0.  Never changes a count.  INVAL otherwise. */
+int  lpf_set_level(lpf_paths* p, int max_level);
 
 /* Tuning hook: a CTA of the eval kernel is n_teams teams that share the row bands it holds in
  * shared memory; every team walks its own work unit (the segments are distributed, the image is shared).

@@ -178,6 +178,7 @@ cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed,
                         int n_phase, int phase0, unsigned int* counter, int n_sm, cudaStream_t st);
 cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem, int max_smem, int* blocks_per_sm);
 cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st);
+cudaError_t launch_shallow(const EvalParams& p, const ShallowList& sl, cudaStream_t st);
 cudaError_t launch_mirror(unsigned long long* counts, int S, long long n_arrays, int n_sm, cudaStream_t st);
 cudaError_t launch_objective(const long long* counts, const long long* target, int B, long long K,
                              unsigned long long* sse, int n_sm, cudaStream_t st);
@@ -189,7 +190,7 @@ cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W
 static std::array<int64_t, 8> plan_key(const lpf_paths* p, int B, int H, int W, int n_phase, unsigned flags,
                                        bool masked) {
   return {B, H, W, n_phase, (int64_t)flags, masked ? 1 : 0, 100 * p->tile_tx + p->tile_ty,
-          p->cta_warps + 100 * p->n_teams};
+          p->cta_warps + 100 * p->n_teams + 10000 * (p->max_level + 1)};
 }
 
 static int check_eval_args(const lpf_paths* p, int B, int H, int W, unsigned flags) {
@@ -207,9 +208,10 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   if (p->plans.count(key)) return LPF_OK;
   EvalPlan pl;
   Geom& g = pl.g;
-  // the eroded planes serve the trie program; m = 0 has nothing but the root, which only the plain program counts
-  const bool use_e2 = !(flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)) && p->m >= 1;
-  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, use_e2, &g))
+  // the eroded planes serve the trie program (choose_geom caps the level at m: m = 0 has nothing but the root)
+  const int max_level =
+      (flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)) ? 0 : (p->max_level >= 0 ? p->max_level : MAX_LEVEL);
+  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, max_level, &g))
     return LPF_E_UNSUPPORTED;
   pl.Bpad = (B + g.G - 1) / g.G * g.G;
   long long off = 0;
@@ -261,7 +263,7 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   Program* pr = nullptr;
   for (;; q /= 2) {
     try {
-      pr = &get_program(p, q, flags, g.v[0].stride, g.v[1].stride, g.v[0].e2_band_off, g.v[1].e2_band_off);
+      pr = &get_program(p, q, flags, g.v[0].stride, g.v[1].stride, g.K, g.v[0].band_words, g.v[1].band_words);
     } catch (const std::bad_alloc&) {
       return LPF_E_NOMEM;
     }
@@ -323,11 +325,12 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
         if (x & E_TERMINAL) ++pl.terminals;
       }
     }
-    if ((uint32_t)(pr->entries[first] >> 32) & E_ROOTCOUNT_HI) ++pl.terminals;
   }
   const long long total_work = (long long)pl.n_chunks * pl.n_gp;
   if (total_work >= (1ll << 32)) return LPF_E_UNSUPPORTED;
   pl.grid = (int)std::min<long long>(total_work, (long long)p->n_sm * occ);
+  pl.occ = occ;
+  shallow_terminals(p, pr->K, &pl.shallow);
 
   // workspace: the packed octant views, then the compact row-major / column-major bit images of stage 1, then (for
   // lpf_eval_masked) the views and the base bit images of the start mask (one image, one plane)
@@ -483,15 +486,18 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   for (int o = 0; o < 4; ++o) ep.mask_off[o] = pl.gm.v[o].packed_off;
   const bool timed = p->timing && !order.capturing;
   if (timed) LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_start, st));
-  LPF_CUDA(launch_eval(ep, pl.grid, pl.g.NT * pl.g.threads, pl.smem, st));
+  if (pl.grid > 0) LPF_CUDA(launch_eval(ep, pl.grid, pl.g.NT * pl.g.threads, pl.smem, st));
   if (timed) {
     LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_stop, st));
     p->timed_once = 1;
   }
+  const int n_shallow = pl.shallow.n[0] + pl.shallow.n[1] + pl.shallow.n[2] + pl.shallow.n[3];
+  if (n_shallow > 0) LPF_CUDA(launch_shallow(ep, pl.shallow, st));   // level K: the vectors shorter than K
   LPF_CUDA(launch_mirror((unsigned long long*)counts, S, n_arrays, p->n_sm, st));
   LPF_CUDA(order.done());
 
-  p->last_info[0] = start_mask ? 6 : 4;                  // kernels launched (pack base, pack views, eval, mirror)
+  // kernels launched (pack base, pack views, eval, mirror; shallow kernel at level K; two more packs for a start mask)
+  p->last_info[0] = (start_mask ? 6 : 4) + (n_shallow > 0 ? 1 : 0);
   p->last_info[1] = (long long)pl.n_chunks * pl.n_gp;    // chunks of NT work units x (image group, phase plane)
   p->last_info[2] = (int64_t)pl.pr->entries.size();      // program entries (all four octants)
   p->last_info[3] = pl.grid;
@@ -499,11 +505,14 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   p->last_info[5] = (int64_t)pl.smem;
   p->last_info[6] = pl.g.TX * 1000 + pl.g.TY * 100 + pl.pr->n_slots;   // thread tile TX, TY and mask-stack slots
   p->last_info[7] = pl.g.G;
-  p->last_info[8] = pl.g.v[0].e2_band_off ? 1 : 0;       // eroded planes in shared memory (else the plain plane)
+  p->last_info[8] = pl.g.K;                              // erosion level: 2^K eroded planes in shared memory (0: plain)
   p->last_info[9] = pl.fused_pairs;                      // per image-phase and start word: 2 SHF + 1 LOP3 each
   p->last_info[10] = pl.singles;                         //   1 SHF + 1 LOP3 each
   p->last_info[11] = pl.terminals;                       //   1 POPC + 1 add each
   p->last_info[12] = pl.piece_nodes;
+  p->last_info[13] = pl.g.NT;
+  p->last_info[14] = pl.occ;
+  p->last_info[15] = n_shallow;
   return LPF_OK;
 }
 
@@ -580,6 +589,12 @@ extern "C" int lpf_set_tile(lpf_paths* p, int tx, int ty, int cta_warps) {
   return LPF_OK;
 }
 
+extern "C" int lpf_set_level(lpf_paths* p, int max_level) {
+  if (!p || max_level < -1 || max_level > MAX_LEVEL) return LPF_E_INVAL;
+  p->max_level = max_level;
+  return LPF_OK;
+}
+
 extern "C" int lpf_set_teams(lpf_paths* p, int n_teams) {
   if (!p || n_teams < 0 || n_teams > EVAL_CTA_MAX_THREADS / 32) return LPF_E_INVAL;
   p->n_teams = n_teams;
@@ -595,9 +610,9 @@ extern "C" int lpf_last_eval_kernel_ms(const lpf_paths* p, float* ms) {
   return LPF_OK;
 }
 
-extern "C" int lpf_last_launch_info(const lpf_paths* p, int64_t* out13) {
-  if (!p || !out13) return LPF_E_INVAL;
-  std::memcpy(out13, p->last_info, sizeof(p->last_info));
+extern "C" int lpf_last_launch_info(const lpf_paths* p, int64_t* out16) {
+  if (!p || !out16) return LPF_E_INVAL;
+  std::memcpy(out16, p->last_info, sizeof(p->last_info));
   return LPF_OK;
 }
 

@@ -48,22 +48,22 @@ inline void from_view(int o, int av, int bv, int* a, int* b) {
 // ---- node program entry (uint64), DESIGN.md "Node program" -------------------------------
 // low word x:
 //   [ 0.. 4] sh      = a' & 31        bit offset of the window inside its word
-//   [ 5] RELOAD      row or word column differs from the previous entry: reload the row strip
-//   [ 6] TERMINAL    this prefix is a whole path P_v: count it
-//   [ 7] SAVE        copy the running mask to stack slot sslot (node has >= 2 children in its piece)
+//   [ 5] RELOAD      row, word column or plane differs from the previous entry: reload the row strip
+//   [ 6] TERMINAL    the last node of the entry is a whole path P_v: count it
+//   [ 7] SAVE        copy the running mask to stack slot sslot (the last node has >= 2 children in its piece)
 //   [ 8] RESTORE     parent mask comes from stack slot rslot (not from the previous entry)
-//   [ 9] INIT        parent mask is "every valid start pixel" (first entry of a work item / chain)
-//   [10] PAIR        this node's own mask is never needed (not TERMINAL, not SAVE) and the next entry is its
-//                    direct child: the walker fuses both windows into one 3-input AND (M & W1 & W2)
-//   [11] E2          the entry stands for TWO nodes, this one and its direct child (a'+1, b') in the same word column:
-//                    its window is read from the eroded plane E2 = row & (row >> 1), whose word offset is already
-//                    added to `off`; TERMINAL, SAVE and cidx are the child's
-//   [12..31] off     = b' * stride + (a' >> 5), word offset of the window in the packed view
+//   [ 9] INIT        parent mask is "every valid start pixel" (first entry of a work item, and only there)
+//   [10] PAIR        this entry's own mask is never needed (not TERMINAL, not SAVE) and the next entry continues from
+//                    it: the walker fuses both windows into one 3-input AND (M & W1 & W2)
+//   [11] ERODED      level K >= 1: the window is read from eroded plane q (high word) and covers the K + 1 pixels
+//                    (a' + j, b' + s_1 + .. + s_j), j = 0..K, s_j = bit j-1 of q; the first `back` of them are nodes
+//                    already in the mask (AND is idempotent), the rest are the nodes of this entry, the last of which
+//                    owns TERMINAL, SAVE and cidx.  The plane's word offset q * band_words is already added to `off`.
+//   [12..31] off     = b' * stride + (a' >> 5) (+ q * band_words), word offset of the window in shared memory
 // high word y:
 //   [ 0..19] cidx    = (dy + m) * (2m + 1) + (dx + m), index into counts[2m+1][2m+1] (image coordinates)
-//   [20..23] rslot
-//   [24..27] sslot
-//   [28] BACK        (with E2) the entry is a single node read as E2 at (a'-1, b'): the extra pixel is its parent's
+//   [20..22] rslot   [23..25] sslot
+//   [26..28] q       pattern of the eroded plane      [29..30] back   (both for the host test; the kernel needs neither)
 constexpr uint32_t E_SH_MASK = 31u;
 constexpr uint32_t E_RELOAD = 1u << 5;
 constexpr uint32_t E_TERMINAL = 1u << 6;
@@ -71,15 +71,15 @@ constexpr uint32_t E_SAVE = 1u << 7;
 constexpr uint32_t E_RESTORE = 1u << 8;
 constexpr uint32_t E_INIT = 1u << 9;
 constexpr uint32_t E_PAIR = 1u << 10;
-constexpr uint32_t E_E2 = 1u << 11;
-constexpr uint32_t E_BACK_HI = 1u << 28;
-constexpr uint32_t E_D2_HI = 1u << 29;        // high word: the entry reads the D2 plane (pixel & lower-right neighbour)
-constexpr uint32_t E_ROOTCOUNT_HI = 1u << 30; // high word, INIT entries of the eroded program: count v = 0 here   // high word: an E2 entry of ONE node, window one pixel to the left (for tests)
+constexpr uint32_t E_ERODED = 1u << 11;
 constexpr int E_OFF_SHIFT = 12;
 constexpr uint32_t E_CIDX_MASK = (1u << 20) - 1u;
 constexpr int E_RSLOT_SHIFT = 20;
-constexpr int E_SSLOT_SHIFT = 24;
-constexpr uint32_t E_SLOT_MASK = 15u;
+constexpr int E_SSLOT_SHIFT = 23;
+constexpr uint32_t E_SLOT_MASK = 7u;
+constexpr int E_Q_SHIFT = 26;
+constexpr int E_BACK_SHIFT = 29;
+static_assert(STACK_SLOTS_BUDGET <= 8, "three bits per mask-stack slot");
 
 constexpr int MAX_M = 511;
 
@@ -99,7 +99,8 @@ struct Program {         // one linearisation of the four octant tries for one s
   std::vector<int64_t> items;          // [n_items][4] = first entry, count, octant, 0; sorted by count, descending
   int n_slots = 0;
   int stride[4] = {0, 0, 0, 0};
-  int e2_off[4] = {0, 0, 0, 0};        // word offset of the E2 plane of each view in shared memory (0: none)
+  int K = 0;                           // erosion level (0: plain program)
+  int band_words[4] = {0, 0, 0, 0};    // level K: eroded plane q of view o sits at q * band_words[o] in shared memory
   uint64_t* d_entries = nullptr;       // device copy, uploaded by lpf_reserve (lpf_api.cu)
   uint32_t* d_skip = nullptr;
 };
@@ -109,10 +110,11 @@ struct Program {         // one linearisation of the four octant tries for one s
 struct EvalPlan {
   Geom g;                              // views with their offsets inside one phase plane of the packed workspace
   Geom gm;                             // the same views for the start mask of lpf_eval_masked (one image, one plane)
+  ShallowList shallow;                 // level K: terminals above depth K
   Program* pr = nullptr;
   int32_t* d_work = nullptr;           // [n_chunks][NT][4] = first entry, count, octant | strip band << 4, row band
   int64_t n_chunks = 0;
-  int Bpad = 0, n_gp = 0, grid = 0, prune = 0;
+  int Bpad = 0, n_gp = 0, grid = 0, prune = 0, occ = 0;
   size_t smem = 0;
   size_t views_bytes = 0, base_words = 0, mask_views_bytes = 0, mask_base_bytes = 0, need = 0;
   // what the walker executes per image-phase and start word (lpf_last_launch_info): pairs of entries folded into one
@@ -131,8 +133,8 @@ struct lpf_paths {
   int64_t sum_len = 0;
   int64_t n_trie_nodes = 0;          // distinct prefixes of all P_v, v in D (one trie, image coordinates)
   std::vector<lpf::Node> oct[4];     // per-octant prefix tries in view coordinates; [0] = root (0,0)
-  // key: (piece_nodes, program kind, stride0, stride1, E2 offset 0, E2 offset 1)   (views 3, 2 as views 0, 1)
-  std::map<std::tuple<int, unsigned, int, int, int, int>, lpf::Program> programs;
+  // key: (piece_nodes, program kind, stride0, stride1, level K, band words 0, band words 1)   (views 3, 2 as views 0, 1)
+  std::map<std::tuple<int, unsigned, int, int, int, int, int>, lpf::Program> programs;
   // key: B, H, W, phases, flags, masked, 100 tile_tx + tile_ty, cta_warps
   std::map<std::array<int64_t, 8>, lpf::EvalPlan> plans;
   // device workspace (sized by lpf_reserve; a call for a shape that was not reserved reserves it first)
@@ -163,11 +165,12 @@ struct lpf_paths {
   // lpf_set_timing: CUDA events recorded around the eval kernel alone
   int tile_tx = 0, tile_ty = 0, cta_warps = 0;   // lpf_set_tile overrides (0 = automatic)
   int n_teams = 0;                   // teams per CTA override (0 = automatic)
+  int max_level = -1;                // erosion level cap (lpf_set_level; -1 = automatic)
   int timing = 0;
   int timed_once = 0;                // a timed eval has been issued: ev_start / ev_stop hold a measurement
   void* ev_start = nullptr;
   void* ev_stop = nullptr;
-  int64_t last_info[13] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+  int64_t last_info[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
 };
 
 namespace lpf {
@@ -184,8 +187,10 @@ int swap_delta_impl(lpf_paths* p, const uint8_t* image, int H, int W, int phase,
 void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec);
 
 // builds (or returns the cached) program for (piece_nodes, flags, view strides); host side only
-Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int e2off03,
-                     int e2off12);
+Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int K, int bw03,
+                     int bw12);
+// the terminals above depth K of every octant trie (counted by shallow_kernel, not by the program)
+void shallow_terminals(const lpf_paths* p, int K, ShallowList* out);
 // forgets a cached program that was never uploaded (one the kernel cannot take)
 void drop_program(lpf_paths* p, const Program* pr);
 

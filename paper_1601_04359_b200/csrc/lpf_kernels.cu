@@ -111,19 +111,21 @@ __device__ __forceinline__ uint32_t periodic_word(const uint32_t* __restrict__ s
 //   view o of image I (lpf_internal.h): 0: I[y'][x']  1: I[x'][y']  2: I[x'][-y' mod W]  3: I[y'][-x' mod W]
 //   word (r, i) of a view holds x' = (32 i + k) mod Wv, y' = r mod Hv.  Views 0 and 3 read Brow, views 1 and 2 Bcol.
 //   One CTA per tile of PACK_TILE consecutive words of one (phase plane, view, image): it stages the plain words of
-//   the tile and of the row below it in shared memory (each a funnel shift of two base words, wrap words two of them),
-//   derives E2 = pixel & right neighbour and D2 = pixel & lower-right neighbour there (across word and row boundaries)
-//   and writes the planes with fully coalesced stores (a tile is one contiguous block of every plane).
+//   the tile and of the K rows below it in shared memory (each a funnel shift of two base words, wrap words two of
+//   them) and derives the 2^K eroded planes of level K there: plane q at a pixel = AND of the K + 1 pixels reached by
+//   the steps (+1, s_j), s_j = bit j-1 of q (across word and row boundaries).  All planes are written with fully
+//   coalesced stores (a tile is one contiguous block of every plane).
 // ---------------------------------------------------------------------------------------------
 constexpr int PACK_TILE = 4096;
 
+template <int K>
 __global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restrict__ base,
                                                          uint32_t* __restrict__ packed, Geom g, int B, int Bpad,
                                                          int4 tiles, long long ctas_per_plane) {
-  extern __shared__ uint32_t s_plain[];                    // [PACK_TILE + stride + 2]
+  extern __shared__ uint32_t s_plain[];                    // [PACK_TILE + K * stride + 2]
   const int Wc = (g.W + 31) >> 5, Hc = (g.H + 31) >> 5;
   const long long img_words = (long long)g.H * Wc + (long long)g.W * Hc;
-  const int np = g.v[0].e2_view_off > 0 ? 3 : 1;
+  constexpr int NP = K > 0 ? (1 << K) : 0;                 // eroded planes behind the plain one
   // CTA -> (phase plane, view, image, tile)
   const long long cta = blockIdx.x;
   const int plane = (int)(cta / ctas_per_plane);
@@ -135,16 +137,15 @@ __global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restr
   const ViewGeom& v = g.v[o];
   const int b = (int)(rem / tl);
   const int tile = (int)(rem - (long long)b * tl);
-  const int pv = v.view_words / np;                        // words of one plane of one image (rows * stride + padding)
+  const int pv = v.plane_words;                            // words of one plane of one image (rows * stride + padding)
   const int stride = v.stride, rows = v.n_bands * g.band_rows + g.m;
   const int w0 = tile * PACK_TILE, w1 = min(pv, w0 + PACK_TILE);
-  const int n_stage = min(w1 + stride + 2, rows * stride) - w0;      // staged words; beyond them everything is zero
+  const int n_stage = min(w1 + K * stride + 2, rows * stride) - w0;  // staged words; beyond them everything is zero
   uint32_t* dst = packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b * v.view_words;
   if (b >= B) {                                            // padding images of the last CTA group: all-zero planes
-    for (int L = w0 + threadIdx.x; L < w1; L += blockDim.x) {
-      dst[L] = 0u;
-      if (np == 3) { dst[L + v.e2_view_off] = 0u; dst[L + 2 * (size_t)v.e2_view_off] = 0u; }
-    }
+    for (int L = w0 + threadIdx.x; L < w1; L += blockDim.x)
+#pragma unroll
+      for (int q = 0; q <= NP; ++q) dst[L + (size_t)q * pv] = 0u;
     return;
   }
   const uint32_t* bimg = base + ((size_t)plane * B + b) * img_words;
@@ -166,14 +167,31 @@ __global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restr
     const int j = L - w0;
     const uint32_t w00 = j < n_stage ? s_plain[j] : 0u;
     dst[L] = w00;
-    if (np == 3) {
+    if (K > 0) {
       const int r = L / stride, i = L - r * stride;
       const bool more = i + 1 < stride;                    // the word right of the last one of a row reads as zero
-      const uint32_t w01 = (more && j + 1 < n_stage) ? s_plain[j + 1] : 0u;
-      const uint32_t w10 = (j + stride < n_stage) ? s_plain[j + stride] : 0u;
-      const uint32_t w11 = (more && j + stride + 1 < n_stage) ? s_plain[j + stride + 1] : 0u;
-      dst[L + v.e2_view_off] = w00 & __funnelshift_r(w00, w01, 1);
-      dst[L + 2 * (size_t)v.e2_view_off] = w00 & __funnelshift_r(w10, w11, 1);
+      // sh[jj][rr]: the plain window jj pixels to the right and rr rows below this word's pixels
+      uint32_t sh[K + 1][K + 1];
+#pragma unroll
+      for (int rr = 0; rr <= K; ++rr) {
+        const int jr = j + rr * stride;
+        const uint32_t lo = jr < n_stage ? s_plain[jr] : 0u;
+        const uint32_t hi = (more && jr + 1 < n_stage) ? s_plain[jr + 1] : 0u;
+#pragma unroll
+        for (int jj = 1; jj <= K; ++jj)
+          if (rr <= jj) sh[jj][rr] = __funnelshift_r(lo, hi, jj);
+      }
+#pragma unroll
+      for (int q = 0; q < NP; ++q) {
+        uint32_t acc = w00;
+        int rr = 0;
+#pragma unroll
+        for (int jj = 1; jj <= K; ++jj) {
+          rr += (q >> (jj - 1)) & 1;
+          acc &= sh[jj][rr];
+        }
+        dst[L + (size_t)(1 + q) * pv] = acc;
+      }
     }
   }
 }
@@ -283,19 +301,16 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
     const ViewGeom& v = g.v[o];
     const int stride = v.stride;
     if (tid == 0) {
+      // level K: shared memory holds the 2^K eroded bands (they follow the plain view in HBM); level 0: the plain band
       const unsigned bytes = (unsigned)v.band_words * 4u;
-      mbar_expect_tx(&bar, bytes * (unsigned)g.G * (v.e2_band_off ? 2u : 1u));
+      const int np = v.n_planes ? v.n_planes : 1;
+      mbar_expect_tx(&bar, bytes * (unsigned)(g.G * np));
       const uint32_t* src = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b0 * v.view_words +
-                            (size_t)band * g.band_rows * stride;
-      for (int gi = 0; gi < g.G; ++gi) {
-        if (v.e2_band_off) {        // eroded mode: shared memory holds the E2 and the D2 band, the plain view stays in HBM
-          tma_bulk_g2s(smem + (size_t)gi * v.band_pitch, src + (size_t)gi * v.view_words + v.e2_view_off, bytes, &bar);
-          tma_bulk_g2s(smem + (size_t)gi * v.band_pitch + v.e2_band_off,
-                       src + (size_t)gi * v.view_words + 2 * (size_t)v.e2_view_off, bytes, &bar);
-        } else {
-          tma_bulk_g2s(smem + (size_t)gi * v.band_pitch, src + (size_t)gi * v.view_words, bytes, &bar);
-        }
-      }
+                            (size_t)band * g.band_rows * stride + (v.n_planes ? v.plane_words : 0);
+      for (int gi = 0; gi < g.G; ++gi)
+        for (int q = 0; q < np; ++q)
+          tma_bulk_g2s(smem + (size_t)gi * v.band_pitch + (size_t)q * v.band_words,
+                       src + (size_t)gi * v.view_words + (size_t)q * v.plane_words, bytes, &bar);
     }
     // per-item thread geometry (the octant decides the view size)
     const int strip = sband * g.SB + strip_l;
@@ -315,7 +330,7 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
     const int e1 = e + wk.y;
     uint2 cur = __ldg(p.entries + e + lane);                 // the entry array is padded by 64
     // Every item begins with its only INIT entry: the parent mask is "every valid start pixel" (of the selected ones
-    // for L2~; in eroded mode AND the plain word of the start pixels themselves, i.e. the root pixel, from HBM).
+    // for L2~).
 #pragma unroll
     for (int ty = 0; ty < TY; ++ty) {
       const bool rowok = active && (band * g.band_rows + row0 + ty * 32 < v.Hv);
@@ -325,25 +340,12 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
         const uint32_t cm = nb >= 32 ? 0xffffffffu : (nb <= 0 ? 0u : ((1u << nb) - 1u));
         M[ty * TX + t] = rowok ? cm : 0u;
       }
-      if (v.e2_band_off && rowok) {
-        const uint32_t* pw = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b_img * v.view_words +
-                             (size_t)(band * g.band_rows + row0 + ty * 32) * stride + strip * TX;
-#pragma unroll
-        for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __ldg(pw + t);
-      }
       if (p.mask != nullptr && rowok) {                      // L2~: only the selected start pixels
         const uint32_t* mw =
             p.mask + p.mask_off[o] + (size_t)(band * g.band_rows + row0 + ty * 32) * stride + strip * TX;
 #pragma unroll
         for (int t = 0; t < TX; ++t) M[ty * TX + t] &= __ldg(mw + t);
       }
-    }
-    if (__shfl_sync(FULL, cur.y, 0) & E_ROOTCOUNT_HI) {      // eroded mode has no entry for the root: v = 0 is counted here
-      int c = 0;
-#pragma unroll
-      for (int t = 0; t < T; ++t) c += __popc(M[t]);
-      c = __reduce_add_sync(FULL, c);
-      if (c != 0 && store) atomicAdd(cnt + (size_t)(p.S / 2) * p.S + p.S / 2, (unsigned long long)c);
     }
     while (e < e1) {
       const uint2 nxt = __ldg(p.entries + e + 32 + lane);
@@ -459,6 +461,57 @@ __global__ void mirror_kernel(unsigned long long* counts, int S, long long n_arr
 }
 
 // ---------------------------------------------------------------------------------------------
+// shallow vectors (level K >= 1): a window of the eroded program covers K + 1 path pixels, so the vectors whose paths
+// are shorter (depth < K in their octant trie: at most 1 + 2 + 3 of them per octant at K = 3) have no entry.  They are
+// counted here from the plain view in HBM: grid = (n_phase * B, 4 octants); a thread ANDs the plain word of 32 start
+// pixels with the windows of the following path pixels (funnel shifts over the halo), POPC, block reduce, one atomic.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) shallow_kernel(const EvalParams p, const ShallowList sl) {
+  const Geom& g = p.g;
+  const int o = blockIdx.y;
+  const int n = sl.n[o];
+  if (n == 0) return;
+  const ViewGeom& v = g.v[o];
+  const int b = blockIdx.x % p.B, plane = blockIdx.x / p.B;
+  const uint32_t* plain = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b * v.view_words;
+  const uint32_t* mask = p.mask ? p.mask + p.mask_off[o] : nullptr;
+  const int stride = v.stride;
+  int c[6] = {0, 0, 0, 0, 0, 0};
+  for (int idx = threadIdx.x; idx < v.Hv * v.Wc; idx += blockDim.x) {
+    const int r = idx / v.Wc, i = idx - r * v.Wc;
+    const int nb = v.Wv - 32 * i;
+    uint32_t w0 = plain[(size_t)r * stride + i] & (nb >= 32 ? 0xffffffffu : ((1u << nb) - 1u));
+    if (mask) w0 &= mask[(size_t)r * stride + i];
+#pragma unroll
+    for (int t = 0; t < 6; ++t) {
+      if (t >= n) break;
+      uint32_t acc = w0;
+      int rr = r;
+      for (int j = 1; j <= sl.depth[o][t]; ++j) {
+        rr += (sl.steps[o][t] >> (j - 1)) & 1;
+        const uint32_t* q = plain + (size_t)rr * stride + i;
+        acc &= __funnelshift_r(q[0], q[1], j);
+      }
+      c[t] += __popc(acc);
+    }
+  }
+  __shared__ int ws[6][8];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int t = 0; t < 6; ++t) {
+    const int s = __reduce_add_sync(0xffffffffu, c[t]);
+    if (lane == 0) ws[t][warp] = s;
+  }
+  __syncthreads();
+  if (threadIdx.x < n) {
+    long long s = 0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) s += ws[threadIdx.x][w];
+    if (s) atomicAdd(p.counts + (size_t)b * p.image_stride + (size_t)plane * p.S * p.S + sl.cidx[o][threadIdx.x],
+                     (unsigned long long)s);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // objective: sse[b] = sum_k (c[b][k] - t[k])^2, exact in uint64 (Eq. 14 / Eq. 19).
 // grid = (chunks, B); partial sums are combined with one 64-bit atomic per block.
 // ---------------------------------------------------------------------------------------------
@@ -558,17 +611,24 @@ cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed,
   pack_base_kernel<<<(unsigned)blocks, 256, 0, st>>>(images, base, B, g.H, g.W, n_phase, phase0, counter);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  const int np = g.v[0].e2_view_off > 0 ? 3 : 1;
   int tl[4], stride_max = 0;
   long long per_plane = 0;
   for (int o = 0; o < 4; ++o) {
-    tl[o] = (g.v[o].view_words / np + PACK_TILE - 1) / PACK_TILE;
+    tl[o] = (g.v[o].plane_words + PACK_TILE - 1) / PACK_TILE;
     per_plane += (long long)Bpad * tl[o];
     stride_max = std::max(stride_max, g.v[o].stride);
   }
   if (per_plane * n_phase >= (1ll << 31)) return cudaErrorInvalidValue;
-  pack_views_kernel<<<(unsigned)(per_plane * n_phase), 256, (size_t)(PACK_TILE + stride_max + 2) * 4, st>>>(
-      base, packed, g, B, Bpad, make_int4(tl[0], tl[1], tl[2], tl[3]), per_plane);
+  const unsigned grid = (unsigned)(per_plane * n_phase);
+  const size_t smem = (size_t)(PACK_TILE + g.K * stride_max + 2) * 4;
+  const int4 tl4 = make_int4(tl[0], tl[1], tl[2], tl[3]);
+  switch (g.K) {
+    case 0: pack_views_kernel<0><<<grid, 256, smem, st>>>(base, packed, g, B, Bpad, tl4, per_plane); break;
+    case 1: pack_views_kernel<1><<<grid, 256, smem, st>>>(base, packed, g, B, Bpad, tl4, per_plane); break;
+    case 2: pack_views_kernel<2><<<grid, 256, smem, st>>>(base, packed, g, B, Bpad, tl4, per_plane); break;
+    case 3: pack_views_kernel<3><<<grid, 256, smem, st>>>(base, packed, g, B, Bpad, tl4, per_plane); break;
+    default: return cudaErrorInvalidValue;
+  }
   return cudaGetLastError();
 }
 
@@ -589,6 +649,11 @@ cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem,
   eval_fn f = eval_fn_for(p.g.TX, p.g.TY, p.prune != 0);
   if (!f) return cudaErrorInvalidValue;
   f<<<grid, threads, smem, st>>>(p);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_shallow(const EvalParams& p, const ShallowList& sl, cudaStream_t st) {
+  shallow_kernel<<<dim3((unsigned)(p.B * p.n_phase), 4u), 256, 0, st>>>(p, sl);
   return cudaGetLastError();
 }
 

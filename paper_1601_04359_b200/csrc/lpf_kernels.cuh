@@ -9,22 +9,25 @@ namespace lpf {
 // One octant view of one image in HBM / shared memory.
 //   word (r, i), r in [0, rows), i in [0, stride): bit k holds [ view(x' = (32 i + k) mod Wv, y' = r mod Hv) == phase ]
 //   rows = n_bands * band_rows + m (periodic halo below), stride = n_strips * TX + m / 32 + 1, made odd
+constexpr int STACK_SLOTS_BUDGET = 8;   // mask-stack slots per thread (local memory, T words each)
+
 struct ViewGeom {
   int Hv, Wv;        // view height (rows) and width (pixels): octants 0,3: H,W; octants 1,2: W,H
   int Wc;            // ceil(Wv / 32) words that hold start pixels
   int n_strips;      // ceil(Wc / TX) strips of TX words per row
   int stride;        // words per packed row
   int n_bands;       // ceil(Hv / band_rows) bands of start rows
-  int band_words;    // (band_rows + m) * stride rounded up to a multiple of 4: one band (one plane) in shared memory
-  int band_pitch;    // words per image in shared memory: band_words (plain mode) or 2 * band_words (eroded mode)
-  int e2_band_off;   // eroded mode: shared memory holds the E2 band at 0 and the D2 band at this offset; 0: plain mode
-  int view_words;    // whole packed block of one image: plain view, then (eroded mode) the E2 and the D2 view
-  int e2_view_off;   // eroded mode: the E2 view starts here, the D2 view at twice this; 0: plain mode
+  int band_words;    // (band_rows + m) * stride rounded up to a multiple of 4: one band of one plane in shared memory
+  int n_planes;      // planes held in shared memory: 0 = plain mode (the plain band alone), else the 2^K eroded bands
+  int band_pitch;    // words per image in shared memory: max(n_planes, 1) * band_words
+  int plane_words;   // words of one plane of one image in HBM (rows * stride, padded)
+  int view_words;    // whole packed block of one image: the plain view, then (level K) the 2^K eroded views
   long long packed_off;   // word offset of this octant's [Bpad][view_words] block inside one phase plane
 };
 
 struct Geom {
   int H, W, m;
+  int K;             // erosion level: 0 = plain plane; K >= 1: one plane per K-step pattern
   int TX, TY;        // thread tile: TX adjacent words x TY start rows (32 rows apart)
   int band_rows;     // start rows per work item, multiple of 32 * TY
   int SB;            // strips per work item (<= 8)
@@ -40,10 +43,19 @@ struct Geom {
 // host: pick the geometry for (m, H, W, B); false if one band does not fit in shared memory
 //   tx, ty > 0 override the thread tile; cta_warps (1..8) the warps per CTA
 constexpr int EVAL_CTA_MAX_THREADS = 1024;  // a CTA of NT teams (the eval kernel is compiled for 64 registers per thread)
-constexpr int STACK_SLOTS_BUDGET = 8;   // mask-stack slots per thread (local memory, T words each)
-//   use_e2: eroded mode allowed: shared memory holds E2 = pixel & right neighbour and D2 = pixel & lower-right
-//   neighbour instead of the plain plane
-bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2, Geom* out);
+//   max_level: highest erosion level allowed (0: plain plane only); level K keeps one plane per K-step pattern of a
+//   first-octant path in shared memory: plane q at (a, b) = AND of the K + 1 pixels (a + j, b + s_1 + .. + s_j),
+//   s_j = bit j-1 of q
+constexpr int MAX_LEVEL = 3;
+bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int max_level, Geom* out);
+
+// terminals above depth K have no program entry at level K (a window covers K + 1 pixels): shallow_kernel counts them
+struct ShallowList {
+  int n[4];            // per octant
+  int cidx[4][6];      // index into counts[S][S]
+  int depth[4][6];     // path length - 1 (< K <= 3)
+  int steps[4][6];     // bit j-1: step j goes one view row down
+};
 
 struct EvalParams {
   Geom g;

@@ -146,53 +146,48 @@ struct Held {            // the row strip that is in the registers when an entry
   int b = -1, col = -1, plane = -1;
 };
 
-// Emits the entries of one octant.  Two program styles:
-//   plain mode  (d2_off == 0): one entry per node, window read from the plain bit plane
-//   eroded mode (d2_off  > 0): shared memory holds E2 = pixel & right neighbour (at word offset 0) and D2 = pixel &
-//     lower-right neighbour (at d2_off) instead of the plain plane.  Every path step is (+1, 0) or (+1, +1), so
-//       - a node whose own mask is never needed and its only child are ONE entry (window of E2 or D2 at the node),
-//       - any other node is read "backwards": the window of E2 / D2 at its PARENT covers the parent's pixel, which
-//         is already in the mask, and its own;
-//     the root has no entry: INIT loads the plain word of the start pixels from HBM, every child of the root starts
-//     with INIT, and v = 0 is counted by the INIT entry that carries E_ROOTCOUNT_HI.
+// Emits the entries of one octant.  Program styles:
+//   level 0: one entry per node, window read from the plain bit plane
+//   level K >= 1: shared memory holds one eroded plane per K-step pattern q instead of the plain plane: plane q at
+//     (a, b) is the AND of the K + 1 pixels (a + j, b + s_1 + .. + s_j), s_j = bit j-1 of q.  Every path step is
+//     (+1, 0) or (+1, +1), so any K + 1 consecutive nodes of a path are ONE window of one of the 2^K planes:
+//       - a run of nodes whose own masks are never needed (not terminal, one child in the piece) is cut into entries
+//         of K + 1 nodes each,
+//       - a run that ends early (at a terminal, a branching node or a leaf) is read "backwards": the window that ENDS
+//         at its last node also covers some ancestors, which are already in the mask (AND is idempotent);
+//     the nodes above depth K have no entry (no window ends there): every item starts with the window root .. depth K,
+//     and the terminals above depth K are counted by shallow_kernel.
 struct Emitter {
   int m, o, stride;
-  int d2_off;
+  int K, band_words;
   const std::vector<Node>& nd;
   const std::vector<uint8_t>& cut;      // node is the root of a piece
   const std::vector<int32_t>& psize;    // nodes of the subtree that stay in the node's own piece
   Program& out;
-  bool* root_pending;                   // v = 0 still has to be attached to an INIT entry (octant 0, eroded mode)
   int max_slots = 0;
 
-  bool eroded() const { return d2_off > 0; }
-
-  // window at view pixel (a, b) on plane 0 plain / 1 E2 / 2 D2; TERMINAL / SAVE / count index belong to node `tail`
-  uint64_t entry(int a, int b, int plane, bool back, int tail, uint32_t flags, Held* held, int rslot, int sslot) const {
+  // the entry whose window ends at node `tail` and whose last `s` pixels are new nodes (1 <= s <= K + 1)
+  uint64_t entry(int tail, int s, uint32_t flags, Held* held, int rslot, int sslot) const {
+    int anchor = tail;
+    uint32_t q = 0;
+    for (int j = K; j >= 1; --j) {                   // step j of the window leads to its pixel j
+      const int par = nd[anchor].parent;
+      q |= (uint32_t)(nd[anchor].b - nd[par].b) << (j - 1);
+      anchor = par;
+    }
+    const int a = nd[anchor].a, b = nd[anchor].b;
+    const int plane = K > 0 ? (int)q : -1;
     const bool direct = !(flags & (E_RESTORE | E_INIT));
     if (!direct || held->b != b || held->col != (a >> 5) || held->plane != plane) flags |= E_RELOAD;
     held->b = b; held->col = a >> 5; held->plane = plane;
-    const uint32_t off = (uint32_t)(b * stride + (a >> 5) + (plane == 2 ? d2_off : 0));
-    const uint32_t x = (uint32_t)(a & 31) | flags | (plane ? E_E2 : 0u) | (off << E_OFF_SHIFT);
+    const uint32_t off = (uint32_t)(b * stride + (a >> 5) + (K > 0 ? (int)q * band_words : 0));
+    const uint32_t x = (uint32_t)(a & 31) | flags | (K > 0 ? E_ERODED : 0u) | (off << E_OFF_SHIFT);
     int ia, ib;
     from_view(o, nd[tail].a, nd[tail].b, &ia, &ib);
     const uint32_t cidx = (uint32_t)((ib + m) * (2 * m + 1) + (ia + m));
-    uint32_t y = cidx | ((uint32_t)rslot << E_RSLOT_SHIFT) | ((uint32_t)sslot << E_SSLOT_SHIFT) |
-                 (back ? E_BACK_HI : 0u) | (plane == 2 ? E_D2_HI : 0u);
-    if ((flags & E_INIT) && root_pending && *root_pending) {
-      y |= E_ROOTCOUNT_HI;
-      *root_pending = false;
-    }
+    const uint32_t y = cidx | ((uint32_t)rslot << E_RSLOT_SHIFT) | ((uint32_t)sslot << E_SSLOT_SHIFT) |
+                       (q << E_Q_SHIFT) | ((uint32_t)(K + 1 - s) << E_BACK_SHIFT);
     return (uint64_t)x | ((uint64_t)y << 32);
-  }
-
-  // the entry of `node` alone (backward window in eroded mode) or, if `child` >= 0, of node and child merged
-  uint64_t node_entry(int node, int child, uint32_t flags, Held* held, int rslot, int sslot) const {
-    if (!eroded()) return entry(nd[node].a, nd[node].b, 0, false, node, flags, held, rslot, sslot);
-    if (child >= 0)
-      return entry(nd[node].a, nd[node].b, nd[child].b == nd[node].b ? 1 : 2, false, child, flags, held, rslot, sslot);
-    const int par = nd[node].parent;                 // >= 0: the root has no entry in eroded mode
-    return entry(nd[par].a, nd[par].b, nd[par].b == nd[node].b ? 1 : 2, true, node, flags, held, rslot, sslot);
   }
 
   void kids_of(int node, std::vector<int>* kids) const {
@@ -204,15 +199,17 @@ struct Emitter {
   }
 
   // emits `node` and the part of its subtree inside the piece. src: 0 direct, 1 restore(rslot), 2 init.
-  void emit(int node, int src, int rslot, int depth_slots, bool count_it, Held held) {
+  // pend: ancestors of `node` (its chain from the root) that wait to be covered by the window of this entry.
+  void emit(int node, int src, int rslot, int depth_slots, bool count_it, Held held, int pend) {
     std::vector<int> kids;
     kids_of(node, &kids);
-    int child = -1;
+    int tail = node, s = pend + 1;
     bool term = nd[node].terminal && count_it;
-    if (eroded() && kids.size() == 1 && !term) {     // node's own mask is never needed: fold the only child in
-      child = kids[0];
-      term = nd[child].terminal;
-      kids_of(child, &kids);
+    while (s < K + 1 && !term && kids.size() == 1) { // the tail's own mask is never needed: take its only child in
+      tail = kids[0];
+      ++s;
+      term = nd[tail].terminal;
+      kids_of(tail, &kids);
     }
     uint32_t flags = term ? E_TERMINAL : 0u;
     if (src == 1) flags |= E_RESTORE;
@@ -224,20 +221,45 @@ struct Emitter {
       max_slots = std::max(max_slots, depth_slots + 1);
     }
     const size_t at = out.entries.size();
-    out.entries.push_back(node_entry(node, child, flags, &held, rslot, sslot));
+    out.entries.push_back(entry(tail, s, flags, &held, rslot, sslot));
     out.skip.push_back(0);
     for (size_t i = 0; i < kids.size(); ++i) {
       if (kids.size() == 1) {
-        emit(kids[i], 0, 0, depth_slots, true, held);
+        emit(kids[i], 0, 0, depth_slots, true, held, 0);
       } else if (i == 0) {
-        emit(kids[i], 0, 0, depth_slots + 1, true, held);
+        emit(kids[i], 0, 0, depth_slots + 1, true, held, 0);
       } else if (i + 1 < kids.size()) {
-        emit(kids[i], 1, sslot, depth_slots + 1, true, held);
+        emit(kids[i], 1, sslot, depth_slots + 1, true, held, 0);
       } else {
-        emit(kids[i], 1, sslot, depth_slots, true, held);      // last child: the slot is free again
+        emit(kids[i], 1, sslot, depth_slots, true, held, 0);   // last child: the slot is free again
       }
     }
     out.skip[at] = (uint32_t)(out.entries.size() - at - 1);
+  }
+
+  // one work item: the chain root -> parent(r), recomputed, never counted, never saved, then r and its piece
+  void emit_item(int r, bool count_root) {
+    std::vector<int> chain;
+    for (int u = nd[r].parent; u >= 0; u = nd[u].parent) chain.push_back(u);
+    std::reverse(chain.begin(), chain.end());
+    Held held;
+    bool started = false;
+    int pend = 0;
+    for (size_t i = 0; i < chain.size(); ++i) {
+      if (++pend < K + 1) continue;
+      out.entries.push_back(entry(chain[i], K + 1, started ? 0u : E_INIT, &held, 0, 0));
+      out.skip.push_back(0);
+      started = true;
+      pend = 0;
+    }
+    emit(r, started ? 0 : 2, 0, 0, count_root, held, pend);
+  }
+
+  // the nodes at depth exactly K below `u` that belong to u's piece (level K: the items of a piece rooted above depth K)
+  void at_depth_K(int u, std::vector<int>* found) const {
+    if (nd[u].depth == K) { found->push_back(u); return; }
+    for (int c = nd[u].first_child; c >= 0; c = nd[c].next_sibling)
+      if (!cut[c]) at_depth_K(c, found);
   }
 };
 
@@ -270,6 +292,7 @@ static void push_item(Program& pr, int64_t first, int o) {
 }
 
 static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
+  const int K = pr.K;
   for (int o = 0; o < 4; ++o) {
     const std::vector<Node>& nd = p->oct[o];
     const int N = (int)nd.size();
@@ -281,42 +304,51 @@ static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
       else psize[nd[i].parent] += psize[i];
     }
     cut[0] = 1;
-    bool root_pending = (o == 0) && pr.e2_off[o] > 0;      // eroded mode only: plain mode has a root entry
-    Emitter em{p->m, o, pr.stride[o], pr.e2_off[o], nd, cut, psize, pr, &root_pending};
-    std::vector<int> chain, kids;
+    Emitter em{p->m, o, pr.stride[o], K, pr.band_words[o], nd, cut, psize, pr};
+    std::vector<int> starts;
     for (int r = 0; r < N; ++r) {
       if (!cut[r]) continue;
-      const int64_t first = (int64_t)pr.entries.size();
-      if (em.eroded() && r == 0) {
-        // the root piece: the root has no entry, each of its children in the piece starts from INIT
-        em.kids_of(0, &kids);
-        for (int c : kids) {                               // INIT is only ever the first entry of an item
+      if (nd[r].depth < K) {
+        // a piece rooted above depth K: no window ends up there, so each of its nodes at depth K opens an item
+        // (terminals above depth K are counted by shallow_kernel)
+        starts.clear();
+        em.at_depth_K(r, &starts);
+        for (int d : starts) {
           const int64_t f = (int64_t)pr.entries.size();
-          em.emit(c, 2, 0, 0, true, Held());
+          em.emit_item(d, true);
           push_item(pr, f, o);
         }
         continue;
       }
-      if (r == 0 && o != 0 && psize[0] == 1) continue;   // plain mode: v = 0 is counted in octant 0 only
-      // chain root -> parent(r): recomputed per item, never counted, never saved (eroded mode: without the root)
-      chain.clear();
-      for (int u = nd[r].parent; u >= 0; u = nd[u].parent) chain.push_back(u);
-      std::reverse(chain.begin(), chain.end());
-      Held held;
-      bool started = false;
-      for (size_t i = em.eroded() ? 1 : 0; i < chain.size();) {
-        const bool merge = em.eroded() && i + 1 < chain.size();
-        pr.entries.push_back(em.node_entry(chain[i], merge ? chain[i + 1] : -1, started ? 0u : E_INIT, &held, 0, 0));
-        pr.skip.push_back(0);
-        started = true;
-        i += merge ? 2 : 1;
-      }
-      em.emit(r, started ? 0 : 2, 0, 0, !(r == 0 && o != 0), held);
+      if (r == 0 && o != 0 && psize[0] == 1) continue;   // plain program: v = 0 is counted in octant 0 only
+      const int64_t first = (int64_t)pr.entries.size();
+      em.emit_item(r, !(r == 0 && o != 0));
       push_item(pr, first, o);
     }
     pr.n_slots = std::max(pr.n_slots, em.max_slots);
   }
   sort_items(pr);
+}
+
+// the terminals above depth K of every octant trie, with their paths as step patterns (level K only)
+void shallow_terminals(const lpf_paths* p, int K, ShallowList* out) {
+  std::memset(out, 0, sizeof(*out));
+  const int m = p->m;
+  for (int o = 0; o < 4; ++o) {
+    const std::vector<Node>& nd = p->oct[o];
+    for (int i = 0; i < (int)nd.size(); ++i) {
+      if (nd[i].depth >= K || !nd[i].terminal) continue;
+      int steps = 0;
+      for (int u = i; nd[u].parent >= 0; u = nd[u].parent)
+        steps |= (nd[u].b - nd[nd[u].parent].b) << (nd[u].depth - 1);
+      int ia, ib;
+      from_view(o, nd[i].a, nd[i].b, &ia, &ib);
+      const int k = out->n[o]++;
+      out->cidx[o][k] = (ib + m) * (2 * m + 1) + (ia + m);
+      out->depth[o][k] = nd[i].depth;
+      out->steps[o][k] = steps;
+    }
+  }
 }
 
 // LPF_NO_TRIE: one chain per path, no sharing ("one-path-per-warp" variant of the north star).  An item opens with the
@@ -416,19 +448,21 @@ static void build_s2_program(lpf_paths* p, int piece_nodes, Program& pr) {
   sort_items(pr);
 }
 
-Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int e2off03,
-                     int e2off12) {
+Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int K, int bw03,
+                     int bw12) {
   if (piece_nodes < 0) piece_nodes = 0;
   const unsigned kind = (flags & LPF_S2) ? LPF_S2 : (flags & LPF_NO_TRIE);
-  if (kind != 0) e2off03 = e2off12 = 0;                    // the E2 plane serves the trie program only
-  const std::tuple<int, unsigned, int, int, int, int> key(piece_nodes, kind, stride03, stride12, e2off03, e2off12);
+  if (kind != 0) K = 0;                                    // the eroded planes serve the trie program only
+  if (K == 0) bw03 = bw12 = 0;
+  const std::tuple<int, unsigned, int, int, int, int, int> key(piece_nodes, kind, stride03, stride12, K, bw03, bw12);
   auto it = p->programs.find(key);
   if (it != p->programs.end()) return it->second;
   Program& pr = p->programs[key];
   pr.stride[0] = pr.stride[3] = stride03;
   pr.stride[1] = pr.stride[2] = stride12;
-  pr.e2_off[0] = pr.e2_off[3] = e2off03;
-  pr.e2_off[1] = pr.e2_off[2] = e2off12;
+  pr.K = K;
+  pr.band_words[0] = pr.band_words[3] = bw03;
+  pr.band_words[1] = pr.band_words[2] = bw12;
   if (flags & LPF_S2) build_s2_program(p, piece_nodes, pr);
   else if (flags & LPF_NO_TRIE) build_chain_program(p, piece_nodes, pr);
   else build_trie_program(p, piece_nodes, pr);
@@ -460,57 +494,65 @@ int build_host_table(lpf_paths* p) {
 
 namespace lpf {
 
-static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2,
+static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int K,
                               Geom* out);
 
-static int resident_warps(const Geom& g, int max_smem) {
-  const int per_sm = std::min(32, (max_smem + 1024) / (g.smem_bytes + 1024));
-  return std::min(64, per_sm * (g.threads / 32));
-}
-
-// one plane layout (with or without E2); automatic CTA size: the one that keeps the most warps resident per SM
-// (shared memory is the limiter: a CTA of several small images needs the same bytes per warp whatever its size, so
-// smaller CTAs quantise better)
-static bool choose_geom_plane(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2,
-                              Geom* out) {
-  if (cta_warps >= 1 && cta_warps <= 8) return choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cta_warps, use_e2, out);
-  int best_warps = -1;
-  for (int cw = 8; cw >= 2; cw /= 2) {
-    Geom g;
-    if (!choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cw, use_e2, &g)) continue;
-    const int warps = resident_warps(g, max_smem);
-    if (warps > best_warps + best_warps / 8) {         // a smaller CTA must win by more than 12 %
-      best_warps = warps;
-      *out = g;
-    }
+// Resident warps per SM of a geometry once the CTA is made of teams (lpf_api.cu picks the team count with the
+// occupancy API; this is the same search on a model: 64 registers per thread, i.e. at most 1024 threads per SM).
+static int resident_warps(const Geom& g, int max_smem, int* teams) {
+  const int ctas_smem = std::min(32, (max_smem + 1024) / (g.smem_bytes + 1024));
+  int best = 0;
+  for (int nt = 1; nt * g.threads <= EVAL_CTA_MAX_THREADS && nt <= 8; ++nt) {
+    const int ctas = std::min(ctas_smem, 1024 / (nt * g.threads));
+    const int warps = ctas * nt * (g.threads / 32);
+    if (warps > best) { best = warps; if (teams) *teams = nt; }
   }
-  return best_warps > 0;
+  return best;
 }
 
-// use_e2 = "the eroded program is allowed": its two planes double the shared memory of a band; templates that are
-// large against the image (m close to H: the halo dominates the band) can lose too much residency and then fall
-// back to the plain plane.
-bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2, Geom* out) {
-  Geom plain, eroded;
-  const bool ok_plain = choose_geom_plane(m, H, W, B, max_smem, tx, ty, cta_warps, false, &plain);
-  if (use_e2 && choose_geom_plane(m, H, W, B, max_smem, tx, ty, cta_warps, true, &eroded)) {
-    // measured: the eroded program wins with 16 resident warps against 24 and with 8
-    // against 16, and loses with 8 against 24
-    const int we = resident_warps(eroded, max_smem), wp = ok_plain ? resident_warps(plain, max_smem) : 0;
-    if (we >= 12 || 2 * we >= wp) {
-      *out = eroded;
-      return true;
+// Relative cost of a geometry: program entries at level K (measured on the tries of m = 64 .. 256: 1.9 : 1 : 0.70 :
+// 0.57 for K = 0 .. 3; a little is added for the higher levels, whose entries reload their row strip more often)
+// over the throughput at the resident warps (measured on config 3: 8 warps 0.57, 16 warps 0.87, 24 warps 0.985 of
+// the rate at 32).
+static double geom_cost(const Geom& g, int max_smem) {
+  static const double entries[MAX_LEVEL + 1] = {1.9, 1.0, 0.73, 0.61};
+  const int w = resident_warps(g, max_smem, nullptr);
+  double rate;
+  if (w >= 32) rate = 1.0;
+  else if (w >= 24) rate = 0.985 + 0.015 * (w - 24) / 8.0;
+  else if (w >= 16) rate = 0.87 + 0.115 * (w - 16) / 8.0;
+  else if (w >= 8) rate = 0.57 + 0.30 * (w - 8) / 8.0;
+  else rate = 0.57 * w / 8.0;
+  return entries[g.K] / std::max(rate, 1e-3);
+}
+
+// erosion level and CTA size: the cheapest by geom_cost; a smaller team (fewer images per CTA) or a lower level must
+// win by more than 3 %
+bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int max_level, Geom* out) {
+  max_level = std::max(0, std::min({max_level, MAX_LEVEL, m}));
+  double best = 0;
+  bool found = false;
+  for (int K = max_level; K >= 0; --K)
+    for (int cw = 8; cw >= 1; cw /= 2) {
+      if (cta_warps >= 1 && cta_warps <= 8 && cw != cta_warps) continue;
+      Geom g;
+      if (!choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cw, K, &g)) continue;
+      const double c = geom_cost(g, max_smem);
+      if (!found || c < best * 0.97) {
+        best = c;
+        *out = g;
+        found = true;
+      }
     }
-  }
-  if (ok_plain) *out = plain;
-  return ok_plain;
+  return found;
 }
 
-static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, bool use_e2,
+static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int K,
                               Geom* out) {
   Geom g;
   std::memset(&g, 0, sizeof(g));
-  g.H = H; g.W = W; g.m = m;
+  g.H = H; g.W = W; g.m = m; g.K = K;
+  const int n_planes = K > 0 ? (1 << K) : 0;
   const int wc_max = (std::max(H, W) + 31) / 32;
   if (tx > 0 && ty > 0) {
     g.TX = tx; g.TY = ty;
@@ -545,11 +587,10 @@ static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, 
       ViewGeom& v = g.v[o];
       v.n_bands = (v.Hv + g.band_rows - 1) / g.band_rows;
       v.band_words = ((g.band_rows + m) * v.stride + 3) / 4 * 4;
-      const int plain_view = ((v.n_bands * g.band_rows + m) * v.stride + 3) / 4 * 4 + 4;
-      v.band_pitch = use_e2 ? 2 * v.band_words : v.band_words;
-      v.e2_band_off = use_e2 ? v.band_words : 0;
-      v.view_words = use_e2 ? 3 * plain_view : plain_view;     // eroded mode packs plain | E2 | D2
-      v.e2_view_off = use_e2 ? plain_view : 0;
+      v.plane_words = ((v.n_bands * g.band_rows + m) * v.stride + 3) / 4 * 4 + 4;
+      v.n_planes = n_planes;
+      v.band_pitch = std::max(n_planes, 1) * v.band_words;
+      v.view_words = (1 + n_planes) * v.plane_words;       // level K packs the plain view, then the 2^K eroded views
       bw_max = std::max(bw_max, v.band_pitch);
     }
     const size_t per_image = (size_t)bw_max * 4;     // shared memory holds the G bands only
@@ -558,6 +599,7 @@ static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, 
       G = std::min(G, std::max(B, 1));
       G = (int)std::min<size_t>((size_t)G, ((size_t)max_smem - 1024) / per_image);
       g.G = std::max(G, 1);
+      g.NT = 1;
       g.threads = g.G * g.wpi * 32;
       g.smem_bytes = g.G * bw_max * 4;
       break;
@@ -626,16 +668,18 @@ extern "C" int lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, un
   if (!p || !n_entries || !n_items || !n_slots || !strides) return LPF_E_INVAL;
   if (H < 1 || W < 1 || p->m > std::min(H, W) - 1) return LPF_E_INVAL;
   lpf::Geom g;
+  const int max_level = (flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)) ? 0 : (p->max_level >= 0 ? p->max_level : lpf::MAX_LEVEL);
   if (!lpf::choose_geom(p->m, H, W, 1, p->max_smem > 0 ? p->max_smem : 232448, p->tile_tx, p->tile_ty, p->cta_warps,
-                        !(flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)) && p->m >= 1, &g))
+                        max_level, &g))
     return LPF_E_UNSUPPORTED;
   try {
-    lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride, g.v[0].e2_band_off,
-                                        g.v[1].e2_band_off);
+    lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride, g.K, g.v[0].band_words,
+                                        g.v[1].band_words);
     *n_entries = (int64_t)pr.entries.size();
     *n_items = (int64_t)pr.items.size() / 4;
     *n_slots = pr.n_slots;
-    for (int o = 0; o < 4; ++o) { strides[o] = pr.stride[o]; strides[4 + o] = pr.e2_off[o]; }
+    for (int o = 0; o < 4; ++o) { strides[o] = pr.stride[o]; strides[4 + o] = pr.band_words[o]; }
+    strides[8] = pr.K;
     if (entries) {
       if (cap_entries < *n_entries) return LPF_E_INVAL;
       std::memcpy(entries, pr.entries.data(), sizeof(uint64_t) * pr.entries.size());

@@ -22,7 +22,7 @@ EXPORTS = (
     "lpf_paths_get", "lpf_paths_program", "lpf_eval", "lpf_eval_both", "lpf_objective",
     "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
     "lpf_set_tile", "lpf_alu_peak", "lpf_eval_masked", "lpf_anneal", "lpf_reserve", "lpf_eval_sum",
-    "lpf_anneal_generate", "lpf_set_teams",
+    "lpf_anneal_generate", "lpf_set_teams", "lpf_set_level",
 )
 LPF_PROPOSE_OPPOSITE, LPF_PROPOSE_INTERFACIAL = 1, 2
 LPF_FOR_EVAL, LPF_FOR_EVAL_BOTH, LPF_FOR_MASKED, LPF_FOR_SWAP_DELTA, LPF_FOR_ANNEAL, LPF_FOR_HOST = 1, 2, 4, 8, 16, 32
@@ -98,6 +98,8 @@ def load() -> ctypes.CDLL:
     lib.lpf_set_tile.restype = I
     lib.lpf_set_teams.argtypes = [VP, I]
     lib.lpf_set_teams.restype = I
+    lib.lpf_set_level.argtypes = [VP, I]
+    lib.lpf_set_level.restype = I
     _lib = lib
     return lib
 
@@ -164,11 +166,11 @@ def lpf_paths_get(p: Paths, dx: int, dy: int) -> np.ndarray:
 
 
 def lpf_paths_program(p: Paths, H: int, W: int, piece_nodes: int = 0, flags: int = 0):
-    """(entries uint64 [n], items int64 [k, 4], n_slots, strides [8]: row strides of the 4 views, then their E2 plane
-    word offsets) of the linearised walk program."""
+    """(entries uint64 [n], items int64 [k, 4], n_slots, strides [9]: row strides of the 4 views, the words of one
+    eroded band of each view in shared memory, the level K) of the linearised walk program."""
     lib = load()
     ne, ni, ns = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int()
-    strides = (ctypes.c_int * 8)()
+    strides = (ctypes.c_int * 9)()
     _check(lib.lpf_paths_program(p.handle, int(H), int(W), int(piece_nodes), int(flags), None, 0, ctypes.byref(ne),
                                  None, 0, ctypes.byref(ni), ctypes.byref(ns), strides), "lpf_paths_program")
     entries = np.zeros(ne.value, dtype=np.uint64)
@@ -414,10 +416,10 @@ def lpf_eval_host(p: Paths, images_host, phase: int, counts_host=None, flags: in
 
 def lpf_last_launch_info(p: Paths) -> dict:
     lib = load()
-    out = (ctypes.c_int64 * 13)()
+    out = (ctypes.c_int64 * 16)()
     _check(lib.lpf_last_launch_info(p.handle, out), "lpf_last_launch_info")
-    keys = ("kernels", "work_items", "program_entries", "grid", "block", "smem_bytes", "tile", "G", "eroded",
-            "fused_pairs", "singles", "terminals", "piece_nodes")
+    keys = ("kernels", "work_items", "program_entries", "grid", "block", "smem_bytes", "tile", "G", "level",
+            "fused_pairs", "singles", "terminals", "piece_nodes", "teams", "ctas_per_sm", "shallow_vectors")
     return dict(zip(keys, [int(v) for v in out]))
 
 
@@ -435,6 +437,10 @@ def lpf_alu_peak(device: int = 0) -> dict:
 def lpf_set_tile(p: Paths, tx: int = 0, ty: int = 0, cta_warps: int = 0) -> None:
     """Tuning hook: thread tile (TX words x TY rows) and warps per CTA of the eval kernel; 0 = automatic."""
     _check(load().lpf_set_tile(p.handle, int(tx), int(ty), int(cta_warps)), "lpf_set_tile")
+
+
+def lpf_set_level(p: Paths, max_level: int = -1) -> None:
+    _check(load().lpf_set_level(p.handle, int(max_level)), "lpf_set_level")
 
 
 def lpf_set_teams(p: Paths, n_teams: int = 0) -> None:

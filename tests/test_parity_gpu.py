@@ -205,7 +205,7 @@ def test_config3_whole_template_against_the_oracle_digest():
         bad = [(ph, r) for ph in (0, 1) for r in range(2 * m + 1) if crc(got[ph, r]) != rows[(ph, r)]]
         assert not bad, (flags, bad[:10])
         assert sha(got) == want_sha, flags
-        assert lpf.lpf_last_launch_info(paths(m))["eroded"] == (0 if flags & lpf.LPF_NO_E2 else 1)
+        assert lpf.lpf_last_launch_info(paths(m))["level"] == (0 if flags & lpf.LPF_NO_E2 else 2)
 
 
 def test_config4_sampled_images_properties_and_objective():
@@ -566,20 +566,39 @@ def test_hypothesis_generated_small_cases():
 
 # ---- the plain-plane program at full size, the automatic fall-back, the boundary contract --------------------
 
-def test_no_e2_and_plain_fallback_at_full_size():
-    """LPF_NO_E2 on a 256 x 384 image and a shape where the geometry chooser itself falls back to the plain plane
-    (300 x 300, m = 299: the two eroded bands would leave too few resident warps); which program ran is read from
-    lpf_last_launch_info.  Sampled vectors against the oracle, both phases, plus Eq. 10 / Eq. 12."""
-    for H, W, m, flags, eroded in ((256, 384, 120, lpf.LPF_NO_E2, 0), (256, 384, 120, 0, 1), (300, 300, 299, 0, 0)):
+def test_every_erosion_level_and_team_count_at_full_size():
+    """The plain program (LPF_NO_E2 and level 0) and the eroded programs of level 1, 2, 3 on a 256 x 384 image, a shape
+    where only the lower levels fit in shared memory (300 x 300, m = 299), and fixed team counts; which program ran
+    is read from lpf_last_launch_info.  Sampled vectors (all the short ones among them: at level K the vectors shorter
+    than K are counted by their own kernel) against the oracle, both phases, plus Eq. 10 / Eq. 12."""
+    cases = [(256, 384, 120, lpf.LPF_NO_E2, -1, 0, 0), (256, 384, 120, 0, 0, 0, 0), (256, 384, 120, 0, 1, 0, 1),
+             (256, 384, 120, 0, 2, 0, 2), (256, 384, 120, 0, 3, 0, 3), (256, 384, 120, 0, -1, 1, None),
+             (256, 384, 120, 0, 2, 3, 2), (300, 300, 299, 0, -1, 0, None), (300, 300, 299, 0, 0, 0, 0)]
+    for H, W, m, flags, level, teams, want_level in cases:
         img = inputs.disks(H, W, 7.0, 0.45, inputs.seed_for(8, H + m))
         rng = np.random.default_rng(m)
         vecs = rng.integers(-m, m + 1, size=(300, 2))
         vecs[:6] = [(0, 0), (m, m), (-m, m), (m, 0), (0, m), (-m, 1)]
-        got = lpf.lpf_eval_both(paths(m), dev(img[None]), flags).cpu().numpy()[0]
-        assert lpf.lpf_last_launch_info(paths(m))["eroded"] == eroded, (H, W, m, flags)
+        short = np.array([(dx, dy) for dy in range(-3, 4) for dx in range(-3, 4)])
+        vecs = np.concatenate([vecs, short])
+        p = lpf.lpf_build_paths(m, 0)
+        try:
+            lpf.lpf_set_level(p, level)
+            lpf.lpf_set_teams(p, teams)
+            got = lpf.lpf_eval_both(p, dev(img[None]), flags).cpu().numpy()[0]
+            info = lpf.lpf_last_launch_info(p)
+        finally:
+            lpf.lpf_free_paths(p)
+        if want_level is not None:
+            assert info["level"] == want_level, (H, W, m, flags, level, info)
+        else:
+            assert 1 <= info["level"] <= 3, info
+        if teams:
+            assert info["teams"] == teams
+        assert info["shallow_vectors"] == [0, 1, 5, 13][info["level"]]
         for phase in (0, 1):
             want, _ = orc.counts_list(img, phase, vecs)
-            assert np.array_equal(got[phase][vecs[:, 1] + m, vecs[:, 0] + m], want), (H, W, m, flags, phase)
+            assert np.array_equal(got[phase][vecs[:, 1] + m, vecs[:, 0] + m], want), (H, W, m, flags, level, phase)
             _properties(got[phase], img, phase, m)
 
 

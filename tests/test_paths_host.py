@@ -94,8 +94,8 @@ def _decode(entries):
     x = (entries & np.uint64(0xffffffff)).astype(np.int64)
     y = (entries >> np.uint64(32)).astype(np.int64)
     return dict(sh=x & 31, reload=(x >> 5) & 1, terminal=(x >> 6) & 1, save=(x >> 7) & 1, restore=(x >> 8) & 1,
-                init=(x >> 9) & 1, pair=(x >> 10) & 1, e2=(x >> 11) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1), rslot=(y >> 20) & 15, sslot=(y >> 24) & 15, back=(y >> 28) & 1,
-                d2=(y >> 29) & 1, rootcount=(y >> 30) & 1)
+                init=(x >> 9) & 1, pair=(x >> 10) & 1, eroded=(x >> 11) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1),
+                rslot=(y >> 20) & 7, sslot=(y >> 23) & 7, q=(y >> 26) & 7, back=(y >> 29) & 3)
 
 
 def _from_view(o, a, b):
@@ -103,17 +103,29 @@ def _from_view(o, a, b):
     return [(a, b), (b, a), (-b, a), (-a, b)][o]
 
 
-@pytest.mark.parametrize("m,H,W,piece,flags", [(5, 8, 8, 0, 0), (12, 40, 100, 16, 0), (33, 64, 64, 256, 0),
-                                               (70, 300, 128, 512, 0), (12, 13, 13, 0, lpf.LPF_NO_TRIE),
-                                               (12, 64, 32, 64, lpf.LPF_NO_TRIE), (33, 64, 64, 256, lpf.LPF_NO_E2),
-                                               (40, 41, 97, 64, lpf.LPF_NO_E2)])
-def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags):
+@pytest.mark.parametrize("m,H,W,piece,flags,level", [
+    (5, 8, 8, 0, 0, -1), (12, 40, 100, 16, 0, -1), (33, 64, 64, 256, 0, -1), (70, 300, 128, 512, 0, -1),
+    (12, 40, 100, 16, 0, 1), (33, 64, 64, 256, 0, 2), (33, 64, 64, 64, 0, 3), (70, 300, 128, 512, 0, 1),
+    (2, 8, 9, 0, 0, 3), (3, 8, 9, 4, 0, 3), (1, 5, 5, 0, 0, -1),
+    (12, 13, 13, 0, lpf.LPF_NO_TRIE, -1), (12, 64, 32, 64, lpf.LPF_NO_TRIE, -1), (33, 64, 64, 256, lpf.LPF_NO_E2, -1),
+    (40, 41, 97, 64, lpf.LPF_NO_E2, -1), (33, 64, 64, 256, 0, 0)])
+def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags, level):
     """Interpret the node program on the host with a stack of pixel lists instead of masks:
     every terminal must be reached exactly once with exactly the pixel list P_v, and the row-strip
-    reload flag must be set whenever the row or word column differs from the previous entry."""
+    reload flag must be set whenever the row, word column or plane differs from the previous entry.
+    At level K >= 1 a window covers K + 1 pixels of which the first `back` must already be the tail of the
+    running list; the vectors shorter than K have no entry (a separate kernel counts them)."""
     p = lpf.lpf_build_paths(m, -1)
+    lpf.lpf_set_level(p, level)
     entries, items, n_slots, strides = lpf.lpf_paths_program(p, H, W, piece, flags)
     d = _decode(entries)
+    K = strides[8]
+    if flags & (lpf.LPF_NO_E2 | lpf.LPF_NO_TRIE) or level == 0:
+        assert K == 0
+    elif level > 0:
+        assert K == min(level, m)                            # these shapes are small: every level fits
+    else:
+        assert 1 <= K <= min(3, m)                           # the default program is an eroded one
     S = 2 * m + 1
     seen = {}
     covered = np.zeros(len(entries), dtype=bool)
@@ -121,40 +133,34 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
     for first, cnt, o, _ in items:
         cur, stack, held = None, {}, None
         assert strides[o] % 2 == 1
-        eroded = strides[4 + o] > 0                          # shared memory holds E2 and D2 instead of the plain plane
-        if eroded:
-            assert not (flags & (lpf.LPF_NO_E2 | lpf.LPF_NO_TRIE))
         for e in range(first, first + cnt):
             assert not covered[e]
             covered[e] = True
             assert bool(d["init"][e]) == (e == first)        # the kernel initialises the mask once, at the item's start
             if d["init"][e]:
-                cur = [(0, 0)] if eroded else []             # eroded mode: INIT loads the root pixel from the plain view
-                if d["rootcount"][e]:
-                    assert eroded and o == 0 and (0, 0) not in seen
-                    seen[(0, 0)] = [(0, 0)]
+                cur = []
             elif d["restore"][e]:
                 cur = list(stack[int(d["rslot"][e])])
-            assert cur is not None and not (d["rootcount"][e] and not d["init"][e])
-            plane = (2 if d["d2"][e] else 1) if d["e2"][e] else 0
-            assert (plane > 0) == eroded
-            bv, col = divmod(int(d["off"][e]) - (strides[4 + o] if plane == 2 else 0), strides[o])
+            assert cur is not None
+            assert bool(d["eroded"][e]) == (K > 0)
+            q, back = int(d["q"][e]), int(d["back"][e])
+            assert q < (1 << K) and back <= K
+            bv, col = divmod(int(d["off"][e]) - q * strides[4 + o], strides[o])
             av = col * 32 + int(d["sh"][e])
-            assert 0 <= bv <= av <= m
+            plane = q if K else -1
             if d["reload"][e]:
                 held = (bv, col, plane)
             assert held == (bv, col, plane), "stale row strip"
-            if plane == 0:
-                assert not d["back"][e]
-                cur = cur + [_from_view(o, av, bv)]
-            else:
-                second = (av + 1, bv) if plane == 1 else (av + 1, bv + 1)    # E2: right neighbour, D2: lower right
-                assert second[1] <= second[0] <= m
-                if d["back"][e]:                             # one node, read at its parent: the first pixel is old
-                    assert cur[-1] == _from_view(o, av, bv)
-                else:                                        # a node whose mask is never needed and its only child
-                    cur = cur + [_from_view(o, av, bv)]
-                cur = cur + [_from_view(o, *second)]
+            window = [(av, bv)]                              # the K + 1 pixels of plane q at (av, bv)
+            for j in range(1, K + 1):
+                window.append((window[-1][0] + 1, window[-1][1] + ((q >> (j - 1)) & 1)))
+            for a, b in window:
+                assert 0 <= b <= a <= m
+            window = [_from_view(o, a, b) for a, b in window]
+            if d["init"][e]:
+                assert back == 0 and window[0] == (0, 0)     # every item starts at the root with a full window
+            assert back == 0 or cur[-back:] == window[:back]  # pixels that are already in the mask
+            cur = cur + window[back:]
             if d["terminal"][e]:
                 cidx = int(d["cidx"][e])
                 dy, dx = cidx // S - m, cidx % S - m
@@ -164,14 +170,17 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
             if d["save"][e]:
                 assert int(d["sslot"][e]) < max(n_slots, 1)
                 stack[int(d["sslot"][e])] = list(cur)
-            # PAIR: this node's own mask is never needed and the next entry of the item continues from it
+            # PAIR: this entry's own mask is never needed and the next entry of the item continues from it
             want_pair = (not d["terminal"][e] and not d["save"][e] and e + 1 < first + cnt
                          and not d["init"][e + 1] and not d["restore"][e + 1])
             assert bool(d["pair"][e]) == bool(want_pair)
     assert covered.all()
-    assert len(seen) == 2 * m * m + 2 * m + 1
-    if not (flags & (lpf.LPF_NO_E2 | lpf.LPF_NO_TRIE)) and m >= 1:
-        assert d["e2"].all() and d["d2"].any() and (~d["d2"].astype(bool)).any()   # the default program is the eroded one
+    # vectors whose path has fewer than K + 1 pixels have no entry
+    short = [(dx, dy) for dy in range(0, m + 1) for dx in range(-m, m + 1)
+             if orc.in_half(dx, dy) and max(abs(dx), abs(dy)) < K]
+    assert len(short) == (2 * (K - 1) * (K - 1) + 2 * (K - 1) + 1 if K else 0)
+    assert not (set(short) & set(seen))
+    assert len(seen) + len(short) == 2 * m * m + 2 * m + 1
     for (dx, dy), pix in seen.items():
         assert orc.in_half(dx, dy)
         assert pix == [tuple(int(t) for t in r) for r in orc.path(dx, dy)], (dx, dy)
