@@ -245,8 +245,8 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
     if (best_warps < 1) return LPF_E_UNSUPPORTED;
   }
 
-  // work units: about 20 chunks of NT units per resident CTA (measured optimum on configs 2-4), pieces of
-  // 256 .. 16384 trie nodes, and at least 2 NT pieces per octant so that the teams of a CTA find work on one band
+  // work units: about 20 per resident team (measured on configs 2-4: the optimum is flat between 10 and 30), pieces
+  // of 256 .. 16384 trie nodes, and at least 2 NT pieces per octant so that the teams of a CTA find work on one key
   const int resident_guess = p->n_sm * std::max(occ, 1);
   long long n_nodes = 0;
   for (int o = 0; o < 4; ++o) n_nodes += (long long)p->oct[o].size();
@@ -259,7 +259,7 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
     piece = std::max<long long>(32, std::min<long long>(p->n_half / want_items, 4096));
     q = 32;
   }
-  while (q * 2 <= piece) q *= 2;                   // quantised so that nearby shapes share one cached program
+  while ((long long)q * q * 2 <= piece * piece) q *= 2;   // nearest power of two: nearby shapes share one cached program
   Program* pr = nullptr;
   for (;; q /= 2) {
     try {
@@ -276,36 +276,33 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   if (rc != LPF_OK) return rc;
   pl.pr = pr;
 
-  // the work list: items expanded over the strip bands of their octant are the units of one (octant, row band); the
-  // units of a key, big first, are cut into chunks of NT (the last one padded with empty units), big chunks first
-  std::vector<int32_t> work;
-  {
-    const size_t n_items = pr->items.size() / 4;
-    std::vector<std::array<int32_t, 4>> chunks_first;      // first unit of every chunk (sort key) + position
-    std::vector<std::array<int32_t, 4>> units, all;
-    for (int o = 0; o < 4; ++o)
-      for (int band = 0; band < g.v[o].n_bands; ++band) {
-        units.clear();
-        const int sb = (g.v[o].n_strips + g.SB - 1) / g.SB;
-        for (size_t i = 0; i < n_items; ++i) {             // items are sorted by size, descending
-          if ((int)pr->items[4 * i + 2] != o) continue;
-          for (int s = 0; s < sb; ++s)
-            units.push_back({(int32_t)pr->items[4 * i], (int32_t)pr->items[4 * i + 1], o | (s << 4), band});
-        }
-        while (units.size() % (size_t)g.NT) units.push_back({0, 0, o, band});
-        for (size_t u = 0; u < units.size(); u += (size_t)g.NT) {
-          chunks_first.push_back({units[u][1], (int32_t)(all.size() / (size_t)g.NT), 0, 0});
-          for (int t = 0; t < g.NT; ++t) all.push_back(units[u + t]);
+  // the work list: the items of an octant expanded over its strip bands are the units of one (octant, row band),
+  // big first; a key of the kernel is such a pair on one (image group, phase plane)
+  std::vector<int32_t> units, obtab;
+  const size_t n_items = pr->items.size() / 4;
+  for (int o = 0; o < 4; ++o) {
+    const int sb = (g.v[o].n_strips + g.SB - 1) / g.SB;
+    for (int band = 0; band < g.v[o].n_bands; ++band) {
+      const int32_t first = (int32_t)(units.size() / 4);
+      for (size_t i = 0; i < n_items; ++i) {               // items are sorted by size, descending
+        if ((int)pr->items[4 * i + 2] != o) continue;
+        for (int s = 0; s < sb; ++s) {
+          units.push_back((int32_t)pr->items[4 * i]);
+          units.push_back((int32_t)pr->items[4 * i + 1]);
+          units.push_back(s);
+          units.push_back(0);
         }
       }
-    std::stable_sort(chunks_first.begin(), chunks_first.end(),
-                     [](const std::array<int32_t, 4>& a, const std::array<int32_t, 4>& b) { return a[0] > b[0]; });
-    for (const auto& c : chunks_first)
-      for (int t = 0; t < g.NT; ++t)
-        for (int k = 0; k < 4; ++k) work.push_back(all[(size_t)c[1] * g.NT + t][k]);
+      const int32_t cnt = (int32_t)(units.size() / 4) - first;
+      if (cnt == 0) continue;                              // an octant without vectors (tiny m)
+      obtab.push_back(first);
+      obtab.push_back(cnt);
+      obtab.push_back(o);
+      obtab.push_back(band);
+    }
   }
-  pl.n_chunks = (int64_t)work.size() / 4 / g.NT;
-  const size_t n_items = pr->items.size() / 4;
+  pl.n_ob = (int)(obtab.size() / 4);
+  pl.n_units = (int64_t)units.size() / 4;
   // the walker's loop replayed on the host (eval_kernel_v3: chunks of 32 entries, a PAIR entry that is not the last of
   // its chunk is folded with its successor): the data operations the design executes per start word
   pl.piece_nodes = q;
@@ -326,9 +323,13 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
       }
     }
   }
-  const long long total_work = (long long)pl.n_chunks * pl.n_gp;
-  if (total_work >= (1ll << 32)) return LPF_E_UNSUPPORTED;
-  pl.grid = (int)std::min<long long>(total_work, (long long)p->n_sm * occ);
+  const long long n_keys = (long long)pl.n_ob * pl.n_gp;
+  pl.grid = (int)std::max<long long>(0, std::min<long long>(pl.n_units * pl.n_gp, (long long)p->n_sm * occ));
+  // passes of the share cursor over the keys: enough to attach every CTA of the grid, and two more for helping out
+  const long long passes = n_keys > 0 ? (pl.grid + n_keys - 1) / n_keys + 2 : 0;
+  if (n_keys * passes >= (1ll << 31)) return LPF_E_UNSUPPORTED;
+  pl.n_keys = n_keys;
+  pl.n_shares = n_keys * passes;
   pl.occ = occ;
   shallow_terminals(p, pr->K, &pl.shallow);
 
@@ -347,14 +348,21 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   pl.need = pl.views_bytes + pl.base_words * 4 + pl.mask_views_bytes + pl.mask_base_bytes;
   rc = grow(&p->d_packed, &p->packed_bytes, pl.need);
   if (rc != LPF_OK) return rc;
+  // units, (octant, row band) table and the counters (share cursor + one per key) in one allocation
   int32_t* d_work = nullptr;
-  cudaError_t e = cudaMalloc(&d_work, sizeof(int32_t) * std::max<size_t>(work.size(), 4));
-  if (e == cudaSuccess) e = cudaMemcpy(d_work, work.data(), sizeof(int32_t) * work.size(), cudaMemcpyHostToDevice);
+  const size_t work_ints = units.size() + obtab.size();
+  cudaError_t e = cudaMalloc(&d_work, sizeof(int32_t) * (std::max<size_t>(work_ints, 4) + (size_t)n_keys + 4));
+  if (e == cudaSuccess && !units.empty())
+    e = cudaMemcpy(d_work, units.data(), sizeof(int32_t) * units.size(), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess && !obtab.empty())
+    e = cudaMemcpy(d_work + units.size(), obtab.data(), sizeof(int32_t) * obtab.size(), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) {
     if (d_work) cudaFree(d_work);
     return cuda_fail(e);
   }
   pl.d_work = d_work;
+  pl.d_obtab = d_work + units.size();
+  pl.d_counters = (unsigned int*)(d_work + work_ints);
   try {
     p->plans[key] = pl;
   } catch (const std::bad_alloc&) {
@@ -469,8 +477,12 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   ep.g = pl.g;
   ep.entries = (const uint2*)pl.pr->d_entries;
   ep.skip = pl.pr->d_skip;
-  ep.work = (const int4*)pl.d_work;
-  ep.n_chunks = (int)pl.n_chunks;
+  ep.units = (const int4*)pl.d_work;
+  ep.obtab = (const int4*)pl.d_obtab;
+  ep.n_ob = pl.n_ob;
+  ep.n_keys = (unsigned int)pl.n_keys;
+  ep.n_shares = (unsigned int)pl.n_shares;
+  ep.counters = pl.d_counters;
   ep.n_gp = pl.n_gp;
   ep.B = B;
   ep.n_phase = n_phase;
@@ -479,12 +491,13 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   ep.counts = (unsigned long long*)counts;
   ep.S = S;
   ep.image_stride = sum_over_batch ? 0 : (long long)n_phase * S * S;
-  ep.counter = p->d_counter;
   ep.prune = pl.prune;
   ep.n_slots = pl.pr->n_slots;
   ep.mask = start_mask ? d_mask : nullptr;
   for (int o = 0; o < 4; ++o) ep.mask_off[o] = pl.gm.v[o].packed_off;
   const bool timed = p->timing && !order.capturing;
+  if (pl.grid > 0)
+    LPF_CUDA(cudaMemsetAsync(pl.d_counters, 0, sizeof(unsigned int) * ((size_t)pl.n_keys + 1), st));
   if (timed) LPF_CUDA(cudaEventRecord((cudaEvent_t)p->ev_start, st));
   if (pl.grid > 0) LPF_CUDA(launch_eval(ep, pl.grid, pl.g.NT * pl.g.threads, pl.smem, st));
   if (timed) {
@@ -498,7 +511,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
 
   // kernels launched (pack base, pack views, eval, mirror; shallow kernel at level K; two more packs for a start mask)
   p->last_info[0] = (start_mask ? 6 : 4) + (n_shallow > 0 ? 1 : 0);
-  p->last_info[1] = (long long)pl.n_chunks * pl.n_gp;    // chunks of NT work units x (image group, phase plane)
+  p->last_info[1] = pl.n_units * pl.n_gp;                // work units x (image group, phase plane)
   p->last_info[2] = (int64_t)pl.pr->entries.size();      // program entries (all four octants)
   p->last_info[3] = pl.grid;
   p->last_info[4] = pl.g.NT * pl.g.threads;              // CTA = NT teams

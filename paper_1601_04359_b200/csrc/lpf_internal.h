@@ -112,8 +112,11 @@ struct EvalPlan {
   Geom gm;                             // the same views for the start mask of lpf_eval_masked (one image, one plane)
   ShallowList shallow;                 // level K: terminals above depth K
   Program* pr = nullptr;
-  int32_t* d_work = nullptr;           // [n_chunks][NT][4] = first entry, count, octant | strip band << 4, row band
-  int64_t n_chunks = 0;
+  int32_t* d_work = nullptr;           // work units [n_units][4] = first entry, entries, strip band, 0 (one allocation
+  int32_t* d_obtab = nullptr;          //   with) the (octant, row band) table [n_ob][4] = first unit, units, octant, band
+  unsigned int* d_counters = nullptr;  //   and the share cursor + one unit counter per key
+  int64_t n_units = 0, n_keys = 0, n_shares = 0;
+  int n_ob = 0;
   int Bpad = 0, n_gp = 0, grid = 0, prune = 0, occ = 0;
   size_t smem = 0;
   size_t views_bytes = 0, base_words = 0, mask_views_bytes = 0, mask_base_bytes = 0, need = 0;

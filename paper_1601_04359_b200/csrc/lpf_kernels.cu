@@ -261,13 +261,14 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
   constexpr unsigned FULL = 0xffffffffu;
   extern __shared__ __align__(128) uint32_t smem[];
   __shared__ __align__(8) uint64_t bar;
-  __shared__ unsigned int s_work;
+  __shared__ unsigned int s_key;
+  __shared__ unsigned int s_unit[2][32];
 
   const Geom& g = p.g;
   const int tid = threadIdx.x, lane = tid & 31;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // provably warp-uniform: the team's unit stays in uniform registers
   const int team_warps = g.G * g.wpi;
-  const int team = warp / team_warps;                   // teams walk different items on the same bands
+  const int team = warp / team_warps;                   // teams walk different units on the same bands
   const int wteam = warp - team * team_warps;
   const int img_local = wteam / g.wpi;
   const int ww = wteam - img_local * g.wpi;
@@ -282,50 +283,83 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
     mbar_init(&bar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  __syncthreads();
   unsigned parity = 0;
-  const unsigned total_work = (unsigned)p.n_chunks * (unsigned)p.n_gp;
   const int groups_per_plane = p.Bpad / g.G;
+  unsigned flip = 0;
 
+  // A key = (image group, phase plane, octant, row band): the bands one CTA holds in shared memory.  Shares of the keys
+  // are handed out by one cursor, pass after pass over all keys in alternating direction: the first passes attach every
+  // CTA of the grid to a key, the later ones let a CTA that has run out of work help on a key that is still open (the
+  // most recently started ones come first).  The units of a key (program item x strip band, big first) are handed out
+  // to the TEAMS by the key's own counter, so a team never waits for another one before the key is exhausted.
   for (;;) {
-    if (tid == 0) s_work = atomicAdd(p.counter, 1u);
-    __syncthreads();                 // everybody is also done reading the previous band
-    const unsigned work = s_work;
-    if (work >= total_work) break;
-    const int ci = (int)(work / (unsigned)p.n_gp);          // big chunks first, over all groups
-    const int gp = (int)(work - (unsigned)ci * (unsigned)p.n_gp);
+    __syncthreads();                 // everybody is done reading the previous bands (and the mbarrier is initialised)
+    if (tid == 0) {
+      unsigned key = 0xffffffffu;
+      for (;;) {
+        const unsigned s = atomicAdd(p.counters, 1u);
+        if (s >= p.n_shares) break;
+        const unsigned pass = s / p.n_keys, idx = s - pass * p.n_keys;
+        const unsigned k = (pass & 1u) ? p.n_keys - 1u - idx : idx;
+        const int4 ob = __ldg(p.obtab + k % (unsigned)p.n_ob);
+        if (*(volatile unsigned int*)(p.counters + 1 + k) < (unsigned)ob.y) { key = k; break; }
+      }
+      s_key = key;
+      if (key != 0xffffffffu) {
+        const int4 ob = __ldg(p.obtab + key % (unsigned)p.n_ob);
+        const int gp = (int)(key / (unsigned)p.n_ob);
+        const int plane = gp / groups_per_plane;
+        const int b0 = (gp - plane * groups_per_plane) * g.G;
+        const ViewGeom& v = g.v[ob.z];
+        // level K: shared memory holds the 2^K eroded bands (they follow the plain view in HBM); level 0: the plain band
+        const unsigned bytes = (unsigned)v.band_words * 4u;
+        const int np = v.n_planes ? v.n_planes : 1;
+        mbar_expect_tx(&bar, bytes * (unsigned)(g.G * np));
+        const uint32_t* src = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b0 * v.view_words +
+                              (size_t)ob.w * g.band_rows * v.stride + (v.n_planes ? v.plane_words : 0);
+        for (int gi = 0; gi < g.G; ++gi)
+          for (int q = 0; q < np; ++q)
+            tma_bulk_g2s(smem + (size_t)gi * v.band_pitch + (size_t)q * v.band_words,
+                         src + (size_t)gi * v.view_words + (size_t)q * v.plane_words, bytes, &bar);
+      }
+    }
+    __syncthreads();
+    const unsigned key = __shfl_sync(FULL, s_key, 0);
+    if (key == 0xffffffffu) break;
+    const int4 ob = __ldg(p.obtab + key % (unsigned)p.n_ob);     // first unit, units, octant, row band
+    const int gp = (int)(key / (unsigned)p.n_ob);
     const int plane = gp / groups_per_plane;
     const int b0 = (gp - plane * groups_per_plane) * g.G;
-    const int4 wk = __ldg(p.work + (size_t)ci * g.NT + team);   // the units of a chunk share octant and row band
-    const int o = wk.z & 15, sband = wk.z >> 4, band = wk.w;
+    const int o = ob.z, band = ob.w;
     const ViewGeom& v = g.v[o];
     const int stride = v.stride;
-    if (tid == 0) {
-      // level K: shared memory holds the 2^K eroded bands (they follow the plain view in HBM); level 0: the plain band
-      const unsigned bytes = (unsigned)v.band_words * 4u;
-      const int np = v.n_planes ? v.n_planes : 1;
-      mbar_expect_tx(&bar, bytes * (unsigned)(g.G * np));
-      const uint32_t* src = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b0 * v.view_words +
-                            (size_t)band * g.band_rows * stride + (v.n_planes ? v.plane_words : 0);
-      for (int gi = 0; gi < g.G; ++gi)
-        for (int q = 0; q < np; ++q)
-          tma_bulk_g2s(smem + (size_t)gi * v.band_pitch + (size_t)q * v.band_words,
-                       src + (size_t)gi * v.view_words + (size_t)q * v.plane_words, bytes, &bar);
-    }
-    // per-item thread geometry (the octant decides the view size)
-    const int strip = sband * g.SB + strip_l;
-    const bool active = strip < v.n_strips;
-    const char* base =
-        (const char*)(smem + (size_t)img_local * v.band_pitch + row0 * stride + (active ? strip : 0) * TX);
     const int rowstep = 32 * stride * 4;                     // bytes between the TY start rows of a thread
     const int b_img = b0 + img_local;
     unsigned long long* cnt = p.counts + (size_t)b_img * p.image_stride + (size_t)plane * p.S * p.S;
     const bool store = (lane == 0) && (b_img < p.B);
     mbar_wait(&bar, parity);
     parity ^= 1u;
-    __syncthreads();                 // s_work may be rewritten only after everyone has read it
 
-    if (wk.y == 0) continue;         // padding unit of a partial chunk: this team idles (the band is still shared)
+   for (;;) {                        // the team's units of this key
+    unsigned u;
+    if (team_warps == 1) {
+      u = 0;
+      if (lane == 0) u = atomicAdd(p.counters + 1 + key, 1u);
+    } else {
+      if (wteam == 0 && lane == 0) s_unit[flip][team] = atomicAdd(p.counters + 1 + key, 1u);
+      asm volatile("bar.sync %0, %1;" ::"r"(1 + team), "r"(team_warps * 32) : "memory");
+      u = s_unit[flip][team];
+      flip ^= 1u;                    // the other slot next time: nobody can still be reading it
+    }
+    u = __shfl_sync(FULL, u, 0);     // provably warp-uniform: the walker's control flow stays on the uniform datapath
+    if (__all_sync(FULL, u >= (unsigned)ob.y)) break;     // a vote: ptxas keeps the loop on the uniform datapath
+    const int4 wk = __ldg(p.units + ob.x + u);               // first entry, entries, strip band
+    const int sband = wk.z;
+    // per-unit thread geometry (the octant decides the view size)
+    const int strip = sband * g.SB + strip_l;
+    const bool active = strip < v.n_strips;
+    const char* base =
+        (const char*)(smem + (size_t)img_local * v.band_pitch + row0 * stride + (active ? strip : 0) * TX);
     int e = wk.x;
     const int e1 = e + wk.y;
     uint2 cur = __ldg(p.entries + e + lane);                 // the entry array is padded by 64
@@ -409,6 +443,7 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
             for (int t = 0; t < T; ++t) c += __popc(M[t]);
             c = __reduce_add_sync(FULL, c);
             if (c != 0) {
+
               if (store) atomicAdd(cnt + (y & E_CIDX_MASK), (unsigned long long)c);
             } else if (PRUNE) {          // paper's "enhanced" rule: nothing below can count
               const int sk = (int)__ldg(p.skip + e + i);
@@ -429,6 +464,7 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
         cur = nxt;
       }
     }
+   }
   }
 }
 

@@ -61,9 +61,13 @@ struct EvalParams {
   Geom g;
   const uint2* entries;
   const uint32_t* skip;
-  const int4* work;           // [n_chunks][NT] units = first entry, count (0: padding), octant | strip band << 4,
-                              // row band; the NT units of a chunk share octant and row band; big chunks first
-  int n_chunks;
+  const int4* units;          // work units = first entry, entries, strip band, 0; the units of one (octant, row band)
+                              // are consecutive, big first
+  const int4* obtab;          // [n_ob] (octant, row band) pairs = first unit, units, octant, row band
+  int n_ob;
+  unsigned int n_keys;        // n_gp * n_ob keys = (image group, phase plane, octant, row band); key = gp * n_ob + ob
+  unsigned int n_shares;      // n_keys * passes: how often the cursor hands out every key
+  unsigned int* counters;     // [0] the share cursor, [1 + key] units of the key handed out; zeroed before the launch
   int n_gp;                   // ceil(B / G) * n_phase (image group x phase plane)
   int B;
   int n_phase;                // 1 or 2 phase planes in `packed`
@@ -72,7 +76,6 @@ struct EvalParams {
   unsigned long long* counts; // [B][n_phase][S][S]  (lpf_eval_sum: [n_phase][S][S], image_stride 0)
   long long image_stride;     // elements between the count arrays of consecutive images: n_phase * S * S, or 0
   int S;                      // 2m + 1
-  unsigned int* counter;      // dynamic work counter, zeroed by the pack kernel
   int prune;
   int n_slots;                // mask-stack slots of the program (<= STACK_SLOTS_BUDGET)
   const uint32_t* mask;       // lpf_eval_masked: packed views of the start mask (one image), or nullptr
