@@ -211,7 +211,8 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   // the eroded planes serve the trie program (choose_geom caps the level at m: m = 0 has nothing but the root)
   const int max_level =
       (flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)) ? 0 : (p->max_level >= 0 ? p->max_level : MAX_LEVEL);
-  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, max_level, &g))
+  const int max_teams = max_teams_of(p);
+  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, max_level, max_teams, &g))
     return LPF_E_UNSUPPORTED;
   pl.Bpad = (B + g.G - 1) / g.G * g.G;
   long long off = 0;
@@ -235,8 +236,10 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   {
     int best_warps = 0;
     g.NT = 1;
-    for (int nt = 1; nt * g.threads <= EVAL_CTA_MAX_THREADS; ++nt) {
-      if (p->n_teams > 0 && nt != p->n_teams) continue;
+    // teams of several warps meet at a named barrier of their own: ids 1 .. 15
+    const int nt_max = g.threads > 32 ? 15 : 32;
+    for (int nt = 1; nt * g.threads <= EVAL_CTA_MAX_THREADS && nt <= nt_max; ++nt) {
+      if (p->n_teams > 0 ? nt != p->n_teams : nt > max_teams) continue;
       int o_nt = 0;
       LPF_CUDA(eval_occupancy(g.TX, g.TY, pl.prune != 0, nt * g.threads, pl.smem, p->max_smem, &o_nt));
       const int warps = o_nt * nt * (g.threads / 32);

@@ -192,6 +192,7 @@ void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec);
 // builds (or returns the cached) program for (piece_nodes, flags, view strides); host side only
 Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int K, int bw03,
                      int bw12);
+int max_teams_of(const lpf_paths* p);
 // the terminals above depth K of every octant trie (counted by shallow_kernel, not by the program)
 void shallow_terminals(const lpf_paths* p, int K, ShallowList* out);
 // forgets a cached program that was never uploaded (one the kernel cannot take)

@@ -47,7 +47,9 @@ constexpr int EVAL_CTA_MAX_THREADS = 1024;  // a CTA of NT teams (the eval kerne
 //   first-octant path in shared memory: plane q at (a, b) = AND of the K + 1 pixels (a + j, b + s_1 + .. + s_j),
 //   s_j = bit j-1 of q
 constexpr int MAX_LEVEL = 3;
-bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int max_level, Geom* out);
+//   max_teams: teams of one CTA that can find work on one key (lpf_internal.h: max_teams_of)
+bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int max_level, int max_teams,
+                 Geom* out);
 
 // terminals above depth K have no program entry at level K (a window covers K + 1 pixels): shallow_kernel counts them
 struct ShallowList {

@@ -499,10 +499,11 @@ static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, 
 
 // Resident warps per SM of a geometry once the CTA is made of teams (lpf_api.cu picks the team count with the
 // occupancy API; this is the same search on a model: 64 registers per thread, i.e. at most 1024 threads per SM).
-static int resident_warps(const Geom& g, int max_smem, int* teams) {
+// max_teams: teams that can find work on one key (a small trie has few pieces).
+static int resident_warps(const Geom& g, int max_smem, int max_teams, int* teams) {
   const int ctas_smem = std::min(32, (max_smem + 1024) / (g.smem_bytes + 1024));
   int best = 0;
-  for (int nt = 1; nt * g.threads <= EVAL_CTA_MAX_THREADS && nt <= 8; ++nt) {
+  for (int nt = 1; nt * g.threads <= EVAL_CTA_MAX_THREADS && nt <= std::max(1, std::min(8, max_teams)); ++nt) {
     const int ctas = std::min(ctas_smem, 1024 / (nt * g.threads));
     const int warps = ctas * nt * (g.threads / 32);
     if (warps > best) { best = warps; if (teams) *teams = nt; }
@@ -514,9 +515,9 @@ static int resident_warps(const Geom& g, int max_smem, int* teams) {
 // 0.57 for K = 0 .. 3; a little is added for the higher levels, whose entries reload their row strip more often)
 // over the throughput at the resident warps (measured on config 3: 8 warps 0.57, 16 warps 0.87, 24 warps 0.985 of
 // the rate at 32).
-static double geom_cost(const Geom& g, int max_smem) {
+static double geom_cost(const Geom& g, int max_smem, int max_teams) {
   static const double entries[MAX_LEVEL + 1] = {1.9, 1.0, 0.73, 0.61};
-  const int w = resident_warps(g, max_smem, nullptr);
+  const int w = resident_warps(g, max_smem, max_teams, nullptr);
   double rate;
   if (w >= 32) rate = 1.0;
   else if (w >= 24) rate = 0.985 + 0.015 * (w - 24) / 8.0;
@@ -526,18 +527,30 @@ static double geom_cost(const Geom& g, int max_smem) {
   return entries[g.K] / std::max(rate, 1e-3);
 }
 
-// erosion level and CTA size: the cheapest by geom_cost; a smaller team (fewer images per CTA) or a lower level must
-// win by more than 3 %
-bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int max_level, Geom* out) {
+// teams that find work on one key: two pieces of at least 256 trie nodes each per team and octant
+int max_teams_of(const lpf_paths* p) {
+  long long n_nodes = 0;
+  for (int o = 0; o < 4; ++o) n_nodes += (long long)p->oct[o].size();
+  return (int)std::max<long long>(1, std::min<long long>(32, n_nodes / 4 / 512));
+}
+
+// erosion level and team size: the cheapest by geom_cost.  Small teams come first -- two warps, then one, four, eight
+// (measured: config 3 3.73 / 3.76 / 3.89 / 3.78 ms, config 4 2.66 / 2.65 / 2.73 / 2.86 ms, 300 x 300 with m = 299
+// 4.10 / 5.42 / 4.57 / 4.57 ms: small keys balance better and leave room for a higher level); a later candidate or a
+// lower level must win by more than 3 %.
+bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int max_level, int max_teams,
+                 Geom* out) {
   max_level = std::max(0, std::min({max_level, MAX_LEVEL, m}));
   double best = 0;
   bool found = false;
+  static const int team_warps[4] = {2, 1, 4, 8};
   for (int K = max_level; K >= 0; --K)
-    for (int cw = 8; cw >= 1; cw /= 2) {
+    for (int ci = 0; ci < 4; ++ci) {
+      const int cw = team_warps[ci];
       if (cta_warps >= 1 && cta_warps <= 8 && cw != cta_warps) continue;
       Geom g;
       if (!choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cw, K, &g)) continue;
-      const double c = geom_cost(g, max_smem);
+      const double c = geom_cost(g, max_smem, max_teams);
       if (!found || c < best * 0.97) {
         best = c;
         *out = g;
@@ -670,7 +683,7 @@ extern "C" int lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, un
   lpf::Geom g;
   const int max_level = (flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)) ? 0 : (p->max_level >= 0 ? p->max_level : lpf::MAX_LEVEL);
   if (!lpf::choose_geom(p->m, H, W, 1, p->max_smem > 0 ? p->max_smem : 232448, p->tile_tx, p->tile_ty, p->cta_warps,
-                        max_level, &g))
+                        max_level, lpf::max_teams_of(p), &g))
     return LPF_E_UNSUPPORTED;
   try {
     lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride, g.K, g.v[0].band_words,
