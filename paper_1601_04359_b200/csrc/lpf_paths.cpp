@@ -503,7 +503,8 @@ static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, 
 static int resident_warps(const Geom& g, int max_smem, int max_teams, int* teams) {
   const int ctas_smem = std::min(32, (max_smem + 1024) / (g.smem_bytes + 1024));
   int best = 0;
-  for (int nt = 1; nt * g.threads <= EVAL_CTA_MAX_THREADS && nt <= std::max(1, std::min(8, max_teams)); ++nt) {
+  const int nt_max = std::max(1, std::min(g.threads > 32 ? 15 : 32, max_teams));   // named barriers 1 .. 15
+  for (int nt = 1; nt * g.threads <= EVAL_CTA_MAX_THREADS && nt <= nt_max; ++nt) {
     const int ctas = std::min(ctas_smem, 1024 / (nt * g.threads));
     const int warps = ctas * nt * (g.threads / 32);
     if (warps > best) { best = warps; if (teams) *teams = nt; }

@@ -205,7 +205,7 @@ def test_config3_whole_template_against_the_oracle_digest():
         bad = [(ph, r) for ph in (0, 1) for r in range(2 * m + 1) if crc(got[ph, r]) != rows[(ph, r)]]
         assert not bad, (flags, bad[:10])
         assert sha(got) == want_sha, flags
-        assert lpf.lpf_last_launch_info(paths(m))["level"] == (0 if flags & lpf.LPF_NO_E2 else 2)
+        assert lpf.lpf_last_launch_info(paths(m))["level"] == (0 if flags & lpf.LPF_NO_E2 else 3)
 
 
 def test_config4_sampled_images_properties_and_objective():
