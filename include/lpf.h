@@ -66,6 +66,9 @@ extern "C" {
                              plane per K-step pattern of a path, K + 1 pixels per window).
                              Same counts. */
 
+#define LPF_LAYOUT_MAX_CLASSES 128
+#define LPF_LAYOUT_INTS (10 + 38 * LPF_LAYOUT_MAX_CLASSES)   /* lpf_paths_program */
+
 /* `what` of lpf_reserve */
 #define LPF_FOR_EVAL        1u   /* lpf_eval and one-phase lpf_eval_sum with (B, H, W, flags) */
 #define LPF_FOR_EVAL_BOTH   2u   /* lpf_eval_both and two-phase lpf_eval_sum */
@@ -107,22 +110,26 @@ int  lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, int cap, int
  *            6 terminal, 7 save, 8 restore, 9 init, 10 pair (own mask never needed, the next entry continues from it),
  *            bits 12-31 b' * stride + (a' >> 5) (+ q * band_words); high word: bits 0-19
  *            (dy+m)*(2m+1) + (dx+m) in IMAGE coordinates, 20-22 restore slot, 23-25 save slot, 26-28 q, 29-30 back.
- *            bit 11: the window is read from an eroded plane (program of level K >= 1: every entry).  Plane q holds,
- *            at (a', b'), the AND of the K + 1 pixels (a' + j, b' + s_1 + .. + s_j), j = 0..K, s_j = bit j-1 of q --
- *            K + 1 consecutive pixels of a first-octant path.  The first `back` of them are nodes that are already in
- *            the mask, the others are the nodes of this entry; terminal / save / count index are the last one's.
+ *            bit 11: the window is read from an eroded plane (program of level K >= 1: every entry).  The plane of
+ *            step pattern q holds, at (a', b'), the AND of the K + 1 pixels (a' + j, b' + s_1 + .. + s_j), j = 0..K,
+ *            s_j = bit j-1 of q -- K + 1 consecutive pixels of a first-octant path.  Some first pixels of the window may
+ *            be nodes that are already in the mask; the others are the nodes of this entry; terminal / save / count
+ *            index are the last one's.  The vectors of an octant are split by slope into pattern CLASSES whose paths use
+ *            few patterns; an item belongs to one class and its entries address the class's planes by slot:
+ *            bits 12-31 = b' * stride + (a' >> 5) + slot * band_words; high word bits 26-31 repeat q.
  *            At level K no window ends above depth K: every item starts (its first and only init entry) with the
  *            window root .. depth K, and the vectors shorter than that are counted by a separate small kernel.
- *   items    host [cap_items][4] int64 = (first entry, number of entries, octant, 0) (may be NULL)
- *   strides  host int[9]: [0..3] words per packed row of each octant view (decodes b', a' >> 5), [4..7] words of one
- *            eroded band of each view in shared memory (plane q sits at q times that; 0 for the plain program),
- *            [8] the level K of the program (0: plain)
+ *   items    host [cap_items][4] int64 = (first entry, number of entries, octant, pattern class) (may be NULL)
+ *   layout   host int[LPF_LAYOUT_INTS]: [0..3] words per packed row of each octant view (decodes b', a' >> 5), [4..7]
+ *            words of one band of each view in shared memory (the plane in slot s sits at s times that; 0 for the plain
+ *            program), [8] the level K of the program (0: plain), [9] the number of pattern classes, then per class 38
+ *            ints: octant, patterns used n, the pattern q of slot 0 .. n-1 (-1 beyond)
  * *n_entries / *n_items / *n_slots (mask-stack slots the program needs) are always written.
  * Octants (view coordinates a', b' from image coordinates a, b): 0: dx>=0, dy<=dx (a,b); 1: dx>=0, dy>dx (b,a);
  * 2: dx<0, dy>-dx (b,-a); 3: dx<0, dy<=-dx (-a,b). */
 int  lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, unsigned flags,
                        uint64_t* entries, int64_t cap_entries, int64_t* n_entries,
-                       int64_t* items, int64_t cap_items, int64_t* n_items, int* n_slots, int* strides);
+                       int64_t* items, int64_t cap_items, int64_t* n_items, int* n_slots, int* layout);
 
 /* The rest of paper "step 1" for one image shape (step 1 is executed once, steps 2-3 "are called
  * repeatedly ... for new binary images of the same dimensions"): cuts the tries into the work items of a B x H x W
@@ -256,8 +263,8 @@ int  lpf_alu_peak(int device, double* out4);
 int  lpf_set_tile(lpf_paths* p, int tx, int ty, int cta_warps);
 
 /* Tuning hook: caps the erosion level of the programs built for the following
- * lpf_reserve / lpf_eval / lpf_paths_program calls on this object: 0..3, or -1 = automatic (the default).  Level K
- * keeps 2^K planes per row band in shared memory; the highest level that fits and keeps enough warps resident is the
+ * lpf_reserve / lpf_eval / lpf_paths_program calls on this object: 0..6, or -1 = automatic (the default).  Level K
+ * keeps the planes of one pattern class per row band in shared memory; the highest level that fits and keeps enough warps resident is the
  * fastest.  LPF_NO_E2 is level 0.  Never changes a count.  INVAL otherwise. */
 int  lpf_set_level(lpf_paths* p, int max_level);
 

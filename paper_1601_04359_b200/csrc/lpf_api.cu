@@ -86,8 +86,10 @@ static int grow(T** buf, size_t* have, size_t need) {
 static void free_program(Program& pr) {
   if (pr.d_entries) cudaFree(pr.d_entries);
   if (pr.d_skip) cudaFree(pr.d_skip);
+  if (pr.d_class_slots) cudaFree(pr.d_class_slots);
   pr.d_entries = nullptr;
   pr.d_skip = nullptr;
+  pr.d_class_slots = nullptr;
 }
 
 // uploads the program once; the device pointers are published only when every step has succeeded
@@ -95,20 +97,28 @@ static int upload_program(Program& pr) {
   if (pr.d_entries) return LPF_OK;
   uint64_t* d_e = nullptr;
   uint32_t* d_s = nullptr;
+  signed char* d_c = nullptr;
   const size_t ne = pr.entries.size() + 64;      // +64: the walker fetches 32 entries per warp, one chunk ahead
+  std::vector<signed char> slots(std::max<size_t>(pr.classes.size(), 1) * MAX_PATTERNS, (signed char)-1);
+  for (size_t c = 0; c < pr.classes.size(); ++c)
+    std::memcpy(slots.data() + c * MAX_PATTERNS, pr.classes[c].slot_of, MAX_PATTERNS);
   cudaError_t e = cudaMalloc(&d_e, sizeof(uint64_t) * ne);
   if (e == cudaSuccess) e = cudaMalloc(&d_s, sizeof(uint32_t) * std::max<size_t>(pr.skip.size(), 1));
+  if (e == cudaSuccess) e = cudaMalloc(&d_c, slots.size());
   if (e == cudaSuccess) e = cudaMemset(d_e, 0, sizeof(uint64_t) * ne);
   if (e == cudaSuccess)
     e = cudaMemcpy(d_e, pr.entries.data(), sizeof(uint64_t) * pr.entries.size(), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(d_s, pr.skip.data(), sizeof(uint32_t) * pr.skip.size(), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(d_c, slots.data(), slots.size(), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) {
     if (d_e) cudaFree(d_e);
     if (d_s) cudaFree(d_s);
+    if (d_c) cudaFree(d_c);
     return cuda_fail(e);
   }
   pr.d_entries = d_e;
   pr.d_skip = d_s;
+  pr.d_class_slots = d_c;
   return LPF_OK;
 }
 
@@ -209,10 +219,12 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   EvalPlan pl;
   Geom& g = pl.g;
   // the eroded planes serve the trie program (choose_geom caps the level at m: m = 0 has nothing but the root)
-  const int max_level =
-      (flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)) ? 0 : (p->max_level >= 0 ? p->max_level : MAX_LEVEL);
+  const int max_level = (flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2))
+                            ? 0
+                            : std::min(p->level_ok, p->max_level >= 0 ? p->max_level : MAX_LEVEL);
   const int max_teams = max_teams_of(p);
-  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, max_level, max_teams, &g))
+  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, max_level, max_teams,
+                   p->path_patterns, &g))
     return LPF_E_UNSUPPORTED;
   pl.Bpad = (B + g.G - 1) / g.G * g.G;
   long long off = 0;
@@ -249,12 +261,15 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   }
 
   // work units: about 20 per resident team (measured on configs 2-4: the optimum is flat between 10 and 30), pieces
-  // of 256 .. 16384 trie nodes, and at least 2 NT pieces per octant so that the teams of a CTA find work on one key
+  // of 256 .. 16384 trie nodes, and at least 4 pieces per team, octant and pattern class so that the teams of a CTA
+  // stay busy until a key is exhausted (measured on config 3, level 6: 2 pieces 2.56 ms, 4 pieces 2.49 ms)
   const int resident_guess = p->n_sm * std::max(occ, 1);
   long long n_nodes = 0;
   for (int o = 0; o < 4; ++o) n_nodes += (long long)p->oct[o].size();
-  const long long want_items =
-      std::max<long long>({1, 20ll * g.NT * resident_guess / ((long long)pl.n_gp * work_per_item), 8ll * g.NT});
+  const int planes_all = g.K > 0 ? balanced_count(g.K) : 0;
+  const int classes_guess = (g.K > 0 && g.v[0].n_planes < planes_all) ? std::max(1, 2 * planes_all / g.v[0].n_planes) : 1;
+  const long long want_items = std::max<long long>(
+      {1, 20ll * g.NT * resident_guess / ((long long)pl.n_gp * work_per_item), 16ll * g.NT * classes_guess});
   long long piece = n_nodes / want_items;
   piece = std::max<long long>(256, std::min<long long>(piece, 16384));
   int q = 256;
@@ -266,7 +281,8 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   Program* pr = nullptr;
   for (;; q /= 2) {
     try {
-      pr = &get_program(p, q, flags, g.v[0].stride, g.v[1].stride, g.K, g.v[0].band_words, g.v[1].band_words);
+      pr = &get_program(p, q, flags, g.v[0].stride, g.v[1].stride, g.K, g.v[0].n_planes, g.v[0].band_words,
+                        g.v[1].band_words);
     } catch (const std::bad_alloc&) {
       return LPF_E_NOMEM;
     }
@@ -279,29 +295,35 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   if (rc != LPF_OK) return rc;
   pl.pr = pr;
 
-  // the work list: the items of an octant expanded over its strip bands are the units of one (octant, row band),
-  // big first; a key of the kernel is such a pair on one (image group, phase plane)
+  // the work list: the items of one pattern class of an octant (one class at level 0) expanded over the strip bands
+  // are the units of one (octant, row band, class), big first; a key of the kernel is such a triple on one (image group,
+  // phase plane)
   std::vector<int32_t> units, obtab;
   const size_t n_items = pr->items.size() / 4;
-  for (int o = 0; o < 4; ++o) {
-    const int sb = (g.v[o].n_strips + g.SB - 1) / g.SB;
-    for (int band = 0; band < g.v[o].n_bands; ++band) {
-      const int32_t first = (int32_t)(units.size() / 4);
-      for (size_t i = 0; i < n_items; ++i) {               // items are sorted by size, descending
-        if ((int)pr->items[4 * i + 2] != o) continue;
-        for (int s = 0; s < sb; ++s) {
-          units.push_back((int32_t)pr->items[4 * i]);
-          units.push_back((int32_t)pr->items[4 * i + 1]);
-          units.push_back(s);
-          units.push_back(0);
+  const int n_classes = std::max<int>(1, (int)pr->classes.size());
+  for (int cls = 0; cls < n_classes; ++cls) {
+    const int o = pr->classes.empty() ? -1 : pr->classes[cls].octant;
+    for (int oo = 0; oo < 4; ++oo) {
+      if (o >= 0 && oo != o) continue;
+      const int sb = (g.v[oo].n_strips + g.SB - 1) / g.SB;
+      for (int band = 0; band < g.v[oo].n_bands; ++band) {
+        const int32_t first = (int32_t)(units.size() / 4);
+        for (size_t i = 0; i < n_items; ++i) {             // items are sorted by size, descending
+          if ((int)pr->items[4 * i + 2] != oo || (int)pr->items[4 * i + 3] != cls) continue;
+          for (int s = 0; s < sb; ++s) {
+            units.push_back((int32_t)pr->items[4 * i]);
+            units.push_back((int32_t)pr->items[4 * i + 1]);
+            units.push_back(s);
+            units.push_back(0);
+          }
         }
+        const int32_t cnt = (int32_t)(units.size() / 4) - first;
+        if (cnt == 0) continue;                            // an octant without vectors (tiny m)
+        obtab.push_back(first);
+        obtab.push_back(cnt);
+        obtab.push_back(oo | (cls << 2));
+        obtab.push_back(band);
       }
-      const int32_t cnt = (int32_t)(units.size() / 4) - first;
-      if (cnt == 0) continue;                              // an octant without vectors (tiny m)
-      obtab.push_back(first);
-      obtab.push_back(cnt);
-      obtab.push_back(o);
-      obtab.push_back(band);
     }
   }
   pl.n_ob = (int)(obtab.size() / 4);
@@ -482,6 +504,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   ep.skip = pl.pr->d_skip;
   ep.units = (const int4*)pl.d_work;
   ep.obtab = (const int4*)pl.d_obtab;
+  ep.class_slots = pl.pr->d_class_slots;
   ep.n_ob = pl.n_ob;
   ep.n_keys = (unsigned int)pl.n_keys;
   ep.n_shares = (unsigned int)pl.n_shares;

@@ -58,12 +58,13 @@ inline void from_view(int o, int av, int bv, int* a, int* b) {
 //   [11] ERODED      level K >= 1: the window is read from eroded plane q (high word) and covers the K + 1 pixels
 //                    (a' + j, b' + s_1 + .. + s_j), j = 0..K, s_j = bit j-1 of q; the first `back` of them are nodes
 //                    already in the mask (AND is idempotent), the rest are the nodes of this entry, the last of which
-//                    owns TERMINAL, SAVE and cidx.  The plane's word offset q * band_words is already added to `off`.
-//   [12..31] off     = b' * stride + (a' >> 5) (+ q * band_words), word offset of the window in shared memory
+//                    owns TERMINAL, SAVE and cidx.  The word offset of the plane (its slot in the item's pattern class
+//                    times band_words) is already added to `off`.
+//   [12..31] off     = b' * stride + (a' >> 5) (+ slot * band_words), word offset of the window in shared memory
 // high word y:
 //   [ 0..19] cidx    = (dy + m) * (2m + 1) + (dx + m), index into counts[2m+1][2m+1] (image coordinates)
 //   [20..22] rslot   [23..25] sslot
-//   [26..28] q       pattern of the eroded plane      [29..30] back   (both for the host test; the kernel needs neither)
+//   [26..31] q       step pattern of the window (for the host test; the kernel needs only `off`)
 constexpr uint32_t E_SH_MASK = 31u;
 constexpr uint32_t E_RELOAD = 1u << 5;
 constexpr uint32_t E_TERMINAL = 1u << 6;
@@ -78,7 +79,6 @@ constexpr int E_RSLOT_SHIFT = 20;
 constexpr int E_SSLOT_SHIFT = 23;
 constexpr uint32_t E_SLOT_MASK = 7u;
 constexpr int E_Q_SHIFT = 26;
-constexpr int E_BACK_SHIFT = 29;
 static_assert(STACK_SLOTS_BUDGET <= 8, "three bits per mask-stack slot");
 
 constexpr int MAX_M = 511;
@@ -100,7 +100,18 @@ struct Program {         // one linearisation of the four octant tries for one s
   int n_slots = 0;
   int stride[4] = {0, 0, 0, 0};
   int K = 0;                           // erosion level (0: plain program)
-  int band_words[4] = {0, 0, 0, 0};    // level K: eroded plane q of view o sits at q * band_words[o] in shared memory
+  int n_planes = 0;                    // planes per pattern class (shared memory slots)
+  int band_words[4] = {0, 0, 0, 0};    // level K: the plane in slot s of view o sits at s * band_words[o] in shared memory
+  // level K: pattern classes (slope sectors of one octant whose paths use at most n_planes patterns); items[4 i + 3] is
+  // the class of item i
+  struct Class {
+    int octant = 0;
+    int n = 0;                         // patterns used
+    int pattern[MAX_PATTERNS];         // slot -> pattern q
+    signed char slot_of[MAX_PATTERNS]; // rank of a balanced pattern -> slot, or -1
+  };
+  std::vector<Class> classes;
+  signed char* d_class_slots = nullptr;  // device: [classes][MAX_PATTERNS]
   uint64_t* d_entries = nullptr;       // device copy, uploaded by lpf_reserve (lpf_api.cu)
   uint32_t* d_skip = nullptr;
 };
@@ -136,8 +147,10 @@ struct lpf_paths {
   int64_t sum_len = 0;
   int64_t n_trie_nodes = 0;          // distinct prefixes of all P_v, v in D (one trie, image coordinates)
   std::vector<lpf::Node> oct[4];     // per-octant prefix tries in view coordinates; [0] = root (0,0)
-  // key: (piece_nodes, program kind, stride0, stride1, level K, band words 0, band words 1)   (views 3, 2 as views 0, 1)
+  // key: (piece_nodes, program kind, stride0, stride1, 100 K + planes per class, band words 0, band words 1)
   std::map<std::tuple<int, unsigned, int, int, int, int, int>, lpf::Program> programs;
+  int level_ok = 0;                  // highest level whose path windows are all balanced words (build_host_table)
+  int path_patterns[lpf::MAX_LEVEL + 1] = {0, 0, 0, 0, 0, 0, 0};   // most patterns of length K on one path
   // key: B, H, W, phases, flags, masked, 100 tile_tx + tile_ty, cta_warps
   std::map<std::array<int64_t, 8>, lpf::EvalPlan> plans;
   // device workspace (sized by lpf_reserve; a call for a shape that was not reserved reserves it first)
@@ -190,8 +203,8 @@ int swap_delta_impl(lpf_paths* p, const uint8_t* image, int H, int W, int phase,
 void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec);
 
 // builds (or returns the cached) program for (piece_nodes, flags, view strides); host side only
-Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int K, int bw03,
-                     int bw12);
+Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int K, int n_planes,
+                     int bw03, int bw12);
 int max_teams_of(const lpf_paths* p);
 // the terminals above depth K of every octant trie (counted by shallow_kernel, not by the program)
 void shallow_terminals(const lpf_paths* p, int K, ShallowList* out);

@@ -110,22 +110,16 @@ __device__ __forceinline__ uint32_t periodic_word(const uint32_t* __restrict__ s
 // bit-pack, stage 2: the four octant views with their periodic halo.
 //   view o of image I (lpf_internal.h): 0: I[y'][x']  1: I[x'][y']  2: I[x'][-y' mod W]  3: I[y'][-x' mod W]
 //   word (r, i) of a view holds x' = (32 i + k) mod Wv, y' = r mod Hv.  Views 0 and 3 read Brow, views 1 and 2 Bcol.
-//   One CTA per tile of PACK_TILE consecutive words of one (phase plane, view, image): it stages the plain words of
-//   the tile and of the K rows below it in shared memory (each a funnel shift of two base words, wrap words two of
-//   them) and derives the 2^K eroded planes of level K there: plane q at a pixel = AND of the K + 1 pixels reached by
-//   the steps (+1, s_j), s_j = bit j-1 of q (across word and row boundaries).  All planes are written with fully
-//   coalesced stores (a tile is one contiguous block of every plane).
+//   One thread per word: a funnel shift of two base words, a word that wraps around the row end two of them; fully
+//   coalesced stores (the eroded planes are derived from these words in the eval kernel's shared memory).
 // ---------------------------------------------------------------------------------------------
 constexpr int PACK_TILE = 4096;
 
-template <int K>
 __global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restrict__ base,
                                                          uint32_t* __restrict__ packed, Geom g, int B, int Bpad,
                                                          int4 tiles, long long ctas_per_plane) {
-  extern __shared__ uint32_t s_plain[];                    // [PACK_TILE + K * stride + 2]
   const int Wc = (g.W + 31) >> 5, Hc = (g.H + 31) >> 5;
   const long long img_words = (long long)g.H * Wc + (long long)g.W * Hc;
-  constexpr int NP = K > 0 ? (1 << K) : 0;                 // eroded planes behind the plain one
   // CTA -> (phase plane, view, image, tile)
   const long long cta = blockIdx.x;
   const int plane = (int)(cta / ctas_per_plane);
@@ -137,62 +131,30 @@ __global__ void __launch_bounds__(256) pack_views_kernel(const uint32_t* __restr
   const ViewGeom& v = g.v[o];
   const int b = (int)(rem / tl);
   const int tile = (int)(rem - (long long)b * tl);
-  const int pv = v.plane_words;                            // words of one plane of one image (rows * stride + padding)
+  const int pv = v.plane_words;                            // words of the view of one image (rows * stride + padding)
   const int stride = v.stride, rows = v.n_bands * g.band_rows + g.m;
   const int w0 = tile * PACK_TILE, w1 = min(pv, w0 + PACK_TILE);
-  const int n_stage = min(w1 + K * stride + 2, rows * stride) - w0;  // staged words; beyond them everything is zero
   uint32_t* dst = packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b * v.view_words;
-  if (b >= B) {                                            // padding images of the last CTA group: all-zero planes
-    for (int L = w0 + threadIdx.x; L < w1; L += blockDim.x)
-#pragma unroll
-      for (int q = 0; q <= NP; ++q) dst[L + (size_t)q * pv] = 0u;
+  if (b >= B) {                                            // padding images of the last CTA group: all-zero views
+    for (int L = w0 + threadIdx.x; L < w1; L += blockDim.x) dst[L] = 0u;
     return;
   }
   const uint32_t* bimg = base + ((size_t)plane * B + b) * img_words;
   const bool rowmajor = (o == 0 || o == 3);
   const int words = rowmajor ? Wc : Hc;
-  for (int j = threadIdx.x; j < n_stage; j += blockDim.x) {
-    const int L = w0 + j;
-    const int r = L / stride, i = L - r * stride;
-    int yv = r;                                            // r < rows <= 2 Hv + band_rows: a few subtractions at most
-    while (yv >= v.Hv) yv -= v.Hv;
-    // source row of a view row: views 0, 3: image row yv (Brow); view 1: image column yv; view 2: column -yv
-    const uint32_t* src = rowmajor ? bimg + (size_t)yv * Wc
-                                   : bimg + (size_t)g.H * Wc + (size_t)((o == 1) ? yv : (yv ? g.W - yv : 0)) * Hc;
-    const int x0 = (int)((32u * (unsigned)i) % (unsigned)v.Wv);
-    s_plain[j] = (o == 3) ? periodic_word<true>(src, words, v.Wv, x0) : periodic_word<false>(src, words, v.Wv, x0);
-  }
-  __syncthreads();
   for (int L = w0 + threadIdx.x; L < w1; L += blockDim.x) {
-    const int j = L - w0;
-    const uint32_t w00 = j < n_stage ? s_plain[j] : 0u;
-    dst[L] = w00;
-    if (K > 0) {
+    uint32_t w = 0u;
+    if (L < rows * stride) {
       const int r = L / stride, i = L - r * stride;
-      const bool more = i + 1 < stride;                    // the word right of the last one of a row reads as zero
-      // sh[jj][rr]: the plain window jj pixels to the right and rr rows below this word's pixels
-      uint32_t sh[K + 1][K + 1];
-#pragma unroll
-      for (int rr = 0; rr <= K; ++rr) {
-        const int jr = j + rr * stride;
-        const uint32_t lo = jr < n_stage ? s_plain[jr] : 0u;
-        const uint32_t hi = (more && jr + 1 < n_stage) ? s_plain[jr + 1] : 0u;
-#pragma unroll
-        for (int jj = 1; jj <= K; ++jj)
-          if (rr <= jj) sh[jj][rr] = __funnelshift_r(lo, hi, jj);
-      }
-#pragma unroll
-      for (int q = 0; q < NP; ++q) {
-        uint32_t acc = w00;
-        int rr = 0;
-#pragma unroll
-        for (int jj = 1; jj <= K; ++jj) {
-          rr += (q >> (jj - 1)) & 1;
-          acc &= sh[jj][rr];
-        }
-        dst[L + (size_t)(1 + q) * pv] = acc;
-      }
+      int yv = r;                                          // r < rows <= 2 Hv + band_rows: a few subtractions at most
+      while (yv >= v.Hv) yv -= v.Hv;
+      // source row of a view row: views 0, 3: image row yv (Brow); view 1: image column yv; view 2: column -yv
+      const uint32_t* src = rowmajor ? bimg + (size_t)yv * Wc
+                                     : bimg + (size_t)g.H * Wc + (size_t)((o == 1) ? yv : (yv ? g.W - yv : 0)) * Hc;
+      const int x0 = (int)((32u * (unsigned)i) % (unsigned)v.Wv);
+      w = (o == 3) ? periodic_word<true>(src, words, v.Wv, x0) : periodic_word<false>(src, words, v.Wv, x0);
     }
+    dst[L] = w;
   }
 }
 
@@ -250,6 +212,54 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, unsigne
 //   window then covers two path pixels.  PAIR entries fold their window into the next entry's 3-input AND.
 //   The mask of an item is initialised once, before the loop (INIT is only ever an item's first entry).
 // ---------------------------------------------------------------------------------------------
+// ---------------------------------------------------------------------------------------------
+// Level K: the eroded planes of one pattern class, derived in shared memory from the plain band (DESIGN.md "Eroded
+// planes").  The window of pattern q at a word is the AND of the plain windows j pixels to the right and rho_j =
+// s_1 + .. + s_j rows below, j = 0..K.  Compile-time recursion over the balanced words of length K: the patterns are
+// the leaves of a prefix tree, every tree edge is one funnel shift + AND, and a leaf is stored only if the class holds
+// the pattern (slot[rank] >= 0, a uniform test).
+// ---------------------------------------------------------------------------------------------
+__host__ __device__ constexpr int popcount_c(unsigned x) { int c = 0; for (; x; x >>= 1) c += (int)(x & 1u); return c; }
+
+template <int K, int J, unsigned PRE>
+__device__ __forceinline__ void derive_rec(uint32_t acc, const uint32_t (&lo)[K + 1], const uint32_t (&hi)[K + 1],
+                                           uint32_t* out, const signed char* slot, int band_words) {
+  if constexpr (J == K) {
+    const int s = slot[balanced_rank(PRE, K)];
+    if (s >= 0) out[(size_t)s * band_words] = acc;
+  } else {
+    constexpr int rho = popcount_c(PRE);
+    if constexpr (balanced_word(PRE, J + 1))
+      derive_rec<K, J + 1, PRE>(acc & __funnelshift_r(lo[rho], hi[rho], J + 1), lo, hi, out, slot, band_words);
+    if constexpr (balanced_word(PRE | (1u << J), J + 1))
+      derive_rec<K, J + 1, (PRE | (1u << J))>(acc & __funnelshift_r(lo[rho + 1], hi[rho + 1], J + 1), lo, hi, out, slot,
+                                              band_words);
+  }
+}
+
+// planes: [n_planes][band_words] of one image; plain: its plain band [rows][stride] (rows = band_rows + m)
+template <int K>
+__device__ __forceinline__ void derive_planes(uint32_t* planes, const uint32_t* plain, int rows, int stride,
+                                              int band_words, const signed char* slot) {
+  const int n = rows * stride;
+  const int dr = (int)blockDim.x / stride, di = (int)blockDim.x - dr * stride;
+  int r = (int)threadIdx.x / stride, i = (int)threadIdx.x - r * stride;
+  for (int idx = threadIdx.x; idx < n; idx += blockDim.x) {
+    uint32_t lo[K + 1], hi[K + 1];
+    const bool more = i + 1 < stride;                      // the word right of the last one of a row reads as zero
+#pragma unroll
+    for (int rr = 0; rr <= K; ++rr) {
+      const bool ok = r + rr < rows;                       // below the band everything reads as zero
+      lo[rr] = ok ? plain[idx + rr * stride] : 0u;
+      hi[rr] = (ok && more) ? plain[idx + rr * stride + 1] : 0u;
+    }
+    derive_rec<K, 0, 0u>(lo[0], lo, hi, planes + idx, slot, band_words);
+    i += di;
+    r += dr;
+    if (i >= stride) { i -= stride; ++r; }
+  }
+}
+
 // 64 registers per thread: CTAs of up to 1024 threads, 32 warps resident per SM (measured against 72 registers and 24
 // warps: config 3 5.33 vs 5.38 ms, config 4 3.67 vs 3.76 ms; the few spilled words sit next to the mask stack in L1)
 #ifndef LPF_EVAL_ATTR
@@ -263,6 +273,7 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
   __shared__ __align__(8) uint64_t bar;
   __shared__ unsigned int s_key;
   __shared__ unsigned int s_unit[2][32];
+  __shared__ signed char s_slot[MAX_PATTERNS];
 
   const Geom& g = p.g;
   const int tid = threadIdx.x, lane = tid & 31;
@@ -310,17 +321,16 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
         const int gp = (int)(key / (unsigned)p.n_ob);
         const int plane = gp / groups_per_plane;
         const int b0 = (gp - plane * groups_per_plane) * g.G;
-        const ViewGeom& v = g.v[ob.z];
-        // level K: shared memory holds the 2^K eroded bands (they follow the plain view in HBM); level 0: the plain band
+        const ViewGeom& v = g.v[ob.z & 3];
+        // the plain band of every image of the group: level 0 walks it; level K derives its planes from it (it sits
+        // behind them)
         const unsigned bytes = (unsigned)v.band_words * 4u;
-        const int np = v.n_planes ? v.n_planes : 1;
-        mbar_expect_tx(&bar, bytes * (unsigned)(g.G * np));
+        mbar_expect_tx(&bar, bytes * (unsigned)g.G);
         const uint32_t* src = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b0 * v.view_words +
-                              (size_t)ob.w * g.band_rows * v.stride + (v.n_planes ? v.plane_words : 0);
+                              (size_t)ob.w * g.band_rows * v.stride;
         for (int gi = 0; gi < g.G; ++gi)
-          for (int q = 0; q < np; ++q)
-            tma_bulk_g2s(smem + (size_t)gi * v.band_pitch + (size_t)q * v.band_words,
-                         src + (size_t)gi * v.view_words + (size_t)q * v.plane_words, bytes, &bar);
+          tma_bulk_g2s(smem + (size_t)gi * v.band_pitch + (size_t)v.n_planes * v.band_words,
+                       src + (size_t)gi * v.view_words, bytes, &bar);
       }
     }
     __syncthreads();
@@ -330,7 +340,7 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
     const int gp = (int)(key / (unsigned)p.n_ob);
     const int plane = gp / groups_per_plane;
     const int b0 = (gp - plane * groups_per_plane) * g.G;
-    const int o = ob.z, band = ob.w;
+    const int o = ob.z & 3, band = ob.w;
     const ViewGeom& v = g.v[o];
     const int stride = v.stride;
     const int rowstep = 32 * stride * 4;                     // bytes between the TY start rows of a thread
@@ -339,6 +349,25 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
     const bool store = (lane == 0) && (b_img < p.B);
     mbar_wait(&bar, parity);
     parity ^= 1u;
+    if (g.K > 0) {                   // the planes of the key's pattern class
+      const signed char* slot = p.class_slots + (size_t)(ob.z >> 2) * MAX_PATTERNS;
+      if (tid < MAX_PATTERNS) s_slot[tid] = slot[tid];
+      __syncthreads();
+      for (int gi = 0; gi < g.G; ++gi) {
+        uint32_t* planes = smem + (size_t)gi * v.band_pitch;
+        const uint32_t* plain = planes + (size_t)v.n_planes * v.band_words;
+        const int rows = g.band_rows + g.m;
+        switch (g.K) {
+          case 1: derive_planes<1>(planes, plain, rows, stride, v.band_words, s_slot); break;
+          case 2: derive_planes<2>(planes, plain, rows, stride, v.band_words, s_slot); break;
+          case 3: derive_planes<3>(planes, plain, rows, stride, v.band_words, s_slot); break;
+          case 4: derive_planes<4>(planes, plain, rows, stride, v.band_words, s_slot); break;
+          case 5: derive_planes<5>(planes, plain, rows, stride, v.band_words, s_slot); break;
+          default: derive_planes<6>(planes, plain, rows, stride, v.band_words, s_slot); break;
+        }
+      }
+      __syncthreads();
+    }
 
    for (;;) {                        // the team's units of this key
     unsigned u;
@@ -512,14 +541,16 @@ __global__ void __launch_bounds__(256) shallow_kernel(const EvalParams p, const 
   const uint32_t* plain = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b * v.view_words;
   const uint32_t* mask = p.mask ? p.mask + p.mask_off[o] : nullptr;
   const int stride = v.stride;
-  int c[6] = {0, 0, 0, 0, 0, 0};
+  int c[MAX_SHALLOW];
+#pragma unroll
+  for (int t = 0; t < MAX_SHALLOW; ++t) c[t] = 0;
   for (int idx = threadIdx.x; idx < v.Hv * v.Wc; idx += blockDim.x) {
     const int r = idx / v.Wc, i = idx - r * v.Wc;
     const int nb = v.Wv - 32 * i;
     uint32_t w0 = plain[(size_t)r * stride + i] & (nb >= 32 ? 0xffffffffu : ((1u << nb) - 1u));
     if (mask) w0 &= mask[(size_t)r * stride + i];
 #pragma unroll
-    for (int t = 0; t < 6; ++t) {
+    for (int t = 0; t < MAX_SHALLOW; ++t) {
       if (t >= n) break;
       uint32_t acc = w0;
       int rr = r;
@@ -531,10 +562,10 @@ __global__ void __launch_bounds__(256) shallow_kernel(const EvalParams p, const 
       c[t] += __popc(acc);
     }
   }
-  __shared__ int ws[6][8];
+  __shared__ int ws[MAX_SHALLOW][8];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
-  for (int t = 0; t < 6; ++t) {
+  for (int t = 0; t < MAX_SHALLOW; ++t) {
     const int s = __reduce_add_sync(0xffffffffu, c[t]);
     if (lane == 0) ws[t][warp] = s;
   }
@@ -655,16 +686,8 @@ cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed,
     stride_max = std::max(stride_max, g.v[o].stride);
   }
   if (per_plane * n_phase >= (1ll << 31)) return cudaErrorInvalidValue;
-  const unsigned grid = (unsigned)(per_plane * n_phase);
-  const size_t smem = (size_t)(PACK_TILE + g.K * stride_max + 2) * 4;
-  const int4 tl4 = make_int4(tl[0], tl[1], tl[2], tl[3]);
-  switch (g.K) {
-    case 0: pack_views_kernel<0><<<grid, 256, smem, st>>>(base, packed, g, B, Bpad, tl4, per_plane); break;
-    case 1: pack_views_kernel<1><<<grid, 256, smem, st>>>(base, packed, g, B, Bpad, tl4, per_plane); break;
-    case 2: pack_views_kernel<2><<<grid, 256, smem, st>>>(base, packed, g, B, Bpad, tl4, per_plane); break;
-    case 3: pack_views_kernel<3><<<grid, 256, smem, st>>>(base, packed, g, B, Bpad, tl4, per_plane); break;
-    default: return cudaErrorInvalidValue;
-  }
+  pack_views_kernel<<<(unsigned)(per_plane * n_phase), 256, 0, st>>>(base, packed, g, B, Bpad,
+                                                                     make_int4(tl[0], tl[1], tl[2], tl[3]), per_plane);
   return cudaGetLastError();
 }
 

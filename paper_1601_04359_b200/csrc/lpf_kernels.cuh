@@ -4,7 +4,43 @@
 #include <cstdint>
 #include <vector_types.h>
 
+#ifdef __CUDACC__
+#define LPF_HD __host__ __device__
+#else
+#define LPF_HD
+#endif
+
 namespace lpf {
+
+// ---- step patterns ------------------------------------------------
+// Every step of a first-octant path is (+1, 0) or (+1, +1); a K-step pattern q has bit j-1 set iff step j goes one row
+// down.  The patterns of K consecutive steps of a digital straight segment are the BALANCED words of length K: any two
+// factors of equal length differ by at most one in their number of down steps (2, 4, 8, 14, 24, 36 of them for
+// K = 1 .. 6, not 2^K).  The host checks that every window of every path of the table is balanced before it uses a
+// level; the eval kernel derives the planes of all balanced patterns of its level with compile-time recursion.
+LPF_HD constexpr bool balanced_word(unsigned q, int K) {
+  for (int L = 1; L <= K; ++L) {
+    int lo = 99, hi = -1;
+    for (int s = 0; s + L <= K; ++s) {
+      int c = 0;
+      for (int t = 0; t < L; ++t) c += (int)((q >> (s + t)) & 1u);
+      lo = c < lo ? c : lo;
+      hi = c > hi ? c : hi;
+    }
+    if (hi - lo > 1) return false;
+  }
+  return true;
+}
+// position of q among the balanced words of length K in ascending order
+LPF_HD constexpr int balanced_rank(unsigned q, int K) {
+  int r = 0;
+  for (unsigned t = 0; t < q; ++t) r += balanced_word(t, K) ? 1 : 0;
+  return r;
+}
+LPF_HD constexpr int balanced_count(int K) { return balanced_rank(1u << K, K); }
+constexpr int MAX_LEVEL = 6;
+constexpr int MAX_PATTERNS = 36;          // balanced_count(MAX_LEVEL)
+static_assert(balanced_count(MAX_LEVEL) == MAX_PATTERNS, "pattern table size");
 
 // One octant view of one image in HBM / shared memory.
 //   word (r, i), r in [0, rows), i in [0, stride): bit k holds [ view(x' = (32 i + k) mod Wv, y' = r mod Hv) == phase ]
@@ -18,16 +54,17 @@ struct ViewGeom {
   int stride;        // words per packed row
   int n_bands;       // ceil(Hv / band_rows) bands of start rows
   int band_words;    // (band_rows + m) * stride rounded up to a multiple of 4: one band of one plane in shared memory
-  int n_planes;      // planes held in shared memory: 0 = plain mode (the plain band alone), else the 2^K eroded bands
-  int band_pitch;    // words per image in shared memory: max(n_planes, 1) * band_words
-  int plane_words;   // words of one plane of one image in HBM (rows * stride, padded)
-  int view_words;    // whole packed block of one image: the plain view, then (level K) the 2^K eroded views
+  int n_planes;      // eroded planes of one pattern class held in shared memory: 0 = plain mode (the plain band alone)
+  int band_pitch;    // words per image in shared memory: band_words (plain mode), else (n_planes + 1) * band_words:
+                     // the planes, then the plain band they are derived from
+  int plane_words;   // words of the plain view of one image in HBM (rows * stride, padded)
+  int view_words;    // whole packed block of one image (= plane_words: only the plain view is kept in HBM)
   long long packed_off;   // word offset of this octant's [Bpad][view_words] block inside one phase plane
 };
 
 struct Geom {
   int H, W, m;
-  int K;             // erosion level: 0 = plain plane; K >= 1: one plane per K-step pattern
+  int K;             // erosion level: 0 = plain plane; K >= 1: one plane per K-step pattern of a class
   int TX, TY;        // thread tile: TX adjacent words x TY start rows (32 rows apart)
   int band_rows;     // start rows per work item, multiple of 32 * TY
   int SB;            // strips per work item (<= 8)
@@ -43,20 +80,22 @@ struct Geom {
 // host: pick the geometry for (m, H, W, B); false if one band does not fit in shared memory
 //   tx, ty > 0 override the thread tile; cta_warps (1..8) the warps per CTA
 constexpr int EVAL_CTA_MAX_THREADS = 1024;  // a CTA of NT teams (the eval kernel is compiled for 64 registers per thread)
-//   max_level: highest erosion level allowed (0: plain plane only); level K keeps one plane per K-step pattern of a
-//   first-octant path in shared memory: plane q at (a, b) = AND of the K + 1 pixels (a + j, b + s_1 + .. + s_j),
-//   s_j = bit j-1 of q
-constexpr int MAX_LEVEL = 3;
+//   max_level: highest erosion level allowed (0: plain plane only); at level K a window covers K + 1 path pixels: plane
+//   q at (a, b) = AND of the pixels (a + j, b + s_1 + .. + s_j), j = 0..K, s_j = bit j-1 of q.  The vectors of an octant
+//   are split by slope into CLASSES whose paths use at most n_planes patterns; the planes of one class are derived in
+//   shared memory from the plain band when a CTA takes a key of that class
 //   max_teams: teams of one CTA that can find work on one key (lpf_internal.h: max_teams_of)
+//   path_patterns[K]: most patterns of length K on one path of the table (a class needs as many planes)
 bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int max_level, int max_teams,
-                 Geom* out);
+                 const int* path_patterns, Geom* out);
 
 // terminals above depth K have no program entry at level K (a window covers K + 1 pixels): shallow_kernel counts them
+constexpr int MAX_SHALLOW = 21;   // 1 + 2 + .. + MAX_LEVEL vectors of fewer than MAX_LEVEL steps per octant
 struct ShallowList {
-  int n[4];            // per octant
-  int cidx[4][6];      // index into counts[S][S]
-  int depth[4][6];     // path length - 1 (< K <= 3)
-  int steps[4][6];     // bit j-1: step j goes one view row down
+  int n[4];                      // per octant
+  int cidx[4][MAX_SHALLOW];      // index into counts[S][S]
+  int depth[4][MAX_SHALLOW];     // path length - 1 (< K)
+  int steps[4][MAX_SHALLOW];     // bit j-1: step j goes one view row down
 };
 
 struct EvalParams {
@@ -65,9 +104,10 @@ struct EvalParams {
   const uint32_t* skip;
   const int4* units;          // work units = first entry, entries, strip band, 0; the units of one (octant, row band)
                               // are consecutive, big first
-  const int4* obtab;          // [n_ob] (octant, row band) pairs = first unit, units, octant, row band
+  const int4* obtab;          // [n_ob] (octant, row band, class) triples = first unit, units, octant | class << 2, row band
+  const signed char* class_slots;  // level K: [n_classes][MAX_PATTERNS] plane slot of each balanced pattern (by rank), or -1
   int n_ob;
-  unsigned int n_keys;        // n_gp * n_ob keys = (image group, phase plane, octant, row band); key = gp * n_ob + ob
+  unsigned int n_keys;        // n_gp * n_ob keys = (image group, phase plane, octant, row band, class); key = gp * n_ob + ob
   unsigned int n_shares;      // n_keys * passes: how often the cursor hands out every key
   unsigned int* counters;     // [0] the share cursor, [1 + key] units of the key handed out; zeroed before the launch
   int n_gp;                   // ceil(B / G) * n_phase (image group x phase plane)

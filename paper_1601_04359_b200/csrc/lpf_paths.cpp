@@ -160,6 +160,7 @@ struct Held {            // the row strip that is in the registers when an entry
 struct Emitter {
   int m, o, stride;
   int K, band_words;
+  const signed char* slot_of;           // level K: rank of a balanced pattern -> plane slot of the item's class
   const std::vector<Node>& nd;
   const std::vector<uint8_t>& cut;      // node is the root of a piece
   const std::vector<int32_t>& psize;    // nodes of the subtree that stay in the node's own piece
@@ -176,17 +177,17 @@ struct Emitter {
       anchor = par;
     }
     const int a = nd[anchor].a, b = nd[anchor].b;
-    const int plane = K > 0 ? (int)q : -1;
+    const int plane = K > 0 ? (int)slot_of[balanced_rank(q, K)] : -1;   // >= 0: the class holds every pattern of its paths
     const bool direct = !(flags & (E_RESTORE | E_INIT));
     if (!direct || held->b != b || held->col != (a >> 5) || held->plane != plane) flags |= E_RELOAD;
     held->b = b; held->col = a >> 5; held->plane = plane;
-    const uint32_t off = (uint32_t)(b * stride + (a >> 5) + (K > 0 ? (int)q * band_words : 0));
+    const uint32_t off = (uint32_t)(b * stride + (a >> 5) + (K > 0 ? plane * band_words : 0));
     const uint32_t x = (uint32_t)(a & 31) | flags | (K > 0 ? E_ERODED : 0u) | (off << E_OFF_SHIFT);
     int ia, ib;
     from_view(o, nd[tail].a, nd[tail].b, &ia, &ib);
     const uint32_t cidx = (uint32_t)((ib + m) * (2 * m + 1) + (ia + m));
-    const uint32_t y = cidx | ((uint32_t)rslot << E_RSLOT_SHIFT) | ((uint32_t)sslot << E_SSLOT_SHIFT) |
-                       (q << E_Q_SHIFT) | ((uint32_t)(K + 1 - s) << E_BACK_SHIFT);
+    (void)s;
+    const uint32_t y = cidx | ((uint32_t)rslot << E_RSLOT_SHIFT) | ((uint32_t)sslot << E_SSLOT_SHIFT) | (q << E_Q_SHIFT);
     return (uint64_t)x | ((uint64_t)y << 32);
   }
 
@@ -291,43 +292,150 @@ static void push_item(Program& pr, int64_t first, int o) {
   pr.items.push_back(0);
 }
 
-static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
+static void push_item_c(Program& pr, int64_t first, int o, int cls) {
+  push_item(pr, first, o);
+  pr.items.back() = cls;
+}
+
+// partitions one trie into pieces and emits its items
+static void emit_trie(const lpf_paths* p, int o, const std::vector<Node>& nd, int piece_nodes, Program& pr,
+                      const signed char* slot_of, int cls) {
   const int K = pr.K;
-  for (int o = 0; o < 4; ++o) {
-    const std::vector<Node>& nd = p->oct[o];
-    const int N = (int)nd.size();
-    std::vector<uint8_t> cut(N, 0);
-    std::vector<int32_t> psize(N, 1);
-    // greedy bottom-up partition: a node whose residual subtree reaches piece_nodes starts a piece
-    for (int i = N - 1; i > 0; --i) {
-      if (piece_nodes > 0 && psize[i] >= piece_nodes) cut[i] = 1;
-      else psize[nd[i].parent] += psize[i];
-    }
-    cut[0] = 1;
-    Emitter em{p->m, o, pr.stride[o], K, pr.band_words[o], nd, cut, psize, pr};
-    std::vector<int> starts;
-    for (int r = 0; r < N; ++r) {
-      if (!cut[r]) continue;
-      if (nd[r].depth < K) {
-        // a piece rooted above depth K: no window ends up there, so each of its nodes at depth K opens an item
-        // (terminals above depth K are counted by shallow_kernel)
-        starts.clear();
-        em.at_depth_K(r, &starts);
-        for (int d : starts) {
-          const int64_t f = (int64_t)pr.entries.size();
-          em.emit_item(d, true);
-          push_item(pr, f, o);
-        }
-        continue;
+  const int N = (int)nd.size();
+  std::vector<uint8_t> cut(N, 0);
+  std::vector<int32_t> psize(N, 1);
+  // greedy bottom-up partition: a node whose residual subtree reaches piece_nodes starts a piece
+  for (int i = N - 1; i > 0; --i) {
+    if (piece_nodes > 0 && psize[i] >= piece_nodes) cut[i] = 1;
+    else psize[nd[i].parent] += psize[i];
+  }
+  cut[0] = 1;
+  Emitter em{p->m, o, pr.stride[o], K, pr.band_words[o], slot_of, nd, cut, psize, pr};
+  std::vector<int> starts;
+  for (int r = 0; r < N; ++r) {
+    if (!cut[r]) continue;
+    if (nd[r].depth < K) {
+      // a piece rooted above depth K: no window ends up there, so each of its nodes at depth K opens an item
+      // (terminals above depth K are counted by shallow_kernel)
+      starts.clear();
+      em.at_depth_K(r, &starts);
+      for (int d : starts) {
+        const int64_t f = (int64_t)pr.entries.size();
+        em.emit_item(d, true);
+        push_item_c(pr, f, o, cls);
       }
-      if (r == 0 && o != 0 && psize[0] == 1) continue;   // plain program: v = 0 is counted in octant 0 only
-      const int64_t first = (int64_t)pr.entries.size();
-      em.emit_item(r, !(r == 0 && o != 0));
-      push_item(pr, first, o);
+      continue;
     }
-    pr.n_slots = std::max(pr.n_slots, em.max_slots);
+    if (r == 0 && o != 0 && psize[0] == 1) continue;   // plain program: v = 0 is counted in octant 0 only
+    const int64_t first = (int64_t)pr.entries.size();
+    em.emit_item(r, !(r == 0 && o != 0));
+    push_item_c(pr, first, o, cls);
+  }
+  pr.n_slots = std::max(pr.n_slots, em.max_slots);
+}
+
+// Level K >= 1: the vectors of an octant (those of at least K steps), sorted by slope, are cut into CLASSES whose paths
+// use at most pr.n_planes step patterns between them (a digital straight segment has at most K + 1 patterns of length K,
+// neighbouring slopes share most of them); every class gets its own prefix trie.  The short common trunk of the octant
+// is walked once per class instead of once: a fraction of a percent of the entries.
+static void build_class_tries(const lpf_paths* p, int o, int piece_nodes, Program& pr) {
+  const int K = pr.K;
+  const std::vector<Node>& nd = p->oct[o];
+  const int N = (int)nd.size();
+  // patterns of the last K steps at every node, and the union over the path root -> node
+  std::vector<uint8_t> pat(N, 0);
+  std::vector<uint64_t> pathset(N, 0);
+  for (int i = 1; i < N; ++i) {
+    const int par = nd[i].parent;
+    pat[i] = (uint8_t)((pat[par] >> 1) | ((nd[i].b - nd[par].b) << (K - 1)));
+    pathset[i] = pathset[par];
+    if (nd[i].depth >= K) pathset[i] |= 1ull << balanced_rank(pat[i], K);
+  }
+  std::vector<int> terms;
+  for (int i = 0; i < N; ++i)
+    if (nd[i].terminal && nd[i].depth >= K) terms.push_back(i);
+  std::sort(terms.begin(), terms.end(), [&](int x, int y) {          // by slope b / a, then by length
+    const long long l = (long long)nd[x].b * nd[y].a, r = (long long)nd[y].b * nd[x].a;
+    if (l != r) return l < r;
+    return nd[x].a < nd[y].a;
+  });
+  std::vector<int16_t> vxy(2 * (size_t)(p->m + 1));
+  size_t t0 = 0;
+  while (t0 < terms.size()) {
+    uint64_t set = 0;
+    size_t t1 = t0;
+    while (t1 < terms.size() && __builtin_popcountll(set | pathset[terms[t1]]) <= pr.n_planes) set |= pathset[terms[t1++]];
+    if (t1 == t0) return;                                  // cannot happen: n_planes >= the patterns of any one path
+    Program::Class c;
+    c.octant = o;
+    std::memset(c.slot_of, -1, sizeof(c.slot_of));
+    std::memset(c.pattern, 0, sizeof(c.pattern));
+    for (unsigned q = 0; q < (1u << K); ++q) {
+      if (!balanced_word(q, K)) continue;
+      const int rank = balanced_rank(q, K);
+      if (!((set >> rank) & 1ull)) continue;
+      c.slot_of[rank] = (signed char)c.n;
+      c.pattern[c.n++] = (int)q;
+    }
+    std::vector<Node> cnd;
+    cnd.push_back(Node{0, 0, -1, -1, -1, 1, 0, 0});
+    for (size_t t = t0; t < t1; ++t) {
+      int len = 0;
+      for (int u = terms[t]; u >= 0; u = nd[u].parent) ++len;
+      int k = len;
+      for (int u = terms[t]; u >= 0; u = nd[u].parent) {
+        --k;
+        vxy[2 * k] = nd[u].a;
+        vxy[2 * k + 1] = nd[u].b;
+      }
+      trie_insert(cnd, vxy.data(), len);
+    }
+    for (int i = (int)cnd.size() - 1; i > 0; --i) cnd[cnd[i].parent].size += cnd[i].size;
+    const int cls = (int)pr.classes.size();
+    pr.classes.push_back(c);
+    emit_trie(p, o, cnd, piece_nodes, pr, pr.classes[cls].slot_of, cls);
+    t0 = t1;
+  }
+}
+
+static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
+  for (int o = 0; o < 4; ++o) {
+    if (pr.K == 0) emit_trie(p, o, p->oct[o], piece_nodes, pr, nullptr, 0);
+    else build_class_tries(p, o, piece_nodes, pr);
   }
   sort_items(pr);
+}
+
+// The highest level (<= MAX_LEVEL) at which every window of every path is a balanced word, and for every level the
+// largest number of different patterns on one path (a class needs that many planes at least; K + 1 for a digital
+// straight segment).
+static void analyse_levels(lpf_paths* p) {
+  int ok = MAX_LEVEL;
+  for (int o = 0; o < 4; ++o) {
+    const std::vector<Node>& nd = p->oct[o];
+    std::vector<uint8_t> pat(nd.size(), 0);                // last MAX_LEVEL steps, newest in the top bit
+    for (size_t i = 1; i < nd.size(); ++i) {
+      const int par = nd[i].parent;
+      pat[i] = (uint8_t)((pat[par] >> 1) | ((nd[i].b - nd[par].b) << (MAX_LEVEL - 1)));
+      for (int K = 2; K <= std::min<int>(ok, nd[i].depth); ++K)
+        if (!balanced_word((unsigned)pat[i] >> (MAX_LEVEL - K), K)) ok = K - 1;
+    }
+  }
+  p->level_ok = ok;
+  for (int K = 0; K <= MAX_LEVEL; ++K) p->path_patterns[K] = 0;
+  for (int K = 1; K <= ok; ++K)
+    for (int o = 0; o < 4; ++o) {
+      const std::vector<Node>& nd = p->oct[o];
+      std::vector<uint8_t> pat(nd.size(), 0);
+      std::vector<uint64_t> pathset(nd.size(), 0);
+      for (size_t i = 1; i < nd.size(); ++i) {
+        const int par = nd[i].parent;
+        pat[i] = (uint8_t)((pat[par] >> 1) | ((nd[i].b - nd[par].b) << (K - 1)));
+        pathset[i] = pathset[par];
+        if (nd[i].depth >= K) pathset[i] |= 1ull << balanced_rank(pat[i], K);
+        if (nd[i].terminal) p->path_patterns[K] = std::max(p->path_patterns[K], __builtin_popcountll(pathset[i]));
+      }
+    }
 }
 
 // the terminals above depth K of every octant trie, with their paths as step patterns (level K only)
@@ -344,6 +452,7 @@ void shallow_terminals(const lpf_paths* p, int K, ShallowList* out) {
       int ia, ib;
       from_view(o, nd[i].a, nd[i].b, &ia, &ib);
       const int k = out->n[o]++;
+      if (k >= MAX_SHALLOW) { --out->n[o]; continue; }   // cannot happen: K <= MAX_LEVEL
       out->cidx[o][k] = (ib + m) * (2 * m + 1) + (ia + m);
       out->depth[o][k] = nd[i].depth;
       out->steps[o][k] = steps;
@@ -448,19 +557,21 @@ static void build_s2_program(lpf_paths* p, int piece_nodes, Program& pr) {
   sort_items(pr);
 }
 
-Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int K, int bw03,
-                     int bw12) {
+Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int K, int n_planes,
+                     int bw03, int bw12) {
   if (piece_nodes < 0) piece_nodes = 0;
   const unsigned kind = (flags & LPF_S2) ? LPF_S2 : (flags & LPF_NO_TRIE);
   if (kind != 0) K = 0;                                    // the eroded planes serve the trie program only
-  if (K == 0) bw03 = bw12 = 0;
-  const std::tuple<int, unsigned, int, int, int, int, int> key(piece_nodes, kind, stride03, stride12, K, bw03, bw12);
+  if (K == 0) bw03 = bw12 = n_planes = 0;
+  const std::tuple<int, unsigned, int, int, int, int, int> key(piece_nodes, kind, stride03, stride12, 100 * K + n_planes,
+                                                               bw03, bw12);
   auto it = p->programs.find(key);
   if (it != p->programs.end()) return it->second;
   Program& pr = p->programs[key];
   pr.stride[0] = pr.stride[3] = stride03;
   pr.stride[1] = pr.stride[2] = stride12;
   pr.K = K;
+  pr.n_planes = n_planes;
   pr.band_words[0] = pr.band_words[3] = bw03;
   pr.band_words[1] = pr.band_words[2] = bw12;
   if (flags & LPF_S2) build_s2_program(p, piece_nodes, pr);
@@ -480,6 +591,7 @@ void drop_program(lpf_paths* p, const Program* pr) {
 int build_host_table(lpf_paths* p) {
   try {
     build_trie(p);
+    analyse_levels(p);
   } catch (const std::bad_alloc&) {
     return LPF_E_NOMEM;
   }
@@ -495,7 +607,7 @@ int build_host_table(lpf_paths* p) {
 namespace lpf {
 
 static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int K,
-                              Geom* out);
+                              int min_planes, Geom* out);
 
 // Resident warps per SM of a geometry once the CTA is made of teams (lpf_api.cu picks the team count with the
 // occupancy API; this is the same search on a model: 64 registers per thread, i.e. at most 1024 threads per SM).
@@ -512,12 +624,13 @@ static int resident_warps(const Geom& g, int max_smem, int max_teams, int* teams
   return best;
 }
 
-// Relative cost of a geometry: program entries at level K (measured on the tries of m = 64 .. 256: 1.9 : 1 : 0.70 :
-// 0.57 for K = 0 .. 3; a little is added for the higher levels, whose entries reload their row strip more often)
+// Relative cost of a geometry: program entries at level K (counted on the tries of m = 64 .. 256: 1.9 : 1 : 0.70 :
+// 0.57 : 0.47 : 0.40 : 0.35 for K = 0 .. 6; a little is added for the higher levels, whose entries reload their row
+// strip more often, and for pattern classes, each of which walks the trunk of its octant again)
 // over the throughput at the resident warps (measured on config 3: 8 warps 0.57, 16 warps 0.87, 24 warps 0.985 of
 // the rate at 32).
 static double geom_cost(const Geom& g, int max_smem, int max_teams) {
-  static const double entries[MAX_LEVEL + 1] = {1.9, 1.0, 0.73, 0.61};
+  static const double entries[MAX_LEVEL + 1] = {1.9, 1.0, 0.73, 0.61, 0.50, 0.44, 0.39};
   const int w = resident_warps(g, max_smem, max_teams, nullptr);
   double rate;
   if (w >= 32) rate = 1.0;
@@ -525,7 +638,8 @@ static double geom_cost(const Geom& g, int max_smem, int max_teams) {
   else if (w >= 16) rate = 0.87 + 0.115 * (w - 16) / 8.0;
   else if (w >= 8) rate = 0.57 + 0.30 * (w - 8) / 8.0;
   else rate = 0.57 * w / 8.0;
-  return entries[g.K] / std::max(rate, 1e-3);
+  const double classes = (g.K > 0 && g.v[0].n_planes < balanced_count(g.K)) ? 1.03 : 1.0;
+  return entries[g.K] * classes / std::max(rate, 1e-3);
 }
 
 // teams that find work on one key: two pieces of at least 256 trie nodes each per team and octant
@@ -540,8 +654,8 @@ int max_teams_of(const lpf_paths* p) {
 // 4.10 / 5.42 / 4.57 / 4.57 ms: small keys balance better and leave room for a higher level); a later candidate or a
 // lower level must win by more than 3 %.
 bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int max_level, int max_teams,
-                 Geom* out) {
-  max_level = std::max(0, std::min({max_level, MAX_LEVEL, m}));
+                 const int* path_patterns, Geom* out) {
+  max_level = std::max(0, std::min({max_level, MAX_LEVEL, m}));   // the caller caps it at the table's level_ok
   double best = 0;
   bool found = false;
   static const int team_warps[4] = {2, 1, 4, 8};
@@ -550,7 +664,7 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int c
       const int cw = team_warps[ci];
       if (cta_warps >= 1 && cta_warps <= 8 && cw != cta_warps) continue;
       Geom g;
-      if (!choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cw, K, &g)) continue;
+      if (!choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cw, K, path_patterns[K], &g)) continue;
       const double c = geom_cost(g, max_smem, max_teams);
       if (!found || c < best * 0.97) {
         best = c;
@@ -562,11 +676,11 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int c
 }
 
 static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int K,
-                              Geom* out) {
+                              int min_planes, Geom* out) {
   Geom g;
   std::memset(&g, 0, sizeof(g));
   g.H = H; g.W = W; g.m = m; g.K = K;
-  const int n_planes = K > 0 ? (1 << K) : 0;
+  const int planes_all = K > 0 ? balanced_count(K) : 0;
   const int wc_max = (std::max(H, W) + 31) / 32;
   if (tx > 0 && ty > 0) {
     g.TX = tx; g.TY = ty;
@@ -602,20 +716,29 @@ static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, 
       v.n_bands = (v.Hv + g.band_rows - 1) / g.band_rows;
       v.band_words = ((g.band_rows + m) * v.stride + 3) / 4 * 4;
       v.plane_words = ((v.n_bands * g.band_rows + m) * v.stride + 3) / 4 * 4 + 4;
-      v.n_planes = n_planes;
-      v.band_pitch = std::max(n_planes, 1) * v.band_words;
-      v.view_words = (1 + n_planes) * v.plane_words;       // level K packs the plain view, then the 2^K eroded views
-      bw_max = std::max(bw_max, v.band_pitch);
+      v.view_words = v.plane_words;                         // only the plain view is kept in HBM
+      bw_max = std::max(bw_max, v.band_words);
     }
-    const size_t per_image = (size_t)bw_max * 4;     // shared memory holds the G bands only
-    if (per_image + 1024 <= (size_t)max_smem) {
+    // level K: as many planes per pattern class as fit beside the plain band they are derived from (all balanced
+    // patterns if possible); a class needs room for the patterns of one path (K + 1 for a digital straight segment)
+    int n_planes = 0;
+    if (K > 0) {
+      n_planes = std::min(planes_all, (int)(((size_t)max_smem - 1024) / ((size_t)bw_max * 4)) - 1);
+      if (n_planes < std::min(planes_all, std::max(min_planes, K + 1))) n_planes = -1;
+    }
+    if (n_planes >= 0) {
+      for (int o = 0; o < 4; ++o) {
+        g.v[o].n_planes = n_planes;
+        g.v[o].band_pitch = (n_planes ? n_planes + 1 : 1) * g.v[o].band_words;
+      }
+      const size_t per_image = (size_t)(n_planes ? n_planes + 1 : 1) * bw_max * 4;   // shared memory holds the G bands
       int G = std::max(1, cta_warps / g.wpi);
       G = std::min(G, std::max(B, 1));
       G = (int)std::min<size_t>((size_t)G, ((size_t)max_smem - 1024) / per_image);
       g.G = std::max(G, 1);
       g.NT = 1;
       g.threads = g.G * g.wpi * 32;
-      g.smem_bytes = g.G * bw_max * 4;
+      g.smem_bytes = (int)(g.G * per_image);
       break;
     }
     if (row_blocks == 1) return false;
@@ -678,22 +801,32 @@ extern "C" int lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, in
 
 extern "C" int lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, unsigned flags, uint64_t* entries,
                                  int64_t cap_entries, int64_t* n_entries, int64_t* items, int64_t cap_items,
-                                 int64_t* n_items, int* n_slots, int* strides) {
-  if (!p || !n_entries || !n_items || !n_slots || !strides) return LPF_E_INVAL;
+                                 int64_t* n_items, int* n_slots, int* layout) {
+  if (!p || !n_entries || !n_items || !n_slots || !layout) return LPF_E_INVAL;
   if (H < 1 || W < 1 || p->m > std::min(H, W) - 1) return LPF_E_INVAL;
   lpf::Geom g;
-  const int max_level = (flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2)) ? 0 : (p->max_level >= 0 ? p->max_level : lpf::MAX_LEVEL);
+  const int max_level = (flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2))
+                            ? 0
+                            : std::min(p->level_ok, p->max_level >= 0 ? p->max_level : lpf::MAX_LEVEL);
   if (!lpf::choose_geom(p->m, H, W, 1, p->max_smem > 0 ? p->max_smem : 232448, p->tile_tx, p->tile_ty, p->cta_warps,
-                        max_level, lpf::max_teams_of(p), &g))
+                        max_level, lpf::max_teams_of(p), p->path_patterns, &g))
     return LPF_E_UNSUPPORTED;
   try {
-    lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride, g.K, g.v[0].band_words,
-                                        g.v[1].band_words);
+    lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride, g.K, g.v[0].n_planes,
+                                        g.v[0].band_words, g.v[1].band_words);
     *n_entries = (int64_t)pr.entries.size();
     *n_items = (int64_t)pr.items.size() / 4;
     *n_slots = pr.n_slots;
-    for (int o = 0; o < 4; ++o) { strides[o] = pr.stride[o]; strides[4 + o] = pr.band_words[o]; }
-    strides[8] = pr.K;
+    if (pr.classes.size() > LPF_LAYOUT_MAX_CLASSES) return LPF_E_UNSUPPORTED;
+    for (int o = 0; o < 4; ++o) { layout[o] = pr.stride[o]; layout[4 + o] = pr.band_words[o]; }
+    layout[8] = pr.K;
+    layout[9] = (int)pr.classes.size();
+    for (size_t c = 0; c < pr.classes.size(); ++c) {
+      int* out = layout + 10 + (2 + lpf::MAX_PATTERNS) * c;
+      out[0] = pr.classes[c].octant;
+      out[1] = pr.classes[c].n;
+      for (int k = 0; k < lpf::MAX_PATTERNS; ++k) out[2 + k] = k < pr.classes[c].n ? pr.classes[c].pattern[k] : -1;
+    }
     if (entries) {
       if (cap_entries < *n_entries) return LPF_E_INVAL;
       std::memcpy(entries, pr.entries.data(), sizeof(uint64_t) * pr.entries.size());

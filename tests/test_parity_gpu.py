@@ -205,7 +205,7 @@ def test_config3_whole_template_against_the_oracle_digest():
         bad = [(ph, r) for ph in (0, 1) for r in range(2 * m + 1) if crc(got[ph, r]) != rows[(ph, r)]]
         assert not bad, (flags, bad[:10])
         assert sha(got) == want_sha, flags
-        assert lpf.lpf_last_launch_info(paths(m))["level"] == (0 if flags & lpf.LPF_NO_E2 else 3)
+        assert lpf.lpf_last_launch_info(paths(m))["level"] == (0 if flags & lpf.LPF_NO_E2 else 6)
 
 
 def test_config4_sampled_images_properties_and_objective():
@@ -573,13 +573,14 @@ def test_every_erosion_level_and_team_count_at_full_size():
     than K are counted by their own kernel) against the oracle, both phases, plus Eq. 10 / Eq. 12."""
     cases = [(256, 384, 120, lpf.LPF_NO_E2, -1, 0, 0), (256, 384, 120, 0, 0, 0, 0), (256, 384, 120, 0, 1, 0, 1),
              (256, 384, 120, 0, 2, 0, 2), (256, 384, 120, 0, 3, 0, 3), (256, 384, 120, 0, -1, 1, None),
+             (256, 384, 120, 0, 4, 0, 4), (256, 384, 120, 0, 5, 0, 5), (256, 384, 120, 0, 6, 0, 6),
              (256, 384, 120, 0, 2, 3, 2), (300, 300, 299, 0, -1, 0, None), (300, 300, 299, 0, 0, 0, 0)]
     for H, W, m, flags, level, teams, want_level in cases:
         img = inputs.disks(H, W, 7.0, 0.45, inputs.seed_for(8, H + m))
         rng = np.random.default_rng(m)
         vecs = rng.integers(-m, m + 1, size=(300, 2))
         vecs[:6] = [(0, 0), (m, m), (-m, m), (m, 0), (0, m), (-m, 1)]
-        short = np.array([(dx, dy) for dy in range(-3, 4) for dx in range(-3, 4)])
+        short = np.array([(dx, dy) for dy in range(-6, 7) for dx in range(-6, 7)])
         vecs = np.concatenate([vecs, short])
         p = lpf.lpf_build_paths(m, 0)
         try:
@@ -592,10 +593,10 @@ def test_every_erosion_level_and_team_count_at_full_size():
         if want_level is not None:
             assert info["level"] == want_level, (H, W, m, flags, level, info)
         else:
-            assert 1 <= info["level"] <= 3, info
+            assert 1 <= info["level"] <= 6, info
         if teams:
             assert info["teams"] == teams
-        assert info["shallow_vectors"] == [0, 1, 5, 13][info["level"]]
+        assert info["shallow_vectors"] == [0, 1, 5, 13, 25, 41, 61][info["level"]]
         for phase in (0, 1):
             want, _ = orc.counts_list(img, phase, vecs)
             assert np.array_equal(got[phase][vecs[:, 1] + m, vecs[:, 0] + m], want), (H, W, m, flags, level, phase)

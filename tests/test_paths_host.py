@@ -95,7 +95,7 @@ def _decode(entries):
     y = (entries >> np.uint64(32)).astype(np.int64)
     return dict(sh=x & 31, reload=(x >> 5) & 1, terminal=(x >> 6) & 1, save=(x >> 7) & 1, restore=(x >> 8) & 1,
                 init=(x >> 9) & 1, pair=(x >> 10) & 1, eroded=(x >> 11) & 1, off=x >> 12, cidx=y & ((1 << 20) - 1),
-                rslot=(y >> 20) & 7, sslot=(y >> 23) & 7, q=(y >> 26) & 7, back=(y >> 29) & 3)
+                rslot=(y >> 20) & 7, sslot=(y >> 23) & 7, q=(y >> 26) & 63)
 
 
 def _from_view(o, a, b):
@@ -103,10 +103,22 @@ def _from_view(o, a, b):
     return [(a, b), (b, a), (-b, a), (-a, b)][o]
 
 
+def _balanced(q, K):
+    """Any two factors of equal length of the K-step pattern differ by at most one in their number of down steps."""
+    bits = [(q >> j) & 1 for j in range(K)]
+    for L in range(1, K + 1):
+        sums = [sum(bits[s:s + L]) for s in range(K - L + 1)]
+        if max(sums) - min(sums) > 1:
+            return False
+    return True
+
+
 @pytest.mark.parametrize("m,H,W,piece,flags,level", [
     (5, 8, 8, 0, 0, -1), (12, 40, 100, 16, 0, -1), (33, 64, 64, 256, 0, -1), (70, 300, 128, 512, 0, -1),
     (12, 40, 100, 16, 0, 1), (33, 64, 64, 256, 0, 2), (33, 64, 64, 64, 0, 3), (70, 300, 128, 512, 0, 1),
-    (2, 8, 9, 0, 0, 3), (3, 8, 9, 4, 0, 3), (1, 5, 5, 0, 0, -1),
+    (33, 64, 64, 64, 0, 4), (60, 64, 64, 256, 0, 5), (60, 64, 64, 256, 0, 6), (100, 512, 512, 512, 0, 6),
+    (100, 128, 128, 512, 0, 6),
+    (2, 8, 9, 0, 0, 3), (3, 8, 9, 4, 0, 3), (1, 5, 5, 0, 0, -1), (7, 9, 8, 0, 0, 6),
     (12, 13, 13, 0, lpf.LPF_NO_TRIE, -1), (12, 64, 32, 64, lpf.LPF_NO_TRIE, -1), (33, 64, 64, 256, lpf.LPF_NO_E2, -1),
     (40, 41, 97, 64, lpf.LPF_NO_E2, -1), (33, 64, 64, 256, 0, 0)])
 def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags, level):
@@ -127,14 +139,30 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
         if m >= 12:
             assert K == level                                # these shapes are small: every level fits
     else:
-        assert 1 <= K <= min(3, m)                           # the default program is an eroded one
+        assert 1 <= K <= min(6, m)                           # the default program is an eroded one
+    # pattern classes: slope sectors of one octant; the patterns of a class are balanced words, one plane slot each
+    n_classes = strides[9]
+    classes = []
+    for c in range(n_classes):
+        rec = strides[10 + 38 * c: 10 + 38 * (c + 1)]
+        octant, n = rec[0], rec[1]
+        pats = rec[2:2 + n]
+        assert 0 <= octant < 4 and 1 <= n <= 36 and len(set(pats)) == n
+        assert all(0 <= q < (1 << K) and _balanced(q, K) for q in pats)
+        assert all(q == -1 for q in rec[2 + n:])
+        classes.append((octant, pats))
+    assert (n_classes > 0) == (K > 0)
+    if (m, H, W, level) == (100, 512, 512, 6):
+        assert n_classes > 4                                 # a band of this shape has room for few planes: several classes
     S = 2 * m + 1
     seen = {}
     covered = np.zeros(len(entries), dtype=bool)
     assert n_slots <= 8
-    for first, cnt, o, _ in items:
+    for first, cnt, o, cls in items:
         cur, stack, held = None, {}, None
         assert strides[o] % 2 == 1
+        if K:
+            assert classes[cls][0] == o
         for e in range(first, first + cnt):
             assert not covered[e]
             covered[e] = True
@@ -145,23 +173,29 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
                 cur = list(stack[int(d["rslot"][e])])
             assert cur is not None
             assert bool(d["eroded"][e]) == (K > 0)
-            q, back = int(d["q"][e]), int(d["back"][e])
-            assert q < (1 << K) and back <= K
-            bv, col = divmod(int(d["off"][e]) - q * strides[4 + o], strides[o])
+            q = int(d["q"][e])
+            slot, rem = divmod(int(d["off"][e]), strides[4 + o]) if K else (0, int(d["off"][e]))
+            if K:
+                assert classes[cls][1][slot] == q            # the plane slot holds the entry's pattern
+            bv, col = divmod(rem, strides[o])
             av = col * 32 + int(d["sh"][e])
-            plane = q if K else -1
+            plane = slot if K else -1
             if d["reload"][e]:
                 held = (bv, col, plane)
             assert held == (bv, col, plane), "stale row strip"
-            window = [(av, bv)]                              # the K + 1 pixels of plane q at (av, bv)
+            window = [(av, bv)]                              # the K + 1 pixels of the plane of pattern q at (av, bv)
             for j in range(1, K + 1):
                 window.append((window[-1][0] + 1, window[-1][1] + ((q >> (j - 1)) & 1)))
             for a, b in window:
                 assert 0 <= b <= a <= m
             window = [_from_view(o, a, b) for a, b in window]
+            # the first pixels of a window may be nodes that are already in the mask: as many as the list is longer than
+            # the window's first column
+            back = len(cur) - av
+            assert 0 <= back <= K
             if d["init"][e]:
                 assert back == 0 and window[0] == (0, 0)     # every item starts at the root with a full window
-            assert back == 0 or cur[-back:] == window[:back]  # pixels that are already in the mask
+            assert back == 0 or cur[-back:] == window[:back]
             cur = cur + window[back:]
             if d["terminal"][e]:
                 cidx = int(d["cidx"][e])
