@@ -142,6 +142,25 @@ void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec) {
 
 // ---- program emission ----------------------------------------------------------------------
 
+// balanced_word / balanced_rank (lpf_kernels.cuh) as tables: the host asks for them once per trie node
+struct PatternTables {
+  uint8_t ok[MAX_LEVEL + 1][1 << MAX_LEVEL];
+  int8_t rank[MAX_LEVEL + 1][1 << MAX_LEVEL];
+  PatternTables() {
+    for (int K = 0; K <= MAX_LEVEL; ++K) {
+      int r = 0;
+      for (unsigned q = 0; q < (1u << MAX_LEVEL); ++q) {
+        ok[K][q] = (q < (1u << K)) && balanced_word(q, K);
+        rank[K][q] = (int8_t)(ok[K][q] ? r++ : -1);
+      }
+    }
+  }
+};
+static const PatternTables& pattern_tables() {
+  static const PatternTables t;
+  return t;
+}
+
 struct Held {            // the row strip that is in the registers when an entry runs
   int b = -1, col = -1, plane = -1;
 };
@@ -177,7 +196,7 @@ struct Emitter {
       anchor = par;
     }
     const int a = nd[anchor].a, b = nd[anchor].b;
-    const int plane = K > 0 ? (int)slot_of[balanced_rank(q, K)] : -1;   // >= 0: the class holds every pattern of its paths
+    const int plane = K > 0 ? (int)slot_of[pattern_tables().rank[K][q]] : -1;   // >= 0: the class holds every pattern of its paths
     const bool direct = !(flags & (E_RESTORE | E_INIT));
     if (!direct || held->b != b || held->col != (a >> 5) || held->plane != plane) flags |= E_RELOAD;
     held->b = b; held->col = a >> 5; held->plane = plane;
@@ -349,7 +368,7 @@ static void build_class_tries(const lpf_paths* p, int o, int piece_nodes, Progra
     const int par = nd[i].parent;
     pat[i] = (uint8_t)((pat[par] >> 1) | ((nd[i].b - nd[par].b) << (K - 1)));
     pathset[i] = pathset[par];
-    if (nd[i].depth >= K) pathset[i] |= 1ull << balanced_rank(pat[i], K);
+    if (nd[i].depth >= K) pathset[i] |= 1ull << pattern_tables().rank[K][pat[i]];
   }
   std::vector<int> terms;
   for (int i = 0; i < N; ++i)
@@ -371,8 +390,8 @@ static void build_class_tries(const lpf_paths* p, int o, int piece_nodes, Progra
     std::memset(c.slot_of, -1, sizeof(c.slot_of));
     std::memset(c.pattern, 0, sizeof(c.pattern));
     for (unsigned q = 0; q < (1u << K); ++q) {
-      if (!balanced_word(q, K)) continue;
-      const int rank = balanced_rank(q, K);
+      if (!pattern_tables().ok[K][q]) continue;
+      const int rank = pattern_tables().rank[K][q];
       if (!((set >> rank) & 1ull)) continue;
       c.slot_of[rank] = (signed char)c.n;
       c.pattern[c.n++] = (int)q;
@@ -418,7 +437,7 @@ static void analyse_levels(lpf_paths* p) {
       const int par = nd[i].parent;
       pat[i] = (uint8_t)((pat[par] >> 1) | ((nd[i].b - nd[par].b) << (MAX_LEVEL - 1)));
       for (int K = 2; K <= std::min<int>(ok, nd[i].depth); ++K)
-        if (!balanced_word((unsigned)pat[i] >> (MAX_LEVEL - K), K)) ok = K - 1;
+        if (!pattern_tables().ok[K][(unsigned)pat[i] >> (MAX_LEVEL - K)]) ok = K - 1;
     }
   }
   p->level_ok = ok;
@@ -432,7 +451,7 @@ static void analyse_levels(lpf_paths* p) {
         const int par = nd[i].parent;
         pat[i] = (uint8_t)((pat[par] >> 1) | ((nd[i].b - nd[par].b) << (K - 1)));
         pathset[i] = pathset[par];
-        if (nd[i].depth >= K) pathset[i] |= 1ull << balanced_rank(pat[i], K);
+        if (nd[i].depth >= K) pathset[i] |= 1ull << pattern_tables().rank[K][pat[i]];
         if (nd[i].terminal) p->path_patterns[K] = std::max(p->path_patterns[K], __builtin_popcountll(pathset[i]));
       }
     }
