@@ -79,6 +79,15 @@ def design_ops(w, launch):
     return w["B"] * w["n_phase"] * nw * per_word
 
 
+def design_smem_bytes(w, launch):
+    """Shared-memory bytes the DESIGN loads at minimum: an entry that changes row, word column or plane reloads its row
+    strip, TY * (TX + 1) words per thread for TX * TY start words (tile code = 1000 TX + 100 TY + slots), i.e.
+    (TX + 1) / TX words per start word; counted from the uploaded program (`reloads`), times start words, images, phases."""
+    tx = launch["tile"] // 1000
+    nw = w["H"] * w["W"] // 32
+    return w["B"] * w["n_phase"] * nw * launch["reloads"] * (tx + 1) / tx * 4.0
+
+
 def csrc_digest():
     """sha256 over the CUDA/C++ sources and the public header: the key of profiles/capture_index.csv, so that ncu
     figures are only quoted for the kernels they were captured from."""
@@ -375,7 +384,7 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
-    def measure(wl, steps, warmup, with_e2e, strong=False):
+    def measure(wl, steps, warmup, with_e2e, strong=False, level=-1):
         """Times `steps` steps of workload wl. Returns dict of results for this rank (max over ranks applied).
         strong: all ranks hold the same batch, rank r evaluates the images lpf_dist.shard_range(B, r, world) and the
         per-rank count slices are all-gathered (the one collective of the split path) inside the timed region."""
@@ -385,6 +394,7 @@ def main():
         imgs = imgs[b0:b1]
         B_loc = b1 - b0
         p = lpf.lpf_build_paths(wl["m"], local_rank)      # paper step 1: untimed
+        lpf.lpf_set_level(p, level)                       # -1: automatic (the design variants cap the erosion level)
         info = lpf.lpf_paths_info(p)
         d_imgs = torch.from_numpy(imgs).cuda()
         Sw = 2 * wl["m"] + 1
@@ -618,8 +628,9 @@ def main():
     tests_per_step = lpf_dist.sum_over_ranks(nominal_tests(dict(w, B=r["images_per_gpu"])), device="cuda")
     value = tests_per_step * args.steps / (r["total_ms"] * 1e-3)
     # roofline of the dominant kernel (eval): a UTILISATION of the ALU pipe -- the data operations the design executes
-    # at minimum (design_ops, from the uploaded program) over kernel time x derived ALU peak.  The survey's op model
-    # (more ops than the design needs since PAIR fusion and the eroded planes) is kept as frac_vs_survey_ops.
+    # at minimum (design_ops, from the uploaded program) over kernel time x derived ALU peak -- and, next to it, of the
+    # shared-memory pipe, which binds since the eroded planes (design_smem_bytes over kernel time x 128 B/clk/SM).  The
+    # survey's op model (more ops than the design needs) is kept as frac_vs_survey_ops.
     w_loc = dict(w, B=r["images_per_gpu"])               # the eval kernel of THIS rank (strong scaling: its shard)
     d_ops = design_ops(w_loc, r["launch"])
     s_ops = survey_ops(w_loc, r["info"])
@@ -631,6 +642,8 @@ def main():
     sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     peak_ops = SM_COUNT * ALU_LANES_PER_CLK_PER_SM * sm_max_mhz * 1e6
     achieved = d_ops / (r["kernel_ms"] * 1e-3)
+    smem_peak = SM_COUNT * 128.0 * sm_max_mhz * 1e6      # 32 banks x 4 B per clock and SM
+    smem_rate = design_smem_bytes(w_loc, r["launch"]) / (r["kernel_ms"] * 1e-3)
     measured = lpf.lpf_alu_peak(local_rank) if rank == 0 else None     # live LOP3 / SHF / pair-pattern / POPC rates
     cap = capture_lookup(args.workload, args.flags)                     # ncu --set full of THESE sources, or None
     line = {
@@ -645,6 +658,10 @@ def main():
                      "frac": achieved / peak_ops,
                      "traffic": None if cap is None else cap["dram_read_bytes"] + cap["dram_write_bytes"],
                      "frac_vs_survey_ops": s_ops / (r["kernel_ms"] * 1e-3) / peak_ops,
+                     "shared_memory": {"achieved": smem_rate / 1e12, "peak": smem_peak / 1e12, "unit": "TB/s",
+                                       "frac": smem_rate / smem_peak,
+                                       "how": "row-strip reloads of the uploaded program x (TX + 1) / TX words per start "
+                                              "word / kernel time; peak = 148 SM x 128 B/clk x sm_max_mhz"},
                      "ncu": cap, "csrc_sha256": csrc_digest(),
                      "peak_measured": None if measured is None else
                      {"lop3": measured["lop3"] / 1e12, "shf": measured["shf"] / 1e12,
@@ -658,8 +675,10 @@ def main():
                      "note": "frac = data ops the design executes at minimum (per start word: 2 SHF + 1 LOP3 per fused "
                              "pair of program entries, 1 SHF + 1 LOP3 per single entry, POPC + add per terminal; counted "
                              "from the uploaded program) / (kernel time x peak); frac_vs_survey_ops uses SURVEY 8(d)'s "
-                             "2 ops per word-node, which the design undercuts, and may exceed 1; `ncu` = pipe figures of "
-                             "a committed ncu capture of exactly these sources (profiles/capture_index.csv) or null"},
+                             "2 ops per word-node, which the design undercuts, and may exceed 1; shared_memory = the "
+                             "same kind of utilisation for the shared-memory pipe (the binding unit: every entry reloads "
+                             "a row strip); `ncu` = pipe figures of a committed ncu capture of exactly these sources "
+                             "(profiles/capture_index.csv) or null"},
         "e2e": {"value": tests_per_step / r["e2e_s"], "unit": UNIT, "h2d_bytes_per_step": r["e2e"]["h2d"],
                 "d2h_bytes_per_step": r["e2e"]["d2h"]},
         "gpu_launches": r["launches_per_step"] * args.steps,
@@ -677,14 +696,17 @@ def main():
             extra[name] = {"value": nominal_tests(wl) * k / (rr["total_ms"] * 1e-3), "unit": UNIT,
                            "ms_per_step": rr["total_ms"] / k, "kernel_ms": rr["kernel_ms"],
                            "roofline_frac": design_ops(wl, rr["launch"]) / (rr["kernel_ms"] * 1e-3) / peak_ops,
+                           "smem_frac": design_smem_bytes(wl, rr["launch"]) / (rr["kernel_ms"] * 1e-3) / smem_peak,
+                           "level": rr["launch"]["level"], "classes": rr["launch"]["classes"],
                            "frac_vs_survey_ops": survey_ops(wl, rr["info"]) / (rr["kernel_ms"] * 1e-3) / peak_ops,
                            "ncu": cap2}
         # the design variants the north star asks to compare, eval kernel alone on the headline workload
         variants = {}
-        for vname, vflags in (("trie_pair_e2", 0), ("trie_no_e2", lpf.LPF_NO_E2), ("trie_prune", lpf.LPF_PRUNE),
-                              ("one_chain_per_path", lpf.LPF_NO_TRIE)):
+        for vname, vflags, vlevel in (("trie_default", 0, -1), ("trie_level3", 0, 3), ("trie_level2", 0, 2),
+                                      ("trie_level1", 0, 1), ("trie_no_e2", lpf.LPF_NO_E2, -1),
+                                      ("trie_prune", lpf.LPF_PRUNE, -1), ("one_chain_per_path", lpf.LPF_NO_TRIE, -1)):
             flags_saved, flags = flags, vflags
-            variants[vname + "_kernel_ms"] = measure(w, 3, 1, False)["kernel_ms"]
+            variants[vname + "_kernel_ms"] = measure(w, 3, 1, False, level=vlevel)["kernel_ms"]
             flags = flags_saved
         extra["variants_" + args.workload] = variants
         extra["cfg5"] = measure_swaps()

@@ -240,9 +240,10 @@ int  lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, int H, int W
  * per team, the erosion level K of the program (0: the plain plane); then what the walker executes per image-phase and
  * per start WORD, counted by replaying its loop over the program on the host: pairs of entries folded into one
  * 3-input AND (2 SHF + 1 LOP3 each), entries executed on their own (1 SHF + 1 LOP3), terminal entries (1 POPC +
- * 1 add), the trie nodes per program piece; the teams per CTA, the CTAs resident per SM, and the vectors shorter than K
- * that the small extra kernel counts.  out = host int64[16]. */
-int  lpf_last_launch_info(const lpf_paths* p, int64_t* out16);
+ * 1 add), the trie nodes per program piece; the teams per CTA, the CTAs resident per SM, the vectors shorter than K
+ * that the small extra kernel counts, the entries that reload their row strip from shared memory (TY * (TX + 1) 32-bit
+ * loads per thread each) and the number of pattern classes.  out = host int64[18]. */
+int  lpf_last_launch_info(const lpf_paths* p, int64_t* out18);
 
 /* Measurement hook: with enable != 0 every lpf_eval / lpf_eval_both on this object
  * records one CUDA event before and one after the eval kernel (the dominant kernel) on the caller's

@@ -188,7 +188,7 @@ cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed,
                         int n_phase, int phase0, unsigned int* counter, int n_sm, cudaStream_t st);
 cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem, int max_smem, int* blocks_per_sm);
 cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st);
-cudaError_t launch_shallow(const EvalParams& p, const ShallowList& sl, cudaStream_t st);
+cudaError_t launch_shallow(const EvalParams& p, const ShallowList& sl, int n_sm, cudaStream_t st);
 cudaError_t launch_mirror(unsigned long long* counts, int S, long long n_arrays, int n_sm, cudaStream_t st);
 cudaError_t launch_objective(const long long* counts, const long long* target, int B, long long K,
                              unsigned long long* sse, int n_sm, cudaStream_t st);
@@ -337,10 +337,12 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
       const int n = (int)std::min<int64_t>(32, cnt - c0);
       for (int k = 0; k < n; ++k) {
         uint32_t x = (uint32_t)pr->entries[first + c0 + k];
+        if (x & E_RELOAD) ++pl.reloads;
         if ((x & E_PAIR) && k + 1 < n) {
           ++pl.fused_pairs;
           ++k;
           x = (uint32_t)pr->entries[first + c0 + k];
+          if (x & E_RELOAD) ++pl.reloads;
         } else {
           ++pl.singles;
         }
@@ -531,7 +533,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
     p->timed_once = 1;
   }
   const int n_shallow = pl.shallow.n[0] + pl.shallow.n[1] + pl.shallow.n[2] + pl.shallow.n[3];
-  if (n_shallow > 0) LPF_CUDA(launch_shallow(ep, pl.shallow, st));   // level K: the vectors shorter than K
+  if (n_shallow > 0) LPF_CUDA(launch_shallow(ep, pl.shallow, p->n_sm, st));   // level K: the vectors shorter than K
   LPF_CUDA(launch_mirror((unsigned long long*)counts, S, n_arrays, p->n_sm, st));
   LPF_CUDA(order.done());
 
@@ -552,6 +554,8 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   p->last_info[13] = pl.g.NT;
   p->last_info[14] = pl.occ;
   p->last_info[15] = n_shallow;
+  p->last_info[16] = pl.reloads;                         // entries that reload their row strip: TY * (TX + 1) LDS.32 each
+  p->last_info[17] = (int64_t)pl.pr->classes.size();     // pattern classes (all octants)
   return LPF_OK;
 }
 
@@ -649,9 +653,9 @@ extern "C" int lpf_last_eval_kernel_ms(const lpf_paths* p, float* ms) {
   return LPF_OK;
 }
 
-extern "C" int lpf_last_launch_info(const lpf_paths* p, int64_t* out16) {
-  if (!p || !out16) return LPF_E_INVAL;
-  std::memcpy(out16, p->last_info, sizeof(p->last_info));
+extern "C" int lpf_last_launch_info(const lpf_paths* p, int64_t* out18) {
+  if (!p || !out18) return LPF_E_INVAL;
+  std::memcpy(out18, p->last_info, sizeof(p->last_info));
   return LPF_OK;
 }
 

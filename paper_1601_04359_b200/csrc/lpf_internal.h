@@ -133,7 +133,7 @@ struct EvalPlan {
   size_t views_bytes = 0, base_words = 0, mask_views_bytes = 0, mask_base_bytes = 0, need = 0;
   // what the walker executes per image-phase and start word (lpf_last_launch_info): pairs of entries folded into one
   // 3-input AND, entries executed on their own, terminal entries (POPC + add), trie nodes per piece
-  int64_t fused_pairs = 0, singles = 0, terminals = 0, piece_nodes = 0;
+  int64_t fused_pairs = 0, singles = 0, terminals = 0, piece_nodes = 0, reloads = 0;
 };
 
 }  // namespace lpf
@@ -186,7 +186,7 @@ struct lpf_paths {
   int timed_once = 0;                // a timed eval has been issued: ev_start / ev_stop hold a measurement
   void* ev_start = nullptr;
   void* ev_stop = nullptr;
-  int64_t last_info[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+  int64_t last_info[18] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
 };
 
 namespace lpf {

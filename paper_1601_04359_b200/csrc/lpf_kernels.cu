@@ -527,11 +527,33 @@ __global__ void mirror_kernel(unsigned long long* counts, int S, long long n_arr
 
 // ---------------------------------------------------------------------------------------------
 // shallow vectors (level K >= 1): a window of the eroded program covers K + 1 path pixels, so the vectors whose paths
-// are shorter (depth < K in their octant trie: at most 1 + 2 + 3 of them per octant at K = 3) have no entry.  They are
-// counted here from the plain view in HBM: grid = (n_phase * B, 4 octants); a thread ANDs the plain word of 32 start
-// pixels with the windows of the following path pixels (funnel shifts over the halo), POPC, block reduce, one atomic.
+// are shorter (depth < K in their octant trie: at most 1 + 2 + .. + K of them per octant) have no entry.  They are
+// counted here from the plain view in HBM: grid = (n_phase * B, 4 octants, row chunks).  A thread loads the plain
+// words of 32 start pixels and of the K - 1 rows below and walks the prefix tree of the balanced step patterns with
+// compile-time recursion (one funnel shift + AND per edge, as derive_planes does); where a prefix is one of the
+// octant's short vectors (sl.node, a uniform test) it counts: POPC, warp reduce, one shared-memory atomic per warp.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) shallow_kernel(const EvalParams p, const ShallowList sl) {
+template <int J, unsigned PRE>
+__device__ __forceinline__ void shallow_rec(uint32_t acc, const uint32_t (&lo)[MAX_LEVEL], const uint32_t (&hi)[MAX_LEVEL],
+                                            int K, const signed char* node, int* s_cnt, bool lane0) {
+  const int t = node[shallow_base(J) + balanced_rank(PRE, J)];
+  if (t >= 0) {
+    const int c = __reduce_add_sync(0xffffffffu, __popc(acc));
+    if (lane0 && c) atomicAdd(&s_cnt[t], c);
+  }
+  if constexpr (J + 1 < MAX_LEVEL) {
+    if (J + 1 < K) {
+      constexpr int rho = popcount_c(PRE);
+      if constexpr (balanced_word(PRE, J + 1))
+        shallow_rec<J + 1, PRE>(acc & __funnelshift_r(lo[rho], hi[rho], J + 1), lo, hi, K, node, s_cnt, lane0);
+      if constexpr (balanced_word(PRE | (1u << J), J + 1))
+        shallow_rec<J + 1, (PRE | (1u << J))>(acc & __funnelshift_r(lo[rho + 1], hi[rho + 1], J + 1), lo, hi, K, node,
+                                              s_cnt, lane0);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256) shallow_kernel(const EvalParams p, const ShallowList sl, int rows_per_chunk) {
   const Geom& g = p.g;
   const int o = blockIdx.y;
   const int n = sl.n[o];
@@ -541,41 +563,34 @@ __global__ void __launch_bounds__(256) shallow_kernel(const EvalParams p, const 
   const uint32_t* plain = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b * v.view_words;
   const uint32_t* mask = p.mask ? p.mask + p.mask_off[o] : nullptr;
   const int stride = v.stride;
-  int c[MAX_SHALLOW];
+  __shared__ int s_cnt[MAX_SHALLOW];
+  if (threadIdx.x < MAX_SHALLOW) s_cnt[threadIdx.x] = 0;
+  __syncthreads();
+  const int r0 = blockIdx.z * rows_per_chunk, r1 = min(v.Hv, r0 + rows_per_chunk);
+  const int n_words = max(0, r1 - r0) * v.Wc;
+  const bool lane0 = (threadIdx.x & 31) == 0;
+  for (int base = 0; base < n_words; base += blockDim.x) {   // uniform trip count: the warp reduces together
+    const int idx = base + threadIdx.x;
+    uint32_t lo[MAX_LEVEL], hi[MAX_LEVEL];
 #pragma unroll
-  for (int t = 0; t < MAX_SHALLOW; ++t) c[t] = 0;
-  for (int idx = threadIdx.x; idx < v.Hv * v.Wc; idx += blockDim.x) {
-    const int r = idx / v.Wc, i = idx - r * v.Wc;
-    const int nb = v.Wv - 32 * i;
-    uint32_t w0 = plain[(size_t)r * stride + i] & (nb >= 32 ? 0xffffffffu : ((1u << nb) - 1u));
-    if (mask) w0 &= mask[(size_t)r * stride + i];
+    for (int rr = 0; rr < MAX_LEVEL; ++rr) lo[rr] = hi[rr] = 0u;
+    uint32_t w0 = 0u;
+    if (idx < n_words) {
+      const int r = r0 + idx / v.Wc, i = idx % v.Wc;
+      const int nb = v.Wv - 32 * i;
+      const uint32_t* q = plain + (size_t)r * stride + i;    // the view has m >= K - 1 halo rows below and one word right
 #pragma unroll
-    for (int t = 0; t < MAX_SHALLOW; ++t) {
-      if (t >= n) break;
-      uint32_t acc = w0;
-      int rr = r;
-      for (int j = 1; j <= sl.depth[o][t]; ++j) {
-        rr += (sl.steps[o][t] >> (j - 1)) & 1;
-        const uint32_t* q = plain + (size_t)rr * stride + i;
-        acc &= __funnelshift_r(q[0], q[1], j);
-      }
-      c[t] += __popc(acc);
+      for (int rr = 0; rr < MAX_LEVEL; ++rr)
+        if (rr < g.K) { lo[rr] = q[(size_t)rr * stride]; hi[rr] = q[(size_t)rr * stride + 1]; }
+      w0 = lo[0] & (nb >= 32 ? 0xffffffffu : ((1u << nb) - 1u));   // start pixels x' < Wv only
+      if (mask) w0 &= mask[(size_t)r * stride + i];
     }
-  }
-  __shared__ int ws[MAX_SHALLOW][8];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-  for (int t = 0; t < MAX_SHALLOW; ++t) {
-    const int s = __reduce_add_sync(0xffffffffu, c[t]);
-    if (lane == 0) ws[t][warp] = s;
+    shallow_rec<0, 0u>(w0, lo, hi, g.K, sl.node[o], s_cnt, lane0);
   }
   __syncthreads();
-  if (threadIdx.x < n) {
-    long long s = 0;
-    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) s += ws[threadIdx.x][w];
-    if (s) atomicAdd(p.counts + (size_t)b * p.image_stride + (size_t)plane * p.S * p.S + sl.cidx[o][threadIdx.x],
-                     (unsigned long long)s);
-  }
+  if (threadIdx.x < n && s_cnt[threadIdx.x])
+    atomicAdd(p.counts + (size_t)b * p.image_stride + (size_t)plane * p.S * p.S + sl.cidx[o][threadIdx.x],
+              (unsigned long long)s_cnt[threadIdx.x]);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -711,8 +726,15 @@ cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem,
   return cudaGetLastError();
 }
 
-cudaError_t launch_shallow(const EvalParams& p, const ShallowList& sl, cudaStream_t st) {
-  shallow_kernel<<<dim3((unsigned)(p.B * p.n_phase), 4u), 256, 0, st>>>(p, sl);
+cudaError_t launch_shallow(const EvalParams& p, const ShallowList& sl, int n_sm, cudaStream_t st) {
+  // row chunks: about two CTAs per SM in all
+  int hv_max = 0;
+  for (int o = 0; o < 4; ++o) hv_max = std::max(hv_max, p.g.v[o].Hv);
+  const long long blocks = (long long)p.B * p.n_phase * 4;
+  int nz = (int)std::max<long long>(1, std::min<long long>((2ll * n_sm + blocks - 1) / blocks, (hv_max + 7) / 8));
+  const int rows_per_chunk = (hv_max + nz - 1) / nz;
+  nz = (hv_max + rows_per_chunk - 1) / rows_per_chunk;
+  shallow_kernel<<<dim3((unsigned)(p.B * p.n_phase), 4u, (unsigned)nz), 256, 0, st>>>(p, sl, rows_per_chunk);
   return cudaGetLastError();
 }
 

@@ -91,11 +91,14 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int c
 
 // terminals above depth K have no program entry at level K (a window covers K + 1 pixels): shallow_kernel counts them
 constexpr int MAX_SHALLOW = 21;   // 1 + 2 + .. + MAX_LEVEL vectors of fewer than MAX_LEVEL steps per octant
+// prefix tree of the balanced step patterns of fewer than MAX_LEVEL steps: node (J steps, pattern PRE) has the index
+// shallow_base(J) + balanced_rank(PRE, J)
+LPF_HD constexpr int shallow_base(int J) { int b = 0; for (int j = 0; j < J; ++j) b += balanced_count(j); return b; }
+constexpr int SHALLOW_NODES = shallow_base(MAX_LEVEL);   // 1 + 2 + 4 + 8 + 14 + 24
 struct ShallowList {
-  int n[4];                      // per octant
-  int cidx[4][MAX_SHALLOW];      // index into counts[S][S]
-  int depth[4][MAX_SHALLOW];     // path length - 1 (< K)
-  int steps[4][MAX_SHALLOW];     // bit j-1: step j goes one view row down
+  int n[4];                          // vectors per octant
+  int cidx[4][MAX_SHALLOW];          // their index into counts[S][S]
+  signed char node[4][SHALLOW_NODES];// prefix-tree node -> position in the octant's list, or -1
 };
 
 struct EvalParams {

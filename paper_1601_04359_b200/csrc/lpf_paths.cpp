@@ -460,21 +460,21 @@ static void analyse_levels(lpf_paths* p) {
 // the terminals above depth K of every octant trie, with their paths as step patterns (level K only)
 void shallow_terminals(const lpf_paths* p, int K, ShallowList* out) {
   std::memset(out, 0, sizeof(*out));
+  std::memset(out->node, -1, sizeof(out->node));
   const int m = p->m;
   for (int o = 0; o < 4; ++o) {
     const std::vector<Node>& nd = p->oct[o];
     for (int i = 0; i < (int)nd.size(); ++i) {
       if (nd[i].depth >= K || !nd[i].terminal) continue;
-      int steps = 0;
+      unsigned steps = 0;
       for (int u = i; nd[u].parent >= 0; u = nd[u].parent)
-        steps |= (nd[u].b - nd[nd[u].parent].b) << (nd[u].depth - 1);
+        steps |= (unsigned)(nd[u].b - nd[nd[u].parent].b) << (nd[u].depth - 1);
       int ia, ib;
       from_view(o, nd[i].a, nd[i].b, &ia, &ib);
+      if (out->n[o] >= MAX_SHALLOW) continue;            // cannot happen: K <= MAX_LEVEL
       const int k = out->n[o]++;
-      if (k >= MAX_SHALLOW) { --out->n[o]; continue; }   // cannot happen: K <= MAX_LEVEL
       out->cidx[o][k] = (ib + m) * (2 * m + 1) + (ia + m);
-      out->depth[o][k] = nd[i].depth;
-      out->steps[o][k] = steps;
+      out->node[o][shallow_base(nd[i].depth) + pattern_tables().rank[nd[i].depth][steps]] = (signed char)k;
     }
   }
 }

@@ -417,10 +417,11 @@ def lpf_eval_host(p: Paths, images_host, phase: int, counts_host=None, flags: in
 
 def lpf_last_launch_info(p: Paths) -> dict:
     lib = load()
-    out = (ctypes.c_int64 * 16)()
+    out = (ctypes.c_int64 * 18)()
     _check(lib.lpf_last_launch_info(p.handle, out), "lpf_last_launch_info")
     keys = ("kernels", "work_items", "program_entries", "grid", "block", "smem_bytes", "tile", "G", "level",
-            "fused_pairs", "singles", "terminals", "piece_nodes", "teams", "ctas_per_sm", "shallow_vectors")
+            "fused_pairs", "singles", "terminals", "piece_nodes", "teams", "ctas_per_sm", "shallow_vectors",
+            "reloads", "classes")
     return dict(zip(keys, [int(v) for v in out]))
 
 
