@@ -235,7 +235,7 @@ int  lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, int H, int W
                    int64_t* counts_host, unsigned flags);
 
 /* Counters of the most recent lpf_eval / lpf_eval_both on this object (host values known at
- * launch time): kernels launched, work chunks (NT units each) x (image group, phase), program entries walked per
+ * launch time): kernels launched, work units x (image group, phase), program entries walked per
  * image-phase, grid, block, dynamic shared memory bytes, thread tile code (1000 TX + 100 TY + mask-stack slots), images
  * per team, the erosion level K of the program (0: the plain plane); then what the walker executes per image-phase and
  * per start WORD, counted by replaying its loop over the program on the host: pairs of entries folded into one

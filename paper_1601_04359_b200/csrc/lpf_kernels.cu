@@ -1,9 +1,11 @@
 // lpf_kernels.cu -- CUDA kernels of liblpf.so (sm_100a).
 //   pack_base_kernel  uint8 image -> row-major and column-major bit images, 32 px / word, one coalesced pass
-//   pack_views_kernel the four octant views per image (plain, and the eroded planes E2 / D2), each with its periodic
-//                     halo laid out exactly as the eval kernel wants it in shared memory (a2)
-//   eval_kernel_v3<.> the hot loop: walk the node program with a running AND mask (a3), POPC +
-//                     warp reduce at terminals (a4), optional zero-mask pruning (a5)
+//   pack_views_kernel the four octant views per image, each with its periodic halo laid out exactly as the eval kernel
+//                     wants a row band in shared memory (a2)
+//   eval_kernel_v3<.> the hot loop: TMA-stage a row band, derive the eroded planes of a pattern class from it, walk
+//                     the node program with a running AND mask (a3), POPC + warp reduce at terminals (a4), optional
+//                     zero-mask pruning (a5)
+//   shallow_kernel    the vectors of fewer steps than a window of the eroded program covers
 //   mirror_kernel     counts[-v] = counts[v] (a6)
 //   objective_kernel  sum (c - t)^2 per image (a8, Eq. 14/19)
 //   swap_delta_kernel_v3 + swap_mirror_kernel  per-proposal count deltas (a9)
@@ -195,21 +197,22 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, unsigne
 
 // ---------------------------------------------------------------------------------------------
 // eval kernel, version 3: register strips on octant views, lean interpreter.
-//   CTA = G images x wpi warps; every warp of the CTA walks the same work item = (program item, row band,
-//   strip band) on the same phase plane.  Lane = start row inside a block of 32 rows, warp = (strip, row
-//   block): a thread owns the TX x-adjacent start words [strip*TX, strip*TX+TX) of TY start rows (32 apart).
-//   It keeps the TX+1 words of the CURRENT path row in registers (R), so a node that stays in the same row
-//   and word column costs TX x (SHF + LOP3) and no load at all; a node that changes row reloads TX+1 words
-//   (odd row stride: the 32 lanes hit 32 different banks).
+//   CTA = NT teams of G images x wpi warps.  The CTA holds the bands of one KEY -- (image group, phase plane, octant,
+//   row band, pattern class) -- in shared memory; every team walks its own work UNIT = (program item, strip band) of
+//   that key.  Lane = start row inside a block of 32 rows, warp = (strip, row block): a thread
+//   owns the TX x-adjacent start words [strip*TX, strip*TX+TX) of TY start rows (32 apart).
+//   It keeps the TX+1 words of the CURRENT path row in registers (R), so an entry that stays in the same row, word
+//   column and plane costs TX x (SHF + LOP3) and no load at all; any other reloads TX+1 words (odd row stride: the 32
+//   lanes hit 32 different banks).
 //   Program fetch: each warp loads 32 entries at a time, one per lane (one coalesced 256 B request, issued a
-//   whole chunk ahead), and broadcasts them node by node with SHFL; the high word (count index, slots) is
+//   whole chunk ahead), and broadcasts them entry by entry with SHFL; the high word (count index, slots) is
 //   fetched only by the rare entries that need it.
-//   Saved masks of the depth-first walk live in LOCAL memory (saves/restores are ~2.6 % of the nodes each;
-//   the lines stay in L1), so the hot loop carries no stack registers and shared memory holds only the
-//   bands: 4-5 CTAs per SM instead of 2 (measured: config 3 15.4 -> 11.6 ms against a shared-memory stack).
-//   The kernel does not know about planes: in eroded mode shared memory holds the E2 and
-//   the D2 band instead of the plain one, an entry's offset field already points into the right plane, and one
-//   window then covers two path pixels.  PAIR entries fold their window into the next entry's 3-input AND.
+//   Saved masks of the depth-first walk live in LOCAL memory (saves/restores are a few % of the entries each; the
+//   lines stay in L1), so the hot loop carries no stack registers.
+//   The walker does not know about planes: at level K >= 1 shared memory holds the eroded
+//   planes of the key's pattern class (derived from the plain band when the key is taken), an entry's offset field
+//   already points into the right plane, and one window covers K + 1 path pixels.  PAIR entries fold their window
+//   into the next entry's 3-input AND.
 //   The mask of an item is initialised once, before the loop (INIT is only ever an item's first entry).
 // ---------------------------------------------------------------------------------------------
 // ---------------------------------------------------------------------------------------------

@@ -680,8 +680,9 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int c
   static const int team_warps[4] = {2, 1, 4, 8};
   for (int K = max_level; K >= 0; --K)
     for (int ci = 0; ci < 4; ++ci) {
-      const int cw = team_warps[ci];
-      if (cta_warps >= 1 && cta_warps <= 8 && cw != cta_warps) continue;
+      const bool fixed = cta_warps >= 1 && cta_warps <= 8;   // lpf_set_tile: that team size only
+      if (fixed && ci > 0) break;
+      const int cw = fixed ? cta_warps : team_warps[ci];
       Geom g;
       if (!choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cw, K, path_patterns[K], &g)) continue;
       const double c = geom_cost(g, max_smem, max_teams);

@@ -564,6 +564,43 @@ def test_hypothesis_generated_small_cases():
     check()
 
 
+def test_hypothesis_generated_levels_teams_and_tiles():
+    """Random shapes up to 96 x 160 with a capped erosion level (1..6: pattern classes, derived planes, the short-vector
+    kernel), a fixed team count and thread tile (hypothesis, derandomised): full-template bit-exact parity."""
+    from hypothesis import given, settings, strategies as st
+
+    @settings(max_examples=120, deadline=None, derandomize=True)
+    @given(st.integers(2, 96), st.integers(2, 160), st.floats(0.2, 0.97), st.integers(0, 2 ** 31 - 1),
+           st.integers(1, 6), st.integers(0, 3), st.sampled_from([(0, 0), (4, 2), (8, 1), (4, 4), (8, 2), (16, 1)]),
+           st.integers(0, 8), st.integers(1, 2), st.data())
+    def check(H, W, fill, seed, level, teams, tile, cta_warps, B, data):
+        m = data.draw(st.integers(1, min(H, W) - 1))
+        rng = np.random.default_rng(seed)
+        imgs = (rng.random((B, H, W)) < fill).astype(np.uint8)
+        p = paths(m)
+        lpf.lpf_set_level(p, level)
+        lpf.lpf_set_tile(p, tile[0], tile[1], cta_warps)
+        try:
+            try:
+                lpf.lpf_set_teams(p, teams)
+                both = lpf.lpf_eval_both(p, dev(imgs)).cpu().numpy()
+            except lpf.LpfError as e:                # a fixed team count that the shape cannot take is refused
+                assert e.code == lpf.LPF_E_UNSUPPORTED and teams > 0
+                lpf.lpf_set_teams(p, 0)
+                both = lpf.lpf_eval_both(p, dev(imgs)).cpu().numpy()
+            assert lpf.lpf_last_launch_info(p)["level"] <= level
+        finally:
+            lpf.lpf_set_level(p, -1)
+            lpf.lpf_set_teams(p, 0)
+            lpf.lpf_set_tile(p, 0, 0, 0)
+        for b in range(B):
+            for phase in (0, 1):
+                want = orc.counts(imgs[b], phase, m, full_template=(H * W <= 600))
+                assert np.array_equal(both[b, phase], want), (H, W, m, level, teams, tile, cta_warps, b, phase)
+
+    check()
+
+
 # ---- the plain-plane program at full size, the automatic fall-back, the boundary contract --------------------
 
 def test_every_erosion_level_and_team_count_at_full_size():
