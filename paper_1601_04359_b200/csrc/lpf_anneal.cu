@@ -67,6 +67,8 @@ struct AnnealArgs {
   long long N;
   const int4* rec;             // swap-delta node records
   int n_nodes;
+  const int4* rrec;            // reversed trie of the swap delta, or null
+  const unsigned int* dense;   // bit k: phase plane k is dense (per-node walks instead of the reversed trie)
   int* delta;                  // [n_ph][K_max][S][S], zero on entry and again on exit
   long long ph_stride;
   int K_max;
@@ -166,6 +168,7 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
   const int n_chunks = (int)((per_prop + 1023) / 1024);
   int K = min(16, a.K_max);
   long long win_next = 0, win_acc = 0;
+  const unsigned int dense_mask = __ldg(a.dense);         // swaps keep the volume fractions: fixed for the chain
   for (int batch = 0;; ++batch) {
     const long long next = ld_cg(&a.state->next);
     if (next >= a.N) break;
@@ -175,7 +178,7 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
       const int j = unit / n_slices, slice = unit - j * n_slices;
       if (next + j >= a.N) continue;
       if (a.policy == 0) {
-        swap_delta_unit(sm, stk, sh, H, W, m, a.pairs, a.N, next + j, a.rec, a.n_nodes, a.delta + (long long)j * K2,
+        swap_delta_unit(sm, stk, sh, H, W, m, a.pairs, a.N, next + j, a.rec, a.n_nodes, a.rrec, dense_mask, a.delta + (long long)j * K2,
                         n_ph, a.ph_stride, 1, slice, n_slices);
       } else {                                               // Q = modify(P): the operator draws its pixels from P
         __syncthreads();                                     // the previous unit is finished with s_pair
@@ -190,7 +193,7 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
           }
         }
         __syncthreads();
-        swap_delta_unit(sm, stk, sh, H, W, m, s_pair, 1, 0, a.rec, a.n_nodes, a.delta + (long long)j * K2, n_ph,
+        swap_delta_unit(sm, stk, sh, H, W, m, s_pair, 1, 0, a.rec, a.n_nodes, a.rrec, dense_mask, a.delta + (long long)j * K2, n_ph,
                         a.ph_stride, 1, slice, n_slices);
       }
     }
@@ -411,6 +414,7 @@ static int anneal_impl(lpf_paths* p, uint8_t* image, int H, int W, int phase, co
       AnnealArgs a;
       a.state = d_state; a.padded = padded; a.H = H; a.W = W; a.m = p->m; a.phase = phase; a.n_ph = n_ph;
       a.pairs = pairs; a.pairs_out = pairs_out; a.policy = policy; a.seed = seed; a.log_u = log_u; a.N = N; a.rec = (const int4*)p->d_swap_rec; a.n_nodes = (int)p->n_trie_nodes;
+      a.rrec = (const int4*)p->d_swap_rrec; a.dense = p->d_counter + 2;
       a.delta = d_delta; a.ph_stride = ph_stride; a.K_max = K_max; a.dE = d_dE; a.counts = (long long*)counts;
       a.target = (const long long*)target; a.image = image; a.accept_log = accept_log; a.wh2 = wh2; a.T_mult = T_mult;
       a.c_max = c_max; a.s_max = s_max;

@@ -166,6 +166,7 @@ extern "C" void lpf_free_paths(lpf_paths* p) {
     if (p->d_packed) cudaFree(p->d_packed);
     if (p->d_counter) cudaFree(p->d_counter);
     if (p->d_swap_rec) cudaFree(p->d_swap_rec);
+    if (p->d_swap_rrec) cudaFree(p->d_swap_rrec);
     if (p->d_swap_bits) cudaFree(p->d_swap_bits);
     if (p->d_an_state) cudaFree(p->d_an_state);
     if (p->d_an_delta) cudaFree(p->d_an_delta);
@@ -194,8 +195,8 @@ cudaError_t launch_objective(const long long* counts, const long long* target, i
                              unsigned long long* sse, int n_sm, cudaStream_t st);
 cudaError_t swap_delta_prepare(size_t smem);
 cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W, int m, int phase, const int* pairs,
-                              long long n, const int32_t* rec, int n_nodes, int* delta, long long plane_stride,
-                              unsigned int* counter, int n_sm, cudaStream_t st);
+                              long long n, const int32_t* rec, int n_nodes, const int32_t* rrec, int* delta,
+                              long long plane_stride, unsigned int* counter, int n_sm, cudaStream_t st);
 
 static std::array<int64_t, 8> plan_key(const lpf_paths* p, int B, int H, int W, int n_phase, unsigned flags,
                                        bool masked) {
@@ -410,17 +411,27 @@ static int reserve_swap(lpf_paths* p, int H, int W) {
   if (!dg.ok) return LPF_E_CUDA;
   if (!p->d_swap_rec) {
     try {
-      std::vector<int32_t> rec;
-      build_swap_records(p, rec);
+      std::vector<int32_t> rec, rrec;
+      build_swap_records(p, rec, rrec, SWAP_REV_MAX_NODES);
       if ((int64_t)rec.size() != 4 * p->n_trie_nodes) return LPF_E_INVAL;
       int32_t* d = nullptr;
+      int32_t* dr = nullptr;
       cudaError_t e = cudaMalloc(&d, sizeof(int32_t) * rec.size());
       if (e == cudaSuccess) e = cudaMemcpy(d, rec.data(), sizeof(int32_t) * rec.size(), cudaMemcpyHostToDevice);
+      if (e == cudaSuccess && !rrec.empty()) {
+        e = cudaMalloc(&dr, sizeof(int32_t) * rrec.size());
+        if (e == cudaSuccess) e = cudaMemcpy(dr, rrec.data(), sizeof(int32_t) * rrec.size(), cudaMemcpyHostToDevice);
+      }
       if (e != cudaSuccess) {
         if (d) cudaFree(d);
+        if (dr) cudaFree(dr);
         return cuda_fail(e);
       }
       p->d_swap_rec = d;
+      p->d_swap_rrec = dr;
+      p->n_swap_rev = (int64_t)rrec.size() / 4;
+      p->n_swap_rev1 = 0;                            // children of the reversed root: preorder, sibling chain from 1
+      for (int64_t i = 1; i < p->n_swap_rev; i += rrec[4 * i + 2]) ++p->n_swap_rev1;
     } catch (const std::bad_alloc&) {
       return LPF_E_NOMEM;
     }
@@ -696,7 +707,8 @@ int swap_delta_impl(lpf_paths* p, const uint8_t* image, int H, int W, int phase,
   StreamOrder order(p, st);
   LPF_CUDA(order.err);
   LPF_CUDA(launch_swap_delta(image, p->d_swap_bits, H, W, p->m, phase, pairs, (long long)n, p->d_swap_rec,
-                             (int)p->n_trie_nodes, delta, (long long)plane_stride, p->d_counter + 1, p->n_sm, st));
+                             (int)p->n_trie_nodes, p->d_swap_rrec, delta, (long long)plane_stride, p->d_counter + 1,
+                             p->n_sm, st));
   LPF_CUDA(order.done());
   return LPF_OK;
 }

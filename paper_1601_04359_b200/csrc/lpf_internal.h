@@ -82,6 +82,7 @@ constexpr int E_Q_SHIFT = 26;
 static_assert(STACK_SLOTS_BUDGET <= 8, "three bits per mask-stack slot");
 
 constexpr int MAX_M = 511;
+constexpr int64_t SWAP_REV_MAX_NODES = 4 << 20;   // reversed trie of lpf_swap_delta: 64 MB of records at most (m <= ~100)
 
 struct Node {
   int16_t a, b;          // pixel offset of this node (last pixel of the prefix), view coordinates
@@ -159,6 +160,9 @@ struct lpf_paths {
   unsigned int* d_counter = nullptr;
   // swap-delta node records: the image-coordinate trie in preorder, 16 bytes per node (built by lpf_reserve)
   int32_t* d_swap_rec = nullptr;     // [n_trie_nodes][4]
+  int32_t* d_swap_rrec = nullptr;    // reversed trie [n_swap_rev][4], or null (table too large: per-node walks instead)
+  int64_t n_swap_rev = 0;
+  int n_swap_rev1 = 0;               // children of the reversed trie's root (the unit of slicing)
   uint32_t* d_swap_bits = nullptr;   // packed base image of the last lpf_swap_delta call
   size_t swap_bits_bytes = 0;
   // lpf_anneal: chain state, speculative deltas and their error changes
@@ -200,7 +204,8 @@ int swap_delta_impl(lpf_paths* p, const uint8_t* image, int H, int W, int phase,
                     int32_t* delta, int64_t plane_stride, void* stream);
 
 // the image-coordinate trie in preorder for lpf_swap_delta (lpf_paths.cpp)
-void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec);
+// also the reversed trie (rrec, left empty if it would exceed max_rev nodes)
+void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec, std::vector<int32_t>& rrec, int64_t max_rev);
 
 // builds (or returns the cached) program for (piece_nodes, flags, view strides); host side only
 Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int K, int n_planes,

@@ -98,7 +98,7 @@ static void build_trie(lpf_paths* p) {
 //   [2] nodes in the subtree, self included (first child = index + 1, next sibling = index + [2])
 //   [3] bits 0-19: (b+m)(2m+1)+(a+m) if the prefix is a whole path P_v, else 0xFFFFF; bits 20-23: 3 (sa+1) + (sb+1)
 //       for the step (sa, sb) from the parent; bit 24: the node has a next sibling
-void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec) {
+void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec, std::vector<int32_t>& rrec, int64_t max_rev) {
   const int m = p->m;
   std::vector<Node> nd;
   nd.push_back(Node{0, 0, -1, -1, -1, 1, 0, 0});
@@ -118,6 +118,7 @@ void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec) {
     }
   }
   rec.assign(4 * N, 0);
+  std::vector<int32_t> pre(N, 0);                   // trie index -> preorder position
   std::vector<std::pair<int, int>> stack{{0, 0}};   // (trie index, has next sibling)
   int32_t at = 0;
   std::vector<int> kids;
@@ -132,11 +133,85 @@ void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec) {
     rec[4 * (size_t)at + 1] = rep[u];
     rec[4 * (size_t)at + 2] = nd[u].size;
     rec[4 * (size_t)at + 3] = (int32_t)(cidx | ((uint32_t)step << 20) | ((uint32_t)sib << 24));
+    pre[u] = at;
     ++at;
     kids.clear();
     for (int c = nd[u].first_child; c >= 0; c = nd[c].next_sibling) kids.push_back(c);
     // popped in reverse push order: the first pushed child is emitted last and has no next sibling
     for (size_t k = 0; k < kids.size(); ++k) stack.push_back({kids[k], k == 0 ? 0 : 1});
+  }
+
+  // The REVERSED trie: for every node u its steps read backwards, u -> root, inserted as a
+  // word over the 9 step codes.  A node of this trie at depth j is a walk of j steps back from the pixel that a segment
+  // must contain; it is COMPLETE for the trie node u of depth j whose whole backward walk it is.  Walks of different
+  // nodes share their beginnings, so testing the prefix root -> u of every u costs one pixel test per distinct backward
+  // walk that is still in phase, not one walk per u.  One record per node in preorder:
+  //   [0] (ra & 0xffff) | (rb << 16)  offset of the walk's end from the pixel (minus the sum of its steps)
+  //   [1] preorder index of the trie node it is complete for, or -1
+  //   [2] nodes in the subtree, self included   [3] bit 0: the node has a next sibling
+  rrec.clear();
+  struct RNode { int32_t child[9]; int32_t fwd; int16_t a, b; };
+  std::vector<RNode> rn;
+  RNode root;
+  for (int k = 0; k < 9; ++k) root.child[k] = -1;
+  root.fwd = 0; root.a = 0; root.b = 0;
+  rn.push_back(root);
+  bool too_big = false;
+  for (size_t u = 1; u < N && !too_big; ++u) {
+    int cur = 0;
+    for (int w = (int)u; nd[w].parent >= 0; w = nd[w].parent) {
+      const int par = nd[w].parent;
+      const int sa = nd[w].a - nd[par].a, sb = nd[w].b - nd[par].b;
+      const int code = 3 * (sa + 1) + (sb + 1);
+      int c = rn[cur].child[code];
+      if (c < 0) {
+        if ((int64_t)rn.size() >= max_rev) { too_big = true; break; }
+        RNode x;
+        for (int k = 0; k < 9; ++k) x.child[k] = -1;
+        x.fwd = -1;
+        x.a = (int16_t)(rn[cur].a - sa);
+        x.b = (int16_t)(rn[cur].b - sb);
+        c = (int)rn.size();
+        rn.push_back(x);
+        rn[cur].child[code] = c;
+      }
+      cur = c;
+    }
+    if (!too_big) rn[cur].fwd = pre[u];
+  }
+  if (too_big) return;                               // the caller keeps the per-node walks for this table
+  const size_t R = rn.size();
+  std::vector<int32_t> rsize(R, 1);
+  // subtree sizes by an explicit post-order
+  std::vector<std::pair<int, int>> st2{{0, 0}};      // (node, next child code to look at)
+  while (!st2.empty()) {
+    auto& top = st2.back();
+    int k = top.second;
+    while (k < 9 && rn[top.first].child[k] < 0) ++k;
+    if (k < 9) {
+      top.second = k + 1;
+      st2.push_back({rn[top.first].child[k], 0});
+    } else {
+      const int done = top.first;
+      st2.pop_back();
+      if (!st2.empty()) rsize[st2.back().first] += rsize[done];
+    }
+  }
+  rrec.assign(4 * R, 0);
+  std::vector<std::pair<int, int>> st3{{0, 0}};
+  int32_t rat = 0;
+  while (!st3.empty()) {
+    const int u = st3.back().first, sib = st3.back().second;
+    st3.pop_back();
+    rrec[4 * (size_t)rat + 0] = (int32_t)(((uint32_t)(uint16_t)rn[u].a) | ((uint32_t)(uint16_t)rn[u].b << 16));
+    rrec[4 * (size_t)rat + 1] = rn[u].fwd;
+    rrec[4 * (size_t)rat + 2] = rsize[u];
+    rrec[4 * (size_t)rat + 3] = sib;
+    ++rat;
+    kids.clear();
+    for (int k = 0; k < 9; ++k)
+      if (rn[u].child[k] >= 0) kids.push_back(rn[u].child[k]);
+    for (size_t k = 0; k < kids.size(); ++k) st3.push_back({kids[k], k == 0 ? 0 : 1});
   }
 }
 

@@ -5,9 +5,13 @@
 //              - #{segments of vector v that contain w and lie in phase in I }
 //   A segment of v that has pixel px at path position k starts at s = px - P_v[k]; P_v[0..k] is a trie node N, so
 //   the candidates are exactly the pairs (trie node N, terminal D in the subtree of N) with start s_N = px - o_N.
-//   (A) lane per node N: the prefix root -> N must be in phase from s_N.  The parent's pixel is one of the 8
-//       neighbours of px (register mask lookup: most nodes stop there); the other ancestors' pixels are stepped
-//       backwards with Bresenham error arithmetic on a vector that runs through N -- no loads but the image bits.
+//   (A) the prefix root -> N must be in phase from s_N.  With the REVERSED trie (lpf_paths.cpp; tables of m up to
+//       about 100): the walks N -> root of all nodes, read as offsets from px, share their beginnings, so they are
+//       explored depth-first from px like the subtrees of (B) -- one pixel test per distinct backward walk that is still
+//       in phase; a walk that is complete for a node N makes (N, its end pixel) a survivor.  Without it (large tables):
+//       lane per node N; the parent's pixel is one of the 8 neighbours of px (register mask lookup: most nodes stop
+//       there), then the far end, then the other ancestors' pixels are stepped backwards with Bresenham error
+//       arithmetic on a vector that runs through N -- no loads but the image bits.
 //   (B) the subtrees of all surviving (N, start) are explored by the whole CTA from one stack in shared memory: a
 //       thread pops one node, tests its pixel, counts it if it is a terminal, and pushes its next sibling (always)
 //       and its first child (if the pixel is in phase).  A dead prefix kills every vector below it at once.
@@ -32,6 +36,7 @@ struct SwapPass {                   // one (proposal, pixel) pass, in shared mem
   int ox, oy;                       // pixel that reads as out of phase in this pass (w in I'), or -1
   unsigned nb;                      // in-phase bits of the 8 neighbours px - step, by step code
   int sign;                         // +1: u on I', -1: w on I
+  int rev;                          // (A) by the reversed trie (else by the per-node walks)
   int pbase;                        // word offset of this pass's phase plane in the shared-memory bit images
   long long out_off;                // offset of this pass's [S][S] delta array from the CTA's first one
 };
@@ -43,15 +48,18 @@ struct SwapShared {                 // per-CTA scratch of swap_delta_unit
 };
 
 // One unit of swap-delta work of a CTA of 256 threads: the proposals pairs[first_prop .. first_prop + sw) (those below
-// n; sw <= SWAP_SW) against node slice `slice` of `n_slices` equal slices of the trie.  Adds into out0 [sw][S][S]
+// n; sw <= SWAP_SW) against node slice `slice` of `n_slices` equal slices of the trie (passes on a dense phase plane,
+// bit k of dense_mask, or rrec == nullptr) and against the children c of the reversed trie's root with c % n_slices ==
+// slice (passes on a sparse plane).  Adds into out0 [sw][S][S]
 // (canonical half only; plane k at + k * plane_stride), which must have been zeroed.
 //   P    shared memory: [n_planes][H + 2m][ceil((W + 2m) / 32)] bits of the base image with its halo of m pixels
 //   stk  shared memory: the CTA's stack of 8 * SWAP_STACK items (8 bytes each)
 __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, SwapShared& sh, int H, int W, int m,
                                                 const int* __restrict__ pairs, long long n, long long first_prop,
-                                                const int4* __restrict__ rec, int n_nodes, int* __restrict__ out0,
-                                                int n_planes, long long plane_stride, int sw, int slice,
-                                                int n_slices) {
+                                                const int4* __restrict__ rec, int n_nodes,
+                                                const int4* __restrict__ rrec, unsigned dense_mask,
+                                                int* __restrict__ out0, int n_planes, long long plane_stride, int sw,
+                                                int slice, int n_slices) {
   const int PWc = (W + 2 * m + 31) >> 5, PH = H + 2 * m;                // padded bit image: halo of m pixels all round
   const int tid = threadIdx.x, lane = tid & 31;
   const int plane_words = PH * PWc;
@@ -90,6 +98,7 @@ __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, S
             sp.nb |= bit << code;
           }
           sp.sign = pass ? -1 : 1;
+          sp.rev = (rrec != nullptr) && !((dense_mask >> pl) & 1u);
           sp.pbase = pl * plane_words;
           sp.out_off = (long long)pl * plane_stride + (long long)j * K;
           sh.pass[slot + pass] = sp;
@@ -126,6 +135,32 @@ __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, S
       cur += r.z;
     }
   };
+  // the same for the reversed trie: node j of rrec is the end of a backward walk from the pass's pixel; if it is in
+  // phase and complete for trie node N, then (N, that pixel) is a survivor: N is counted and its subtree scanned
+  auto rvisit_serial = [&](int j, int qi, const int4& r) -> bool {
+    const int x = wrap_coord(sh.pass[qi].px + (short)(r.x & 0xffff), W), y = wrap_coord(sh.pass[qi].py + (r.x >> 16), H);
+    const bool in = pbit(P + sh.pass[qi].pbase, x, y) && !(x == sh.pass[qi].ox && y == sh.pass[qi].oy);
+    if (in && r.y >= 0) {
+      const int4 rN = __ldg(rec + r.y);
+      if ((rN.w & 0xFFFFF) != 0xFFFFF) atomicAdd(out0 + sh.pass[qi].out_off + (rN.w & 0xFFFFF), sh.pass[qi].sign);
+      scan_range(r.y + 1, r.y + rN.z, qi, x, y);
+    }
+    return in;
+  };
+  auto rscan_range = [&](int j, int end, int qi) {
+    while (j < end) {
+      const int4 r = __ldg(rrec + j);
+      j += rvisit_serial(j, qi, r) ? 1 : r.z;
+    }
+  };
+  auto rscan_siblings = [&](int cur, int qi) {
+    for (;;) {
+      const int4 r = __ldg(rrec + cur);
+      if (rvisit_serial(cur, qi, r)) rscan_range(cur + 1, cur + r.z, qi);
+      if (!(r.w & 1)) break;
+      cur += r.z;
+    }
+  };
   // reserves cnt slots of the CTA's stack for this warp and returns the first; slots at or beyond CAP do not exist:
   // their owners walk their items serially instead, and the stack top is clamped before the next pop
   auto reserve = [&](int cnt) -> int {
@@ -134,10 +169,40 @@ __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, S
     return __shfl_sync(0xffffffffu, base, 0);
   };
 
+  constexpr unsigned REV = 0x80000000u;                    // stack item: a node of the reversed trie
   // the node range is sliced, so that a small batch of proposals still fills the chip
   const int slice_nodes = (n_nodes + n_slices - 1) / n_slices;
-  const int n_begin = slice * slice_nodes, n_end = min(n_nodes, n_begin + slice_nodes);
-  const int n_iter = (n_end - n_begin + (int)blockDim.x - 1) / (int)blockDim.x;
+  bool any_scan = false;
+  for (int q = 0; q < np; ++q) any_scan |= !sh.pass[q].rev;
+  const int n_begin = slice * slice_nodes, n_end = any_scan ? min(n_nodes, n_begin + slice_nodes) : n_begin;
+  const int n_iter = max(1, (n_end - n_begin + (int)blockDim.x - 1) / (int)blockDim.x);
+  if (tid < np && sh.pass[tid].rev) {
+    // (A) with the reversed trie: v = 0 (the pixel itself is in phase by construction) and the segments that START at
+    // the pixel, then this slice's children of the reversed root go on the stack; each is pushed on its own, so the
+    // sibling chain is not followed for them
+    const int q = tid;
+    if (slice == 0) {                                      // the root is a survivor at the pixel itself: (B) from there
+      atomicAdd(out0 + sh.pass[q].out_off + (__ldg(rec).w & 0xFFFFF), sh.pass[q].sign);
+      if (n_nodes > 1) {
+        const int pos = atomicAdd(&sh.top, 1);
+        const int px = sh.pass[q].px, py = sh.pass[q].py;
+        if (pos < CAP) stk[pos] = make_uint2(1u | ((unsigned)q << 24), (unsigned)px | ((unsigned)py << 16));
+        else scan_siblings(1, q, px, py);
+      }
+    }
+    int c = 1, k = 0;
+    for (;;) {
+      const int4 r = __ldg(rrec + c);
+      if (k % n_slices == slice) {
+        const int pos = atomicAdd(&sh.top, 1);
+        if (pos < CAP) stk[pos] = make_uint2((unsigned)c | ((unsigned)q << 24) | REV, 1u);   // y = 1: no sibling push
+        else if (rvisit_serial(c, q, r)) rscan_range(c + 1, c + r.z, q);
+      }
+      if (!(r.w & 1)) break;
+      c += r.z;
+      ++k;
+    }
+  }
   for (int itn = 0; itn < n_iter; ++itn) {
     const int N = n_begin + itn * blockDim.x + tid;
     int4 rN = make_int4(0, 0, 0, 0);
@@ -156,7 +221,7 @@ __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, S
     for (int q = 0; q < np; ++q) {
       const unsigned nb = sh.pass[q].nb;
       const uint32_t* Pq = P + sh.pass[q].pbase;
-      bool alive = (N < n_end) && (d == 0 || ((nb >> codeN) & 1u));
+      bool alive = (N < n_end) && !sh.pass[q].rev && (d == 0 || ((nb >> codeN) & 1u));
       if (!__any_sync(0xffffffffu, alive)) continue;       // typical for u: an isolated pixel kills all 32 at once
       const int ox = sh.pass[q].ox, oy = sh.pass[q].oy;
       const int sx = wrap_coord(sh.pass[q].px - oNx, W), sy = wrap_coord(sh.pass[q].py - oNy, H);
@@ -212,33 +277,65 @@ __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, S
       __syncthreads();                                     // every thread has read top and its item
       if (tid == 0) sh.top = n - take;
       __syncthreads();
-      bool p_sib = false, p_child = false;
-      int i = 0, qi = 0, isx = 0, isy = 0, size_i = 0;
+      bool p_sib = false, p_child = false, p_fwd = false, rev = false;
+      int i = 0, qi = 0, isx = 0, isy = 0, size_i = 0, fN = 0, fsize = 0, fx = 0, fy = 0;
       if (it.x != DUMMY) {
         i = (int)(it.x & 0xFFFFFF);
-        qi = (int)(it.x >> 24);
-        isx = (int)(it.y & 0xffff);
-        isy = (int)(it.y >> 16);
-        const int4 r = __ldg(rec + i);
-        size_i = r.z;
-        p_child = visit(i, qi, isx, isy, r) && r.z > 1;
-        p_sib = (r.w >> 24) & 1;
-        if (p_sib) it.x += (unsigned)r.z;                  // next sibling = i + subtree size
+        qi = (int)((it.x >> 24) & 0x7Fu);
+        rev = (it.x & REV) != 0;
+        if (!rev) {
+          isx = (int)(it.y & 0xffff);
+          isy = (int)(it.y >> 16);
+          const int4 r = __ldg(rec + i);
+          size_i = r.z;
+          p_child = visit(i, qi, isx, isy, r) && r.z > 1;
+          p_sib = (r.w >> 24) & 1;
+          if (p_sib) it.x += (unsigned)r.z;                // next sibling = i + subtree size
+        } else {
+          // the end of a backward walk from the pass's pixel: in phase -> its extensions; complete for trie node fN ->
+          // (fN, this pixel) is a survivor of (A): count it, and its first child is the start of (B)
+          const int4 r = __ldg(rrec + i);
+          size_i = r.z;
+          fx = wrap_coord(sh.pass[qi].px + (short)(r.x & 0xffff), W);
+          fy = wrap_coord(sh.pass[qi].py + (r.x >> 16), H);
+          const bool in = pbit(P + sh.pass[qi].pbase, fx, fy) && !(fx == sh.pass[qi].ox && fy == sh.pass[qi].oy);
+          p_child = in && r.z > 1;
+          p_sib = (r.w & 1) && it.y == 0u;                 // the root's children were pushed one by one (y = 1)
+          if (p_sib) it.x += (unsigned)r.z;
+          if (in && r.y >= 0) {
+            fN = r.y;
+            const int4 rN = __ldg(rec + fN);
+            fsize = rN.z;
+            if ((rN.w & 0xFFFFF) != 0xFFFFF) atomicAdd(out0 + sh.pass[qi].out_off + (rN.w & 0xFFFFF), sh.pass[qi].sign);
+            p_fwd = rN.z > 1;
+          }
+        }
       }
       const unsigned ms = __ballot_sync(0xffffffffu, p_sib);
       const unsigned mc = __ballot_sync(0xffffffffu, p_child);
-      const int ns = __popc(ms), nc = __popc(mc);
-      if (ns + nc) {
-        const int base = reserve(ns + nc);
-        if (base + ns + nc <= CAP) {
-          if (p_sib) stk[base + __popc(ms & lt)] = it;
-          if (p_child) stk[base + ns + __popc(mc & lt)] = make_uint2((unsigned)(i + 1) | (it.x & 0xFF000000u), it.y);
+      const unsigned mf = __ballot_sync(0xffffffffu, p_fwd);
+      const int ns = __popc(ms), nc = __popc(mc), nf = __popc(mf);
+      if (ns + nc + nf) {
+        const int base = reserve(ns + nc + nf);
+        if (base + ns + nc + nf <= CAP) {
+          if (p_sib) stk[base + __popc(ms & lt)] = make_uint2(it.x, rev ? 0u : it.y);
+          if (p_child)
+            stk[base + ns + __popc(mc & lt)] = make_uint2((unsigned)(i + 1) | (it.x & 0xFF000000u), rev ? 0u : it.y);
+          if (p_fwd)
+            stk[base + ns + nc + __popc(mf & lt)] =
+                make_uint2((unsigned)(fN + 1) | ((unsigned)qi << 24), (unsigned)fx | ((unsigned)fy << 16));
         } else {
           // the stack cannot take this warp's pushes: every lane walks the remainder of its own item serially, and
           // the part of the reservation that lies inside the stack is marked unused
-          for (int k = base + lane; k < min(base + ns + nc, CAP); k += 32) stk[k] = make_uint2(DUMMY, 0);
-          if (p_child) scan_range(i + 1, i + size_i, qi, isx, isy);
-          if (p_sib) scan_siblings(i + size_i, qi, isx, isy);
+          for (int k = base + lane; k < min(base + ns + nc + nf, CAP); k += 32) stk[k] = make_uint2(DUMMY, 0);
+          if (!rev) {
+            if (p_child) scan_range(i + 1, i + size_i, qi, isx, isy);
+            if (p_sib) scan_siblings(i + size_i, qi, isx, isy);
+          } else {
+            if (p_fwd) scan_range(fN + 1, fN + fsize, qi, fx, fy);
+            if (p_child) rscan_range(i + 1, i + size_i, qi);
+            if (p_sib) rscan_siblings(i + size_i, qi);
+          }
         }
       }
       __syncthreads();                                     // all pushes of this round are in
