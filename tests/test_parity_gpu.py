@@ -323,6 +323,31 @@ def test_swap_delta_dense_image_overflows_the_warp_stacks():
     assert int(d_img.sum()) > 0.95 * H * W
 
 
+def test_swap_delta_sparse_phase_with_large_live_regions_on_the_reversed_trie():
+    """Broad stripes that fill 47 % of the image: the phase counts as sparse (below one half), so the backward walks run
+    on the reversed trie, but inside a stripe almost every walk survives: the CTA's stack overflows and the serial
+    fall-back over the reversed trie runs.  The complementary phase (53 %, per-node walks) rides along.  Every delta
+    against full re-evaluation on the GPU, a few against the oracle."""
+    H, W, m = 192, 256, 64
+    img = np.zeros((H, W), dtype=np.uint8)
+    img[:, 10:70] = 1
+    img[:, 130:190] = 1
+    rng = np.random.default_rng(47)
+    img[rng.random((H, W)) < 0.002] ^= 1                      # a few defects so that not everything is one run
+    assert 0.44 < img.mean() < 0.5
+    p = paths(m)
+    pairs = inputs.swap_pairs(img, 48, 47)
+    d_img, d_pairs = dev(img[None]), dev(pairs)
+    for phase in (1, 0):
+        base = lpf.lpf_eval(p, d_img, phase)[0]
+        d = lpf.lpf_swap_delta(p, d_img, phase, d_pairs)
+        re = lpf.lpf_eval(p, _swapped_images(d_img, d_pairs), phase) - base[None]
+        assert bool((re == d.to(torch.int64)).all()), phase
+        dn = d.cpu().numpy()
+        for i in range(2):
+            assert np.array_equal(dn[i], orc.swap_delta_local(img, phase, m, pairs[i])), (phase, i)
+
+
 def test_swap_delta_small_and_degenerate_pairs():
     rng = np.random.default_rng(9)
     H, W, m = 20, 45, 11
