@@ -220,3 +220,27 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
     for (dx, dy), pix in seen.items():
         assert orc.in_half(dx, dy)
         assert pix == [tuple(int(t) for t in r) for r in orc.path(dx, dy)], (dx, dy)
+
+
+def test_balanced_pattern_counts_and_classes_of_config3():
+    """The K-step patterns of digital straight segments are the balanced words: 2, 4, 8, 14, 24, 36 of them for K = 1..6
+    (1 + sum over i <= K of (K - i + 1) phi(i), the number of factors of length K of Sturmian words).  The program of
+    config 3 (512 x 512, m = 256) is of level 6 with at most 7 planes per class -- what fits in shared memory beside the
+    plain band -- and its classes together cover every pattern."""
+    from math import gcd
+    for K, want in zip(range(1, 7), (2, 4, 8, 14, 24, 36)):
+        phi = lambda n: sum(1 for k in range(1, n + 1) if gcd(k, n) == 1)
+        assert want == 1 + sum((K - i + 1) * phi(i) for i in range(1, K + 1))
+        assert want == sum(1 for q in range(1 << K) if _balanced(q, K))
+    p = lpf.lpf_build_paths(256, -1)
+    entries, items, n_slots, layout = lpf.lpf_paths_program(p, 512, 512, 1024, 0)
+    assert layout[8] == 6 and n_slots <= 8
+    n_classes = layout[9]
+    per_octant = {}
+    for c in range(n_classes):
+        rec = layout[10 + 38 * c: 10 + 38 * (c + 1)]
+        assert 1 <= rec[1] <= 7
+        per_octant.setdefault(rec[0], set()).update(rec[2:2 + rec[1]])
+    assert n_classes == 48 and sorted(per_octant) == [0, 1, 2, 3]
+    assert all(len(v) == 36 for v in per_octant.values())
+    assert len(entries) < 900000                                 # 5.0 M trie nodes: more than 5.5 nodes per entry
