@@ -778,7 +778,7 @@ cudaError_t launch_objective(const long long* counts, const long long* target, i
   cudaError_t e = cudaMemsetAsync(sse, 0, sizeof(unsigned long long) * (size_t)B, st);
   if (e != cudaSuccess) return e;
   long long chunks = (K + 256 * 8 - 1) / (256 * 8);
-  const long long want = ((long long)n_sm * 8 + B - 1) / B;     // enough blocks to fill the chip
+  const long long want = ((long long)n_sm * 32 + B - 1) / B;    // enough blocks to fill the chip and keep loads in flight
   if (chunks > want) chunks = want;
   if (chunks < 1) chunks = 1;
   // gridDim.y <= 65535: fold larger batches
