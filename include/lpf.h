@@ -67,7 +67,7 @@ extern "C" {
                              Same counts. */
 
 #define LPF_LAYOUT_MAX_CLASSES 128
-#define LPF_LAYOUT_INTS (10 + 38 * LPF_LAYOUT_MAX_CLASSES)   /* lpf_paths_program */
+#define LPF_LAYOUT_INTS (10 + 40 * LPF_LAYOUT_MAX_CLASSES)   /* lpf_paths_program */
 
 /* `what` of lpf_reserve */
 #define LPF_FOR_EVAL        1u   /* lpf_eval and one-phase lpf_eval_sum with (B, H, W, flags) */
@@ -116,14 +116,15 @@ int  lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, int cap, int
  *            be nodes that are already in the mask; the others are the nodes of this entry; terminal / save / count
  *            index are the last one's.  The vectors of an octant are split by slope into pattern CLASSES whose paths use
  *            few patterns; an item belongs to one class and its entries address the class's planes by slot:
- *            bits 12-31 = b' * stride + (a' >> 5) + slot * band_words; high word bits 26-31 repeat q.
+ *            bits 12-31 = b' * stride + (a' >> 5) + slot * (band words of the class); high word bits 26-31 repeat q.
  *            At level K no window ends above depth K: every item starts (its first and only init entry) with the
  *            window root .. depth K, and the vectors shorter than that are counted by a separate small kernel.
  *   items    host [cap_items][4] int64 = (first entry, number of entries, octant, pattern class) (may be NULL)
  *   layout   host int[LPF_LAYOUT_INTS]: [0..3] words per packed row of each octant view (decodes b', a' >> 5), [4..7]
- *            words of one band of each view in shared memory (the plane in slot s sits at s times that; 0 for the plain
- *            program), [8] the level K of the program (0: plain), [9] the number of pattern classes, then per class 38
- *            ints: octant, patterns used n, the pattern q of slot 0 .. n-1 (-1 beyond)
+ *            words of one full-height band of each view (0 for the plain program), [8] the level K of the program
+ *            (0: plain), [9] the number of pattern classes, then per class 40 ints: octant, patterns used n, words of one
+ *            band of THIS class in shared memory (the plane in slot s sits at s times that; a class keeps only the rows
+ *            its paths reach), rows of that band, the pattern q of slot 0 .. n-1 (-1 beyond)
  * *n_entries / *n_items / *n_slots (mask-stack slots the program needs) are always written.
  * Octants (view coordinates a', b' from image coordinates a, b): 0: dx>=0, dy<=dx (a,b); 1: dx>=0, dy>dx (b,a);
  * 2: dx<0, dy>-dx (b,-a); 3: dx<0, dy<=-dx (-a,b). */

@@ -87,9 +87,11 @@ static void free_program(Program& pr) {
   if (pr.d_entries) cudaFree(pr.d_entries);
   if (pr.d_skip) cudaFree(pr.d_skip);
   if (pr.d_class_slots) cudaFree(pr.d_class_slots);
+  if (pr.d_class_geom) cudaFree(pr.d_class_geom);
   pr.d_entries = nullptr;
   pr.d_skip = nullptr;
   pr.d_class_slots = nullptr;
+  pr.d_class_geom = nullptr;
 }
 
 // uploads the program once; the device pointers are published only when every step has succeeded
@@ -98,27 +100,38 @@ static int upload_program(Program& pr) {
   uint64_t* d_e = nullptr;
   uint32_t* d_s = nullptr;
   signed char* d_c = nullptr;
+  int* d_g = nullptr;
   const size_t ne = pr.entries.size() + 64;      // +64: the walker fetches 32 entries per warp, one chunk ahead
   std::vector<signed char> slots(std::max<size_t>(pr.classes.size(), 1) * MAX_PATTERNS, (signed char)-1);
   for (size_t c = 0; c < pr.classes.size(); ++c)
     std::memcpy(slots.data() + c * MAX_PATTERNS, pr.classes[c].slot_of, MAX_PATTERNS);
+  std::vector<int> geom(std::max<size_t>(pr.classes.size(), 1) * 4, 0);
+  for (size_t c = 0; c < pr.classes.size(); ++c) {
+    geom[4 * c] = pr.classes[c].band_words;
+    geom[4 * c + 1] = pr.classes[c].rows;
+    geom[4 * c + 2] = pr.classes[c].n;
+  }
   cudaError_t e = cudaMalloc(&d_e, sizeof(uint64_t) * ne);
   if (e == cudaSuccess) e = cudaMalloc(&d_s, sizeof(uint32_t) * std::max<size_t>(pr.skip.size(), 1));
   if (e == cudaSuccess) e = cudaMalloc(&d_c, slots.size());
+  if (e == cudaSuccess) e = cudaMalloc(&d_g, sizeof(int) * geom.size());
   if (e == cudaSuccess) e = cudaMemset(d_e, 0, sizeof(uint64_t) * ne);
   if (e == cudaSuccess)
     e = cudaMemcpy(d_e, pr.entries.data(), sizeof(uint64_t) * pr.entries.size(), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(d_s, pr.skip.data(), sizeof(uint32_t) * pr.skip.size(), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(d_c, slots.data(), slots.size(), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(d_g, geom.data(), sizeof(int) * geom.size(), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) {
     if (d_e) cudaFree(d_e);
     if (d_s) cudaFree(d_s);
     if (d_c) cudaFree(d_c);
+    if (d_g) cudaFree(d_g);
     return cuda_fail(e);
   }
   pr.d_entries = d_e;
   pr.d_skip = d_s;
   pr.d_class_slots = d_c;
+  pr.d_class_geom = d_g;
   return LPF_OK;
 }
 
@@ -269,6 +282,10 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   for (int o = 0; o < 4; ++o) n_nodes += (long long)p->oct[o].size();
   const int planes_all = g.K > 0 ? balanced_count(g.K) : 0;
   const int classes_guess = (g.K > 0 && g.v[0].n_planes < planes_all) ? std::max(1, 2 * planes_all / g.v[0].n_planes) : 1;
+  // wider classes for the shallow slopes (their bands are lower: more planes fit) mean more units per key but fewer
+  // keys; only while about four keys per resident CTA remain (measured: config 3 2.49 -> 2.26 ms, but config 2, with 96
+  // keys for 148 CTAs already, 0.125 -> 0.135 ms)
+  const bool widen = (long long)pl.n_gp * work_per_item * 4 * classes_guess >= 4ll * resident_guess;
   const long long want_items = std::max<long long>(
       {1, 20ll * g.NT * resident_guess / ((long long)pl.n_gp * work_per_item), 16ll * g.NT * classes_guess});
   long long piece = n_nodes / want_items;
@@ -283,7 +300,7 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   for (;; q /= 2) {
     try {
       pr = &get_program(p, q, flags, g.v[0].stride, g.v[1].stride, g.K, g.v[0].n_planes, g.v[0].band_words,
-                        g.v[1].band_words);
+                        g.v[1].band_words, g.band_rows, widen);
     } catch (const std::bad_alloc&) {
       return LPF_E_NOMEM;
     }
@@ -518,6 +535,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   ep.units = (const int4*)pl.d_work;
   ep.obtab = (const int4*)pl.d_obtab;
   ep.class_slots = pl.pr->d_class_slots;
+  ep.class_geom = (const int4*)pl.pr->d_class_geom;
   ep.n_ob = pl.n_ob;
   ep.n_keys = (unsigned int)pl.n_keys;
   ep.n_shares = (unsigned int)pl.n_shares;

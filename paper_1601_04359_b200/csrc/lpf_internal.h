@@ -101,18 +101,23 @@ struct Program {         // one linearisation of the four octant tries for one s
   int n_slots = 0;
   int stride[4] = {0, 0, 0, 0};
   int K = 0;                           // erosion level (0: plain program)
-  int n_planes = 0;                    // planes per pattern class (shared memory slots)
+  int n_planes = 0;                    // full-height planes the geometry reserved per image (beside the plain band)
+  int band_rows = 0;                   // start rows of a band
+  bool widen = false;                  // classes of shallow slopes take the planes their lower bands leave room for
   int band_words[4] = {0, 0, 0, 0};    // level K: the plane in slot s of view o sits at s * band_words[o] in shared memory
   // level K: pattern classes (slope sectors of one octant whose paths use at most n_planes patterns); items[4 i + 3] is
   // the class of item i
   struct Class {
     int octant = 0;
+    int rows = 0;                      // rows of the class's band: band_rows + the largest b' of its paths + 1
+    int band_words = 0;                // words of one of its planes in shared memory (rows * stride, padded)
     int n = 0;                         // patterns used
     int pattern[MAX_PATTERNS];         // slot -> pattern q
     signed char slot_of[MAX_PATTERNS]; // rank of a balanced pattern -> slot, or -1
   };
   std::vector<Class> classes;
   signed char* d_class_slots = nullptr;  // device: [classes][MAX_PATTERNS]
+  int* d_class_geom = nullptr;           // device: [classes][4] = band words, rows, planes, -
   uint64_t* d_entries = nullptr;       // device copy, uploaded by lpf_reserve (lpf_api.cu)
   uint32_t* d_skip = nullptr;
 };
@@ -209,7 +214,7 @@ void build_swap_records(const lpf_paths* p, std::vector<int32_t>& rec, std::vect
 
 // builds (or returns the cached) program for (piece_nodes, flags, view strides); host side only
 Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int K, int n_planes,
-                     int bw03, int bw12);
+                     int bw03, int bw12, int band_rows, bool widen);
 int max_teams_of(const lpf_paths* p);
 // the terminals above depth K of every octant trie (counted by shallow_kernel, not by the program)
 void shallow_terminals(const lpf_paths* p, int K, ShallowList* out);

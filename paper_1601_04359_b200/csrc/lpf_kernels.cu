@@ -326,14 +326,20 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
         const int b0 = (gp - plane * groups_per_plane) * g.G;
         const ViewGeom& v = g.v[ob.z & 3];
         // the plain band of every image of the group: level 0 walks it; level K derives its planes from it (it sits
-        // behind them)
-        const unsigned bytes = (unsigned)v.band_words * 4u;
+        // behind them).  A pattern class keeps only the rows its paths reach: its own band words, rows and planes.
+        int bw = v.band_words, np_c = 0;
+        if (g.K > 0) {
+          const int4 cg = __ldg(p.class_geom + (ob.z >> 2));
+          bw = cg.x;
+          np_c = cg.z;
+        }
+        const unsigned bytes = (unsigned)bw * 4u;
         mbar_expect_tx(&bar, bytes * (unsigned)g.G);
         const uint32_t* src = p.packed + (size_t)plane * g.plane_words + v.packed_off + (size_t)b0 * v.view_words +
                               (size_t)ob.w * g.band_rows * v.stride;
         for (int gi = 0; gi < g.G; ++gi)
-          tma_bulk_g2s(smem + (size_t)gi * v.band_pitch + (size_t)v.n_planes * v.band_words,
-                       src + (size_t)gi * v.view_words, bytes, &bar);
+          tma_bulk_g2s(smem + (size_t)gi * v.band_pitch + (size_t)np_c * bw, src + (size_t)gi * v.view_words, bytes,
+                       &bar);
       }
     }
     __syncthreads();
@@ -354,19 +360,19 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
     parity ^= 1u;
     if (g.K > 0) {                   // the planes of the key's pattern class
       const signed char* slot = p.class_slots + (size_t)(ob.z >> 2) * MAX_PATTERNS;
+      const int4 cg = __ldg(p.class_geom + (ob.z >> 2));     // band words, rows, planes of the class
       if (tid < MAX_PATTERNS) s_slot[tid] = slot[tid];
       __syncthreads();
       for (int gi = 0; gi < g.G; ++gi) {
         uint32_t* planes = smem + (size_t)gi * v.band_pitch;
-        const uint32_t* plain = planes + (size_t)v.n_planes * v.band_words;
-        const int rows = g.band_rows + g.m;
+        const uint32_t* plain = planes + (size_t)cg.z * cg.x;
         switch (g.K) {
-          case 1: derive_planes<1>(planes, plain, rows, stride, v.band_words, s_slot); break;
-          case 2: derive_planes<2>(planes, plain, rows, stride, v.band_words, s_slot); break;
-          case 3: derive_planes<3>(planes, plain, rows, stride, v.band_words, s_slot); break;
-          case 4: derive_planes<4>(planes, plain, rows, stride, v.band_words, s_slot); break;
-          case 5: derive_planes<5>(planes, plain, rows, stride, v.band_words, s_slot); break;
-          default: derive_planes<6>(planes, plain, rows, stride, v.band_words, s_slot); break;
+          case 1: derive_planes<1>(planes, plain, cg.y, stride, cg.x, s_slot); break;
+          case 2: derive_planes<2>(planes, plain, cg.y, stride, cg.x, s_slot); break;
+          case 3: derive_planes<3>(planes, plain, cg.y, stride, cg.x, s_slot); break;
+          case 4: derive_planes<4>(planes, plain, cg.y, stride, cg.x, s_slot); break;
+          case 5: derive_planes<5>(planes, plain, cg.y, stride, cg.x, s_slot); break;
+          default: derive_planes<6>(planes, plain, cg.y, stride, cg.x, s_slot); break;
         }
       }
       __syncthreads();

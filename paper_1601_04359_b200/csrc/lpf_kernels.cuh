@@ -54,7 +54,8 @@ struct ViewGeom {
   int stride;        // words per packed row
   int n_bands;       // ceil(Hv / band_rows) bands of start rows
   int band_words;    // (band_rows + m) * stride rounded up to a multiple of 4: one band of one plane in shared memory
-  int n_planes;      // eroded planes of one pattern class held in shared memory: 0 = plain mode (the plain band alone)
+  int n_planes;      // full-height eroded planes that fit in shared memory beside the plain band: 0 = plain mode (the
+                     // plain band alone).  A pattern class keeps only the rows its paths reach and may hold more.
   int band_pitch;    // words per image in shared memory: band_words (plain mode), else (n_planes + 1) * band_words:
                      // the planes, then the plain band they are derived from
   int plane_words;   // words of the plain view of one image in HBM (rows * stride, padded)
@@ -109,6 +110,7 @@ struct EvalParams {
                               // are consecutive, big first
   const int4* obtab;          // [n_ob] (octant, row band, class) triples = first unit, units, octant | class << 2, row band
   const signed char* class_slots;  // level K: [n_classes][MAX_PATTERNS] plane slot of each balanced pattern (by rank), or -1
+  const int4* class_geom;          // level K: [n_classes] = words of one band of the class, its rows, its planes, -
   int n_ob;
   unsigned int n_keys;        // n_gp * n_ob keys = (image group, phase plane, octant, row band, class); key = gp * n_ob + ob
   unsigned int n_shares;      // n_keys * passes: how often the cursor hands out every key

@@ -393,7 +393,7 @@ static void push_item_c(Program& pr, int64_t first, int o, int cls) {
 
 // partitions one trie into pieces and emits its items
 static void emit_trie(const lpf_paths* p, int o, const std::vector<Node>& nd, int piece_nodes, Program& pr,
-                      const signed char* slot_of, int cls) {
+                      const signed char* slot_of, int cls, int band_words) {
   const int K = pr.K;
   const int N = (int)nd.size();
   std::vector<uint8_t> cut(N, 0);
@@ -404,7 +404,7 @@ static void emit_trie(const lpf_paths* p, int o, const std::vector<Node>& nd, in
     else psize[nd[i].parent] += psize[i];
   }
   cut[0] = 1;
-  Emitter em{p->m, o, pr.stride[o], K, pr.band_words[o], slot_of, nd, cut, psize, pr};
+  Emitter em{p->m, o, pr.stride[o], K, band_words, slot_of, nd, cut, psize, pr};
   std::vector<int> starts;
   for (int r = 0; r < N; ++r) {
     if (!cut[r]) continue;
@@ -454,14 +454,33 @@ static void build_class_tries(const lpf_paths* p, int o, int piece_nodes, Progra
     return nd[x].a < nd[y].a;
   });
   std::vector<int16_t> vxy(2 * (size_t)(p->m + 1));
+  // shared memory of one image: the n_planes + 1 full-height bands the geometry reserved.  A class only needs the rows
+  // its paths reach (band_rows + the largest b'), so a class of shallow slopes has room for more planes -- wider
+  // classes, more units per key, fewer keys (pr.widen; not when the keys are few already: lpf_api.cu).
+  const long long budget = (long long)(pr.n_planes + 1) * pr.band_words[o];
   size_t t0 = 0;
   while (t0 < terms.size()) {
     uint64_t set = 0;
     size_t t1 = t0;
-    while (t1 < terms.size() && __builtin_popcountll(set | pathset[terms[t1]]) <= pr.n_planes) set |= pathset[terms[t1++]];
+    int bmax = 0, rows_c = 0, bw_c = 0;
+    while (t1 < terms.size()) {
+      const uint64_t ns = set | pathset[terms[t1]];
+      const int bm = std::max(bmax, (int)nd[terms[t1]].b);
+      const int rows = std::min(pr.band_rows + p->m, pr.band_rows + bm + 1);
+      const int bw = (rows * pr.stride[o] + 3) / 4 * 4;
+      const int room = (int)std::min<long long>(pr.widen ? MAX_PATTERNS : pr.n_planes, budget / bw - 1);
+      if (__builtin_popcountll(ns) > room) break;
+      set = ns;
+      bmax = bm;
+      rows_c = rows;
+      bw_c = bw;
+      ++t1;
+    }
     if (t1 == t0) return;                                  // cannot happen: n_planes >= the patterns of any one path
     Program::Class c;
     c.octant = o;
+    c.rows = rows_c;
+    c.band_words = bw_c;
     std::memset(c.slot_of, -1, sizeof(c.slot_of));
     std::memset(c.pattern, 0, sizeof(c.pattern));
     for (unsigned q = 0; q < (1u << K); ++q) {
@@ -487,14 +506,14 @@ static void build_class_tries(const lpf_paths* p, int o, int piece_nodes, Progra
     for (int i = (int)cnd.size() - 1; i > 0; --i) cnd[cnd[i].parent].size += cnd[i].size;
     const int cls = (int)pr.classes.size();
     pr.classes.push_back(c);
-    emit_trie(p, o, cnd, piece_nodes, pr, pr.classes[cls].slot_of, cls);
+    emit_trie(p, o, cnd, piece_nodes, pr, pr.classes[cls].slot_of, cls, bw_c);
     t0 = t1;
   }
 }
 
 static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
   for (int o = 0; o < 4; ++o) {
-    if (pr.K == 0) emit_trie(p, o, p->oct[o], piece_nodes, pr, nullptr, 0);
+    if (pr.K == 0) emit_trie(p, o, p->oct[o], piece_nodes, pr, nullptr, 0, 0);
     else build_class_tries(p, o, piece_nodes, pr);
   }
   sort_items(pr);
@@ -652,13 +671,13 @@ static void build_s2_program(lpf_paths* p, int piece_nodes, Program& pr) {
 }
 
 Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03, int stride12, int K, int n_planes,
-                     int bw03, int bw12) {
+                     int bw03, int bw12, int band_rows, bool widen) {
   if (piece_nodes < 0) piece_nodes = 0;
   const unsigned kind = (flags & LPF_S2) ? LPF_S2 : (flags & LPF_NO_TRIE);
   if (kind != 0) K = 0;                                    // the eroded planes serve the trie program only
-  if (K == 0) bw03 = bw12 = n_planes = 0;
-  const std::tuple<int, unsigned, int, int, int, int, int> key(piece_nodes, kind, stride03, stride12, 100 * K + n_planes,
-                                                               bw03, bw12);
+  if (K == 0) bw03 = bw12 = n_planes = band_rows = 0;
+  const std::tuple<int, unsigned, int, int, int, int, int> key(piece_nodes, kind, stride03, stride12,
+                                                               1000000 * (widen ? 1 : 0) + 100000 * band_rows + 100 * K + n_planes, bw03, bw12);
   auto it = p->programs.find(key);
   if (it != p->programs.end()) return it->second;
   Program& pr = p->programs[key];
@@ -666,6 +685,8 @@ Program& get_program(lpf_paths* p, int piece_nodes, unsigned flags, int stride03
   pr.stride[1] = pr.stride[2] = stride12;
   pr.K = K;
   pr.n_planes = n_planes;
+  pr.band_rows = band_rows;
+  pr.widen = widen;
   pr.band_words[0] = pr.band_words[3] = bw03;
   pr.band_words[1] = pr.band_words[2] = bw12;
   if (flags & LPF_S2) build_s2_program(p, piece_nodes, pr);
@@ -908,7 +929,7 @@ extern "C" int lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, un
     return LPF_E_UNSUPPORTED;
   try {
     lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride, g.K, g.v[0].n_planes,
-                                        g.v[0].band_words, g.v[1].band_words);
+                                        g.v[0].band_words, g.v[1].band_words, g.band_rows, true);
     *n_entries = (int64_t)pr.entries.size();
     *n_items = (int64_t)pr.items.size() / 4;
     *n_slots = pr.n_slots;
@@ -917,10 +938,12 @@ extern "C" int lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, un
     layout[8] = pr.K;
     layout[9] = (int)pr.classes.size();
     for (size_t c = 0; c < pr.classes.size(); ++c) {
-      int* out = layout + 10 + (2 + lpf::MAX_PATTERNS) * c;
+      int* out = layout + 10 + (4 + lpf::MAX_PATTERNS) * c;
       out[0] = pr.classes[c].octant;
       out[1] = pr.classes[c].n;
-      for (int k = 0; k < lpf::MAX_PATTERNS; ++k) out[2 + k] = k < pr.classes[c].n ? pr.classes[c].pattern[k] : -1;
+      out[2] = pr.classes[c].band_words;
+      out[3] = pr.classes[c].rows;
+      for (int k = 0; k < lpf::MAX_PATTERNS; ++k) out[4 + k] = k < pr.classes[c].n ? pr.classes[c].pattern[k] : -1;
     }
     if (entries) {
       if (cap_entries < *n_entries) return LPF_E_INVAL;

@@ -167,11 +167,11 @@ def lpf_paths_get(p: Paths, dx: int, dy: int) -> np.ndarray:
 
 def lpf_paths_program(p: Paths, H: int, W: int, piece_nodes: int = 0, flags: int = 0):
     """(entries uint64 [n], items int64 [k, 4], n_slots, layout: row strides of the 4 views, the words of one band of
-    each view in shared memory, the level K, the number of pattern classes, then 38 ints per class: octant, patterns
+    each view in shared memory, the level K, the number of pattern classes, then 40 ints per class: octant, patterns
     used, pattern of each slot) of the linearised walk program."""
     lib = load()
     ne, ni, ns = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int()
-    strides = (ctypes.c_int * (10 + 38 * 128))()
+    strides = (ctypes.c_int * (10 + 40 * 128))()
     _check(lib.lpf_paths_program(p.handle, int(H), int(W), int(piece_nodes), int(flags), None, 0, ctypes.byref(ne),
                                  None, 0, ctypes.byref(ni), ctypes.byref(ns), strides), "lpf_paths_program")
     entries = np.zeros(ne.value, dtype=np.uint64)

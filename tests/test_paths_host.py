@@ -144,13 +144,16 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
     n_classes = strides[9]
     classes = []
     for c in range(n_classes):
-        rec = strides[10 + 38 * c: 10 + 38 * (c + 1)]
-        octant, n = rec[0], rec[1]
-        pats = rec[2:2 + n]
+        rec = strides[10 + 40 * c: 10 + 40 * (c + 1)]
+        octant, n, bw, rows = rec[0], rec[1], rec[2], rec[3]
+        pats = rec[4:4 + n]
         assert 0 <= octant < 4 and 1 <= n <= 36 and len(set(pats)) == n
         assert all(0 <= q < (1 << K) and _balanced(q, K) for q in pats)
-        assert all(q == -1 for q in rec[2 + n:])
-        classes.append((octant, pats))
+        assert all(q == -1 for q in rec[4 + n:])
+        # the class's band: only the rows its paths reach, never more than the full-height band, and its n planes and
+        # the plain band fit where the geometry reserved full-height bands
+        assert rows * strides[octant] <= bw <= strides[4 + octant] and bw % 4 == 0
+        classes.append((octant, pats, bw, rows))
     assert (n_classes > 0) == (K > 0)
     if (m, H, W, level) == (100, 512, 512, 6):
         assert n_classes > 4                                 # a band of this shape has room for few planes: several classes
@@ -174,7 +177,7 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
             assert cur is not None
             assert bool(d["eroded"][e]) == (K > 0)
             q = int(d["q"][e])
-            slot, rem = divmod(int(d["off"][e]), strides[4 + o]) if K else (0, int(d["off"][e]))
+            slot, rem = divmod(int(d["off"][e]), classes[cls][2]) if K else (0, int(d["off"][e]))
             if K:
                 assert classes[cls][1][slot] == q            # the plane slot holds the entry's pattern
             bv, col = divmod(rem, strides[o])
@@ -188,6 +191,7 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
                 window.append((window[-1][0] + 1, window[-1][1] + ((q >> (j - 1)) & 1)))
             for a, b in window:
                 assert 0 <= b <= a <= m
+                assert not K or b < classes[cls][3]          # inside the class's band (start row 0)
             window = [_from_view(o, a, b) for a, b in window]
             # the first pixels of a window may be nodes that are already in the mask: as many as the list is longer than
             # the window's first column
@@ -225,8 +229,8 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
 def test_balanced_pattern_counts_and_classes_of_config3():
     """The K-step patterns of digital straight segments are the balanced words: 2, 4, 8, 14, 24, 36 of them for K = 1..6
     (1 + sum over i <= K of (K - i + 1) phi(i), the number of factors of length K of Sturmian words).  The program of
-    config 3 (512 x 512, m = 256) is of level 6 with at most 7 planes per class -- what fits in shared memory beside the
-    plain band -- and its classes together cover every pattern."""
+    config 3 (512 x 512, m = 256) is of level 6; a class has as many planes as fit in shared memory beside its plain band
+    (7 at full band height, more for the shallow slopes whose bands are lower), and the classes together cover every pattern."""
     from math import gcd
     for K, want in zip(range(1, 7), (2, 4, 8, 14, 24, 36)):
         phi = lambda n: sum(1 for k in range(1, n + 1) if gcd(k, n) == 1)
@@ -238,9 +242,9 @@ def test_balanced_pattern_counts_and_classes_of_config3():
     n_classes = layout[9]
     per_octant = {}
     for c in range(n_classes):
-        rec = layout[10 + 38 * c: 10 + 38 * (c + 1)]
-        assert 1 <= rec[1] <= 7
-        per_octant.setdefault(rec[0], set()).update(rec[2:2 + rec[1]])
-    assert n_classes == 48 and sorted(per_octant) == [0, 1, 2, 3]
+        rec = layout[10 + 40 * c: 10 + 40 * (c + 1)]
+        assert 1 <= rec[1] <= 36 and (rec[1] + 1) * rec[2] <= 8 * layout[4 + rec[0]]    # planes + plain band fit
+        per_octant.setdefault(rec[0], set()).update(rec[4:4 + rec[1]])
+    assert 20 <= n_classes <= 48 and sorted(per_octant) == [0, 1, 2, 3]
     assert all(len(v) == 36 for v in per_octant.values())
     assert len(entries) < 900000                                 # 5.0 M trie nodes: more than 5.5 nodes per entry
