@@ -67,7 +67,7 @@ extern "C" {
                              Same counts. */
 
 #define LPF_LAYOUT_MAX_CLASSES 128
-#define LPF_LAYOUT_INTS (10 + 40 * LPF_LAYOUT_MAX_CLASSES)   /* lpf_paths_program */
+#define LPF_LAYOUT_INTS (10 + 41 * LPF_LAYOUT_MAX_CLASSES)   /* lpf_paths_program */
 
 /* `what` of lpf_reserve */
 #define LPF_FOR_EVAL        1u   /* lpf_eval and one-phase lpf_eval_sum with (B, H, W, flags) */
@@ -122,9 +122,10 @@ int  lpf_paths_get(const lpf_paths* p, int dx, int dy, int16_t* xy, int cap, int
  *   items    host [cap_items][4] int64 = (first entry, number of entries, octant, pattern class) (may be NULL)
  *   layout   host int[LPF_LAYOUT_INTS]: [0..3] words per packed row of each octant view (decodes b', a' >> 5), [4..7]
  *            words of one full-height band of each view (0 for the plain program), [8] the level K of the program
- *            (0: plain), [9] the number of pattern classes, then per class 40 ints: octant, patterns used n, words of one
+ *            (0: plain), [9] the number of pattern classes, then per class 41 ints: octant, patterns used n, words of one
  *            band of THIS class in shared memory (the plane in slot s sits at s times that; a class keeps only the rows
- *            its paths reach), rows of that band, the pattern q of slot 0 .. n-1 (-1 beyond)
+ *            its paths reach), rows of that band, the level of the class (the K of ITS windows: the program's, or lower
+ *            for steep slopes of a template that is large against the image), the pattern q of slot 0 .. n-1 (-1 beyond)
  * *n_entries / *n_items / *n_slots (mask-stack slots the program needs) are always written.
  * Octants (view coordinates a', b' from image coordinates a, b): 0: dx>=0, dy<=dx (a,b); 1: dx>=0, dy>dx (b,a);
  * 2: dx<0, dy>-dx (b,-a); 3: dx<0, dy<=-dx (-a,b). */
@@ -269,6 +270,13 @@ int  lpf_set_tile(lpf_paths* p, int tx, int ty, int cta_warps);
  * keeps the planes of one pattern class per row band in shared memory; the highest level that fits and keeps enough warps resident is the
  * fastest.  LPF_NO_E2 is level 0.  Never changes a count.  INVAL otherwise. */
 int  lpf_set_level(lpf_paths* p, int max_level);
+
+/* Tuning hook: the dynamic shared memory one CTA of the eval kernel may use, in bytes, for
+ * the following lpf_reserve / lpf_eval / lpf_paths_program calls on this object: >= 16384, or 0 = all the device gives
+ * (the default; more than the device gives is the same).  With less room fewer planes fit beside a band: the bands get
+ * lower, then the pattern classes of steep slopes run at lower levels than the program's (as they do for templates
+ * that are large against the image), then the level drops.  Never changes a count.  INVAL otherwise. */
+int  lpf_set_shared_memory(lpf_paths* p, int bytes);
 
 /* Tuning hook: a CTA of the eval kernel is n_teams teams that share the row bands it holds in
  * shared memory; every team walks its own work unit (the segments are distributed, the image is shared).

@@ -110,6 +110,7 @@ static int upload_program(Program& pr) {
     geom[4 * c] = pr.classes[c].band_words;
     geom[4 * c + 1] = pr.classes[c].rows;
     geom[4 * c + 2] = pr.classes[c].n;
+    geom[4 * c + 3] = pr.classes[c].level;
   }
   cudaError_t e = cudaMalloc(&d_e, sizeof(uint64_t) * ne);
   if (e == cudaSuccess) e = cudaMalloc(&d_s, sizeof(uint32_t) * std::max<size_t>(pr.skip.size(), 1));
@@ -214,7 +215,7 @@ cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W
 static std::array<int64_t, 8> plan_key(const lpf_paths* p, int B, int H, int W, int n_phase, unsigned flags,
                                        bool masked) {
   return {B, H, W, n_phase, (int64_t)flags, masked ? 1 : 0, 100 * p->tile_tx + p->tile_ty,
-          p->cta_warps + 100 * p->n_teams + 10000 * (p->max_level + 1)};
+          p->cta_warps + 100 * p->n_teams + 10000 * (p->max_level + 1) + 100000 * (int64_t)p->smem_limit};
 }
 
 static int check_eval_args(const lpf_paths* p, int B, int H, int W, unsigned flags) {
@@ -237,8 +238,8 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
                             ? 0
                             : std::min(p->level_ok, p->max_level >= 0 ? p->max_level : MAX_LEVEL);
   const int max_teams = max_teams_of(p);
-  if (!choose_geom(p->m, H, W, B, p->max_smem, p->tile_tx, p->tile_ty, p->cta_warps, max_level, max_teams,
-                   p->path_patterns, &g))
+  if (!choose_geom(p->m, H, W, B, p->max_smem, p->smem_limit, p->tile_tx, p->tile_ty, p->cta_warps, max_level,
+                   max_teams, p->path_patterns, &g))
     return LPF_E_UNSUPPORTED;
   pl.Bpad = (B + g.G - 1) / g.G * g.G;
   long long off = 0;
@@ -575,7 +576,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   p->last_info[5] = (int64_t)pl.smem;
   p->last_info[6] = pl.g.TX * 1000 + pl.g.TY * 100 + pl.pr->n_slots;   // thread tile TX, TY and mask-stack slots
   p->last_info[7] = pl.g.G;
-  p->last_info[8] = pl.g.K;                              // erosion level: 2^K eroded planes in shared memory (0: plain)
+  p->last_info[8] = pl.g.K;                              // erosion level of the program (0: plain; classes may run lower)
   p->last_info[9] = pl.fused_pairs;                      // per image-phase and start word: 2 SHF + 1 LOP3 each
   p->last_info[10] = pl.singles;                         //   1 SHF + 1 LOP3 each
   p->last_info[11] = pl.terminals;                       //   1 POPC + 1 add each
@@ -664,6 +665,12 @@ extern "C" int lpf_set_tile(lpf_paths* p, int tx, int ty, int cta_warps) {
 extern "C" int lpf_set_level(lpf_paths* p, int max_level) {
   if (!p || max_level < -1 || max_level > MAX_LEVEL) return LPF_E_INVAL;
   p->max_level = max_level;
+  return LPF_OK;
+}
+
+extern "C" int lpf_set_shared_memory(lpf_paths* p, int bytes) {
+  if (!p || bytes < 0 || (bytes > 0 && bytes < 16384)) return LPF_E_INVAL;
+  p->smem_limit = bytes;
   return LPF_OK;
 }
 

@@ -111,13 +111,14 @@ struct Program {         // one linearisation of the four octant tries for one s
     int octant = 0;
     int rows = 0;                      // rows of the class's band: band_rows + the largest b' of its paths + 1
     int band_words = 0;                // words of one of its planes in shared memory (rows * stride, padded)
+    int level = 0;                     // its own level K_c <= the program's (steep classes of large templates: lower)
     int n = 0;                         // patterns used
     int pattern[MAX_PATTERNS];         // slot -> pattern q
     signed char slot_of[MAX_PATTERNS]; // rank of a balanced pattern -> slot, or -1
   };
   std::vector<Class> classes;
   signed char* d_class_slots = nullptr;  // device: [classes][MAX_PATTERNS]
-  int* d_class_geom = nullptr;           // device: [classes][4] = band words, rows, planes, -
+  int* d_class_geom = nullptr;           // device: [classes][4] = band words, rows, planes, level
   uint64_t* d_entries = nullptr;       // device copy, uploaded by lpf_reserve (lpf_api.cu)
   uint32_t* d_skip = nullptr;
 };
@@ -191,6 +192,7 @@ struct lpf_paths {
   int tile_tx = 0, tile_ty = 0, cta_warps = 0;   // lpf_set_tile overrides (0 = automatic)
   int n_teams = 0;                   // teams per CTA override (0 = automatic)
   int max_level = -1;                // erosion level cap (lpf_set_level; -1 = automatic)
+  int smem_limit = 0;                // shared memory one eval CTA may use, bytes (lpf_set_shared_memory; 0 = all)
   int timing = 0;
   int timed_once = 0;                // a timed eval has been issued: ev_start / ev_stop hold a measurement
   void* ev_start = nullptr;

@@ -360,13 +360,13 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
     parity ^= 1u;
     if (g.K > 0) {                   // the planes of the key's pattern class
       const signed char* slot = p.class_slots + (size_t)(ob.z >> 2) * MAX_PATTERNS;
-      const int4 cg = __ldg(p.class_geom + (ob.z >> 2));     // band words, rows, planes of the class
-      if (tid < MAX_PATTERNS) s_slot[tid] = slot[tid];
+      const int4 cg = __ldg(p.class_geom + (ob.z >> 2));     // band words, rows, planes, level of the class
+      for (int i = tid; i < MAX_PATTERNS; i += (int)blockDim.x) s_slot[i] = slot[i];   // a CTA may be one warp
       __syncthreads();
       for (int gi = 0; gi < g.G; ++gi) {
         uint32_t* planes = smem + (size_t)gi * v.band_pitch;
         const uint32_t* plain = planes + (size_t)cg.z * cg.x;
-        switch (g.K) {
+        switch (cg.w) {
           case 1: derive_planes<1>(planes, plain, cg.y, stride, cg.x, s_slot); break;
           case 2: derive_planes<2>(planes, plain, cg.y, stride, cg.x, s_slot); break;
           case 3: derive_planes<3>(planes, plain, cg.y, stride, cg.x, s_slot); break;

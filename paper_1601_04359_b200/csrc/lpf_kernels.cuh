@@ -86,9 +86,11 @@ constexpr int EVAL_CTA_MAX_THREADS = 1024;  // a CTA of NT teams (the eval kerne
 //   are split by slope into CLASSES whose paths use at most n_planes patterns; the planes of one class are derived in
 //   shared memory from the plain band when a CTA takes a key of that class
 //   max_teams: teams of one CTA that can find work on one key (lpf_internal.h: max_teams_of)
-//   path_patterns[K]: most patterns of length K on one path of the table (a class needs as many planes)
-bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int max_level, int max_teams,
-                 const int* path_patterns, Geom* out);
+//   path_patterns[K]: most patterns of length K on one path of the table (a class needs as many planes; where the
+//   bands cannot be made low enough for that, the classes of steep slopes run at lower levels: Program::Class::level)
+//   max_smem: opt-in shared memory of an SM's CTA; cta_smem: what one CTA may use of it (0 = all; lpf_set_shared_memory)
+bool choose_geom(int m, int H, int W, int B, int max_smem, int cta_smem, int tx, int ty, int cta_warps, int max_level,
+                 int max_teams, const int* path_patterns, Geom* out);
 
 // terminals above depth K have no program entry at level K (a window covers K + 1 pixels): shallow_kernel counts them
 constexpr int MAX_SHALLOW = 21;   // 1 + 2 + .. + MAX_LEVEL vectors of fewer than MAX_LEVEL steps per octant
@@ -110,7 +112,7 @@ struct EvalParams {
                               // are consecutive, big first
   const int4* obtab;          // [n_ob] (octant, row band, class) triples = first unit, units, octant | class << 2, row band
   const signed char* class_slots;  // level K: [n_classes][MAX_PATTERNS] plane slot of each balanced pattern (by rank), or -1
-  const int4* class_geom;          // level K: [n_classes] = words of one band of the class, its rows, its planes, -
+  const int4* class_geom;          // level K: [n_classes] = words of one band of the class, its rows, its planes, its level
   int n_ob;
   unsigned int n_keys;        // n_gp * n_ob keys = (image group, phase plane, octant, row band, class); key = gp * n_ob + ob
   unsigned int n_shares;      // n_keys * passes: how often the cursor hands out every key

@@ -244,7 +244,7 @@ struct Held {            // the row strip that is in the registers when an entry
 //   level 0: one entry per node, window read from the plain bit plane
 //   level K >= 1: shared memory holds one eroded plane per K-step pattern q instead of the plain plane: plane q at
 //     (a, b) is the AND of the K + 1 pixels (a + j, b + s_1 + .. + s_j), s_j = bit j-1 of q.  Every path step is
-//     (+1, 0) or (+1, +1), so any K + 1 consecutive nodes of a path are ONE window of one of the 2^K planes:
+//     (+1, 0) or (+1, +1), so any K + 1 consecutive nodes of a path are ONE window of one of the pattern planes:
 //       - a run of nodes whose own masks are never needed (not terminal, one child in the piece) is cut into entries
 //         of K + 1 nodes each,
 //       - a run that ends early (at a terminal, a branching node or a leaf) is read "backwards": the window that ENDS
@@ -393,8 +393,7 @@ static void push_item_c(Program& pr, int64_t first, int o, int cls) {
 
 // partitions one trie into pieces and emits its items
 static void emit_trie(const lpf_paths* p, int o, const std::vector<Node>& nd, int piece_nodes, Program& pr,
-                      const signed char* slot_of, int cls, int band_words) {
-  const int K = pr.K;
+                      const signed char* slot_of, int cls, int band_words, int K) {
   const int N = (int)nd.size();
   std::vector<uint8_t> cut(N, 0);
   std::vector<int32_t> psize(N, 1);
@@ -433,21 +432,28 @@ static void emit_trie(const lpf_paths* p, int o, const std::vector<Node>& nd, in
 // neighbouring slopes share most of them); every class gets its own prefix trie.  The short common trunk of the octant
 // is walked once per class instead of once: a fraction of a percent of the entries.
 static void build_class_tries(const lpf_paths* p, int o, int piece_nodes, Program& pr) {
-  const int K = pr.K;
+  const int Kmax = pr.K;
   const std::vector<Node>& nd = p->oct[o];
   const int N = (int)nd.size();
-  // patterns of the last K steps at every node, and the union over the path root -> node
+  // patterns of the last K steps at every node, and the union over the path root -> node, for the level in use
   std::vector<uint8_t> pat(N, 0);
   std::vector<uint64_t> pathset(N, 0);
-  for (int i = 1; i < N; ++i) {
-    const int par = nd[i].parent;
-    pat[i] = (uint8_t)((pat[par] >> 1) | ((nd[i].b - nd[par].b) << (K - 1)));
-    pathset[i] = pathset[par];
-    if (nd[i].depth >= K) pathset[i] |= 1ull << pattern_tables().rank[K][pat[i]];
-  }
+  int K = 0;
+  auto patterns_of_level = [&](int level) {
+    K = level;
+    pat[0] = 0;
+    pathset[0] = 0;
+    for (int i = 1; i < N; ++i) {
+      const int par = nd[i].parent;
+      pat[i] = (uint8_t)((pat[par] >> 1) | ((nd[i].b - nd[par].b) << (K - 1)));
+      pathset[i] = pathset[par];
+      if (nd[i].depth >= K) pathset[i] |= 1ull << pattern_tables().rank[K][pat[i]];
+    }
+  };
+  // the vectors of fewer than Kmax steps are counted by shallow_kernel, whatever the level of their class would be
   std::vector<int> terms;
   for (int i = 0; i < N; ++i)
-    if (nd[i].terminal && nd[i].depth >= K) terms.push_back(i);
+    if (nd[i].terminal && nd[i].depth >= Kmax) terms.push_back(i);
   std::sort(terms.begin(), terms.end(), [&](int x, int y) {          // by slope b / a, then by length
     const long long l = (long long)nd[x].b * nd[y].a, r = (long long)nd[y].b * nd[x].a;
     if (l != r) return l < r;
@@ -456,19 +462,35 @@ static void build_class_tries(const lpf_paths* p, int o, int piece_nodes, Progra
   std::vector<int16_t> vxy(2 * (size_t)(p->m + 1));
   // shared memory of one image: the n_planes + 1 full-height bands the geometry reserved.  A class only needs the rows
   // its paths reach (band_rows + the largest b'), so a class of shallow slopes has room for more planes -- wider
-  // classes, more units per key, fewer keys (pr.widen; not when the keys are few already: lpf_api.cu).
+  // classes, more units per key, fewer keys (pr.widen; not when the keys are few already: lpf_api.cu).  Where even
+  // the patterns of ONE path do not fit at level Kmax (steep slopes of a template that is large against the image: a
+  // plane is band_rows + m rows), the class takes the highest level that leaves room for them.
   const long long budget = (long long)(pr.n_planes + 1) * pr.band_words[o];
+  auto room_at = [&](int bmax_c, int level, int* rows_out, int* bw_out) {
+    const int rows = std::min(pr.band_rows + p->m, pr.band_rows + bmax_c + 1);
+    const int bw = (rows * pr.stride[o] + 3) / 4 * 4;
+    if (rows_out) *rows_out = rows;
+    if (bw_out) *bw_out = bw;
+    const int cap = pr.widen ? MAX_PATTERNS : std::max(pr.n_planes, 2);
+    return (int)std::min<long long>({(long long)cap, (long long)balanced_count(level), budget / bw - 1});
+  };
   size_t t0 = 0;
   while (t0 < terms.size()) {
+    // the level of the class: the highest at which the patterns of one path fit (K + 1 of them)
+    int level = Kmax;
+    for (; level > 1; --level) {
+      const int room = room_at(nd[terms[t0]].b, level, nullptr, nullptr);
+      if (room >= std::min(balanced_count(level), p->path_patterns[level])) break;
+    }
+    if (level != K) patterns_of_level(level);
     uint64_t set = 0;
     size_t t1 = t0;
     int bmax = 0, rows_c = 0, bw_c = 0;
     while (t1 < terms.size()) {
       const uint64_t ns = set | pathset[terms[t1]];
       const int bm = std::max(bmax, (int)nd[terms[t1]].b);
-      const int rows = std::min(pr.band_rows + p->m, pr.band_rows + bm + 1);
-      const int bw = (rows * pr.stride[o] + 3) / 4 * 4;
-      const int room = (int)std::min<long long>(pr.widen ? MAX_PATTERNS : pr.n_planes, budget / bw - 1);
+      int rows = 0, bw = 0;
+      const int room = room_at(bm, K, &rows, &bw);
       if (__builtin_popcountll(ns) > room) break;
       set = ns;
       bmax = bm;
@@ -476,11 +498,12 @@ static void build_class_tries(const lpf_paths* p, int o, int piece_nodes, Progra
       bw_c = bw;
       ++t1;
     }
-    if (t1 == t0) return;                                  // cannot happen: n_planes >= the patterns of any one path
+    if (t1 == t0) return;                                  // cannot happen: level 1 has two patterns and two planes fit
     Program::Class c;
     c.octant = o;
     c.rows = rows_c;
     c.band_words = bw_c;
+    c.level = K;
     std::memset(c.slot_of, -1, sizeof(c.slot_of));
     std::memset(c.pattern, 0, sizeof(c.pattern));
     for (unsigned q = 0; q < (1u << K); ++q) {
@@ -506,14 +529,14 @@ static void build_class_tries(const lpf_paths* p, int o, int piece_nodes, Progra
     for (int i = (int)cnd.size() - 1; i > 0; --i) cnd[cnd[i].parent].size += cnd[i].size;
     const int cls = (int)pr.classes.size();
     pr.classes.push_back(c);
-    emit_trie(p, o, cnd, piece_nodes, pr, pr.classes[cls].slot_of, cls, bw_c);
+    emit_trie(p, o, cnd, piece_nodes, pr, pr.classes[cls].slot_of, cls, bw_c, K);
     t0 = t1;
   }
 }
 
 static void build_trie_program(lpf_paths* p, int piece_nodes, Program& pr) {
   for (int o = 0; o < 4; ++o) {
-    if (pr.K == 0) emit_trie(p, o, p->oct[o], piece_nodes, pr, nullptr, 0, 0);
+    if (pr.K == 0) emit_trie(p, o, p->oct[o], piece_nodes, pr, nullptr, 0, 0, 0);
     else build_class_tries(p, o, piece_nodes, pr);
   }
   sort_items(pr);
@@ -754,7 +777,10 @@ static double geom_cost(const Geom& g, int max_smem, int max_teams) {
   else if (w >= 8) rate = 0.57 + 0.30 * (w - 8) / 8.0;
   else rate = 0.57 * w / 8.0;
   const double classes = (g.K > 0 && g.v[0].n_planes < balanced_count(g.K)) ? 1.03 : 1.0;
-  return entries[g.K] * classes / std::max(rate, 1e-3);
+  // classes of mixed levels (fewer full-height planes than the K + 1 patterns of a path): the steepest class runs at
+  // level n_planes - 1, the shallow ones at K
+  const int k_steep = g.K > 0 ? std::max(1, std::min(g.K, g.v[0].n_planes - 1)) : 0;
+  return 0.5 * (entries[g.K] + entries[k_steep]) * classes / std::max(rate, 1e-3);
 }
 
 // teams that find work on one key: two pieces of at least 256 trie nodes each per team and octant
@@ -768,8 +794,9 @@ int max_teams_of(const lpf_paths* p) {
 // (measured: config 3 3.73 / 3.76 / 3.89 / 3.78 ms, config 4 2.66 / 2.65 / 2.73 / 2.86 ms, 300 x 300 with m = 299
 // 4.10 / 5.42 / 4.57 / 4.57 ms: small keys balance better and leave room for a higher level); a later candidate or a
 // lower level must win by more than 3 %.
-bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int cta_warps, int max_level, int max_teams,
-                 const int* path_patterns, Geom* out) {
+bool choose_geom(int m, int H, int W, int B, int max_smem, int cta_smem, int tx, int ty, int cta_warps, int max_level,
+                 int max_teams, const int* path_patterns, Geom* out) {
+  cta_smem = cta_smem > 0 ? std::min(cta_smem, max_smem) : max_smem;   // lpf_set_shared_memory
   max_level = std::max(0, std::min({max_level, MAX_LEVEL, m}));   // the caller caps it at the table's level_ok
   double best = 0;
   bool found = false;
@@ -780,7 +807,7 @@ bool choose_geom(int m, int H, int W, int B, int max_smem, int tx, int ty, int c
       if (fixed && ci > 0) break;
       const int cw = fixed ? cta_warps : team_warps[ci];
       Geom g;
-      if (!choose_geom_fixed(m, H, W, B, max_smem, tx, ty, cw, K, path_patterns[K], &g)) continue;
+      if (!choose_geom_fixed(m, H, W, B, cta_smem, tx, ty, cw, K, path_patterns[K], &g)) continue;
       const double c = geom_cost(g, max_smem, max_teams);
       if (!found || c < best * 0.97) {
         best = c;
@@ -823,6 +850,10 @@ static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, 
   int row_blocks = std::max(1, cta_warps / g.SB);
   const int max_blocks = (hv_max + rows_per_warp - 1) / rows_per_warp;
   row_blocks = std::min(row_blocks, max_blocks);
+  const int row_blocks0 = row_blocks;
+  // first choice: bands low enough that every class has room for the patterns of one path at level K; where no band
+  // is (a template that is large against the image), the steep classes run at lower levels (build_class_tries)
+  bool mixed = false;
   for (;;) {
     g.band_rows = rows_per_warp * row_blocks;
     g.wpi = g.SB * row_blocks;
@@ -840,7 +871,8 @@ static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, 
     int n_planes = 0;
     if (K > 0) {
       n_planes = std::min(planes_all, (int)(((size_t)max_smem - 1024) / ((size_t)bw_max * 4)) - 1);
-      if (n_planes < std::min(planes_all, std::max(min_planes, K + 1))) n_planes = -1;
+      const int need = mixed ? 2 : std::min(planes_all, std::max(min_planes, K + 1));   // level 1: two patterns
+      if (n_planes < need) n_planes = -1;
     }
     if (n_planes >= 0) {
       for (int o = 0; o < 4; ++o) {
@@ -857,7 +889,12 @@ static bool choose_geom_fixed(int m, int H, int W, int B, int max_smem, int tx, 
       g.smem_bytes = (int)(g.G * per_image);
       break;
     }
-    if (row_blocks == 1) return false;
+    if (row_blocks == 1) {
+      if (mixed || K < 2) return false;
+      mixed = true;
+      row_blocks = row_blocks0;
+      continue;
+    }
     row_blocks /= 2;
   }
   *out = g;
@@ -924,8 +961,8 @@ extern "C" int lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, un
   const int max_level = (flags & (LPF_NO_E2 | LPF_NO_TRIE | LPF_S2))
                             ? 0
                             : std::min(p->level_ok, p->max_level >= 0 ? p->max_level : lpf::MAX_LEVEL);
-  if (!lpf::choose_geom(p->m, H, W, 1, p->max_smem > 0 ? p->max_smem : 232448, p->tile_tx, p->tile_ty, p->cta_warps,
-                        max_level, lpf::max_teams_of(p), p->path_patterns, &g))
+  if (!lpf::choose_geom(p->m, H, W, 1, p->max_smem > 0 ? p->max_smem : 232448, p->smem_limit, p->tile_tx, p->tile_ty,
+                        p->cta_warps, max_level, lpf::max_teams_of(p), p->path_patterns, &g))
     return LPF_E_UNSUPPORTED;
   try {
     lpf::Program& pr = lpf::get_program(p, piece_nodes, flags, g.v[0].stride, g.v[1].stride, g.K, g.v[0].n_planes,
@@ -938,12 +975,13 @@ extern "C" int lpf_paths_program(lpf_paths* p, int H, int W, int piece_nodes, un
     layout[8] = pr.K;
     layout[9] = (int)pr.classes.size();
     for (size_t c = 0; c < pr.classes.size(); ++c) {
-      int* out = layout + 10 + (4 + lpf::MAX_PATTERNS) * c;
+      int* out = layout + 10 + (5 + lpf::MAX_PATTERNS) * c;
       out[0] = pr.classes[c].octant;
       out[1] = pr.classes[c].n;
       out[2] = pr.classes[c].band_words;
       out[3] = pr.classes[c].rows;
-      for (int k = 0; k < lpf::MAX_PATTERNS; ++k) out[4 + k] = k < pr.classes[c].n ? pr.classes[c].pattern[k] : -1;
+      out[4] = pr.classes[c].level;
+      for (int k = 0; k < lpf::MAX_PATTERNS; ++k) out[5 + k] = k < pr.classes[c].n ? pr.classes[c].pattern[k] : -1;
     }
     if (entries) {
       if (cap_entries < *n_entries) return LPF_E_INVAL;

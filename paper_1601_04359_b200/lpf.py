@@ -22,7 +22,7 @@ EXPORTS = (
     "lpf_paths_get", "lpf_paths_program", "lpf_eval", "lpf_eval_both", "lpf_objective",
     "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
     "lpf_set_tile", "lpf_alu_peak", "lpf_eval_masked", "lpf_anneal", "lpf_reserve", "lpf_eval_sum",
-    "lpf_anneal_generate", "lpf_set_teams", "lpf_set_level",
+    "lpf_anneal_generate", "lpf_set_teams", "lpf_set_level", "lpf_set_shared_memory",
 )
 LPF_PROPOSE_OPPOSITE, LPF_PROPOSE_INTERFACIAL = 1, 2
 LPF_FOR_EVAL, LPF_FOR_EVAL_BOTH, LPF_FOR_MASKED, LPF_FOR_SWAP_DELTA, LPF_FOR_ANNEAL, LPF_FOR_HOST = 1, 2, 4, 8, 16, 32
@@ -100,6 +100,8 @@ def load() -> ctypes.CDLL:
     lib.lpf_set_teams.restype = I
     lib.lpf_set_level.argtypes = [VP, I]
     lib.lpf_set_level.restype = I
+    lib.lpf_set_shared_memory.argtypes = [VP, I]
+    lib.lpf_set_shared_memory.restype = I
     _lib = lib
     return lib
 
@@ -167,11 +169,11 @@ def lpf_paths_get(p: Paths, dx: int, dy: int) -> np.ndarray:
 
 def lpf_paths_program(p: Paths, H: int, W: int, piece_nodes: int = 0, flags: int = 0):
     """(entries uint64 [n], items int64 [k, 4], n_slots, layout: row strides of the 4 views, the words of one band of
-    each view in shared memory, the level K, the number of pattern classes, then 40 ints per class: octant, patterns
+    each view in shared memory, the level K, the number of pattern classes, then 41 ints per class: octant, patterns
     used, pattern of each slot) of the linearised walk program."""
     lib = load()
     ne, ni, ns = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int()
-    strides = (ctypes.c_int * (10 + 40 * 128))()
+    strides = (ctypes.c_int * (10 + 41 * 128))()
     _check(lib.lpf_paths_program(p.handle, int(H), int(W), int(piece_nodes), int(flags), None, 0, ctypes.byref(ne),
                                  None, 0, ctypes.byref(ni), ctypes.byref(ns), strides), "lpf_paths_program")
     entries = np.zeros(ne.value, dtype=np.uint64)
@@ -443,6 +445,11 @@ def lpf_set_tile(p: Paths, tx: int = 0, ty: int = 0, cta_warps: int = 0) -> None
 
 def lpf_set_level(p: Paths, max_level: int = -1) -> None:
     _check(load().lpf_set_level(p.handle, int(max_level)), "lpf_set_level")
+
+
+def lpf_set_shared_memory(p: Paths, nbytes: int = 0) -> None:
+    """Tuning hook: dynamic shared memory one CTA of the eval kernel may use (>= 16384; 0 = all of the device's)."""
+    _check(load().lpf_set_shared_memory(p.handle, int(nbytes)), "lpf_set_shared_memory")
 
 
 def lpf_set_teams(p: Paths, n_teams: int = 0) -> None:

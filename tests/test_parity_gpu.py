@@ -100,10 +100,12 @@ def test_ragged_shapes_both_phases_all_flags(H, W, m):
             assert np.array_equal(got, want), (phase, flags)
 
 
-@pytest.mark.parametrize("size", [50, 200])
+@pytest.mark.parametrize("size", [50, 200, 500])
 def test_tab1_morphologies_entire_domain(size):
     """The paper's Tab. 1 workloads: chess with 10x10 px fields and 4x4 px squares, ALL segments up to
-    (W-1, H-1) (m = size - 1, widths that are not multiples of 32), standard and enhanced, sampled vectors."""
+    (W-1, H-1) (m = size - 1, widths that are not multiples of 32), standard and enhanced, sampled vectors.  At 500 a
+    plane is 563 rows and two of them fit in shared memory beside the plain band: the pattern classes run at mixed
+    levels (6 for the shallow slopes down to 1 for the steepest)."""
     m = size - 1
     rng = np.random.default_rng(size)
     vecs = rng.integers(-m, m + 1, size=(150, 2))
@@ -622,6 +624,43 @@ def test_hypothesis_generated_levels_teams_and_tiles():
             for phase in (0, 1):
                 want = orc.counts(imgs[b], phase, m, full_template=(H * W <= 600))
                 assert np.array_equal(both[b, phase], want), (H, W, m, level, teams, tile, cta_warps, b, phase)
+
+    check()
+
+
+def test_hypothesis_generated_mixed_class_levels_with_little_shared_memory():
+    """Random shapes up to 96 x 160 with 16 .. 40 KiB of shared memory for a CTA (lpf_set_shared_memory): fewer planes
+    fit beside a band than one path has patterns at the program's level, so the pattern classes of steep slopes run at
+    lower levels than those of shallow slopes (what happens to templates that are large against the image at the full
+    227 KiB).  Hypothesis, derandomised: full-template bit-exact parity, both phases."""
+    from hypothesis import given, settings, strategies as st
+
+    @settings(max_examples=60, deadline=None, derandomize=True)
+    @given(st.integers(24, 96), st.integers(24, 160), st.floats(0.3, 0.97), st.integers(0, 2 ** 31 - 1),
+           st.integers(16, 40), st.integers(0, 3), st.sampled_from([(0, 0), (4, 2), (8, 1), (4, 4)]), st.data())
+    def check(H, W, fill, seed, kib, teams, tile, data):
+        m = data.draw(st.integers(min(H, W) // 2, min(H, W) - 1))
+        rng = np.random.default_rng(seed)
+        img = (rng.random((1, H, W)) < fill).astype(np.uint8)
+        p = paths(m)
+        lpf.lpf_set_shared_memory(p, kib * 1024)
+        lpf.lpf_set_tile(p, tile[0], tile[1], 0)
+        try:
+            try:
+                lpf.lpf_set_teams(p, teams)
+                both = lpf.lpf_eval_both(p, dev(img)).cpu().numpy()
+            except lpf.LpfError as e:
+                assert e.code == lpf.LPF_E_UNSUPPORTED and teams > 0
+                lpf.lpf_set_teams(p, 0)
+                both = lpf.lpf_eval_both(p, dev(img)).cpu().numpy()
+            assert lpf.lpf_last_launch_info(p)["smem_bytes"] <= kib * 1024
+        finally:
+            lpf.lpf_set_shared_memory(p, 0)
+            lpf.lpf_set_teams(p, 0)
+            lpf.lpf_set_tile(p, 0, 0, 0)
+        for phase in (0, 1):
+            want = orc.counts(img[0], phase, m, full_template=(H * W <= 600))
+            assert np.array_equal(both[0, phase], want), (H, W, m, kib, teams, tile, phase)
 
     check()
 

@@ -120,7 +120,10 @@ def _balanced(q, K):
     (100, 128, 128, 512, 0, 6),
     (2, 8, 9, 0, 0, 3), (3, 8, 9, 4, 0, 3), (1, 5, 5, 0, 0, -1), (7, 9, 8, 0, 0, 6),
     (12, 13, 13, 0, lpf.LPF_NO_TRIE, -1), (12, 64, 32, 64, lpf.LPF_NO_TRIE, -1), (33, 64, 64, 256, lpf.LPF_NO_E2, -1),
-    (40, 41, 97, 64, lpf.LPF_NO_E2, -1), (33, 64, 64, 256, 0, 0)])
+    (40, 41, 97, 64, lpf.LPF_NO_E2, -1), (33, 64, 64, 256, 0, 0),
+    # little shared memory: the classes of steep slopes run at lower levels than the program's (negative level = that
+    # many KiB for a CTA, automatic level)
+    (40, 64, 64, 64, 0, -24), (40, 64, 64, 0, 0, -32), (24, 33, 40, 16, 0, -16), (33, 64, 96, 64, 0, -20)])
 def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags, level):
     """Interpret the node program on the host with a stack of pixel lists instead of masks:
     every terminal must be reached exactly once with exactly the pixel list P_v, and the row-strip
@@ -128,6 +131,10 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
     At level K >= 1 a window covers K + 1 pixels of which the first `back` must already be the tail of the
     running list; the vectors shorter than K have no entry (a separate kernel counts them)."""
     p = lpf.lpf_build_paths(m, -1)
+    smem_kib = 0
+    if level < -1:
+        smem_kib, level = -level, -1
+        lpf.lpf_set_shared_memory(p, smem_kib * 1024)
     lpf.lpf_set_level(p, level)
     entries, items, n_slots, strides = lpf.lpf_paths_program(p, H, W, piece, flags)
     d = _decode(entries)
@@ -144,17 +151,19 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
     n_classes = strides[9]
     classes = []
     for c in range(n_classes):
-        rec = strides[10 + 40 * c: 10 + 40 * (c + 1)]
-        octant, n, bw, rows = rec[0], rec[1], rec[2], rec[3]
-        pats = rec[4:4 + n]
-        assert 0 <= octant < 4 and 1 <= n <= 36 and len(set(pats)) == n
-        assert all(0 <= q < (1 << K) and _balanced(q, K) for q in pats)
-        assert all(q == -1 for q in rec[4 + n:])
+        rec = strides[10 + 41 * c: 10 + 41 * (c + 1)]
+        octant, n, bw, rows, Kc = rec[0], rec[1], rec[2], rec[3], rec[4]
+        pats = rec[5:5 + n]
+        assert 0 <= octant < 4 and 1 <= n <= 36 and len(set(pats)) == n and 1 <= Kc <= K
+        assert all(0 <= q < (1 << Kc) and _balanced(q, Kc) for q in pats)
+        assert all(q == -1 for q in rec[5 + n:])
         # the class's band: only the rows its paths reach, never more than the full-height band, and its n planes and
         # the plain band fit where the geometry reserved full-height bands
         assert rows * strides[octant] <= bw <= strides[4 + octant] and bw % 4 == 0
-        classes.append((octant, pats, bw, rows))
+        classes.append((octant, pats, bw, rows, Kc))
     assert (n_classes > 0) == (K > 0)
+    if smem_kib:                                             # mixed levels: a steep class below a shallow one
+        assert len({c[4] for c in classes}) > 1 or max(c[4] for c in classes) < K
     if (m, H, W, level) == (100, 512, 512, 6):
         assert n_classes > 4                                 # a band of this shape has room for few planes: several classes
     S = 2 * m + 1
@@ -186,8 +195,9 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
             if d["reload"][e]:
                 held = (bv, col, plane)
             assert held == (bv, col, plane), "stale row strip"
-            window = [(av, bv)]                              # the K + 1 pixels of the plane of pattern q at (av, bv)
-            for j in range(1, K + 1):
+            Kc = classes[cls][4] if K else 0                 # the level of the item's class
+            window = [(av, bv)]                              # the Kc + 1 pixels of the plane of pattern q at (av, bv)
+            for j in range(1, Kc + 1):
                 window.append((window[-1][0] + 1, window[-1][1] + ((q >> (j - 1)) & 1)))
             for a, b in window:
                 assert 0 <= b <= a <= m
@@ -196,7 +206,7 @@ def test_program_walk_reproduces_every_canonical_path_once(m, H, W, piece, flags
             # the first pixels of a window may be nodes that are already in the mask: as many as the list is longer than
             # the window's first column
             back = len(cur) - av
-            assert 0 <= back <= K
+            assert 0 <= back <= Kc
             if d["init"][e]:
                 assert back == 0 and window[0] == (0, 0)     # every item starts at the root with a full window
             assert back == 0 or cur[-back:] == window[:back]
@@ -242,9 +252,12 @@ def test_balanced_pattern_counts_and_classes_of_config3():
     n_classes = layout[9]
     per_octant = {}
     for c in range(n_classes):
-        rec = layout[10 + 40 * c: 10 + 40 * (c + 1)]
+        rec = layout[10 + 41 * c: 10 + 41 * (c + 1)]
         assert 1 <= rec[1] <= 36 and (rec[1] + 1) * rec[2] <= 8 * layout[4 + rec[0]]    # planes + plain band fit
-        per_octant.setdefault(rec[0], set()).update(rec[4:4 + rec[1]])
+        if rec[4] == 6:
+            per_octant.setdefault(rec[0], set()).update(rec[5:5 + rec[1]])
+        else:
+            assert rec[4] == 5 and rec[1] <= 7                   # the steepest classes: room for 7 planes only
     assert 20 <= n_classes <= 48 and sorted(per_octant) == [0, 1, 2, 3]
-    assert all(len(v) == 36 for v in per_octant.values())
+    assert all(30 <= len(v) <= 36 for v in per_octant.values())
     assert len(entries) < 900000                                 # 5.0 M trie nodes: more than 5.5 nodes per entry
