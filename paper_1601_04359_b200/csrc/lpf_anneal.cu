@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
       const int j = unit / n_slices, slice = unit - j * n_slices;
       if (next + j >= a.N) continue;
       if (a.policy == 0) {
-        swap_delta_unit(sm, stk, sh, H, W, m, a.pairs, a.N, next + j, a.rec, a.n_nodes, rrec, dense_mask, a.delta + (long long)j * K2,
+        swap_delta_unit<2, false>(sm, stk, sh, H, W, m, a.pairs, a.N, next + j, a.rec, a.n_nodes, rrec, dense_mask, a.delta + (long long)j * K2,
                         n_ph, a.ph_stride, 1, slice, n_slices);
       } else {                                               // Q = modify(P): the operator draws its pixels from P
         __syncthreads();                                     // the previous unit is finished with s_pair
@@ -197,7 +197,7 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
           }
         }
         __syncthreads();
-        swap_delta_unit(sm, stk, sh, H, W, m, s_pair, 1, 0, a.rec, a.n_nodes, rrec, dense_mask, a.delta + (long long)j * K2, n_ph,
+        swap_delta_unit<2, false>(sm, stk, sh, H, W, m, s_pair, 1, 0, a.rec, a.n_nodes, rrec, dense_mask, a.delta + (long long)j * K2, n_ph,
                         a.ph_stride, 1, slice, n_slices);
       }
     }

@@ -694,7 +694,7 @@ __global__ void __launch_bounds__(256) swap_delta_kernel_v3(const uint32_t* __re
   uint2* stk = (uint2*)(sm + ((n_planes * plane_words + 1) & ~1));
   for (int i = threadIdx.x; i < n_planes * plane_words; i += blockDim.x) sm[i] = bits[i];
   const long long S2 = (long long)(2 * m + 1) * (2 * m + 1);
-  swap_delta_unit(sm, stk, sh, H, W, m, pairs, n, (long long)blockIdx.x * sw, rec, n_nodes, rrec, __ldg(dense),
+  swap_delta_unit<3, true>(sm, stk, sh, H, W, m, pairs, n, (long long)blockIdx.x * sw, rec, n_nodes, rrec, __ldg(dense),
                   delta + (long long)blockIdx.x * sw * S2, n_planes, plane_stride, sw, blockIdx.y, gridDim.y);
 }
 

@@ -54,6 +54,11 @@ struct SwapShared {                 // per-CTA scratch of swap_delta_unit
 // (canonical half only; plane k at + k * plane_stride), which must have been zeroed.
 //   P    shared memory: [n_planes][H + 2m][ceil((W + 2m) / 32)] bits of the base image with its halo of m pixels
 //   stk  shared memory: the CTA's stack of 8 * SWAP_STACK items (8 bytes each)
+//   CHAIN: trie nodes of an only-child chain visited per pop of (B); FAST_WALK: the branch-free form of the backward walk
+//   of (A).  Measured on config 5 / the annealing benchmark: the batched kernel is fastest with 3 and the branch-free
+//   walk (phase 1 1.90e6 -> 2.24e6 swaps/s, phase 0 6.5e4 -> 9.9e4), the annealing chain (small units, 48 registers) with 2
+//   and the plain walk (1.96e4 -> 2.15e4 proposals/s; the branch-free walk costs it 16 registers: 1.79e4).
+template <int CHAIN, bool FAST_WALK>
 __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, SwapShared& sh, int H, int W, int m,
                                                 const int* __restrict__ pairs, long long n, long long first_prop,
                                                 const int4* __restrict__ rec, int n_nodes,
@@ -235,12 +240,33 @@ __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, S
           const int PW = PWc * 32;
           const int dmaj = xmaj ? sxs : sys * PW, dmin = xmaj ? sys * PW : sxs;
           int L = (sy + m + oNy) * PW + (sx + m + oNx);      // pixel px itself (position d)
-          for (int k = d - 1; k >= 1; --k) {
-            e -= 2 * mn;
-            L -= dmaj;
-            if (e < 0) { e += 2 * nn; L -= dmin; }
-            if (k == d - 1) continue;
-            if (!((Pq[L >> 5] >> (L & 31)) & 1u)) { alive = false; break; }
+          if constexpr (FAST_WALK) {
+            // branch-free steps and a 32-bit shared-memory address: 11 instructions per pixel instead of 29
+            const int two_mn = 2 * mn, two_nn = 2 * nn;
+            const unsigned pq_s = (unsigned)__cvta_generic_to_shared(Pq);
+            {                                                // position d - 1 was the neighbour test
+              e -= two_mn;
+              const int neg = e >> 31;
+              e += neg & two_nn;
+              L -= dmaj + (neg & dmin);
+            }
+            for (int k = d - 2; k >= 1; --k) {
+              e -= two_mn;
+              const int neg = e >> 31;
+              e += neg & two_nn;
+              L -= dmaj + (neg & dmin);
+              unsigned wv;
+              asm volatile("ld.shared.u32 %0, [%1];" : "=r"(wv) : "r"(pq_s + 4u * (unsigned)(L >> 5)));
+              if (!((wv >> (L & 31)) & 1u)) { alive = false; break; }
+            }
+          } else {
+            for (int k = d - 1; k >= 1; --k) {
+              e -= 2 * mn;
+              L -= dmaj;
+              if (e < 0) { e += 2 * nn; L -= dmin; }
+              if (k == d - 1) continue;
+              if (!((Pq[L >> 5] >> (L & 31)) & 1u)) { alive = false; break; }
+            }
           }
         } else {
           for (int k = d - 1; k >= 1; --k) {
@@ -286,11 +312,28 @@ __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, S
         if (!rev) {
           isx = (int)(it.y & 0xffff);
           isy = (int)(it.y >> 16);
-          const int4 r = __ldg(rec + i);
-          size_i = r.z;
-          p_child = visit(i, qi, isx, isy, r) && r.z > 1;
-          p_sib = (r.w >> 24) & 1;
-          if (p_sib) it.x += (unsigned)r.z;                // next sibling = i + subtree size
+          // An only child follows its parent in the preorder array, and most of the trie is unary chains (about 36
+          // nodes per vector at m = 64): the next CHAIN - 1 records are loaded with the node's own (independent loads
+          // of one or two cache lines), and a chain of only children is visited in this pop instead of going through
+          // the stack node by node.
+          int4 r[CHAIN];
+#pragma unroll
+          for (int c = 0; c < CHAIN; ++c) r[c] = __ldg(rec + min(i + c, n_nodes - 1));
+          p_sib = (r[0].w >> 24) & 1;
+          if (p_sib) it.x += (unsigned)r[0].z;             // next sibling = i + subtree size
+          bool in = visit(i, qi, isx, isy, r[0]);
+          size_i = r[0].z;
+#pragma unroll
+          for (int c = 1; c < CHAIN; ++c) {
+            if (in && size_i > 1 && !((r[c].w >> 24) & 1)) {   // alive, has a child, and that child has no sibling
+              ++i;
+              size_i = r[c].z;
+              in = visit(i, qi, isx, isy, r[c]);
+            } else {
+              break;
+            }
+          }
+          p_child = in && size_i > 1;
         } else {
           // the end of a backward walk from the pass's pixel: in phase -> its extensions; complete for trie node fN ->
           // (fN, this pixel) is a survivor of (A): count it, and its first child is the start of (B)
@@ -330,7 +373,7 @@ __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, S
           for (int k = base + lane; k < min(base + ns + nc + nf, CAP); k += 32) stk[k] = make_uint2(DUMMY, 0);
           if (!rev) {
             if (p_child) scan_range(i + 1, i + size_i, qi, isx, isy);
-            if (p_sib) scan_siblings(i + size_i, qi, isx, isy);
+            if (p_sib) scan_siblings((int)(it.x & 0xFFFFFFu), qi, isx, isy);   // it.x was advanced to the sibling
           } else {
             if (p_fwd) scan_range(fN + 1, fN + fsize, qi, fx, fy);
             if (p_child) rscan_range(i + 1, i + size_i, qi);
