@@ -50,6 +50,7 @@ extern "C" {
 #define LPF_E_NOMEM       -2   /* host or device allocation failed */
 #define LPF_E_CUDA        -3   /* a CUDA runtime call failed (see lpf_last_cuda_error) */
 #define LPF_E_UNSUPPORTED -4   /* shape outside what the kernels take (m > 511, one row band + halo > shared memory) */
+#define LPF_E_TOO_LARGE   -5   /* lpf_swap_delta_static: the image needs more than LPF_STATIC_SCRATCH_BYTES of scratch */
 
 /* flags of lpf_eval / lpf_eval_both */
 #define LPF_PRUNE    1u   /* paper's "enhanced" variant: skip a sub-trie whose running
@@ -193,6 +194,24 @@ int  lpf_objective(const int64_t* counts, const int64_t* target, int B, int64_t 
  * does not fit the shared memory of one block, or when the trie has 2^24 nodes or more (m > ~380). */
 int  lpf_swap_delta(const lpf_paths* p, const uint8_t* image, int H, int W, int phase,
                     const int32_t* pairs, int64_t n, int32_t* delta, void* stream);
+
+/* lpf_swap_delta for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments, same result, but the scratch of the evaluation (the bit images of
+ * the phase and their copy with a halo of m pixels) lives in ONE array of LPF_STATIC_SCRATCH_BYTES in the library's
+ * device image, which every GPU that loads the library holds until the process exits.  The call never calls
+ * cudaMalloc, cudaFree or an allocating library routine: it enqueues memsets and kernels on `stream` and returns.
+ *   - The node records of the trie belong to p and are uploaded by lpf_reserve(p, 1, H, W, 0, LPF_FOR_SWAP_DELTA)
+ *     (any H, W: they do not depend on the shape) or by an earlier lpf_swap_delta: LPF_E_INVAL if neither happened.
+ *   - LPF_E_TOO_LARGE if 4 * (H*ceil(W/32) + W*ceil(H/32) + (H+2m)*ceil((W+2m)/32)) + 256 bytes exceed
+ *     LPF_STATIC_SCRATCH_BYTES = 256 KiB (config 5, 256 x 256 with m = 64, needs 35 KB; 768 x 768 with m = 32 fits,
+ *     1024 x 1024 does not).  Otherwise the errors of lpf_swap_delta.
+ *   - All calls on one GPU share the array, whatever their lpf_paths or stream: calls that overlap on the GPU race;
+ *     order them (one stream, or events).  The array keeps the last call's contents; every call clears what it reads.
+ *   - The first call on a device looks up the array's device address (cudaGetSymbolAddress; the runtime may load the
+ *     library's device image then): make it before a graph capture begins. */
+#define LPF_STATIC_SCRATCH_BYTES (256 * 1024)
+int  lpf_swap_delta_static(const lpf_paths* p, const uint8_t* image, int H, int W, int phase,
+                           const int32_t* pairs, int64_t n, int32_t* delta, void* stream);
 
 /* Simulated annealing of Alg. 3 with the two-pixel swap and the least-square
  * error of Eq. 19 on the lineal path descriptor; Tab. 2's parameters are arguments.  Readings A1-A5 of

@@ -14,7 +14,7 @@ _ROOT = os.path.dirname(_PKG)
 CSRC = os.path.join(_PKG, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_PKG, "liblpf.so")
-SOURCES = ["lpf_api.cu", "lpf_kernels.cu", "lpf_peak.cu", "lpf_anneal.cu", "lpf_paths.cpp"]
+SOURCES = ["lpf_api.cu", "lpf_kernels.cu", "lpf_peak.cu", "lpf_anneal.cu", "lpf_static.cu", "lpf_paths.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

@@ -912,6 +912,7 @@ extern "C" const char* lpf_strerror(int code) {
     case LPF_E_NOMEM: return "out of memory";
     case LPF_E_CUDA: return "CUDA runtime error";
     case LPF_E_UNSUPPORTED: return "unsupported shape";
+    case LPF_E_TOO_LARGE: return "image needs more scratch than LPF_STATIC_SCRATCH_BYTES (lpf_swap_delta_static)";
     default: return "unknown error";
   }
 }

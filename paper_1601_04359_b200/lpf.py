@@ -14,7 +14,8 @@ import numpy as np
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "liblpf.so")
 
-LPF_OK, LPF_E_INVAL, LPF_E_NOMEM, LPF_E_CUDA, LPF_E_UNSUPPORTED = 0, -1, -2, -3, -4
+LPF_OK, LPF_E_INVAL, LPF_E_NOMEM, LPF_E_CUDA, LPF_E_UNSUPPORTED, LPF_E_TOO_LARGE = 0, -1, -2, -3, -4, -5
+LPF_STATIC_SCRATCH_BYTES = 256 * 1024
 LPF_PRUNE, LPF_NO_TRIE, LPF_S2, LPF_NO_E2 = 1, 2, 4, 8
 
 EXPORTS = (
@@ -23,6 +24,7 @@ EXPORTS = (
     "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
     "lpf_set_tile", "lpf_alu_peak", "lpf_eval_masked", "lpf_anneal", "lpf_reserve", "lpf_eval_sum",
     "lpf_anneal_generate", "lpf_set_teams", "lpf_set_level", "lpf_set_shared_memory",
+    "lpf_swap_delta_static",
 )
 LPF_PROPOSE_OPPOSITE, LPF_PROPOSE_INTERFACIAL = 1, 2
 LPF_FOR_EVAL, LPF_FOR_EVAL_BOTH, LPF_FOR_MASKED, LPF_FOR_SWAP_DELTA, LPF_FOR_ANNEAL, LPF_FOR_HOST = 1, 2, 4, 8, 16, 32
@@ -84,6 +86,8 @@ def load() -> ctypes.CDLL:
     lib.lpf_objective.restype = I
     lib.lpf_swap_delta.argtypes = [VP, VP, I, I, I, VP, I64, VP, VP]
     lib.lpf_swap_delta.restype = I
+    lib.lpf_swap_delta_static.argtypes = [VP, VP, I, I, I, VP, I64, VP, VP]
+    lib.lpf_swap_delta_static.restype = I
     lib.lpf_eval_host.argtypes = [VP, VP, I, I, I, I, VP, U]
     lib.lpf_eval_host.restype = I
     lib.lpf_last_launch_info.argtypes = [VP, PI64]
@@ -393,6 +397,28 @@ def lpf_swap_delta(p: Paths, image, phase: int, pairs, out=None, stream=None):
     _on_device(p, out)
     _check(lib.lpf_swap_delta(p.handle, image.data_ptr(), H, W, int(phase), pairs.data_ptr(), n, out.data_ptr(),
                               _stream_ptr(stream, image, pairs)), "lpf_swap_delta")
+    return out
+
+
+def lpf_swap_delta_static(p: Paths, image, phase: int, pairs, out, stream=None):
+    """lpf_swap_delta with its scratch in the library's static device array (at most LPF_STATIC_SCRATCH_BYTES): the call
+    allocates nothing, so `out` (int32 [n, 2m+1, 2m+1]) is the caller's.  The trie records must have been uploaded by
+    lpf_reserve(..., LPF_FOR_SWAP_DELTA); calls that overlap on one GPU race on the array."""
+    torch = _torch()
+    lib = load()
+    image = _dev_images(image, 3, p)
+    if image.shape[0] != 1:
+        raise ValueError("lpf_swap_delta_static takes one base image")
+    _, H, W = image.shape
+    assert pairs.is_cuda and pairs.dtype == torch.int32 and pairs.dim() == 2 and pairs.shape[1] == 4
+    assert pairs.is_contiguous()
+    _on_device(p, pairs)
+    n = pairs.shape[0]
+    S = 2 * p.m + 1
+    assert out.is_cuda and out.dtype == torch.int32 and out.is_contiguous() and out.numel() == n * S * S
+    _on_device(p, out)
+    _check(lib.lpf_swap_delta_static(p.handle, image.data_ptr(), H, W, int(phase), pairs.data_ptr(), n,
+                                     out.data_ptr(), _stream_ptr(stream, image, pairs)), "lpf_swap_delta_static")
     return out
 
 
