@@ -426,7 +426,9 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
       uint32_t x = __shfl_sync(FULL, cur.x, 0);
 #pragma unroll 1
       for (int i = 0; i < n; ++i) {
-        uint32_t xn = __shfl_sync(FULL, cur.x, i + 1);
+        // the next program word, broadcast by a warp reduction: REDUX writes a uniform register directly and leaves the
+        // shared-memory pipe, which the strip reloads keep busy, one instruction per entry (a shuffle goes through it)
+        uint32_t xn = __reduce_or_sync(FULL, lane == i + 1 ? cur.x : 0u);
         if (x & E_RESTORE) {
           const uint32_t y = __shfl_sync(FULL, cur.y, i);
           const uint32_t* s = stk + ((y >> E_RSLOT_SHIFT) & E_SLOT_MASK) * T;
@@ -449,7 +451,7 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
             for (int t = 0; t < TX; ++t) Wp[ty * TX + t] = __funnelshift_r(R[ty][t], R[ty][t + 1], x);
           x = xn;
           ++i;
-          xn = __shfl_sync(FULL, cur.x, i + 1);
+          xn = __reduce_or_sync(FULL, lane == i + 1 ? cur.x : 0u);
           if (x & E_RELOAD) {
             const char* rp = base + ((x >> (E_OFF_SHIFT - 2)) & ~3u);
 #pragma unroll

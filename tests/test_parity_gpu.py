@@ -665,6 +665,56 @@ def test_hypothesis_generated_mixed_class_levels_with_little_shared_memory():
     check()
 
 
+def test_random_mid_size_shapes_flags_teams_and_shared_memory_limits():
+    """36 seeded random cases between the hypothesis shapes and the configs: 40..640 pixels a side, templates up to the
+    whole domain (m = min(H, W) - 1, at most 511), disks / Bernoulli / Gaussian-field images, every flag, fixed team
+    counts and shared-memory limits (so: every level, mixed class levels, the plain fall-back).  Sampled vectors (the
+    template's corners, 40 random ones, 20 short ones) against the oracle, both phases, plus point symmetry."""
+    rng = np.random.default_rng(20260601)
+    for case in range(36):
+        H, W = int(rng.integers(40, 640)), int(rng.integers(40, 640))
+        mode = int(rng.integers(0, 4))
+        m = min(H, W) - 1 if mode == 0 else int(rng.integers(1, min(H, W) if mode == 1 else min(H, W, 200)))
+        m = min(m, 511)
+        flags = int(rng.choice([0, 0, 0, lpf.LPF_PRUNE, lpf.LPF_NO_E2, lpf.LPF_S2, lpf.LPF_NO_TRIE if m <= 64 else 0]))
+        if flags & lpf.LPF_S2:                       # the oracle's S2 is the O(WH S^2) definition: a smaller case
+            H, W = min(H, 200), min(W, 200)
+            m = min(m, 40, H - 1, W - 1)
+        kind = int(rng.integers(0, 3))
+        seed = int(rng.integers(1 << 30))
+        if kind == 0:
+            img = inputs.disks(H, W, float(rng.uniform(2, 12)), float(rng.uniform(0.1, 0.8)), seed)
+        elif kind == 1:
+            img = inputs.bernoulli(H, W, float(rng.uniform(0.5, 0.99)), seed)
+        else:
+            img = inputs.gaussian_field(H, W, float(rng.uniform(3, 20)), float(rng.uniform(0.2, 0.8)), seed)
+        smem = int(rng.choice([0, 0, 0, 64, 100, 160])) * 1024
+        teams = int(rng.choice([0, 0, 0, 1, 2, 5]))
+        p = lpf.lpf_build_paths(m, 0)
+        try:
+            lpf.lpf_set_shared_memory(p, smem)
+            try:
+                lpf.lpf_set_teams(p, teams)
+                got = lpf.lpf_eval_both(p, dev(img[None]), flags).cpu().numpy()[0]
+            except lpf.LpfError as e:
+                assert e.code == lpf.LPF_E_UNSUPPORTED and teams > 0
+                lpf.lpf_set_teams(p, 0)
+                got = lpf.lpf_eval_both(p, dev(img[None]), flags).cpu().numpy()[0]
+        finally:
+            lpf.lpf_free_paths(p)
+        vecs = rng.integers(-m, m + 1, size=(40, 2))
+        vecs[:4] = [(0, 0), (m, m), (-m, m), (m, 0)]
+        k = min(m, 7)
+        vecs = np.concatenate([vecs, rng.integers(-k, k + 1, size=(20, 2))])
+        for phase in (0, 1):
+            if flags & lpf.LPF_S2:
+                want = orc.s2_counts(img, phase, m)[vecs[:, 1] + m, vecs[:, 0] + m]
+            else:
+                want, _ = orc.counts_list(img, phase, vecs)
+            assert np.array_equal(got[phase][vecs[:, 1] + m, vecs[:, 0] + m], want), (case, H, W, m, flags, smem, teams)
+            assert np.array_equal(got[phase], got[phase][::-1, ::-1]), (case, H, W, m, flags)
+
+
 # ---- the plain-plane program at full size, the automatic fall-back, the boundary contract --------------------
 
 def test_every_erosion_level_and_team_count_at_full_size():
