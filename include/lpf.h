@@ -286,8 +286,10 @@ int  lpf_set_tile(lpf_paths* p, int tx, int ty, int cta_warps);
 
 /* Tuning hook: caps the erosion level of the programs built for the following
  * lpf_reserve / lpf_eval / lpf_paths_program calls on this object: 0..6, or -1 = automatic (the default).  Level K
- * keeps the planes of one pattern class per row band in shared memory; the highest level that fits and keeps enough warps resident is the
- * fastest.  LPF_NO_E2 is level 0.  Never changes a count.  INVAL otherwise. */
+ * keeps the planes of one pattern class per row band in shared memory; the highest level that fits and keeps enough
+ * warps resident is the fastest.  Where a template is large against the image, the classes of steep slopes run below
+ * the program's level (the level of each class is in the layout of lpf_paths_program).  LPF_NO_E2 is level 0.  Never
+ * changes a count.  INVAL otherwise. */
 int  lpf_set_level(lpf_paths* p, int max_level);
 
 /* Tuning hook: the dynamic shared memory one CTA of the eval kernel may use, in bytes, for

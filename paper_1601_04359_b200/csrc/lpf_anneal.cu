@@ -145,8 +145,8 @@ __device__ __forceinline__ int4 propose_pair(const uint8_t* image, int H, int W,
 //   (C) SDP = SDQ: the accepted proposal's delta is added to the descriptor (both halves), every delta is zeroed
 //       again, every CTA patches its bit planes.
 // The proposals after an accepted one saw a stale image: they are not consumed and come back in the next batch, so
-// the chain is exactly the sequential one for any K; K follows the acceptance rate (about three expected acceptances
-// per batch).  Memory that other CTAs write during the launch (state, delta, dE, counts) is read with ld.global.cg.
+// the chain is exactly the sequential one for any K; K follows the acceptance rate (about 1 / rate + 1).  Memory that
+// other CTAs write during the launch (state, delta, dE, counts) is read with ld.global.cg.
 __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
   cg::grid_group grid = cg::this_grid();
   extern __shared__ __align__(16) uint32_t sm[];
@@ -332,7 +332,11 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
         }
       }
     }
-    // batch size for the next rounds: about three expected acceptances per batch, revised every 16 batches
+    // Batch size for the next rounds, revised every 16 batches: one more than the expected run up to the first acceptance.
+    // A batch costs about a + b K (a: the three grid barriers and the deepest exploration, b: the work of one proposal,
+    // a / b ~ 10 on the 100 x 100 benchmark) and consumes (1 - (1 - r)^K) / r proposals at acceptance rate r; the ratio
+    // peaks near K = 1 / r + 1 (measured against three expected acceptances per batch in powers of two, the rule before:
+    // r = 0.85: 2.1e4 -> 3.4e4 proposals/s, 0.45: 1.5e4 -> 2.2e4, 0.11: 3.1e4 -> 5.0e4, 0.03: 3.8e4 -> 7.3e4).
     if ((batch & 15) == 15) {
       const long long nx = ld_cg(&a.state->next), ac = ld_cg(&a.state->accepted);
       const long long dn = nx - win_next, da = ac - win_acc;
@@ -340,10 +344,7 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
       win_acc = ac;
       if (dn > 0) {
         const double rate = (double)max(1ll, da) / (double)dn;
-        const int want = (int)fmin(256.0, fmax(8.0, 3.0 / rate));
-        K = 8;
-        while (K < want) K *= 2;
-        K = min(K, a.K_max);
+        K = min(a.K_max, (int)fmin(256.0, fmax(2.0, 1.0 / rate + 1.5)));
       }
     }
     grid.sync();

@@ -56,8 +56,8 @@ struct SwapShared {                 // per-CTA scratch of swap_delta_unit
 //   stk  shared memory: the CTA's stack of 8 * SWAP_STACK items (8 bytes each)
 //   CHAIN: trie nodes of an only-child chain visited per pop of (B); FAST_WALK: the branch-free form of the backward walk
 //   of (A).  Measured on config 5 / the annealing benchmark: the batched kernel is fastest with 3 and the branch-free
-//   walk (phase 1 1.90e6 -> 2.24e6 swaps/s, phase 0 6.5e4 -> 9.9e4), the annealing chain (small units, 48 registers) with 2
-//   and the plain walk (1.96e4 -> 2.15e4 proposals/s; the branch-free walk costs it 16 registers: 1.79e4).
+//   walk (phase 1 1.90e6 -> 2.25e6 swaps/s, phase 0 6.5e4 -> 9.9e4), the annealing chain (small units) with 2 and the
+//   plain walk (1.96e4 -> 2.14e4 proposals/s; 3 nodes per pop: 2.04e4, the branch-free walk: 1.79e4).
 template <int CHAIN, bool FAST_WALK>
 __device__ __forceinline__ void swap_delta_unit(const uint32_t* P, uint2* stk, SwapShared& sh, int H, int W, int m,
                                                 const int* __restrict__ pairs, long long n, long long first_prop,
