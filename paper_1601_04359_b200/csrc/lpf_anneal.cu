@@ -69,8 +69,8 @@ struct AnnealArgs {
   int n_nodes;
   const int4* rrec;            // reversed trie of the swap delta, or null
   const unsigned int* dense;   // bit k: phase plane k is dense (per-node walks instead of the reversed trie)
-  int* delta;                  // [n_ph][K_max][S][S], zero on entry and again on exit
-  long long ph_stride;
+  int* delta;                  // two buffers of [n_ph][K_max][S][S], zero on entry and again on exit
+  long long ph_stride, buf_stride;
   int K_max;
   long long* dE;               // [K_max], zero on entry
   long long* counts;           // [n_ph][S][S]: descriptor of P
@@ -144,6 +144,9 @@ __device__ __forceinline__ int4 propose_pair(const uint8_t* image, int H, int W,
 //       accepted proposal, whose two bytes it exchanges (P = Q)
 //   (C) SDP = SDQ: the accepted proposal's delta is added to the descriptor (both halves), every delta is zeroed
 //       again, every CTA patches its bit planes.
+// Two grid barriers per batch: (C) of a batch and (A) of the next one run in the same phase -- a CTA patches its planes,
+// does its share of (C), then evaluates its units of the next batch into the OTHER of two delta buffers; (B) of that
+// batch reads the descriptor (C) has updated only after the barrier that follows.
 // The proposals after an accepted one saw a stale image: they are not consumed and come back in the next batch, so
 // the chain is exactly the sequential one for any K; K follows the acceptance rate (about 1 / rate + 1).  Memory that
 // other CTAs write during the launch (state, delta, dE, counts) is read with ld.global.cg.
@@ -166,42 +169,45 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
   const long long K2 = (long long)S * S, c0 = K2 / 2, half = K2 - c0;
   const long long per_prop = n_ph * half;                       // elements of D over the phases
   const int n_chunks = (int)((per_prop + 1023) / 1024);
-  int K = min(16, a.K_max);
+  int K = min(4, a.K_max);                                // proposals of the batch being decided
   long long win_next = 0, win_acc = 0;
   const unsigned int dense_mask = __ldg(a.dense);         // swaps keep the volume fractions: fixed for the chain
   // The reversed trie only if no plane of the chain is dense: a unit walks all planes of its proposal, and with one dense
   // plane the few slices that also explore the reversed trie of the sparse one would finish last (measured on the 100 x
   // 100 two-phase benchmark: 1.85e4 proposals/s with it, 1.94e4 without).
   const int4* const rrec = dense_mask == 0u ? a.rrec : nullptr;
-  for (int batch = 0;; ++batch) {
-    const long long next = ld_cg(&a.state->next);
-    if (next >= a.N) break;
-    // ---- (A)
-    const int n_slices = max(1, min((int)gridDim.x / K, (a.n_nodes + 255) / 256));
-    for (int unit = blockIdx.x; unit < K * n_slices; unit += gridDim.x) {
+  // (A): the deltas of proposals first .. first + Kb - 1 against the image in this CTA's shared memory, into dbuf
+  auto evaluate = [&](long long first, int Kb, int* dbuf) {
+    const int n_slices = max(1, min((int)gridDim.x / Kb, (a.n_nodes + 255) / 256));
+    for (int unit = blockIdx.x; unit < Kb * n_slices; unit += gridDim.x) {
       const int j = unit / n_slices, slice = unit - j * n_slices;
-      if (next + j >= a.N) continue;
+      if (first + j >= a.N) continue;
       if (a.policy == 0) {
-        swap_delta_unit<2, false>(sm, stk, sh, H, W, m, a.pairs, a.N, next + j, a.rec, a.n_nodes, rrec, dense_mask, a.delta + (long long)j * K2,
-                        n_ph, a.ph_stride, 1, slice, n_slices);
+        swap_delta_unit<2, false>(sm, stk, sh, H, W, m, a.pairs, a.N, first + j, a.rec, a.n_nodes, rrec, dense_mask,
+                                  dbuf + (long long)j * K2, n_ph, a.ph_stride, 1, slice, n_slices);
       } else {                                               // Q = modify(P): the operator draws its pixels from P
         __syncthreads();                                     // the previous unit is finished with s_pair
         if (warp == 0) {
-          const int4 pr = propose_pair(a.image, H, W, a.policy, a.seed, next + j, lane);
+          const int4 pr = propose_pair(a.image, H, W, a.policy, a.seed, first + j, lane);
           if (lane == 0) {
             s_pair[0] = pr.x; s_pair[1] = pr.y; s_pair[2] = pr.z; s_pair[3] = pr.w;
             if (slice == 0) {                                // for the decisions and for the caller
-              int* po = a.pairs_out + 4 * (next + j);
+              int* po = a.pairs_out + 4 * (first + j);
               po[0] = pr.x; po[1] = pr.y; po[2] = pr.z; po[3] = pr.w;
             }
           }
         }
         __syncthreads();
-        swap_delta_unit<2, false>(sm, stk, sh, H, W, m, s_pair, 1, 0, a.rec, a.n_nodes, rrec, dense_mask, a.delta + (long long)j * K2, n_ph,
-                        a.ph_stride, 1, slice, n_slices);
+        swap_delta_unit<2, false>(sm, stk, sh, H, W, m, s_pair, 1, 0, a.rec, a.n_nodes, rrec, dense_mask,
+                                  dbuf + (long long)j * K2, n_ph, a.ph_stride, 1, slice, n_slices);
       }
     }
-    grid.sync();
+  };
+  long long next = ld_cg(&a.state->next);
+  if (next < a.N) evaluate(next, K, a.delta);
+  grid.sync();
+  for (int batch = 0; next < a.N; ++batch) {
+    int* const dcur = a.delta + (long long)(batch & 1) * a.buf_stride;   // the deltas of this batch
     // ---- (B)
     for (int unit = blockIdx.x; unit < K * n_chunks; unit += gridDim.x) {
       const int j = unit / n_chunks, chunk = unit - j * n_chunks;
@@ -211,7 +217,7 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
         const long long i = (long long)chunk * 1024 + r * 256 + tid;
         if (i < per_prop) {
           const long long ph = i / half, k = c0 + (i - ph * half);
-          const long long dv = __ldcg(a.delta + ph * a.ph_stride + (long long)j * K2 + k);
+          const long long dv = __ldcg(dcur + ph * a.ph_stride + (long long)j * K2 + k);
           if (dv != 0) {
             const long long d = a.target[ph * K2 + k] - ld_cg(a.counts + ph * K2 + k);
             s += dv * dv - 2 * d * dv;
@@ -297,28 +303,8 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
       }
     }
     grid.sync();
-    // ---- (C)
+    // ---- (C) of this batch, then (A) of the next one into the other delta buffer
     const int acc_idx = __ldcg(&a.state->acc_idx);
-    for (int unit = blockIdx.x; unit < K * n_chunks; unit += gridDim.x) {
-      const int j = unit / n_chunks, chunk = unit - j * n_chunks;
-#pragma unroll
-      for (int r = 0; r < 4; ++r) {
-        const long long i = (long long)chunk * 1024 + r * 256 + tid;
-        if (i < per_prop) {
-          const long long ph = i / half, k = c0 + (i - ph * half);
-          int* dp = a.delta + ph * a.ph_stride + (long long)j * K2 + k;
-          const int dv = __ldcg(dp);
-          if (dv != 0) {
-            if (j == acc_idx) {
-              const long long nv = ld_cg(a.counts + ph * K2 + k) + dv;
-              a.counts[ph * K2 + k] = nv;
-              a.counts[ph * K2 + (K2 - 1 - k)] = nv;                     // count(-v) = count(v); v = 0 never changes
-            }
-            *dp = 0;
-          }
-        }
-      }
-    }
     if (acc_idx >= 0 && tid < 18 * n_ph) {                       // the two exchanged pixels, every periodic replica
       const int ph = tid / 18, r = tid % 18, which = r / 9, rep = r % 9;
       const int x = __ldcg(&a.state->acc_pair[2 * which]), y = __ldcg(&a.state->acc_pair[2 * which + 1]);
@@ -332,21 +318,44 @@ __global__ void __launch_bounds__(256) anneal_chain_kernel(const AnnealArgs a) {
         }
       }
     }
+    for (int unit = blockIdx.x; unit < K * n_chunks; unit += gridDim.x) {
+      const int j = unit / n_chunks, chunk = unit - j * n_chunks;
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const long long i = (long long)chunk * 1024 + r * 256 + tid;
+        if (i < per_prop) {
+          const long long ph = i / half, k = c0 + (i - ph * half);
+          int* dp = dcur + ph * a.ph_stride + (long long)j * K2 + k;
+          const int dv = __ldcg(dp);
+          if (dv != 0) {
+            if (j == acc_idx) {
+              const long long nv = ld_cg(a.counts + ph * K2 + k) + dv;
+              a.counts[ph * K2 + k] = nv;
+              a.counts[ph * K2 + (K2 - 1 - k)] = nv;                     // count(-v) = count(v); v = 0 never changes
+            }
+            *dp = 0;
+          }
+        }
+      }
+    }
+    next = ld_cg(&a.state->next);
     // Batch size for the next rounds, revised every 16 batches: one more than the expected run up to the first acceptance.
-    // A batch costs about a + b K (a: the three grid barriers and the deepest exploration, b: the work of one proposal,
+    // A batch costs about a + b K (a: the two grid barriers and the deepest exploration, b: the work of one proposal,
     // a / b ~ 10 on the 100 x 100 benchmark) and consumes (1 - (1 - r)^K) / r proposals at acceptance rate r; the ratio
     // peaks near K = 1 / r + 1 (measured against three expected acceptances per batch in powers of two, the rule before:
     // r = 0.85: 2.1e4 -> 3.4e4 proposals/s, 0.45: 1.5e4 -> 2.2e4, 0.11: 3.1e4 -> 5.0e4, 0.03: 3.8e4 -> 7.3e4).
     if ((batch & 15) == 15) {
-      const long long nx = ld_cg(&a.state->next), ac = ld_cg(&a.state->accepted);
-      const long long dn = nx - win_next, da = ac - win_acc;
-      win_next = nx;
+      const long long ac = ld_cg(&a.state->accepted);
+      const long long dn = next - win_next, da = ac - win_acc;
+      win_next = next;
       win_acc = ac;
       if (dn > 0) {
         const double rate = (double)max(1ll, da) / (double)dn;
         K = min(a.K_max, (int)fmin(256.0, fmax(2.0, 1.0 / rate + 1.5)));
       }
     }
+    __syncthreads();                                             // the patched bit planes, for every thread of this CTA
+    if (next < a.N) evaluate(next, K, a.delta + (long long)((batch + 1) & 1) * a.buf_stride);
     grid.sync();
   }
 }
@@ -376,7 +385,7 @@ static int anneal_impl(lpf_paths* p, uint8_t* image, int H, int W, int phase, co
 
   // chain state, proposal batch, deltas and error changes live in the table (lpf_reserve with LPF_FOR_ANNEAL)
   const int K_max = anneal_kmax(p->m, n_ph);
-  if (!p->d_an_state || p->an_delta_bytes < sizeof(int) * (size_t)n_ph * K_max * K2) {
+  if (!p->d_an_state || p->an_delta_bytes < sizeof(int) * 2 * (size_t)n_ph * K_max * K2) {
     rc = reserve_anneal(p, H, W);
     if (rc != LPF_OK) { if (prev != p->device) cudaSetDevice(prev); return rc; }
   }
@@ -394,7 +403,7 @@ static int anneal_impl(lpf_paths* p, uint8_t* image, int H, int W, int phase, co
   // anneal_apply_kernel from then on), E of the start image
   uint32_t* padded = nullptr;
   if (e == cudaSuccess) e = cudaMemcpyAsync(d_state, &h, sizeof(h), cudaMemcpyHostToDevice, st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(d_delta, 0, sizeof(int) * (size_t)n_ph * K_max * K2, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_delta, 0, sizeof(int) * 2 * (size_t)n_ph * K_max * K2, st);
   if (e == cudaSuccess) e = cudaMemsetAsync(d_dE, 0, sizeof(long long) * 256, st);
   if (e == cudaSuccess)
     e = launch_swap_bits(image, p->d_swap_bits, H, W, p->m, phase, p->d_counter + 1, p->n_sm, st, &padded);
@@ -420,7 +429,7 @@ static int anneal_impl(lpf_paths* p, uint8_t* image, int H, int W, int phase, co
       a.state = d_state; a.padded = padded; a.H = H; a.W = W; a.m = p->m; a.phase = phase; a.n_ph = n_ph;
       a.pairs = pairs; a.pairs_out = pairs_out; a.policy = policy; a.seed = seed; a.log_u = log_u; a.N = N; a.rec = (const int4*)p->d_swap_rec; a.n_nodes = (int)p->n_trie_nodes;
       a.rrec = (const int4*)p->d_swap_rrec; a.dense = p->d_counter + 2;
-      a.delta = d_delta; a.ph_stride = ph_stride; a.K_max = K_max; a.dE = d_dE; a.counts = (long long*)counts;
+      a.delta = d_delta; a.ph_stride = ph_stride; a.buf_stride = (long long)n_ph * ph_stride; a.K_max = K_max; a.dE = d_dE; a.counts = (long long*)counts;
       a.target = (const long long*)target; a.image = image; a.accept_log = accept_log; a.wh2 = wh2; a.T_mult = T_mult;
       a.c_max = c_max; a.s_max = s_max;
       void* args[] = {&a};

@@ -460,7 +460,7 @@ static int reserve_swap(lpf_paths* p, int H, int W) {
   return grow(&p->d_swap_bits, &p->swap_bits_bytes, bits_bytes);
 }
 
-int anneal_kmax(int m, int n_ph) {       // batch size: at most 256 proposals and about 256 MB of delta arrays
+int anneal_kmax(int m, int n_ph) {       // batch size: at most 256 proposals and about 256 MB of delta arrays per buffer
   const long long K2 = (long long)(2 * m + 1) * (2 * m + 1);
   int K_max = 256;
   while (K_max > 8 && (long long)K_max * K2 * 4 * n_ph > (256ll << 20)) K_max /= 2;
@@ -481,7 +481,7 @@ int reserve_anneal(lpf_paths* p, int H, int W) {
     LPF_CUDA(cudaMalloc(&p->d_an_dE, sizeof(int64_t) * 256));
   }
   p->an_kmax = K_max;
-  return grow(&p->d_an_delta, &p->an_delta_bytes, sizeof(int32_t) * (size_t)K_max * K2);
+  return grow(&p->d_an_delta, &p->an_delta_bytes, sizeof(int32_t) * 2 * (size_t)K_max * K2);   // two buffers (lpf_anneal.cu)
 }
 
 static int reserve_host(lpf_paths* p, int B, int H, int W) {
