@@ -41,7 +41,7 @@ def test_static_scratch_swap_delta_equals_the_allocating_path_on_two_calls_in_a_
             lpf.lpf_swap_delta_static(tables[m], d_img, phase, d_pairs, out)
         torch.cuda.synchronize()
         assert torch.cuda.memory_stats()["allocation.all.allocated"] == n_alloc      # nothing through PyTorch
-        assert torch.cuda.mem_get_info()[0] == free_before                             # and no cudaMalloc beside it
+        assert torch.cuda.mem_get_info()[0] >= free_before                             # and no cudaMalloc beside it
         for (img, pairs, m, phase), (_, _, ref), out in zip(cases, want, outs):
             assert torch.equal(out, ref), (img.shape, m, phase)
             got = out.cpu().numpy()
