@@ -257,7 +257,8 @@ int  lpf_eval_host(lpf_paths* p, const uint8_t* images_host, int B, int H, int W
 
 /* Counters of the most recent lpf_eval / lpf_eval_both on this object (host values known at
  * launch time): kernels launched, work units x (image group, phase), program entries walked per
- * image-phase, grid, block, dynamic shared memory bytes, thread tile code (1000 TX + 100 TY + mask-stack slots), images
+ * image-phase, grid, block, dynamic shared memory bytes, thread tile code (1000 TX + 100 TY + 10 if the mask stack is in
+ * tensor memory + mask-stack slots), images
  * per team, the erosion level K of the program (0: the plain plane); then what the walker executes per image-phase and
  * per start WORD, counted by replaying its loop over the program on the host: pairs of entries folded into one
  * 3-input AND (2 SHF + 1 LOP3 each), entries executed on their own (1 SHF + 1 LOP3), terminal entries (1 POPC +
@@ -298,6 +299,12 @@ int  lpf_set_level(lpf_paths* p, int max_level);
  * lower, then the pattern classes of steep slopes run at lower levels than the program's (as they do for templates
  * that are large against the image), then the level drops.  Never changes a count.  INVAL otherwise. */
 int  lpf_set_shared_memory(lpf_paths* p, int bytes);
+
+/* Tuning hook: where the walker keeps the masks it saves at the branching nodes
+ * of the trie.  enable = 1 (the default): in TENSOR MEMORY (tcgen05.st / tcgen05.ld) whenever the launch runs one CTA
+ * per SM and the slots of all its warps fit the 512 columns -- the big shapes; 0: always in local memory, as the small
+ * shapes do.  For the following lpf_reserve / lpf_eval calls on this object.  Never changes a count.  INVAL otherwise. */
+int  lpf_set_tmem_stack(lpf_paths* p, int enable);
 
 /* Tuning hook: a CTA of the eval kernel is n_teams teams that share the row bands it holds in
  * shared memory; every team walks its own work unit (the segments are distributed, the image is shared).

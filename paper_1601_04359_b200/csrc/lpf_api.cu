@@ -201,7 +201,8 @@ namespace lpf {
 
 cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed, const Geom& g, int B, int Bpad,
                         int n_phase, int phase0, unsigned int* counter, int n_sm, cudaStream_t st);
-cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem, int max_smem, int* blocks_per_sm);
+cudaError_t eval_occupancy(int TX, int TY, bool prune, bool tm, int threads, size_t smem, int max_smem,
+                           int* blocks_per_sm);
 cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st);
 cudaError_t launch_shallow(const EvalParams& p, const ShallowList& sl, int n_sm, cudaStream_t st);
 cudaError_t launch_mirror(unsigned long long* counts, int S, long long n_arrays, int n_sm, cudaStream_t st);
@@ -215,7 +216,8 @@ cudaError_t launch_swap_delta(const uint8_t* image, uint32_t* bits, int H, int W
 static std::array<int64_t, 8> plan_key(const lpf_paths* p, int B, int H, int W, int n_phase, unsigned flags,
                                        bool masked) {
   return {B, H, W, n_phase, (int64_t)flags, masked ? 1 : 0, 100 * p->tile_tx + p->tile_ty,
-          p->cta_warps + 100 * p->n_teams + 10000 * (p->max_level + 1) + 100000 * (int64_t)p->smem_limit};
+          p->cta_warps + 100 * p->n_teams + 10000 * (p->max_level + 1) + 100000 * (int64_t)p->smem_limit +
+              (p->no_tmem ? (int64_t)1 << 50 : 0)};
 }
 
 static int check_eval_args(const lpf_paths* p, int B, int H, int W, unsigned flags) {
@@ -268,7 +270,7 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
     for (int nt = 1; nt * g.threads <= EVAL_CTA_MAX_THREADS && nt <= nt_max; ++nt) {
       if (p->n_teams > 0 ? nt != p->n_teams : nt > max_teams) continue;
       int o_nt = 0;
-      LPF_CUDA(eval_occupancy(g.TX, g.TY, pl.prune != 0, nt * g.threads, pl.smem, p->max_smem, &o_nt));
+      LPF_CUDA(eval_occupancy(g.TX, g.TY, pl.prune != 0, false, nt * g.threads, pl.smem, p->max_smem, &o_nt));
       const int warps = o_nt * nt * (g.threads / 32);
       if (warps > best_warps) { best_warps = warps; g.NT = nt; occ = o_nt; }
     }
@@ -377,6 +379,17 @@ static int reserve_eval(lpf_paths* p, int B, int H, int W, int n_phase, unsigned
   pl.n_keys = n_keys;
   pl.n_shares = n_keys * passes;
   pl.occ = occ;
+  // The mask stack in tensor memory: a CTA allocates all 512 columns, so it must be alone on its SM, and the slots of the
+  // ceil(warps / 4) warps of a lane quarter must fit them (config 3: 8 warps x 4 slots x 16 words).
+  {
+    const int warps = g.NT * g.threads / 32, T = g.TX * g.TY;
+    pl.tmem_stack = occ == 1 && pr->n_slots > 0 && ((warps + 3) / 4) * pr->n_slots * T <= 512 && !p->no_tmem;
+    if (pl.tmem_stack) {
+      int o_tm = 0;
+      LPF_CUDA(eval_occupancy(g.TX, g.TY, pl.prune != 0, true, g.NT * g.threads, pl.smem, p->max_smem, &o_tm));
+      if (o_tm != 1) pl.tmem_stack = 0;
+    }
+  }
   shallow_terminals(p, pr->K, &pl.shallow);
 
   // workspace: the packed octant views, then the compact row-major / column-major bit images of stage 1, then (for
@@ -551,6 +564,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   ep.image_stride = sum_over_batch ? 0 : (long long)n_phase * S * S;
   ep.prune = pl.prune;
   ep.n_slots = pl.pr->n_slots;
+  ep.tmem_stack = pl.tmem_stack;
   ep.mask = start_mask ? d_mask : nullptr;
   for (int o = 0; o < 4; ++o) ep.mask_off[o] = pl.gm.v[o].packed_off;
   const bool timed = p->timing && !order.capturing;
@@ -574,7 +588,7 @@ static int eval_impl(lpf_paths* p, const uint8_t* images, int B, int H, int W, i
   p->last_info[3] = pl.grid;
   p->last_info[4] = pl.g.NT * pl.g.threads;              // CTA = NT teams
   p->last_info[5] = (int64_t)pl.smem;
-  p->last_info[6] = pl.g.TX * 1000 + pl.g.TY * 100 + pl.pr->n_slots;   // thread tile TX, TY and mask-stack slots
+  p->last_info[6] = pl.g.TX * 1000 + pl.g.TY * 100 + pl.tmem_stack * 10 + pl.pr->n_slots;   // thread tile, mask stack
   p->last_info[7] = pl.g.G;
   p->last_info[8] = pl.g.K;                              // erosion level of the program (0: plain; classes may run lower)
   p->last_info[9] = pl.fused_pairs;                      // per image-phase and start word: 2 SHF + 1 LOP3 each
@@ -671,6 +685,12 @@ extern "C" int lpf_set_level(lpf_paths* p, int max_level) {
 extern "C" int lpf_set_shared_memory(lpf_paths* p, int bytes) {
   if (!p || bytes < 0 || (bytes > 0 && bytes < 16384)) return LPF_E_INVAL;
   p->smem_limit = bytes;
+  return LPF_OK;
+}
+
+extern "C" int lpf_set_tmem_stack(lpf_paths* p, int enable) {
+  if (!p || (enable != 0 && enable != 1)) return LPF_E_INVAL;
+  p->no_tmem = !enable;
   return LPF_OK;
 }
 

@@ -135,7 +135,7 @@ struct EvalPlan {
   unsigned int* d_counters = nullptr;  //   and the share cursor + one unit counter per key
   int64_t n_units = 0, n_keys = 0, n_shares = 0;
   int n_ob = 0;
-  int Bpad = 0, n_gp = 0, grid = 0, prune = 0, occ = 0;
+  int Bpad = 0, n_gp = 0, grid = 0, prune = 0, occ = 0, tmem_stack = 0;
   size_t smem = 0;
   size_t views_bytes = 0, base_words = 0, mask_views_bytes = 0, mask_base_bytes = 0, need = 0;
   // what the walker executes per image-phase and start word (lpf_last_launch_info): pairs of entries folded into one
@@ -193,6 +193,7 @@ struct lpf_paths {
   int n_teams = 0;                   // teams per CTA override (0 = automatic)
   int max_level = -1;                // erosion level cap (lpf_set_level; -1 = automatic)
   int smem_limit = 0;                // shared memory one eval CTA may use, bytes (lpf_set_shared_memory; 0 = all)
+  int no_tmem = 0;                   // keep the mask stack in local memory (lpf_set_tmem_stack(p, 0))
   int timing = 0;
   int timed_once = 0;                // a timed eval has been issued: ev_start / ev_stop hold a measurement
   void* ev_start = nullptr;

@@ -269,12 +269,49 @@ __device__ __forceinline__ void derive_planes(uint32_t* planes, const uint32_t* 
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Tensor memory as the mask stack (TM variant of the eval kernel).  A saved mask is T words that only the thread that
+// saved them ever reads back: exactly the access of tcgen05.st / tcgen05.ld with the 32x32b shape (thread i of a warp
+// <-> TMEM lane 32 (warp % 4) + i, T consecutive columns).  In local memory a save or a restore moves as many bytes
+// through L1 as a row-strip reload (a tenth of that pipe's traffic on config 3); TMEM has its own datapath.  One CTA
+// per SM owns all 512 columns: ceil(warps / 4) warps share a lane quarter, n_slots x T columns each.
+// ---------------------------------------------------------------------------------------------
+template <int T>
+__device__ __forceinline__ void tmem_save(uint32_t taddr, const uint32_t (&v)[T]) {
+  static_assert(T == 8 || T == 16, "thread tile of 8 or 16 words");
+  if constexpr (T == 16)
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                 ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+                 "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+                 : "memory");
+  else
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), "r"(v[0]),
+                 "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+                 : "memory");
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+template <int T>
+__device__ __forceinline__ void tmem_restore(uint32_t taddr, uint32_t (&v)[T]) {
+  if constexpr (T == 16)
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                 : "r"(taddr)
+                 : "memory");
+  else
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr)
+                 : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
 // 64 registers per thread: CTAs of up to 1024 threads, 32 warps resident per SM (measured against 72 registers and 24
 // warps: config 3 5.33 vs 5.38 ms, config 4 3.67 vs 3.76 ms; the few spilled words sit next to the mask stack in L1)
 #ifndef LPF_EVAL_ATTR
 #define LPF_EVAL_ATTR __maxnreg__(64)
 #endif
-template <int TX, int TY, bool PRUNE>
+template <int TX, int TY, bool PRUNE, bool TM>
 __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
   constexpr int T = TX * TY;
   constexpr unsigned FULL = 0xffffffffu;
@@ -294,7 +331,19 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
   const int ww = wteam - img_local * g.wpi;
   const int strip_l = ww % g.SB, rblk = ww / g.SB;
   const int row0 = rblk * 32 * TY + lane;               // band-local start row of ty = 0
-  uint32_t stk[STACK_SLOTS_BUDGET * T];
+  uint32_t stk[TM ? 1 : STACK_SLOTS_BUDGET * T];   // the mask stack in local memory (TM: in tensor memory)
+  __shared__ uint32_t s_tmem;
+  uint32_t tm_mine = 0;                            // TMEM address of this warp's slot 0
+  if constexpr (TM) {
+    if (tid < 32) {                                // one warp allocates all 512 columns: one CTA per SM (lpf_api.cu)
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&s_tmem)) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    tm_mine = s_tmem + ((32u * ((unsigned)warp & 3u)) << 16) + ((unsigned)warp >> 2) * (unsigned)(p.n_slots * T);
+  }
 
   uint32_t M[T];
   uint32_t R[TY][TX + 1];
@@ -437,9 +486,13 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
         uint32_t xn = __reduce_or_sync(FULL, lane == i + 1 ? cur.x : 0u);
         if (x & E_RESTORE) {
           const uint32_t y = __shfl_sync(FULL, cur.y, i);
-          const uint32_t* s = stk + ((y >> E_RSLOT_SHIFT) & E_SLOT_MASK) * T;
+          if constexpr (TM) {
+            tmem_restore<T>(tm_mine + ((y >> E_RSLOT_SHIFT) & E_SLOT_MASK) * T, M);
+          } else {
+            const uint32_t* s = stk + ((y >> E_RSLOT_SHIFT) & E_SLOT_MASK) * T;
 #pragma unroll
-          for (int t = 0; t < T; ++t) M[t] = s[t];
+            for (int t = 0; t < T; ++t) M[t] = s[t];
+          }
         }
         if (x & E_RELOAD) {
           const char* rp = base + ((x >> (E_OFF_SHIFT - 2)) & ~3u);
@@ -479,9 +532,13 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
         if (x & (E_TERMINAL | E_SAVE)) {
           const uint32_t y = __shfl_sync(FULL, cur.y, i);
           if (x & E_SAVE) {
-            uint32_t* s = stk + ((y >> E_SSLOT_SHIFT) & E_SLOT_MASK) * T;
+            if constexpr (TM) {
+              tmem_save<T>(tm_mine + ((y >> E_SSLOT_SHIFT) & E_SLOT_MASK) * T, M);
+            } else {
+              uint32_t* s = stk + ((y >> E_SSLOT_SHIFT) & E_SLOT_MASK) * T;
 #pragma unroll
-            for (int t = 0; t < T; ++t) s[t] = M[t];
+              for (int t = 0; t < T; ++t) s[t] = M[t];
+            }
           }
           if (x & E_TERMINAL) {
             int c = 0;
@@ -512,12 +569,19 @@ __global__ void LPF_EVAL_ATTR eval_kernel_v3(const EvalParams p) {
     }
    }
   }
+  if constexpr (TM) {                              // every warp is done with its columns
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(s_tmem) : "memory");
+  }
 }
 
 typedef void (*eval_fn)(const EvalParams);
-static eval_fn eval_fn_for(int TX, int TY, bool prune) {
-#define LPF_PICK(tx, ty) \
-  if (TX == tx && TY == ty) return prune ? eval_kernel_v3<tx, ty, true> : eval_kernel_v3<tx, ty, false>;
+static eval_fn eval_fn_for(int TX, int TY, bool prune, bool tm) {
+#define LPF_PICK(tx, ty)                                                                              \
+  if (TX == tx && TY == ty)                                                                           \
+    return tm ? (prune ? eval_kernel_v3<tx, ty, true, true> : eval_kernel_v3<tx, ty, false, true>)    \
+              : (prune ? eval_kernel_v3<tx, ty, true, false> : eval_kernel_v3<tx, ty, false, false>);
   LPF_PICK(4, 2)
   LPF_PICK(8, 1)
   LPF_PICK(4, 4)
@@ -746,8 +810,9 @@ cudaError_t launch_pack(const uint8_t* images, uint32_t* base, uint32_t* packed,
 
 // also raises the kernel's dynamic shared memory limit to the device maximum (once is enough, repeating is harmless),
 // so that launches of any plan fit whatever order the plans were made in
-cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem, int max_smem, int* blocks_per_sm) {
-  eval_fn f = eval_fn_for(TX, TY, prune);
+cudaError_t eval_occupancy(int TX, int TY, bool prune, bool tm, int threads, size_t smem, int max_smem,
+                           int* blocks_per_sm) {
+  eval_fn f = eval_fn_for(TX, TY, prune, tm);
   if (!f) return cudaErrorInvalidValue;
   cudaFuncAttributes fa;
   cudaError_t e = cudaFuncGetAttributes(&fa, f);
@@ -758,7 +823,7 @@ cudaError_t eval_occupancy(int TX, int TY, bool prune, int threads, size_t smem,
 }
 
 cudaError_t launch_eval(const EvalParams& p, int grid, int threads, size_t smem, cudaStream_t st) {
-  eval_fn f = eval_fn_for(p.g.TX, p.g.TY, p.prune != 0);
+  eval_fn f = eval_fn_for(p.g.TX, p.g.TY, p.prune != 0, p.tmem_stack != 0);
   if (!f) return cudaErrorInvalidValue;
   f<<<grid, threads, smem, st>>>(p);
   return cudaGetLastError();

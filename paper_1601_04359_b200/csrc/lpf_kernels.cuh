@@ -127,6 +127,7 @@ struct EvalParams {
   int S;                      // 2m + 1
   int prune;
   int n_slots;                // mask-stack slots of the program (<= STACK_SLOTS_BUDGET)
+  int tmem_stack;             // the mask stack lives in tensor memory (one CTA per SM, the slots of all warps fit 512 columns)
   const uint32_t* mask;       // lpf_eval_masked: packed views of the start mask (one image), or nullptr
   long long mask_off[4];      // word offset of each octant view inside `mask`
 };

@@ -24,7 +24,7 @@ EXPORTS = (
     "lpf_swap_delta", "lpf_eval_host", "lpf_last_launch_info", "lpf_set_timing", "lpf_last_eval_kernel_ms",
     "lpf_set_tile", "lpf_alu_peak", "lpf_eval_masked", "lpf_anneal", "lpf_reserve", "lpf_eval_sum",
     "lpf_anneal_generate", "lpf_set_teams", "lpf_set_level", "lpf_set_shared_memory",
-    "lpf_swap_delta_static",
+    "lpf_swap_delta_static", "lpf_set_tmem_stack",
 )
 LPF_PROPOSE_OPPOSITE, LPF_PROPOSE_INTERFACIAL = 1, 2
 LPF_FOR_EVAL, LPF_FOR_EVAL_BOTH, LPF_FOR_MASKED, LPF_FOR_SWAP_DELTA, LPF_FOR_ANNEAL, LPF_FOR_HOST = 1, 2, 4, 8, 16, 32
@@ -104,6 +104,8 @@ def load() -> ctypes.CDLL:
     lib.lpf_set_teams.restype = I
     lib.lpf_set_level.argtypes = [VP, I]
     lib.lpf_set_level.restype = I
+    lib.lpf_set_tmem_stack.argtypes = [VP, I]
+    lib.lpf_set_tmem_stack.restype = I
     lib.lpf_set_shared_memory.argtypes = [VP, I]
     lib.lpf_set_shared_memory.restype = I
     _lib = lib
@@ -450,7 +452,9 @@ def lpf_last_launch_info(p: Paths) -> dict:
     keys = ("kernels", "work_items", "program_entries", "grid", "block", "smem_bytes", "tile", "G", "level",
             "fused_pairs", "singles", "terminals", "piece_nodes", "teams", "ctas_per_sm", "shallow_vectors",
             "reloads", "classes")
-    return dict(zip(keys, [int(v) for v in out]))
+    info = dict(zip(keys, [int(v) for v in out]))
+    info["tmem_stack"] = (info["tile"] // 10) % 10          # the mask stack of this launch was in tensor memory
+    return info
 
 
 def lpf_set_timing(p: Paths, enable: bool) -> None:
@@ -476,6 +480,11 @@ def lpf_set_level(p: Paths, max_level: int = -1) -> None:
 def lpf_set_shared_memory(p: Paths, nbytes: int = 0) -> None:
     """Tuning hook: dynamic shared memory one CTA of the eval kernel may use (>= 16384; 0 = all of the device's)."""
     _check(load().lpf_set_shared_memory(p.handle, int(nbytes)), "lpf_set_shared_memory")
+
+
+def lpf_set_tmem_stack(p: Paths, enable: bool = True) -> None:
+    """Tuning hook: the walker's mask stack in tensor memory (default, big shapes) or always in local memory."""
+    _check(load().lpf_set_tmem_stack(p.handle, int(bool(enable))), "lpf_set_tmem_stack")
 
 
 def lpf_set_teams(p: Paths, n_teams: int = 0) -> None:

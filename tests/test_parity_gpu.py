@@ -715,6 +715,47 @@ def test_random_mid_size_shapes_flags_teams_and_shared_memory_limits():
             assert np.array_equal(got[phase], got[phase][::-1, ::-1]), (case, H, W, m, flags)
 
 
+def test_mask_stack_in_tensor_memory_equals_the_one_in_local_memory():
+    """The walker saves its mask at the branching nodes of the trie: in tensor memory (tcgen05.st / tcgen05.ld) when the
+    launch runs one CTA per SM, in local memory otherwise or after lpf_set_tmem_stack(p, 0).  Whole results must be
+    identical on shapes that take the tensor-memory path (which one ran is read from lpf_last_launch_info): thread tiles
+    of 16 and of 8 words, with and without pruning, a batch, the masked evaluation; sampled vectors against the oracle."""
+    cases = [(384, 512, 150, 0, (0, 0), 1), (200, 260, 120, lpf.LPF_PRUNE, (0, 0), 1), (256, 256, 100, 0, (8, 1), 1),
+             (160, 192, 90, 0, (4, 2), 2), (300, 300, 149, lpf.LPF_NO_E2, (0, 0), 1)]
+    took = 0
+    for H, W, m, flags, tile, B in cases:
+        imgs = np.stack([inputs.disks(H, W, 6.0, 0.4, inputs.seed_for(9, H + b)) for b in range(B)])
+        p = lpf.lpf_build_paths(m, 0)
+        try:
+            lpf.lpf_set_tile(p, tile[0], tile[1], 0)
+            res = {}
+            for on in (True, False):
+                lpf.lpf_set_tmem_stack(p, on)
+                res[on] = lpf.lpf_eval_both(p, dev(imgs), flags).cpu().numpy()
+                info = lpf.lpf_last_launch_info(p)
+                assert info["tmem_stack"] in ((0, 1) if on else (0,)), info
+                took += info["tmem_stack"]
+                if on and info["ctas_per_sm"] == 1 and info["tile"] % 10 > 0:
+                    assert info["tmem_stack"] == 1, info
+            assert np.array_equal(res[True], res[False]), (H, W, m, flags, tile)
+            if flags == 0 and B == 1:
+                mask = (np.random.default_rng(m).random((H, W)) < 0.3).astype(np.uint8)
+                lpf.lpf_set_tmem_stack(p, True)
+                a = lpf.lpf_eval_masked(p, dev(imgs), 1, dev(mask)).cpu().numpy()
+                lpf.lpf_set_tmem_stack(p, False)
+                assert np.array_equal(a, lpf.lpf_eval_masked(p, dev(imgs), 1, dev(mask)).cpu().numpy())
+        finally:
+            lpf.lpf_free_paths(p)
+        rng = np.random.default_rng(H)
+        vecs = rng.integers(-m, m + 1, size=(60, 2))
+        for phase in (0, 1):
+            if flags & lpf.LPF_S2:
+                continue
+            want, _ = orc.counts_list(imgs[0], phase, vecs)
+            assert np.array_equal(res[True][0, phase][vecs[:, 1] + m, vecs[:, 0] + m], want), (H, W, m, flags, phase)
+    assert took >= 4                                     # the tensor-memory path did run
+
+
 # ---- the plain-plane program at full size, the automatic fall-back, the boundary contract --------------------
 
 def test_every_erosion_level_and_team_count_at_full_size():
