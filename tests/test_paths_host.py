@@ -44,7 +44,16 @@ def test_error_codes_on_host():
     out = (ctypes.c_int64 * 49)()
     assert lib.lpf_eval(p.handle, buf, 1, 8, 8, 1, out, 0, None) == lpf.LPF_E_INVAL
     assert lib.lpf_swap_delta(p.handle, buf, 8, 8, 1, buf, 1, out, None) == lpf.LPF_E_INVAL
+    assert lib.lpf_swap_delta_static(p.handle, buf, 8, 8, 1, buf, 1, out, None) == lpf.LPF_E_INVAL
     assert lib.lpf_strerror(lpf.LPF_E_UNSUPPORTED) == b"unsupported shape"
+    assert b"LPF_STATIC_SCRATCH_BYTES" in lib.lpf_strerror(lpf.LPF_E_TOO_LARGE)
+    # the tuning hooks check their arguments
+    for fn, bad in ((lib.lpf_set_tmem_stack, (2, -1)), (lib.lpf_set_level, (7, -2)), (lib.lpf_set_teams, (33, -1)),
+                    (lib.lpf_set_shared_memory, (1000, -1))):
+        for v in bad:
+            assert fn(p.handle, v) == lpf.LPF_E_INVAL, (fn, v)
+        assert fn(None, 0) == lpf.LPF_E_INVAL
+    assert lib.lpf_set_tmem_stack(p.handle, 0) == lpf.LPF_OK and lib.lpf_set_tmem_stack(p.handle, 1) == lpf.LPF_OK
     lpf.lpf_free_paths(p)
 
 
